@@ -1,0 +1,727 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, single-threaded CPU implementation of the batched Stratego
+// environment step of arxiv 2511.07312 ("Ataraxos"), written from the rules
+// text of the paper.  It shares no code, header, table or helper with the CUDA
+// path under paper_2511_07312_b200/csrc/ and neither imports the other.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may load this library.
+//
+// Citations: P:NNN = /root/reference/PAPER.md line NNN.  BJ = BASELINE.json.
+// R#n = reading n of the paper listed in DESIGN.md ("Readings").
+//
+// Parity status of each function (what pins it, see tests/test_oracle_*.py):
+//   philox4x32_10      pinned: Random123 known-answer vectors.
+//   battle             pinned: rules text P:208-210 enumerated as a 120-entry table.
+//   setup              pinned: multiset, chi-square marginals, count 1.41e33.
+//   legal moves        pinned: hand-worked positions E1-E5, closed form at ply 0,
+//                      mirror/rotation metamorphic maps, naive Python enumerator.
+//   two-square (non-Scout) pinned: BJ wording "A->B,B->A,A->B then B->A illegal".
+//   two-square (Scout overlap reading R#6)   PARITY UNPINNED against the paper
+//                      (P:246 only says "special care"); fixed by worked example E5.
+//   step / terminal    pinned: invariants, worked endings.
+//   reveal-on-long-Scout-move (R#10), reward timing (R#13), absolute
+//   orientation (R#1), setup rejection (R#5): PARITY UNPINNED (paper silent).
+//   encode             pinned: partition property, start-position counts,
+//                      information-state property.
+//   replay ring        pinned: FIFO content, chi-square of indices.
+//   determinise        pinned: multiset/constraint/obs-equality properties.
+//
+// Layouts:
+//   canonical line, 128 B per game:
+//     0..99   cell bytes: bits0-3 type (0 empty, 1 Spy,2 Scout,3 Miner,4 Sergeant,
+//             5 Lieutenant,6 Captain,7 Major,8 Colonel,9 General,10 Marshal,
+//             11 Flag,12 Bomb, 15 lake)  [type order P:499], bit4 owner (0 red,
+//             1 blue), bit5 moved, bit6 revealed
+//     100..115 history entry j = (from,to) of ply t-1-j, 0xFF,0xFF if none
+//     116..117 ply (LE u16)   118..119 battleless count (LE u16)
+//     120 flags: bit0 done, bits2-4 reason (1 flag,2 no-move win,3 no-move draw,
+//             4 ply cap,5 battleless)    121 result (int8, red's)
+//     122..123 zero           124..127 epoch (LE u32)
+//   cell c = 10*row + col; red home rows 0-3, blue home rows 6-9;
+//   lakes {42,43,52,53,46,47,56,57} (BJ configs[0]: c5-d6, g5-h6).
+//   action a = from*36 + dir*9 + (dist-1); dir 0:+row 1:+col 2:-row 3:-col.
+//   mask bit a -> word a>>5, bit a&31; 113 words per game.
+
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <new>
+
+namespace {
+
+constexpr int kCells = 100;
+constexpr int kLine = 128;
+constexpr int kMaskWords = 113;
+constexpr int kPlanes = 44;
+constexpr int kObs = kPlanes * kCells;  // 4400 bf16 per game
+
+constexpr int T_EMPTY = 0, T_SPY = 1, T_SCOUT = 2, T_MINER = 3, T_MARSHAL = 10,
+              T_FLAG = 11, T_BOMB = 12, T_LAKE = 15;
+constexpr uint8_t B_OWNER = 0x10, B_MOVED = 0x20, B_REVEALED = 0x40;
+
+constexpr int ORC_OK = 0, ORC_BAD_ARG = -1, ORC_BAD_STATE = -2, ORC_ILLEGAL_ACTION = -4;
+
+enum { TAG_SETUP_RED = 0, TAG_SETUP_BLUE = 1, TAG_ACTION = 2, TAG_SAMPLE = 3, TAG_DETERMINISE = 4 };
+enum { REASON_NONE = 0, REASON_FLAG = 1, REASON_NOMOVE_WIN = 2, REASON_NOMOVE_DRAW = 3,
+       REASON_PLY_CAP = 4, REASON_BATTLELESS = 5 };
+
+struct Config {  // mirrors the field order of the product's strat_config on purpose
+                 // (same C-ABI shape), but is declared independently.
+  int32_t num_games;
+  int32_t variant;  // 0 classic, 1 barrage
+  uint64_t seed;
+  int32_t max_plies;       // 0 = none (hard cap 65535, the u16 ply field)
+  int32_t max_battleless;  // 0 = off
+  int32_t auto_reset;
+  int32_t two_square;
+  int32_t device;  // unused here
+  int32_t reserved;
+  uint64_t game_base;  // global index of game 0 (RNG keying under sharding)
+};
+
+struct Game {
+  uint8_t cell[kCells];
+  uint8_t hist[8][2];
+  int ply;
+  int battleless;
+  bool done;
+  int reason;
+  int result;  // red's
+  uint32_t epoch;
+  // Two-square state machine: "tracking the last four positions occupied
+  // by the last-acting piece for each player".
+  int chain_len[2];
+  int chain[2][4];
+};
+
+struct Env {
+  Config cfg;
+  std::vector<Game> g;
+  int error;
+};
+
+// ---------------------------------------------------------------- geometry
+bool is_lake(int c) {
+  return c == 42 || c == 43 || c == 52 || c == 53 || c == 46 || c == 47 || c == 56 || c == 57;
+}
+int type_of(uint8_t b) { return b & 15; }
+int owner_of(uint8_t b) { return (b >> 4) & 1; }
+bool is_piece(uint8_t b) { return type_of(b) >= 1 && type_of(b) <= 12; }
+bool is_movable_type(int t) { return t >= 1 && t <= 10; }
+const int DROW[4] = {1, 0, -1, 0};
+const int DCOL[4] = {0, 1, 0, -1};
+
+// ---------------------------------------------------------------- C1 RNG
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw 2011, "Parallel random numbers: as
+// easy as 1, 2, 3").  BJ north_star: "Philox4x32-10-seeded".
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Draw d of a stream instance = word d&3 of block d>>2 (R#3).
+uint32_t stream_draw(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2_base, uint32_t tag, int d) {
+  uint32_t ctr[4] = {c0, c1, c2_base + (uint32_t)(d >> 2), tag};
+  uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t out[4];
+  philox4x32_10(ctr, key, out);
+  return out[d & 3];
+}
+
+// Bounded integer in [0,n): (u*n) >> 32 (R#3; no rejection, deterministic).
+uint32_t bounded(uint32_t u, uint32_t n) { return (uint32_t)(((uint64_t)u * n) >> 32); }
+
+// ---------------------------------------------------------------- C2 setup
+// BJ configs[0]: Flag 1, Bomb 6, Spy 1, Scout 8, Miner 5, Sergeant 4, Lieutenant 4,
+// Captain 4, Major 3, Colonel 2, General 1, Marshal 1, in that listed order.
+// BJ configs[1]: Flag, Marshal, General, Miner, Scout x2, Spy, Bomb, then 32 empties.
+void multiset(int variant, int A[40]) {
+  int n = 0;
+  if (variant == 0) {
+    const int types[12] = {11, 12, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10};
+    const int count[12] = {1, 6, 1, 8, 5, 4, 4, 4, 3, 2, 1, 1};
+    for (int k = 0; k < 12; ++k)
+      for (int i = 0; i < count[k]; ++i) A[n++] = types[k];
+  } else {
+    const int b[8] = {11, 10, 9, 3, 2, 2, 1, 12};
+    for (int k = 0; k < 8; ++k) A[n++] = b[k];
+    while (n < 40) A[n++] = 0;
+  }
+}
+
+// R#5: a side's setup is redrawn until it owns a movable piece with an on-board,
+// non-lake 4-neighbour not holding one of its own pieces.
+bool side_can_ever_move(const uint8_t cell[kCells], int side) {
+  for (int c = 0; c < kCells; ++c) {
+    uint8_t b = cell[c];
+    if (!is_piece(b) || owner_of(b) != side || !is_movable_type(type_of(b))) continue;
+    int r = c / 10, q = c % 10;
+    for (int d = 0; d < 4; ++d) {
+      int rr = r + DROW[d], qq = q + DCOL[d];
+      if (rr < 0 || rr > 9 || qq < 0 || qq > 9) continue;
+      int t = rr * 10 + qq;
+      if (is_lake(t)) continue;
+      if (is_piece(cell[t]) && owner_of(cell[t]) == side) continue;
+      return true;
+    }
+  }
+  return false;
+}
+
+void setup_side(const Config& cfg, uint32_t gidx, uint32_t epoch, int side, uint8_t cell[kCells]) {
+  for (uint32_t attempt = 0;; ++attempt) {
+    int A[40];
+    multiset(cfg.variant, A);
+    // Descending Fisher-Yates (R#4): for i = 39..1: j = bounded(draw[39-i], i+1).
+    for (int i = 39; i >= 1; --i) {
+      uint32_t u = stream_draw(cfg.seed, gidx, epoch, attempt << 8,
+                               side == 0 ? TAG_SETUP_RED : TAG_SETUP_BLUE, 39 - i);
+      int j = (int)bounded(u, (uint32_t)(i + 1));
+      int tmp = A[i]; A[i] = A[j]; A[j] = tmp;
+    }
+    int base = side == 0 ? 0 : 60;
+    for (int i = 0; i < 40; ++i)
+      cell[base + i] = A[i] == 0 ? 0 : (uint8_t)(A[i] | (side ? B_OWNER : 0));
+    if (side_can_ever_move(cell, side)) return;
+  }
+}
+
+void clear_dynamic(Game& gm) {
+  memset(gm.hist, 0xFF, sizeof gm.hist);
+  gm.ply = 0; gm.battleless = 0; gm.done = false; gm.reason = 0; gm.result = 0;
+  gm.chain_len[0] = gm.chain_len[1] = 0;
+}
+
+void new_game(const Config& cfg, uint32_t gidx, Game& gm) {  // epoch already set
+  memset(gm.cell, 0, sizeof gm.cell);
+  for (int c = 0; c < kCells; ++c)
+    if (is_lake(c)) gm.cell[c] = T_LAKE;
+  clear_dynamic(gm);
+  // Each side depends on its own pieces only, so the order of the two is immaterial.
+  setup_side(cfg, gidx, gm.epoch, 0, gm.cell);
+  setup_side(cfg, gidx, gm.epoch, 1, gm.cell);
+}
+
+// ---------------------------------------------------------------- C3 legal moves
+// Two-square rule: "prohibits a piece from crossing the same square
+// boundary on more than three consecutive turns of its owner".  Reading R#6: the
+// candidate move of the chain's piece is banned iff the chain holds four positions
+// (three consecutive moves of that piece), the three moves and the candidate lie on
+// one row or column, and the four of them cross at least one common boundary.
+bool two_square_banned(const Game& gm, int side, int from, int to) {
+  if (gm.chain_len[side] != 4) return false;
+  const int* p = gm.chain[side];
+  if (p[3] != from) return false;
+  int pos[5] = {p[0], p[1], p[2], p[3], to};
+  bool same_row = true, same_col = true;
+  for (int i = 1; i < 5; ++i) {
+    if (pos[i] / 10 != pos[0] / 10) same_row = false;
+    if (pos[i] % 10 != pos[0] % 10) same_col = false;
+  }
+  if (!same_row && !same_col) return false;
+  // Coordinate along the line; boundary b lies between coordinates b and b+1.
+  int x[5];
+  for (int i = 0; i < 5; ++i) x[i] = same_row ? pos[i] % 10 : pos[i] / 10;
+  for (int b = 0; b < 9; ++b) {
+    bool all = true;
+    for (int m = 0; m < 4; ++m) {
+      int lo = x[m] < x[m + 1] ? x[m] : x[m + 1];
+      int hi = x[m] < x[m + 1] ? x[m + 1] : x[m];
+      if (!(lo <= b && b < hi)) all = false;
+    }
+    if (all) return true;
+  }
+  return false;
+}
+
+// Is (from,dir,dist) a legal move for `side` on this board?  P:210: movable pieces
+// move one square in a cardinal direction onto an empty square or an opponent's
+// piece; Scouts any number of squares "so long as the movement does not jump over a
+// lake or an occupied square".
+bool move_is_legal(const Game& gm, const Config& cfg, int side, int from, int dir, int dist) {
+  uint8_t b = gm.cell[from];
+  if (!is_piece(b) || owner_of(b) != side) return false;
+  int t = type_of(b);
+  if (!is_movable_type(t)) return false;          // Bomb and Flag never move
+  if (dist >= 2 && t != T_SCOUT) return false;
+  int r = from / 10, q = from % 10;
+  for (int k = 1; k <= dist; ++k) {
+    int rr = r + DROW[dir] * k, qq = q + DCOL[dir] * k;
+    if (rr < 0 || rr > 9 || qq < 0 || qq > 9) return false;
+    int c = rr * 10 + qq;
+    if (is_lake(c)) return false;
+    if (k < dist) {
+      if (gm.cell[c] != 0) return false;          // may not jump
+    } else {
+      if (is_piece(gm.cell[c]) && owner_of(gm.cell[c]) == side) return false;
+    }
+  }
+  int to = (r + DROW[dir] * dist) * 10 + (q + DCOL[dir] * dist);
+  if (cfg.two_square && two_square_banned(gm, side, from, to)) return false;
+  return true;
+}
+
+// Number of legal moves of `side` (as if it were its turn), optionally setting mask bits.
+int gen_moves(const Game& gm, const Config& cfg, int side, uint32_t* mask) {
+  int n = 0;
+  for (int from = 0; from < kCells; ++from)
+    for (int dir = 0; dir < 4; ++dir)
+      for (int dist = 1; dist <= 9; ++dist)
+        if (move_is_legal(gm, cfg, side, from, dir, dist)) {
+          int a = from * 36 + dir * 9 + (dist - 1);
+          if (mask) mask[a >> 5] |= 1u << (a & 31);
+          ++n;
+        }
+  return n;
+}
+
+// ---------------------------------------------------------------- C4 battle
+// P:208-210 + Extended Data Fig. 3b as spelled out in BJ north_star: equal ranks both
+// removed, Spy attacking Marshal wins, Miner defuses Bomb, every other attacker on a
+// Bomb is lost, capturing the Flag ends the game.  +1 attacker wins, -1 loses, 0 tie.
+int battle(int att, int def) {
+  if (def == T_FLAG) return +1;
+  if (def == T_BOMB) return att == T_MINER ? +1 : -1;
+  if (att == T_SPY && def == T_MARSHAL) return +1;
+  if (att > def) return +1;   // "higher numbered piece defeats the lower"
+  if (att < def) return -1;
+  return 0;
+}
+
+int effective_ply_cap(const Config& cfg) {
+  return (cfg.max_plies >= 1 && cfg.max_plies <= 65535) ? cfg.max_plies : 65535;
+}
+
+void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
+  Game& gm = e->g[gi];
+  const Config& cfg = e->cfg;
+  if (gm.done) {  // R#15: frozen
+    *reward = 0;
+    *done_out = (uint8_t)(1 | (gm.reason << 2));
+    return;
+  }
+  int side = gm.ply & 1;  // red moves first
+  bool ok = action >= 0 && action < 3600;
+  int from = 0, dir = 0, dist = 1;
+  if (ok) {
+    from = action / 36; dir = (action % 36) / 9; dist = action % 9 + 1;
+    ok = move_is_legal(gm, cfg, side, from, dir, dist);
+  }
+  if (!ok) {
+    if (e->error == 0) e->error = ORC_ILLEGAL_ACTION;
+    *reward = 0; *done_out = 0;
+    return;
+  }
+  int to = (from / 10 + DROW[dir] * dist) * 10 + (from % 10 + DCOL[dir] * dist);
+  // 1. two-square chain of the mover.
+  if (gm.chain_len[side] > 0 && gm.chain[side][gm.chain_len[side] - 1] == from) {
+    if (gm.chain_len[side] == 4) {
+      for (int i = 0; i < 3; ++i) gm.chain[side][i] = gm.chain[side][i + 1];
+      gm.chain_len[side] = 3;
+    }
+    gm.chain[side][gm.chain_len[side]++] = to;
+  } else {
+    gm.chain[side][0] = from; gm.chain[side][1] = to; gm.chain_len[side] = 2;
+  }
+  for (int j = 7; j >= 1; --j) { gm.hist[j][0] = gm.hist[j - 1][0]; gm.hist[j][1] = gm.hist[j - 1][1]; }
+  gm.hist[0][0] = (uint8_t)from; gm.hist[0][1] = (uint8_t)to;
+  // 2. mover's bits.
+  uint8_t P = gm.cell[from] | B_MOVED;
+  if (dist >= 2) P |= B_REVEALED;  // R#10
+  uint8_t T = gm.cell[to];
+  bool flag_captured = false;
+  if (T == 0) {                    // 3. plain move
+    gm.cell[to] = P; gm.cell[from] = 0;
+    gm.battleless += 1;
+  } else {                         // 4. battle: both revealed
+    gm.battleless = 0;
+    P |= B_REVEALED; T |= B_REVEALED;
+    int out = battle(type_of(P), type_of(T));
+    if (out > 0) {
+      if (type_of(T) == T_FLAG) flag_captured = true;
+      gm.cell[to] = P; gm.cell[from] = 0;
+    } else if (out < 0) {
+      gm.cell[from] = 0; gm.cell[to] = T;   // R#11: defender's moved bit unchanged
+      gm.chain_len[side] = 0;
+    } else {
+      gm.cell[from] = 0; gm.cell[to] = 0;
+      gm.chain_len[side] = 0;
+    }
+  }
+  // 5. terminal tests, R#12 order.
+  gm.ply += 1;
+  int mover_result = side == 0 ? +1 : -1;
+  if (flag_captured) {
+    gm.done = true; gm.reason = REASON_FLAG; gm.result = mover_result;
+  } else if (gen_moves(gm, cfg, gm.ply & 1, nullptr) == 0) {
+    gm.done = true;
+    if (gen_moves(gm, cfg, side, nullptr) == 0) { gm.reason = REASON_NOMOVE_DRAW; gm.result = 0; }
+    else { gm.reason = REASON_NOMOVE_WIN; gm.result = mover_result; }
+  } else if (gm.ply >= effective_ply_cap(cfg)) {
+    gm.done = true; gm.reason = REASON_PLY_CAP; gm.result = 0;
+  } else if (cfg.max_battleless > 0 && gm.battleless >= cfg.max_battleless) {
+    gm.done = true; gm.reason = REASON_BATTLELESS; gm.result = 0;
+  }
+  // 6. outputs (R#13, R#14).
+  *reward = gm.done ? (int8_t)gm.result : 0;
+  *done_out = (uint8_t)((gm.done ? 1 : 0) | (side << 1) | ((gm.done ? gm.reason : 0) << 2));
+  if (gm.done && cfg.auto_reset) {  // R#16
+    gm.epoch += 1;
+    new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm);
+  }
+}
+
+// ---------------------------------------------------------------- canonical line
+void write_line(const Game& gm, uint8_t* L) {
+  memset(L, 0, kLine);
+  memcpy(L, gm.cell, kCells);
+  for (int j = 0; j < 8; ++j) { L[100 + 2 * j] = gm.hist[j][0]; L[101 + 2 * j] = gm.hist[j][1]; }
+  L[116] = (uint8_t)(gm.ply & 255); L[117] = (uint8_t)(gm.ply >> 8);
+  L[118] = (uint8_t)(gm.battleless & 255); L[119] = (uint8_t)(gm.battleless >> 8);
+  L[120] = (uint8_t)((gm.done ? 1 : 0) | (gm.reason << 2));
+  L[121] = (uint8_t)(int8_t)gm.result;
+  L[124] = (uint8_t)gm.epoch; L[125] = (uint8_t)(gm.epoch >> 8);
+  L[126] = (uint8_t)(gm.epoch >> 16); L[127] = (uint8_t)(gm.epoch >> 24);
+}
+
+// Rebuild one player's chain by replaying that player's moves found in the 8-ply
+// history window, oldest first (the chain needs the last three only).  Pieces that
+// died leave a cell their owner cannot move from next, so plain replay is exact.
+void rebuild_chains(Game& gm) {
+  gm.chain_len[0] = gm.chain_len[1] = 0;
+  for (int j = 7; j >= 0; --j) {
+    if (gm.hist[j][0] == 0xFF) continue;
+    int ply_of_move = gm.ply - 1 - j;
+    if (ply_of_move < 0) continue;
+    int side = ply_of_move & 1;
+    int from = gm.hist[j][0], to = gm.hist[j][1];
+    if (gm.chain_len[side] > 0 && gm.chain[side][gm.chain_len[side] - 1] == from) {
+      if (gm.chain_len[side] == 4) {
+        for (int i = 0; i < 3; ++i) gm.chain[side][i] = gm.chain[side][i + 1];
+        gm.chain_len[side] = 3;
+      }
+      gm.chain[side][gm.chain_len[side]++] = to;
+    } else {
+      gm.chain[side][0] = from; gm.chain[side][1] = to; gm.chain_len[side] = 2;
+    }
+  }
+  // A chain whose last position no longer holds a piece of that player is dead.
+  for (int s = 0; s < 2; ++s) {
+    if (gm.chain_len[s] == 0) continue;
+    uint8_t b = gm.cell[gm.chain[s][gm.chain_len[s] - 1]];
+    if (!is_piece(b) || owner_of(b) != s) gm.chain_len[s] = 0;
+  }
+}
+
+void read_line(const uint8_t* L, Game& gm) {
+  memcpy(gm.cell, L, kCells);
+  for (int j = 0; j < 8; ++j) { gm.hist[j][0] = L[100 + 2 * j]; gm.hist[j][1] = L[101 + 2 * j]; }
+  gm.ply = L[116] | (L[117] << 8);
+  gm.battleless = L[118] | (L[119] << 8);
+  gm.done = (L[120] & 1) != 0;
+  gm.reason = (L[120] >> 2) & 7;
+  gm.result = (int8_t)L[121];
+  gm.epoch = (uint32_t)L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
+  rebuild_chains(gm);
+}
+
+// ---------------------------------------------------------------- C5 encode
+// BJ configs[0]: 12 own-type planes, 12 revealed-opponent-type planes, hidden opponent
+// moved / unmoved, lake, empty, from/to planes of the last 8 plies; type order P:499.
+void encode_game(const Game& gm, uint16_t* obs) {
+  const uint16_t ONE = 0x3F80;  // bf16 1.0
+  for (int i = 0; i < kObs; ++i) obs[i] = 0;
+  int p = gm.ply & 1;
+  for (int c = 0; c < kCells; ++c) {
+    uint8_t b = gm.cell[c];
+    int plane;
+    if (type_of(b) == T_LAKE) plane = 26;
+    else if (b == 0) plane = 27;                       // R#17: empty excludes lakes
+    else if (owner_of(b) == p) plane = type_of(b) - 1;
+    else if (b & B_REVEALED) plane = 12 + type_of(b) - 1;
+    else if (b & B_MOVED) plane = 24;
+    else plane = 25;
+    obs[plane * kCells + c] = ONE;
+  }
+  for (int j = 0; j < 8; ++j) {
+    if (gm.hist[j][0] == 0xFF) continue;
+    obs[(28 + 2 * j) * kCells + gm.hist[j][0]] = ONE;
+    obs[(29 + 2 * j) * kCells + gm.hist[j][1]] = ONE;
+  }
+}
+
+// ---------------------------------------------------------------- C6 replay ring
+struct Replay {
+  int64_t per_slot, slots, capacity, head, filled;
+  std::vector<uint16_t> obs;
+  std::vector<uint32_t> mask;
+  std::vector<int16_t> action;
+  std::vector<int8_t> reward;
+  std::vector<uint8_t> done;
+};
+
+}  // namespace
+
+// ======================================================================= C ABI
+extern "C" {
+
+int orc_create(const Config* cfg, Env** out) {
+  if (!cfg || !out || cfg->num_games <= 0 || (cfg->variant != 0 && cfg->variant != 1)) return ORC_BAD_ARG;
+  Env* e = new (std::nothrow) Env;
+  if (!e) return ORC_BAD_ARG;
+  e->cfg = *cfg;
+  e->g.resize((size_t)cfg->num_games);
+  e->error = 0;
+  for (int i = 0; i < cfg->num_games; ++i) {
+    e->g[i].epoch = 0;
+    new_game(e->cfg, (uint32_t)(cfg->game_base + (uint64_t)i), e->g[i]);
+  }
+  *out = e;
+  return ORC_OK;
+}
+
+int orc_destroy(Env* e) { delete e; return ORC_OK; }
+
+int orc_reset(Env* e, uint64_t seed) {
+  if (!e) return ORC_BAD_ARG;
+  e->cfg.seed = seed;
+  e->error = 0;
+  for (int i = 0; i < e->cfg.num_games; ++i) {
+    e->g[i].epoch = 0;
+    new_game(e->cfg, (uint32_t)(e->cfg.game_base + (uint64_t)i), e->g[i]);
+  }
+  return ORC_OK;
+}
+
+int orc_reset_from(Env* e, const uint8_t* boards) {
+  if (!e || !boards) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) read_line(boards + (size_t)i * kLine, e->g[i]);
+  return ORC_OK;
+}
+
+int orc_get_boards(const Env* e, uint8_t* boards) {
+  if (!e || !boards) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) write_line(e->g[i], boards + (size_t)i * kLine);
+  return ORC_OK;
+}
+
+int orc_legal_mask(const Env* e, uint32_t* mask) {
+  if (!e || !mask) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) {
+    uint32_t* m = mask + (size_t)i * kMaskWords;
+    for (int w = 0; w < kMaskWords; ++w) m[w] = 0;
+    const Game& gm = e->g[i];
+    if (!gm.done) gen_moves(gm, e->cfg, gm.ply & 1, m);  // R#15: finished -> zero mask
+  }
+  return ORC_OK;
+}
+
+// C3a (P:480 SampleRandomLegalAction): r-th set bit, r = bounded(u, popcount),
+// u = word 0 of the ACTION block keyed by (global game, epoch, ply).
+int orc_sample_uniform(const Env* e, const uint32_t* mask, int16_t* actions) {
+  if (!e || !mask || !actions) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) {
+    const uint32_t* m = mask + (size_t)i * kMaskWords;
+    int n = 0;
+    for (int a = 0; a < 3600; ++a) n += (m[a >> 5] >> (a & 31)) & 1;
+    if (n == 0) { actions[i] = -1; continue; }
+    const Game& gm = e->g[i];
+    uint32_t u = stream_draw(e->cfg.seed, (uint32_t)(e->cfg.game_base + (uint64_t)i), gm.epoch,
+                             (uint32_t)gm.ply, TAG_ACTION, 0);
+    int r = (int)bounded(u, (uint32_t)n);
+    int16_t chosen = -1;
+    for (int a = 0; a < 3600; ++a)
+      if ((m[a >> 5] >> (a & 31)) & 1) {
+        if (r == 0) { chosen = (int16_t)a; break; }
+        --r;
+      }
+    actions[i] = chosen;
+  }
+  return ORC_OK;
+}
+
+int orc_step(Env* e, const int16_t* actions, int8_t* reward, uint8_t* done) {
+  if (!e || !actions || !reward || !done) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) step_game(e, i, actions[i], &reward[i], &done[i]);
+  return ORC_OK;
+}
+
+int orc_encode_obs(const Env* e, uint16_t* obs) {
+  if (!e || !obs) return ORC_BAD_ARG;
+  for (int i = 0; i < e->cfg.num_games; ++i) encode_game(e->g[i], obs + (size_t)i * kObs);
+  return ORC_OK;
+}
+
+int orc_check(Env* e) {
+  if (!e) return ORC_BAD_ARG;
+  int err = e->error;
+  return err;
+}
+
+int orc_clear_error(Env* e) { if (!e) return ORC_BAD_ARG; e->error = 0; return ORC_OK; }
+
+// ---- replay ring (C6, BJ configs[3]; R#19, R#20)
+int orc_replay_create(int32_t per_slot, int32_t slots, Replay** out) {
+  if (!out || per_slot <= 0 || slots <= 0) return ORC_BAD_ARG;
+  Replay* r = new (std::nothrow) Replay;
+  if (!r) return ORC_BAD_ARG;
+  r->per_slot = per_slot; r->slots = slots; r->capacity = (int64_t)per_slot * slots;
+  r->head = 0; r->filled = 0;
+  r->obs.assign((size_t)r->capacity * kObs, 0);
+  r->mask.assign((size_t)r->capacity * kMaskWords, 0);
+  r->action.assign((size_t)r->capacity, 0);
+  r->reward.assign((size_t)r->capacity, 0);
+  r->done.assign((size_t)r->capacity, 0);
+  *out = r;
+  return ORC_OK;
+}
+
+int orc_replay_destroy(Replay* r) { delete r; return ORC_OK; }
+
+int orc_replay_push(Replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
+                    const int8_t* reward, const uint8_t* done, int32_t n) {
+  if (!r || n < 0 || n > r->capacity) return ORC_BAD_ARG;
+  for (int i = 0; i < n; ++i) {
+    int64_t p = (r->head + i) % r->capacity;
+    memcpy(&r->obs[(size_t)p * kObs], obs + (size_t)i * kObs, kObs * sizeof(uint16_t));
+    memcpy(&r->mask[(size_t)p * kMaskWords], mask + (size_t)i * kMaskWords, kMaskWords * sizeof(uint32_t));
+    r->action[(size_t)p] = action[i];
+    r->reward[(size_t)p] = reward[i];
+    r->done[(size_t)p] = done[i];
+  }
+  r->head = (r->head + n) % r->capacity;
+  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+  return ORC_OK;
+}
+
+// Element j reads physical record bounded(draw j, filled); SAMPLE stream: c0 = block,
+// (c1,c2) = draw_index lo,hi.  `indices` (optional) receives the physical indices.
+int orc_replay_sample(const Replay* r, uint64_t seed, uint64_t draw_index, int32_t batch,
+                      uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
+                      int64_t* indices) {
+  if (!r || batch < 0) return ORC_BAD_ARG;
+  if (r->filled == 0) return ORC_BAD_STATE;
+  for (int j = 0; j < batch; ++j) {
+    uint32_t ctr[4] = {(uint32_t)(j >> 2), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), TAG_SAMPLE};
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t o[4];
+    philox4x32_10(ctr, key, o);
+    int64_t p = (int64_t)bounded(o[j & 3], (uint32_t)r->filled);
+    if (indices) indices[j] = p;
+    if (obs) memcpy(obs + (size_t)j * kObs, &r->obs[(size_t)p * kObs], kObs * sizeof(uint16_t));
+    if (mask) memcpy(mask + (size_t)j * kMaskWords, &r->mask[(size_t)p * kMaskWords], kMaskWords * sizeof(uint32_t));
+    if (action) action[j] = r->action[(size_t)p];
+    if (reward) reward[j] = r->reward[(size_t)p];
+    if (done) done[j] = r->done[(size_t)p];
+  }
+  return ORC_OK;
+}
+
+// Raw record p of the ring (tests compare ring contents).
+int orc_replay_read(const Replay* r, int64_t p, uint16_t* obs, uint32_t* mask, int16_t* action,
+                    int8_t* reward, uint8_t* done) {
+  if (!r || p < 0 || p >= r->capacity) return ORC_BAD_ARG;
+  memcpy(obs, &r->obs[(size_t)p * kObs], kObs * sizeof(uint16_t));
+  memcpy(mask, &r->mask[(size_t)p * kMaskWords], kMaskWords * sizeof(uint32_t));
+  *action = r->action[(size_t)p]; *reward = r->reward[(size_t)p]; *done = r->done[(size_t)p];
+  return ORC_OK;
+}
+
+int64_t orc_replay_head(const Replay* r) { return r ? r->head : -1; }
+int64_t orc_replay_filled(const Replay* r) { return r ? r->filled : -1; }
+
+// ---- C7 determinise (BJ configs[4]): for output game G = r*S + s, permute the types of
+// the searcher's opponent's unrevealed pieces uniformly over their squares, rejecting
+// any permutation that puts a Bomb or Flag on a piece that has moved.  `attempts`
+// (optional, [R*S]) receives the number of attempts used.  R#22: at most 4096 attempts.
+int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, Env* out, int32_t* attempts) {
+  if (!roots || !out || samples_per_root <= 0) return ORC_BAD_ARG;
+  int R = roots->cfg.num_games;
+  if ((int64_t)R * samples_per_root != out->cfg.num_games) return ORC_BAD_ARG;
+  for (int r = 0; r < R; ++r) {
+    const Game& root = roots->g[r];
+    int searcher = root.ply & 1;
+    int H[40], T[40], n = 0;
+    for (int c = 0; c < kCells; ++c) {
+      uint8_t b = root.cell[c];
+      if (is_piece(b) && owner_of(b) != searcher && !(b & B_REVEALED)) {
+        if (n >= 40) return ORC_BAD_STATE;
+        H[n] = c; T[n] = type_of(b); ++n;
+      }
+    }
+    for (int s = 0; s < samples_per_root; ++s) {
+      int G = r * samples_per_root + s;
+      uint32_t gidx = (uint32_t)(out->cfg.game_base + (uint64_t)G);
+      Game gm = root;
+      int P[40];
+      int attempt = 0;
+      for (;; ++attempt) {
+        if (attempt >= 4096) return ORC_BAD_STATE;
+        for (int i = 0; i < n; ++i) P[i] = T[i];
+        for (int i = n - 1; i >= 1; --i) {
+          uint32_t u = stream_draw(seed, gidx, (uint32_t)attempt, 0, TAG_DETERMINISE, n - 1 - i);
+          int j = (int)bounded(u, (uint32_t)(i + 1));
+          int tmp = P[i]; P[i] = P[j]; P[j] = tmp;
+        }
+        bool okp = true;
+        for (int i = 0; i < n; ++i)
+          if ((P[i] == T_BOMB || P[i] == T_FLAG) && (root.cell[H[i]] & B_MOVED)) okp = false;
+        if (okp) break;
+      }
+      for (int i = 0; i < n; ++i) gm.cell[H[i]] = (uint8_t)((root.cell[H[i]] & 0xF0) | P[i]);
+      if (attempts) attempts[G] = attempt + 1;
+      out->g[G] = gm;
+    }
+  }
+  return ORC_OK;
+}
+
+// Per-root reduction of rollout returns (R#23): return = red's result from the
+// searcher's perspective, 0 if the game is unfinished.  out[r] = {sum, wins, losses}.
+int orc_reduce_returns(const Env* games, const uint8_t* root_side, int32_t samples_per_root, int32_t* out) {
+  if (!games || !root_side || !out || samples_per_root <= 0) return ORC_BAD_ARG;
+  if (games->cfg.num_games % samples_per_root) return ORC_BAD_ARG;
+  int R = games->cfg.num_games / samples_per_root;
+  for (int r = 0; r < R; ++r) {
+    int sum = 0, wins = 0, losses = 0;
+    for (int s = 0; s < samples_per_root; ++s) {
+      const Game& gm = games->g[(size_t)r * samples_per_root + s];
+      int ret = gm.done ? gm.result * (root_side[r] == 0 ? +1 : -1) : 0;
+      sum += ret; if (ret > 0) ++wins; if (ret < 0) ++losses;
+    }
+    out[3 * r] = sum; out[3 * r + 1] = wins; out[3 * r + 2] = losses;
+  }
+  return ORC_OK;
+}
+
+// ---- probes used by the pins only
+void orc_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox4x32_10(ctr, key, out); }
+int orc_battle(int att, int def) { return battle(att, def); }
+int orc_is_lake(int c) { return is_lake(c) ? 1 : 0; }
+void orc_multiset(int variant, int32_t out[40]) { int A[40]; multiset(variant, A); for (int i = 0; i < 40; ++i) out[i] = A[i]; }
+// chain of player `side` of game gi: returns length, fills pos[4].
+int orc_chain(const Env* e, int gi, int side, int32_t pos[4]) {
+  const Game& gm = e->g[gi];
+  for (int i = 0; i < gm.chain_len[side]; ++i) pos[i] = gm.chain[side][i];
+  return gm.chain_len[side];
+}
+// Number of legal moves of `side` as if it were its turn (GetHasLegalMovement).
+int orc_count_moves(const Env* e, int gi, int side) { return gen_moves(e->g[gi], e->cfg, side, nullptr); }
+
+}  // extern "C"
