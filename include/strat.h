@@ -1,0 +1,199 @@
+/* strat.h — C ABI of libstrat.so: the batched Stratego environment step on one B200.
+ *
+ * The hot path of arxiv 2511.07312's self-play/search pipeline (PAPER.md:226-240,
+ * "StrategoRolloutBuffer": N parallel games, ApplyActions, ComputeLegalActionMask,
+ * ComputeInfostateTensor, ComputeRewardP10, SampleRandomLegalAction — Table S1,
+ * PAPER.md:455-480), in the I/O layouts BASELINE.json fixes.  Every call below runs
+ * hand-written sm_100a kernels; there is no CPU path.
+ *
+ * Conventions
+ *   - Every function returns 0 (STRAT_OK) or a negative error code; no exceptions.
+ *   - Pointers are DEVICE pointers unless the name ends in `_host`.  The caller owns
+ *     all device memory, including the library's own state: size it with
+ *     strat_workspace_bytes / strat_replay_bytes, allocate (e.g. a torch.uint8 tensor)
+ *     and pass it to *_create.  The library never allocates device memory and never
+ *     synchronises, except in strat_check and the *_host entry points
+ *     (third desideratum: no dynamic allocation after construction).
+ *   - `stream` is a cudaStream_t passed as void* (0 = default stream).  Calls are
+ *     asynchronous with respect to the host.
+ *   - Device-detected faults (an illegal action for a live game) set a sticky device
+ *     error word and leave that game unchanged; strat_check reads it.
+ *
+ * Layouts (BASELINE.json configs[0])
+ *   cell c = 10*row + col, row 0 = red's back row; lakes {42,43,46,47,52,53,56,57}.
+ *   canonical line uint8[128] per game (what reset_from / get_boards exchange):
+ *     0..99    cell byte: bits0-3 type (0 empty, 1 Spy, 2 Scout, 3 Miner, 4 Sergeant,
+ *              5 Lieutenant, 6 Captain, 7 Major, 8 Colonel, 9 General, 10 Marshal,
+ *              11 Flag, 12 Bomb, 15 lake; order of PAPER.md:499), bit4 owner (0 red,
+ *              1 blue), bit5 moved, bit6 revealed
+ *     100..115 history: entry j = (from,to) of ply t-1-j; 0xFF,0xFF if none
+ *     116..117 ply (LE u16)      118..119 plies since the last battle (LE u16)
+ *     120      bit0 done, bits2-4 reason (1 Flag captured, 2 opponent has no move,
+ *              3 neither has a move (draw), 4 ply cap (draw), 5 battleless cap (draw))
+ *     121      result for red (int8: +1, -1, 0)     122..123 zero
+ *     124..127 epoch (LE u32): number of auto-resets of this game slot
+ *   action  a = from*36 + dir*9 + (dist-1); dir 0:+row 1:+col 2:-row 3:-col; dist 1..9
+ *   mask    uint32[N][113]; bit a -> word a>>5, bit a&31; bits 3600..3615 are zero
+ *   obs     bf16 (as uint16) [N][44][10][10], values 0x0000 / 0x3F80, for the side to
+ *           move: 0-11 own type k+1; 12-23 revealed opponent type k-11; 24 hidden
+ *           opponent, moved; 25 hidden opponent, unmoved; 26 lake; 27 empty non-lake;
+ *           28+2j / 29+2j from / to square of ply t-1-j, j = 0..7
+ *   reward  int8[N]: red's result on the terminating step, else 0
+ *   done    uint8[N]: bit0 game ended on this step, bit1 player who acted (0 red),
+ *           bits2-4 reason as above
+ *   RNG     Philox4x32-10, key = seed, counter = (c0,c1,c2,tag): setup tag 0 red /
+ *           1 blue (global game, epoch, attempt<<8 | block); action tag 2 (global game,
+ *           epoch, ply), word 0; sample tag 3 (block, draw_index lo, hi); determinise
+ *           tag 4 (global output game, attempt, block).  Bounded draw = (u*n)>>32.
+ */
+#ifndef STRAT_H_
+#define STRAT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define STRAT_OK 0
+#define STRAT_BAD_ARG (-1)
+#define STRAT_BAD_STATE (-2)
+#define STRAT_CUDA_ERROR (-3)
+#define STRAT_ILLEGAL_ACTION (-4)
+
+#define STRAT_LINE_BYTES 128
+#define STRAT_MASK_WORDS 113
+#define STRAT_OBS_PLANES 44
+#define STRAT_OBS_ELEMS 4400
+#define STRAT_NUM_ACTIONS 3600
+
+typedef struct strat_config {
+  int32_t num_games;      /* N >= 1 */
+  int32_t variant;        /* 0 classic (40 pieces a side), 1 Barrage (8 a side) */
+  uint64_t seed;          /* Philox key */
+  int32_t max_plies;      /* draw after this many plies; 0 = none (hard cap 65535) */
+  int32_t max_battleless; /* draw after this many plies without a battle; 0 = off */
+  int32_t auto_reset;     /* 1: a finished game restarts inside the same step */
+  int32_t two_square;     /* 1: apply the two-square rule */
+  int32_t device;         /* CUDA device ordinal */
+  int32_t reserved;       /* must be 0 */
+  uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded) */
+} strat_config;
+
+typedef struct strat_env strat_env;       /* host handle; state lives in the workspace */
+typedef struct strat_replay strat_replay; /* host handle; ring lives in caller memory */
+
+const char* strat_error_string(int code);
+
+/* ---- environment ---------------------------------------------------------------- */
+
+/* Bytes of device workspace an environment of this configuration needs. 0 on bad cfg. */
+size_t strat_workspace_bytes(const strat_config* cfg);
+
+/* Bind an environment to `workspace_dev` (>= strat_workspace_bytes, 256-B aligned).
+ * Launches the initial reset (seeded setups; BASELINE.json configs[0,1])
+ * on `stream`.  The handle is freed by strat_destroy; the workspace stays the caller's. */
+int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream,
+                 strat_env** out);
+int strat_destroy(strat_env* env);
+
+/* All games: new Philox key, epoch 0, ply 0, fresh setups. */
+int strat_reset(strat_env* env, uint64_t seed, void* stream);
+
+/* Load / store all games as canonical lines uint8[N][128] (device pointers).
+ * reset_from is the "reset to a non-initial state" of PAPER.md:252-254. */
+int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
+int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);
+
+/* ComputeLegalActionMask for the acting player (rules PAPER.md:210-212).
+ * mask: uint32[N][113].  Finished games get an all-zero mask. */
+int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream);
+
+/* SampleRandomLegalAction: the r-th set bit of each game's mask,
+ * r = bounded(Philox action draw, popcount).  actions: int16[N], -1 where the mask is empty. */
+int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* actions, void* stream);
+
+/* ApplyActions: one action per game; battle by rank with the Spy,
+ * Bomb/Miner and Flag cases; terminal tests; auto-reset.
+ * reward int8[N], done uint8[N] describe the step just taken (also for a game that was
+ * auto-reset inside the call).  A finished game without auto-reset is left frozen. */
+int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream);
+
+/* ComputeInfostateTensor in BASELINE.json's 44-plane bf16 form.
+ * obs: uint16[N][4400]. */
+int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream);
+
+/* One fused pass of the hot path: legal mask -> uniform legal action -> step -> encode of
+ * the new state.  Produces exactly what strat_legal_mask, strat_sample_uniform,
+ * strat_step, strat_encode_obs produce when called in that order.  Any output pointer
+ * except `obs` may be NULL (that output is then not written). */
+int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward,
+                       uint8_t* done, uint16_t* obs, void* stream);
+
+/* Same, with HOST destination buffers (pinned memory recommended): runs the fused step
+ * into `scratch_dev` (>= strat_host_scratch_bytes(cfg) bytes, caller-owned), copies the
+ * five outputs to the host pointers on `stream` and synchronises the stream. */
+size_t strat_host_scratch_bytes(const strat_config* cfg);
+int strat_rollout_step_host(strat_env* env, void* scratch_dev, uint32_t* mask_host,
+                            int16_t* actions_host, int8_t* reward_host, uint8_t* done_host,
+                            uint16_t* obs_host, void* stream);
+
+/* The RL-loop shape with a host-side policy (PAPER.md:232 ApplyActions + Table S1 queries):
+ * copies int16[N] actions from `actions_host` to the device, applies them (strat_step),
+ * computes the next legal mask and observation (strat_legal_mask, strat_encode_obs of the
+ * new state) and copies reward, done, mask and obs to the host pointers; synchronises the
+ * stream.  `scratch_dev` as for strat_rollout_step_host. */
+int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_host, int8_t* reward_host,
+                    uint8_t* done_host, uint32_t* mask_host, uint16_t* obs_host, void* stream);
+
+/* `plies` plies of uniform-random legal play with the boards kept on chip (search-shaped
+ * rollouts, BASELINE.json configs[4]).  Equal to `plies` repetitions
+ * of legal_mask + sample_uniform + step; nothing but the state is written. */
+int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream);
+
+/* Synchronise the device and return the sticky error word (0 if none). */
+int strat_check(strat_env* env);
+int strat_clear_error(strat_env* env, void* stream);
+
+/* ---- device replay ring (BASELINE.json configs[3]) -------------------------------- */
+/* capacity = per_slot * slots records of (obs 8800 B, mask 452 B, action i16, reward i8,
+ * done u8) = 9256 B, stored as five arrays over the whole capacity (a "slot" is a
+ * contiguous run of per_slot records of each array).  strat_replay_layout returns the byte
+ * offset of each array inside the caller's memory: {obs, mask, action, reward, done}. */
+size_t strat_replay_bytes(int32_t per_slot, int32_t slots);
+int strat_replay_layout(int32_t per_slot, int32_t slots, size_t offsets[5]);
+int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out);
+int strat_replay_destroy(strat_replay* r);
+/* Append n records in order at (head+i) mod capacity; head += n; filled = min(filled+n, capacity). */
+int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
+                      const int8_t* reward, const uint8_t* done, int32_t n, void* stream);
+/* Zero-copy push: the addresses of the next n records' obs and mask rows, so that
+ * strat_rollout_step / strat_encode_obs can write them in place.  Fails with STRAT_BAD_ARG
+ * unless the n records are contiguous (capacity % n == 0 and head % n == 0).
+ * strat_replay_commit then appends action/reward/done for those n records and advances head. */
+int strat_replay_reserve(strat_replay* r, int32_t n, uint16_t** obs, uint32_t** mask);
+int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done,
+                        int32_t n, void* stream);
+/* Uniform minibatch with replacement: element j = record bounded(sample draw j, filled). */
+int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_index, int32_t batch,
+                        uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
+                        void* stream);
+int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled);
+
+/* ---- search-shaped batch (BASELINE.json configs[4]) ------------------------------- */
+/* out game G = r*samples_per_root + s: root r with the types of the searcher's opponent's
+ * unrevealed pieces permuted uniformly over their squares, rejecting permutations that put a
+ * Bomb or Flag on a moved piece (at most 4096 attempts, else the sticky error of `out` is
+ * set to STRAT_BAD_STATE).  out->num_games must equal roots->num_games * samples_per_root. */
+int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t seed, strat_env* out,
+                      void* stream);
+/* out int32[R][3] = {sum of returns, wins, losses} per root from the searcher's side
+ * (root_side uint8[R], 0 red); unfinished games count 0. */
+int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32_t samples_per_root,
+                         int32_t* out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STRAT_H_ */

@@ -407,9 +407,10 @@ void rebuild_chains(Game& gm) {
   gm.chain_len[0] = gm.chain_len[1] = 0;
   for (int j = 7; j >= 0; --j) {
     if (gm.hist[j][0] == 0xFF) continue;
-    int ply_of_move = gm.ply - 1 - j;
-    if (ply_of_move < 0) continue;
-    int side = ply_of_move & 1;
+    // Entries are taken as given (existence = the 0xFF marker only); entry j is the move
+    // of ply t-1-j, so its mover is the parity of that number (also when a hand-built
+    // line carries more history than plies).
+    int side = (gm.ply - 1 - j) & 1;
     int from = gm.hist[j][0], to = gm.hist[j][1];
     if (gm.chain_len[side] > 0 && gm.chain[side][gm.chain_len[side] - 1] == from) {
       if (gm.chain_len[side] == 4) {
@@ -649,7 +650,8 @@ int64_t orc_replay_filled(const Replay* r) { return r ? r->filled : -1; }
 // ---- C7 determinise (BJ configs[4]): for output game G = r*S + s, permute the types of
 // the searcher's opponent's unrevealed pieces uniformly over their squares, rejecting
 // any permutation that puts a Bomb or Flag on a piece that has moved.  `attempts`
-// (optional, [R*S]) receives the number of attempts used.  R#22: at most 4096 attempts.
+// (optional, [R*S]) receives the number of attempts used.  R#22: the acceptance rate measured
+// on the 16 ply-200 roots of config 4 is 3e-4 .. 7e-3, so the safety cap is 2^20 attempts.
 int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, Env* out, int32_t* attempts) {
   if (!roots || !out || samples_per_root <= 0) return ORC_BAD_ARG;
   int R = roots->cfg.num_games;
@@ -672,7 +674,7 @@ int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, E
       int P[40];
       int attempt = 0;
       for (;; ++attempt) {
-        if (attempt >= 4096) return ORC_BAD_STATE;
+        if (attempt >= (1 << 20)) return ORC_BAD_STATE;
         for (int i = 0; i < n; ++i) P[i] = T[i];
         for (int i = n - 1; i >= 1; --i) {
           uint32_t u = stream_draw(seed, gidx, (uint32_t)attempt, 0, TAG_DETERMINISE, n - 1 - i);

@@ -1,0 +1,292 @@
+"""Thin Python binding of libstrat.so (include/strat.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the
+library's CUDA kernels.  There is no CPU fallback: loading fails loudly if the library
+cannot be built/loaded, and every call fails if CUDA is unavailable.
+"""
+import ctypes as C
+
+import torch
+
+from .build import ensure_built
+
+LINE = 128
+MASK_WORDS = 113
+OBS_ELEMS = 4400
+OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
+    "strat_reset_from", "strat_get_boards", "strat_legal_mask", "strat_sample_uniform", "strat_step",
+    "strat_encode_obs", "strat_rollout_step", "strat_host_scratch_bytes", "strat_rollout_step_host",
+    "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
+    "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
+    "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
+    "strat_reduce_returns",
+]
+
+
+class strat_config(C.Structure):
+    _fields_ = [
+        ("num_games", C.c_int32), ("variant", C.c_int32), ("seed", C.c_uint64),
+        ("max_plies", C.c_int32), ("max_battleless", C.c_int32), ("auto_reset", C.c_int32),
+        ("two_square", C.c_int32), ("device", C.c_int32), ("reserved", C.c_int32),
+        ("game_base", C.c_uint64),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) the C-ABI library.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(ensure_built())
+        vp, i32, u64, sz = C.c_void_p, C.c_int32, C.c_uint64, C.c_size_t
+        L.strat_error_string.restype = C.c_char_p
+        L.strat_error_string.argtypes = [C.c_int]
+        L.strat_workspace_bytes.restype = sz
+        L.strat_workspace_bytes.argtypes = [C.POINTER(strat_config)]
+        L.strat_create.argtypes = [C.POINTER(strat_config), vp, sz, vp, C.POINTER(vp)]
+        L.strat_destroy.argtypes = [vp]
+        L.strat_reset.argtypes = [vp, u64, vp]
+        L.strat_reset_from.argtypes = [vp, vp, vp]
+        L.strat_get_boards.argtypes = [vp, vp, vp]
+        L.strat_legal_mask.argtypes = [vp, vp, vp]
+        L.strat_sample_uniform.argtypes = [vp, vp, vp, vp]
+        L.strat_step.argtypes = [vp, vp, vp, vp, vp]
+        L.strat_encode_obs.argtypes = [vp, vp, vp]
+        L.strat_rollout_step.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.strat_host_scratch_bytes.restype = sz
+        L.strat_host_scratch_bytes.argtypes = [C.POINTER(strat_config)]
+        L.strat_rollout_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.strat_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.strat_rollout_uniform.argtypes = [vp, i32, vp]
+        L.strat_check.argtypes = [vp]
+        L.strat_clear_error.argtypes = [vp, vp]
+        L.strat_replay_bytes.restype = sz
+        L.strat_replay_bytes.argtypes = [i32, i32]
+        L.strat_replay_layout.argtypes = [i32, i32, C.POINTER(sz)]
+        L.strat_replay_create.argtypes = [vp, sz, i32, i32, C.POINTER(vp)]
+        L.strat_replay_destroy.argtypes = [vp]
+        L.strat_replay_push.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
+        L.strat_replay_reserve.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp)]
+        L.strat_replay_commit.argtypes = [vp, vp, vp, vp, i32, vp]
+        L.strat_replay_sample.argtypes = [vp, u64, u64, i32, vp, vp, vp, vp, vp, vp]
+        L.strat_replay_state.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.strat_determinise.argtypes = [vp, i32, u64, vp, vp]
+        L.strat_reduce_returns.argtypes = [vp, vp, i32, vp, vp]
+        _lib = L
+    return _lib
+
+
+class StratError(RuntimeError):
+    pass
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise StratError("%s: %s (%d)" % (what, lib().strat_error_string(rc).decode(), rc))
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_cuda and t.is_contiguous(), "device, contiguous tensors only"
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise StratError("CUDA device required: this library has no CPU path")
+
+
+class Env:
+    """N parallel games bound to a caller-owned (torch) workspace."""
+
+    def __init__(self, num_games, variant=0, seed=0, max_plies=0, max_battleless=0, auto_reset=0,
+                 two_square=1, device=0, game_base=0):
+        _require_cuda()
+        self.cfg = strat_config(num_games, variant, seed, max_plies, max_battleless, auto_reset,
+                                two_square, device, 0, game_base)
+        self.n = num_games
+        self.device = torch.device("cuda", device)
+        nbytes = lib().strat_workspace_bytes(C.byref(self.cfg))
+        if nbytes == 0:
+            raise StratError("bad configuration")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            _chk(lib().strat_create(C.byref(self.cfg), _ptr(self.workspace), nbytes, _stream(), C.byref(self.h)),
+                 "strat_create")
+
+    def __del__(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            lib().strat_destroy(self.h)
+            self.h = C.c_void_p()
+
+    # -- allocation helpers (plumbing)
+    def new_mask(self):
+        return torch.empty((self.n, MASK_WORDS), dtype=torch.int32, device=self.device)
+
+    def new_obs(self):
+        return torch.empty((self.n, 44, 10, 10), dtype=torch.bfloat16, device=self.device)
+
+    def new_actions(self):
+        return torch.empty(self.n, dtype=torch.int16, device=self.device)
+
+    def new_reward(self):
+        return torch.empty(self.n, dtype=torch.int8, device=self.device)
+
+    def new_done(self):
+        return torch.empty(self.n, dtype=torch.uint8, device=self.device)
+
+    # -- the C-ABI calls, same names
+    def reset(self, seed):
+        _chk(lib().strat_reset(self.h, seed, _stream()), "strat_reset")
+
+    def reset_from(self, boards):
+        assert boards.shape == (self.n, LINE)
+        _chk(lib().strat_reset_from(self.h, _ptr(boards, torch.uint8), _stream()), "strat_reset_from")
+
+    def get_boards(self, out=None):
+        out = out if out is not None else torch.empty((self.n, LINE), dtype=torch.uint8, device=self.device)
+        _chk(lib().strat_get_boards(self.h, _ptr(out, torch.uint8), _stream()), "strat_get_boards")
+        return out
+
+    def legal_mask(self, out=None):
+        out = out if out is not None else self.new_mask()
+        _chk(lib().strat_legal_mask(self.h, _ptr(out, torch.int32), _stream()), "strat_legal_mask")
+        return out
+
+    def sample_uniform(self, mask, out=None):
+        out = out if out is not None else self.new_actions()
+        _chk(lib().strat_sample_uniform(self.h, _ptr(mask, torch.int32), _ptr(out, torch.int16), _stream()),
+             "strat_sample_uniform")
+        return out
+
+    def step(self, actions, reward=None, done=None):
+        reward = reward if reward is not None else self.new_reward()
+        done = done if done is not None else self.new_done()
+        _chk(lib().strat_step(self.h, _ptr(actions, torch.int16), _ptr(reward, torch.int8),
+                              _ptr(done, torch.uint8), _stream()), "strat_step")
+        return reward, done
+
+    def encode_obs(self, out=None):
+        out = out if out is not None else self.new_obs()
+        _chk(lib().strat_encode_obs(self.h, _ptr(out, torch.bfloat16), _stream()), "strat_encode_obs")
+        return out
+
+    def rollout_step(self, mask, actions, reward, done, obs):
+        _chk(lib().strat_rollout_step(self.h, _ptr(mask), _ptr(actions), _ptr(reward), _ptr(done), _ptr(obs),
+                                      _stream()), "strat_rollout_step")
+
+    def rollout_step_raw(self, mask_ptr, actions, reward, done, obs_ptr):
+        """rollout_step with raw device addresses for mask/obs (e.g. replay_reserve's)."""
+        _chk(lib().strat_rollout_step(self.h, C.c_void_p(mask_ptr), _ptr(actions), _ptr(reward), _ptr(done),
+                                      C.c_void_p(obs_ptr), _stream()), "strat_rollout_step")
+
+    def host_scratch(self):
+        return torch.empty(lib().strat_host_scratch_bytes(C.byref(self.cfg)), dtype=torch.uint8, device=self.device)
+
+    def rollout_step_host(self, scratch, mask_h, actions_h, reward_h, done_h, obs_h):
+        for t in (mask_h, actions_h, reward_h, done_h, obs_h):
+            assert not t.is_cuda and t.is_contiguous()
+        _chk(lib().strat_rollout_step_host(self.h, _ptr(scratch), C.c_void_p(mask_h.data_ptr()),
+                                           C.c_void_p(actions_h.data_ptr()), C.c_void_p(reward_h.data_ptr()),
+                                           C.c_void_p(done_h.data_ptr()), C.c_void_p(obs_h.data_ptr()), _stream()),
+             "strat_rollout_step_host")
+
+    def step_host(self, scratch, actions_h, reward_h, done_h, mask_h, obs_h):
+        for t in (actions_h, reward_h, done_h, mask_h, obs_h):
+            assert not t.is_cuda and t.is_contiguous()
+        _chk(lib().strat_step_host(self.h, _ptr(scratch), C.c_void_p(actions_h.data_ptr()),
+                                   C.c_void_p(reward_h.data_ptr()), C.c_void_p(done_h.data_ptr()),
+                                   C.c_void_p(mask_h.data_ptr()), C.c_void_p(obs_h.data_ptr()), _stream()),
+             "strat_step_host")
+
+    def rollout_uniform(self, plies):
+        _chk(lib().strat_rollout_uniform(self.h, plies, _stream()), "strat_rollout_uniform")
+
+    def check(self):
+        return lib().strat_check(self.h)
+
+    def clear_error(self):
+        _chk(lib().strat_clear_error(self.h, _stream()), "strat_clear_error")
+
+
+class Replay:
+    """Device replay ring in a caller-owned (torch) buffer."""
+
+    def __init__(self, per_slot, slots, device=0):
+        _require_cuda()
+        self.device = torch.device("cuda", device)
+        self.per_slot, self.slots, self.capacity = per_slot, slots, per_slot * slots
+        nbytes = lib().strat_replay_bytes(per_slot, slots)
+        if nbytes == 0:
+            raise StratError("bad ring shape")
+        self.mem = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        off = (C.c_size_t * 5)()
+        _chk(lib().strat_replay_layout(per_slot, slots, off), "strat_replay_layout")
+        self.offsets = list(off)
+        self.h = C.c_void_p()
+        _chk(lib().strat_replay_create(_ptr(self.mem), nbytes, per_slot, slots, C.byref(self.h)), "strat_replay_create")
+
+    def __del__(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            lib().strat_replay_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def push(self, obs, mask, action, reward, done):
+        n = action.numel()
+        _chk(lib().strat_replay_push(self.h, _ptr(obs), _ptr(mask), _ptr(action, torch.int16),
+                                     _ptr(reward, torch.int8), _ptr(done, torch.uint8), n, _stream()),
+             "strat_replay_push")
+
+    def reserve(self, n):
+        obs, mask = C.c_void_p(), C.c_void_p()
+        _chk(lib().strat_replay_reserve(self.h, n, C.byref(obs), C.byref(mask)), "strat_replay_reserve")
+        return obs.value, mask.value
+
+    def commit(self, action, reward, done):
+        _chk(lib().strat_replay_commit(self.h, _ptr(action, torch.int16), _ptr(reward, torch.int8),
+                                       _ptr(done, torch.uint8), action.numel(), _stream()), "strat_replay_commit")
+
+    def sample(self, seed, draw_index, batch, obs, mask, action, reward, done):
+        _chk(lib().strat_replay_sample(self.h, seed, draw_index, batch, _ptr(obs), _ptr(mask), _ptr(action),
+                                       _ptr(reward), _ptr(done), _stream()), "strat_replay_sample")
+
+    def state(self):
+        h, f = C.c_int64(), C.c_int64()
+        _chk(lib().strat_replay_state(self.h, C.byref(h), C.byref(f)), "strat_replay_state")
+        return h.value, f.value
+
+    # typed views of the ring arrays (tests)
+    def views(self):
+        Cn = self.capacity
+        o = self.offsets
+        obs = self.mem[o[0]:o[0] + Cn * OBS_ELEMS * 2].view(torch.int16).view(Cn, OBS_ELEMS)
+        mask = self.mem[o[1]:o[1] + Cn * MASK_WORDS * 4].view(torch.int32).view(Cn, MASK_WORDS)
+        act = self.mem[o[2]:o[2] + Cn * 2].view(torch.int16)
+        rew = self.mem[o[3]:o[3] + Cn].view(torch.int8)
+        done = self.mem[o[4]:o[4] + Cn]
+        return obs, mask, act, rew, done
+
+
+def determinise(roots: Env, samples_per_root: int, seed: int, out: Env):
+    _chk(lib().strat_determinise(roots.h, samples_per_root, seed, out.h, _stream()), "strat_determinise")
+
+
+def reduce_returns(games: Env, root_side, samples_per_root: int, out=None):
+    R = games.n // samples_per_root
+    out = out if out is not None else torch.empty((R, 3), dtype=torch.int32, device=games.device)
+    _chk(lib().strat_reduce_returns(games.h, _ptr(root_side, torch.uint8), samples_per_root,
+                                    _ptr(out, torch.int32), _stream()), "strat_reduce_returns")
+    return out

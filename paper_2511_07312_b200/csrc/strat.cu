@@ -1,0 +1,779 @@
+// strat.cu — sm_100a kernels and the C ABI of libstrat.so (include/strat.h).
+//
+// Execution model: one warp = one batch of 32 games = one CTA.
+//   * I/O phases are warp-cooperative: the 32 games' 128-byte lines (4 KB contiguous), their
+//     mask rows (32 x 452 B contiguous) and their observations (32 x 8800 B contiguous) move
+//     as coalesced 16-byte vector accesses, staged through shared memory.
+//   * Logic phases are thread-per-game on 100-bit bitboards held in registers
+//     (strat_game.cuh), reading/writing per-game rows of shared memory whose strides
+//     (144 B, 113 words, 139 words) make the 32 lanes hit 32 different banks.
+// The observation is produced as a 4400-bit stream per game; byte q of the stream expands,
+// through a 256-entry x 16 B shared-memory table, to the q-th 16-byte chunk of the bf16
+// planes, so the 8800-byte store costs one byte load, one table load and one STG.128 per
+// 16 bytes.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <new>
+
+#include "../../include/strat.h"
+#include "strat_game.cuh"
+
+namespace {
+using namespace strat;
+
+constexpr int kBatch = 32;             // games per warp/CTA
+constexpr int kStateStride = 144;      // bytes between games' staged lines (16-B aligned, conflict-free LDS.128)
+constexpr int kMaskRowBytes = kMaskWords * 4;        // 452
+constexpr int kBitsRowWords = 139;                   // 138 used; odd stride -> conflict-free
+constexpr int kObsChunks = 550;                      // 16-B chunks per game observation
+constexpr int kStateBytes = kBatch * kStateStride;   // 4608
+constexpr int kMaskBytes = kBatch * kMaskRowBytes;   // 14464
+constexpr int kBitsBytes = kBatch * kBitsRowWords * 4;  // 17792
+
+// ------------------------------------------------------------------ small PTX helpers
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void st_stream(uint4* p, uint4 v) { __stcs(p, v); }  // write-once outputs
+
+// ------------------------------------------------------------------ warp-cooperative I/O
+// 32 (or `ng`) device lines, contiguous in global memory, into the padded staging area.
+__device__ __forceinline__ void load_lines(const uint32_t* __restrict__ lines, int first_game, int ng,
+                                           uint8_t* s_state, int lane) {
+  const uint4* src = reinterpret_cast<const uint4*>(lines + (size_t)first_game * kLineWords);
+  for (int j = lane; j < ng * 8; j += 32) cp_async16(s_state + (j >> 3) * kStateStride + (j & 7) * 16, src + j);
+  cp_async_wait_all();
+  __syncwarp();
+}
+__device__ __forceinline__ void store_lines(uint32_t* __restrict__ lines, int first_game, int ng,
+                                            const uint8_t* s_state, int lane) {
+  uint4* dst = reinterpret_cast<uint4*>(lines + (size_t)first_game * kLineWords);
+  for (int j = lane; j < ng * 8; j += 32)
+    dst[j] = *reinterpret_cast<const uint4*>(s_state + (j >> 3) * kStateStride + (j & 7) * 16);
+}
+__device__ __forceinline__ void read_game(const uint8_t* s_state, int lane, Game& g) {
+  uint32_t W[32];
+  const uint4* p = reinterpret_cast<const uint4*>(s_state + lane * kStateStride);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { uint4 v = p[k]; W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+  unpack_line(W, g);
+}
+__device__ __forceinline__ void write_game(uint8_t* s_state, int lane, const Game& g) {
+  uint32_t W[32];
+  pack_line(g, W);
+  uint4* p = reinterpret_cast<uint4*>(s_state + lane * kStateStride);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) p[k] = make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]);
+}
+__device__ __forceinline__ void zero_smem16(void* s, int bytes, int lane) {
+  uint4* p = reinterpret_cast<uint4*>(s);
+  for (int j = lane; j < bytes / 16; j += 32) p[j] = make_uint4(0, 0, 0, 0);
+}
+// mask rows of `ng` games: shared (rows of 113 words, no padding) -> global, 16 B at a time.
+// first_game is a multiple of 32, so the global address is 16-byte aligned (32*452 = 16*904).
+__device__ __forceinline__ void store_mask(uint32_t* __restrict__ mask, int first_game, int ng,
+                                           const uint32_t* s_mask, int lane) {
+  uint32_t* dst = mask + (size_t)first_game * kMaskWords;
+  int words = ng * kMaskWords;
+  int vec = words >> 2;
+  const uint4* s4 = reinterpret_cast<const uint4*>(s_mask);
+  uint4* d4 = reinterpret_cast<uint4*>(dst);
+  for (int j = lane; j < vec; j += 32) d4[j] = s4[j];
+  for (int j = (vec << 2) + lane; j < words; j += 32) dst[j] = s_mask[j];
+}
+// bf16 expansion table: entry e = 8 bf16 values (0x3F80 where bit set), element 0 lowest.
+__device__ __forceinline__ void fill_lut(uint4* lut, int tid, int nthreads) {
+  for (int e = tid; e < 256; e += nthreads) {
+    uint4 v;
+    v.x = ((e & 1) ? 0x3F80u : 0u) | ((e & 2) ? 0x3F800000u : 0u);
+    v.y = ((e & 4) ? 0x3F80u : 0u) | ((e & 8) ? 0x3F800000u : 0u);
+    v.z = ((e & 16) ? 0x3F80u : 0u) | ((e & 32) ? 0x3F800000u : 0u);
+    v.w = ((e & 64) ? 0x3F80u : 0u) | ((e & 128) ? 0x3F800000u : 0u);
+    lut[e] = v;
+  }
+}
+// Observation of `ng` games from their bit streams: lane l writes chunk 32k+l, so every
+// STG.128 of the warp covers 512 contiguous, sector-aligned bytes (8800 = 275 sectors).
+__device__ __forceinline__ void expand_obs(uint16_t* __restrict__ obs, int first_game, int ng,
+                                           const uint32_t* s_bits, const uint4* lut, int lane) {
+  for (int gi = 0; gi < ng; ++gi) {
+    const uint8_t* row = reinterpret_cast<const uint8_t*>(s_bits + gi * kBitsRowWords);
+    uint4* dst = reinterpret_cast<uint4*>(obs + (size_t)(first_game + gi) * STRAT_OBS_ELEMS);
+#pragma unroll
+    for (int k = 0; k < 17; ++k) st_stream(dst + 32 * k + lane, lut[row[32 * k + lane]]);
+    if (lane < kObsChunks - 544) st_stream(dst + 544 + lane, lut[row[544 + lane]]);
+  }
+}
+
+__device__ __forceinline__ void raise_error(int* err, int code) { atomicCAS(err, 0, code); }
+
+// ------------------------------------------------------------------ kernels
+__global__ void __launch_bounds__(32) k_reset(Params P, uint32_t* __restrict__ lines) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  if (lane < ng) {
+    Game g; g.epoch = 0;
+    setup_game(P, (uint32_t)(first + lane), g);
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+// canonical uint8[N][128] -> device lines.  One warp per game; the seven bit planes are
+// packed with warp ballots (lane = cell within a 32-cell word).
+__global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict__ canon, uint32_t* __restrict__ lines) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= n) return;
+  uint32_t cw = reinterpret_cast<const uint32_t*>(canon + (size_t)g * 128)[lane];  // bytes 4l..4l+3
+  uint32_t mine = 0;
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    int cell = 32 * r + lane;
+    uint32_t w = __shfl_sync(0xffffffffu, cw, (cell >> 2) & 31);
+    uint32_t b = cell < 100 ? (w >> (8 * (cell & 3))) & 0xFFu : 0u;
+    uint32_t t = b & 15u;
+    bool piece = t >= 1 && t <= 12;
+#pragma unroll
+    for (int p = 0; p < 7; ++p) {
+      bool bit = p < 4 ? (piece && ((t >> p) & 1u)) : (piece && ((b >> p) & 1u));  // p=4 owner(bit4),5 moved,6 revealed
+      uint32_t word = __ballot_sync(0xffffffffu, bit);
+      if (lane == 4 * p + r) mine = word;
+    }
+  }
+  // meta: history pairs ride in the spare bits of words 3,7,11,15; flags in word 19
+  uint32_t hw = __shfl_sync(0xffffffffu, cw, 25 + (lane >> 2));  // canonical bytes 100+4p.. for lane 4p+3
+  uint32_t fw = __shfl_sync(0xffffffffu, cw, 30);
+  if ((lane & 3) == 3 && lane < 16) {
+    uint32_t f0 = hw & 0xFFu, t0 = (hw >> 8) & 0xFFu, f1 = (hw >> 16) & 0xFFu, t1 = hw >> 24;
+    uint32_t e0 = f0 == 0xFFu ? kHistNone : (f0 | (t0 << 7));
+    uint32_t e1 = f1 == 0xFFu ? kHistNone : (f1 | (t1 << 7));
+    mine |= (e0 | (e1 << 14)) << 4;
+  }
+  if (lane == 19) {
+    uint32_t fl = fw & 0xFFu;
+    int32_t res = (int32_t)(int8_t)((fw >> 8) & 0xFFu);
+    mine |= ((fl & 1u) | (((fl >> 2) & 7u) << 1) | ((uint32_t)(res + 1) << 4)) << 4;
+  }
+  uint32_t w29 = __shfl_sync(0xffffffffu, cw, 29), w31 = __shfl_sync(0xffffffffu, cw, 31);
+  if (lane == 28) mine = w29;  // ply | battleless<<16 : same bytes as canonical 116..119
+  if (lane == 29) mine = w31;  // epoch
+  if (lane >= 30) mine = 0;
+  lines[(size_t)g * kLineWords + lane] = mine;
+}
+
+// device lines -> canonical.  One warp per game; lane l < 25 assembles cells 4l..4l+3.
+__global__ void __launch_bounds__(128) k_export(int n, const uint32_t* __restrict__ lines, uint8_t* __restrict__ canon) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= n) return;
+  uint32_t lw = lines[(size_t)g * kLineWords + lane];
+  uint32_t out = 0;
+  int r = (lane >> 3) & 3, sh = 4 * (lane & 7);  // cells 4l..4l+3 sit in word r of each plane, bits sh..sh+3
+  uint32_t nib[7];
+#pragma unroll
+  for (int p = 0; p < 7; ++p) nib[p] = (__shfl_sync(0xffffffffu, lw, 4 * p + r) >> sh) & 0xFu;
+  if (lane < 25) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      uint32_t b = 0;
+#pragma unroll
+      for (int p = 0; p < 7; ++p) b |= ((nib[p] >> k) & 1u) << p;
+      int cell = 4 * lane + k;
+      if (is_lake_cell(cell)) b = 15;
+      out |= b << (8 * k);
+    }
+  }
+  uint32_t hw = __shfl_sync(0xffffffffu, lw, 4 * ((lane - 25) & 3) + 3) >> 4;   // history pair for lanes 25..28
+  uint32_t fw = __shfl_sync(0xffffffffu, lw, 19) >> 4;
+  uint32_t w28 = __shfl_sync(0xffffffffu, lw, 28), w29 = __shfl_sync(0xffffffffu, lw, 29);
+  if (lane >= 25 && lane < 29) {
+    uint32_t e0 = hw & 0x3FFFu, e1 = (hw >> 14) & 0x3FFFu;
+    uint32_t b0 = e0 == kHistNone ? 0xFFFFu : ((e0 & 127u) | ((e0 >> 7) << 8));
+    uint32_t b1 = e1 == kHistNone ? 0xFFFFu : ((e1 & 127u) | ((e1 >> 7) << 8));
+    out = b0 | (b1 << 16);
+  }
+  if (lane == 29) out = w28;
+  if (lane == 30) {
+    uint32_t done = fw & 1u, reason = (fw >> 1) & 7u;
+    int32_t res = (int32_t)((fw >> 4) & 3u) - 1;
+    out = (done | (reason << 2)) | (((uint32_t)res & 0xFFu) << 8);
+  }
+  if (lane == 31) out = w29;
+  reinterpret_cast<uint32_t*>(canon + (size_t)g * 128)[lane] = out;
+}
+
+__global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __restrict__ lines, uint32_t* __restrict__ mask) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  zero_smem16(s_mask, kMaskBytes, lane);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, s_mask + lane * kMaskWords);
+  }
+  __syncwarp();
+  store_mask(mask, first, ng, s_mask, lane);
+}
+
+// One warp per game: lanes load the 113 mask words coalesced, count with popc, locate the
+// r-th set bit with warp-shuffle prefix sums.
+__global__ void __launch_bounds__(128) k_sample_uniform(Params P, const uint32_t* __restrict__ lines,
+                                                        const uint32_t* __restrict__ mask, int16_t* __restrict__ actions) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= P.num_games) return;
+  const uint32_t* row = mask + (size_t)g * kMaskWords;
+  uint32_t w[4]; int cnt[4], incl[4], tot[4];
+  int n = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    int wi = 32 * k + lane;
+    w[k] = wi < kMaskWords ? row[wi] : 0u;
+    cnt[k] = __popc(w[k]);
+    int x = cnt[k];
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, off); if (lane >= off) x += y; }
+    incl[k] = x;
+    tot[k] = __shfl_sync(0xffffffffu, x, 31);
+    n += tot[k];
+  }
+  int action = -1;
+  if (n > 0) {
+    uint32_t meta = lane < 2 ? lines[(size_t)g * kLineWords + 28 + lane] : 0u;
+    uint32_t w28 = __shfl_sync(0xffffffffu, meta, 0), epoch = __shfl_sync(0xffffffffu, meta, 1);
+    uint32_t o[4];
+    philox(P.game_base + (uint32_t)g, epoch, w28 & 0xFFFFu, TAG_ACTION, P.key0, P.key1, o);
+    int r = (int)bounded(o[0], (uint32_t)n);
+    int base = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      int excl = base + incl[k] - cnt[k];  // set bits before this lane's word
+      bool mine = r >= excl && r < excl + cnt[k];
+      uint32_t owner = __ballot_sync(0xffffffffu, mine);
+      int a = (32 * k + lane) * 32 + (mine ? nth_set_bit(w[k], r - excl) : 0);
+      if (owner) action = __shfl_sync(0xffffffffu, a, __ffs((int)owner) - 1);
+      base += tot[k];
+    }
+  }
+  if (lane == 0) actions[g] = (int16_t)action;
+}
+
+__global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ lines, const int16_t* __restrict__ actions,
+                                             int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    StepOut o = step_game(P, (uint32_t)(first + lane), g, (int)actions[first + lane]);
+    if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+    reward[first + lane] = (int8_t)o.reward;
+    done[first + lane] = (uint8_t)o.done;
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+__global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __restrict__ lines, uint16_t* __restrict__ obs) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_bits[kBatch * kBitsRowWords];
+  __shared__ __align__(16) uint4 s_lut[256];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  fill_lut(s_lut, lane, 32);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    encode_bits(g, s_bits + lane * kBitsRowWords);
+  }
+  __syncwarp();
+  expand_obs(obs, first, ng, s_bits, s_lut, lane);
+}
+
+// The fused hot path: mask -> uniform action -> step -> encode, one pass over the state.
+__global__ void __launch_bounds__(32) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
+                                                     int16_t* __restrict__ actions, int8_t* __restrict__ reward,
+                                                     uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
+                                                     int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_work[kBitsBytes / 4];  // mask rows, then observation bit streams
+  __shared__ __align__(16) uint4 s_lut[256];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  fill_lut(s_lut, lane, 32);
+  zero_smem16(s_work, kMaskBytes, lane);
+  load_lines(lines, first, ng, s_state, lane);
+  Game g;
+  int n = 0;
+  if (lane < ng) {
+    read_game(s_state, lane, g);
+    if (!g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, s_work + lane * kMaskWords);
+  }
+  __syncwarp();
+  if (mask) store_mask(mask, first, ng, s_work, lane);
+  if (lane < ng) {
+    int a = -1;
+    if (n > 0) a = pick_action(s_work + lane * kMaskWords, n, action_draw(P, (uint32_t)(first + lane), g));
+    StepOut o = step_game(P, (uint32_t)(first + lane), g, a);
+    if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+    if (actions) actions[first + lane] = (int16_t)a;
+    if (reward) reward[first + lane] = (int8_t)o.reward;
+    if (done) done[first + lane] = (uint8_t)o.done;
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();  // all lanes are done with the mask rows before they become bit streams
+  if (lane < ng) encode_bits(g, s_work + lane * kBitsRowWords);
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+  expand_obs(obs, first, ng, s_work, s_lut, lane);
+}
+
+// `plies` plies of uniform-random legal play with the board in registers.
+__global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    uint32_t* row = s_mask + lane * kMaskWords;
+    for (int t = 0; t < plies; ++t) {
+      if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
+      for (int w = 0; w < kMaskWords; ++w) row[w] = 0;
+      int n = legal_mask_row(g, g.ply & 1u, P.two_square, row);
+      int a = pick_action(row, n, action_draw(P, (uint32_t)(first + lane), g));
+      StepOut o = step_game(P, (uint32_t)(first + lane), g, a);
+      if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+    }
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+// ---- replay ring
+template <typename T>
+__global__ void k_copy(const T* __restrict__ src, T* __restrict__ dst, size_t count) {
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) dst[i] = src[i];
+}
+// one warp per batch element: draw the record index, gather the record.
+__global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
+                                                       uint32_t filled, const uint16_t* __restrict__ r_obs,
+                                                       const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
+                                                       const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
+                                                       uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
+                                                       int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int j = blockIdx.x * 4 + warp;
+  if (j >= batch) return;
+  uint32_t o[4];
+  philox((uint32_t)(j >> 2), d0, d1, TAG_SAMPLE, k0, k1, o);
+  uint32_t u = (j & 3) == 0 ? o[0] : (j & 3) == 1 ? o[1] : (j & 3) == 2 ? o[2] : o[3];
+  size_t p = bounded(u, filled);
+  if (obs) {
+    const uint4* s = reinterpret_cast<const uint4*>(r_obs + p * STRAT_OBS_ELEMS);
+    uint4* d = reinterpret_cast<uint4*>(obs + (size_t)j * STRAT_OBS_ELEMS);
+    for (int q = lane; q < kObsChunks; q += 32) d[q] = __ldcs(s + q);
+  }
+  if (mask)
+    for (int q = lane; q < kMaskWords; q += 32) mask[(size_t)j * kMaskWords + q] = r_mask[p * kMaskWords + q];
+  if (lane == 0) {
+    if (act) act[j] = r_act[p];
+    if (rew) rew[j] = r_rew[p];
+    if (done) done[j] = r_done[p];
+  }
+}
+
+// ---- search-shaped batch
+__global__ void __launch_bounds__(32) k_determinise(int num_out, int samples_per_root, uint32_t k0, uint32_t k1, uint32_t out_base,
+                                                    const uint32_t* __restrict__ roots, uint32_t* __restrict__ out,
+                                                    int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, num_out - first);
+  if (lane < ng) {
+    int G = first + lane, r = G / samples_per_root;
+    uint32_t W[32];
+    const uint4* p = reinterpret_cast<const uint4*>(roots + (size_t)r * kLineWords);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { uint4 v = __ldg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+    Game root, g;
+    unpack_line(W, root);
+    if (!determinise_game(root, k0, k1, out_base + (uint32_t)G, g)) raise_error(err, STRAT_BAD_STATE);
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(out, first, ng, s_state, lane);
+}
+
+__global__ void __launch_bounds__(256) k_reduce_returns(const uint32_t* __restrict__ lines, const uint8_t* __restrict__ root_side,
+                                                        int samples_per_root, int32_t* __restrict__ out) {
+  __shared__ int s_sum[8], s_win[8], s_loss[8];
+  int r = blockIdx.x;
+  int sign = root_side[r] == 0 ? 1 : -1;
+  int sum = 0, win = 0, loss = 0;
+  for (int s = threadIdx.x; s < samples_per_root; s += blockDim.x) {
+    uint32_t f = lines[((size_t)r * samples_per_root + s) * kLineWords + 19] >> 4;
+    int ret = (f & 1u) ? ((int)((f >> 4) & 3u) - 1) * sign : 0;
+    sum += ret; win += ret > 0; loss += ret < 0;
+  }
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) {
+    sum += __shfl_down_sync(0xffffffffu, sum, off);
+    win += __shfl_down_sync(0xffffffffu, win, off);
+    loss += __shfl_down_sync(0xffffffffu, loss, off);
+  }
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) { s_sum[warp] = sum; s_win[warp] = win; s_loss[warp] = loss; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int a = 0, b = 0, c = 0;
+    for (int k = 0; k < 8; ++k) { a += s_sum[k]; b += s_win[k]; c += s_loss[k]; }
+    out[3 * r] = a; out[3 * r + 1] = b; out[3 * r + 2] = c;
+  }
+}
+
+__global__ void k_set_int(int* p, int v) { *p = v; }
+
+// ------------------------------------------------------------------ host side
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool cfg_ok(const strat_config* c) {
+  return c && c->num_games >= 1 && (c->variant == 0 || c->variant == 1) && c->max_plies >= 0 &&
+         c->max_battleless >= 0 && c->reserved == 0;
+}
+inline Params make_params(const strat_config& c) {
+  Params P;
+  P.key0 = (uint32_t)c.seed; P.key1 = (uint32_t)(c.seed >> 32);
+  P.game_base = (uint32_t)c.game_base;
+  P.num_games = c.num_games; P.variant = c.variant;
+  P.ply_cap = (c.max_plies >= 1 && c.max_plies <= 65535) ? c.max_plies : 65535;
+  P.max_battleless = c.max_battleless; P.auto_reset = c.auto_reset ? 1 : 0; P.two_square = c.two_square ? 1 : 0;
+  return P;
+}
+inline int launch_status() { return cudaGetLastError() == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR; }
+inline int batches(int n) { return (n + kBatch - 1) / kBatch; }
+
+template <typename T>
+void copy_elems(const T* src, T* dst, size_t count, cudaStream_t s) {
+  if (count == 0) return;
+  // widen to 16-byte vectors when both ends and the size allow it
+  size_t bytes = count * sizeof(T);
+  if ((((uintptr_t)src | (uintptr_t)dst | bytes) & 15) == 0) {
+    size_t n16 = bytes / 16;
+    int blocks = (int)((n16 + 255) / 256 < 148 * 16 ? (n16 + 255) / 256 : 148 * 16);
+    k_copy<uint4><<<blocks, 256, 0, s>>>(reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst), n16);
+  } else {
+    int blocks = (int)((count + 255) / 256 < 148 * 16 ? (count + 255) / 256 : 148 * 16);
+    k_copy<T><<<blocks, 256, 0, s>>>(src, dst, count);
+  }
+}
+// records [0,n) of the source go to ring positions (head+i) mod capacity: at most two runs.
+template <typename T>
+void push_array(const T* src, T* ring, size_t per_rec, int64_t head, int64_t cap, int64_t n, cudaStream_t s) {
+  int64_t first = n < cap - head ? n : cap - head;
+  copy_elems<T>(src, ring + (size_t)head * per_rec, (size_t)first * per_rec, s);
+  copy_elems<T>(src + (size_t)first * per_rec, ring, (size_t)(n - first) * per_rec, s);
+}
+
+}  // namespace
+
+struct strat_env {
+  strat_config cfg;
+  strat::Params P;
+  uint32_t* lines;
+  int* err;
+};
+
+struct strat_replay {
+  int64_t per_slot, slots, capacity, head, filled;
+  uint16_t* obs; uint32_t* mask; int16_t* action; int8_t* reward; uint8_t* done;
+};
+
+extern "C" {
+
+const char* strat_error_string(int code) {
+  switch (code) {
+    case STRAT_OK: return "ok";
+    case STRAT_BAD_ARG: return "bad argument";
+    case STRAT_BAD_STATE: return "bad state";
+    case STRAT_CUDA_ERROR: return "CUDA error";
+    case STRAT_ILLEGAL_ACTION: return "illegal action for a live game";
+    default: return "unknown error";
+  }
+}
+
+size_t strat_workspace_bytes(const strat_config* cfg) {
+  if (!cfg_ok(cfg)) return 0;
+  return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256;
+}
+
+int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream, strat_env** out) {
+  if (!cfg_ok(cfg) || !workspace_dev || !out || bytes < strat_workspace_bytes(cfg) ||
+      ((uintptr_t)workspace_dev & 255) != 0)
+    return STRAT_BAD_ARG;
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return STRAT_CUDA_ERROR;
+  strat_env* e = new (std::nothrow) strat_env;
+  if (!e) return STRAT_BAD_ARG;
+  e->cfg = *cfg;
+  e->P = make_params(*cfg);
+  e->lines = reinterpret_cast<uint32_t*>(workspace_dev);
+  e->err = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(workspace_dev) +
+                                  align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256));
+  *out = e;
+  return strat_reset(e, cfg->seed, stream);
+}
+
+int strat_destroy(strat_env* env) { delete env; return STRAT_OK; }
+
+int strat_reset(strat_env* env, uint64_t seed, void* stream) {
+  if (!env) return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  env->cfg.seed = seed;
+  env->P = make_params(env->cfg);
+  k_set_int<<<1, 1, 0, s>>>(env->err, 0);
+  k_reset<<<batches(env->P.num_games), 32, 0, s>>>(env->P, env->lines);
+  return launch_status();
+}
+
+int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
+  if (!env || !boards) return STRAT_BAD_ARG;
+  int n = env->P.num_games;
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  return launch_status();
+}
+
+int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream) {
+  if (!env || !boards) return STRAT_BAD_ARG;
+  int n = env->P.num_games;
+  k_export<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, env->lines, boards);
+  return launch_status();
+}
+
+int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream) {
+  if (!env || !mask) return STRAT_BAD_ARG;
+  k_legal_mask<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
+  return launch_status();
+}
+
+int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* actions, void* stream) {
+  if (!env || !mask || !actions) return STRAT_BAD_ARG;
+  int n = env->P.num_games;
+  k_sample_uniform<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions);
+  return launch_status();
+}
+
+int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream) {
+  if (!env || !actions || !reward || !done) return STRAT_BAD_ARG;
+  k_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err);
+  return launch_status();
+}
+
+int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
+  if (!env || !obs) return STRAT_BAD_ARG;
+  k_encode_obs<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, obs);
+  return launch_status();
+}
+
+int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done,
+                       uint16_t* obs, void* stream) {
+  if (!env || !obs) return STRAT_BAD_ARG;
+  k_rollout_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward,
+                                                                            done, obs, env->err);
+  return launch_status();
+}
+
+size_t strat_host_scratch_bytes(const strat_config* cfg) {
+  if (!cfg_ok(cfg)) return 0;
+  size_t n = (size_t)cfg->num_games;
+  return align_up(n * STRAT_OBS_ELEMS * 2, 256) + align_up(n * STRAT_MASK_WORDS * 4, 256) + align_up(n * 2, 256) +
+         align_up(n, 256) + align_up(n, 256);
+}
+
+int strat_rollout_step_host(strat_env* env, void* scratch_dev, uint32_t* mask_host, int16_t* actions_host,
+                            int8_t* reward_host, uint8_t* done_host, uint16_t* obs_host, void* stream) {
+  if (!env || !scratch_dev || !mask_host || !actions_host || !reward_host || !done_host || !obs_host)
+    return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  size_t n = (size_t)env->P.num_games;
+  uint8_t* p = reinterpret_cast<uint8_t*>(scratch_dev);
+  uint16_t* obs = reinterpret_cast<uint16_t*>(p); p += align_up(n * STRAT_OBS_ELEMS * 2, 256);
+  uint32_t* mask = reinterpret_cast<uint32_t*>(p); p += align_up(n * STRAT_MASK_WORDS * 4, 256);
+  int16_t* act = reinterpret_cast<int16_t*>(p); p += align_up(n * 2, 256);
+  int8_t* rew = reinterpret_cast<int8_t*>(p); p += align_up(n, 256);
+  uint8_t* done = p;
+  int rc = strat_rollout_step(env, mask, act, rew, done, obs, stream);
+  if (rc != STRAT_OK) return rc;
+  bool ok = cudaMemcpyAsync(obs_host, obs, n * STRAT_OBS_ELEMS * 2, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(mask_host, mask, n * STRAT_MASK_WORDS * 4, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(actions_host, act, n * 2, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(reward_host, rew, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(done_host, done, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaStreamSynchronize(s) == cudaSuccess;
+  return ok ? STRAT_OK : STRAT_CUDA_ERROR;
+}
+
+int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_host, int8_t* reward_host,
+                    uint8_t* done_host, uint32_t* mask_host, uint16_t* obs_host, void* stream) {
+  if (!env || !scratch_dev || !actions_host || !reward_host || !done_host || !mask_host || !obs_host)
+    return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  size_t n = (size_t)env->P.num_games;
+  uint8_t* p = reinterpret_cast<uint8_t*>(scratch_dev);
+  uint16_t* obs = reinterpret_cast<uint16_t*>(p); p += align_up(n * STRAT_OBS_ELEMS * 2, 256);
+  uint32_t* mask = reinterpret_cast<uint32_t*>(p); p += align_up(n * STRAT_MASK_WORDS * 4, 256);
+  int16_t* act = reinterpret_cast<int16_t*>(p); p += align_up(n * 2, 256);
+  int8_t* rew = reinterpret_cast<int8_t*>(p); p += align_up(n, 256);
+  uint8_t* done = p;
+  if (cudaMemcpyAsync(act, actions_host, n * 2, cudaMemcpyHostToDevice, s) != cudaSuccess) return STRAT_CUDA_ERROR;
+  int rc = strat_step(env, act, rew, done, stream);
+  if (rc == STRAT_OK) rc = strat_legal_mask(env, mask, stream);
+  if (rc == STRAT_OK) rc = strat_encode_obs(env, obs, stream);
+  if (rc != STRAT_OK) return rc;
+  bool ok = cudaMemcpyAsync(reward_host, rew, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(done_host, done, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(mask_host, mask, n * STRAT_MASK_WORDS * 4, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(obs_host, obs, n * STRAT_OBS_ELEMS * 2, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+  ok = ok && cudaStreamSynchronize(s) == cudaSuccess;
+  return ok ? STRAT_OK : STRAT_CUDA_ERROR;
+}
+
+int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream) {
+  if (!env || plies < 0) return STRAT_BAD_ARG;
+  k_rollout_uniform<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
+  return launch_status();
+}
+
+int strat_check(strat_env* env) {
+  if (!env) return STRAT_BAD_ARG;
+  if (cudaDeviceSynchronize() != cudaSuccess) return STRAT_CUDA_ERROR;
+  int v = 0;
+  if (cudaMemcpy(&v, env->err, sizeof v, cudaMemcpyDeviceToHost) != cudaSuccess) return STRAT_CUDA_ERROR;
+  return v;
+}
+
+int strat_clear_error(strat_env* env, void* stream) {
+  if (!env) return STRAT_BAD_ARG;
+  k_set_int<<<1, 1, 0, (cudaStream_t)stream>>>(env->err, 0);
+  return launch_status();
+}
+
+// ---- replay ring
+int strat_replay_layout(int32_t per_slot, int32_t slots, size_t off[5]) {
+  if (per_slot <= 0 || slots <= 0 || !off) return STRAT_BAD_ARG;
+  size_t C = (size_t)per_slot * (size_t)slots, p = 0;
+  off[0] = p; p += align_up(C * STRAT_OBS_ELEMS * 2, 256);
+  off[1] = p; p += align_up(C * STRAT_MASK_WORDS * 4, 256);
+  off[2] = p; p += align_up(C * 2, 256);
+  off[3] = p; p += align_up(C, 256);
+  off[4] = p;
+  return STRAT_OK;
+}
+
+size_t strat_replay_bytes(int32_t per_slot, int32_t slots) {
+  size_t off[5];
+  if (strat_replay_layout(per_slot, slots, off) != STRAT_OK) return 0;
+  return off[4] + align_up((size_t)per_slot * (size_t)slots, 256);
+}
+
+int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out) {
+  size_t need = strat_replay_bytes(per_slot, slots);
+  if (!mem_dev || !out || need == 0 || bytes < need || ((uintptr_t)mem_dev & 255) != 0) return STRAT_BAD_ARG;
+  strat_replay* r = new (std::nothrow) strat_replay;
+  if (!r) return STRAT_BAD_ARG;
+  size_t off[5];
+  strat_replay_layout(per_slot, slots, off);
+  uint8_t* b = reinterpret_cast<uint8_t*>(mem_dev);
+  r->per_slot = per_slot; r->slots = slots; r->capacity = (int64_t)per_slot * slots; r->head = 0; r->filled = 0;
+  r->obs = reinterpret_cast<uint16_t*>(b + off[0]); r->mask = reinterpret_cast<uint32_t*>(b + off[1]);
+  r->action = reinterpret_cast<int16_t*>(b + off[2]); r->reward = reinterpret_cast<int8_t*>(b + off[3]);
+  r->done = b + off[4];
+  *out = r;
+  return STRAT_OK;
+}
+
+int strat_replay_destroy(strat_replay* r) { delete r; return STRAT_OK; }
+
+int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
+                      const int8_t* reward, const uint8_t* done, int32_t n, void* stream) {
+  if (!r || !obs || !mask || !action || !reward || !done || n < 0 || n > r->capacity) return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  push_array<uint16_t>(obs, r->obs, STRAT_OBS_ELEMS, r->head, r->capacity, n, s);
+  push_array<uint32_t>(mask, r->mask, STRAT_MASK_WORDS, r->head, r->capacity, n, s);
+  push_array<int16_t>(action, r->action, 1, r->head, r->capacity, n, s);
+  push_array<int8_t>(reward, r->reward, 1, r->head, r->capacity, n, s);
+  push_array<uint8_t>(done, r->done, 1, r->head, r->capacity, n, s);
+  r->head = (r->head + n) % r->capacity;
+  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+  return launch_status();
+}
+
+int strat_replay_reserve(strat_replay* r, int32_t n, uint16_t** obs, uint32_t** mask) {
+  if (!r || !obs || !mask || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0) return STRAT_BAD_ARG;
+  *obs = r->obs + (size_t)r->head * STRAT_OBS_ELEMS;
+  *mask = r->mask + (size_t)r->head * STRAT_MASK_WORDS;
+  return STRAT_OK;
+}
+
+int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done, int32_t n,
+                        void* stream) {
+  if (!r || !action || !reward || !done || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0)
+    return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  copy_elems<int16_t>(action, r->action + r->head, (size_t)n, s);
+  copy_elems<int8_t>(reward, r->reward + r->head, (size_t)n, s);
+  copy_elems<uint8_t>(done, r->done + r->head, (size_t)n, s);
+  r->head = (r->head + n) % r->capacity;
+  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+  return launch_status();
+}
+
+int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_index, int32_t batch, uint16_t* obs,
+                        uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done, void* stream) {
+  if (!r || batch < 0) return STRAT_BAD_ARG;
+  if (r->filled == 0) return STRAT_BAD_STATE;
+  if (batch == 0) return STRAT_OK;
+  k_replay_sample<<<(batch + 3) / 4, 128, 0, (cudaStream_t)stream>>>(
+      (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), batch,
+      (uint32_t)r->filled, r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done);
+  return launch_status();
+}
+
+int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled) {
+  if (!r) return STRAT_BAD_ARG;
+  if (head) *head = r->head;
+  if (filled) *filled = r->filled;
+  return STRAT_OK;
+}
+
+// ---- search-shaped batch
+int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t seed, strat_env* out, void* stream) {
+  if (!roots || !out || samples_per_root <= 0 ||
+      (int64_t)roots->P.num_games * samples_per_root != (int64_t)out->P.num_games)
+    return STRAT_BAD_ARG;
+  k_determinise<<<batches(out->P.num_games), 32, 0, (cudaStream_t)stream>>>(
+      out->P.num_games, samples_per_root, (uint32_t)seed, (uint32_t)(seed >> 32), out->P.game_base, roots->lines,
+      out->lines, out->err);
+  return launch_status();
+}
+
+int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32_t samples_per_root, int32_t* out,
+                         void* stream) {
+  if (!games || !root_side || !out || samples_per_root <= 0 || games->P.num_games % samples_per_root != 0)
+    return STRAT_BAD_ARG;
+  int R = games->P.num_games / samples_per_root;
+  k_reduce_returns<<<R, 256, 0, (cudaStream_t)stream>>>(games->lines, root_side, samples_per_root, out);
+  return launch_status();
+}
+
+}  // extern "C"

@@ -1,0 +1,668 @@
+// strat_game.cuh — per-game Stratego logic on 100-bit bitboards, one thread per game.
+//
+// The device keeps each game as ONE 128-byte line in a bit-sliced form: seven 100-bit
+// planes (type bits T0..T3, owner, moved, revealed) in four 32-bit words each, with the
+// 8-ply history, flags and counters packed into the spare bits (layout below).  Every
+// rule then becomes a handful of 32-bit logic ops on whole boards instead of loops over
+// cells: legal single-step moves are four shifted ANDs, the 28 board planes of the
+// observation are LOP3 combinations of the seven state planes.
+//
+// Rules follow PAPER.md:208-212 (movement, battle, win/draw, two-square rule) with the
+// readings R#1..R#23 listed in DESIGN.md.
+#pragma once
+#include <stdint.h>
+
+#ifdef STRAT_HOST_DEBUG  // developer-only: lets the scalar logic be stepped on a CPU.
+#define SD static inline
+static inline int sd_popc(uint32_t x) { return __builtin_popcount(x); }
+static inline int sd_ffs(uint32_t x) { return __builtin_ffs((int)x); }
+static inline uint32_t sd_mulhi(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) >> 32); }
+static inline uint32_t sd_fsr(uint32_t lo, uint32_t hi, int s) { return (uint32_t)((((uint64_t)hi << 32) | lo) >> s); }
+static inline uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return (uint32_t)(((((uint64_t)hi << 32) | lo) << s) >> 32); }
+static inline int min(int a, int b) { return a < b ? a : b; }
+static inline int max(int a, int b) { return a > b ? a : b; }
+#define STRAT_UNROLL
+#else
+#define STRAT_UNROLL _Pragma("unroll")
+#define SD __device__ __forceinline__
+SD int sd_popc(uint32_t x) { return __popc(x); }
+SD int sd_ffs(uint32_t x) { return __ffs((int)x); }
+SD uint32_t sd_mulhi(uint32_t a, uint32_t b) { return __umulhi(a, b); }
+SD uint32_t sd_fsr(uint32_t lo, uint32_t hi, int s) { return __funnelshift_r(lo, hi, s); }
+SD uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return __funnelshift_l(lo, hi, s); }
+#endif
+
+namespace strat {
+
+constexpr int kLineWords = 32;
+constexpr int kMaskWords = 113;
+constexpr int kObsStreamWords = 138;  // 4400 bits
+constexpr int T_SPY = 1, T_SCOUT = 2, T_MINER = 3, T_MARSHAL = 10, T_FLAG = 11, T_BOMB = 12;
+constexpr int REASON_FLAG = 1, REASON_NOMOVE_WIN = 2, REASON_NOMOVE_DRAW = 3, REASON_PLY_CAP = 4,
+              REASON_BATTLELESS = 5;
+constexpr uint32_t TAG_SETUP_RED = 0, TAG_SETUP_BLUE = 1, TAG_ACTION = 2, TAG_SAMPLE = 3, TAG_DETERMINISE = 4;
+constexpr uint32_t kHistNone = 0x3FFF;
+
+struct Params {  // per-environment constants handed to every kernel by value
+  uint32_t key0, key1;     // Philox key = seed
+  uint32_t game_base;      // global index of local game 0
+  int32_t num_games;
+  int32_t variant;
+  int32_t ply_cap;         // effective: 1..65535
+  int32_t max_battleless;  // 0 = off
+  int32_t auto_reset;
+  int32_t two_square;
+};
+
+// ------------------------------------------------------------------ 100-bit boards
+struct BB { uint32_t w[4]; };  // cell c -> word c>>5, bit c&31; w[3] uses bits 0..3
+
+constexpr uint32_t col_word(int col, int i) {
+  uint32_t m = 0;
+  for (int r = 0; r < 10; ++r) {
+    int c = 10 * r + col;
+    if ((c >> 5) == i) m |= 1u << (c & 31);
+  }
+  return m;
+}
+constexpr uint32_t lake_word(int i) {
+  uint32_t m = 0;
+  const int L[8] = {42, 43, 46, 47, 52, 53, 56, 57};
+  for (int k = 0; k < 8; ++k)
+    if ((L[k] >> 5) == i) m |= 1u << (L[k] & 31);
+  return m;
+}
+// Board constants as literals (device code cannot index host constexpr arrays); the
+// static_asserts tie them to the geometry.
+#define STRAT_LAKE_W1 0x0330CC00u   /* cells 42,43,46,47,52,53,56,57 all lie in word 1 */
+static_assert(lake_word(0) == 0 && lake_word(1) == STRAT_LAKE_W1 && lake_word(2) == 0 && lake_word(3) == 0, "lakes");
+static_assert(col_word(0, 0) == 0x40100401u && col_word(0, 1) == 0x10040100u && col_word(0, 2) == 0x04010040u &&
+              col_word(0, 3) == 0u, "col 0");
+static_assert(col_word(9, 0) == 0x20080200u && col_word(9, 1) == 0x08020080u && col_word(9, 2) == 0x02008020u &&
+              col_word(9, 3) == 0x8u, "col 9");
+enum BoardConst { kLake, kNotLake, kNotCol0, kNotCol9 };
+SD bool is_lake_cell(int c) { return (c >> 5) == 1 && ((STRAT_LAKE_W1 >> (c & 31)) & 1u); }
+
+SD BB bb_zero() { BB r; r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0; return r; }
+SD BB bb_and(BB a, BB b) { BB r;
+STRAT_UNROLL
+for (int i = 0; i < 4; ++i) r.w[i] = a.w[i] & b.w[i]; return r; }
+SD BB bb_or(BB a, BB b) { BB r;
+STRAT_UNROLL
+for (int i = 0; i < 4; ++i) r.w[i] = a.w[i] | b.w[i]; return r; }
+SD BB bb_andn(BB a, BB b) { BB r;
+STRAT_UNROLL
+for (int i = 0; i < 4; ++i) r.w[i] = a.w[i] & ~b.w[i]; return r; }  // a & ~b
+SD BB bb_const(BoardConst k) {
+  BB r;
+  if (k == kLake)         { r.w[0] = 0u;           r.w[1] = STRAT_LAKE_W1;  r.w[2] = 0u;           r.w[3] = 0u; }
+  else if (k == kNotLake) { r.w[0] = 0xFFFFFFFFu;  r.w[1] = ~STRAT_LAKE_W1; r.w[2] = 0xFFFFFFFFu;  r.w[3] = 0xFu; }
+  else if (k == kNotCol0) { r.w[0] = ~0x40100401u; r.w[1] = ~0x10040100u;   r.w[2] = ~0x04010040u; r.w[3] = 0xFu; }
+  else                    { r.w[0] = ~0x20080200u; r.w[1] = ~0x08020080u;   r.w[2] = ~0x02008020u; r.w[3] = 0x7u; }
+  return r;
+}
+SD bool bb_any(BB a) { return (a.w[0] | a.w[1] | a.w[2] | a.w[3]) != 0; }
+SD int bb_popc(BB a) { return sd_popc(a.w[0]) + sd_popc(a.w[1]) + sd_popc(a.w[2]) + sd_popc(a.w[3]); }
+// r[c] = a[c+S]
+template <int S> SD BB bb_down(BB a) {
+  BB r;
+  r.w[0] = sd_fsr(a.w[0], a.w[1], S); r.w[1] = sd_fsr(a.w[1], a.w[2], S);
+  r.w[2] = sd_fsr(a.w[2], a.w[3], S); r.w[3] = a.w[3] >> S;
+  return r;
+}
+// r[c] = a[c-S]
+template <int S> SD BB bb_up(BB a) {
+  BB r;
+  r.w[3] = sd_fsl(a.w[2], a.w[3], S) & 0xFu; r.w[2] = sd_fsl(a.w[1], a.w[2], S);
+  r.w[1] = sd_fsl(a.w[0], a.w[1], S); r.w[0] = a.w[0] << S;
+  return r;
+}
+SD uint32_t bb_word(const BB& a, int i) {
+  uint32_t x = a.w[0];
+  x = i == 1 ? a.w[1] : x; x = i == 2 ? a.w[2] : x; x = i == 3 ? a.w[3] : x;
+  return x;
+}
+SD uint32_t bb_test(const BB& a, int c) { return (bb_word(a, c >> 5) >> (c & 31)) & 1u; }
+// single-cell selector: m[i] = bit of cell c in word i
+struct CellSel { uint32_t m[4]; };
+SD CellSel cell_sel(int c) {
+  CellSel s; uint32_t bit = 1u << (c & 31); int wi = c >> 5;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) s.m[i] = wi == i ? bit : 0u;
+  return s;
+}
+SD void bb_put(BB& a, const CellSel& s, uint32_t v) {  // set cell to v (0/1)
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) a.w[i] = (a.w[i] & ~s.m[i]) | (v ? s.m[i] : 0u);
+}
+SD uint32_t bb_get(const BB& a, const CellSel& s) {
+  return ((a.w[0] & s.m[0]) | (a.w[1] & s.m[1]) | (a.w[2] & s.m[2]) | (a.w[3] & s.m[3])) != 0;
+}
+
+// ------------------------------------------------------------------ Philox4x32-10
+SD void philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t out[4]) {
+STRAT_UNROLL
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = sd_mulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = sd_mulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+SD uint32_t bounded(uint32_t u, uint32_t n) { return sd_mulhi(u, n); }
+
+// ------------------------------------------------------------------ game state
+// Device line, 32 words:  word 4p+i = plane p (0 T0, 1 T1, 2 T2, 3 T3, 4 owner, 5 moved,
+// 6 revealed), cells 32i..32i+31.  Word 4p+3 holds cells 96..99 in bits 0..3 and 28 spare
+// bits: planes 0..3 carry history entries 2p (bits 4..17) and 2p+1 (bits 18..31), an entry
+// being from | to<<7 (0x3FFF = none); plane 4 carries flags (bit 4 done, bits 5..7 reason,
+// bits 8..9 result+1).  Word 28 = ply | battleless<<16, word 29 = epoch, 30..31 zero.
+struct Game {
+  BB t0, t1, t2, t3, own, mvd, rev;
+  uint32_t h[4];
+  uint32_t done, reason;
+  int32_t result;
+  uint32_t ply, battleless, epoch;
+};
+
+SD void unpack_line(const uint32_t* W, Game& g) {
+  BB* pl[7] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own, &g.mvd, &g.rev};
+  STRAT_UNROLL
+  for (int p = 0; p < 7; ++p) {
+    STRAT_UNROLL
+    for (int i = 0; i < 3; ++i) pl[p]->w[i] = W[4 * p + i];
+    pl[p]->w[3] = W[4 * p + 3] & 0xFu;
+  }
+  STRAT_UNROLL
+  for (int p = 0; p < 4; ++p) g.h[p] = W[4 * p + 3] >> 4;
+  uint32_t f = W[19] >> 4;
+  g.done = f & 1u; g.reason = (f >> 1) & 7u; g.result = (int32_t)((f >> 4) & 3u) - 1;
+  g.ply = W[28] & 0xFFFFu; g.battleless = W[28] >> 16; g.epoch = W[29];
+}
+SD void pack_line(const Game& g, uint32_t* W) {
+  const BB* pl[7] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own, &g.mvd, &g.rev};
+  STRAT_UNROLL
+  for (int p = 0; p < 7; ++p)
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) W[4 * p + i] = pl[p]->w[i];
+  STRAT_UNROLL
+  for (int p = 0; p < 4; ++p) W[4 * p + 3] |= g.h[p] << 4;
+  W[19] |= (g.done | (g.reason << 1) | ((uint32_t)(g.result + 1) << 4)) << 4;
+  W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = 0; W[31] = 0;
+}
+SD uint32_t hist_entry(const Game& g, int j) { return (g.h[j >> 1] >> (14 * (j & 1))) & 0x3FFFu; }
+SD void hist_push(Game& g, uint32_t e) {
+  uint32_t carry = e;
+  STRAT_UNROLL
+  for (int p = 0; p < 4; ++p) {
+    uint32_t out = g.h[p] >> 14;
+    g.h[p] = ((g.h[p] << 14) | carry) & 0x0FFFFFFFu;
+    carry = out;
+  }
+}
+SD void hist_clear(Game& g) {
+STRAT_UNROLL
+for (int p = 0; p < 4; ++p) g.h[p] = 0x0FFFFFFFu; }
+
+SD BB occupied(const Game& g) { return bb_or(bb_or(g.t0, g.t1), bb_or(g.t2, g.t3)); }
+SD BB owned_by(const Game& g, BB occ, int side) {
+  BB r;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) r.w[i] = occ.w[i] & (side ? g.own.w[i] : ~g.own.w[i]); return r;
+}
+
+// ------------------------------------------------------------------ two-square rule
+// P:212 / R#6.  The side's last three moves are history entries first, first+2, first+4
+// (first = 1 when it is that side's turn, else 0).  If they are consecutive moves of one
+// piece along one line whose crossed boundaries intersect, moves of that piece (now at
+// `from`) in direction `dir` of distance >= k are banned.
+struct Ban { int from, dir, k; };
+SD Ban two_square_ban(const Game& g, int side, int enabled) {
+  Ban b; b.from = -1; b.dir = 0; b.k = 99;
+  if (!enabled) return b;
+  int first = ((int)(g.ply & 1u) == side) ? 1 : 0;
+  uint32_t e3 = hist_entry(g, first), e2 = hist_entry(g, first + 2), e1 = hist_entry(g, first + 4);
+  if (e3 == kHistNone || e2 == kHistNone || e1 == kHistNone) return b;
+  int p0 = e1 & 127, p1 = e1 >> 7, f2 = e2 & 127, p2 = e2 >> 7, f3 = e3 & 127, p3 = e3 >> 7;
+  if (p1 != f2 || p2 != f3) return b;
+  int r0 = p0 / 10, r1 = p1 / 10, r2 = p2 / 10, r3 = p3 / 10;
+  int c0 = p0 - 10 * r0, c1 = p1 - 10 * r1, c2 = p2 - 10 * r2, c3 = p3 - 10 * r3;
+  bool same_row = r0 == r1 && r1 == r2 && r2 == r3;
+  bool same_col = c0 == c1 && c1 == c2 && c2 == c3;
+  if (!same_row && !same_col) return b;
+  int x0 = same_row ? c0 : r0, x1 = same_row ? c1 : r1, x2 = same_row ? c2 : r2, x3 = same_row ? c3 : r3;
+  int lo = max(max(min(x0, x1), min(x1, x2)), min(x2, x3));
+  int hi = min(min(max(x0, x1), max(x1, x2)), max(x2, x3));
+  if (lo >= hi) return b;
+  b.from = p3;
+  if (x3 > x2) { b.dir = same_row ? 3 : 2; b.k = x3 - hi + 1; }
+  else         { b.dir = same_row ? 1 : 0; b.k = lo - x3 + 1; }
+  return b;
+}
+
+// ------------------------------------------------------------------ move generation
+struct Moves {
+  BB d[4];      // d[dir][c] = piece of `side` at c may move one square in dir (after bans)
+  BB scouts;    // own Scouts
+  BB empty;     // empty non-lake squares
+  BB ok;        // squares a piece of `side` may land on (empty or enemy, not lake)
+  Ban ban;
+};
+SD void single_step_moves(const Game& g, int side, int two_square, Moves& m) {
+  BB occ = occupied(g);
+  BB mine = owned_by(g, occ, side);
+  BB notlake = bb_const(kNotLake);
+  m.ok = bb_andn(notlake, mine);
+  m.empty = bb_andn(notlake, occ);
+  // immovable types: Flag 1011, Bomb 1100  ->  T3 & (T2 | (T1 & T0))
+  BB imm = bb_and(g.t3, bb_or(g.t2, bb_and(g.t1, g.t0)));
+  BB movable = bb_andn(mine, imm);
+  m.scouts = bb_andn(bb_andn(bb_andn(bb_and(mine, g.t1), g.t0), g.t2), g.t3);
+  m.d[0] = bb_and(movable, bb_down<10>(m.ok));
+  m.d[2] = bb_and(movable, bb_up<10>(m.ok));
+  m.d[1] = bb_and(bb_and(movable, bb_down<1>(m.ok)), bb_const(kNotCol9));
+  m.d[3] = bb_and(bb_and(movable, bb_up<1>(m.ok)), bb_const(kNotCol0));
+  m.ban = two_square_ban(g, side, two_square);
+  if (m.ban.from >= 0 && m.ban.k <= 1) {
+    CellSel s = cell_sel(m.ban.from);
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d)
+      if (d == m.ban.dir)
+      STRAT_UNROLL
+      for (int i = 0; i < 4; ++i) m.d[d].w[i] &= ~s.m[i];
+  }
+}
+// GetHasLegalMovement: a banned distance bans every longer one (R#6), so a side
+// has a legal move iff it has a legal single-step move.
+SD bool has_legal_move(const Game& g, int side, int two_square) {
+  Moves m; single_step_moves(g, side, two_square, m);
+  return bb_any(bb_or(bb_or(m.d[0], m.d[1]), bb_or(m.d[2], m.d[3])));
+}
+
+// Longest legal distance of the piece at c in direction d, given its single step is legal.
+SD int ray_length(const Moves& m, int c, int d, int row, int col, bool scout) {
+  int len = 1;
+  if (scout) {
+    int maxk = d == 0 ? 9 - row : d == 1 ? 9 - col : d == 2 ? row : col;
+    int delta = d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1;
+    int p = c + delta;
+    while (len < maxk && bb_test(m.empty, p) && bb_test(m.ok, p + delta)) { ++len; p += delta; }
+  }
+  if (m.ban.from == c && m.ban.dir == d) len = min(len, m.ban.k - 1);
+  return len;
+}
+
+// Legal mask of `side` into `row` (113 words, already zero).  Returns the number of legal
+// actions.  Pieces are visited in ascending cell order, so bits are produced in ascending
+// action order: a = from*36 + dir*9 + dist-1.
+SD int legal_mask_row(const Game& g, int side, int two_square, uint32_t* row) {
+  Moves m; single_step_moves(g, side, two_square, m);
+  int n = 0;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    uint32_t any = m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i];
+    while (any) {
+      int b = sd_ffs(any) - 1;
+      any &= any - 1;
+      int c = 32 * i + b;
+      bool scout = (m.scouts.w[i] >> b) & 1u;
+      int r = c / 10, q = c - 10 * r;
+      uint64_t field = 0;
+      STRAT_UNROLL
+      for (int d = 0; d < 4; ++d) {
+        if ((m.d[d].w[i] >> b) & 1u) {
+          int len = ray_length(m, c, d, r, q, scout);
+          n += len;
+          field |= (uint64_t)((1u << len) - 1u) << (9 * d);
+        }
+      }
+      int pos = 36 * c, wi = pos >> 5, sh = pos & 31;
+      field <<= sh;  // 36 + 28 <= 64
+      row[wi] |= (uint32_t)field;
+      uint32_t hi = (uint32_t)(field >> 32);
+      if (hi) row[wi + 1] |= hi;
+    }
+  }
+  return n;
+}
+
+// r-th (from 0) set bit of a word
+SD int nth_set_bit(uint32_t w, int r) {
+  int pos = 0;
+STRAT_UNROLL
+  for (int s = 16; s >= 1; s >>= 1) {
+    int c = sd_popc(w & (((1u << s) - 1u) << pos));
+    if (r >= c) { r -= c; pos += s; }
+  }
+  return pos;
+}
+// SampleRandomLegalAction, C3a: r-th set bit of the row, n = its popcount.
+SD int pick_action(const uint32_t* row, int n, uint32_t u) {
+  if (n == 0) return -1;
+  int r = (int)bounded(u, (uint32_t)n);
+  for (int w = 0; w < kMaskWords; ++w) {
+    int c = sd_popc(row[w]);
+    if (r < c) return 32 * w + nth_set_bit(row[w], r);
+    r -= c;
+  }
+  return -1;
+}
+SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
+  uint32_t o[4];
+  philox(P.game_base + local_game, g.epoch, g.ply, TAG_ACTION, P.key0, P.key1, o);
+  return o[0];
+}
+
+// Is action a legal for the side to move?  (step validates what it is given)
+SD bool action_is_legal(const Game& g, int side, int two_square, int a) {
+  if (a < 0 || a >= 3600) return false;
+  int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
+  Moves m; single_step_moves(g, side, two_square, m);
+  if (!bb_test(m.d[d], from)) return false;
+  if (dist == 1) return true;
+  if (!bb_test(m.scouts, from)) return false;
+  int r = from / 10, q = from - 10 * r;
+  return dist <= ray_length(m, from, d, r, q, true);
+}
+
+// ------------------------------------------------------------------ setup (C2)
+SD void put_piece(Game& g, int c, int type, int owner) {
+  CellSel s = cell_sel(c);
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    g.t0.w[i] |= (type & 1) ? s.m[i] : 0u; g.t1.w[i] |= (type & 2) ? s.m[i] : 0u;
+    g.t2.w[i] |= (type & 4) ? s.m[i] : 0u; g.t3.w[i] |= (type & 8) ? s.m[i] : 0u;
+    g.own.w[i] |= owner ? s.m[i] : 0u;
+  }
+}
+SD uint32_t multiset_type(int variant, int i) {
+  if (variant == 0) {
+    // Flag, Bomb x6, Spy, Scout x8, Miner x5, Sergeant x4, Lieutenant x4, Captain x4,
+    // Major x3, Colonel x2, General, Marshal  (BASELINE.json configs[0] order)
+    return i < 1 ? 11 : i < 7 ? 12 : i < 8 ? 1 : i < 16 ? 2 : i < 21 ? 3 : i < 25 ? 4 : i < 29 ? 5
+         : i < 33 ? 6 : i < 36 ? 7 : i < 38 ? 8 : i < 39 ? 9 : 10;
+  }
+  // Barrage: Flag, Marshal, General, Miner, Scout, Scout, Spy, Bomb, 32 empties
+  return i == 0 ? 11 : i == 1 ? 10 : i == 2 ? 9 : i == 3 ? 3 : i == 4 ? 2 : i == 5 ? 2 : i == 6 ? 1
+       : i == 7 ? 12 : 0;
+}
+// Fresh game for (global game, g.epoch): both sides by descending Fisher-Yates over the
+// listed multiset, redrawn until the side can ever move (R#4, R#5).
+SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
+  g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
+  hist_clear(g);
+  g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0;
+  uint32_t gidx = P.game_base + local_game;
+  for (int side = 0; side < 2; ++side) {
+    for (uint32_t attempt = 0;; ++attempt) {
+      uint8_t A[40];
+      for (int i = 0; i < 40; ++i) A[i] = (uint8_t)multiset_type(P.variant, i);
+      uint32_t o[4] = {0, 0, 0, 0};
+      for (int i = 39; i >= 1; --i) {
+        int d = 39 - i;
+        if ((d & 3) == 0) philox(gidx, g.epoch, (attempt << 8) | (uint32_t)(d >> 2),
+                                 side ? TAG_SETUP_BLUE : TAG_SETUP_RED, P.key0, P.key1, o);
+        uint32_t u = (d & 3) == 0 ? o[0] : (d & 3) == 1 ? o[1] : (d & 3) == 2 ? o[2] : o[3];
+        int j = (int)bounded(u, (uint32_t)(i + 1));
+        uint8_t t = A[i]; A[i] = A[j]; A[j] = t;
+      }
+      Game trial = g;
+      int base = side ? 60 : 0;
+      for (int i = 0; i < 40; ++i)
+        if (A[i]) put_piece(trial, base + i, A[i], side);
+      // can this side ever move: a movable own piece next to a non-lake square without an own piece
+      BB occ = occupied(trial);
+      BB mine = owned_by(trial, occ, side);
+      BB ok = bb_andn(bb_const(kNotLake), mine);
+      BB imm = bb_and(trial.t3, bb_or(trial.t2, bb_and(trial.t1, trial.t0)));
+      BB mv = bb_andn(mine, imm);
+      BB can = bb_or(bb_or(bb_and(mv, bb_down<10>(ok)), bb_and(mv, bb_up<10>(ok))),
+                     bb_or(bb_and(bb_and(mv, bb_down<1>(ok)), bb_const(kNotCol9)),
+                           bb_and(bb_and(mv, bb_up<1>(ok)), bb_const(kNotCol0))));
+      if (bb_any(can)) { g = trial; break; }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ step (C4)
+// +1 attacker wins, -1 attacker loses, 0 both removed (Ext. Data Fig. 3b)
+SD int battle(int att, int def) {
+  if (def == T_FLAG) return 1;
+  if (def == T_BOMB) return att == T_MINER ? 1 : -1;
+  if (att == T_SPY && def == T_MARSHAL) return 1;
+  return att > def ? 1 : att < def ? -1 : 0;
+}
+
+struct StepOut { int reward; uint32_t done; bool illegal; };
+
+SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
+  StepOut o; o.illegal = false;
+  if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
+  int side = g.ply & 1u;
+  if (!action_is_legal(g, side, P.two_square, a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
+  int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
+  int to = from + dist * (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
+  CellSel sf = cell_sel(from), st = cell_sel(to);
+  int pt = bb_get(g.t0, sf) | (bb_get(g.t1, sf) << 1) | (bb_get(g.t2, sf) << 2) | (bb_get(g.t3, sf) << 3);
+  uint32_t prev = bb_get(g.rev, sf);
+  int tt = bb_get(g.t0, st) | (bb_get(g.t1, st) << 1) | (bb_get(g.t2, st) << 2) | (bb_get(g.t3, st) << 3);
+  hist_push(g, (uint32_t)from | ((uint32_t)to << 7));
+  // the origin square empties in every case
+  bb_put(g.t0, sf, 0); bb_put(g.t1, sf, 0); bb_put(g.t2, sf, 0); bb_put(g.t3, sf, 0);
+  bb_put(g.own, sf, 0); bb_put(g.mvd, sf, 0); bb_put(g.rev, sf, 0);
+  bool flag_captured = false;
+  int outcome = 1;  // plain move = the mover arrives
+  if (tt == 0) {
+    g.battleless += 1;
+    prev |= dist >= 2 ? 1u : 0u;  // R#10: a long move shows a Scout
+  } else {
+    g.battleless = 0;
+    prev = 1;                     // battle: both revealed
+    outcome = battle(pt, tt);
+    flag_captured = tt == T_FLAG;
+  }
+  if (outcome > 0) {              // mover occupies the target
+    bb_put(g.t0, st, pt & 1); bb_put(g.t1, st, (pt >> 1) & 1); bb_put(g.t2, st, (pt >> 2) & 1);
+    bb_put(g.t3, st, (pt >> 3) & 1);
+    bb_put(g.own, st, side); bb_put(g.mvd, st, 1); bb_put(g.rev, st, prev);
+  } else if (outcome < 0) {       // defender stays, now revealed (R#11: moved bit unchanged)
+    bb_put(g.rev, st, 1);
+  } else {                        // both removed
+    bb_put(g.t0, st, 0); bb_put(g.t1, st, 0); bb_put(g.t2, st, 0); bb_put(g.t3, st, 0);
+    bb_put(g.own, st, 0); bb_put(g.mvd, st, 0); bb_put(g.rev, st, 0);
+  }
+  g.ply += 1;
+  int mover_result = side == 0 ? 1 : -1;
+  // terminal tests in R#12 order
+  if (flag_captured) { g.done = 1; g.reason = REASON_FLAG; g.result = mover_result; }
+  else if (!has_legal_move(g, side ^ 1, P.two_square)) {
+    g.done = 1;
+    if (!has_legal_move(g, side, P.two_square)) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
+    else { g.reason = REASON_NOMOVE_WIN; g.result = mover_result; }
+  }
+  else if ((int)g.ply >= P.ply_cap) { g.done = 1; g.reason = REASON_PLY_CAP; g.result = 0; }
+  else if (P.max_battleless > 0 && (int)g.battleless >= P.max_battleless) {
+    g.done = 1; g.reason = REASON_BATTLELESS; g.result = 0;
+  }
+  o.reward = g.done ? g.result : 0;
+  o.done = g.done | ((uint32_t)side << 1) | ((g.done ? g.reason : 0u) << 2);
+  if (g.done && P.auto_reset) { g.epoch += 1; setup_game(P, local_game, g); }  // R#16
+  return o;
+}
+
+// ------------------------------------------------------------------ observation bits (C5)
+// The 44 planes as one 4400-bit stream (plane p at bit 100p) = 138 words.  Byte q of the
+// stream is exactly the 8 bf16 values of the q-th 16-byte chunk of the game's observation.
+SD BB type_is(const Game& g, BB base, int v) {
+  BB r;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i)
+    r.w[i] = base.w[i] & ((v & 1) ? g.t0.w[i] : ~g.t0.w[i]) & ((v & 2) ? g.t1.w[i] : ~g.t1.w[i]) &
+             ((v & 4) ? g.t2.w[i] : ~g.t2.w[i]) & ((v & 8) ? g.t3.w[i] : ~g.t3.w[i]);
+  return r;
+}
+SD BB hist_plane(uint32_t e, int which) {
+  if (e == kHistNone) return bb_zero();
+  CellSel s = cell_sel(which ? (int)(e >> 7) : (int)(e & 127));
+  BB r;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) r.w[i] = s.m[i]; return r;
+}
+// append `count` (<= 8) planes starting at stream bit 100*first_plane (a multiple of 800 bits
+// = 25 words, so every shift below is a compile-time constant once unrolled)
+template <int COUNT> SD void pack_planes(const BB (&pl)[8], uint32_t* out) {
+  constexpr int NW = (COUNT * 100 + 31) / 32;
+  uint32_t o[NW];
+STRAT_UNROLL
+  for (int k = 0; k < NW; ++k) o[k] = 0;
+STRAT_UNROLL
+  for (int p = 0; p < COUNT; ++p)
+STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      const int nb = i == 3 ? 4 : 32, pos = 100 * p + 32 * i, wi = pos >> 5, sh = pos & 31;
+      o[wi] |= pl[p].w[i] << sh;
+      if (sh != 0 && sh + nb > 32) o[wi + 1] |= pl[p].w[i] >> (32 - sh);
+    }
+STRAT_UNROLL
+  for (int k = 0; k < NW; ++k) out[k] = o[k];
+}
+SD void encode_bits(const Game& g, uint32_t* out /* 138 words */) {
+  int side = g.ply & 1u;
+  BB occ = occupied(g);
+  BB mine = owned_by(g, occ, side);
+  BB enemy = bb_andn(occ, mine);
+  BB seen = bb_and(enemy, g.rev);
+  BB pl[8];
+STRAT_UNROLL
+  for (int k = 0; k < 8; ++k) pl[k] = type_is(g, mine, k + 1);                  // planes 0-7
+  pack_planes<8>(pl, out);
+STRAT_UNROLL
+  for (int k = 0; k < 4; ++k) pl[k] = type_is(g, mine, k + 9);                  // 8-11
+STRAT_UNROLL
+  for (int k = 0; k < 4; ++k) pl[4 + k] = type_is(g, seen, k + 1);              // 12-15
+  pack_planes<8>(pl, out + 25);
+STRAT_UNROLL
+  for (int k = 0; k < 8; ++k) pl[k] = type_is(g, seen, k + 5);                  // 16-23
+  pack_planes<8>(pl, out + 50);
+  BB hidden = bb_andn(enemy, g.rev);
+  pl[0] = bb_and(hidden, g.mvd);                                                 // 24
+  pl[1] = bb_andn(hidden, g.mvd);                                                // 25
+  pl[2] = bb_const(kLake);                                                       // 26
+  pl[3] = bb_andn(bb_const(kNotLake), occ);                                      // 27
+  pl[4] = hist_plane(hist_entry(g, 0), 0); pl[5] = hist_plane(hist_entry(g, 0), 1);   // 28,29
+  pl[6] = hist_plane(hist_entry(g, 1), 0); pl[7] = hist_plane(hist_entry(g, 1), 1);   // 30,31
+  pack_planes<8>(pl, out + 75);
+STRAT_UNROLL
+  for (int j = 0; j < 4; ++j) {                                                  // 32-39
+    pl[2 * j] = hist_plane(hist_entry(g, 2 + j), 0); pl[2 * j + 1] = hist_plane(hist_entry(g, 2 + j), 1);
+  }
+  pack_planes<8>(pl, out + 100);
+STRAT_UNROLL
+  for (int j = 0; j < 2; ++j) {                                                  // 40-43
+    pl[2 * j] = hist_plane(hist_entry(g, 6 + j), 0); pl[2 * j + 1] = hist_plane(hist_entry(g, 6 + j), 1);
+  }
+  pack_planes<4>(pl, out + 125);
+}
+
+// ------------------------------------------------------------------ canonical <-> device line
+SD void import_canonical(const uint8_t* L, Game& g) {
+  g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
+  for (int c = 0; c < 100; ++c) {
+    uint32_t b = L[c], t = b & 15u;
+    if (t == 0 || t == 15) continue;
+    put_piece(g, c, (int)t, (b >> 4) & 1u);
+    CellSel s = cell_sel(c);
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      g.mvd.w[i] |= (b & 0x20u) ? s.m[i] : 0u; g.rev.w[i] |= (b & 0x40u) ? s.m[i] : 0u;
+    }
+  }
+  STRAT_UNROLL
+  for (int p = 0; p < 4; ++p) {
+    uint32_t e[2];
+    STRAT_UNROLL
+    for (int k = 0; k < 2; ++k) {
+      uint32_t f = L[100 + 2 * (2 * p + k)], t = L[101 + 2 * (2 * p + k)];
+      e[k] = (f == 0xFF) ? kHistNone : (f | (t << 7));
+    }
+    g.h[p] = e[0] | (e[1] << 14);
+  }
+  g.ply = L[116] | ((uint32_t)L[117] << 8);
+  g.battleless = L[118] | ((uint32_t)L[119] << 8);
+  g.done = L[120] & 1u; g.reason = (L[120] >> 2) & 7u; g.result = (int32_t)(int8_t)L[121];
+  g.epoch = L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
+}
+SD void export_canonical(const Game& g, uint8_t* L) {
+  for (int c = 0; c < 100; ++c) {
+    uint32_t t = bb_test(g.t0, c) | (bb_test(g.t1, c) << 1) | (bb_test(g.t2, c) << 2) | (bb_test(g.t3, c) << 3);
+    uint32_t b = t | (bb_test(g.own, c) << 4) | (bb_test(g.mvd, c) << 5) | (bb_test(g.rev, c) << 6);
+    if (is_lake_cell(c)) b = 15;
+    L[c] = (uint8_t)b;
+  }
+  STRAT_UNROLL
+  for (int j = 0; j < 8; ++j) {
+    uint32_t e = hist_entry(g, j);
+    L[100 + 2 * j] = e == kHistNone ? 0xFF : (uint8_t)(e & 127);
+    L[101 + 2 * j] = e == kHistNone ? 0xFF : (uint8_t)(e >> 7);
+  }
+  L[116] = (uint8_t)g.ply; L[117] = (uint8_t)(g.ply >> 8);
+  L[118] = (uint8_t)g.battleless; L[119] = (uint8_t)(g.battleless >> 8);
+  L[120] = (uint8_t)(g.done | (g.reason << 2)); L[121] = (uint8_t)(int8_t)g.result;
+  L[122] = 0; L[123] = 0;
+  L[124] = (uint8_t)g.epoch; L[125] = (uint8_t)(g.epoch >> 8); L[126] = (uint8_t)(g.epoch >> 16);
+  L[127] = (uint8_t)(g.epoch >> 24);
+}
+
+// ------------------------------------------------------------------ determinise (C7)
+// Re-type the hidden pieces of the searcher's opponent: uniform permutation of their types
+// over their squares (descending Fisher-Yates on DETERMINISE draws), rejecting any
+// permutation that puts a Bomb or Flag on a moved piece.  Position i is final once its swap is
+// done, so a violation there rejects the attempt at once; the accepted attempt and its result
+// are those of the plain draw-everything-then-test loop.  Returns the attempts used, or 0 if
+// the safety cap of 2^20 was hit (R#22: measured acceptance on ply-200 roots is 3e-4..7e-3).
+SD int determinise_game(const Game& root, uint32_t k0, uint32_t k1, uint32_t gidx, Game& out) {
+  out = root;
+  int searcher = root.ply & 1u;
+  BB occ = occupied(root);
+  BB enemy = bb_andn(occ, owned_by(root, occ, searcher));
+  BB hidden = bb_andn(enemy, root.rev);
+  uint8_t H[40], T[40], Pm[40];
+  int n = 0;
+  for (int i = 0; i < 4; ++i) {
+    uint32_t w = hidden.w[i];
+    while (w && n < 40) {
+      int b = sd_ffs(w) - 1; w &= w - 1;
+      int c = 32 * i + b;
+      H[n] = (uint8_t)(c | (bb_test(root.mvd, c) << 7));  // bit 7: this piece has moved
+      T[n] = (uint8_t)(bb_test(root.t0, c) | (bb_test(root.t1, c) << 1) | (bb_test(root.t2, c) << 2) |
+                       (bb_test(root.t3, c) << 3));
+      ++n;
+    }
+  }
+  int attempt = 0;
+  for (;; ++attempt) {
+    if (attempt >= (1 << 20)) return 0;
+    for (int i = 0; i < n; ++i) Pm[i] = T[i];
+    uint32_t o[4] = {0, 0, 0, 0};
+    bool ok = true;
+    for (int i = n - 1; i >= 1; --i) {
+      int d = n - 1 - i;
+      if ((d & 3) == 0) philox(gidx, (uint32_t)attempt, (uint32_t)(d >> 2), TAG_DETERMINISE, k0, k1, o);
+      uint32_t u = (d & 3) == 0 ? o[0] : (d & 3) == 1 ? o[1] : (d & 3) == 2 ? o[2] : o[3];
+      int j = (int)bounded(u, (uint32_t)(i + 1));
+      uint8_t t = Pm[j]; Pm[j] = Pm[i]; Pm[i] = t;
+      if ((t == T_BOMB || t == T_FLAG) && (H[i] & 0x80)) { ok = false; break; }
+    }
+    if (ok && n > 0 && (Pm[0] == T_BOMB || Pm[0] == T_FLAG) && (H[0] & 0x80)) ok = false;
+    if (ok) break;
+  }
+  for (int i = 0; i < n; ++i) {
+    CellSel s = cell_sel(H[i] & 0x7F);
+    bb_put(out.t0, s, Pm[i] & 1); bb_put(out.t1, s, (Pm[i] >> 1) & 1);
+    bb_put(out.t2, s, (Pm[i] >> 2) & 1); bb_put(out.t3, s, (Pm[i] >> 3) & 1);
+  }
+  return attempt + 1;
+}
+
+}  // namespace strat

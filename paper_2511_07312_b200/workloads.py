@@ -87,3 +87,24 @@ def board_str(line):
                 row.append(("b" if b & OWNER else "r") + sym[t])
         rows.append(" ".join(row))
     return "\n".join(rows)
+
+
+def capture_at_ply(env_get_boards, env_play_one_ply, num_games, ply):
+    """Root positions for the search-shaped batch (BASELINE.json configs[4]: "each reached by
+    200 uniform-random plies from a seeded classic setup").  Drives ANY environment exposing
+    the two callables (an auto-resetting env playing uniform-random legal actions) and keeps,
+    for every game slot, the first line whose ply counter equals `ply` while the game is
+    live; a game that ends earlier restarts (next epoch) and is captured in a later epoch.
+    Pure bookkeeping: no rule or RNG arithmetic here."""
+    roots = np.zeros((num_games, LINE), np.uint8)
+    have = np.zeros(num_games, bool)
+    for _ in range(100000):
+        b = env_get_boards()
+        p = b[:, 116].astype(int) | (b[:, 117].astype(int) << 8)
+        hit = (~have) & (p == ply) & ((b[:, 120] & 1) == 0)
+        roots[hit] = b[hit]
+        have |= hit
+        if have.all():
+            return roots
+        env_play_one_ply()
+    raise RuntimeError("roots not reached")

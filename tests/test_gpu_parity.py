@@ -1,0 +1,331 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle: bit-exact boards, masks,
+actions, rewards, done bytes and bf16 planes on the same seeded inputs."""
+import json
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import orc
+from paper_2511_07312_b200 import binding as B
+from paper_2511_07312_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _mask_np(t):
+    return _np(t).view(np.uint32)
+
+
+def _obs_np(t):
+    return _np(t.view(torch.int16)).view(np.uint16)
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _pair(n, **kw):
+    return B.Env(n, **kw), orc.Env(n, **kw)
+
+
+# ----------------------------------------------------------------------------- reset / lines
+@pytest.mark.parametrize("variant,n,seed,base", [(0, 300, 0, 0), (1, 77, 5, 0), (0, 33, 2**40 + 7, 1000)])
+def test_reset_matches_oracle(variant, n, seed, base):
+    g, o = _pair(n, variant=variant, seed=seed, game_base=base)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    g.reset(seed + 1); o.reset(seed + 1)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == 0
+
+
+def test_reset_from_get_boards_roundtrip_on_oracle_positions():
+    o = orc.Env(203, seed=3, max_plies=500, auto_reset=1)
+    g = B.Env(203, seed=99)
+    for step in range(330):
+        o.step(o.sample_uniform(o.legal_mask()))
+        if step % 30 == 29:
+            b = o.get_boards()
+            g.reset_from(_dev(b))
+            assert np.array_equal(_np(g.get_boards()), b)
+
+
+# ----------------------------------------------------------------------------- call by call
+@pytest.mark.parametrize("variant,n,plies,cap", [(0, 131, 400, 350), (1, 97, 600, 2000)])
+def test_each_call_on_injected_oracle_states(variant, n, plies, cap):
+    """The oracle plays; before every ply its state is injected with reset_from and each
+    C-ABI call is compared on its own."""
+    kw = dict(variant=variant, seed=17, max_plies=cap, auto_reset=0)
+    g, o = _pair(n, **kw)
+    for t in range(plies):
+        b = o.get_boards()
+        g.reset_from(_dev(b))
+        om = o.legal_mask()
+        gm = g.legal_mask()
+        assert np.array_equal(_mask_np(gm), om), t
+        oa = o.sample_uniform(om)
+        ga = g.sample_uniform(gm)
+        assert np.array_equal(_np(ga), oa), t
+        assert np.array_equal(_obs_np(g.encode_obs()), o.encode_obs().reshape(n, 44, 10, 10)), t
+        orr, od = o.step(oa)
+        gr, gd = g.step(ga)
+        assert np.array_equal(_np(gr), orr) and np.array_equal(_np(gd), od), t
+        assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+    assert g.check() == 0
+    assert (o.get_boards()[:, 120] & 1).sum() > 0  # some games ended inside the test
+
+
+def test_hand_worked_positions_on_gpu(golden_dir):
+    for pos in json.load(open(os.path.join(golden_dir, "positions.json")))["positions"]:
+        pieces = {c: W.piece(t, o) for c, t, o in pos["pieces"]}
+        g = B.Env(1)
+        g.reset_from(_dev(W.make_line(pieces)[None, :]))
+        for a in pos["play"]:
+            g.step(_dev(np.array([a], np.int16)))
+        assert g.check() == 0
+        assert W.mask_to_actions(_mask_np(g.legal_mask())[0]) == pos["expect"], pos["name"]
+
+
+def test_illegal_action_sets_sticky_error():
+    g, o = _pair(40, seed=1)
+    a = o.sample_uniform(o.legal_mask())
+    a[7] = 5
+    a[20] = -1
+    before = _np(g.get_boards()).copy()
+    r, d = g.step(_dev(a))
+    assert g.check() == B.ILLEGAL_ACTION
+    after = _np(g.get_boards())
+    orr, od = o.step(a)
+    assert np.array_equal(after, o.get_boards())
+    assert np.array_equal(before[7], after[7]) and np.array_equal(before[20], after[20])
+    assert np.array_equal(_np(r), orr) and np.array_equal(_np(d), od)
+    g.clear_error()
+    assert g.check() == 0
+
+
+# ----------------------------------------------------------------------------- rollouts (configs 0-2)
+def _run_separate(g, o, steps, every=1):
+    n = g.n
+    for t in range(steps):
+        gm = g.legal_mask(); ga = g.sample_uniform(gm); gr, gd = g.step(ga)
+        om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        assert np.array_equal(_np(ga), oa), t
+        assert np.array_equal(_np(gr), orr) and np.array_equal(_np(gd), od), t
+        if t % every == 0 or t == steps - 1:
+            assert np.array_equal(_mask_np(gm), om), t
+            assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+            assert np.array_equal(_obs_np(g.encode_obs()), o.encode_obs().reshape(n, 44, 10, 10)), t
+    assert g.check() == 0 and o.check() == 0
+
+
+def test_config0_classic_256_games_256_plies():
+    c = W.CONFIGS[0]
+    g, o = _pair(c["num_games"], variant=c["variant"], seed=c["seed"], max_plies=c["max_plies"],
+                 auto_reset=c["auto_reset"])
+    _run_separate(g, o, c["steps"])
+
+
+def _run_fused(g, o, steps, every=1, lo=0):
+    """fused rollout_step of the big env g vs oracle o that mirrors games lo..lo+o.n"""
+    n, k = g.n, o.n
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(steps):
+        om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        g.rollout_step(mask, act, rew, done, obs)
+        s = slice(lo, lo + k)
+        assert np.array_equal(_np(act[s]), oa), t
+        assert np.array_equal(_np(rew[s]), orr) and np.array_equal(_np(done[s]), od), t
+        if t % every == 0 or t == steps - 1:
+            assert np.array_equal(_mask_np(mask[s]), om), t
+            assert np.array_equal(_obs_np(obs[s]), o.encode_obs().reshape(k, 44, 10, 10)), t
+            assert np.array_equal(_np(g.get_boards()[s]), o.get_boards()), t
+    assert g.check() == 0
+
+
+def test_fused_step_small_with_auto_reset_and_ragged_tail():
+    kw = dict(variant=0, seed=4, max_plies=90, auto_reset=1)
+    g, o = _pair(1000, **kw)  # 1000 = 31 full batches + a tail of 8; every game resets 3 times
+    _run_fused(g, o, 300, every=7)
+    assert (o.get_boards()[:, 124] >= 3).all()
+
+
+def test_fused_step_null_outputs():
+    g1 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
+    g2 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
+    obs1, obs2 = g1.new_obs(), g2.new_obs()
+    mask, act, rew, done = g1.new_mask(), g1.new_actions(), g1.new_reward(), g1.new_done()
+    for _ in range(100):
+        g1.rollout_step(mask, act, rew, done, obs1)
+        g2.rollout_step(None, None, None, None, obs2)
+    assert torch.equal(obs1.view(torch.int16), obs2.view(torch.int16))
+    assert torch.equal(g1.get_boards(), g2.get_boards())
+
+
+def test_config1_barrage_4096_to_termination_sampled():
+    c = W.CONFIGS[1]
+    kw = dict(variant=1, seed=c["seed"], max_plies=c["max_plies"], auto_reset=0)
+    g = B.Env(c["num_games"], **kw)
+    lo = 4096 - 40  # the oracle mirrors the last 40 games (keyed by global index) ...
+    o = orc.Env(40, game_base=lo, **kw)
+    o2 = orc.Env(24, game_base=1000, **kw)  # ... and 24 from the middle
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(c["steps"]):
+        g.rollout_step(mask, act, rew, done, obs)
+        for oo, base in ((o, lo), (o2, 1000)):
+            om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
+            s = slice(base, base + oo.n)
+            assert np.array_equal(_np(act[s]), oa) and np.array_equal(_np(rew[s]), orr), t
+            assert np.array_equal(_np(done[s]), od), t
+            if t % 100 == 0:
+                assert np.array_equal(_mask_np(mask[s]), om), t
+                assert np.array_equal(_obs_np(obs[s]), oo.encode_obs().reshape(oo.n, 44, 10, 10)), t
+    b = _np(g.get_boards())
+    assert np.array_equal(b[lo:], o.get_boards()) and np.array_equal(b[1000:1024], o2.get_boards())
+    assert (b[:, 120] & 1).all()  # 2000-ply cap: every game is over
+    reasons = np.bincount((b[:, 120] >> 2) & 7, minlength=6)
+    assert reasons[0] == 0 and reasons[1] > 0 and reasons.sum() == 4096
+    # frozen games: zero mask, action -1, reward 0
+    assert not _mask_np(g.legal_mask()).any()
+    assert g.check() == 0
+
+
+def test_config2_full_size_sampled_games():
+    """N = 65,536 in the launch configuration bench.py times; the oracle mirrors three
+    32-game ranges (first, middle, last) by global game index."""
+    c = W.CONFIGS[2]
+    kw = dict(variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
+    g = B.Env(c["num_games"], **kw)
+    ranges = [0, 31337 // 32 * 32, 65536 - 32]
+    os_ = [orc.Env(32, game_base=lo, **kw) for lo in ranges]
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(260):
+        g.rollout_step(mask, act, rew, done, obs)
+        for oo, lo in zip(os_, ranges):
+            om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
+            s = slice(lo, lo + 32)
+            assert np.array_equal(_np(act[s]), oa) and np.array_equal(_np(rew[s]), orr), t
+            assert np.array_equal(_np(done[s]), od), t
+            if t % 20 == 0 or t == 259:
+                assert np.array_equal(_mask_np(mask[s]), om), t
+                assert np.array_equal(_obs_np(obs[s]), oo.encode_obs().reshape(32, 44, 10, 10)), t
+    b = _np(g.get_boards())
+    for oo, lo in zip(os_, ranges):
+        assert np.array_equal(b[lo:lo + 32], oo.get_boards())
+    # properties that hold at any size
+    x = (_obs_np(obs) == 0x3F80)
+    assert set(np.unique(_obs_np(obs[:4096]))) <= {0, 0x3F80}
+    assert (x[:, :28].sum(axis=1) == 1).all()
+    assert g.check() == 0
+
+
+# ----------------------------------------------------------------------------- replay ring (config 3 shape)
+def test_replay_ring_push_commit_sample_match_oracle():
+    n, per_slot, slots = 96, 64, 6  # capacity 384 = 4 pushes of 96
+    kw = dict(variant=0, seed=8, max_plies=60, auto_reset=1)
+    g, o = _pair(n, **kw)
+    ring, oring = B.Replay(per_slot, slots), orc.Replay(per_slot, slots)
+    obs = g.encode_obs()
+    batch = 512
+    s_obs = torch.empty((batch, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    s_mask = torch.empty((batch, 113), dtype=torch.int32, device="cuda")
+    s_act = torch.empty(batch, dtype=torch.int16, device="cuda")
+    s_rew = torch.empty(batch, dtype=torch.int8, device="cuda")
+    s_done = torch.empty(batch, dtype=torch.uint8, device="cuda")
+    for t in range(11):  # wraps the ring twice
+        oobs = o.encode_obs(); om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        oring.push(oobs, om, oa, orr, od)
+        gm = g.legal_mask(); ga = g.sample_uniform(gm); gr, gd = g.step(ga)
+        ring.push(obs, gm, ga, gr, gd)
+        obs = g.encode_obs()
+        assert ring.state() == (oring.head, oring.filled)
+        ring.sample(1234, t, batch, s_obs, s_mask, s_act, s_rew, s_done)
+        eo, em, ea, er, ed, idx = oring.sample(1234, t, batch)
+        assert np.array_equal(_obs_np(s_obs), eo) and np.array_equal(_mask_np(s_mask), em), t
+        assert np.array_equal(_np(s_act), ea) and np.array_equal(_np(s_rew), er) and np.array_equal(_np(s_done), ed), t
+    vo, vm, va, vr, vd = ring.views()
+    for p in range(ring.capacity):
+        eo, em, ea, er, ed = oring.read(p)
+        assert np.array_equal(_np(vo[p]).view(np.uint16), eo.reshape(-1))
+        assert np.array_equal(_np(vm[p]).view(np.uint32), em)
+        assert (int(va[p]), int(vr[p]), int(vd[p])) == (ea, er, ed)
+
+
+def test_replay_zero_copy_reserve_commit_equals_push():
+    n = 64
+    kw = dict(variant=0, seed=3, max_plies=50, auto_reset=1)
+    g1, g2 = B.Env(n, **kw), B.Env(n, **kw)
+    r1, r2 = B.Replay(32, 8), B.Replay(32, 8)  # capacity 256 = 4 x 64
+    act, rew, done = g1.new_actions(), g1.new_reward(), g1.new_done()
+    mask, obs = g1.new_mask(), g1.new_obs()
+    # path 1: copy push of (obs_t, mask_t, a_t, r_t, done_t)
+    obs_t = g1.encode_obs()
+    # path 2: obs_t / mask_t are written in place into the ring's next records
+    o_ptr, m_ptr = r2.reserve(n)
+    B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")
+    for t in range(9):
+        m = g1.legal_mask(); a = g1.sample_uniform(m); r, d = g1.step(a)
+        r1.push(obs_t, m, a, r, d)
+        obs_t = g1.encode_obs()
+        # zero-copy: mask_t goes to the reserved rows, obs_{t+1} to the rows reserved next
+        B._chk(B.lib().strat_legal_mask(g2.h, m_ptr, B._stream()), "mask")
+        a2 = g2.sample_uniform(_view_mask(r2, m_ptr, n))
+        r_, d_ = g2.step(a2)
+        r2.commit(a2, r_, d_)
+        o_ptr, m_ptr = r2.reserve(n)
+        B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")
+    # r2 holds one extra obs (the reserved next rows); compare committed records only
+    h, f = r1.state()
+    assert (h, f) == r2.state()
+    v1, v2 = r1.views(), r2.views()
+    keep = torch.ones(r1.capacity, dtype=torch.bool, device="cuda")
+    keep[h:h + n] = False  # oldest rows: overwritten in r2 by the in-place obs_{t+1}
+    for a_, b_ in zip(v1[2:], v2[2:]):
+        assert torch.equal(a_, b_)
+    assert torch.equal(v1[1][keep], v2[1][keep])
+    assert torch.equal(v1[0][keep], v2[0][keep])
+
+
+def _view_mask(ring, ptr, n):
+    base = ring.mem.data_ptr() + ring.offsets[1]
+    first = (ptr - base) // (113 * 4)
+    return ring.views()[1][first:first + n]
+
+
+# ----------------------------------------------------------------------------- search-shaped batch (config 4 shape)
+def test_determinise_rollout_reduce_match_oracle():
+    R, S, plies = 4, 96, 64
+    src = orc.Env(R, seed=0, max_plies=1000, auto_reset=1)
+    rb = W.capture_at_ply(src.get_boards, lambda: src.step(src.sample_uniform(src.legal_mask())), R, 200)
+    assert ((rb[:, 116].astype(int) | (rb[:, 117].astype(int) << 8)) == 200).all()
+    roots_o = orc.Env(R, seed=0)
+    roots_o.reset_from(rb)
+    side = np.array([(int(rb[r, 116]) | (int(rb[r, 117]) << 8)) & 1 for r in range(R)], np.uint8)
+    roots_g = B.Env(R, seed=0)
+    roots_g.reset_from(_dev(rb))
+    out_o = orc.Env(R * S, seed=0)
+    out_g = B.Env(R * S, seed=0)
+    orc.determinise(roots_o, S, 4242, out_o)
+    B.determinise(roots_g, S, 4242, out_g)
+    assert np.array_equal(_np(out_g.get_boards()), out_o.get_boards())
+    for _ in range(plies):
+        out_o.step(out_o.sample_uniform(out_o.legal_mask()))
+    out_g.rollout_uniform(plies)
+    assert np.array_equal(_np(out_g.get_boards()), out_o.get_boards())
+    red_o = orc.reduce_returns(out_o, side, S)
+    red_g = B.reduce_returns(out_g, _dev(side), S)
+    assert np.array_equal(_np(red_g), red_o)
+    assert out_g.check() == 0
+
+
+def test_rollout_uniform_equals_repeated_calls_with_auto_reset():
+    kw = dict(variant=0, seed=12, max_plies=70, auto_reset=1)
+    g1, g2 = B.Env(333, **kw), B.Env(333, **kw)
+    g1.rollout_uniform(150)
+    for _ in range(150):
+        g2.step(g2.sample_uniform(g2.legal_mask()))
+    assert torch.equal(g1.get_boards(), g2.get_boards())
