@@ -168,8 +168,8 @@ def run_b200(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     n = CFG["num_games"]
-    kw = dict(variant=CFG["variant"], seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1, device=local,
-              game_base=rank * n)  # weak scaling: every rank owns n independent games, no data-path collective
+    kw = W.shard_for_rank(CFG, rank, world)  # weak scaling: n independent games per rank, no data-path collective
+    kw["device"] = local
     env = B.Env(n, **kw)
     mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
     stream = torch.cuda.current_stream()

@@ -108,3 +108,12 @@ def capture_at_ply(env_get_boards, env_play_one_ply, num_games, ply):
             return roots
         env_play_one_ply()
     raise RuntimeError("roots not reached")
+
+
+def shard_for_rank(cfg, rank, world):
+    """Weak-scaling shard of a config for one rank: every rank owns `num_games` independent
+    games whose RNG streams are keyed by the global index game_base + local index, so the
+    union over ranks equals one world*num_games-game run.  No collective on the data path."""
+    assert 0 <= rank < world
+    return dict(variant=cfg["variant"], seed=cfg["seed"], max_plies=cfg["max_plies"],
+                auto_reset=cfg["auto_reset"], game_base=rank * cfg["num_games"])

@@ -1,0 +1,71 @@
+"""N>1 path on CPU: two gloo ranks, each running its shard (keyed by global game index);
+the gathered result must equal the unsharded run.  Exercises the shard description that
+bench.py uses under torchrun (workloads.shard_for_rank) with the oracle as the engine."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2511_07312_b200 import workloads as W
+
+CFG = dict(name="shard_test", variant=0, num_games=48, seed=5, max_plies=60, auto_reset=1)
+STEPS = 130
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _play(env, steps):
+    rewards = []
+    for _ in range(steps):
+        r, d = env.step(env.sample_uniform(env.legal_mask()))
+        rewards.append(r.copy())
+    return env.get_boards(), np.stack(rewards)
+
+
+def _worker(rank, world, port, out_path):
+    from oracle import orc
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    kw = W.shard_for_rank(CFG, rank, world)
+    env = orc.Env(CFG["num_games"], **kw)
+    boards, rewards = _play(env, STEPS)
+    t = torch.from_numpy(boards)
+    gathered = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(gathered, t)           # test plumbing only: the data path has no collective
+    elapsed = torch.tensor([float(rank + 1)])
+    dist.all_reduce(elapsed, op=dist.ReduceOp.MAX)  # bench.py's only reduction: max time
+    if rank == 0:
+        np.save(out_path, torch.cat(gathered).numpy())
+        assert elapsed.item() == float(world)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_shards_equal_unsharded_run(tmp_path):
+    from oracle import orc
+    world = 2
+    out = str(tmp_path / "gathered.npy")
+    mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+    sharded = np.load(out)
+    full = orc.Env(world * CFG["num_games"], variant=CFG["variant"], seed=CFG["seed"],
+                   max_plies=CFG["max_plies"], auto_reset=1)
+    boards, _ = _play(full, STEPS)
+    assert np.array_equal(sharded, boards)
+    assert (boards[:, 124] >= 2).all()  # every game went through at least two auto-resets
+
+
+def test_shard_description():
+    a = W.shard_for_rank(W.CONFIGS[2], 0, 8)
+    b = W.shard_for_rank(W.CONFIGS[2], 7, 8)
+    assert a["game_base"] == 0 and b["game_base"] == 7 * 65536
+    assert {k: v for k, v in a.items() if k != "game_base"} == {k: v for k, v in b.items() if k != "game_base"}
