@@ -216,7 +216,8 @@ __global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __r
   load_lines(lines, first, ng, s_state, lane);
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
-    if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, s_mask + lane * kMaskWords);
+    int cnt[4];
+    if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, s_mask + lane * kMaskWords, cnt);
   }
   __syncwarp();
   store_mask(mask, first, ng, s_mask, lane);
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
   load_lines(lines, first, ng, s_state, lane);
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
-    StepOut o = step_game(P, (uint32_t)(first + lane), g, (int)actions[first + lane]);
+    StepOut o = step_game<true>(P, (uint32_t)(first + lane), g, (int)actions[first + lane]);
     if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
     reward[first + lane] = (int8_t)o.reward;
     done[first + lane] = (uint8_t)o.done;
@@ -313,18 +314,17 @@ __global__ void __launch_bounds__(32) k_rollout_step(Params P, uint32_t* __restr
   zero_smem16(s_work, kMaskBytes, lane);
   load_lines(lines, first, ng, s_state, lane);
   Game g;
-  int n = 0;
+  int n = 0, cnt[4] = {0, 0, 0, 0};
   if (lane < ng) {
     read_game(s_state, lane, g);
-    if (!g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, s_work + lane * kMaskWords);
+    if (!g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, s_work + lane * kMaskWords, cnt);
   }
   __syncwarp();
   if (mask) store_mask(mask, first, ng, s_work, lane);
   if (lane < ng) {
     int a = -1;
-    if (n > 0) a = pick_action(s_work + lane * kMaskWords, n, action_draw(P, (uint32_t)(first + lane), g));
-    StepOut o = step_game(P, (uint32_t)(first + lane), g, a);
-    if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+    if (n > 0) a = pick_action(s_work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+    StepOut o = step_game<false>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
     if (actions) actions[first + lane] = (int16_t)a;
     if (reward) reward[first + lane] = (int8_t)o.reward;
     if (done) done[first + lane] = (uint8_t)o.done;
@@ -350,10 +350,10 @@ __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __re
     for (int t = 0; t < plies; ++t) {
       if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
       for (int w = 0; w < kMaskWords; ++w) row[w] = 0;
-      int n = legal_mask_row(g, g.ply & 1u, P.two_square, row);
-      int a = pick_action(row, n, action_draw(P, (uint32_t)(first + lane), g));
-      StepOut o = step_game(P, (uint32_t)(first + lane), g, a);
-      if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+      int cnt[4];
+      int n = legal_mask_row(g, g.ply & 1u, P.two_square, row, cnt);
+      int a = pick_action(row, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+      step_game<false>(P, (uint32_t)(first + lane), g, a);
     }
     write_game(s_state, lane, g);
   }

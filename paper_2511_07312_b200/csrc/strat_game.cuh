@@ -16,6 +16,7 @@
 #define SD static inline
 static inline int sd_popc(uint32_t x) { return __builtin_popcount(x); }
 static inline int sd_ffs(uint32_t x) { return __builtin_ffs((int)x); }
+static inline int sd_clz(uint32_t x) { return x ? __builtin_clz(x) : 32; }
 static inline uint32_t sd_mulhi(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) >> 32); }
 static inline uint32_t sd_fsr(uint32_t lo, uint32_t hi, int s) { return (uint32_t)((((uint64_t)hi << 32) | lo) >> s); }
 static inline uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return (uint32_t)(((((uint64_t)hi << 32) | lo) << s) >> 32); }
@@ -27,6 +28,7 @@ static inline int max(int a, int b) { return a > b ? a : b; }
 #define SD __device__ __forceinline__
 SD int sd_popc(uint32_t x) { return __popc(x); }
 SD int sd_ffs(uint32_t x) { return __ffs((int)x); }
+SD int sd_clz(uint32_t x) { return __clz((int)x); }
 SD uint32_t sd_mulhi(uint32_t a, uint32_t b) { return __umulhi(a, b); }
 SD uint32_t sd_fsr(uint32_t lo, uint32_t hi, int s) { return __funnelshift_r(lo, hi, s); }
 SD uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return __funnelshift_l(lo, hi, s); }
@@ -280,51 +282,91 @@ SD bool has_legal_move(const Game& g, int side, int two_square) {
   return bb_any(bb_or(bb_or(m.d[0], m.d[1]), bb_or(m.d[2], m.d[3])));
 }
 
-// Longest legal distance of the piece at c in direction d, given its single step is legal.
-SD int ray_length(const Moves& m, int c, int d, int row, int col, bool scout) {
-  int len = 1;
-  if (scout) {
-    int maxk = d == 0 ? 9 - row : d == 1 ? 9 - col : d == 2 ? row : col;
-    int delta = d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1;
-    int p = c + delta;
-    while (len < maxk && bb_test(m.empty, p) && bb_test(m.ok, p + delta)) { ++len; p += delta; }
+// ---- Scout rays without loops: pull the Scout's row and column out of the boards as 10-bit
+// lines and count empties with ffs/clz.
+SD uint32_t row_bits(const BB& a, int r) {  // bit i = cell 10r+i
+  int pos = 10 * r, wi = pos >> 5, sh = pos & 31;  // wi in 0..2
+  uint32_t lo = wi == 0 ? a.w[0] : wi == 1 ? a.w[1] : a.w[2];
+  uint32_t hi = wi == 0 ? a.w[1] : wi == 1 ? a.w[2] : a.w[3];
+  return sd_fsr(lo, hi, sh) & 0x3FFu;
+}
+SD uint32_t col_bits(const BB& a, int q) {  // bit i = cell 10i+q
+  // shift the board down by q, keep column 0, then squeeze the stride-10 bits together with
+  // one multiply per word (all partial products land on distinct bits)
+  uint32_t s0 = sd_fsr(a.w[0], a.w[1], q), s1 = sd_fsr(a.w[1], a.w[2], q), s2 = sd_fsr(a.w[2], a.w[3], q);
+  uint32_t x0 = ((s0 & 0x40100401u) * 0x08040201u) >> 27;  // cells 0,10,20,30   -> rows 0..3
+  uint32_t x1 = ((s1 & 0x10040100u) * 0x00100804u) >> 28;  // cells 40,50,60     -> rows 4..6
+  uint32_t x2 = ((s2 & 0x04010040u) * 0x00402010u) >> 28;  // cells 70,80,90     -> rows 7..9
+  return x0 | (x1 << 4) | (x2 << 7);
+}
+// e = empty squares of a 10-cell line, k = squares the mover may land on; from coordinate x.
+SD int ray_up(uint32_t e, uint32_t k, int x) {
+  uint32_t blockers = ((~e & 0x3FFu) >> (x + 1)) | (1u << (9 - x));  // + board-edge sentinel
+  int ne = sd_ffs(blockers) - 1;                                       // consecutive empties
+  return ne + (int)((k >> (x + 1 + ne)) & 1u);                         // + capture of the blocker
+}
+SD int ray_down(uint32_t e, uint32_t k, int x) {
+  uint32_t blockers = ~e & ((1u << x) - 1u);
+  int p = 31 - sd_clz(blockers);                                       // nearest blocker, -1 if none
+  return (x - 1 - p) + (int)(((k << 1) >> (p + 1)) & 1u);
+}
+// Longest legal distance of a Scout at c=(r,q) in each direction (0 if none), bans applied.
+SD void scout_rays(const Moves& m, int c, int r, int q, int len[4]) {
+  uint32_t er = row_bits(m.empty, r), kr = row_bits(m.ok, r);
+  uint32_t ec = col_bits(m.empty, q), kc = col_bits(m.ok, q);
+  len[0] = ray_up(ec, kc, r); len[1] = ray_up(er, kr, q);
+  len[2] = ray_down(ec, kc, r); len[3] = ray_down(er, kr, q);
+  if (m.ban.from == c) {
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d)
+      if (d == m.ban.dir) len[d] = min(len[d], m.ban.k - 1);
   }
-  if (m.ban.from == c && m.ban.dir == d) len = min(len, m.ban.k - 1);
-  return len;
+}
+
+SD void mask_or_field(uint32_t* row, int c, uint64_t field) {  // the 36 action bits of cell c
+  int pos = 36 * c, wi = pos >> 5, sh = pos & 31;
+  field <<= sh;  // 36 + 28 <= 64
+  row[wi] |= (uint32_t)field;
+  uint32_t hi = (uint32_t)(field >> 32);
+  if (hi) row[wi + 1] |= hi;
 }
 
 // Legal mask of `side` into `row` (113 words, already zero).  Returns the number of legal
-// actions.  Pieces are visited in ascending cell order, so bits are produced in ascending
-// action order: a = from*36 + dir*9 + dist-1.
-SD int legal_mask_row(const Game& g, int side, int two_square, uint32_t* row) {
+// actions and, in cnt[i], how many of them start from cells 32i..32i+31 (= mask words
+// 36i..36i+35; used by pick_action).  a = from*36 + dir*9 + dist-1.
+SD int legal_mask_row(const Game& g, int side, int two_square, uint32_t* row, int cnt[4]) {
   Moves m; single_step_moves(g, side, two_square, m);
-  int n = 0;
+  // pieces that move one square: four bits per piece, no branches
   STRAT_UNROLL
   for (int i = 0; i < 4; ++i) {
-    uint32_t any = m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i];
+    uint32_t sc = m.scouts.w[i];
+    uint32_t d0 = m.d[0].w[i] & ~sc, d1 = m.d[1].w[i] & ~sc, d2 = m.d[2].w[i] & ~sc, d3 = m.d[3].w[i] & ~sc;
+    cnt[i] = sd_popc(d0) + sd_popc(d1) + sd_popc(d2) + sd_popc(d3);
+    uint32_t any = d0 | d1 | d2 | d3;
     while (any) {
       int b = sd_ffs(any) - 1;
       any &= any - 1;
-      int c = 32 * i + b;
-      bool scout = (m.scouts.w[i] >> b) & 1u;
-      int r = c / 10, q = c - 10 * r;
-      uint64_t field = 0;
-      STRAT_UNROLL
-      for (int d = 0; d < 4; ++d) {
-        if ((m.d[d].w[i] >> b) & 1u) {
-          int len = ray_length(m, c, d, r, q, scout);
-          n += len;
-          field |= (uint64_t)((1u << len) - 1u) << (9 * d);
-        }
-      }
-      int pos = 36 * c, wi = pos >> 5, sh = pos & 31;
-      field <<= sh;  // 36 + 28 <= 64
-      row[wi] |= (uint32_t)field;
-      uint32_t hi = (uint32_t)(field >> 32);
-      if (hi) row[wi + 1] |= hi;
+      uint32_t f = ((d0 >> b) & 1u) | (((d1 >> b) & 1u) << 9) | (((d2 >> b) & 1u) << 18) | (((d3 >> b) & 1u) << 27);
+      mask_or_field(row, 32 * i + b, (uint64_t)f);
     }
   }
-  return n;
+  // Scouts: up to nine bits per direction
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & m.scouts.w[i];
+    while (ss) {
+      int b = sd_ffs(ss) - 1;
+      ss &= ss - 1;
+      int c = 32 * i + b, r = c / 10, q = c - 10 * r;
+      int len[4];
+      scout_rays(m, c, r, q, len);
+      cnt[i] += len[0] + len[1] + len[2] + len[3];
+      uint64_t field = (uint64_t)((1u << len[0]) - 1u) | ((uint64_t)((1u << len[1]) - 1u) << 9) |
+                       ((uint64_t)((1u << len[2]) - 1u) << 18) | ((uint64_t)((1u << len[3]) - 1u) << 27);
+      mask_or_field(row, c, field);
+    }
+  }
+  return cnt[0] + cnt[1] + cnt[2] + cnt[3];
 }
 
 // r-th (from 0) set bit of a word
@@ -337,11 +379,14 @@ STRAT_UNROLL
   }
   return pos;
 }
-// SampleRandomLegalAction, C3a: r-th set bit of the row, n = its popcount.
-SD int pick_action(const uint32_t* row, int n, uint32_t u) {
+// SampleRandomLegalAction, C3a: the r-th set bit of the row, r = bounded(u, n).
+// cnt[i] = set bits in mask words 36i..36i+35, so only one 36-word stretch is scanned.
+SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
   if (n == 0) return -1;
   int r = (int)bounded(u, (uint32_t)n);
-  for (int w = 0; w < kMaskWords; ++w) {
+  int w0 = 0;
+  if (r >= cnt[0]) { r -= cnt[0]; w0 = 36; if (r >= cnt[1]) { r -= cnt[1]; w0 = 72; if (r >= cnt[2]) { r -= cnt[2]; w0 = 108; } } }
+  for (int w = w0; w < kMaskWords; ++w) {
     int c = sd_popc(row[w]);
     if (r < c) return 32 * w + nth_set_bit(row[w], r);
     r -= c;
@@ -363,7 +408,10 @@ SD bool action_is_legal(const Game& g, int side, int two_square, int a) {
   if (dist == 1) return true;
   if (!bb_test(m.scouts, from)) return false;
   int r = from / 10, q = from - 10 * r;
-  return dist <= ray_length(m, from, d, r, q, true);
+  int len[4];
+  scout_rays(m, from, r, q, len);
+  int ld = d == 0 ? len[0] : d == 1 ? len[1] : d == 2 ? len[2] : len[3];
+  return dist <= ld;
 }
 
 // ------------------------------------------------------------------ setup (C2)
@@ -436,11 +484,13 @@ SD int battle(int att, int def) {
 
 struct StepOut { int reward; uint32_t done; bool illegal; };
 
+// kValidate = false only when `a` was just drawn from this state's own legal mask.
+template <bool kValidate>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   StepOut o; o.illegal = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
   int side = g.ply & 1u;
-  if (!action_is_legal(g, side, P.two_square, a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
+  if (kValidate && !action_is_legal(g, side, P.two_square, a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
   int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
   int to = from + dist * (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
   CellSel sf = cell_sel(from), st = cell_sel(to);
