@@ -237,17 +237,135 @@ def run_b200(args):
         dist.destroy_process_group()
 
 
+def _peak_line(achieved):
+    peak, src = measured_peak_gbs()
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": None, "peak_source": src, "frac_of_nominal_8000": achieved / 8000.0}
+
+
+def run_cfg3(args):
+    """BASELINE.json configs[3]: 262,144 games; every step also appends the transition to a
+    64 x 131,072-record device ring (zero-copy: the fused step writes mask_t and obs_{t+1} in
+    place) and gathers a uniform 4,096-transition minibatch."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    c = W.CONFIGS[3]
+    n = c["num_games"]
+    env = B.Env(n, variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
+    ring = B.Replay(c["ring_per_slot"], c["ring_slots"])
+    act, rew, done = env.new_actions(), env.new_reward(), env.new_done()
+    bs = c["sample_batch"]
+    s_obs = torch.empty((bs, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    s_mask = torch.empty((bs, 113), dtype=torch.int32, device="cuda")
+    s_act = torch.empty(bs, dtype=torch.int16, device="cuda")
+    s_rew = torch.empty(bs, dtype=torch.int8, device="cuda")
+    s_done = torch.empty(bs, dtype=torch.uint8, device="cuda")
+    o_ptr, _ = ring.reserve(n, 0)
+    B._chk(B.lib().strat_encode_obs(env.h, o_ptr, B._stream()), "encode")
+
+    def step(t):
+        _, m_ptr = ring.reserve(n, 0)
+        o_next, _ = ring.reserve(n, 1)
+        env.rollout_step_raw(m_ptr, act, rew, done, o_next)
+        ring.commit(act, rew, done)
+        ring.sample(c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
+
+    for t in range(args.warmup):
+        step(t)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for t in range(args.steps):
+        step(args.warmup + t)
+    e1.record()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    assert env.check() == 0
+    ms = e0.elapsed_time(e1)
+    per_game = ALGO_BYTES_PER_GAME_STEP + 8 + 2 * bs * W.TRANSITION_BYTES / n  # + commit copies + gather R/W
+    line = {
+        "metric": METRIC, "value": n * args.steps / (ms / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": c["name"], "games_per_gpu": n, "ring": "%d x %d records, %.1f GB" % (
+            c["ring_slots"], c["ring_per_slot"], ring.mem.numel() / 1e9), "sample_batch": bs,
+            "push": "zero-copy (fused step writes mask_t / obs_t+1 into the ring rows)"},
+        "roofline": dict(_peak_line(per_game * n / (ms / args.steps / 1e3) / 1e9), kernel="k_rollout_step + k_copy x3 + k_replay_sample",
+                         algorithmic_bytes_per_game_step=per_game),
+        "gpu_launches": 5 * args.steps, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
+def run_cfg4(args):
+    """BASELINE.json configs[4]: 16 roots (ply 200) x 16,384 determinisations, 64-ply uniform
+    rollouts with the boards on chip, per-root reduction.  A 'step' = the whole batch."""
+    import numpy as np
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    c = W.CONFIGS[4]
+    R, S, plies = c["num_roots"], c["samples_per_root"], c["rollout_plies"]
+    src = B.Env(R, variant=0, seed=c["seed"], max_plies=1000, auto_reset=1)
+
+    def play():
+        src.step(src.sample_uniform(src.legal_mask()))
+
+    rb = W.capture_at_ply(lambda: src.get_boards().cpu().numpy(), play, R, c["root_plies"])
+    roots = B.Env(R, variant=0, seed=c["seed"])
+    roots.reset_from(torch.from_numpy(rb).cuda())
+    side = torch.from_numpy(((rb[:, 116].astype(np.int64) | (rb[:, 117].astype(np.int64) << 8)) & 1).astype(np.uint8)).cuda()
+    out = B.Env(R * S, variant=0, seed=c["seed"], max_plies=0, auto_reset=0)
+    red = torch.empty((R, 3), dtype=torch.int32, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    t_det = t_roll = t_red = 0.0
+    steps = max(1, min(args.steps, 20))
+    for k in range(min(args.warmup, 3) + steps):
+        ev[0].record()
+        B.determinise(roots, S, 1000 + k, out)
+        ev[1].record()
+        out.rollout_uniform(plies)
+        ev[2].record()
+        B.reduce_returns(out, side, S, red)
+        ev[3].record()
+        torch.cuda.synchronize()
+        if k >= min(args.warmup, 3):
+            t_det += ev[0].elapsed_time(ev[1]); t_roll += ev[1].elapsed_time(ev[2]); t_red += ev[2].elapsed_time(ev[3])
+    assert out.check() == 0 and roots.check() == 0
+    total = t_det + t_roll + t_red
+    line = {
+        "metric": METRIC, "value": R * S * plies * steps / (total / 1e3), "unit": UNIT, "n_gpus": 1, "steps": steps,
+        "warmup": min(args.warmup, 3), "ms_per_step": total / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": c["name"], "roots": R, "samples_per_root": S, "rollout_plies": plies,
+                   "ms_determinise": t_det / steps, "ms_rollout": t_roll / steps, "ms_reduce": t_red / steps,
+                   "rollout_env_steps_per_sec": R * S * plies * steps / (t_roll / 1e3),
+                   "note": "ALU/latency-bound: boards stay in registers for all 64 plies (256 B of HBM per game)",
+                   "returns_sum_wins_losses_root0": red[0].tolist()},
+        "gpu_launches": 3 * steps,
+    }
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4"],
+                    help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4], 1 GPU")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "cfg3":
+        run_cfg3(args)
+    elif args.workload == "cfg4":
+        run_cfg4(args)
     else:
         run_b200(args)
 

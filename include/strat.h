@@ -168,11 +168,14 @@ int strat_replay_destroy(strat_replay* r);
 /* Append n records in order at (head+i) mod capacity; head += n; filled = min(filled+n, capacity). */
 int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
                       const int8_t* reward, const uint8_t* done, int32_t n, void* stream);
-/* Zero-copy push: the addresses of the next n records' obs and mask rows, so that
- * strat_rollout_step / strat_encode_obs can write them in place.  Fails with STRAT_BAD_ARG
- * unless the n records are contiguous (capacity % n == 0 and head % n == 0).
+/* Zero-copy push: the addresses of the obs and mask rows of the n records starting at
+ * head + ahead*n (ahead = 0: the records the next commit appends; ahead = 1: the block after
+ * it), so that strat_rollout_step / strat_encode_obs / strat_legal_mask can write them in
+ * place: in self-play record t = (obs_t, mask_t, a_t, r_t, done_t), obs_t is produced by step
+ * t-1 (ahead = 1 at that time) and mask_t by step t (ahead = 0).  Fails with STRAT_BAD_ARG
+ * unless blocks are contiguous (capacity % n == 0 and head % n == 0).
  * strat_replay_commit then appends action/reward/done for those n records and advances head. */
-int strat_replay_reserve(strat_replay* r, int32_t n, uint16_t** obs, uint32_t** mask);
+int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** obs, uint32_t** mask);
 int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done,
                         int32_t n, void* stream);
 /* Uniform minibatch with replacement: element j = record bounded(sample draw j, filled). */
@@ -183,9 +186,11 @@ int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled);
 
 /* ---- search-shaped batch (BASELINE.json configs[4]) ------------------------------- */
 /* out game G = r*samples_per_root + s: root r with the types of the searcher's opponent's
- * unrevealed pieces permuted uniformly over their squares, rejecting permutations that put a
- * Bomb or Flag on a moved piece (at most 4096 attempts, else the sticky error of `out` is
- * set to STRAT_BAD_STATE).  out->num_games must equal roots->num_games * samples_per_root. */
+ * unrevealed pieces re-dealt uniformly over their squares among the arrangements that put no
+ * Bomb or Flag on a moved piece: each hidden Bomb/Flag draws a free hidden square, redrawing
+ * while it is a moved piece's (rejection); the movable types are shuffled over the rest
+ * (R22).  More than 4096 draws for one game sets the sticky error of `out` to
+ * STRAT_BAD_STATE.  out->num_games must equal roots->num_games * samples_per_root. */
 int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t seed, strat_env* out,
                       void* stream);
 /* out int32[R][3] = {sum of returns, wins, losses} per root from the searcher's side

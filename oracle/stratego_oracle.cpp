@@ -25,7 +25,8 @@
 //   encode             pinned: partition property, start-position counts,
 //                      information-state property.
 //   replay ring        pinned: FIFO content, chi-square of indices.
-//   determinise        pinned: multiset/constraint/obs-equality properties.
+//   determinise        pinned: multiset/constraint/obs-equality properties, chi-square of
+//                      Bomb/Flag placement over the unmoved squares.
 //
 // Layouts:
 //   canonical line, 128 B per game:
@@ -647,11 +648,23 @@ int orc_replay_read(const Replay* r, int64_t p, uint16_t* obs, uint32_t* mask, i
 int64_t orc_replay_head(const Replay* r) { return r ? r->head : -1; }
 int64_t orc_replay_filled(const Replay* r) { return r ? r->filled : -1; }
 
-// ---- C7 determinise (BJ configs[4]): for output game G = r*S + s, permute the types of
-// the searcher's opponent's unrevealed pieces uniformly over their squares, rejecting
-// any permutation that puts a Bomb or Flag on a piece that has moved.  `attempts`
-// (optional, [R*S]) receives the number of attempts used.  R#22: the acceptance rate measured
-// on the 16 ply-200 roots of config 4 is 3e-4 .. 7e-3, so the safety cap is 2^20 attempts.
+// ---- C7 determinise (BJ configs[4]): for output game G = r*S + s, re-type the searcher's
+// opponent's unrevealed pieces with a uniformly random arrangement of their multiset that is
+// consistent with the public history (no Bomb or Flag on a piece that has moved).
+// Reading R#22: BJ says "permuted uniformly with rejection of any permutation that places a
+// Bomb or Flag on a moved piece".  Rejecting whole permutations accepts with probability
+// 3.9e-6 .. 2.6e-2 on the 16 ply-200 roots of config 4 (measured), i.e. up to ~250,000
+// attempts per sample, so the rejection is applied per placed piece instead, which yields the
+// same uniform distribution over consistent arrangements:
+//   1. each hidden Bomb/Flag, in ascending order of its original square, draws a square
+//      uniformly among the hidden squares still free, redrawing while that square holds a
+//      moved piece (rejection);
+//   2. the remaining (movable) types, in ascending order of their original squares, are
+//      shuffled by descending Fisher-Yates and dealt to the free squares in their list order.
+// The free-square list starts as the hidden squares ascending; taking entry i replaces it by
+// the last entry.  One DETERMINISE stream per output game: draw d = word d&3 of block d>>2,
+// counter (global G, 0, block).  More than 4096 draws -> BAD_STATE.  `attempts` (optional,
+// [R*S]) receives the number of draws used.
 int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, Env* out, int32_t* attempts) {
   if (!roots || !out || samples_per_root <= 0) return ORC_BAD_ARG;
   int R = roots->cfg.num_games;
@@ -671,23 +684,36 @@ int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, E
       int G = r * samples_per_root + s;
       uint32_t gidx = (uint32_t)(out->cfg.game_base + (uint64_t)G);
       Game gm = root;
-      int P[40];
-      int attempt = 0;
-      for (;; ++attempt) {
-        if (attempt >= (1 << 20)) return ORC_BAD_STATE;
-        for (int i = 0; i < n; ++i) P[i] = T[i];
-        for (int i = n - 1; i >= 1; --i) {
-          uint32_t u = stream_draw(seed, gidx, (uint32_t)attempt, 0, TAG_DETERMINISE, n - 1 - i);
-          int j = (int)bounded(u, (uint32_t)(i + 1));
-          int tmp = P[i]; P[i] = P[j]; P[j] = tmp;
+      int freeSq[40], m = n, d = 0;
+      for (int i = 0; i < n; ++i) freeSq[i] = H[i];
+      // 1. Bombs and Flag onto unmoved squares
+      for (int j = 0; j < n; ++j) {
+        if (T[j] != T_BOMB && T[j] != T_FLAG) continue;
+        for (;;) {
+          if (d >= 4096) return ORC_BAD_STATE;
+          uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
+          int idx = (int)bounded(u, (uint32_t)m);
+          int sq = freeSq[idx];
+          if (root.cell[sq] & B_MOVED) continue;  // rejection
+          gm.cell[sq] = (uint8_t)((root.cell[sq] & 0xF0) | T[j]);
+          freeSq[idx] = freeSq[m - 1];
+          --m;
+          break;
         }
-        bool okp = true;
-        for (int i = 0; i < n; ++i)
-          if ((P[i] == T_BOMB || P[i] == T_FLAG) && (root.cell[H[i]] & B_MOVED)) okp = false;
-        if (okp) break;
       }
-      for (int i = 0; i < n; ++i) gm.cell[H[i]] = (uint8_t)((root.cell[H[i]] & 0xF0) | P[i]);
-      if (attempts) attempts[G] = attempt + 1;
+      // 2. movable types over the remaining squares
+      int Tm[40], k = 0;
+      for (int j = 0; j < n; ++j)
+        if (T[j] != T_BOMB && T[j] != T_FLAG) Tm[k++] = T[j];
+      if (k != m) return ORC_BAD_STATE;
+      for (int i = k - 1; i >= 1; --i) {
+        if (d >= 4096) return ORC_BAD_STATE;
+        uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
+        int j = (int)bounded(u, (uint32_t)(i + 1));
+        int tmp = Tm[i]; Tm[i] = Tm[j]; Tm[j] = tmp;
+      }
+      for (int i = 0; i < k; ++i) gm.cell[freeSq[i]] = (uint8_t)((root.cell[freeSq[i]] & 0xF0) | Tm[i]);
+      if (attempts) attempts[G] = d;
       out->g[G] = gm;
     }
   }

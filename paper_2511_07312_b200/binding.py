@@ -71,7 +71,7 @@ def lib():
         L.strat_replay_create.argtypes = [vp, sz, i32, i32, C.POINTER(vp)]
         L.strat_replay_destroy.argtypes = [vp]
         L.strat_replay_push.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
-        L.strat_replay_reserve.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp)]
+        L.strat_replay_reserve.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(vp)]
         L.strat_replay_commit.argtypes = [vp, vp, vp, vp, i32, vp]
         L.strat_replay_sample.argtypes = [vp, u64, u64, i32, vp, vp, vp, vp, vp, vp]
         L.strat_replay_state.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -250,9 +250,9 @@ class Replay:
                                      _ptr(reward, torch.int8), _ptr(done, torch.uint8), n, _stream()),
              "strat_replay_push")
 
-    def reserve(self, n):
+    def reserve(self, n, ahead=0):
         obs, mask = C.c_void_p(), C.c_void_p()
-        _chk(lib().strat_replay_reserve(self.h, n, C.byref(obs), C.byref(mask)), "strat_replay_reserve")
+        _chk(lib().strat_replay_reserve(self.h, n, ahead, C.byref(obs), C.byref(mask)), "strat_replay_reserve")
         return obs.value, mask.value
 
     def commit(self, action, reward, done):

@@ -718,10 +718,12 @@ int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask
   return launch_status();
 }
 
-int strat_replay_reserve(strat_replay* r, int32_t n, uint16_t** obs, uint32_t** mask) {
-  if (!r || !obs || !mask || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0) return STRAT_BAD_ARG;
-  *obs = r->obs + (size_t)r->head * STRAT_OBS_ELEMS;
-  *mask = r->mask + (size_t)r->head * STRAT_MASK_WORDS;
+int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** obs, uint32_t** mask) {
+  if (!r || !obs || !mask || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0 || ahead < 0)
+    return STRAT_BAD_ARG;
+  size_t first = (size_t)((r->head + (int64_t)ahead * n) % r->capacity);
+  *obs = r->obs + first * STRAT_OBS_ELEMS;
+  *mask = r->mask + first * STRAT_MASK_WORDS;
   return STRAT_OK;
 }
 

@@ -665,54 +665,70 @@ SD void export_canonical(const Game& g, uint8_t* L) {
 }
 
 // ------------------------------------------------------------------ determinise (C7)
-// Re-type the hidden pieces of the searcher's opponent: uniform permutation of their types
-// over their squares (descending Fisher-Yates on DETERMINISE draws), rejecting any
-// permutation that puts a Bomb or Flag on a moved piece.  Position i is final once its swap is
-// done, so a violation there rejects the attempt at once; the accepted attempt and its result
-// are those of the plain draw-everything-then-test loop.  Returns the attempts used, or 0 if
-// the safety cap of 2^20 was hit (R#22: measured acceptance on ply-200 roots is 3e-4..7e-3).
+// Re-type the hidden pieces of the searcher's opponent with a uniformly random arrangement
+// consistent with the public history (R#22): each hidden Bomb/Flag, in ascending order of its
+// original square, draws a free hidden square, redrawing while that square holds a moved piece;
+// the movable types are then shuffled (descending Fisher-Yates) and dealt to the remaining
+// free squares.  One DETERMINISE draw stream per output game.  Returns draws used, 0 on the
+// 4096-draw safety cap.
+struct DrawStream {
+  uint32_t gidx, k0, k1, o[4];
+  int d;
+};
+SD uint32_t next_draw(DrawStream& s) {
+  if ((s.d & 3) == 0) philox(s.gidx, 0u, (uint32_t)(s.d >> 2), TAG_DETERMINISE, s.k0, s.k1, s.o);
+  int k = s.d & 3;
+  ++s.d;
+  return k == 0 ? s.o[0] : k == 1 ? s.o[1] : k == 2 ? s.o[2] : s.o[3];
+}
 SD int determinise_game(const Game& root, uint32_t k0, uint32_t k1, uint32_t gidx, Game& out) {
   out = root;
   int searcher = root.ply & 1u;
   BB occ = occupied(root);
   BB enemy = bb_andn(occ, owned_by(root, occ, searcher));
   BB hidden = bb_andn(enemy, root.rev);
-  uint8_t H[40], T[40], Pm[40];
+  uint8_t freeSq[40], T[40], Tm[40];  // freeSq bit 7: the piece on that square has moved
   int n = 0;
   for (int i = 0; i < 4; ++i) {
     uint32_t w = hidden.w[i];
     while (w && n < 40) {
       int b = sd_ffs(w) - 1; w &= w - 1;
       int c = 32 * i + b;
-      H[n] = (uint8_t)(c | (bb_test(root.mvd, c) << 7));  // bit 7: this piece has moved
+      freeSq[n] = (uint8_t)(c | (bb_test(root.mvd, c) << 7));
       T[n] = (uint8_t)(bb_test(root.t0, c) | (bb_test(root.t1, c) << 1) | (bb_test(root.t2, c) << 2) |
                        (bb_test(root.t3, c) << 3));
       ++n;
     }
   }
-  int attempt = 0;
-  for (;; ++attempt) {
-    if (attempt >= (1 << 20)) return 0;
-    for (int i = 0; i < n; ++i) Pm[i] = T[i];
-    uint32_t o[4] = {0, 0, 0, 0};
-    bool ok = true;
-    for (int i = n - 1; i >= 1; --i) {
-      int d = n - 1 - i;
-      if ((d & 3) == 0) philox(gidx, (uint32_t)attempt, (uint32_t)(d >> 2), TAG_DETERMINISE, k0, k1, o);
-      uint32_t u = (d & 3) == 0 ? o[0] : (d & 3) == 1 ? o[1] : (d & 3) == 2 ? o[2] : o[3];
-      int j = (int)bounded(u, (uint32_t)(i + 1));
-      uint8_t t = Pm[j]; Pm[j] = Pm[i]; Pm[i] = t;
-      if ((t == T_BOMB || t == T_FLAG) && (H[i] & 0x80)) { ok = false; break; }
+  DrawStream ds; ds.gidx = gidx; ds.k0 = k0; ds.k1 = k1; ds.d = 0;
+  ds.o[0] = ds.o[1] = ds.o[2] = ds.o[3] = 0;
+  int m = n, k = 0;
+  for (int j = 0; j < n; ++j) {
+    int t = T[j];
+    if (t != T_BOMB && t != T_FLAG) { Tm[k++] = (uint8_t)t; continue; }
+    for (;;) {
+      if (ds.d >= 4096) return 0;
+      int idx = (int)bounded(next_draw(ds), (uint32_t)m);
+      int sq = freeSq[idx];
+      if (sq & 0x80) continue;  // a moved piece cannot be a Bomb or the Flag
+      CellSel s = cell_sel(sq);
+      bb_put(out.t0, s, t & 1); bb_put(out.t1, s, (t >> 1) & 1); bb_put(out.t2, s, (t >> 2) & 1); bb_put(out.t3, s, (t >> 3) & 1);
+      freeSq[idx] = freeSq[m - 1];
+      --m;
+      break;
     }
-    if (ok && n > 0 && (Pm[0] == T_BOMB || Pm[0] == T_FLAG) && (H[0] & 0x80)) ok = false;
-    if (ok) break;
   }
-  for (int i = 0; i < n; ++i) {
-    CellSel s = cell_sel(H[i] & 0x7F);
-    bb_put(out.t0, s, Pm[i] & 1); bb_put(out.t1, s, (Pm[i] >> 1) & 1);
-    bb_put(out.t2, s, (Pm[i] >> 2) & 1); bb_put(out.t3, s, (Pm[i] >> 3) & 1);
+  for (int i = k - 1; i >= 1; --i) {
+    if (ds.d >= 4096) return 0;
+    int j = (int)bounded(next_draw(ds), (uint32_t)(i + 1));
+    uint8_t t = Tm[i]; Tm[i] = Tm[j]; Tm[j] = t;
   }
-  return attempt + 1;
+  for (int i = 0; i < k; ++i) {
+    CellSel s = cell_sel(freeSq[i] & 0x7F);
+    int t = Tm[i];
+    bb_put(out.t0, s, t & 1); bb_put(out.t1, s, (t >> 1) & 1); bb_put(out.t2, s, (t >> 2) & 1); bb_put(out.t3, s, (t >> 3) & 1);
+  }
+  return ds.d > 0 ? ds.d : 1;
 }
 
 }  // namespace strat

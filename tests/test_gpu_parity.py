@@ -256,44 +256,35 @@ def test_replay_ring_push_commit_sample_match_oracle():
 
 
 def test_replay_zero_copy_reserve_commit_equals_push():
+    """Self-play loop of config 3 two ways: (1) separate calls + copying push, (2) the fused
+    step writing mask_t and obs_{t+1} straight into the ring rows + commit."""
     n = 64
     kw = dict(variant=0, seed=3, max_plies=50, auto_reset=1)
     g1, g2 = B.Env(n, **kw), B.Env(n, **kw)
-    r1, r2 = B.Replay(32, 8), B.Replay(32, 8)  # capacity 256 = 4 x 64
-    act, rew, done = g1.new_actions(), g1.new_reward(), g1.new_done()
-    mask, obs = g1.new_mask(), g1.new_obs()
-    # path 1: copy push of (obs_t, mask_t, a_t, r_t, done_t)
+    r1, r2 = B.Replay(32, 8), B.Replay(32, 8)  # capacity 256 = 4 blocks of 64
+    act, rew, done = g2.new_actions(), g2.new_reward(), g2.new_done()
     obs_t = g1.encode_obs()
-    # path 2: obs_t / mask_t are written in place into the ring's next records
-    o_ptr, m_ptr = r2.reserve(n)
-    B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")
-    for t in range(9):
+    o_ptr, _ = r2.reserve(n, 0)
+    B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")  # obs_0 in place
+    for t in range(9):  # wraps the ring twice
         m = g1.legal_mask(); a = g1.sample_uniform(m); r, d = g1.step(a)
         r1.push(obs_t, m, a, r, d)
         obs_t = g1.encode_obs()
-        # zero-copy: mask_t goes to the reserved rows, obs_{t+1} to the rows reserved next
-        B._chk(B.lib().strat_legal_mask(g2.h, m_ptr, B._stream()), "mask")
-        a2 = g2.sample_uniform(_view_mask(r2, m_ptr, n))
-        r_, d_ = g2.step(a2)
-        r2.commit(a2, r_, d_)
-        o_ptr, m_ptr = r2.reserve(n)
-        B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")
-    # r2 holds one extra obs (the reserved next rows); compare committed records only
-    h, f = r1.state()
-    assert (h, f) == r2.state()
+        _, m_ptr = r2.reserve(n, 0)        # mask_t -> the rows being completed
+        o_next, _ = r2.reserve(n, 1)       # obs_{t+1} -> the rows of the next block
+        g2.rollout_step_raw(m_ptr, act, rew, done, o_next)
+        r2.commit(act, rew, done)
+    assert r1.state() == r2.state()
+    h, _ = r1.state()
     v1, v2 = r1.views(), r2.views()
     keep = torch.ones(r1.capacity, dtype=torch.bool, device="cuda")
-    keep[h:h + n] = False  # oldest rows: overwritten in r2 by the in-place obs_{t+1}
-    for a_, b_ in zip(v1[2:], v2[2:]):
+    keep[h:h + n] = False  # r2 already holds obs_9 in the block the next commit will complete
+    for a_, b_ in zip(v1[1:], v2[1:]):
         assert torch.equal(a_, b_)
-    assert torch.equal(v1[1][keep], v2[1][keep])
     assert torch.equal(v1[0][keep], v2[0][keep])
+    assert torch.equal(v2[0][h:h + n].view(n, -1), obs_t.view(torch.int16).view(n, -1))
+    assert torch.equal(g1.get_boards(), g2.get_boards())
 
-
-def _view_mask(ring, ptr, n):
-    base = ring.mem.data_ptr() + ring.offsets[1]
-    first = (ptr - base) // (113 * 4)
-    return ring.views()[1][first:first + n]
 
 
 # ----------------------------------------------------------------------------- search-shaped batch (config 4 shape)

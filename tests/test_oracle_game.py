@@ -426,3 +426,30 @@ def test_determinise_properties_and_rollout_reduce():
         res = fb[r * S:(r + 1) * S, 121].view(np.int8).astype(int) * (fb[r * S:(r + 1) * S, 120] & 1)
         ret = res * (1 if side[r] == 0 else -1)
         assert red[r].tolist() == [ret.sum(), (ret > 0).sum(), (ret < 0).sum()]
+
+
+def test_determinise_is_uniform_over_consistent_arrangements():
+    # Small hand-built root: blue hides Flag, Bomb, Spy, Scout on 4 squares of which one has
+    # moved.  Consistent arrangements: Flag and Bomb on two of the three unmoved squares
+    # (3*2 = 6 ordered ways) x 2 orders of {Spy, Scout} on the rest = 12, each with p = 1/12.
+    pieces = {0: W.piece(W.FLAG, 0), 11: W.piece(W.MARSHAL, 0),
+              88: W.piece(W.FLAG, 1), 89: W.piece(W.BOMB, 1), 78: W.piece(W.SPY, 1),
+              68: W.piece(W.SCOUT, 1, moved=True), 99: W.piece(W.MINER, 1, revealed=True)}
+    root = orc.Env(1)
+    root.reset_from(W.make_line(pieces, ply=10)[None])
+    S = 12000
+    out = orc.Env(S)
+    draws = orc.determinise(root, S, seed=5, out=out)
+    b = out.get_boards()
+    hid = [68, 78, 88, 89]
+    keys = {}
+    for s in range(S):
+        t = tuple(int(b[s, c]) & 15 for c in hid)
+        keys[t] = keys.get(t, 0) + 1
+        assert (b[s, 68] & 15) in (W.SPY, W.SCOUT)            # the moved piece is never Bomb/Flag
+        assert b[s, 99] == pieces[99] and b[s, 11] == pieces[11]
+    assert len(keys) == 12
+    exp = S / 12.0
+    chi2 = sum((v - exp) ** 2 / exp for v in keys.values())
+    assert chi2 < 40.0, chi2  # 11 dof
+    assert draws.min() >= 3 and draws.max() < 60
