@@ -13,6 +13,7 @@
 // 16 bytes.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <new>
 
 #include "../../include/strat.h"
@@ -337,6 +338,243 @@ __global__ void __launch_bounds__(32) k_rollout_step(Params P, uint32_t* __restr
   expand_obs(obs, first, ng, s_work, s_lut, lane);
 }
 
+// ---- the fused hot path, warp-specialised and persistent -------------------------------
+// One CTA = one LOGIC warp + one STORE warp sharing two staging buffers.  The logic warp
+// walks batches of 32 games (thread per game): state line straight from global into
+// registers, mask rows into the stage, mask/action/reward/done/state out, then the new
+// state's 4400-bit observation stream into the same stage.  The store warp expands finished
+// stages to bf16 and streams them out.  The two are decoupled by mbarriers, so on every SM
+// observation stores of batch i flow while batch i+1 is still in its (latency-bound) rule
+// logic; with one-warp CTAs all resident warps ran logic, then stores, in lockstep.
+#ifdef STRAT_PROF  // developer build only (_work/): per-phase cycle counters
+__device__ unsigned long long g_prof[32];
+__device__ unsigned long long g_trace[8192 * 6];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ unsigned smid() { unsigned r; asm volatile("mov.u32 %0, %smid;" : "=r"(r)); return r; }
+#define TRACE(b, k, v) do { if (lane == 0 && (b) < 8192) g_trace[(b) * 6 + (k)] = (v); } while (0)
+#define PROF_T(v) long long v = clock64()
+#define PROF_ADD(slot, a, b) do { if (lane == 0) atomicAdd(&g_prof[slot], (unsigned long long)((b) - (a))); } while (0)
+#else
+#define PROF_T(v)
+#define PROF_ADD(slot, a, b)
+#define TRACE(b, k, v)
+#endif
+constexpr int kWsStages = 2;
+constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+  uint32_t a = smem_u32(b), ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+// nibble -> 4 bf16 (0x3F80 where the bit is set); 16 entries x 8 B = one bank row, so the
+// two LDS.64 per 16-byte chunk never conflict.
+__device__ __forceinline__ void fill_lut16(uint2* lut, int tid) {
+  if (tid < 16) {
+    uint2 v;
+    v.x = ((tid & 1) ? 0x3F80u : 0u) | ((tid & 2) ? 0x3F800000u : 0u);
+    v.y = ((tid & 4) ? 0x3F80u : 0u) | ((tid & 8) ? 0x3F800000u : 0u);
+    lut[tid] = v;
+  }
+}
+__device__ __forceinline__ void expand_obs16(uint16_t* __restrict__ obs, int first_game, int ng,
+                                             const uint32_t* s_bits, const uint2* lut, int lane) {
+  for (int gi = 0; gi < ng; ++gi) {
+    const uint8_t* row = reinterpret_cast<const uint8_t*>(s_bits + gi * kBitsRowWords);
+    uint4* dst = reinterpret_cast<uint4*>(obs + (size_t)(first_game + gi) * STRAT_OBS_ELEMS);
+#pragma unroll
+    for (int k = 0; k < 17; ++k) {
+      uint32_t b = row[32 * k + lane];
+      uint2 lo = lut[b & 15u], hi = lut[b >> 4];
+      st_stream(dst + 32 * k + lane, make_uint4(lo.x, lo.y, hi.x, hi.y));
+    }
+    if (lane < kObsChunks - 544) {
+      uint32_t b = row[544 + lane];
+      uint2 lo = lut[b & 15u], hi = lut[b >> 4];
+      st_stream(dst + 544 + lane, make_uint4(lo.x, lo.y, hi.x, hi.y));
+    }
+  }
+}
+__device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ lines, int game, Game& g) {
+  uint32_t W[32];
+  const uint4* p = reinterpret_cast<const uint4*>(lines + (size_t)game * kLineWords);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { uint4 v = __ldcg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+  unpack_line(W, g);
+}
+__device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, int game, const Game& g) {
+  uint32_t W[32];
+  pack_line(g, W);
+  uint4* p = reinterpret_cast<uint4*>(lines + (size_t)game * kLineWords);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) __stcg(p + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+}
+
+// Warp-cooperative auto-reset of the games flagged in `rs` (bit = lane = game of the batch):
+// the result equals setup_game (C2: descending Fisher-Yates over the listed multiset, one
+// Philox stream per side).  The 2 x 10 Philox blocks of a game are drawn by 20 lanes at once,
+// the sequential swaps run on a 40-byte row of shared memory, and the bit planes are built
+// with warp ballots (lane = cell of a 32-cell word).  Attempt 0 of both sides is produced
+// here; a side that fails the mobility test (R#5, p ~ 2e-6) sends that game through the
+// thread-per-game setup_game, which redraws.  `scratch` >= 3,200 words.
+__device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t rs, Game& g, uint32_t* scratch, int lane) {
+  const uint32_t full = 0xffffffffu;
+  uint32_t* sD = scratch;                                        // [32][2][40] draws
+  uint8_t* sA = reinterpret_cast<uint8_t*>(scratch + 32 * 80);  // [32][2][40] piece types
+  for (uint32_t m = rs; m; m &= m - 1) {
+    int owner = __ffs((int)m) - 1;
+    uint32_t epoch = __shfl_sync(full, g.epoch, owner);
+    if (lane < 20) {
+      int side = lane >= 10 ? 1 : 0, blk = lane - 10 * side;
+      uint32_t o[4];
+      philox(P.game_base + (uint32_t)(first + owner), epoch, (uint32_t)blk, side ? TAG_SETUP_BLUE : TAG_SETUP_RED,
+             P.key0, P.key1, o);
+      uint32_t* d = sD + owner * 80 + side * 40 + 4 * blk;
+      d[0] = o[0]; d[1] = o[1]; d[2] = o[2]; d[3] = o[3];
+    }
+    for (int i = lane; i < 80; i += 32) sA[owner * 80 + i] = (uint8_t)multiset_type(P.variant, i < 40 ? i : i - 40);
+  }
+  __syncwarp();
+  if ((rs >> lane) & 1u) {
+    for (int side = 0; side < 2; ++side) {
+      uint8_t* A = sA + lane * 80 + side * 40;
+      const uint32_t* D = sD + lane * 80 + side * 40;
+      for (int i = 39; i >= 1; --i) {
+        int j = (int)bounded(D[39 - i], (uint32_t)(i + 1));
+        uint8_t t = A[i]; A[i] = A[j]; A[j] = t;
+      }
+    }
+  }
+  __syncwarp();
+  for (uint32_t m = rs; m; m &= m - 1) {
+    int owner = __ffs((int)m) - 1;
+    const uint8_t* A = sA + owner * 80;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      int c = 32 * w + lane;
+      uint32_t t = c < 40 ? A[c] : (c >= 60 && c < 100) ? A[c - 20] : 0u;
+      uint32_t b0 = __ballot_sync(full, t & 1u), b1 = __ballot_sync(full, t & 2u), b2 = __ballot_sync(full, t & 4u),
+               b3 = __ballot_sync(full, t & 8u), bo = __ballot_sync(full, t != 0u && c >= 60);
+      if (lane == owner) { g.t0.w[w] = b0; g.t1.w[w] = b1; g.t2.w[w] = b2; g.t3.w[w] = b3; g.own.w[w] = bo; }
+    }
+  }
+  if ((rs >> lane) & 1u) {
+    g.mvd = g.rev = bb_zero();
+    hist_clear(g);
+    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0;
+    if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
+  }
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
+                                                        int16_t* __restrict__ actions, int8_t* __restrict__ reward,
+                                                        uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
+                                                        uint32_t* __restrict__ ticket, uint32_t ticket_base) {
+  __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
+  __shared__ __align__(8) uint2 s_lut[16];
+  __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
+  __shared__ int s_batch[kWsStages];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nbatches = (P.num_games + kBatch - 1) / kBatch;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < kWsStages; ++s) { mbar_init(&s_full[s], 32); mbar_init(&s_empty[s], 32); }
+  }
+  fill_lut16(s_lut, threadIdx.x);
+  __syncthreads();
+  if (warp == 0) {
+    // ------------------------------------------------ logic warp (thread per game)
+    // batches: the first one is the CTA's own index, the rest are drawn from a ticket counter
+    // that only ever counts up (this launch owns tickets ticket_base .. ticket_base+nbatches-grid-1
+    // and consumes exactly nbatches - grid + grid of them), so slow batches do not stall a queue.
+    int b = blockIdx.x;
+    for (int it = 0;; ++it) {
+      const int stage = it % kWsStages, round = it / kWsStages;
+      uint32_t* work = s_stage[stage];
+      PROF_T(t0);
+      if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
+      if (it > 0) {
+        uint32_t tk = 0;
+        if (lane == 0) tk = atomicAdd(ticket, 1u) - ticket_base;
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        b = tk < (uint32_t)(nbatches - (int)gridDim.x) ? (int)(gridDim.x + tk) : -1;
+      }
+      if (b < 0) {
+        if (lane == 0) s_batch[stage] = -1;
+        mbar_arrive(&s_full[stage]);
+        break;
+      }
+      const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      PROF_T(t1);
+      TRACE(b, 0, gtime()); TRACE(b, 4, smid()); TRACE(b, 5, blockIdx.x);
+      zero_smem16(work, kMaskBytes, lane);
+      Game g;
+      int n = 0, cnt[4] = {0, 0, 0, 0};
+      if (lane < ng) load_game_global(lines, first + lane, g);
+      __syncwarp();
+      PROF_T(t2);
+      if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);
+      __syncwarp();
+      PROF_T(t3);
+      if (mask) store_mask(mask, first, ng, work, lane);
+      PROF_T(t4);
+      bool reset_me = false;
+      if (lane < ng) {
+        int a = -1;
+        if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+        StepOut o = step_game<false, true>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+        if (actions) actions[first + lane] = (int16_t)a;
+        if (reward) reward[first + lane] = (int8_t)o.reward;
+        if (done) done[first + lane] = (uint8_t)o.done;
+        reset_me = o.needs_reset;
+      }
+      uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
+      if (rs) coop_setup(P, first, rs, g, work, lane);
+      if (lane < ng) store_game_global(lines, first + lane, g);
+      __syncwarp();  // the stage becomes bit streams
+      PROF_T(t5);
+      if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
+      __syncwarp();
+      PROF_T(t6);
+      if (lane == 0) s_batch[stage] = b;
+      mbar_arrive(&s_full[stage]);
+      TRACE(b, 1, gtime());
+      PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4); PROF_ADD(4, t4, t5);
+      PROF_ADD(5, t5, t6); PROF_ADD(6, t0, t6); PROF_ADD(7, 0, 1);
+    }
+  } else {
+    // ------------------------------------------------ store warp (lane per 16-byte chunk)
+    for (int it = 0;; ++it) {
+      const int stage = it % kWsStages, round = it / kWsStages;
+      PROF_T(t0);
+      mbar_wait(&s_full[stage], (uint32_t)round & 1u);
+      const int b = s_batch[stage];
+      if (b < 0) break;
+      const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      PROF_T(t1);
+      TRACE(b, 2, gtime());
+      expand_obs16(obs, first, ng, s_stage[stage], s_lut, lane);
+      TRACE(b, 3, gtime());
+      PROF_T(t2);
+      mbar_arrive(&s_empty[stage]);
+      PROF_ADD(8, t0, t1); PROF_ADD(9, t1, t2); PROF_ADD(10, 0, 1);
+    }
+  }
+}
+
 // `plies` plies of uniform-random legal play with the board in registers.
 __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
@@ -493,6 +731,9 @@ struct strat_env {
   strat::Params P;
   uint32_t* lines;
   int* err;
+  uint32_t* ticket;      // device batch-ticket counter (monotonic), see k_rollout_step_ws
+  uint32_t ticket_base;  // first ticket of the next launch
+  int num_sms;
 };
 
 struct strat_replay {
@@ -530,6 +771,11 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->lines = reinterpret_cast<uint32_t*>(workspace_dev);
   e->err = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(workspace_dev) +
                                   align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256));
+  e->ticket = reinterpret_cast<uint32_t*>(e->err) + 16;
+  e->ticket_base = 0;
+  k_set_int<<<1, 1, 0, (cudaStream_t)stream>>>(reinterpret_cast<int*>(e->ticket), 0);
+  e->num_sms = 148;
+  cudaDeviceGetAttribute(&e->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
   *out = e;
   return strat_reset(e, cfg->seed, stream);
 }
@@ -588,8 +834,17 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done,
                        uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;
-  k_rollout_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward,
-                                                                            done, obs, env->err);
+  static const int impl = getenv("STRAT_ROLLOUT_IMPL") ? atoi(getenv("STRAT_ROLLOUT_IMPL")) : 1;
+  static const int per_sm = getenv("STRAT_CTAS_PER_SM") ? atoi(getenv("STRAT_CTAS_PER_SM")) : 6;
+  if (impl == 0) {
+    k_rollout_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward,
+                                                                              done, obs, env->err);
+  } else {
+    int nb = batches(env->P.num_games), grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
+    k_rollout_step_ws<<<grid, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward, done, obs,
+                                                            env->ticket, env->ticket_base);
+    env->ticket_base += (uint32_t)nb;  // nb - grid successful draws + one failing draw per CTA
+  }
   return launch_status();
 }
 
@@ -777,5 +1032,16 @@ int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32
   k_reduce_returns<<<R, 256, 0, (cudaStream_t)stream>>>(games->lines, root_side, samples_per_root, out);
   return launch_status();
 }
+
+#ifdef STRAT_PROF
+int strat_debug_prof(unsigned long long* out_host, int clear) {
+  if (cudaMemcpyFromSymbol(out_host, g_prof, sizeof(g_prof)) != cudaSuccess) return STRAT_CUDA_ERROR;
+  if (clear) { unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_prof, z, sizeof(z)); }
+  return STRAT_OK;
+}
+int strat_debug_trace(unsigned long long* out_host) {
+  return cudaMemcpyFromSymbol(out_host, g_trace, sizeof(g_trace)) == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR;
+}
+#endif
 
 }  // extern "C"

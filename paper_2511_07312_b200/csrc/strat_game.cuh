@@ -435,6 +435,19 @@ SD uint32_t multiset_type(int variant, int i) {
   return i == 0 ? 11 : i == 1 ? 10 : i == 2 ? 9 : i == 3 ? 3 : i == 4 ? 2 : i == 5 ? 2 : i == 6 ? 1
        : i == 7 ? 12 : 0;
 }
+// R#5: can this side ever move: a movable own piece next to a non-lake square without an own
+// piece (depends on the side's own pieces only).
+SD bool side_can_ever_move(const Game& t, int side) {
+  BB occ = occupied(t);
+  BB mine = owned_by(t, occ, side);
+  BB ok = bb_andn(bb_const(kNotLake), mine);
+  BB imm = bb_and(t.t3, bb_or(t.t2, bb_and(t.t1, t.t0)));
+  BB mv = bb_andn(mine, imm);
+  BB can = bb_or(bb_or(bb_and(mv, bb_down<10>(ok)), bb_and(mv, bb_up<10>(ok))),
+                 bb_or(bb_and(bb_and(mv, bb_down<1>(ok)), bb_const(kNotCol9)),
+                       bb_and(bb_and(mv, bb_up<1>(ok)), bb_const(kNotCol0))));
+  return bb_any(can);
+}
 // Fresh game for (global game, g.epoch): both sides by descending Fisher-Yates over the
 // listed multiset, redrawn until the side can ever move (R#4, R#5).
 SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
@@ -459,16 +472,7 @@ SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
       int base = side ? 60 : 0;
       for (int i = 0; i < 40; ++i)
         if (A[i]) put_piece(trial, base + i, A[i], side);
-      // can this side ever move: a movable own piece next to a non-lake square without an own piece
-      BB occ = occupied(trial);
-      BB mine = owned_by(trial, occ, side);
-      BB ok = bb_andn(bb_const(kNotLake), mine);
-      BB imm = bb_and(trial.t3, bb_or(trial.t2, bb_and(trial.t1, trial.t0)));
-      BB mv = bb_andn(mine, imm);
-      BB can = bb_or(bb_or(bb_and(mv, bb_down<10>(ok)), bb_and(mv, bb_up<10>(ok))),
-                     bb_or(bb_and(bb_and(mv, bb_down<1>(ok)), bb_const(kNotCol9)),
-                           bb_and(bb_and(mv, bb_up<1>(ok)), bb_const(kNotCol0))));
-      if (bb_any(can)) { g = trial; break; }
+      if (side_can_ever_move(trial, side)) { g = trial; break; }
     }
   }
 }
@@ -482,12 +486,14 @@ SD int battle(int att, int def) {
   return att > def ? 1 : att < def ? -1 : 0;
 }
 
-struct StepOut { int reward; uint32_t done; bool illegal; };
+struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; };
 
 // kValidate = false only when `a` was just drawn from this state's own legal mask.
-template <bool kValidate>
+// kDeferReset: the caller performs the auto-reset itself (epoch is already advanced) when
+// o.needs_reset is set; the result must equal setup_game(P, local_game, g).
+template <bool kValidate, bool kDeferReset = false>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
-  StepOut o; o.illegal = false;
+  StepOut o; o.illegal = false; o.needs_reset = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
   int side = g.ply & 1u;
   if (kValidate && !action_is_legal(g, side, P.two_square, a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
@@ -537,7 +543,10 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   }
   o.reward = g.done ? g.result : 0;
   o.done = g.done | ((uint32_t)side << 1) | ((g.done ? g.reason : 0u) << 2);
-  if (g.done && P.auto_reset) { g.epoch += 1; setup_game(P, local_game, g); }  // R#16
+  if (g.done && P.auto_reset) {  // R#16
+    g.epoch += 1;
+    if (kDeferReset) o.needs_reset = true; else setup_game(P, local_game, g);
+  }
   return o;
 }
 
