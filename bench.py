@@ -184,16 +184,23 @@ def run_b200(args):
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    # events only at chunk boundaries: consecutive fused steps overlap on the device (programmatic
+    # dependent launch), and an event record between two launches would serialise them
+    chunk = max(1, args.steps // 20)
+    marks = list(range(0, args.steps, chunk)) + [args.steps]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in marks]
     ev[0].record(stream)
+    nxt = 1
     for k in range(args.steps):
         env.rollout_step(mask, act, rew, done, obs)
-        ev[k + 1].record(stream)
+        if k + 1 == marks[nxt]:
+            ev[nxt].record(stream)
+            nxt += 1
     barrier()
     sampler.stop_flag = True
     sampler.join()
     total_ms = ev[0].elapsed_time(ev[-1])
-    per_step = sorted(ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps))
+    per_step = sorted(ev[i].elapsed_time(ev[i + 1]) / (marks[i + 1] - marks[i]) for i in range(len(marks) - 1))
     median_ms = per_step[len(per_step) // 2]
     assert env.check() == 0
     t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")

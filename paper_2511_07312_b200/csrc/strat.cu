@@ -1,19 +1,19 @@
 // strat.cu — sm_100a kernels and the C ABI of libstrat.so (include/strat.h).
 //
-// Execution model: one warp = one batch of 32 games = one CTA.
-//   * I/O phases are warp-cooperative: the 32 games' 128-byte lines (4 KB contiguous), their
-//     mask rows (32 x 452 B contiguous) and their observations (32 x 8800 B contiguous) move
-//     as coalesced 16-byte vector accesses, staged through shared memory.
-//   * Logic phases are thread-per-game on 100-bit bitboards held in registers
-//     (strat_game.cuh), reading/writing per-game rows of shared memory whose strides
-//     (144 B, 113 words, 139 words) make the 32 lanes hit 32 different banks.
-// The observation is produced as a 4400-bit stream per game; byte q of the stream expands,
-// through a 256-entry x 16 B shared-memory table, to the q-th 16-byte chunk of the bf16
-// planes, so the 8800-byte store costs one byte load, one table load and one STG.128 per
-// 16 bytes.
+// Execution model: a batch = 32 consecutive games.
+//   * Logic is thread-per-game on 100-bit bitboards held in registers (strat_game.cuh),
+//     reading/writing per-game rows of shared memory whose strides (144 B, 113 words, 139 words)
+//     make the 32 lanes hit 32 different banks.
+//   * I/O is warp-cooperative: mask rows (32 x 452 B contiguous) and observations (32 x 8800 B
+//     contiguous) leave as coalesced 16-byte vector stores staged through shared memory.
+//   * The observation is produced as a 4400-bit stream per game; byte q of the stream expands,
+//     through a small shared-memory table, to the q-th 16-byte chunk of the bf16 planes.
+//   * The fused step (k_rollout_step) is persistent and warp-specialised: per CTA one logic
+//     warp and one store warp, decoupled by mbarriers; consecutive launches overlap through
+//     programmatic dependent launch and are ordered batch by batch with version flags.
+//   * The single-purpose kernels (k_legal_mask, k_step, k_encode_obs, ...) run one warp per CTA.
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <stdlib.h>
 #include <new>
 
 #include "../../include/strat.h"
@@ -29,7 +29,6 @@ constexpr int kBitsRowWords = 139;                   // 138 used; odd stride -> 
 constexpr int kObsChunks = 550;                      // 16-B chunks per game observation
 constexpr int kStateBytes = kBatch * kStateStride;   // 4608
 constexpr int kMaskBytes = kBatch * kMaskRowBytes;   // 14464
-constexpr int kBitsBytes = kBatch * kBitsRowWords * 4;  // 17792
 
 // ------------------------------------------------------------------ small PTX helpers
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -287,7 +286,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
 
 __global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __restrict__ lines, uint16_t* __restrict__ obs) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
-  __shared__ __align__(16) uint32_t s_bits[kBatch * kBitsRowWords];
+  __shared__ __align__(16) uint32_t s_bits[kBatch * kBitsRowWords];  // 17,792 B
   __shared__ __align__(16) uint4 s_lut[256];
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, P.num_games - first);
@@ -299,43 +298,6 @@ __global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __r
   }
   __syncwarp();
   expand_obs(obs, first, ng, s_bits, s_lut, lane);
-}
-
-// The fused hot path: mask -> uniform action -> step -> encode, one pass over the state.
-__global__ void __launch_bounds__(32) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
-                                                     int16_t* __restrict__ actions, int8_t* __restrict__ reward,
-                                                     uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
-                                                     int* __restrict__ err) {
-  __shared__ __align__(16) uint8_t s_state[kStateBytes];
-  __shared__ __align__(16) uint32_t s_work[kBitsBytes / 4];  // mask rows, then observation bit streams
-  __shared__ __align__(16) uint4 s_lut[256];
-  int lane = threadIdx.x, first = blockIdx.x * kBatch;
-  int ng = min(kBatch, P.num_games - first);
-  fill_lut(s_lut, lane, 32);
-  zero_smem16(s_work, kMaskBytes, lane);
-  load_lines(lines, first, ng, s_state, lane);
-  Game g;
-  int n = 0, cnt[4] = {0, 0, 0, 0};
-  if (lane < ng) {
-    read_game(s_state, lane, g);
-    if (!g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, s_work + lane * kMaskWords, cnt);
-  }
-  __syncwarp();
-  if (mask) store_mask(mask, first, ng, s_work, lane);
-  if (lane < ng) {
-    int a = -1;
-    if (n > 0) a = pick_action(s_work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
-    StepOut o = step_game<false>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
-    if (actions) actions[first + lane] = (int16_t)a;
-    if (reward) reward[first + lane] = (int8_t)o.reward;
-    if (done) done[first + lane] = (uint8_t)o.done;
-    write_game(s_state, lane, g);
-  }
-  __syncwarp();  // all lanes are done with the mask rows before they become bit streams
-  if (lane < ng) encode_bits(g, s_work + lane * kBitsRowWords);
-  __syncwarp();
-  store_lines(lines, first, ng, s_state, lane);
-  expand_obs(obs, first, ng, s_work, s_lut, lane);
 }
 
 // ---- the fused hot path, warp-specialised and persistent -------------------------------
@@ -360,6 +322,14 @@ __device__ __forceinline__ unsigned smid() { unsigned r; asm volatile("mov.u32 %
 #define TRACE(b, k, v)
 #endif
 constexpr int kWsStages = 2;
+// Resident CTAs per SM of ONE launch.  Two consecutive launches are co-resident (6 CTAs x 35.7 KB
+// of shared memory per SM): the later one trails the earlier one batch by batch, so the HBM
+// write stream never drains between steps.  Measured on B200 at 65,536 games: 2 -> 88.8 us,
+// 3 -> 87.8 us, 4 -> 90.3 us, 6 -> 93.1 us per step.
+#ifndef STRAT_WS_CTAS_PER_SM
+#define STRAT_WS_CTAS_PER_SM 3
+#endif
+constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
 constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -378,6 +348,27 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok) : "r"(a), "r"(parity) : "memory");
   } while (!ok);
+}
+// Per-batch version flags in global memory: consecutive launches of the fused step overlap
+// (programmatic dependent launch), ordered batch by batch instead of kernel by kernel.
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// whole warp: returns once *flag == want (lane 0 polls; the barrier orders the other lanes)
+__device__ __forceinline__ void flag_wait(const uint32_t* flag, uint32_t want, int lane) {
+  if (lane == 0)
+    while (ld_acquire(flag) != want) __nanosleep(64);
+  __syncwarp();
+}
+// whole warp: publish this warp's prior global writes, then set the flag
+__device__ __forceinline__ void flag_set(uint32_t* flag, uint32_t v, int lane) {
+  __syncwarp();
+  if (lane == 0) { __threadfence(); st_release(flag, v); }
 }
 // nibble -> 4 bf16 (0x3F80 where the bit is set); 16 entries x 8 B = one bank row, so the
 // two LDS.64 per 16-byte chunk never conflict.
@@ -479,10 +470,11 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
+__global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
-                                                        uint32_t* __restrict__ ticket, uint32_t ticket_base) {
+                                                        uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
+                                                        uint32_t* __restrict__ f_obs, uint32_t version) {
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
@@ -495,11 +487,14 @@ __global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __re
   }
   fill_lut16(s_lut, threadIdx.x);
   __syncthreads();
+  // Let the next launch of this kernel become resident now: it orders itself behind this one
+  // batch by batch through f_state / f_obs (it never calls griddepcontrol.wait).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (warp == 0) {
     // ------------------------------------------------ logic warp (thread per game)
-    // batches: the first one is the CTA's own index, the rest are drawn from a ticket counter
-    // that only ever counts up (this launch owns tickets ticket_base .. ticket_base+nbatches-grid-1
-    // and consumes exactly nbatches - grid + grid of them), so slow batches do not stall a queue.
+    // batches: the first one is the CTA's own index, the rest are drawn from this launch's
+    // ticket counter.  atomicInc wraps to 0 after exactly nbatches draws (nbatches - grid
+    // successful ones + one failing draw per CTA), so the counter cleans up after itself.
     int b = blockIdx.x;
     for (int it = 0;; ++it) {
       const int stage = it % kWsStages, round = it / kWsStages;
@@ -508,7 +503,7 @@ __global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __re
       if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
       if (it > 0) {
         uint32_t tk = 0;
-        if (lane == 0) tk = atomicAdd(ticket, 1u) - ticket_base;
+        if (lane == 0) tk = atomicInc(ticket, (uint32_t)nbatches - 1u);
         tk = __shfl_sync(0xffffffffu, tk, 0);
         b = tk < (uint32_t)(nbatches - (int)gridDim.x) ? (int)(gridDim.x + tk) : -1;
       }
@@ -518,6 +513,7 @@ __global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __re
         break;
       }
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      flag_wait(f_state + b, version - 1u, lane);  // the previous launch is done with this batch's state
       PROF_T(t1);
       TRACE(b, 0, gtime()); TRACE(b, 4, smid()); TRACE(b, 5, blockIdx.x);
       zero_smem16(work, kMaskBytes, lane);
@@ -544,6 +540,7 @@ __global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __re
       uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
       if (rs) coop_setup(P, first, rs, g, work, lane);
       if (lane < ng) store_game_global(lines, first + lane, g);
+      flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
       __syncwarp();  // the stage becomes bit streams
       PROF_T(t5);
       if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
@@ -564,9 +561,11 @@ __global__ void __launch_bounds__(64) k_rollout_step_ws(Params P, uint32_t* __re
       const int b = s_batch[stage];
       if (b < 0) break;
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      flag_wait(f_obs + b, version - 1u, lane);  // write-after-write on a reused obs buffer
       PROF_T(t1);
       TRACE(b, 2, gtime());
       expand_obs16(obs, first, ng, s_stage[stage], s_lut, lane);
+      flag_set(f_obs + b, version, lane);
       TRACE(b, 3, gtime());
       PROF_T(t2);
       mbar_arrive(&s_empty[stage]);
@@ -701,6 +700,11 @@ inline Params make_params(const strat_config& c) {
 }
 inline int launch_status() { return cudaGetLastError() == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR; }
 inline int batches(int n) { return (n + kBatch - 1) / kBatch; }
+// A launch cannot start before every CTA of the previous one has started, and each launch in
+// flight holds at least one of the <= 32 x SMs resident CTA slots, so far fewer than kTicketRing
+// launches are ever in flight and two launches never share a ticket counter.
+constexpr int kTicketRing = 8192;
+inline size_t sync_words(int n) { return (size_t)kTicketRing + 2 * (size_t)batches(n); }
 
 template <typename T>
 void copy_elems(const T* src, T* dst, size_t count, cudaStream_t s) {
@@ -731,8 +735,10 @@ struct strat_env {
   strat::Params P;
   uint32_t* lines;
   int* err;
-  uint32_t* ticket;      // device batch-ticket counter (monotonic), see k_rollout_step_ws
-  uint32_t ticket_base;  // first ticket of the next launch
+  uint32_t* tickets;     // ring of kTicketRing self-resetting batch-ticket counters (slot = version % ring)
+  uint32_t* f_state;     // [batches] version of the last fused step that finished the batch's state
+  uint32_t* f_obs;       // [batches] ... that finished the batch's observation stores
+  uint32_t version;      // fused-step launches so far
   int num_sms;
 };
 
@@ -756,7 +762,7 @@ const char* strat_error_string(int code) {
 
 size_t strat_workspace_bytes(const strat_config* cfg) {
   if (!cfg_ok(cfg)) return 0;
-  return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256;
+  return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256 + align_up(sync_words(cfg->num_games) * 4, 256);
 }
 
 int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream, strat_env** out) {
@@ -771,9 +777,14 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->lines = reinterpret_cast<uint32_t*>(workspace_dev);
   e->err = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(workspace_dev) +
                                   align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256));
-  e->ticket = reinterpret_cast<uint32_t*>(e->err) + 16;
-  e->ticket_base = 0;
-  k_set_int<<<1, 1, 0, (cudaStream_t)stream>>>(reinterpret_cast<int*>(e->ticket), 0);
+  e->tickets = reinterpret_cast<uint32_t*>(e->err) + 64;
+  e->f_state = e->tickets + kTicketRing;
+  e->f_obs = e->f_state + batches(cfg->num_games);
+  e->version = 0;
+  if (cudaMemsetAsync(e->tickets, 0, sync_words(cfg->num_games) * 4, (cudaStream_t)stream) != cudaSuccess) {
+    delete e;
+    return STRAT_CUDA_ERROR;
+  }
   e->num_sms = 148;
   cudaDeviceGetAttribute(&e->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
   *out = e;
@@ -834,18 +845,24 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done,
                        uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;
-  static const int impl = getenv("STRAT_ROLLOUT_IMPL") ? atoi(getenv("STRAT_ROLLOUT_IMPL")) : 1;
-  static const int per_sm = getenv("STRAT_CTAS_PER_SM") ? atoi(getenv("STRAT_CTAS_PER_SM")) : 6;
-  if (impl == 0) {
-    k_rollout_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward,
-                                                                              done, obs, env->err);
-  } else {
-    int nb = batches(env->P.num_games), grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
-    k_rollout_step_ws<<<grid, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions, reward, done, obs,
-                                                            env->ticket, env->ticket_base);
-    env->ticket_base += (uint32_t)nb;  // nb - grid successful draws + one failing draw per CTA
-  }
-  return launch_status();
+  const int nb = batches(env->P.num_games);
+  const int grid = nb < env->num_sms * kWsCtasPerSm ? nb : env->num_sms * kWsCtasPerSm;
+  // Programmatic dependent launch: this launch may become resident while the previous launch
+  // in the stream is still running IF that one is also a fused step (it is the only kernel
+  // that executes griddepcontrol.launch_dependents); behind any other kernel the attribute
+  // changes nothing.  Ordering against the previous fused step is per batch (f_state/f_obs).
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(64); lc.dynamicSmemBytes = 0; lc.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  const uint32_t version = env->version + 1;
+  if (cudaLaunchKernelEx(&lc, k_rollout_step, env->P, env->lines, mask, actions, reward, done, obs,
+                         env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version) != cudaSuccess)
+    return STRAT_CUDA_ERROR;
+  env->version = version;
+  return STRAT_OK;
 }
 
 size_t strat_host_scratch_bytes(const strat_config* cfg) {

@@ -27,7 +27,8 @@ def test_library_exports_every_declared_symbol():
 def test_host_only_entry_points():
     L = binding.lib()
     cfg = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0)
-    assert L.strat_workspace_bytes(C.byref(cfg)) == 65536 * 128 + 256
+    ws = L.strat_workspace_bytes(C.byref(cfg))  # lines + error block + ticket ring + 2 flags per 32-game batch
+    assert ws == 65536 * 128 + 256 + (8192 + 2 * 2048) * 4
     bad = binding.strat_config(0, 0, 0, 0, 0, 0, 1, 0, 0, 0)
     assert L.strat_workspace_bytes(C.byref(bad)) == 0
     assert L.strat_error_string(-4) == b"illegal action for a live game"

@@ -166,6 +166,63 @@ def test_fused_step_null_outputs():
     assert torch.equal(g1.get_boards(), g2.get_boards())
 
 
+def test_fused_steps_back_to_back_overlap_equals_synchronised_run():
+    """Consecutive fused steps overlap on the device (programmatic dependent launch, ordered
+    per batch by version flags).  400 launches with no host sync in between, at the bench's
+    size, must leave exactly what a run synchronised after every launch leaves, and what the
+    oracle computes for sampled game ranges."""
+    c = W.CONFIGS[2]
+    kw = dict(variant=0, seed=c["seed"], max_plies=150, auto_reset=1)  # cap 150: every game resets at least twice
+    n, steps = c["num_games"], 400
+    g1, g2 = B.Env(n, **kw), B.Env(n, **kw)
+    outs1 = (g1.new_mask(), g1.new_actions(), g1.new_reward(), g1.new_done(), g1.new_obs())
+    outs2 = (g2.new_mask(), g2.new_actions(), g2.new_reward(), g2.new_done(), g2.new_obs())
+    for _ in range(steps):
+        g1.rollout_step(*outs1)
+    for _ in range(steps):
+        g2.rollout_step(*outs2)
+        torch.cuda.synchronize()
+    assert torch.equal(g1.get_boards(), g2.get_boards())
+    for a, b in zip(outs1, outs2):
+        assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))
+    ranges = [0, 40000 // 32 * 32 + 8, n - 32]
+    for lo in ranges:
+        o = orc.Env(32, game_base=lo, **kw)
+        for _ in range(steps):
+            om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        s = slice(lo, lo + 32)
+        assert np.array_equal(_mask_np(outs1[0][s]), om) and np.array_equal(_np(outs1[1][s]), oa)
+        assert np.array_equal(_np(outs1[2][s]), orr) and np.array_equal(_np(outs1[3][s]), od)
+        assert np.array_equal(_obs_np(outs1[4][s]), o.encode_obs().reshape(32, 44, 10, 10))
+        assert np.array_equal(_np(g1.get_boards()[s]), o.get_boards())
+    assert g1.check() == 0 and g2.check() == 0
+
+
+def test_fused_step_interleaved_with_other_calls():
+    """A fused step after any other state-changing call (and vice versa) sees that call's result."""
+    kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)
+    g, o = _pair(700, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(120):
+        if t % 3 == 2:  # separate calls
+            gm = g.legal_mask(); ga = g.sample_uniform(gm); g.step(ga)
+        elif t % 10 == 5:  # state round trip through the canonical lines
+            g.reset_from(g.get_boards().clone())
+            g.rollout_step(mask, act, rew, done, obs)
+        else:
+            g.rollout_step(mask, act, rew, done, obs)
+        o.step(o.sample_uniform(o.legal_mask()))
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    g.rollout_step(mask, act, rew, done, obs)
+    o.step(o.sample_uniform(o.legal_mask()))
+    assert np.array_equal(_obs_np(obs), o.encode_obs().reshape(700, 44, 10, 10))
+    g.reset(5); o.reset(5)
+    g.rollout_step(mask, act, rew, done, obs)
+    o.step(o.sample_uniform(o.legal_mask()))
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == 0
+
+
 def test_config1_barrage_4096_to_termination_sampled():
     c = W.CONFIGS[1]
     kw = dict(variant=1, seed=c["seed"], max_plies=c["max_plies"], auto_reset=0)
