@@ -25,6 +25,7 @@ METRIC = "stratego_env_steps_per_sec"
 UNIT = "env_steps/s"
 ALGO_BYTES_PER_GAME_STEP = 128 + 128 + 452 + 2 + 1 + 1 + 8800  # state R+W, mask, action, reward, done, obs = 9512
 CFG = W.CONFIGS[2]
+NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.5e6  # profiles/r1_d_rollout_step_full.md (65,536 games per launch)
 
 
 def measured_peak_gbs():
@@ -216,7 +217,7 @@ def run_b200(args):
         peak, peak_src = measured_peak_gbs()
         kernel_ms = total_ms / args.steps  # the step IS one launch of k_rollout_step
         achieved = ALGO_BYTES_PER_GAME_STEP * n / (kernel_ms / 1e3) / 1e9
-        cpu_games, cpu_steps = 1024, 200
+        cpu_games, cpu_steps = 2048, 300
         cpu_rate, cpu_dt = oracle_rate(cpu_games, cpu_steps, 10) if (world == 1 and not args.skip_cpu) else (None, None)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -227,7 +228,11 @@ def run_b200(args):
                        "parallelism": "games sharded over %d GPU(s), no collective" % world,
                        "l2": "outputs 623 MB/step per GPU > 126 MB L2 (no flush needed)"},
             "roofline": {"bound": "hbm", "kernel": "k_rollout_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if n == 65536 else None,
+                         "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch "
+                                           "(profiles/r1_d_rollout_step_full.md)",
+                         "peak_source": peak_src,
+                         "note": "peak is a copy (half reads); a pure write stream exceeds it, hence frac > 1",
                          "algorithmic_bytes_per_game_step": ALGO_BYTES_PER_GAME_STEP,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": None if e2e_value is None else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * n * world,
