@@ -59,6 +59,7 @@ def lib():
         L.orc_replay_head.restype = C.c_int64
         L.orc_replay_filled.argtypes = [vp]
         L.orc_replay_filled.restype = C.c_int64
+        L.orc_sample_indices.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int64, vp]
         L.orc_determinise.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp]
         L.orc_reduce_returns.argtypes = [vp, vp, C.c_int32, vp]
         L.orc_philox.argtypes = [vp, vp, vp]
@@ -194,6 +195,13 @@ class Replay:
     @property
     def filled(self):
         return lib().orc_replay_filled(self.h)
+
+
+def sample_indices(seed, draw_index, batch, filled):
+    idx = np.zeros(batch, np.int64)
+    _chk(lib().orc_sample_indices(seed, draw_index, batch, filled, _p(idx)),
+         "sample_indices")
+    return idx
 
 
 def determinise(roots: Env, samples_per_root: int, seed: int, out: Env):

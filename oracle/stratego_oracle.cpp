@@ -612,19 +612,30 @@ int orc_replay_push(Replay* r, const uint16_t* obs, const uint32_t* mask, const 
   return ORC_OK;
 }
 
-// Element j reads physical record bounded(draw j, filled); SAMPLE stream: c0 = block,
-// (c1,c2) = draw_index lo,hi.  `indices` (optional) receives the physical indices.
+// Physical record index of batch element j (C6 / R#20): bounded(draw j, filled); SAMPLE stream:
+// c0 = block j>>2, (c1,c2) = draw_index lo,hi, word j&3.
+static int64_t sample_index(uint64_t seed, uint64_t draw_index, int j, int64_t filled) {
+  uint32_t ctr[4] = {(uint32_t)(j >> 2), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), TAG_SAMPLE};
+  uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t o[4];
+  philox4x32_10(ctr, key, o);
+  return (int64_t)bounded(o[j & 3], (uint32_t)filled);
+}
+// The indices alone (full-size rings do not fit in host memory; the tests gather on their own).
+int orc_sample_indices(uint64_t seed, uint64_t draw_index, int32_t batch, int64_t filled, int64_t* indices) {
+  if (!indices || batch < 0 || filled <= 0 || filled > 0xFFFFFFFFll) return ORC_BAD_ARG;
+  for (int j = 0; j < batch; ++j) indices[j] = sample_index(seed, draw_index, j, filled);
+  return ORC_OK;
+}
+
+// Element j reads physical record sample_index(j).  `indices` (optional) receives the indices.
 int orc_replay_sample(const Replay* r, uint64_t seed, uint64_t draw_index, int32_t batch,
                       uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
                       int64_t* indices) {
   if (!r || batch < 0) return ORC_BAD_ARG;
   if (r->filled == 0) return ORC_BAD_STATE;
   for (int j = 0; j < batch; ++j) {
-    uint32_t ctr[4] = {(uint32_t)(j >> 2), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), TAG_SAMPLE};
-    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
-    uint32_t o[4];
-    philox4x32_10(ctr, key, o);
-    int64_t p = (int64_t)bounded(o[j & 3], (uint32_t)r->filled);
+    int64_t p = sample_index(seed, draw_index, j, r->filled);
     if (indices) indices[j] = p;
     if (obs) memcpy(obs + (size_t)j * kObs, &r->obs[(size_t)p * kObs], kObs * sizeof(uint16_t));
     if (mask) memcpy(mask + (size_t)j * kMaskWords, &r->mask[(size_t)p * kMaskWords], kMaskWords * sizeof(uint32_t));

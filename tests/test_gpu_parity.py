@@ -344,6 +344,96 @@ def test_replay_zero_copy_reserve_commit_equals_push():
 
 
 
+def test_config3_full_size_ring_zero_copy_and_sample():
+    """BASELINE.json configs[3] at full size in the launch sequence bench.py times: 262,144
+    games, 64 x 131,072-record ring (77.6 GB), zero-copy push + 4,096-sample gather per step.
+    The oracle mirrors three 32-game ranges; 34 steps wrap the ring (capacity = 32 blocks)."""
+    c = W.CONFIGS[3]
+    n, bs = c["num_games"], c["sample_batch"]
+    kw = dict(variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~80 GB of free device memory")
+    g = B.Env(n, **kw)
+    ring = B.Replay(c["ring_per_slot"], c["ring_slots"])
+    cap = ring.capacity
+    ranges = [0, 131072 + 64, n - 32]
+    os_ = [orc.Env(32, game_base=lo, **kw) for lo in ranges]
+    act, rew, done = g.new_actions(), g.new_reward(), g.new_done()
+    s_obs = torch.empty((bs, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    s_mask = torch.empty((bs, 113), dtype=torch.int32, device="cuda")
+    s_act = torch.empty(bs, dtype=torch.int16, device="cuda")
+    s_rew = torch.empty(bs, dtype=torch.int8, device="cuda")
+    s_done = torch.empty(bs, dtype=torch.uint8, device="cuda")
+    o_ptr, _ = ring.reserve(n, 0)
+    B._chk(B.lib().strat_encode_obs(g.h, o_ptr, B._stream()), "encode")
+    vo, vm, va, vr, vd = ring.views()
+    steps, expect = 34, {}
+    for t in range(steps):
+        for oo, lo in zip(os_, ranges):
+            oobs = oo.encode_obs(); om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
+            expect[(t, lo)] = (oobs.reshape(32, -1).copy(), om.copy(), oa.copy(), orr.copy(), od.copy())
+        _, m_ptr = ring.reserve(n, 0)
+        o_next, _ = ring.reserve(n, 1)
+        g.rollout_step_raw(m_ptr, act, rew, done, o_next)
+        ring.commit(act, rew, done)
+        ring.sample(c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
+        head, filled = ring.state()
+        assert head == ((t + 1) * n) % cap and filled == min((t + 1) * n, cap)
+        idx = torch.from_numpy(orc.sample_indices(c["seed"], t, bs, filled)).cuda()
+        assert torch.equal(s_act, va[idx]) and torch.equal(s_rew, vr[idx]) and torch.equal(s_done, vd[idx])
+        assert torch.equal(s_mask, vm[idx])
+        assert torch.equal(s_obs.view(torch.int16).view(bs, -1), vo[idx])
+    for t in range(steps - cap // n, steps):  # the blocks still in the ring
+        p0 = (t * n) % cap
+        for lo in ranges:
+            eo, em, ea, er, ed = expect[(t, lo)]
+            s = slice(p0 + lo, p0 + lo + 32)
+            if t > steps - cap // n:  # the oldest block's obs rows already hold obs of the next record
+                assert np.array_equal(_np(vo[s]).view(np.uint16), eo), (t, lo)
+            assert np.array_equal(_np(vm[s]).view(np.uint32), em), (t, lo)
+            assert np.array_equal(_np(va[s]), ea) and np.array_equal(_np(vr[s]), er) and np.array_equal(_np(vd[s]), ed)
+    b = _np(g.get_boards())
+    for oo, lo in zip(os_, ranges):
+        assert np.array_equal(b[lo:lo + 32], oo.get_boards())
+    assert g.check() == 0
+
+
+def test_config4_full_size_determinise_rollout_reduce():
+    """BASELINE.json configs[4] at full size: 16 oracle-made roots x 16,384 determinisations,
+    64-ply on-chip rollouts, per-root reduction.  Determinised boards are compared for all
+    262,144 games; rollouts on three 64-game ranges; the reduction against the oracle's own
+    reduction of the same final boards."""
+    c = W.CONFIGS[4]
+    R, S, plies = c["num_roots"], c["samples_per_root"], c["rollout_plies"]
+    src = orc.Env(R, seed=c["seed"], max_plies=1000, auto_reset=1)
+    rb = W.capture_at_ply(src.get_boards, lambda: src.step(src.sample_uniform(src.legal_mask())), R, c["root_plies"])
+    side = ((rb[:, 116].astype(np.int64) | (rb[:, 117].astype(np.int64) << 8)) & 1).astype(np.uint8)
+    roots_o = orc.Env(R, seed=c["seed"]); roots_o.reset_from(rb)
+    roots_g = B.Env(R, seed=c["seed"]); roots_g.reset_from(_dev(rb))
+    out_o = orc.Env(R * S, seed=c["seed"])
+    out_g = B.Env(R * S, seed=c["seed"], max_plies=0, auto_reset=0)
+    orc.determinise(roots_o, S, 777, out_o)
+    B.determinise(roots_g, S, 777, out_g)
+    det = out_o.get_boards()
+    assert np.array_equal(_np(out_g.get_boards()), det)
+    out_g.rollout_uniform(plies)
+    fin = _np(out_g.get_boards())
+    for lo in (0, 5 * S + 4000, R * S - 64):
+        o = orc.Env(64, seed=c["seed"], game_base=lo)
+        o.reset_from(det[lo:lo + 64])
+        for _ in range(plies):
+            o.step(o.sample_uniform(o.legal_mask()))
+        assert np.array_equal(fin[lo:lo + 64], o.get_boards()), lo
+    out_o.reset_from(fin)
+    assert np.array_equal(_np(B.reduce_returns(out_g, _dev(side), S)), orc.reduce_returns(out_o, side, S))
+    # properties at full size: plies advance by <= 64, only finished games stop early
+    ply = fin[:, 116].astype(int) | (fin[:, 117].astype(int) << 8)
+    donef = (fin[:, 120] & 1) == 1
+    assert (ply[~donef] == c["root_plies"] + plies).all() and (ply[donef] <= c["root_plies"] + plies).all()
+    assert out_g.check() == 0 and roots_g.check() == 0
+
+
 # ----------------------------------------------------------------------------- search-shaped batch (config 4 shape)
 def test_determinise_rollout_reduce_match_oracle():
     R, S, plies = 4, 96, 64
