@@ -184,6 +184,44 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
                         void* stream);
 int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled);
 
+/* ---- board-history ring and historical queries (Table S1 455-480) ---- */
+/* The paper's rollout buffer: instead of storing information states and masks, keep the game
+ * STATES of the last `length` time steps in a circular, preallocated buffer (128 B per game
+ * and step, 72x smaller than a stored transition) and re-materialise any query on demand.
+ * Time step t is the state after t state updates since attach (CurrentStep);
+ * slot t % length holds, for every game: the device line of the state at t, the action
+ * applied at t (GetPlayedActions) and the reward / done byte that action
+ * produced (ComputeRewardP10).  Valid queries: cur-length <= t < cur for
+ * recorded steps, plus t == cur (the attached environment's live state) for the state
+ * queries.  Memory is the caller's (strat_history_bytes), as everywhere else. */
+typedef struct strat_history strat_history;
+size_t strat_history_bytes(int32_t num_games, int32_t length);
+int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, strat_history** out);
+int strat_history_destroy(strat_history* h);
+/* After attach, every strat_step / strat_rollout_step of `env` first records the state it
+ * starts from, then the action, reward and done byte, and advances CurrentStep by one (the
+ * fused step writes them itself: no copy kernel).  h == NULL detaches.  strat_rollout_uniform
+ * refuses to run (STRAT_BAD_STATE) while a history is attached: it keeps the boards on chip
+ * and records nothing.  Resets are not time steps. */
+int strat_history_attach(strat_env* env, strat_history* h);
+int strat_history_current_step(const strat_history* h, int64_t* step);
+/* ComputeLegalActionMask(t) / ComputeInfostateTensor(t) / BoardStrs(t): same outputs as the
+ * live calls produced (or would have produced) at time step t. */
+int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream);
+int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream);
+int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream);
+/* GetPlayedActions(t), reward(t), done(t): NON-OWNING device pointers into the ring, valid
+ * until `length` further steps have been recorded ("non-owning tensor"). */
+int strat_history_transition(const strat_history* h, int64_t t, const int16_t** actions, const int8_t** reward,
+                             const uint8_t** done);
+/* info int32[N][4] = {ActingPlayer(t), GetNumMoves(t), GetNumMovesSinceLastAttack(t),
+ * done | reason<<2 of the state at t (non-zero only for a frozen finished game; reason 1 =
+ * GetFlagCaptured)}. */
+int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* stream);
+/* Travel back: make the state at time step t the live state of `env` (which need not be the
+ * attached one; "efficient capturing of past states", 252-254). */
+int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream);
+
 /* ---- search-shaped batch (BASELINE.json configs[4]) ------------------------------- */
 /* out game G = r*samples_per_root + s: root r with the types of the searcher's opponent's
  * unrevealed pieces re-dealt uniformly over their squares among the arrangements that put no

@@ -22,7 +22,9 @@ EXPORTS = [
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
-    "strat_reduce_returns",
+    "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
+    "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
+    "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
 ]
 
 
@@ -77,6 +79,19 @@ def lib():
         L.strat_replay_state.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.strat_determinise.argtypes = [vp, i32, u64, vp, vp]
         L.strat_reduce_returns.argtypes = [vp, vp, i32, vp, vp]
+        i64 = C.c_int64
+        L.strat_history_bytes.restype = sz
+        L.strat_history_bytes.argtypes = [i32, i32]
+        L.strat_history_create.argtypes = [vp, sz, i32, i32, C.POINTER(vp)]
+        L.strat_history_destroy.argtypes = [vp]
+        L.strat_history_attach.argtypes = [vp, vp]
+        L.strat_history_current_step.argtypes = [vp, C.POINTER(i64)]
+        L.strat_history_legal_mask.argtypes = [vp, i64, vp, vp]
+        L.strat_history_encode_obs.argtypes = [vp, i64, vp, vp]
+        L.strat_history_get_boards.argtypes = [vp, i64, vp, vp]
+        L.strat_history_transition.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+        L.strat_history_info.argtypes = [vp, i64, vp, vp]
+        L.strat_history_restore.argtypes = [vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -278,6 +293,76 @@ class Replay:
         rew = self.mem[o[3]:o[3] + Cn].view(torch.int8)
         done = self.mem[o[4]:o[4] + Cn]
         return obs, mask, act, rew, done
+
+
+class History:
+    """Board-history ring (the paper's rollout buffer) in a caller-owned (torch) buffer."""
+
+    def __init__(self, num_games, length, device=0):
+        _require_cuda()
+        self.device = torch.device("cuda", device)
+        self.n, self.length = num_games, length
+        nbytes = lib().strat_history_bytes(num_games, length)
+        if nbytes == 0:
+            raise StratError("bad history shape")
+        self.mem = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.h = C.c_void_p()
+        self.env = None
+        _chk(lib().strat_history_create(_ptr(self.mem), nbytes, num_games, length, C.byref(self.h)),
+             "strat_history_create")
+
+    def __del__(self):
+        if getattr(self, "h", None) is not None and self.h.value:
+            lib().strat_history_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def attach(self, env):
+        _chk(lib().strat_history_attach(env.h, self.h), "strat_history_attach")
+        self.env = env  # keeps the environment alive as long as the ring refers to it
+
+    def detach(self):
+        if self.env is not None:
+            _chk(lib().strat_history_attach(self.env.h, None), "strat_history_attach")
+            self.env = None
+
+    def current_step(self):
+        s = C.c_int64()
+        _chk(lib().strat_history_current_step(self.h, C.byref(s)), "strat_history_current_step")
+        return s.value
+
+    def legal_mask(self, t, out=None):
+        out = out if out is not None else torch.empty((self.n, MASK_WORDS), dtype=torch.int32, device=self.device)
+        _chk(lib().strat_history_legal_mask(self.h, t, _ptr(out, torch.int32), _stream()), "strat_history_legal_mask")
+        return out
+
+    def encode_obs(self, t, out=None):
+        out = out if out is not None else torch.empty((self.n, 44, 10, 10), dtype=torch.bfloat16, device=self.device)
+        _chk(lib().strat_history_encode_obs(self.h, t, _ptr(out, torch.bfloat16), _stream()), "strat_history_encode_obs")
+        return out
+
+    def get_boards(self, t, out=None):
+        out = out if out is not None else torch.empty((self.n, LINE), dtype=torch.uint8, device=self.device)
+        _chk(lib().strat_history_get_boards(self.h, t, _ptr(out, torch.uint8), _stream()), "strat_history_get_boards")
+        return out
+
+    def transition(self, t):
+        """Non-owning views (actions int16[N], reward int8[N], done uint8[N]) of time step t."""
+        a, r, d = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _chk(lib().strat_history_transition(self.h, t, C.byref(a), C.byref(r), C.byref(d)), "strat_history_transition")
+        base = self.mem.data_ptr()
+
+        def view(p, nbytes, dtype):
+            return self.mem[p.value - base:p.value - base + nbytes].view(dtype)
+
+        return view(a, 2 * self.n, torch.int16), view(r, self.n, torch.int8), view(d, self.n, torch.uint8)
+
+    def info(self, t, out=None):
+        out = out if out is not None else torch.empty((self.n, 4), dtype=torch.int32, device=self.device)
+        _chk(lib().strat_history_info(self.h, t, _ptr(out, torch.int32), _stream()), "strat_history_info")
+        return out
+
+    def restore(self, t, env):
+        _chk(lib().strat_history_restore(self.h, t, env.h, _stream()), "strat_history_restore")
 
 
 def determinise(roots: Env, samples_per_root: int, seed: int, out: Env):

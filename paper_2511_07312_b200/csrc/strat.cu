@@ -109,6 +109,10 @@ __device__ __forceinline__ void expand_obs(uint16_t* __restrict__ obs, int first
 
 __device__ __forceinline__ void raise_error(int* err, int code) { atomicCAS(err, 0, code); }
 
+// One time step of the board-history ring (strat_history): where a state-advancing kernel
+// records the state it starts from and the transition it makes.  lines == nullptr: no history.
+struct HistSlot { uint32_t* lines; int16_t* act; int8_t* rew; uint8_t* done; };
+
 // ------------------------------------------------------------------ kernels
 __global__ void __launch_bounds__(32) k_reset(Params P, uint32_t* __restrict__ lines) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
@@ -267,17 +271,22 @@ __global__ void __launch_bounds__(128) k_sample_uniform(Params P, const uint32_t
 }
 
 __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ lines, const int16_t* __restrict__ actions,
-                                             int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err) {
+                                             int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err,
+                                             HistSlot hs) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, P.num_games - first);
   load_lines(lines, first, ng, s_state, lane);
+  if (hs.lines) store_lines(hs.lines, first, ng, s_state, lane);  // the state this step starts from
+  __syncwarp();
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
-    StepOut o = step_game<true>(P, (uint32_t)(first + lane), g, (int)actions[first + lane]);
+    int a = (int)actions[first + lane];
+    StepOut o = step_game<true>(P, (uint32_t)(first + lane), g, a);
     if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
     reward[first + lane] = (int8_t)o.reward;
     done[first + lane] = (uint8_t)o.done;
+    if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
     write_game(s_state, lane, g);
   }
   __syncwarp();
@@ -398,11 +407,17 @@ __device__ __forceinline__ void expand_obs16(uint16_t* __restrict__ obs, int fir
     }
   }
 }
-__device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ lines, int game, Game& g) {
+__device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ lines, int game, Game& g,
+                                                 uint32_t* __restrict__ hist_lines) {
   uint32_t W[32];
   const uint4* p = reinterpret_cast<const uint4*>(lines + (size_t)game * kLineWords);
 #pragma unroll
   for (int k = 0; k < 8; ++k) { uint4 v = __ldcg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+  if (hist_lines) {  // board-history ring: the state this step starts from
+    uint4* q = reinterpret_cast<uint4*>(hist_lines + (size_t)game * kLineWords);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) __stcg(q + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+  }
   unpack_line(W, g);
 }
 __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, int game, const Game& g) {
@@ -474,7 +489,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
                                                         uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
-                                                        uint32_t* __restrict__ f_obs, uint32_t version) {
+                                                        uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs) {
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
@@ -519,7 +534,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       zero_smem16(work, kMaskBytes, lane);
       Game g;
       int n = 0, cnt[4] = {0, 0, 0, 0};
-      if (lane < ng) load_game_global(lines, first + lane, g);
+      if (lane < ng) load_game_global(lines, first + lane, g, hs.lines);
       __syncwarp();
       PROF_T(t2);
       if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);
@@ -535,6 +550,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         if (actions) actions[first + lane] = (int16_t)a;
         if (reward) reward[first + lane] = (int8_t)o.reward;
         if (done) done[first + lane] = (uint8_t)o.done;
+        if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
         reset_me = o.needs_reset;
       }
       uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
@@ -681,6 +697,17 @@ __global__ void __launch_bounds__(256) k_reduce_returns(const uint32_t* __restri
   }
 }
 
+// Scalar queries of Table S1 from the state lines of one time step.
+__global__ void __launch_bounds__(256) k_line_info(int n, const uint32_t* __restrict__ lines, int32_t* __restrict__ info) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  const uint32_t* L = lines + (size_t)g * kLineWords;
+  uint32_t w28 = L[28], f = L[19] >> 4;
+  uint32_t ply = w28 & 0xFFFFu, done = f & 1u, reason = (f >> 1) & 7u;
+  int4 v = make_int4((int)(ply & 1u), (int)ply, (int)(w28 >> 16), (int)(done | (reason << 2)));
+  reinterpret_cast<int4*>(info)[g] = v;
+}
+
 __global__ void k_set_int(int* p, int v) { *p = v; }
 
 // ------------------------------------------------------------------ host side
@@ -740,7 +767,36 @@ struct strat_env {
   uint32_t* f_obs;       // [batches] ... that finished the batch's observation stores
   uint32_t version;      // fused-step launches so far
   int num_sms;
+  strat_history* hist;   // attached board-history ring, or nullptr
 };
+
+// Circular buffer of `length` time steps: per step N device lines + N x
+// (action i16, reward i8, done u8).
+struct strat_history {
+  int32_t num_games, length;
+  int64_t cur;                 // CurrentStep: state updates recorded so far
+  uint32_t* lines; int16_t* act; int8_t* rew; uint8_t* done;
+  const strat_env* env;        // attached environment (live state = time step cur)
+  strat::Params P;             // its rule parameters, kept for queries after a detach
+};
+
+namespace {
+inline HistSlot hist_slot(strat_history* h) {
+  HistSlot s = {nullptr, nullptr, nullptr, nullptr};
+  if (h) {
+    size_t k = (size_t)(h->cur % h->length), n = (size_t)h->num_games;
+    s.lines = h->lines + k * n * kLineWords; s.act = h->act + k * n; s.rew = h->rew + k * n; s.done = h->done + k * n;
+  }
+  return s;
+}
+// state lines of time step t, or nullptr if t is outside the ring / not the live state
+inline const uint32_t* hist_lines_at(const strat_history* h, int64_t t) {
+  if (!h) return nullptr;
+  if (t == h->cur) return h->env ? h->env->lines : nullptr;
+  if (t < 0 || t >= h->cur || t < h->cur - h->length) return nullptr;
+  return h->lines + (size_t)(t % h->length) * (size_t)h->num_games * kLineWords;
+}
+}  // namespace
 
 struct strat_replay {
   int64_t per_slot, slots, capacity, head, filled;
@@ -781,6 +837,7 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->f_state = e->tickets + kTicketRing;
   e->f_obs = e->f_state + batches(cfg->num_games);
   e->version = 0;
+  e->hist = nullptr;
   if (cudaMemsetAsync(e->tickets, 0, sync_words(cfg->num_games) * 4, (cudaStream_t)stream) != cudaSuccess) {
     delete e;
     return STRAT_CUDA_ERROR;
@@ -791,7 +848,11 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   return strat_reset(e, cfg->seed, stream);
 }
 
-int strat_destroy(strat_env* env) { delete env; return STRAT_OK; }
+int strat_destroy(strat_env* env) {
+  if (env && env->hist) env->hist->env = nullptr;
+  delete env;
+  return STRAT_OK;
+}
 
 int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   if (!env) return STRAT_BAD_ARG;
@@ -832,7 +893,9 @@ int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* ac
 
 int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream) {
   if (!env || !actions || !reward || !done) return STRAT_BAD_ARG;
-  k_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err);
+  k_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err,
+                                                                     hist_slot(env->hist));
+  if (env->hist) env->hist->cur += 1;
   return launch_status();
 }
 
@@ -859,9 +922,11 @@ int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t*
   lc.attrs = at; lc.numAttrs = 1;
   const uint32_t version = env->version + 1;
   if (cudaLaunchKernelEx(&lc, k_rollout_step, env->P, env->lines, mask, actions, reward, done, obs,
-                         env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version) != cudaSuccess)
+                         env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
+                         hist_slot(env->hist)) != cudaSuccess)
     return STRAT_CUDA_ERROR;
   env->version = version;
+  if (env->hist) env->hist->cur += 1;
   return STRAT_OK;
 }
 
@@ -922,6 +987,7 @@ int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_ho
 
 int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream) {
   if (!env || plies < 0) return STRAT_BAD_ARG;
+  if (env->hist) return STRAT_BAD_STATE;  // on-chip plies are not recorded
   k_rollout_uniform<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
   return launch_status();
 }
@@ -1028,6 +1094,98 @@ int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled) {
   if (head) *head = r->head;
   if (filled) *filled = r->filled;
   return STRAT_OK;
+}
+
+// ---- board-history ring (Table S1)
+size_t strat_history_bytes(int32_t num_games, int32_t length) {
+  if (num_games <= 0 || length <= 0) return 0;
+  size_t n = (size_t)num_games, T = (size_t)length;
+  return align_up(T * n * STRAT_LINE_BYTES, 256) + align_up(T * n * 2, 256) + 2 * align_up(T * n, 256);
+}
+
+int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, strat_history** out) {
+  size_t need = strat_history_bytes(num_games, length);
+  if (!mem_dev || !out || need == 0 || bytes < need || ((uintptr_t)mem_dev & 255) != 0) return STRAT_BAD_ARG;
+  strat_history* h = new (std::nothrow) strat_history;
+  if (!h) return STRAT_BAD_ARG;
+  size_t n = (size_t)num_games, T = (size_t)length;
+  uint8_t* b = reinterpret_cast<uint8_t*>(mem_dev);
+  h->num_games = num_games; h->length = length; h->cur = 0; h->env = nullptr;
+  h->lines = reinterpret_cast<uint32_t*>(b); b += align_up(T * n * STRAT_LINE_BYTES, 256);
+  h->act = reinterpret_cast<int16_t*>(b); b += align_up(T * n * 2, 256);
+  h->rew = reinterpret_cast<int8_t*>(b); b += align_up(T * n, 256);
+  h->done = b;
+  *out = h;
+  return STRAT_OK;
+}
+
+int strat_history_destroy(strat_history* h) {
+  if (h && h->env) const_cast<strat_env*>(h->env)->hist = nullptr;
+  delete h;
+  return STRAT_OK;
+}
+
+int strat_history_attach(strat_env* env, strat_history* h) {
+  if (!env) return STRAT_BAD_ARG;
+  if (h && (h->num_games != env->P.num_games || (h->env && h->env != env))) return STRAT_BAD_ARG;
+  if (env->hist && env->hist != h) env->hist->env = nullptr;
+  env->hist = h;
+  if (h) { h->env = env; h->P = env->P; }
+  return STRAT_OK;
+}
+
+int strat_history_current_step(const strat_history* h, int64_t* step) {
+  if (!h || !step) return STRAT_BAD_ARG;
+  *step = h->cur;
+  return STRAT_OK;
+}
+
+int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !mask) return STRAT_BAD_ARG;
+  const Params& P = h->env ? h->env->P : h->P;
+  k_legal_mask<<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
+  return launch_status();
+}
+
+int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !obs) return STRAT_BAD_ARG;
+  const Params& P = h->env ? h->env->P : h->P;
+  k_encode_obs<<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, obs);
+  return launch_status();
+}
+
+int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !boards) return STRAT_BAD_ARG;
+  k_export<<<(h->num_games + 3) / 4, 128, 0, (cudaStream_t)stream>>>(h->num_games, L, boards);
+  return launch_status();
+}
+
+int strat_history_transition(const strat_history* h, int64_t t, const int16_t** actions, const int8_t** reward,
+                             const uint8_t** done) {
+  if (!h || t < 0 || t >= h->cur || t < h->cur - h->length) return STRAT_BAD_ARG;
+  size_t off = (size_t)(t % h->length) * (size_t)h->num_games;
+  if (actions) *actions = h->act + off;
+  if (reward) *reward = h->rew + off;
+  if (done) *done = h->done + off;
+  return STRAT_OK;
+}
+
+int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !info || ((uintptr_t)info & 15) != 0) return STRAT_BAD_ARG;
+  k_line_info<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, L, info);
+  return launch_status();
+}
+
+int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !env || env->P.num_games != h->num_games) return STRAT_BAD_ARG;
+  if (L != env->lines)
+    copy_elems<uint32_t>(L, env->lines, (size_t)h->num_games * kLineWords, (cudaStream_t)stream);
+  return launch_status();
 }
 
 // ---- search-shaped batch
