@@ -361,14 +361,65 @@ def run_cfg4(args):
     print(json.dumps(line))
 
 
+def run_hist(args):
+    """The paper's own buffer design on the headline workload: the fused step
+    records the 128-byte state of every game and step into a 256-step board-history ring
+    (2.2 GB instead of 155 GB of stored transitions), and masks / information states of past
+    steps are re-materialised on demand."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    n, length = CFG["num_games"], 256
+    env = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1)
+    hist = B.History(n, length)
+    hist.attach(env)
+    mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
+    for _ in range(args.warmup):
+        env.rollout_step(mask, act, rew, done, obs)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    e[0].record()
+    for _ in range(args.steps):
+        env.rollout_step(mask, act, rew, done, obs)
+    e[1].record()
+    cur = hist.current_step()
+    q = max(10, min(args.steps, 200))
+    for k in range(q):  # re-materialise mask + information state of a past step
+        t = cur - 1 - (k * 37) % min(length, cur)
+        hist.legal_mask(t, mask)
+        hist.encode_obs(t, obs)
+    e[2].record()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    assert env.check() == 0
+    ms_step, ms_q = e[0].elapsed_time(e[1]) / args.steps, e[1].elapsed_time(e[2]) / q
+    per_game = ALGO_BYTES_PER_GAME_STEP + 128 + 4  # + recorded state line + action/reward/done
+    line = {
+        "metric": METRIC, "value": n / (ms_step / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8", "data": "synthetic",
+        "config": {"workload": CFG["name"] + " + board-history ring", "games_per_gpu": n, "history_steps": length,
+                   "history_bytes": hist.mem.numel(),
+                   "historical_query": "strat_history_legal_mask + strat_history_encode_obs of a past step",
+                   "ms_per_historical_query": ms_q, "historical_game_queries_per_sec": n / (ms_q / 1e3)},
+        "roofline": dict(_peak_line(per_game * n / (ms_step / 1e3) / 1e9), kernel="k_rollout_step (recording)",
+                         algorithmic_bytes_per_game_step=per_game),
+        "gpu_launches": args.steps + 2 * q, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4"],
-                    help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4], 1 GPU")
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist"],
+                    help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
+                         "hist = cfg2 recording into the board-history ring + historical queries; all 1 GPU")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
     args = ap.parse_args()
@@ -378,6 +429,8 @@ def main():
         run_cfg3(args)
     elif args.workload == "cfg4":
         run_cfg4(args)
+    elif args.workload == "hist":
+        run_hist(args)
     else:
         run_b200(args)
 
