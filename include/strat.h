@@ -131,6 +131,14 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream);
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward,
                        uint8_t* done, uint16_t* obs, void* stream);
 
+/* The data-collection loop with an external policy in one pass (PAPER.md:232 ApplyActions, then
+ * the two queries the next policy call needs): applies `actions` (validated
+ * like strat_step), then writes the legal mask and the observation of the NEW state.  Produces
+ * exactly what strat_step, strat_legal_mask, strat_encode_obs produce in that order.
+ * `mask` may be NULL. */
+int strat_step_observe(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, uint32_t* mask,
+                       uint16_t* obs, void* stream);
+
 /* Same, with HOST destination buffers (pinned memory recommended): runs the fused step
  * into `scratch_dev` (>= strat_host_scratch_bytes(cfg) bytes, caller-owned), copies the
  * five outputs to the host pointers on `stream` and synchronises the stream. */
@@ -140,10 +148,9 @@ int strat_rollout_step_host(strat_env* env, void* scratch_dev, uint32_t* mask_ho
                             uint16_t* obs_host, void* stream);
 
 /* The RL-loop shape with a host-side policy (PAPER.md:232 ApplyActions + Table S1 queries):
- * copies int16[N] actions from `actions_host` to the device, applies them (strat_step),
- * computes the next legal mask and observation (strat_legal_mask, strat_encode_obs of the
- * new state) and copies reward, done, mask and obs to the host pointers; synchronises the
- * stream.  `scratch_dev` as for strat_rollout_step_host. */
+ * copies int16[N] actions from `actions_host` to the device, runs strat_step_observe and
+ * copies reward, done, mask and obs to the host pointers; synchronises the stream.
+ * `scratch_dev` as for strat_rollout_step_host. */
 int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_host, int8_t* reward_host,
                     uint8_t* done_host, uint32_t* mask_host, uint16_t* obs_host, void* stream);
 

@@ -18,7 +18,7 @@ OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
     "strat_reset_from", "strat_get_boards", "strat_legal_mask", "strat_sample_uniform", "strat_step",
-    "strat_encode_obs", "strat_rollout_step", "strat_host_scratch_bytes", "strat_rollout_step_host",
+    "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
@@ -60,6 +60,7 @@ def lib():
         L.strat_step.argtypes = [vp, vp, vp, vp, vp]
         L.strat_encode_obs.argtypes = [vp, vp, vp]
         L.strat_rollout_step.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.strat_step_observe.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_host_scratch_bytes.restype = sz
         L.strat_host_scratch_bytes.argtypes = [C.POINTER(strat_config)]
         L.strat_rollout_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
@@ -144,8 +145,9 @@ class Env:
 
     def __del__(self):
         if getattr(self, "h", None) is not None and self.h.value:
-            lib().strat_destroy(self.h)
-            self.h = C.c_void_p()
+            if _lib is not None:  # module globals may be gone at interpreter shutdown
+                _lib.strat_destroy(self.h)
+            self.h = None
 
     # -- allocation helpers (plumbing)
     def new_mask(self):
@@ -203,6 +205,10 @@ class Env:
         _chk(lib().strat_rollout_step(self.h, _ptr(mask), _ptr(actions), _ptr(reward), _ptr(done), _ptr(obs),
                                       _stream()), "strat_rollout_step")
 
+    def step_observe(self, actions, reward, done, mask, obs):
+        _chk(lib().strat_step_observe(self.h, _ptr(actions, torch.int16), _ptr(reward, torch.int8),
+                                      _ptr(done, torch.uint8), _ptr(mask), _ptr(obs), _stream()), "strat_step_observe")
+
     def rollout_step_raw(self, mask_ptr, actions, reward, done, obs_ptr):
         """rollout_step with raw device addresses for mask/obs (e.g. replay_reserve's)."""
         _chk(lib().strat_rollout_step(self.h, C.c_void_p(mask_ptr), _ptr(actions), _ptr(reward), _ptr(done),
@@ -256,8 +262,9 @@ class Replay:
 
     def __del__(self):
         if getattr(self, "h", None) is not None and self.h.value:
-            lib().strat_replay_destroy(self.h)
-            self.h = C.c_void_p()
+            if _lib is not None:  # module globals may be gone at interpreter shutdown
+                _lib.strat_replay_destroy(self.h)
+            self.h = None
 
     def push(self, obs, mask, action, reward, done):
         n = action.numel()
@@ -313,8 +320,9 @@ class History:
 
     def __del__(self):
         if getattr(self, "h", None) is not None and self.h.value:
-            lib().strat_history_destroy(self.h)
-            self.h = C.c_void_p()
+            if _lib is not None:  # module globals may be gone at interpreter shutdown
+                _lib.strat_history_destroy(self.h)
+            self.h = None
 
     def attach(self, env):
         _chk(lib().strat_history_attach(env.h, self.h), "strat_history_attach")

@@ -485,11 +485,18 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   __syncwarp();
 }
 
+// kExternal = false (strat_rollout_step): mask of the state -> uniform legal action -> step ->
+//   observation of the new state; `actions` is an output.
+// kExternal = true (strat_step_observe): `actions` is the caller's input (validated) -> step ->
+//   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
+//   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
+template <bool kExternal>
 __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
                                                         uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
-                                                        uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs) {
+                                                        uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
+                                                        int* __restrict__ err) {
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
@@ -537,26 +544,52 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       if (lane < ng) load_game_global(lines, first + lane, g, hs.lines);
       __syncwarp();
       PROF_T(t2);
-      if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);
-      __syncwarp();
-      PROF_T(t3);
-      if (mask) store_mask(mask, first, ng, work, lane);
-      PROF_T(t4);
       bool reset_me = false;
-      if (lane < ng) {
-        int a = -1;
-        if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
-        StepOut o = step_game<false, true>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
-        if (actions) actions[first + lane] = (int16_t)a;
-        if (reward) reward[first + lane] = (int8_t)o.reward;
-        if (done) done[first + lane] = (uint8_t)o.done;
-        if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
-        reset_me = o.needs_reset;
+      if (!kExternal) {
+        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);
+        __syncwarp();
+        PROF_T(t3);
+        if (mask) store_mask(mask, first, ng, work, lane);
+        PROF_T(t4);
+        if (lane < ng) {
+          int a = -1;
+          if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+          StepOut o = step_game<false, true>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+          if (actions) actions[first + lane] = (int16_t)a;
+          if (reward) reward[first + lane] = (int8_t)o.reward;
+          if (done) done[first + lane] = (uint8_t)o.done;
+          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          reset_me = o.needs_reset;
+        }
+        uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
+        if (rs) coop_setup(P, first, rs, g, work, lane);
+        if (lane < ng) store_game_global(lines, first + lane, g);
+        flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
+        PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4);
+      } else {
+        if (lane < ng) {
+          int a = (int)actions[first + lane];
+          StepOut o = step_game<true, true>(P, (uint32_t)(first + lane), g, a);
+          if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+          reward[first + lane] = (int8_t)o.reward;
+          done[first + lane] = (uint8_t)o.done;
+          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          reset_me = o.needs_reset;
+        }
+        uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
+        if (rs) {  // the cooperative reset borrows the stage: clear its scratch again afterwards
+          coop_setup(P, first, rs, g, work, lane);
+          zero_smem16(work, kMaskBytes, lane);
+          __syncwarp();
+        }
+        if (lane < ng) {
+          store_game_global(lines, first + lane, g);
+          if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);  // of the NEW state
+        }
+        __syncwarp();
+        if (mask) store_mask(mask, first, ng, work, lane);
+        flag_set(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
       }
-      uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
-      if (rs) coop_setup(P, first, rs, g, work, lane);
-      if (lane < ng) store_game_global(lines, first + lane, g);
-      flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
       __syncwarp();  // the stage becomes bit streams
       PROF_T(t5);
       if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
@@ -565,7 +598,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       if (lane == 0) s_batch[stage] = b;
       mbar_arrive(&s_full[stage]);
       TRACE(b, 1, gtime());
-      PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4); PROF_ADD(4, t4, t5);
+      PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(4, t2, t5);
       PROF_ADD(5, t5, t6); PROF_ADD(6, t0, t6); PROF_ADD(7, 0, 1);
     }
   } else {
@@ -803,6 +836,35 @@ struct strat_replay {
   uint16_t* obs; uint32_t* mask; int16_t* action; int8_t* reward; uint8_t* done;
 };
 
+namespace {
+// Launch of the fused step.  Programmatic dependent launch: the launch may become resident while
+// the previous launch in the stream is still running IF that one is also a fused step (the only
+// kernel that executes griddepcontrol.launch_dependents); behind any other kernel the attribute
+// changes nothing.  Ordering against the previous fused step is per batch (f_state / f_obs).
+template <bool kExternal>
+int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done, uint16_t* obs,
+                 void* stream) {
+  const int nb = batches(env->P.num_games);
+  // a launch that follows a policy kernel has the GPU to itself: one more CTA per SM
+  const int per_sm = kExternal ? kWsCtasPerSm + 1 : kWsCtasPerSm;
+  const int grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(64); lc.dynamicSmemBytes = 0; lc.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  const uint32_t version = env->version + 1;
+  if (cudaLaunchKernelEx(&lc, k_rollout_step<kExternal>, env->P, env->lines, mask, actions, reward, done, obs,
+                         env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
+                         hist_slot(env->hist), env->err) != cudaSuccess)
+    return STRAT_CUDA_ERROR;
+  env->version = version;
+  if (env->hist) env->hist->cur += 1;
+  return STRAT_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char* strat_error_string(int code) {
@@ -908,26 +970,13 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done,
                        uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;
-  const int nb = batches(env->P.num_games);
-  const int grid = nb < env->num_sms * kWsCtasPerSm ? nb : env->num_sms * kWsCtasPerSm;
-  // Programmatic dependent launch: this launch may become resident while the previous launch
-  // in the stream is still running IF that one is also a fused step (it is the only kernel
-  // that executes griddepcontrol.launch_dependents); behind any other kernel the attribute
-  // changes nothing.  Ordering against the previous fused step is per batch (f_state/f_obs).
-  cudaLaunchConfig_t lc = {};
-  lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(64); lc.dynamicSmemBytes = 0; lc.stream = (cudaStream_t)stream;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  lc.attrs = at; lc.numAttrs = 1;
-  const uint32_t version = env->version + 1;
-  if (cudaLaunchKernelEx(&lc, k_rollout_step, env->P, env->lines, mask, actions, reward, done, obs,
-                         env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
-                         hist_slot(env->hist)) != cudaSuccess)
-    return STRAT_CUDA_ERROR;
-  env->version = version;
-  if (env->hist) env->hist->cur += 1;
-  return STRAT_OK;
+  return launch_fused<false>(env, mask, actions, reward, done, obs, stream);
+}
+
+int strat_step_observe(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, uint32_t* mask,
+                       uint16_t* obs, void* stream) {
+  if (!env || !actions || !reward || !done || !obs) return STRAT_BAD_ARG;
+  return launch_fused<true>(env, mask, const_cast<int16_t*>(actions), reward, done, obs, stream);
 }
 
 size_t strat_host_scratch_bytes(const strat_config* cfg) {
@@ -973,9 +1022,7 @@ int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_ho
   int8_t* rew = reinterpret_cast<int8_t*>(p); p += align_up(n, 256);
   uint8_t* done = p;
   if (cudaMemcpyAsync(act, actions_host, n * 2, cudaMemcpyHostToDevice, s) != cudaSuccess) return STRAT_CUDA_ERROR;
-  int rc = strat_step(env, act, rew, done, stream);
-  if (rc == STRAT_OK) rc = strat_legal_mask(env, mask, stream);
-  if (rc == STRAT_OK) rc = strat_encode_obs(env, obs, stream);
+  int rc = strat_step_observe(env, act, rew, done, mask, obs, stream);
   if (rc != STRAT_OK) return rc;
   bool ok = cudaMemcpyAsync(reward_host, rew, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
   ok = ok && cudaMemcpyAsync(done_host, done, n, cudaMemcpyDeviceToHost, s) == cudaSuccess;

@@ -198,6 +198,37 @@ def test_fused_steps_back_to_back_overlap_equals_synchronised_run():
     assert g1.check() == 0 and g2.check() == 0
 
 
+@pytest.mark.parametrize("variant,n,cap", [(0, 1000, 70), (1, 333, 2000)])
+def test_step_observe_equals_step_mask_encode_and_oracle(variant, n, cap):
+    """strat_step_observe (external actions -> step -> mask + obs of the new state, one kernel)
+    against the oracle's step / legal_mask / encode_obs, with auto-reset and a ragged tail."""
+    kw = dict(variant=variant, seed=9, max_plies=cap, auto_reset=1)
+    g, o = _pair(n, **kw)
+    mask, rew, done, obs = g.new_mask(), g.new_reward(), g.new_done(), g.new_obs()
+    om = o.legal_mask()
+    for t in range(200):
+        oa = o.sample_uniform(om)
+        orr, od = o.step(oa)
+        om = o.legal_mask()
+        g.step_observe(_dev(oa), rew, done, mask, obs)
+        assert np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od), t
+        assert np.array_equal(_mask_np(mask), om), t
+        if t % 9 == 0 or t == 199:
+            assert np.array_equal(_obs_np(obs), o.encode_obs().reshape(n, 44, 10, 10)), t
+            assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+    assert g.check() == 0
+    # an illegal action: sticky error, that game unchanged, the others advance
+    oa = o.sample_uniform(om)
+    bad = oa.copy(); bad[3] = 3599
+    before = _np(g.get_boards())[3].copy()
+    g.step_observe(_dev(bad), rew, done, None, obs)
+    assert g.check() == B.ILLEGAL_ACTION
+    after = _np(g.get_boards())
+    assert np.array_equal(after[3], before)
+    o.step(bad)
+    assert np.array_equal(after, o.get_boards())
+
+
 def test_fused_step_interleaved_with_other_calls():
     """A fused step after any other state-changing call (and vice versa) sees that call's result."""
     kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)
