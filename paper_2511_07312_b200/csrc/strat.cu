@@ -623,22 +623,21 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
   }
 }
 
-// `plies` plies of uniform-random legal play with the board in registers.
+// `plies` plies of uniform-random legal play with the board in registers.  The 3600-bit mask is
+// never built: the r-th legal action is found from the move bitboards (sample_action_direct).
+constexpr int kScoutScratch = 9;  // 8 words per game, odd stride
 __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
-  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
+  __shared__ uint32_t s_scouts[kBatch * kScoutScratch];
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, P.num_games - first);
   load_lines(lines, first, ng, s_state, lane);
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
-    uint32_t* row = s_mask + lane * kMaskWords;
     for (int t = 0; t < plies; ++t) {
       if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
-      for (int w = 0; w < kMaskWords; ++w) row[w] = 0;
-      int cnt[4];
-      int n = legal_mask_row(g, g.ply & 1u, P.two_square, row, cnt);
-      int a = pick_action(row, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+      int a = sample_action_direct(g, g.ply & 1u, P.two_square, action_draw(P, (uint32_t)(first + lane), g),
+                                   s_scouts + lane * kScoutScratch);
       step_game<false>(P, (uint32_t)(first + lane), g, a);
     }
     write_game(s_state, lane, g);

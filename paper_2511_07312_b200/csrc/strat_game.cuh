@@ -393,6 +393,62 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
   }
   return -1;
 }
+// SampleRandomLegalAction without materialising the 3600-bit mask (on-chip rollouts): equal to
+// pick_action(legal_mask_row(...)) for the same draw u.  Actions ascend with the from-cell, then
+// the direction, then the distance, so the r-th legal action is found by walking the pieces that
+// can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
+// lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
+SD int sample_action_direct(const Game& g, int side, int two_square, uint32_t u, uint32_t* scouts) {
+  Moves m; single_step_moves(g, side, two_square, m);
+  uint32_t D[4][4];
+  int cnt[4], ns = 0;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    uint32_t sc = m.scouts.w[i];
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d) D[i][d] = m.d[d].w[i] & ~sc;
+    cnt[i] = sd_popc(D[i][0]) + sd_popc(D[i][1]) + sd_popc(D[i][2]) + sd_popc(D[i][3]);
+    uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
+    while (ss) {
+      int b = sd_ffs(ss) - 1;
+      ss &= ss - 1;
+      int c = 32 * i + b, r = c / 10, q = c - 10 * r;
+      int len[4];
+      scout_rays(m, c, r, q, len);
+      cnt[i] += len[0] + len[1] + len[2] + len[3];
+      if (ns < 8) scouts[ns++] = (uint32_t)c | ((uint32_t)len[0] << 8) | ((uint32_t)len[1] << 12) |
+                                ((uint32_t)len[2] << 16) | ((uint32_t)len[3] << 20);
+    }
+  }
+  int n = cnt[0] + cnt[1] + cnt[2] + cnt[3];
+  if (n == 0) return -1;
+  int r = (int)bounded(u, (uint32_t)n);
+  int gi = 0;
+  if (r >= cnt[0]) { r -= cnt[0]; gi = 1; if (r >= cnt[1]) { r -= cnt[1]; gi = 2; if (r >= cnt[2]) { r -= cnt[2]; gi = 3; } } }
+  uint32_t d0 = gi == 0 ? D[0][0] : gi == 1 ? D[1][0] : gi == 2 ? D[2][0] : D[3][0];
+  uint32_t d1 = gi == 0 ? D[0][1] : gi == 1 ? D[1][1] : gi == 2 ? D[2][1] : D[3][1];
+  uint32_t d2 = gi == 0 ? D[0][2] : gi == 1 ? D[1][2] : gi == 2 ? D[2][2] : D[3][2];
+  uint32_t d3 = gi == 0 ? D[0][3] : gi == 1 ? D[1][3] : gi == 2 ? D[2][3] : D[3][3];
+  uint32_t any = d0 | d1 | d2 | d3;
+  int k = 0;
+  while (k < ns && (int)((scouts[k] & 127u) >> 5) < gi) ++k;  // first Scout of this 32-cell group
+  for (;;) {
+    int bn = any ? sd_ffs(any) - 1 : 32;
+    uint32_t e = k < ns ? scouts[k] : 0xFFu;
+    int bs = ((int)((e & 127u) >> 5) == gi && k < ns) ? (int)(e & 31u) : 32;
+    int b, l0, l1, l2, l3;
+    if (bs < bn) { b = bs; l0 = (e >> 8) & 15; l1 = (e >> 12) & 15; l2 = (e >> 16) & 15; l3 = (e >> 20) & 15; ++k; }
+    else { b = bn; l0 = (d0 >> b) & 1; l1 = (d1 >> b) & 1; l2 = (d2 >> b) & 1; l3 = (d3 >> b) & 1; any &= any - 1; }
+    if (b >= 32) return -1;  // unreachable: r < cnt[gi]
+    int c = l0 + l1 + l2 + l3;
+    if (r < c) {
+      int dir = 0;
+      if (r >= l0) { r -= l0; dir = 1; if (r >= l1) { r -= l1; dir = 2; if (r >= l2) { r -= l2; dir = 3; } } }
+      return (32 * gi + b) * 36 + dir * 9 + r;
+    }
+    r -= c;
+  }
+}
 SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
   uint32_t o[4];
   philox(P.game_base + local_game, g.epoch, g.ply, TAG_ACTION, P.key0, P.key1, o);
