@@ -106,6 +106,14 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream);
 int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
 int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);
 
+/* "Pin" the simulation (Reset Behaviour and Support for Search): while a pin
+ * is set, a game that terminates (auto_reset = 1) restarts from ITS pinned state instead of a
+ * fresh setup; only the slot's epoch counter keeps counting up, so every restart plays a new
+ * action stream.  boards: canonical uint8[N][128] (device); pin_lines_dev: N*128 bytes of
+ * caller-owned device memory (16-B aligned) that the library fills and keeps reading until
+ * the pin is removed (boards == NULL).  The current state of the games is not touched. */
+int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* boards, void* stream);
+
 /* ComputeLegalActionMask for the acting player (rules PAPER.md:210-212).
  * mask: uint32[N][113].  Finished games get an all-zero mask. */
 int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream);

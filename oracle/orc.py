@@ -44,6 +44,7 @@ def lib():
         L.orc_reset.argtypes = [vp, C.c_uint64]
         L.orc_reset_from.argtypes = [vp, vp]
         L.orc_get_boards.argtypes = [vp, vp]
+        L.orc_pin_reset_state.argtypes = [vp, vp]
         L.orc_legal_mask.argtypes = [vp, vp]
         L.orc_sample_uniform.argtypes = [vp, vp, vp]
         L.orc_step.argtypes = [vp, vp, vp, vp]
@@ -104,6 +105,15 @@ class Env:
         b = np.ascontiguousarray(boards, dtype=np.uint8)
         assert b.shape == (self.n, LINE)
         _chk(lib().orc_reset_from(self.h, _p(b)), "reset_from")
+
+    def pin_reset_state(self, boards):
+        """boards uint8[N][128], or None to unpin."""
+        if boards is None:
+            _chk(lib().orc_pin_reset_state(self.h, None), "pin_reset_state")
+            return
+        b = np.ascontiguousarray(boards, dtype=np.uint8)
+        assert b.shape == (self.n, LINE)
+        _chk(lib().orc_pin_reset_state(self.h, _p(b)), "pin_reset_state")
 
     def get_boards(self):
         b = np.zeros((self.n, LINE), np.uint8)

@@ -101,6 +101,9 @@ struct Env {
   Config cfg;
   std::vector<Game> g;
   int error;
+  // "Reset Behaviour and Support for Search": terminated boards restart from a
+  // custom non-initial state instead of a fresh setup.  Empty = not pinned.
+  std::vector<uint8_t> pin;
 };
 
 // ---------------------------------------------------------------- geometry
@@ -309,6 +312,8 @@ int effective_ply_cap(const Config& cfg) {
   return (cfg.max_plies >= 1 && cfg.max_plies <= 65535) ? cfg.max_plies : 65535;
 }
 
+void read_line(const uint8_t* L, Game& gm);  // canonical line -> game (defined below)
+
 void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
   Game& gm = e->g[gi];
   const Config& cfg = e->cfg;
@@ -383,8 +388,14 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
   *reward = gm.done ? (int8_t)gm.result : 0;
   *done_out = (uint8_t)((gm.done ? 1 : 0) | (side << 1) | ((gm.done ? gm.reason : 0) << 2));
   if (gm.done && cfg.auto_reset) {  // R#16
-    gm.epoch += 1;
-    new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm);
+    uint32_t epoch = gm.epoch + 1;
+    if (!e->pin.empty()) {  // R#27: the pinned line with the slot's own epoch counter
+      read_line(&e->pin[(size_t)gi * kLine], gm);
+      gm.epoch = epoch;
+    } else {
+      gm.epoch = epoch;
+      new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm);
+    }
   }
 }
 
@@ -514,6 +525,14 @@ int orc_reset(Env* e, uint64_t seed) {
 int orc_reset_from(Env* e, const uint8_t* boards) {
   if (!e || !boards) return ORC_BAD_ARG;
   for (int i = 0; i < e->cfg.num_games; ++i) read_line(boards + (size_t)i * kLine, e->g[i]);
+  return ORC_OK;
+}
+
+// boards == nullptr unpins.
+int orc_pin_reset_state(Env* e, const uint8_t* boards) {
+  if (!e) return ORC_BAD_ARG;
+  if (boards) e->pin.assign(boards, boards + (size_t)e->cfg.num_games * kLine);
+  else e->pin.clear();
   return ORC_OK;
 }
 

@@ -17,7 +17,7 @@ OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
-    "strat_reset_from", "strat_get_boards", "strat_legal_mask", "strat_sample_uniform", "strat_step",
+    "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_legal_mask", "strat_sample_uniform", "strat_step",
     "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
@@ -55,6 +55,7 @@ def lib():
         L.strat_reset.argtypes = [vp, u64, vp]
         L.strat_reset_from.argtypes = [vp, vp, vp]
         L.strat_get_boards.argtypes = [vp, vp, vp]
+        L.strat_pin_reset_state.argtypes = [vp, vp, vp, vp]
         L.strat_legal_mask.argtypes = [vp, vp, vp]
         L.strat_sample_uniform.argtypes = [vp, vp, vp, vp]
         L.strat_step.argtypes = [vp, vp, vp, vp, vp]
@@ -172,6 +173,17 @@ class Env:
     def reset_from(self, boards):
         assert boards.shape == (self.n, LINE)
         _chk(lib().strat_reset_from(self.h, _ptr(boards, torch.uint8), _stream()), "strat_reset_from")
+
+    def pin_reset_state(self, boards):
+        """boards uint8[N][128] on the device, or None to unpin."""
+        if boards is None:
+            _chk(lib().strat_pin_reset_state(self.h, None, None, _stream()), "strat_pin_reset_state")
+            self._pin = None
+            return
+        assert boards.shape == (self.n, LINE)
+        pin = torch.empty((self.n, LINE), dtype=torch.uint8, device=self.device)
+        _chk(lib().strat_pin_reset_state(self.h, _ptr(pin), _ptr(boards, torch.uint8), _stream()), "strat_pin_reset_state")
+        self._pin = pin  # the library reads it until unpinned
 
     def get_boards(self, out=None):
         out = out if out is not None else torch.empty((self.n, LINE), dtype=torch.uint8, device=self.device)

@@ -562,7 +562,8 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
-        if (rs) coop_setup(P, first, rs, g, work, lane);
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        else if (rs) coop_setup(P, first, rs, g, work, lane);
         if (lane < ng) store_game_global(lines, first + lane, g);
         flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
         PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4);
@@ -577,7 +578,8 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
-        if (rs) {  // the cooperative reset borrows the stage: clear its scratch again afterwards
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        else if (rs) {  // the cooperative reset borrows the stage: clear its scratch again afterwards
           coop_setup(P, first, rs, g, work, lane);
           zero_smem16(work, kMaskBytes, lane);
           __syncwarp();
@@ -755,6 +757,7 @@ inline Params make_params(const strat_config& c) {
   P.num_games = c.num_games; P.variant = c.variant;
   P.ply_cap = (c.max_plies >= 1 && c.max_plies <= 65535) ? c.max_plies : 65535;
   P.max_battleless = c.max_battleless; P.auto_reset = c.auto_reset ? 1 : 0; P.two_square = c.two_square ? 1 : 0;
+  P.pin = nullptr;
   return P;
 }
 inline int launch_status() { return cudaGetLastError() == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR; }
@@ -919,7 +922,9 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   if (!env) return STRAT_BAD_ARG;
   cudaStream_t s = (cudaStream_t)stream;
   env->cfg.seed = seed;
+  const uint32_t* pin = env->P.pin;
   env->P = make_params(env->cfg);
+  env->P.pin = pin;
   k_set_int<<<1, 1, 0, s>>>(env->err, 0);
   k_reset<<<batches(env->P.num_games), 32, 0, s>>>(env->P, env->lines);
   return launch_status();
@@ -929,6 +934,16 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   if (!env || !boards) return STRAT_BAD_ARG;
   int n = env->P.num_games;
   k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  return launch_status();
+}
+
+int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* boards, void* stream) {
+  if (!env) return STRAT_BAD_ARG;
+  if (!boards) { env->P.pin = nullptr; return STRAT_OK; }
+  if (!pin_lines_dev || ((uintptr_t)pin_lines_dev & 15) != 0) return STRAT_BAD_ARG;
+  int n = env->P.num_games;
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, reinterpret_cast<uint32_t*>(pin_lines_dev));
+  env->P.pin = reinterpret_cast<const uint32_t*>(pin_lines_dev);
   return launch_status();
 }
 

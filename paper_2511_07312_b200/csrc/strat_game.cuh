@@ -54,6 +54,7 @@ struct Params {  // per-environment constants handed to every kernel by value
   int32_t max_battleless;  // 0 = off
   int32_t auto_reset;
   int32_t two_square;
+  const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
 };
 
 // ------------------------------------------------------------------ 100-bit boards
@@ -533,6 +534,20 @@ SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
   }
 }
 
+// Auto-reset of a finished game whose epoch has already been advanced: a fresh setup, or the
+// game's pinned line with the slot's own epoch (R#27).
+SD void reset_game(const Params& P, uint32_t local_game, Game& g) {
+  if (P.pin) {
+    uint32_t W[32], epoch = g.epoch;
+    STRAT_UNROLL
+    for (int k = 0; k < 32; ++k) W[k] = P.pin[(size_t)local_game * kLineWords + k];
+    unpack_line(W, g);
+    g.epoch = epoch;
+  } else {
+    setup_game(P, local_game, g);
+  }
+}
+
 // ------------------------------------------------------------------ step (C4)
 // +1 attacker wins, -1 attacker loses, 0 both removed (Ext. Data Fig. 3b)
 SD int battle(int att, int def) {
@@ -546,7 +561,7 @@ struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; };
 
 // kValidate = false only when `a` was just drawn from this state's own legal mask.
 // kDeferReset: the caller performs the auto-reset itself (epoch is already advanced) when
-// o.needs_reset is set; the result must equal setup_game(P, local_game, g).
+// o.needs_reset is set; the result must equal reset_game(P, local_game, g).
 template <bool kValidate, bool kDeferReset = false>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   StepOut o; o.illegal = false; o.needs_reset = false;
@@ -601,7 +616,7 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   o.done = g.done | ((uint32_t)side << 1) | ((g.done ? g.reason : 0u) << 2);
   if (g.done && P.auto_reset) {  // R#16
     g.epoch += 1;
-    if (kDeferReset) o.needs_reset = true; else setup_game(P, local_game, g);
+    if (kDeferReset) o.needs_reset = true; else reset_game(P, local_game, g);
   }
   return o;
 }

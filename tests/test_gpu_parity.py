@@ -229,6 +229,49 @@ def test_step_observe_equals_step_mask_encode_and_oracle(variant, n, cap):
     assert np.array_equal(after, o.get_boards())
 
 
+def test_pinned_reset_state_matches_oracle():
+    """Reset Behaviour and Support for Search: finished games restart from
+    their pinned non-initial state, in every state-advancing kernel; unpinning brings fresh
+    setups back."""
+    kw = dict(variant=0, seed=13, max_plies=55, auto_reset=1)
+    n = 500
+    g, o = _pair(n, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for _ in range(30):
+        g.rollout_step(mask, act, rew, done, obs)
+        o.step(o.sample_uniform(o.legal_mask()))
+    pin = o.get_boards()
+    assert np.array_equal(_np(g.get_boards()), pin)
+    g.pin_reset_state(_dev(pin)); o.pin_reset_state(pin)
+    for t in range(90):  # every game hits the 55-ply cap at least three times
+        oa = o.sample_uniform(o.legal_mask()); orr, od = o.step(oa)
+        if t % 3 == 0:
+            g.rollout_step(mask, act, rew, done, obs)
+            assert np.array_equal(_np(act), oa), t
+        elif t % 3 == 1:
+            g.step(_dev(oa), rew, done)
+        else:
+            g.step_observe(_dev(oa), rew, done, mask, obs)
+        assert np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od), t
+    b = o.get_boards()
+    assert np.array_equal(_np(g.get_boards()), b)
+    ply = b[:, 116].astype(int) | (b[:, 117].astype(int) << 8)
+    pin_ply = pin[:, 116].astype(int) | (pin[:, 117].astype(int) << 8)
+    assert (ply >= pin_ply).all() and (b[:, 124] >= 2).all()  # restarted from the pin, epochs count up
+    g.rollout_uniform(40)
+    for _ in range(40):
+        o.step(o.sample_uniform(o.legal_mask()))
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    g.pin_reset_state(None); o.pin_reset_state(None)
+    for _ in range(40):
+        g.rollout_step(mask, act, rew, done, obs)
+        o.step(o.sample_uniform(o.legal_mask()))
+    b = o.get_boards()
+    assert np.array_equal(_np(g.get_boards()), b)
+    assert ((b[:, 116].astype(int) | (b[:, 117].astype(int) << 8)) < 30).any()  # fresh games again
+    assert g.check() == 0
+
+
 def test_fused_step_interleaved_with_other_calls():
     """A fused step after any other state-changing call (and vice versa) sees that call's result."""
     kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)

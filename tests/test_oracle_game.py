@@ -453,3 +453,30 @@ def test_determinise_is_uniform_over_consistent_arrangements():
     chi2 = sum((v - exp) ** 2 / exp for v in keys.values())
     assert chi2 < 40.0, chi2  # 11 dof
     assert draws.min() >= 3 and draws.max() < 60
+
+
+def test_pinned_reset_restarts_from_the_pinned_state():
+    """terminated boards restart from a custom non-initial state.  Pin: the restarted
+    game IS the pinned line (cells, history, counters), only the epoch keeps counting."""
+    o = orc.Env(40, seed=2, max_plies=26, auto_reset=1)
+    for _ in range(12):
+        o.step(o.sample_uniform(o.legal_mask()))
+    pin = o.get_boards()
+    o.pin_reset_state(pin)
+    seen = 0
+    for t in range(40):
+        r, d = o.step(o.sample_uniform(o.legal_mask()))
+        b = o.get_boards()
+        for i in np.nonzero(d & 1)[0]:
+            expect = pin[i].copy()
+            expect[124:128] = b[i, 124:128]          # epoch of the slot
+            assert np.array_equal(b[i], expect)
+            assert int(b[i, 124]) >= 1
+            seen += 1
+    assert seen >= 80  # 14 plies per round: every game restarted at least twice
+    o.pin_reset_state(None)
+    for t in range(20):
+        r, d = o.step(o.sample_uniform(o.legal_mask()))
+        b = o.get_boards()
+        for i in np.nonzero(d & 1)[0]:
+            assert b[i, 116] == 0 and b[i, 117] == 0  # a fresh setup again
