@@ -27,6 +27,9 @@
 //   replay ring        pinned: FIFO content, chi-square of indices.
 //   determinise        pinned: multiset/constraint/obs-equality properties, chi-square of
 //                      Bomb/Flag placement over the unmoved squares.
+//   pinned reset (R#27) pinned: a restarted game equals its pinned line byte for byte except
+//                      the epoch; the reading itself (epoch keeps counting) is PARITY UNPINNED
+//                      against the paper (P:252-254 gives no detail).
 //
 // Layouts:
 //   canonical line, 128 B per game:
