@@ -26,7 +26,7 @@ class Config(C.Structure):
         ("auto_reset", C.c_int32),
         ("two_square", C.c_int32),
         ("device", C.c_int32),
-        ("reserved", C.c_int32),
+        ("chase_rule", C.c_int32),
         ("game_base", C.c_uint64),
     ]
 
@@ -86,9 +86,9 @@ def _chk(rc, what):
 
 class Env:
     def __init__(self, num_games, variant=0, seed=0, max_plies=0, max_battleless=0,
-                 auto_reset=0, two_square=1, game_base=0):
+                 auto_reset=0, two_square=1, game_base=0, chase_rule=0):
         self.cfg = Config(num_games, variant, seed, max_plies, max_battleless, auto_reset,
-                          two_square, 0, 0, game_base)
+                          two_square, 0, chase_rule, game_base)
         self.n = num_games
         self.h = C.c_void_p()
         _chk(lib().orc_create(C.byref(self.cfg), C.byref(self.h)), "create")

@@ -41,6 +41,7 @@
 //     116..117 ply (LE u16)   118..119 battleless count (LE u16)
 //     120 flags: bit0 done, bits2-4 reason (1 flag,2 no-move win,3 no-move draw,
 //             4 ply cap,5 battleless)    121 result (int8, red's)
+//     122..123 chase age of red / blue (R#28; 0 unless chase_rule is on)
 //     122..123 zero           124..127 epoch (LE u32)
 //   cell c = 10*row + col; red home rows 0-3, blue home rows 6-9;
 //   lakes {42,43,52,53,46,47,56,57} (BJ configs[0]: c5-d6, g5-h6).
@@ -81,7 +82,7 @@ struct Config {  // mirrors the field order of the product's strat_config on pur
   int32_t auto_reset;
   int32_t two_square;
   int32_t device;  // unused here
-  int32_t reserved;
+  int32_t chase_rule;      // 1: apply the continuous-chasing rule (R#28)
   uint64_t game_base;  // global index of game 0 (RNG keying under sharding)
 };
 
@@ -98,6 +99,9 @@ struct Game {
   // by the last-acting piece for each player".
   int chain_len[2];
   int chain[2][4];
+  // Continuous-chasing state machine (R#28): number of positions of the player's
+  // running chase, counted from the one right after its first threat; 0 = not chasing.
+  int chase_age[2];
 };
 
 struct Env {
@@ -213,6 +217,7 @@ void clear_dynamic(Game& gm) {
   memset(gm.hist, 0xFF, sizeof gm.hist);
   gm.ply = 0; gm.battleless = 0; gm.done = false; gm.reason = 0; gm.result = 0;
   gm.chain_len[0] = gm.chain_len[1] = 0;
+  gm.chase_age[0] = gm.chase_age[1] = 0;
 }
 
 void new_game(const Config& cfg, uint32_t gidx, Game& gm) {  // epoch already set
@@ -257,6 +262,59 @@ bool two_square_banned(const Game& gm, int side, int from, int to) {
   return false;
 }
 
+// ---- continuous-chasing rule (reading R#28)
+bool adjacent(int a, int b) {
+  int dr = a / 10 - b / 10, dc = a % 10 - b % 10;
+  return (dr == 0 && (dc == 1 || dc == -1)) || (dc == 0 && (dr == 1 || dr == -1));
+}
+// "a threat [is] an action that moves a piece adjacent to a piece of the opponent";
+// a move onto an opponent's piece is a battle, not a threat.
+bool is_threat(const Game& gm, int side, int from, int to) {
+  if (gm.cell[to] != 0) return false;
+  for (int d = 0; d < 4; ++d) {
+    int rr = to / 10 + DROW[d], qq = to % 10 + DCOL[d];
+    if (rr < 0 || rr > 9 || qq < 0 || qq > 9) continue;
+    int c = rr * 10 + qq;
+    if (c == from) continue;  // the square the piece leaves
+    if (is_piece(gm.cell[c]) && owner_of(gm.cell[c]) != side) return true;
+  }
+  return false;
+}
+// "An evade is an action that moves a piece that was threatened on the previous turn away
+// from the piece that threatened it", "to an empty square".  The opponent's
+// chase_age > 0 says its previous ply was a threat; the threatening piece stands on that
+// ply's destination square.
+bool is_evade(const Game& gm, int side, int from, int to) {
+  if (gm.chase_age[side ^ 1] == 0 || gm.hist[0][0] == 0xFF) return false;
+  if (gm.cell[to] != 0) return false;
+  int x = gm.hist[0][1];
+  return adjacent(from, x) && !adjacent(to, x);
+}
+// "a player who is chasing may not make a threat that would result in a position that has
+// already taken place during the chase, unless that threat would return the moved piece to the
+// square it occupied prior to the previous turn of the chasing player".  A position is
+// the type and owner of the piece on every square.  The chase's earlier positions are rebuilt
+// by taking back the logged plies one by one (no battle happens inside a chase); the state
+// remembers 8 plies (R#28).
+bool chase_banned(const Game& gm, int side, int from, int to) {
+  int age = gm.chase_age[side];
+  if (age < 2) return false;
+  if (!is_threat(gm, side, from, to)) return false;
+  int first = ((gm.ply & 1) == side) ? 1 : 0;  // history entry of this player's previous ply
+  if (gm.hist[first][0] != 0xFF && from == gm.hist[first][1] && to == gm.hist[first][0]) return false;
+  uint8_t R[kCells], K[kCells];
+  for (int c = 0; c < kCells; ++c) R[c] = K[c] = (uint8_t)(gm.cell[c] & 0x1F);
+  R[to] = R[from]; R[from] = 0;
+  int back = age - 1 < 8 ? age - 1 : 8;
+  for (int b = 1; b <= back; ++b) {
+    if (gm.hist[b - 1][0] == 0xFF) break;
+    int f = gm.hist[b - 1][0], g = gm.hist[b - 1][1];
+    K[f] = K[g]; K[g] = 0;  // take the ply back
+    if (memcmp(R, K, kCells) == 0) return true;
+  }
+  return false;
+}
+
 // Is (from,dir,dist) a legal move for `side` on this board?  P:210: movable pieces
 // move one square in a cardinal direction onto an empty square or an opponent's
 // piece; Scouts any number of squares "so long as the movement does not jump over a
@@ -281,6 +339,7 @@ bool move_is_legal(const Game& gm, const Config& cfg, int side, int from, int di
   }
   int to = (r + DROW[dir] * dist) * 10 + (q + DCOL[dir] * dist);
   if (cfg.two_square && two_square_banned(gm, side, from, to)) return false;
+  if (cfg.chase_rule && chase_banned(gm, side, from, to)) return false;
   return true;
 }
 
@@ -338,6 +397,19 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
     return;
   }
   int to = (from / 10 + DROW[dir] * dist) * 10 + (from % 10 + DCOL[dir] * dist);
+  // 0. chase state machine (R#28), judged on the position before the move.
+  if (cfg.chase_rule) {
+    bool fight = gm.cell[to] != 0;
+    bool threat = is_threat(gm, side, from, to), evade = is_evade(gm, side, from, to);
+    int q = side ^ 1;
+    if (fight) {
+      gm.chase_age[0] = gm.chase_age[1] = 0;
+    } else {
+      if (gm.chase_age[q] > 0) gm.chase_age[q] = evade ? (gm.chase_age[q] < 255 ? gm.chase_age[q] + 1 : 255) : 0;
+      if (threat) gm.chase_age[side] = gm.chase_age[side] > 0 ? (gm.chase_age[side] < 255 ? gm.chase_age[side] + 1 : 255) : 1;
+      else gm.chase_age[side] = 0;
+    }
+  }
   // 1. two-square chain of the mover.
   if (gm.chain_len[side] > 0 && gm.chain[side][gm.chain_len[side] - 1] == from) {
     if (gm.chain_len[side] == 4) {
@@ -411,6 +483,7 @@ void write_line(const Game& gm, uint8_t* L) {
   L[118] = (uint8_t)(gm.battleless & 255); L[119] = (uint8_t)(gm.battleless >> 8);
   L[120] = (uint8_t)((gm.done ? 1 : 0) | (gm.reason << 2));
   L[121] = (uint8_t)(int8_t)gm.result;
+  L[122] = (uint8_t)gm.chase_age[0]; L[123] = (uint8_t)gm.chase_age[1];
   L[124] = (uint8_t)gm.epoch; L[125] = (uint8_t)(gm.epoch >> 8);
   L[126] = (uint8_t)(gm.epoch >> 16); L[127] = (uint8_t)(gm.epoch >> 24);
 }
@@ -453,6 +526,7 @@ void read_line(const uint8_t* L, Game& gm) {
   gm.done = (L[120] & 1) != 0;
   gm.reason = (L[120] >> 2) & 7;
   gm.result = (int8_t)L[121];
+  gm.chase_age[0] = L[122]; gm.chase_age[1] = L[123];
   gm.epoch = (uint32_t)L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
   rebuild_chains(gm);
 }
