@@ -30,7 +30,10 @@
  *     116..117 ply (LE u16)      118..119 plies since the last battle (LE u16)
  *     120      bit0 done, bits2-4 reason (1 Flag captured, 2 opponent has no move,
  *              3 neither has a move (draw), 4 ply cap (draw), 5 battleless cap (draw))
- *     121      result for red (int8: +1, -1, 0)     122..123 zero
+ *     121      result for red (int8: +1, -1, 0)
+ *     122..123 chase age of red / blue: positions of the player's running chase, counted
+ *              from the one right after its first threat (0 = not chasing; always 0 unless
+ *              chase_rule is on; R28)
  *     124..127 epoch (LE u32): number of auto-resets of this game slot
  *   action  a = from*36 + dir*9 + (dist-1); dir 0:+row 1:+col 2:-row 3:-col; dist 1..9
  *   mask    uint32[N][113]; bit a -> word a>>5, bit a&31; bits 3600..3615 are zero
@@ -77,7 +80,9 @@ typedef struct strat_config {
   int32_t auto_reset;     /* 1: a finished game restarts inside the same step */
   int32_t two_square;     /* 1: apply the two-square rule */
   int32_t device;         /* CUDA device ordinal */
-  int32_t reserved;       /* must be 0 */
+  int32_t chase_rule;     /* 1: apply the continuous-chasing rule (R28: a
+                             chasing player may not make a threat that recreates a position of
+                             the chase's last 8 plies, except by moving straight back), 0: off */
   uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded) */
 } strat_config;
 

@@ -27,6 +27,9 @@
 //   replay ring        pinned: FIFO content, chi-square of indices.
 //   determinise        pinned: multiset/constraint/obs-equality properties, chi-square of
 //                      Bomb/Flag placement over the unmoved squares.
+//   continuous chasing (R#28) pinned: hand-worked chase around a 2x2 block, state-machine
+//                      cases, independent snapshot checker.  The mechanics the paper leaves
+//                      open (what ends a chase, 8-ply memory) are PARITY UNPINNED against it.
 //   pinned reset (R#27) pinned: a restarted game equals its pinned line byte for byte except
 //                      the epoch; the reading itself (epoch keeps counting) is PARITY UNPINNED
 //                      against the paper (P:252-254 gives no detail).

@@ -32,7 +32,7 @@ class strat_config(C.Structure):
     _fields_ = [
         ("num_games", C.c_int32), ("variant", C.c_int32), ("seed", C.c_uint64),
         ("max_plies", C.c_int32), ("max_battleless", C.c_int32), ("auto_reset", C.c_int32),
-        ("two_square", C.c_int32), ("device", C.c_int32), ("reserved", C.c_int32),
+        ("two_square", C.c_int32), ("device", C.c_int32), ("chase_rule", C.c_int32),
         ("game_base", C.c_uint64),
     ]
 
@@ -129,10 +129,10 @@ class Env:
     """N parallel games bound to a caller-owned (torch) workspace."""
 
     def __init__(self, num_games, variant=0, seed=0, max_plies=0, max_battleless=0, auto_reset=0,
-                 two_square=1, device=0, game_base=0):
+                 two_square=1, device=0, game_base=0, chase_rule=0):
         _require_cuda()
         self.cfg = strat_config(num_games, variant, seed, max_plies, max_battleless, auto_reset,
-                                two_square, device, 0, game_base)
+                                two_square, device, chase_rule, game_base)
         self.n = num_games
         self.device = torch.device("cuda", device)
         nbytes = lib().strat_workspace_bytes(C.byref(self.cfg))

@@ -166,7 +166,8 @@ __global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict
   uint32_t w29 = __shfl_sync(0xffffffffu, cw, 29), w31 = __shfl_sync(0xffffffffu, cw, 31);
   if (lane == 28) mine = w29;  // ply | battleless<<16 : same bytes as canonical 116..119
   if (lane == 29) mine = w31;  // epoch
-  if (lane >= 30) mine = 0;
+  if (lane == 30) mine = fw >> 16;  // chase ages: canonical bytes 122..123
+  if (lane == 31) mine = 0;
   lines[(size_t)g * kLineWords + lane] = mine;
 }
 
@@ -195,6 +196,7 @@ __global__ void __launch_bounds__(128) k_export(int n, const uint32_t* __restric
   uint32_t hw = __shfl_sync(0xffffffffu, lw, 4 * ((lane - 25) & 3) + 3) >> 4;   // history pair for lanes 25..28
   uint32_t fw = __shfl_sync(0xffffffffu, lw, 19) >> 4;
   uint32_t w28 = __shfl_sync(0xffffffffu, lw, 28), w29 = __shfl_sync(0xffffffffu, lw, 29);
+  uint32_t w30 = __shfl_sync(0xffffffffu, lw, 30);
   if (lane >= 25 && lane < 29) {
     uint32_t e0 = hw & 0x3FFFu, e1 = (hw >> 14) & 0x3FFFu;
     uint32_t b0 = e0 == kHistNone ? 0xFFFFu : ((e0 & 127u) | ((e0 >> 7) << 8));
@@ -205,12 +207,13 @@ __global__ void __launch_bounds__(128) k_export(int n, const uint32_t* __restric
   if (lane == 30) {
     uint32_t done = fw & 1u, reason = (fw >> 1) & 7u;
     int32_t res = (int32_t)((fw >> 4) & 3u) - 1;
-    out = (done | (reason << 2)) | (((uint32_t)res & 0xFFu) << 8);
+    out = (done | (reason << 2)) | (((uint32_t)res & 0xFFu) << 8) | ((w30 & 0xFFFFu) << 16);
   }
   if (lane == 31) out = w29;
   reinterpret_cast<uint32_t*>(canon + (size_t)g * 128)[lane] = out;
 }
 
+template <bool kChase>
 __global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __restrict__ lines, uint32_t* __restrict__ mask) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
@@ -221,7 +224,7 @@ __global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __r
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
     int cnt[4];
-    if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, s_mask + lane * kMaskWords, cnt);
+    if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), s_mask + lane * kMaskWords, cnt);
   }
   __syncwarp();
   store_mask(mask, first, ng, s_mask, lane);
@@ -270,6 +273,7 @@ __global__ void __launch_bounds__(128) k_sample_uniform(Params P, const uint32_t
   if (lane == 0) actions[g] = (int16_t)action;
 }
 
+template <bool kChase>
 __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ lines, const int16_t* __restrict__ actions,
                                              int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err,
                                              HistSlot hs) {
@@ -282,7 +286,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
     int a = (int)actions[first + lane];
-    StepOut o = step_game<true>(P, (uint32_t)(first + lane), g, a);
+    StepOut o = step_game<true, false, kChase>(P, (uint32_t)(first + lane), g, a);
     if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
     reward[first + lane] = (int8_t)o.reward;
     done[first + lane] = (uint8_t)o.done;
@@ -479,7 +483,7 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   if ((rs >> lane) & 1u) {
     g.mvd = g.rev = bb_zero();
     hist_clear(g);
-    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0;
+    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0;
     if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
   }
   __syncwarp();
@@ -490,7 +494,7 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
 // kExternal = true (strat_step_observe): `actions` is the caller's input (validated) -> step ->
 //   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
 //   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
-template <bool kExternal>
+template <bool kExternal, bool kChase>
 __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
@@ -546,7 +550,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       PROF_T(t2);
       bool reset_me = false;
       if (!kExternal) {
-        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);
+        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt);
         __syncwarp();
         PROF_T(t3);
         if (mask) store_mask(mask, first, ng, work, lane);
@@ -554,7 +558,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         if (lane < ng) {
           int a = -1;
           if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
-          StepOut o = step_game<false, true>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+          StepOut o = step_game<false, true, kChase>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
           if (actions) actions[first + lane] = (int16_t)a;
           if (reward) reward[first + lane] = (int8_t)o.reward;
           if (done) done[first + lane] = (uint8_t)o.done;
@@ -570,7 +574,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       } else {
         if (lane < ng) {
           int a = (int)actions[first + lane];
-          StepOut o = step_game<true, true>(P, (uint32_t)(first + lane), g, a);
+          StepOut o = step_game<true, true, kChase>(P, (uint32_t)(first + lane), g, a);
           if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
           reward[first + lane] = (int8_t)o.reward;
           done[first + lane] = (uint8_t)o.done;
@@ -586,7 +590,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         }
         if (lane < ng) {
           store_game_global(lines, first + lane, g);
-          if (!g.done) legal_mask_row(g, g.ply & 1u, P.two_square, work + lane * kMaskWords, cnt);  // of the NEW state
+          if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt);  // of the NEW state
         }
         __syncwarp();
         if (mask) store_mask(mask, first, ng, work, lane);
@@ -628,6 +632,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
 // `plies` plies of uniform-random legal play with the board in registers.  The 3600-bit mask is
 // never built: the r-th legal action is found from the move bitboards (sample_action_direct).
 constexpr int kScoutScratch = 9;  // 8 words per game, odd stride
+template <bool kChase>
 __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   __shared__ uint32_t s_scouts[kBatch * kScoutScratch];
@@ -638,9 +643,9 @@ __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __re
     Game g; read_game(s_state, lane, g);
     for (int t = 0; t < plies; ++t) {
       if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
-      int a = sample_action_direct(g, g.ply & 1u, P.two_square, action_draw(P, (uint32_t)(first + lane), g),
+      int a = sample_action_direct(g, g.ply & 1u, rules_of<kChase>(P), action_draw(P, (uint32_t)(first + lane), g),
                                    s_scouts + lane * kScoutScratch);
-      step_game<false>(P, (uint32_t)(first + lane), g, a);
+      step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a);
     }
     write_game(s_state, lane, g);
   }
@@ -748,7 +753,7 @@ __global__ void k_set_int(int* p, int v) { *p = v; }
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool cfg_ok(const strat_config* c) {
   return c && c->num_games >= 1 && (c->variant == 0 || c->variant == 1) && c->max_plies >= 0 &&
-         c->max_battleless >= 0 && c->reserved == 0;
+         c->max_battleless >= 0 && (c->chase_rule == 0 || c->chase_rule == 1);
 }
 inline Params make_params(const strat_config& c) {
   Params P;
@@ -757,6 +762,7 @@ inline Params make_params(const strat_config& c) {
   P.num_games = c.num_games; P.variant = c.variant;
   P.ply_cap = (c.max_plies >= 1 && c.max_plies <= 65535) ? c.max_plies : 65535;
   P.max_battleless = c.max_battleless; P.auto_reset = c.auto_reset ? 1 : 0; P.two_square = c.two_square ? 1 : 0;
+  P.chase_rule = c.chase_rule ? 1 : 0;
   P.pin = nullptr;
   return P;
 }
@@ -857,7 +863,8 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = 1;
   const uint32_t version = env->version + 1;
-  if (cudaLaunchKernelEx(&lc, k_rollout_step<kExternal>, env->P, env->lines, mask, actions, reward, done, obs,
+  auto kernel = env->P.chase_rule ? k_rollout_step<kExternal, true> : k_rollout_step<kExternal, false>;
+  if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
                          env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
                          hist_slot(env->hist), env->err) != cudaSuccess)
     return STRAT_CUDA_ERROR;
@@ -956,7 +963,8 @@ int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream) {
 
 int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream) {
   if (!env || !mask) return STRAT_BAD_ARG;
-  k_legal_mask<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
+  if (env->P.chase_rule) k_legal_mask<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
+  else k_legal_mask<false><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
   return launch_status();
 }
 
@@ -969,8 +977,12 @@ int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* ac
 
 int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream) {
   if (!env || !actions || !reward || !done) return STRAT_BAD_ARG;
-  k_step<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err,
-                                                                     hist_slot(env->hist));
+  if (env->P.chase_rule)
+    k_step<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done,
+                                                                             env->err, hist_slot(env->hist));
+  else
+    k_step<false><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done,
+                                                                              env->err, hist_slot(env->hist));
   if (env->hist) env->hist->cur += 1;
   return launch_status();
 }
@@ -1049,7 +1061,10 @@ int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_ho
 int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream) {
   if (!env || plies < 0) return STRAT_BAD_ARG;
   if (env->hist) return STRAT_BAD_STATE;  // on-chip plies are not recorded
-  k_rollout_uniform<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
+  if (env->P.chase_rule)
+    k_rollout_uniform<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
+  else
+    k_rollout_uniform<false><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
   return launch_status();
 }
 
@@ -1205,7 +1220,8 @@ int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, 
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !mask) return STRAT_BAD_ARG;
   const Params& P = h->env ? h->env->P : h->P;
-  k_legal_mask<<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
+  if (P.chase_rule) k_legal_mask<true><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
+  else k_legal_mask<false><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
   return launch_status();
 }
 

@@ -54,8 +54,16 @@ struct Params {  // per-environment constants handed to every kernel by value
   int32_t max_battleless;  // 0 = off
   int32_t auto_reset;
   int32_t two_square;
+  int32_t chase_rule;      // continuous-chasing rule (R#28)
   const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
 };
+
+// Rule switches handed to the move generators: bit 0 two-square rule, bit 1 chasing rule.
+constexpr int RULE_TWO_SQUARE = 1, RULE_CHASE = 2;
+// kChase = false compiles the (rare, register-hungry) chasing-rule paths out of a kernel.
+template <bool kChase> SD int rules_of(const Params& P) {
+  return (P.two_square ? RULE_TWO_SQUARE : 0) | ((kChase && P.chase_rule) ? RULE_CHASE : 0);
+}
 
 // ------------------------------------------------------------------ 100-bit boards
 struct BB { uint32_t w[4]; };  // cell c -> word c>>5, bit c&31; w[3] uses bits 0..3
@@ -160,13 +168,15 @@ SD uint32_t bounded(uint32_t u, uint32_t n) { return sd_mulhi(u, n); }
 // 6 revealed), cells 32i..32i+31.  Word 4p+3 holds cells 96..99 in bits 0..3 and 28 spare
 // bits: planes 0..3 carry history entries 2p (bits 4..17) and 2p+1 (bits 18..31), an entry
 // being from | to<<7 (0x3FFF = none); plane 4 carries flags (bit 4 done, bits 5..7 reason,
-// bits 8..9 result+1).  Word 28 = ply | battleless<<16, word 29 = epoch, 30..31 zero.
+// bits 8..9 result+1).  Word 28 = ply | battleless<<16, word 29 = epoch, word 30 = chase age of
+// red | blue<<8 (R#28), word 31 zero.
 struct Game {
   BB t0, t1, t2, t3, own, mvd, rev;
   uint32_t h[4];
   uint32_t done, reason;
   int32_t result;
   uint32_t ply, battleless, epoch;
+  uint32_t chase;  // chase age of red | blue << 8: positions of the player's running chase (0 = none)
 };
 
 SD void unpack_line(const uint32_t* W, Game& g) {
@@ -181,7 +191,7 @@ SD void unpack_line(const uint32_t* W, Game& g) {
   for (int p = 0; p < 4; ++p) g.h[p] = W[4 * p + 3] >> 4;
   uint32_t f = W[19] >> 4;
   g.done = f & 1u; g.reason = (f >> 1) & 7u; g.result = (int32_t)((f >> 4) & 3u) - 1;
-  g.ply = W[28] & 0xFFFFu; g.battleless = W[28] >> 16; g.epoch = W[29];
+  g.ply = W[28] & 0xFFFFu; g.battleless = W[28] >> 16; g.epoch = W[29]; g.chase = W[30] & 0xFFFFu;
 }
 SD void pack_line(const Game& g, uint32_t* W) {
   const BB* pl[7] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own, &g.mvd, &g.rev};
@@ -192,7 +202,7 @@ SD void pack_line(const Game& g, uint32_t* W) {
   STRAT_UNROLL
   for (int p = 0; p < 4; ++p) W[4 * p + 3] |= g.h[p] << 4;
   W[19] |= (g.done | (g.reason << 1) | ((uint32_t)(g.result + 1) << 4)) << 4;
-  W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = 0; W[31] = 0;
+  W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = g.chase; W[31] = 0;
 }
 SD uint32_t hist_entry(const Game& g, int j) { return (g.h[j >> 1] >> (14 * (j & 1))) & 0x3FFFu; }
 SD void hist_push(Game& g, uint32_t e) {
@@ -244,6 +254,79 @@ SD Ban two_square_ban(const Game& g, int side, int enabled) {
   return b;
 }
 
+// ------------------------------------------------------------------ continuous-chasing rule
+// P:212-218 / R#28.  threat = a move to an empty square that ends next to an opponent's piece;
+// evade = the piece threatened on the previous ply moves, to an empty square, away from the
+// piece that threatened it; a player's chase = its threats alternating with the opponent's
+// evades; g.chase holds each player's chase age (positions since its first threat, 0 = none).
+SD uint32_t chase_age(const Game& g, int side) { return (g.chase >> (8 * side)) & 0xFFu; }
+SD bool cells_adjacent(int a, int b) {
+  int ra = a / 10, rb = b / 10, dr = ra - rb, dc = (a - 10 * ra) - (b - 10 * rb);
+  return dr * dr + dc * dc == 1;
+}
+SD BB neighbours_of(int c) {
+  CellSel s = cell_sel(c);
+  BB one; one.w[0] = s.m[0]; one.w[1] = s.m[1]; one.w[2] = s.m[2]; one.w[3] = s.m[3];
+  return bb_or(bb_or(bb_up<10>(one), bb_down<10>(one)),
+               bb_or(bb_and(bb_up<1>(one), bb_const(kNotCol0)), bb_and(bb_down<1>(one), bb_const(kNotCol9))));
+}
+// The moves of `side` that the chasing rule bans in this position (at most 8: every earlier
+// position of the chase within the 8 logged plies can be recreated by at most one move).
+// A position is the type and owner on every square.  Earlier positions are rebuilt by taking
+// the logged plies back on copies of the five type/owner planes (no battle happens inside a
+// chase); position t-b is recreated by the move c->a iff it differs from the current one on
+// exactly the squares {c, a}, with the current piece of c standing on a.
+// Returned: action indices (the caller still checks that they are otherwise legal).
+SD int chase_banned_actions(const Game& g, int side, BB mine, BB enemy, int banned[8]) {
+  int age = (int)chase_age(g, side);
+  if (age < 2) return 0;
+  int first = ((int)(g.ply & 1u) == side) ? 1 : 0;
+  uint32_t eprev = hist_entry(g, first);  // this player's previous ply
+  int back = min(age - 1, 8), nb = 0;
+  BB k[5] = {g.t0, g.t1, g.t2, g.t3, g.own};
+  for (int b = 1; b <= back; ++b) {
+    uint32_t e = hist_entry(g, b - 1);
+    if (e == kHistNone) break;
+    CellSel sf = cell_sel((int)(e & 127u)), st = cell_sel((int)(e >> 7));
+    STRAT_UNROLL
+    for (int p = 0; p < 5; ++p) { uint32_t v = bb_get(k[p], st); bb_put(k[p], st, 0); bb_put(k[p], sf, v); }
+    uint32_t d[4];
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i)
+      d[i] = (k[0].w[i] ^ g.t0.w[i]) | (k[1].w[i] ^ g.t1.w[i]) | (k[2].w[i] ^ g.t2.w[i]) | (k[3].w[i] ^ g.t3.w[i]) |
+             (k[4].w[i] ^ g.own.w[i]);
+    if (sd_popc(d[0]) + sd_popc(d[1]) + sd_popc(d[2]) + sd_popc(d[3]) != 2) continue;
+    int s1 = -1, s2 = -1;
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      uint32_t w = d[i];
+      while (w) { int sq = 32 * i + sd_ffs(w) - 1; w &= w - 1; if (s1 < 0) s1 = sq; else s2 = sq; }
+    }
+    // c = the square that holds a piece now and is empty in the earlier position; a = the reverse
+    bool occ1 = bb_test(g.t0, s1) | bb_test(g.t1, s1) | bb_test(g.t2, s1) | bb_test(g.t3, s1);
+    int c = occ1 ? s1 : s2, a = occ1 ? s2 : s1;
+    CellSel sc = cell_sel(c), sa = cell_sel(a);
+    bool ok = bb_test(mine, c) != 0;
+    uint32_t cur_a = 0, old_c = 0, same = 1;
+    const BB* cur[5] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own};
+    STRAT_UNROLL
+    for (int p = 0; p < 5; ++p) {
+      if (p < 4) { cur_a |= bb_get(*cur[p], sa); old_c |= bb_get(k[p], sc); }
+      same &= (bb_get(*cur[p], sc) == bb_get(k[p], sa)) ? 1u : 0u;
+    }
+    if (!ok || cur_a || old_c || !same) continue;
+    int ra = a / 10, rc = c / 10, qa = a - 10 * ra, qc = c - 10 * rc;
+    int dir, dist;
+    if (qa == qc) { dir = ra > rc ? 0 : 2; dist = ra > rc ? ra - rc : rc - ra; }
+    else if (ra == rc) { dir = qa > qc ? 1 : 3; dist = qa > qc ? qa - qc : qc - qa; }
+    else continue;
+    if (!bb_any(bb_and(neighbours_of(a), enemy))) continue;                                  // not a threat
+    if (eprev != kHistNone && c == (int)(eprev >> 7) && a == (int)(eprev & 127u)) continue;  // the return move
+    banned[nb++] = c * 36 + dir * 9 + dist - 1;
+  }
+  return nb;
+}
+
 // ------------------------------------------------------------------ move generation
 struct Moves {
   BB d[4];      // d[dir][c] = piece of `side` at c may move one square in dir (after bans)
@@ -252,7 +335,7 @@ struct Moves {
   BB ok;        // squares a piece of `side` may land on (empty or enemy, not lake)
   Ban ban;
 };
-SD void single_step_moves(const Game& g, int side, int two_square, Moves& m) {
+SD void single_step_moves(const Game& g, int side, int rules, Moves& m) {
   BB occ = occupied(g);
   BB mine = owned_by(g, occ, side);
   BB notlake = bb_const(kNotLake);
@@ -266,7 +349,7 @@ SD void single_step_moves(const Game& g, int side, int two_square, Moves& m) {
   m.d[2] = bb_and(movable, bb_up<10>(m.ok));
   m.d[1] = bb_and(bb_and(movable, bb_down<1>(m.ok)), bb_const(kNotCol9));
   m.d[3] = bb_and(bb_and(movable, bb_up<1>(m.ok)), bb_const(kNotCol0));
-  m.ban = two_square_ban(g, side, two_square);
+  m.ban = two_square_ban(g, side, rules & RULE_TWO_SQUARE);
   if (m.ban.from >= 0 && m.ban.k <= 1) {
     CellSel s = cell_sel(m.ban.from);
     STRAT_UNROLL
@@ -277,9 +360,9 @@ SD void single_step_moves(const Game& g, int side, int two_square, Moves& m) {
   }
 }
 // GetHasLegalMovement: a banned distance bans every longer one (R#6), so a side
-// has a legal move iff it has a legal single-step move.
-SD bool has_legal_move(const Game& g, int side, int two_square) {
-  Moves m; single_step_moves(g, side, two_square, m);
+// has a legal move iff it has a legal single-step move - unless the chasing rule takes moves
+// away one by one (has_legal_move below then counts them).
+SD bool has_single_step_move(const Moves& m) {
   return bb_any(bb_or(bb_or(m.d[0], m.d[1]), bb_or(m.d[2], m.d[3])));
 }
 
@@ -324,6 +407,54 @@ SD void scout_rays(const Moves& m, int c, int r, int q, int len[4]) {
   }
 }
 
+// Is action a legal by movement, lakes, blocking and the two-square rule (all in m)?
+SD bool move_in_moves(const Moves& m, int a) {
+  if (a < 0 || a >= 3600) return false;
+  int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
+  if (!bb_test(m.d[d], from)) return false;
+  if (dist == 1) return true;
+  if (!bb_test(m.scouts, from)) return false;
+  int r = from / 10, q = from - 10 * r;
+  int len[4];
+  scout_rays(m, from, r, q, len);
+  int ld = d == 0 ? len[0] : d == 1 ? len[1] : d == 2 ? len[2] : len[3];
+  return dist <= ld;
+}
+// Distinct actions of banned[0..nb) that are legal in m, compacted in place; returns their number.
+SD int keep_legal_banned(const Moves& m, int banned[8], int nb) {
+  int k = 0;
+  for (int i = 0; i < nb; ++i) {
+    bool dup = false;
+    for (int j = 0; j < k; ++j) dup |= banned[j] == banned[i];
+    if (!dup && move_in_moves(m, banned[i])) banned[k++] = banned[i];
+  }
+  return k;
+}
+SD bool has_legal_move(const Game& g, int side, int rules) {
+  Moves m; single_step_moves(g, side, rules, m);
+  if (!has_single_step_move(m)) return false;
+  if (!(rules & RULE_CHASE) || chase_age(g, side) < 2) return true;
+  BB occ = occupied(g), mine = owned_by(g, occ, side);
+  int banned[8];
+  int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+  if (nb == 0) return true;
+  nb = keep_legal_banned(m, banned, nb);
+  int total = 0;  // every legal move without the chasing rule
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    uint32_t sc = m.scouts.w[i];
+    total += sd_popc(m.d[0].w[i] & ~sc) + sd_popc(m.d[1].w[i] & ~sc) + sd_popc(m.d[2].w[i] & ~sc) + sd_popc(m.d[3].w[i] & ~sc);
+    uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
+    while (ss) {
+      int b = sd_ffs(ss) - 1; ss &= ss - 1;
+      int c = 32 * i + b, r = c / 10, q = c - 10 * r, len[4];
+      scout_rays(m, c, r, q, len);
+      total += len[0] + len[1] + len[2] + len[3];
+    }
+  }
+  return total > nb;
+}
+
 SD void mask_or_field(uint32_t* row, int c, uint64_t field) {  // the 36 action bits of cell c
   int pos = 36 * c, wi = pos >> 5, sh = pos & 31;
   field <<= sh;  // 36 + 28 <= 64
@@ -335,8 +466,8 @@ SD void mask_or_field(uint32_t* row, int c, uint64_t field) {  // the 36 action 
 // Legal mask of `side` into `row` (113 words, already zero).  Returns the number of legal
 // actions and, in cnt[i], how many of them start from cells 32i..32i+31 (= mask words
 // 36i..36i+35; used by pick_action).  a = from*36 + dir*9 + dist-1.
-SD int legal_mask_row(const Game& g, int side, int two_square, uint32_t* row, int cnt[4]) {
-  Moves m; single_step_moves(g, side, two_square, m);
+SD int legal_mask_row(const Game& g, int side, int rules, uint32_t* row, int cnt[4]) {
+  Moves m; single_step_moves(g, side, rules, m);
   // pieces that move one square: four bits per piece, no branches
   STRAT_UNROLL
   for (int i = 0; i < 4; ++i) {
@@ -365,6 +496,20 @@ SD int legal_mask_row(const Game& g, int side, int two_square, uint32_t* row, in
       uint64_t field = (uint64_t)((1u << len[0]) - 1u) | ((uint64_t)((1u << len[1]) - 1u) << 9) |
                        ((uint64_t)((1u << len[2]) - 1u) << 18) | ((uint64_t)((1u << len[3]) - 1u) << 27);
       mask_or_field(row, c, field);
+    }
+  }
+  if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: take the chase-banned threats out
+    BB occ = occupied(g), mine = owned_by(g, occ, side);
+    int banned[8];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    for (int i = 0; i < nb; ++i) {
+      uint32_t bit = 1u << (banned[i] & 31);
+      int w = banned[i] >> 5, grp = (banned[i] / 36) >> 5;
+      if (row[w] & bit) {
+        row[w] &= ~bit;
+        STRAT_UNROLL
+        for (int k = 0; k < 4; ++k) cnt[k] -= (k == grp) ? 1 : 0;
+      }
     }
   }
   return cnt[0] + cnt[1] + cnt[2] + cnt[3];
@@ -399,31 +544,9 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
 // the direction, then the distance, so the r-th legal action is found by walking the pieces that
 // can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
 // lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
-SD int sample_action_direct(const Game& g, int side, int two_square, uint32_t u, uint32_t* scouts) {
-  Moves m; single_step_moves(g, side, two_square, m);
-  uint32_t D[4][4];
-  int cnt[4], ns = 0;
-  STRAT_UNROLL
-  for (int i = 0; i < 4; ++i) {
-    uint32_t sc = m.scouts.w[i];
-    STRAT_UNROLL
-    for (int d = 0; d < 4; ++d) D[i][d] = m.d[d].w[i] & ~sc;
-    cnt[i] = sd_popc(D[i][0]) + sd_popc(D[i][1]) + sd_popc(D[i][2]) + sd_popc(D[i][3]);
-    uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
-    while (ss) {
-      int b = sd_ffs(ss) - 1;
-      ss &= ss - 1;
-      int c = 32 * i + b, r = c / 10, q = c - 10 * r;
-      int len[4];
-      scout_rays(m, c, r, q, len);
-      cnt[i] += len[0] + len[1] + len[2] + len[3];
-      if (ns < 8) scouts[ns++] = (uint32_t)c | ((uint32_t)len[0] << 8) | ((uint32_t)len[1] << 12) |
-                                ((uint32_t)len[2] << 16) | ((uint32_t)len[3] << 20);
-    }
-  }
-  int n = cnt[0] + cnt[1] + cnt[2] + cnt[3];
-  if (n == 0) return -1;
-  int r = (int)bounded(u, (uint32_t)n);
+// r-th (from 0) legal action in ascending order, given the per-group counts, the non-Scout
+// direction bits D[group][dir] and the Scouts' packed ray lengths (cell | len0<<8 | .. | len3<<20).
+SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r) {
   int gi = 0;
   if (r >= cnt[0]) { r -= cnt[0]; gi = 1; if (r >= cnt[1]) { r -= cnt[1]; gi = 2; if (r >= cnt[2]) { r -= cnt[2]; gi = 3; } } }
   uint32_t d0 = gi == 0 ? D[0][0] : gi == 1 ? D[1][0] : gi == 2 ? D[2][0] : D[3][0];
@@ -450,6 +573,55 @@ SD int sample_action_direct(const Game& g, int side, int two_square, uint32_t u,
     r -= c;
   }
 }
+// SampleRandomLegalAction without materialising the 3600-bit mask (on-chip rollouts): equal to
+// pick_action(legal_mask_row(...)) for the same draw u.  Actions ascend with the from-cell, then
+// the direction, then the distance, so the r-th legal action is found by walking the pieces that
+// can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
+// lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
+SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint32_t* scouts) {
+  Moves m; single_step_moves(g, side, rules, m);
+  uint32_t D[4][4];
+  int cnt[4], ns = 0;
+  STRAT_UNROLL
+  for (int i = 0; i < 4; ++i) {
+    uint32_t sc = m.scouts.w[i];
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d) D[i][d] = m.d[d].w[i] & ~sc;
+    cnt[i] = sd_popc(D[i][0]) + sd_popc(D[i][1]) + sd_popc(D[i][2]) + sd_popc(D[i][3]);
+    uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
+    while (ss) {
+      int b = sd_ffs(ss) - 1;
+      ss &= ss - 1;
+      int c = 32 * i + b, r = c / 10, q = c - 10 * r;
+      int len[4];
+      scout_rays(m, c, r, q, len);
+      cnt[i] += len[0] + len[1] + len[2] + len[3];
+      if (ns < 8) scouts[ns++] = (uint32_t)c | ((uint32_t)len[0] << 8) | ((uint32_t)len[1] << 12) |
+                                ((uint32_t)len[2] << 16) | ((uint32_t)len[3] << 20);
+    }
+  }
+  int n = cnt[0] + cnt[1] + cnt[2] + cnt[3];
+  if (n == 0) return -1;
+  if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: skip the chase-banned threats
+    BB occ = occupied(g), mine = owned_by(g, occ, side);
+    int banned[8];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    nb = keep_legal_banned(m, banned, nb);
+    if (nb > 0) {
+      if (n == nb) return -1;
+      int r = (int)bounded(u, (uint32_t)(n - nb));
+      // the r-th action that is not banned: skip the banned ones at or below it (fixed point)
+      for (int ra = r;;) {
+        int a = select_action(D, cnt, scouts, ns, ra);
+        int below = 0;
+        for (int i = 0; i < nb; ++i) below += banned[i] <= a ? 1 : 0;
+        if (r + below == ra) return a;
+        ra = r + below;
+      }
+    }
+  }
+  return select_action(D, cnt, scouts, ns, (int)bounded(u, (uint32_t)n));
+}
 SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
   uint32_t o[4];
   philox(P.game_base + local_game, g.epoch, g.ply, TAG_ACTION, P.key0, P.key1, o);
@@ -457,18 +629,17 @@ SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
 }
 
 // Is action a legal for the side to move?  (step validates what it is given)
-SD bool action_is_legal(const Game& g, int side, int two_square, int a) {
-  if (a < 0 || a >= 3600) return false;
-  int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
-  Moves m; single_step_moves(g, side, two_square, m);
-  if (!bb_test(m.d[d], from)) return false;
-  if (dist == 1) return true;
-  if (!bb_test(m.scouts, from)) return false;
-  int r = from / 10, q = from - 10 * r;
-  int len[4];
-  scout_rays(m, from, r, q, len);
-  int ld = d == 0 ? len[0] : d == 1 ? len[1] : d == 2 ? len[2] : len[3];
-  return dist <= ld;
+SD bool action_is_legal(const Game& g, int side, int rules, int a) {
+  Moves m; single_step_moves(g, side, rules, m);
+  if (!move_in_moves(m, a)) return false;
+  if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {
+    BB occ = occupied(g), mine = owned_by(g, occ, side);
+    int banned[8];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    for (int i = 0; i < nb; ++i)
+      if (banned[i] == a) return false;
+  }
+  return true;
 }
 
 // ------------------------------------------------------------------ setup (C2)
@@ -510,7 +681,7 @@ SD bool side_can_ever_move(const Game& t, int side) {
 SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
   g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
   hist_clear(g);
-  g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0;
+  g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0;
   uint32_t gidx = P.game_base + local_game;
   for (int side = 0; side < 2; ++side) {
     for (uint32_t attempt = 0;; ++attempt) {
@@ -562,18 +733,35 @@ struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; };
 // kValidate = false only when `a` was just drawn from this state's own legal mask.
 // kDeferReset: the caller performs the auto-reset itself (epoch is already advanced) when
 // o.needs_reset is set; the result must equal reset_game(P, local_game, g).
-template <bool kValidate, bool kDeferReset = false>
+template <bool kValidate, bool kDeferReset = false, bool kChase = false>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   StepOut o; o.illegal = false; o.needs_reset = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
   int side = g.ply & 1u;
-  if (kValidate && !action_is_legal(g, side, P.two_square, a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
+  if (kValidate && !action_is_legal(g, side, rules_of<kChase>(P), a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
   int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
   int to = from + dist * (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
   CellSel sf = cell_sel(from), st = cell_sel(to);
   int pt = bb_get(g.t0, sf) | (bb_get(g.t1, sf) << 1) | (bb_get(g.t2, sf) << 2) | (bb_get(g.t3, sf) << 3);
   uint32_t prev = bb_get(g.rev, sf);
   int tt = bb_get(g.t0, st) | (bb_get(g.t1, st) << 1) | (bb_get(g.t2, st) << 2) | (bb_get(g.t3, st) << 3);
+  if (kChase && P.chase_rule) {  // chase state machine (R#28), judged on the position before the move
+    uint32_t ap = chase_age(g, side), aq = chase_age(g, side ^ 1);
+    if (tt != 0) {
+      ap = aq = 0;  // a battle ends every chase
+    } else {
+      BB occ0 = occupied(g);
+      BB enemy0 = bb_andn(occ0, owned_by(g, occ0, side));
+      bool threat = bb_any(bb_and(neighbours_of(to), enemy0));
+      if (aq > 0) {  // the opponent's previous ply was a threat by the piece now on x
+        uint32_t e0 = hist_entry(g, 0);
+        bool evade = e0 != kHistNone && cells_adjacent(from, (int)(e0 >> 7)) && !cells_adjacent(to, (int)(e0 >> 7));
+        aq = evade ? (aq < 255u ? aq + 1u : 255u) : 0u;
+      }
+      ap = threat ? (ap > 0 ? (ap < 255u ? ap + 1u : 255u) : 1u) : 0u;
+    }
+    g.chase = side == 0 ? (ap | (aq << 8)) : (aq | (ap << 8));
+  }
   hist_push(g, (uint32_t)from | ((uint32_t)to << 7));
   // the origin square empties in every case
   bb_put(g.t0, sf, 0); bb_put(g.t1, sf, 0); bb_put(g.t2, sf, 0); bb_put(g.t3, sf, 0);
@@ -603,9 +791,9 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   int mover_result = side == 0 ? 1 : -1;
   // terminal tests in R#12 order
   if (flag_captured) { g.done = 1; g.reason = REASON_FLAG; g.result = mover_result; }
-  else if (!has_legal_move(g, side ^ 1, P.two_square)) {
+  else if (!has_legal_move(g, side ^ 1, rules_of<kChase>(P))) {
     g.done = 1;
-    if (!has_legal_move(g, side, P.two_square)) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
+    if (!has_legal_move(g, side, rules_of<kChase>(P))) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
     else { g.reason = REASON_NOMOVE_WIN; g.result = mover_result; }
   }
   else if ((int)g.ply >= P.ply_cap) { g.done = 1; g.reason = REASON_PLY_CAP; g.result = 0; }
@@ -721,6 +909,7 @@ SD void import_canonical(const uint8_t* L, Game& g) {
   g.ply = L[116] | ((uint32_t)L[117] << 8);
   g.battleless = L[118] | ((uint32_t)L[119] << 8);
   g.done = L[120] & 1u; g.reason = (L[120] >> 2) & 7u; g.result = (int32_t)(int8_t)L[121];
+  g.chase = L[122] | ((uint32_t)L[123] << 8);
   g.epoch = L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
 }
 SD void export_canonical(const Game& g, uint8_t* L) {
@@ -739,7 +928,7 @@ SD void export_canonical(const Game& g, uint8_t* L) {
   L[116] = (uint8_t)g.ply; L[117] = (uint8_t)(g.ply >> 8);
   L[118] = (uint8_t)g.battleless; L[119] = (uint8_t)(g.battleless >> 8);
   L[120] = (uint8_t)(g.done | (g.reason << 2)); L[121] = (uint8_t)(int8_t)g.result;
-  L[122] = 0; L[123] = 0;
+  L[122] = (uint8_t)g.chase; L[123] = (uint8_t)(g.chase >> 8);
   L[124] = (uint8_t)g.epoch; L[125] = (uint8_t)(g.epoch >> 8); L[126] = (uint8_t)(g.epoch >> 16);
   L[127] = (uint8_t)(g.epoch >> 24);
 }
