@@ -559,6 +559,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           int a = -1;
           if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
           StepOut o = step_game<false, true, kChase>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+          if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
           if (actions) actions[first + lane] = (int16_t)a;
           if (reward) reward[first + lane] = (int8_t)o.reward;
           if (done) done[first + lane] = (uint8_t)o.done;
@@ -645,7 +646,10 @@ __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __re
       if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
       int a = sample_action_direct(g, g.ply & 1u, rules_of<kChase>(P), action_draw(P, (uint32_t)(first + lane), g),
                                    s_scouts + lane * kScoutScratch);
-      step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a);
+      if (step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
+        raise_error(err, STRAT_ILLEGAL_ACTION);
+        break;
+      }
     }
     write_game(s_state, lane, g);
   }

@@ -738,6 +738,9 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   StepOut o; o.illegal = false; o.needs_reset = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
   int side = g.ply & 1u;
+  // a live game without a legal move (only a hand-built line can be one: play ends such games)
+  // has no action to take: the "action" -1 is illegal like any other
+  if (!kValidate && a < 0) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
   if (kValidate && !action_is_legal(g, side, rules_of<kChase>(P), a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
   int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
   int to = from + dist * (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);

@@ -1,0 +1,131 @@
+"""Edge cases of the C ABI on the GPU: tiny and ragged batches, empty inputs, degenerate
+positions, argument errors."""
+import ctypes as C
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import orc
+from paper_2511_07312_b200 import binding as B
+from paper_2511_07312_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 65])
+def test_tiny_and_ragged_batches_every_call(n):
+    kw = dict(variant=0, seed=n, max_plies=35, auto_reset=1)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(80):
+        om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        if t % 3 == 0:
+            g.rollout_step(mask, act, rew, done, obs)
+        elif t % 3 == 1:
+            g.legal_mask(mask); g.sample_uniform(mask, act); g.step(act, rew, done); g.encode_obs(obs)
+        else:
+            g.legal_mask(mask); g.sample_uniform(mask, act); g.step_observe(act, rew, done, None, obs)
+            g_mask_now = _np(mask).view(np.uint32)
+            assert np.array_equal(g_mask_now, om), t
+        assert np.array_equal(_np(act), oa) and np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od), t
+        assert np.array_equal(_np(obs.view(torch.int16)).view(np.uint16), o.encode_obs()), t
+        assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+    g.rollout_uniform(0)  # zero plies: a no-op
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == 0
+
+
+def test_degenerate_positions():
+    # (a) flags only: the side to move has no legal move and neither has the other -> the mask is
+    #     empty, the sampler returns -1, the fused step leaves the (live, stuck) game as it is
+    flags = {0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE)}
+    # (b) one move available, and it captures the Flag
+    mate = {88: W.piece(W.MINER, W.RED), 0: W.piece(W.FLAG, W.RED), 98: W.piece(W.FLAG, W.BLUE),
+            78: W.piece(W.BOMB, W.BLUE), 87: W.piece(W.BOMB, W.BLUE), 89: W.piece(W.BOMB, W.RED)}
+    # (c) a Scout with the whole file open: nine distances
+    scout = {5: W.piece(W.SCOUT, W.RED), 0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE)}
+    lines = np.stack([W.make_line(flags), W.make_line(mate), W.make_line(scout)])
+    g, o = B.Env(3, seed=1), orc.Env(3, seed=1)
+    g.reset_from(_dev(lines)); o.reset_from(lines)
+    gm = _np(g.legal_mask()).view(np.uint32)
+    assert np.array_equal(gm, o.legal_mask())
+    assert W.mask_to_actions(gm[0]) == []
+    assert W.action_index(5, 0, 9) in W.mask_to_actions(gm[2]) and len(W.mask_to_actions(gm[2])) == 9 + 4 + 4
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    g.rollout_step(mask, act, rew, done, obs)
+    oa = o.sample_uniform(o.legal_mask()); orr, od = o.step(oa)
+    assert np.array_equal(_np(act), oa) and int(_np(act)[0]) == -1
+    assert np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == o.check() == B.ILLEGAL_ACTION  # the stuck live game had no action to take
+    g.clear_error(); o.clear_error()
+    g.rollout_uniform(3)
+    for _ in range(3):
+        o.step(o.sample_uniform(o.legal_mask()))
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == o.check() == B.ILLEGAL_ACTION
+
+
+def test_argument_errors_and_empty_inputs():
+    L = B.lib()
+    g = B.Env(40, seed=1)
+    s = B._stream()
+    assert L.strat_legal_mask(g.h, None, s) == B.BAD_ARG
+    assert L.strat_step(g.h, None, None, None, s) == B.BAD_ARG
+    assert L.strat_rollout_step(g.h, None, None, None, None, None, s) == B.BAD_ARG  # obs is mandatory
+    assert L.strat_rollout_uniform(g.h, -1, s) == B.BAD_ARG
+    assert L.strat_reset_from(g.h, None, s) == B.BAD_ARG
+    bad = B.strat_config(10, 2, 0, 0, 0, 0, 1, 0, 0, 0)  # unknown variant
+    assert L.strat_workspace_bytes(C.byref(bad)) == 0
+    bad = B.strat_config(10, 0, 0, 0, 0, 0, 1, 0, 7, 0)  # chase_rule must be 0 or 1
+    assert L.strat_workspace_bytes(C.byref(bad)) == 0
+    ring = B.Replay(8, 2)
+    obs, mask = g.encode_obs(), g.legal_mask()
+    act = g.sample_uniform(mask); rew, done = g.step(act)
+    so = torch.empty((4, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(B.StratError):  # nothing pushed yet
+        ring.sample(0, 0, 4, so, None, None, None, None)
+    assert L.strat_replay_push(ring.h, B._ptr(obs), B._ptr(mask), B._ptr(act), B._ptr(rew), B._ptr(done), 0, s) == 0
+    assert ring.state() == (0, 0)  # an empty push changes nothing
+    assert L.strat_replay_push(ring.h, B._ptr(obs), B._ptr(mask), B._ptr(act), B._ptr(rew), B._ptr(done), 17, s) == B.BAD_ARG  # > capacity
+    assert L.strat_replay_push(ring.h, B._ptr(obs), B._ptr(mask), B._ptr(act), B._ptr(rew), B._ptr(done), 16, s) == 0
+    assert ring.state() == (0, 16)
+    ring.sample(0, 0, 0, so, None, None, None, None)  # an empty batch is fine
+    with pytest.raises(B.StratError):
+        ring.reserve(5, 0)  # blocks must tile the ring
+    h = B.History(40, 1)  # a one-step ring
+    h.attach(g)
+    g.step(g.sample_uniform(g.legal_mask()))
+    g.step(g.sample_uniform(g.legal_mask()))
+    assert h.current_step() == 2
+    h.legal_mask(1); h.legal_mask(2)
+    with pytest.raises(B.StratError):
+        h.legal_mask(0)  # overwritten
+    assert g.check() == 0
+
+
+def test_sample_uniform_is_uniform_over_the_legal_set():
+    """Chi-square of the sampled rank r = position of the action inside its mask, over many
+    seeds on one position (the closed form: every legal action has probability 1/n)."""
+    line = W.make_line({44: W.piece(W.SCOUT, W.RED), 0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE),
+                        15: W.piece(W.CAPTAIN, W.RED)})
+    n = 20000
+    g = B.Env(n, seed=123)
+    g.reset_from(_dev(np.repeat(line[None, :], n, axis=0)))
+    mask = g.legal_mask()
+    legal = W.mask_to_actions(_np(mask).view(np.uint32)[0])
+    a = _np(g.sample_uniform(mask)).astype(int)
+    counts = np.array([(a == x).sum() for x in legal])
+    assert counts.sum() == n
+    expect = n / len(legal)
+    chi2 = ((counts - expect) ** 2 / expect).sum()
+    assert chi2 < 3 * len(legal) + 30, (chi2, len(legal))
