@@ -129,3 +129,46 @@ def test_sample_uniform_is_uniform_over_the_legal_set():
     expect = n / len(legal)
     chi2 = ((counts - expect) ** 2 / expect).sum()
     assert chi2 < 3 * len(legal) + 30, (chi2, len(legal))
+
+
+def test_random_hand_built_boards_all_calls():
+    """2,000 arbitrary positions (any number of pieces of any type anywhere, random moved /
+    revealed bits, either side to move): mask, observation, sampled action, step, terminal
+    verdicts and the resulting lines against the oracle; then three more plies."""
+    rng = np.random.default_rng(42)
+    n = 2000
+    lines = np.zeros((n, 128), np.uint8)
+    free = [c for c in range(100) if c not in W.LAKES]
+    for i in range(n):
+        k = int(rng.integers(2, 60))
+        cells = rng.choice(free, k, replace=False)
+        pieces = {}
+        for j, c in enumerate(cells):
+            if j < 2:
+                t, owner = W.FLAG, j  # one Flag each
+            else:
+                t, owner = int(rng.integers(1, 13)), int(rng.integers(2))
+                if t == W.FLAG:
+                    t = W.BOMB
+            immobile = t in (W.FLAG, W.BOMB)
+            pieces[int(c)] = W.piece(t, owner, moved=bool(rng.integers(2)) and not immobile, revealed=bool(rng.integers(2)))
+        lines[i] = W.make_line(pieces, ply=int(rng.integers(0, 50)), battleless=int(rng.integers(0, 30)))
+    kw = dict(variant=0, seed=9, max_plies=52, auto_reset=0)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    g.reset_from(_dev(lines)); o.reset_from(lines)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(4):
+        om = o.legal_mask(); oobs = o.encode_obs(); oa = o.sample_uniform(om)
+        assert np.array_equal(_np(g.legal_mask(mask)).view(np.uint32), om), t
+        assert np.array_equal(_np(g.encode_obs(obs).view(torch.int16)).view(np.uint16), oobs), t
+        assert np.array_equal(_np(g.sample_uniform(mask, act)), oa), t
+        live_stuck = (oa < 0) & ((o.get_boards()[:, 120] & 1) == 0)
+        orr, od = o.step(oa)
+        g.step(act, rew, done)
+        assert np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od), t
+        assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+        assert g.check() == o.check() == (B.ILLEGAL_ACTION if live_stuck.any() else 0)
+        g.clear_error(); o.clear_error()
+    reasons = np.bincount((o.get_boards()[:, 120] >> 2) & 7, minlength=6)
+    assert reasons[1] > 0 and reasons[2] > 0 and reasons[4] > 0  # flag captures, no-move wins, ply caps all occurred
