@@ -61,6 +61,8 @@ def lib():
         L.orc_replay_filled.argtypes = [vp]
         L.orc_replay_filled.restype = C.c_int64
         L.orc_sample_indices.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int64, vp]
+        L.orc_search_expand.argtypes = [vp, C.c_int32, C.c_uint64, vp]
+        L.orc_search_policy.argtypes = [vp, vp, C.c_int32, vp, C.c_double, C.c_double, vp, vp, vp]
         L.orc_determinise.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp]
         L.orc_reduce_returns.argtypes = [vp, vp, C.c_int32, vp]
         L.orc_philox.argtypes = [vp, vp, vp]
@@ -218,6 +220,20 @@ def determinise(roots: Env, samples_per_root: int, seed: int, out: Env):
     att = np.zeros(out.n, np.int32)
     _chk(lib().orc_determinise(roots.h, samples_per_root, seed, out.h, _p(att)), "determinise")
     return att
+
+
+def search_expand(roots: Env, rollouts: int, seed: int, out: Env):
+    _chk(lib().orc_search_expand(roots.h, rollouts, seed, out.h), "search_expand")
+
+
+def search_policy(roots: Env, games: Env, rollouts: int, alpha: float, beta: float, pi_theta=None):
+    """-> (qhat, rho, pi_search), float32 [R, 3600] each (computed in double)."""
+    R = roots.n
+    q, rho, pi = (np.zeros((R, 3600), np.float32) for _ in range(3))
+    prior = None if pi_theta is None else np.ascontiguousarray(pi_theta, np.float32)
+    _chk(lib().orc_search_policy(roots.h, games.h, rollouts, None if prior is None else _p(prior), alpha, beta,
+                                 _p(q), _p(rho), _p(pi)), "search_policy")
+    return q, rho, pi
 
 
 def reduce_returns(games: Env, root_side, samples_per_root: int):

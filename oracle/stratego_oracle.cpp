@@ -51,6 +51,7 @@
 //   action a = from*36 + dir*9 + (dist-1); dir 0:+row 1:+col 2:-row 3:-col.
 //   mask bit a -> word a>>5, bit a&31; 113 words per game.
 
+#include <cmath>
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
@@ -775,58 +776,62 @@ int64_t orc_replay_filled(const Replay* r) { return r ? r->filled : -1; }
 // the last entry.  One DETERMINISE stream per output game: draw d = word d&3 of block d>>2,
 // counter (global G, 0, block).  More than 4096 draws -> BAD_STATE.  `attempts` (optional,
 // [R*S]) receives the number of draws used.
+static int determinise_one(const Game& root, uint64_t seed, uint32_t gidx, Game& out, int* draws) {
+  int searcher = root.ply & 1;
+  int H[40], T[40], n = 0;
+  for (int c = 0; c < kCells; ++c) {
+    uint8_t b = root.cell[c];
+    if (is_piece(b) && owner_of(b) != searcher && !(b & B_REVEALED)) {
+      if (n >= 40) return ORC_BAD_STATE;
+      H[n] = c; T[n] = type_of(b); ++n;
+    }
+  }
+  Game gm = root;
+  int freeSq[40], m = n, d = 0;
+  for (int i = 0; i < n; ++i) freeSq[i] = H[i];
+  // 1. Bombs and Flag onto unmoved squares
+  for (int j = 0; j < n; ++j) {
+    if (T[j] != T_BOMB && T[j] != T_FLAG) continue;
+    for (;;) {
+      if (d >= 4096) return ORC_BAD_STATE;
+      uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
+      int idx = (int)bounded(u, (uint32_t)m);
+      int sq = freeSq[idx];
+      if (root.cell[sq] & B_MOVED) continue;  // rejection
+      gm.cell[sq] = (uint8_t)((root.cell[sq] & 0xF0) | T[j]);
+      freeSq[idx] = freeSq[m - 1];
+      --m;
+      break;
+    }
+  }
+  // 2. movable types over the remaining squares
+  int Tm[40], k = 0;
+  for (int j = 0; j < n; ++j)
+    if (T[j] != T_BOMB && T[j] != T_FLAG) Tm[k++] = T[j];
+  if (k != m) return ORC_BAD_STATE;
+  for (int i = k - 1; i >= 1; --i) {
+    if (d >= 4096) return ORC_BAD_STATE;
+    uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
+    int j = (int)bounded(u, (uint32_t)(i + 1));
+    int tmp = Tm[i]; Tm[i] = Tm[j]; Tm[j] = tmp;
+  }
+  for (int i = 0; i < k; ++i) gm.cell[freeSq[i]] = (uint8_t)((root.cell[freeSq[i]] & 0xF0) | Tm[i]);
+  if (draws) *draws = d;
+  out = gm;
+  return ORC_OK;
+}
+
 int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, Env* out, int32_t* attempts) {
   if (!roots || !out || samples_per_root <= 0) return ORC_BAD_ARG;
   int R = roots->cfg.num_games;
   if ((int64_t)R * samples_per_root != out->cfg.num_games) return ORC_BAD_ARG;
-  for (int r = 0; r < R; ++r) {
-    const Game& root = roots->g[r];
-    int searcher = root.ply & 1;
-    int H[40], T[40], n = 0;
-    for (int c = 0; c < kCells; ++c) {
-      uint8_t b = root.cell[c];
-      if (is_piece(b) && owner_of(b) != searcher && !(b & B_REVEALED)) {
-        if (n >= 40) return ORC_BAD_STATE;
-        H[n] = c; T[n] = type_of(b); ++n;
-      }
-    }
+  for (int r = 0; r < R; ++r)
     for (int s = 0; s < samples_per_root; ++s) {
-      int G = r * samples_per_root + s;
-      uint32_t gidx = (uint32_t)(out->cfg.game_base + (uint64_t)G);
-      Game gm = root;
-      int freeSq[40], m = n, d = 0;
-      for (int i = 0; i < n; ++i) freeSq[i] = H[i];
-      // 1. Bombs and Flag onto unmoved squares
-      for (int j = 0; j < n; ++j) {
-        if (T[j] != T_BOMB && T[j] != T_FLAG) continue;
-        for (;;) {
-          if (d >= 4096) return ORC_BAD_STATE;
-          uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
-          int idx = (int)bounded(u, (uint32_t)m);
-          int sq = freeSq[idx];
-          if (root.cell[sq] & B_MOVED) continue;  // rejection
-          gm.cell[sq] = (uint8_t)((root.cell[sq] & 0xF0) | T[j]);
-          freeSq[idx] = freeSq[m - 1];
-          --m;
-          break;
-        }
-      }
-      // 2. movable types over the remaining squares
-      int Tm[40], k = 0;
-      for (int j = 0; j < n; ++j)
-        if (T[j] != T_BOMB && T[j] != T_FLAG) Tm[k++] = T[j];
-      if (k != m) return ORC_BAD_STATE;
-      for (int i = k - 1; i >= 1; --i) {
-        if (d >= 4096) return ORC_BAD_STATE;
-        uint32_t u = stream_draw(seed, gidx, 0, 0, TAG_DETERMINISE, d++);
-        int j = (int)bounded(u, (uint32_t)(i + 1));
-        int tmp = Tm[i]; Tm[i] = Tm[j]; Tm[j] = tmp;
-      }
-      for (int i = 0; i < k; ++i) gm.cell[freeSq[i]] = (uint8_t)((root.cell[freeSq[i]] & 0xF0) | Tm[i]);
+      int G = r * samples_per_root + s, d = 0;
+      int rc = determinise_one(roots->g[r], seed, (uint32_t)(out->cfg.game_base + (uint64_t)G), out->g[G], &d);
+      if (rc != ORC_OK) return rc;
       if (attempts) attempts[G] = d;
-      out->g[G] = gm;
     }
-  }
   return ORC_OK;
 }
 
@@ -844,6 +849,100 @@ int orc_reduce_returns(const Env* games, const uint8_t* root_side, int32_t sampl
       sum += ret; if (ret > 0) ++wins; if (ret < 0) ++losses;
     }
     out[3 * r] = sum; out[3 * r + 1] = wins; out[3 * r + 2] = losses;
+  }
+  return ORC_OK;
+}
+
+// ---- one search step without networks (S3.7; R29)
+// Legal actions of the root's side to move, ascending.
+static int legal_list(const Env* e, const Game& gm, int* list) {
+  if (gm.done) return 0;
+  uint32_t m[kMaskWords];
+  for (int w = 0; w < kMaskWords; ++w) m[w] = 0;
+  gen_moves(gm, e->cfg, gm.ply & 1, m);
+  int L = 0;
+  for (int a = 0; a < 3600; ++a)
+    if (m[a >> 5] & (1u << (a & 31))) list[L++] = a;
+  return L;
+}
+// Steps 1-2: "samples roughly 1,000 / (number of legal actions) possible
+// configurations of the types of the hidden pieces", "at least one rollout for each combination
+// of legal move and sampled opponent configuration.  After the initial move, which is forced,
+// ...".  Root r with L legal actions gets C = max(1, rollouts / L) configurations (the
+// determinisation sampler of C7 stands in for the belief network); slot r*rollouts + c*L + l
+// holds configuration c with the l-th legal action applied; the other slots are frozen.
+int orc_search_expand(const Env* roots, int32_t rollouts, uint64_t seed, Env* out) {
+  if (!roots || !out || rollouts <= 0) return ORC_BAD_ARG;
+  int R = roots->cfg.num_games;
+  if ((int64_t)R * rollouts != out->cfg.num_games || out->cfg.auto_reset) return ORC_BAD_ARG;
+  std::vector<int> list(3600);
+  for (int r = 0; r < R; ++r) {
+    const Game& root = roots->g[r];
+    int L = legal_list(roots, root, list.data());
+    int C = L > 0 ? (rollouts / L > 1 ? rollouts / L : 1) : 0;
+    int64_t used = (int64_t)C * L < rollouts ? (int64_t)C * L : rollouts;
+    for (int s = 0; s < rollouts; ++s) {
+      int G = r * rollouts + s;
+      if (s >= used) {  // unused slot: a frozen game
+        out->g[G] = root;
+        out->g[G].done = true; out->g[G].reason = 0; out->g[G].result = 0;
+        continue;
+      }
+      int c = s / L, l = s % L;
+      uint32_t gidx = (uint32_t)(out->cfg.game_base + (uint64_t)r * rollouts + (uint64_t)c);  // one stream per configuration
+      int rc = determinise_one(root, seed, gidx, out->g[G], nullptr);
+      if (rc != ORC_OK) return rc;
+      int8_t rew; uint8_t dn;
+      step_game(out, G, list[l], &rew, &dn);  // the forced first move
+    }
+  }
+  return ORC_OK;
+}
+// Steps 3-4: qhat(a) = average value over the configurations of the games that
+// started with a - the value is the game's result from the searcher's side once the rollouts
+// are over, 0 if it is still running (stand-in for the move network's value head) - and
+//   pi_search = argmax <qhat, pi> - alpha KL(pi, rho) - beta KL(pi, pi_theta)
+//             \propto [ exp(qhat) rho^alpha pi_theta^beta ]^(1/(alpha+beta))              (7), (8)
+// with rho the magnet policy "that selects a movable piece uniformly at random and then selects
+// a legal move for this piece uniformly at random" and pi_theta the caller's
+// prior over the 3600 actions (nullptr = uniform over the legal ones).  All in double.
+int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, const float* pi_theta, double alpha,
+                      double beta, float* qhat, float* rho, float* pi_search) {
+  if (!roots || !games || rollouts <= 0 || !qhat || !rho || !pi_search || !(alpha + beta > 0)) return ORC_BAD_ARG;
+  int R = roots->cfg.num_games;
+  if ((int64_t)R * rollouts != games->cfg.num_games) return ORC_BAD_ARG;
+  std::vector<int> list(3600);
+  for (int r = 0; r < R; ++r) {
+    float* q = qhat + (size_t)r * 3600; float* rh = rho + (size_t)r * 3600; float* ps = pi_search + (size_t)r * 3600;
+    for (int a = 0; a < 3600; ++a) q[a] = rh[a] = ps[a] = 0.0f;
+    const Game& root = roots->g[r];
+    int L = legal_list(roots, root, list.data());
+    if (L == 0) continue;
+    int C = rollouts / L > 1 ? rollouts / L : 1;
+    int64_t used = (int64_t)C * L < rollouts ? (int64_t)C * L : rollouts;
+    int sign = (root.ply & 1) == 0 ? +1 : -1;
+    int per_cell[kCells] = {0}, pieces = 0;
+    for (int l = 0; l < L; ++l) per_cell[list[l] / 36] += 1;
+    for (int c = 0; c < kCells; ++c) pieces += per_cell[c] > 0;
+    std::vector<double> logit(L);
+    double mx = -1e300;
+    for (int l = 0; l < L; ++l) {
+      int sum = 0, cnt = 0;
+      for (int64_t s = l; s < used; s += L) {
+        const Game& gm = games->g[(size_t)r * rollouts + (size_t)s];
+        sum += gm.done ? gm.result * sign : 0;
+        ++cnt;
+      }
+      double qv = cnt ? (double)sum / cnt : 0.0;
+      double rv = 1.0 / ((double)pieces * per_cell[list[l] / 36]);
+      double pv = pi_theta ? (double)pi_theta[(size_t)r * 3600 + list[l]] : 1.0 / L;
+      q[list[l]] = (float)qv; rh[list[l]] = (float)rv;
+      logit[l] = (qv + alpha * log(rv) + beta * log(pv)) / (alpha + beta);
+      if (logit[l] > mx) mx = logit[l];
+    }
+    double z = 0;
+    for (int l = 0; l < L; ++l) z += exp(logit[l] - mx);
+    for (int l = 0; l < L; ++l) ps[list[l]] = (float)(exp(logit[l] - mx) / z);
   }
   return ORC_OK;
 }
