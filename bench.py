@@ -368,6 +368,52 @@ def run_cfg4(args):
     print(json.dumps(line))
 
 
+def run_search(args):
+    """One network-free search step per root (Table S12: 1,000 rollouts of depth
+    40 over sampled configurations x legal actions, forced first move, eq. 8) for 256 roots at
+    once; uniform policy / game result stand in for the move network's policy / value."""
+    import numpy as np
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    R, rollouts, depth = 256, 1000, 40
+    src = B.Env(R, variant=0, seed=0, max_plies=1000, auto_reset=1)
+    rb = W.capture_at_ply(lambda: src.get_boards().cpu().numpy(), lambda: src.step(src.sample_uniform(src.legal_mask())), R, 200)
+    roots = B.Env(R, variant=0, seed=0)
+    roots.reset_from(torch.from_numpy(rb).cuda())
+    games = B.Env(R * rollouts, variant=0, seed=0, max_plies=0, auto_reset=0)
+    outs = tuple(torch.empty((R, 3600), dtype=torch.float32, device="cuda") for _ in range(3))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    steps = max(1, min(args.steps, 20))
+    t = [0.0, 0.0, 0.0]
+    for k in range(min(args.warmup, 3) + steps):
+        ev[0].record()
+        B.search_expand(roots, rollouts, 500 + k, games)
+        ev[1].record()
+        games.rollout_uniform(depth - 1)
+        ev[2].record()
+        B.search_policy(roots, games, rollouts, 0.002, 0.02, None, outs)
+        ev[3].record()
+        torch.cuda.synchronize()
+        if k >= min(args.warmup, 3):
+            for i in range(3):
+                t[i] += ev[i].elapsed_time(ev[i + 1])
+    assert games.check() == 0 and roots.check() == 0
+    total = sum(t)
+    legal = (outs[2] > 0).sum(dim=1).float().mean().item()
+    line = {
+        "metric": METRIC, "value": R * rollouts * depth * steps / (total / 1e3), "unit": UNIT, "n_gpus": 1, "steps": steps,
+        "warmup": min(args.warmup, 3), "ms_per_step": total / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8 (game), f32 (eq. 8)", "data": "synthetic",
+        "config": {"workload": "search_step_256_roots", "roots": R, "rollouts_per_root": rollouts, "depth": depth,
+                   "ms_expand": t[0] / steps, "ms_rollout": t[1] / steps, "ms_policy": t[2] / steps,
+                   "searched_moves_per_sec": R * steps / (total / 1e3), "mean_legal_actions": legal,
+                   "note": "env-step count includes unused slots' share (rollouts*depth per root); paper: 1.26 s per "
+                           "searched move on one H100 WITH its networks (PAPER.md:200) - context only"},
+        "gpu_launches": 3 * steps,
+    }
+    print(json.dumps(line))
+
+
 def run_hist(args):
     """The paper's own buffer design on the headline workload: the fused step
     records the 128-byte state of every game and step into a 256-step board-history ring
@@ -424,9 +470,10 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist"],
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search"],
                     help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
-                         "hist = cfg2 recording into the board-history ring + historical queries; all 1 GPU")
+                         "hist = cfg2 recording into the board-history ring + historical queries; "
+                         "search = network-free search steps (S3.7) for 256 roots; all 1 GPU")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
     args = ap.parse_args()
@@ -438,6 +485,8 @@ def main():
         run_cfg4(args)
     elif args.workload == "hist":
         run_hist(args)
+    elif args.workload == "search":
+        run_search(args)
     else:
         run_b200(args)
 

@@ -256,6 +256,30 @@ int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t
 int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32_t samples_per_root,
                          int32_t* out, void* stream);
 
+/* ---- one search step without networks (S3.7; R29) -------- */
+/* Steps 1-2: root r with L legal actions gets C = max(1, rollouts / L)
+ * sampled configurations of the opponent's hidden pieces (strat_determinise's sampler stands
+ * in for the belief network, cf. the uniform-belief ablation PAPER.md:277-279) and one game per
+ * (configuration c, legal action l): slot r*rollouts + c*L + l of `out` = configuration c with
+ * the l-th legal action (ascending) applied - the forced first move.  The min(C*L, rollouts)
+ * first slots of a root are used; the rest are frozen finished copies of the root.
+ * out->num_games == roots->num_games * rollouts, out->auto_reset == 0, no history attached.
+ * Then play the remaining depth-1 plies (strat_rollout_uniform: the uniform policy stands in
+ * for the move network) and call strat_search_policy. */
+int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed, strat_env* out, void* stream);
+/* Steps 3-4, float32 [R][3600] each, 0 on illegal actions:
+ *   qhat(a)   = mean over configurations of the value of the game that started with a; the value
+ *               is the game's result from the searcher's side, 0 while it is running (stand-in
+ *               for the move network's value head);
+ *   rho(a)    = magnet policy: 1 / (pieces that can move * moves of a's piece);
+ *   pi_search = [exp(qhat) rho^alpha pi_theta^beta]^(1/(alpha+beta)) normalised over the legal
+ *               actions (eq. 8), the maximiser of <qhat,pi> - alpha KL(pi,rho) - beta KL(pi,pi_theta)
+ *               (eq. 7).  pi_theta: the caller's prior float32 [R][3600] (e.g. the move network's
+ *               policy), or NULL for the uniform distribution over the legal actions.
+ * Paper's values: alpha = 0.002, beta = 0.02, 1,000 rollouts of depth 40 (Table S12). */
+int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
+                        float alpha, float beta, float* qhat, float* rho, float* pi_search, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,6 +30,9 @@
 //   continuous chasing (R#28) pinned: hand-worked chase around a 2x2 block, state-machine
 //                      cases, independent snapshot checker.  The mechanics the paper leaves
 //                      open (what ends a chase, 8-ply memory) are PARITY UNPINNED against it.
+//   search step (R#29)  pinned: expansion structure, hand-computed rho and equal-value limit,
+//                      per-action averaging, KKT conditions of eq. (7) at the eq. (8) output.
+//                      The stand-ins for the networks are this build's (R#29), not the paper's.
 //   pinned reset (R#27) pinned: a restarted game equals its pinned line byte for byte except
 //                      the epoch; the reading itself (epoch keeps counting) is PARITY UNPINNED
 //                      against the paper (P:252-254 gives no detail).

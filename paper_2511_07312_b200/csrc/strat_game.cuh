@@ -527,9 +527,7 @@ STRAT_UNROLL
 }
 // SampleRandomLegalAction, C3a: the r-th set bit of the row, r = bounded(u, n).
 // cnt[i] = set bits in mask words 36i..36i+35, so only one 36-word stretch is scanned.
-SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
-  if (n == 0) return -1;
-  int r = (int)bounded(u, (uint32_t)n);
+SD int pick_rank(const uint32_t* row, const int cnt[4], int r) {
   int w0 = 0;
   if (r >= cnt[0]) { r -= cnt[0]; w0 = 36; if (r >= cnt[1]) { r -= cnt[1]; w0 = 72; if (r >= cnt[2]) { r -= cnt[2]; w0 = 108; } } }
   for (int w = w0; w < kMaskWords; ++w) {
@@ -539,11 +537,10 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
   }
   return -1;
 }
-// SampleRandomLegalAction without materialising the 3600-bit mask (on-chip rollouts): equal to
-// pick_action(legal_mask_row(...)) for the same draw u.  Actions ascend with the from-cell, then
-// the direction, then the distance, so the r-th legal action is found by walking the pieces that
-// can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
-// lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
+SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
+  if (n == 0) return -1;
+  return pick_rank(row, cnt, (int)bounded(u, (uint32_t)n));
+}
 // r-th (from 0) legal action in ascending order, given the per-group counts, the non-Scout
 // direction bits D[group][dir] and the Scouts' packed ray lengths (cell | len0<<8 | .. | len3<<20).
 SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r) {
