@@ -82,7 +82,8 @@ typedef struct strat_config {
   int32_t device;         /* CUDA device ordinal */
   int32_t chase_rule;     /* 1: apply the continuous-chasing rule (R28: a
                              chasing player may not make a threat that recreates a position of
-                             the chase's last 8 plies, except by moving straight back), 0: off */
+                             the chase, except by moving straight back; memory: 63 plies played in
+                             this environment + the 8 plies a loaded line carries), 0: off */
   uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded) */
 } strat_config;
 

@@ -109,6 +109,11 @@ struct Game {
   // Continuous-chasing state machine (R#28): number of positions of the player's
   // running chase, counted from the one right after its first threat; 0 = not chasing.
   int chase_age[2];
+  // Move log of the chasing rule's memory: the last 64 plies played since this state was
+  // set up or loaded (circular by logn).  Not part of the canonical line: a loaded state
+  // remembers the 8 plies its line carries.
+  int logn;
+  uint8_t log[64][2];
 };
 
 struct Env {
@@ -225,6 +230,7 @@ void clear_dynamic(Game& gm) {
   gm.ply = 0; gm.battleless = 0; gm.done = false; gm.reason = 0; gm.result = 0;
   gm.chain_len[0] = gm.chain_len[1] = 0;
   gm.chase_age[0] = gm.chase_age[1] = 0;
+  gm.logn = 0;
 }
 
 void new_game(const Config& cfg, uint32_t gidx, Game& gm) {  // epoch already set
@@ -302,7 +308,7 @@ bool is_evade(const Game& gm, int side, int from, int to) {
 // square it occupied prior to the previous turn of the chasing player".  A position is
 // the type and owner of the piece on every square.  The chase's earlier positions are rebuilt
 // by taking back the logged plies one by one (no battle happens inside a chase); the state
-// remembers 8 plies (R#28).
+// remembers the 8 plies of its line and up to 63 plies played since it was loaded (R#28).
 bool chase_banned(const Game& gm, int side, int from, int to) {
   int age = gm.chase_age[side];
   if (age < 2) return false;
@@ -312,10 +318,18 @@ bool chase_banned(const Game& gm, int side, int from, int to) {
   uint8_t R[kCells], K[kCells];
   for (int c = 0; c < kCells; ++c) R[c] = K[c] = (uint8_t)(gm.cell[c] & 0x1F);
   R[to] = R[from]; R[from] = 0;
-  int back = age - 1 < 8 ? age - 1 : 8;
-  for (int b = 1; b <= back; ++b) {
-    if (gm.hist[b - 1][0] == 0xFF) break;
-    int f = gm.hist[b - 1][0], g = gm.hist[b - 1][1];
+  // look-back b = 1 takes the last ply back, b = 2 the one before, ...: plies 1..8 are in the
+  // line's history, plies up to 63 in the move log if that many were played since the load
+  for (int b = 1; b <= age - 1; ++b) {
+    int f, g;
+    if (b <= 8) {
+      if (gm.hist[b - 1][0] == 0xFF) break;
+      f = gm.hist[b - 1][0]; g = gm.hist[b - 1][1];
+    } else if (b <= gm.logn && b <= 63) {
+      f = gm.log[(gm.logn - b) & 63][0]; g = gm.log[(gm.logn - b) & 63][1];
+    } else {
+      break;
+    }
     K[f] = K[g]; K[g] = 0;  // take the ply back
     if (memcmp(R, K, kCells) == 0) return true;
   }
@@ -429,6 +443,8 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
   }
   for (int j = 7; j >= 1; --j) { gm.hist[j][0] = gm.hist[j - 1][0]; gm.hist[j][1] = gm.hist[j - 1][1]; }
   gm.hist[0][0] = (uint8_t)from; gm.hist[0][1] = (uint8_t)to;
+  gm.log[gm.logn & 63][0] = (uint8_t)from; gm.log[gm.logn & 63][1] = (uint8_t)to;
+  gm.logn += 1;
   // 2. mover's bits.
   uint8_t P = gm.cell[from] | B_MOVED;
   if (dist >= 2) P |= B_REVEALED;  // R#10
@@ -534,6 +550,7 @@ void read_line(const uint8_t* L, Game& gm) {
   gm.reason = (L[120] >> 2) & 7;
   gm.result = (int8_t)L[121];
   gm.chase_age[0] = L[122]; gm.chase_age[1] = L[123];
+  gm.logn = 0;
   gm.epoch = (uint32_t)L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
   rebuild_chains(gm);
 }
@@ -821,6 +838,7 @@ static int determinise_one(const Game& root, uint64_t seed, uint32_t gidx, Game&
   for (int i = 0; i < k; ++i) gm.cell[freeSq[i]] = (uint8_t)((root.cell[freeSq[i]] & 0xF0) | Tm[i]);
   if (draws) *draws = d;
   out = gm;
+  out.logn = 0;  // a copied state remembers the 8 plies of its line
   return ORC_OK;
 }
 

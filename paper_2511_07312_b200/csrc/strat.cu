@@ -224,7 +224,8 @@ __global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __r
   if (lane < ng) {
     Game g; read_game(s_state, lane, g);
     int cnt[4];
-    if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), s_mask + lane * kMaskWords, cnt);
+    if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), s_mask + lane * kMaskWords, cnt,
+                                kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
   }
   __syncwarp();
   store_mask(mask, first, ng, s_mask, lane);
@@ -483,7 +484,7 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   if ((rs >> lane) & 1u) {
     g.mvd = g.rev = bb_zero();
     hist_clear(g);
-    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0;
+    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
     if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
   }
   __syncwarp();
@@ -550,7 +551,8 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       PROF_T(t2);
       bool reset_me = false;
       if (!kExternal) {
-        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt);
+        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
+                                                       kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
         __syncwarp();
         PROF_T(t3);
         if (mask) store_mask(mask, first, ng, work, lane);
@@ -591,7 +593,9 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         }
         if (lane < ng) {
           store_game_global(lines, first + lane, g);
-          if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt);  // of the NEW state
+          if (!g.done)  // of the NEW state
+            legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
+                           kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
         }
         __syncwarp();
         if (mask) store_mask(mask, first, ng, work, lane);
@@ -645,7 +649,7 @@ __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __re
     for (int t = 0; t < plies; ++t) {
       if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
       int a = sample_action_direct(g, g.ply & 1u, rules_of<kChase>(P), action_draw(P, (uint32_t)(first + lane), g),
-                                   s_scouts + lane * kScoutScratch);
+                                   s_scouts + lane * kScoutScratch, kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
       if (step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
         raise_error(err, STRAT_ILLEGAL_ACTION);
         break;
@@ -775,7 +779,8 @@ __global__ void __launch_bounds__(32) k_search_expand(Params Pr, Params Po, int 
     unpack_line(W, root);
     uint32_t* row = s_mask + lane * kMaskWords;
     int cnt[4] = {0, 0, 0, 0};
-    int L = root.done ? 0 : legal_mask_row(root, root.ply & 1u, rules_of<kChase>(Pr), row, cnt);
+    int L = root.done ? 0 : legal_mask_row(root, root.ply & 1u, rules_of<kChase>(Pr), row, cnt,
+                                           kChase ? game_log(Pr, (uint32_t)r) : nullptr);
     int C = L > 0 ? max(1, rollouts / L) : 0;
     int used = min(C * L, rollouts);
     if (s >= used) {  // unused slot: the root, frozen
@@ -823,7 +828,8 @@ __global__ void __launch_bounds__(kPolicyThreads) k_search_policy(Params Pr, int
     Game root;
     unpack_line(W, root);
     int cnt[4] = {0, 0, 0, 0};
-    int L = root.done ? 0 : legal_mask_row(root, root.ply & 1u, rules_of<kChase>(Pr), s_row, cnt);
+    int L = root.done ? 0 : legal_mask_row(root, root.ply & 1u, rules_of<kChase>(Pr), s_row, cnt,
+                                           kChase ? game_log(Pr, (uint32_t)r) : nullptr);
     int k = 0, pieces = 0;
     for (int w = 0; w < kMaskWords; ++w)
       for (uint32_t b = s_row[w]; b; b &= b - 1) {
@@ -872,6 +878,12 @@ __global__ void __launch_bounds__(kPolicyThreads) k_search_policy(Params Pr, int
   for (int l = tid; l < L; l += kPolicyThreads) ps[s_legal[l]] = logit[l] / z;
 }
 
+// A state copied in from elsewhere (history ring) has no move log here: it remembers 8 plies.
+__global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict__ lines) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < n) lines[(size_t)g * kLineWords + 31] = 0;
+}
+
 __global__ void k_set_int(int* p, int v) { *p = v; }
 
 // ------------------------------------------------------------------ host side
@@ -888,6 +900,7 @@ inline Params make_params(const strat_config& c) {
   P.ply_cap = (c.max_plies >= 1 && c.max_plies <= 65535) ? c.max_plies : 65535;
   P.max_battleless = c.max_battleless; P.auto_reset = c.auto_reset ? 1 : 0; P.two_square = c.two_square ? 1 : 0;
   P.chase_rule = c.chase_rule ? 1 : 0;
+  P.movelog = nullptr;
   P.pin = nullptr;
   return P;
 }
@@ -1014,7 +1027,8 @@ const char* strat_error_string(int code) {
 
 size_t strat_workspace_bytes(const strat_config* cfg) {
   if (!cfg_ok(cfg)) return 0;
-  return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256 + align_up(sync_words(cfg->num_games) * 4, 256);
+  return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256 + align_up(sync_words(cfg->num_games) * 4, 256) +
+         (cfg->chase_rule ? (size_t)cfg->num_games * kLogPlies * 2 : 0);  // move logs: the chasing rule's memory
 }
 
 int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream, strat_env** out) {
@@ -1034,6 +1048,8 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->f_obs = e->f_state + batches(cfg->num_games);
   e->version = 0;
   e->hist = nullptr;
+  if (cfg->chase_rule)
+    e->P.movelog = reinterpret_cast<uint16_t*>(reinterpret_cast<uint8_t*>(e->tickets) + align_up(sync_words(cfg->num_games) * 4, 256));
   if (cudaMemsetAsync(e->tickets, 0, sync_words(cfg->num_games) * 4, (cudaStream_t)stream) != cudaSuccess) {
     delete e;
     return STRAT_CUDA_ERROR;
@@ -1055,8 +1071,10 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   cudaStream_t s = (cudaStream_t)stream;
   env->cfg.seed = seed;
   const uint32_t* pin = env->P.pin;
+  uint16_t* movelog = env->P.movelog;
   env->P = make_params(env->cfg);
   env->P.pin = pin;
+  env->P.movelog = movelog;
   k_set_int<<<1, 1, 0, s>>>(env->err, 0);
   k_reset<<<batches(env->P.num_games), 32, 0, s>>>(env->P, env->lines);
   return launch_status();
@@ -1344,7 +1362,8 @@ int strat_history_current_step(const strat_history* h, int64_t* step) {
 int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream) {
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !mask) return STRAT_BAD_ARG;
-  const Params& P = h->env ? h->env->P : h->P;
+  Params P = h->env ? h->env->P : h->P;
+  if (t != h->cur) P.movelog = nullptr;  // a past state is judged with the 8 plies its line remembers
   if (P.chase_rule) k_legal_mask<true><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
   else k_legal_mask<false><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
   return launch_status();
@@ -1385,8 +1404,10 @@ int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* s
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream) {
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !env || env->P.num_games != h->num_games) return STRAT_BAD_ARG;
-  if (L != env->lines)
+  if (L != env->lines) {
     copy_elems<uint32_t>(L, env->lines, (size_t)h->num_games * kLineWords, (cudaStream_t)stream);
+    k_clear_logn<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, env->lines);
+  }
   return launch_status();
 }
 

@@ -23,6 +23,8 @@ static inline uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return (uint32_
 static inline int min(int a, int b) { return a < b ? a : b; }
 static inline int max(int a, int b) { return a > b ? a : b; }
 #define STRAT_UNROLL
+static inline uint16_t sd_ldlog(const uint16_t* p) { return *p; }
+static inline void sd_stlog(uint16_t* p, uint16_t v) { *p = v; }
 #else
 #define STRAT_UNROLL _Pragma("unroll")
 #define SD __device__ __forceinline__
@@ -32,6 +34,9 @@ SD int sd_clz(uint32_t x) { return __clz((int)x); }
 SD uint32_t sd_mulhi(uint32_t a, uint32_t b) { return __umulhi(a, b); }
 SD uint32_t sd_fsr(uint32_t lo, uint32_t hi, int s) { return __funnelshift_r(lo, hi, s); }
 SD uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return __funnelshift_l(lo, hi, s); }
+// move-log accesses go to L2: consecutive launches of the fused step overlap on the device
+SD uint16_t sd_ldlog(const uint16_t* p) { return __ldcg(p); }
+SD void sd_stlog(uint16_t* p, uint16_t v) { __stcg(p, v); }
 #endif
 
 namespace strat {
@@ -44,6 +49,8 @@ constexpr int REASON_FLAG = 1, REASON_NOMOVE_WIN = 2, REASON_NOMOVE_DRAW = 3, RE
               REASON_BATTLELESS = 5;
 constexpr uint32_t TAG_SETUP_RED = 0, TAG_SETUP_BLUE = 1, TAG_ACTION = 2, TAG_SAMPLE = 3, TAG_DETERMINISE = 4;
 constexpr uint32_t kHistNone = 0x3FFF;
+constexpr int kLogPlies = 64;  // move-log entries per game; the chasing rule looks back 63 plies at most
+constexpr int kMaxBans = 63;
 
 struct Params {  // per-environment constants handed to every kernel by value
   uint32_t key0, key1;     // Philox key = seed
@@ -55,6 +62,7 @@ struct Params {  // per-environment constants handed to every kernel by value
   int32_t auto_reset;
   int32_t two_square;
   int32_t chase_rule;      // continuous-chasing rule (R#28)
+  uint16_t* movelog;       // [num_games][64] plies played since the state was loaded (chase_rule only), or null
   const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
 };
 
@@ -63,6 +71,11 @@ constexpr int RULE_TWO_SQUARE = 1, RULE_CHASE = 2;
 // kChase = false compiles the (rare, register-hungry) chasing-rule paths out of a kernel.
 template <bool kChase> SD int rules_of(const Params& P) {
   return (P.two_square ? RULE_TWO_SQUARE : 0) | ((kChase && P.chase_rule) ? RULE_CHASE : 0);
+}
+
+// The move log of one game (chasing rule's memory), or null when the environment keeps none.
+SD uint16_t* game_log(const Params& P, uint32_t local_game) {
+  return P.movelog ? P.movelog + (size_t)local_game * 64 : nullptr;
 }
 
 // ------------------------------------------------------------------ 100-bit boards
@@ -169,7 +182,8 @@ SD uint32_t bounded(uint32_t u, uint32_t n) { return sd_mulhi(u, n); }
 // bits: planes 0..3 carry history entries 2p (bits 4..17) and 2p+1 (bits 18..31), an entry
 // being from | to<<7 (0x3FFF = none); plane 4 carries flags (bit 4 done, bits 5..7 reason,
 // bits 8..9 result+1).  Word 28 = ply | battleless<<16, word 29 = epoch, word 30 = chase age of
-// red | blue<<8 (R#28), word 31 zero.
+// red | blue<<8 (R#28), word 31 = plies in the game's move log (device only; a line that is
+// imported or copied to another environment starts with 0).
 struct Game {
   BB t0, t1, t2, t3, own, mvd, rev;
   uint32_t h[4];
@@ -177,6 +191,7 @@ struct Game {
   int32_t result;
   uint32_t ply, battleless, epoch;
   uint32_t chase;  // chase age of red | blue << 8: positions of the player's running chase (0 = none)
+  uint32_t logn;   // plies appended to this game's move log since the state was set up / loaded
 };
 
 SD void unpack_line(const uint32_t* W, Game& g) {
@@ -191,7 +206,7 @@ SD void unpack_line(const uint32_t* W, Game& g) {
   for (int p = 0; p < 4; ++p) g.h[p] = W[4 * p + 3] >> 4;
   uint32_t f = W[19] >> 4;
   g.done = f & 1u; g.reason = (f >> 1) & 7u; g.result = (int32_t)((f >> 4) & 3u) - 1;
-  g.ply = W[28] & 0xFFFFu; g.battleless = W[28] >> 16; g.epoch = W[29]; g.chase = W[30] & 0xFFFFu;
+  g.ply = W[28] & 0xFFFFu; g.battleless = W[28] >> 16; g.epoch = W[29]; g.chase = W[30] & 0xFFFFu; g.logn = W[31];
 }
 SD void pack_line(const Game& g, uint32_t* W) {
   const BB* pl[7] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own, &g.mvd, &g.rev};
@@ -202,7 +217,7 @@ SD void pack_line(const Game& g, uint32_t* W) {
   STRAT_UNROLL
   for (int p = 0; p < 4; ++p) W[4 * p + 3] |= g.h[p] << 4;
   W[19] |= (g.done | (g.reason << 1) | ((uint32_t)(g.result + 1) << 4)) << 4;
-  W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = g.chase; W[31] = 0;
+  W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = g.chase; W[31] = g.logn;
 }
 SD uint32_t hist_entry(const Game& g, int j) { return (g.h[j >> 1] >> (14 * (j & 1))) & 0x3FFFu; }
 SD void hist_push(Game& g, uint32_t e) {
@@ -270,22 +285,25 @@ SD BB neighbours_of(int c) {
   return bb_or(bb_or(bb_up<10>(one), bb_down<10>(one)),
                bb_or(bb_and(bb_up<1>(one), bb_const(kNotCol0)), bb_and(bb_down<1>(one), bb_const(kNotCol9))));
 }
-// The moves of `side` that the chasing rule bans in this position (at most 8: every earlier
-// position of the chase within the 8 logged plies can be recreated by at most one move).
+// The moves of `side` that the chasing rule bans in this position (at most one per earlier
+// position of the chase: it can be recreated by at most one move).
 // A position is the type and owner on every square.  Earlier positions are rebuilt by taking
 // the logged plies back on copies of the five type/owner planes (no battle happens inside a
 // chase); position t-b is recreated by the move c->a iff it differs from the current one on
 // exactly the squares {c, a}, with the current piece of c standing on a.
 // Returned: action indices (the caller still checks that they are otherwise legal).
-SD int chase_banned_actions(const Game& g, int side, BB mine, BB enemy, int banned[8]) {
+SD int chase_banned_actions(const Game& g, int side, BB mine, BB enemy, const uint16_t* glog, int banned[kMaxBans]) {
   int age = (int)chase_age(g, side);
   if (age < 2) return 0;
   int first = ((int)(g.ply & 1u) == side) ? 1 : 0;
   uint32_t eprev = hist_entry(g, first);  // this player's previous ply
-  int back = min(age - 1, 8), nb = 0;
+  int back = min(age - 1, kMaxBans), nb = 0;
+  int logged = glog ? (int)min(g.logn, (uint32_t)(kLogPlies - 1)) : 0;
   BB k[5] = {g.t0, g.t1, g.t2, g.t3, g.own};
   for (int b = 1; b <= back; ++b) {
-    uint32_t e = hist_entry(g, b - 1);
+    // plies 1..8 back are in the line's history, older ones in the game's move log
+    uint32_t e = b <= 8 ? hist_entry(g, b - 1)
+               : b <= logged ? (uint32_t)sd_ldlog(glog + ((g.logn - (uint32_t)b) & (kLogPlies - 1))) : kHistNone;
     if (e == kHistNone) break;
     CellSel sf = cell_sel((int)(e & 127u)), st = cell_sel((int)(e >> 7));
     STRAT_UNROLL
@@ -421,7 +439,7 @@ SD bool move_in_moves(const Moves& m, int a) {
   return dist <= ld;
 }
 // Distinct actions of banned[0..nb) that are legal in m, compacted in place; returns their number.
-SD int keep_legal_banned(const Moves& m, int banned[8], int nb) {
+SD int keep_legal_banned(const Moves& m, int banned[kMaxBans], int nb) {
   int k = 0;
   for (int i = 0; i < nb; ++i) {
     bool dup = false;
@@ -430,13 +448,13 @@ SD int keep_legal_banned(const Moves& m, int banned[8], int nb) {
   }
   return k;
 }
-SD bool has_legal_move(const Game& g, int side, int rules) {
+SD bool has_legal_move(const Game& g, int side, int rules, const uint16_t* glog = nullptr) {
   Moves m; single_step_moves(g, side, rules, m);
   if (!has_single_step_move(m)) return false;
   if (!(rules & RULE_CHASE) || chase_age(g, side) < 2) return true;
   BB occ = occupied(g), mine = owned_by(g, occ, side);
-  int banned[8];
-  int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+  int banned[kMaxBans];
+  int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), glog, banned);
   if (nb == 0) return true;
   nb = keep_legal_banned(m, banned, nb);
   int total = 0;  // every legal move without the chasing rule
@@ -466,7 +484,7 @@ SD void mask_or_field(uint32_t* row, int c, uint64_t field) {  // the 36 action 
 // Legal mask of `side` into `row` (113 words, already zero).  Returns the number of legal
 // actions and, in cnt[i], how many of them start from cells 32i..32i+31 (= mask words
 // 36i..36i+35; used by pick_action).  a = from*36 + dir*9 + dist-1.
-SD int legal_mask_row(const Game& g, int side, int rules, uint32_t* row, int cnt[4]) {
+SD int legal_mask_row(const Game& g, int side, int rules, uint32_t* row, int cnt[4], const uint16_t* glog = nullptr) {
   Moves m; single_step_moves(g, side, rules, m);
   // pieces that move one square: four bits per piece, no branches
   STRAT_UNROLL
@@ -500,8 +518,8 @@ SD int legal_mask_row(const Game& g, int side, int rules, uint32_t* row, int cnt
   }
   if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: take the chase-banned threats out
     BB occ = occupied(g), mine = owned_by(g, occ, side);
-    int banned[8];
-    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    int banned[kMaxBans];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), glog, banned);
     for (int i = 0; i < nb; ++i) {
       uint32_t bit = 1u << (banned[i] & 31);
       int w = banned[i] >> 5, grp = (banned[i] / 36) >> 5;
@@ -575,7 +593,8 @@ SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t
 // the direction, then the distance, so the r-th legal action is found by walking the pieces that
 // can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
 // lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
-SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint32_t* scouts) {
+SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint32_t* scouts,
+                            const uint16_t* glog = nullptr) {
   Moves m; single_step_moves(g, side, rules, m);
   uint32_t D[4][4];
   int cnt[4], ns = 0;
@@ -601,8 +620,8 @@ SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint
   if (n == 0) return -1;
   if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: skip the chase-banned threats
     BB occ = occupied(g), mine = owned_by(g, occ, side);
-    int banned[8];
-    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    int banned[kMaxBans];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), glog, banned);
     nb = keep_legal_banned(m, banned, nb);
     if (nb > 0) {
       if (n == nb) return -1;
@@ -626,13 +645,13 @@ SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
 }
 
 // Is action a legal for the side to move?  (step validates what it is given)
-SD bool action_is_legal(const Game& g, int side, int rules, int a) {
+SD bool action_is_legal(const Game& g, int side, int rules, int a, const uint16_t* glog = nullptr) {
   Moves m; single_step_moves(g, side, rules, m);
   if (!move_in_moves(m, a)) return false;
   if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {
     BB occ = occupied(g), mine = owned_by(g, occ, side);
-    int banned[8];
-    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), banned);
+    int banned[kMaxBans];
+    int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), glog, banned);
     for (int i = 0; i < nb; ++i)
       if (banned[i] == a) return false;
   }
@@ -678,7 +697,7 @@ SD bool side_can_ever_move(const Game& t, int side) {
 SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
   g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
   hist_clear(g);
-  g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0;
+  g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
   uint32_t gidx = P.game_base + local_game;
   for (int side = 0; side < 2; ++side) {
     for (uint32_t attempt = 0;; ++attempt) {
@@ -738,7 +757,8 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   // a live game without a legal move (only a hand-built line can be one: play ends such games)
   // has no action to take: the "action" -1 is illegal like any other
   if (!kValidate && a < 0) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
-  if (kValidate && !action_is_legal(g, side, rules_of<kChase>(P), a)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
+  uint16_t* glog = kChase ? game_log(P, local_game) : nullptr;
+  if (kValidate && !action_is_legal(g, side, rules_of<kChase>(P), a, glog)) { o.reward = 0; o.done = 0; o.illegal = true; return o; }
   int from = a / 36, rem = a - 36 * from, d = rem / 9, dist = rem - 9 * d + 1;
   int to = from + dist * (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
   CellSel sf = cell_sel(from), st = cell_sel(to);
@@ -761,6 +781,8 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
       ap = threat ? (ap > 0 ? (ap < 255u ? ap + 1u : 255u) : 1u) : 0u;
     }
     g.chase = side == 0 ? (ap | (aq << 8)) : (aq | (ap << 8));
+    if (glog) sd_stlog(glog + (g.logn & (uint32_t)(kLogPlies - 1)), (uint16_t)((uint32_t)from | ((uint32_t)to << 7)));
+    g.logn += 1;
   }
   hist_push(g, (uint32_t)from | ((uint32_t)to << 7));
   // the origin square empties in every case
@@ -791,9 +813,9 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   int mover_result = side == 0 ? 1 : -1;
   // terminal tests in R#12 order
   if (flag_captured) { g.done = 1; g.reason = REASON_FLAG; g.result = mover_result; }
-  else if (!has_legal_move(g, side ^ 1, rules_of<kChase>(P))) {
+  else if (!has_legal_move(g, side ^ 1, rules_of<kChase>(P), glog)) {
     g.done = 1;
-    if (!has_legal_move(g, side, rules_of<kChase>(P))) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
+    if (!has_legal_move(g, side, rules_of<kChase>(P), glog)) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
     else { g.reason = REASON_NOMOVE_WIN; g.result = mover_result; }
   }
   else if ((int)g.ply >= P.ply_cap) { g.done = 1; g.reason = REASON_PLY_CAP; g.result = 0; }
@@ -910,6 +932,7 @@ SD void import_canonical(const uint8_t* L, Game& g) {
   g.battleless = L[118] | ((uint32_t)L[119] << 8);
   g.done = L[120] & 1u; g.reason = (L[120] >> 2) & 7u; g.result = (int32_t)(int8_t)L[121];
   g.chase = L[122] | ((uint32_t)L[123] << 8);
+  g.logn = 0;
   g.epoch = L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
 }
 SD void export_canonical(const Game& g, uint8_t* L) {
@@ -952,6 +975,7 @@ SD uint32_t next_draw(DrawStream& s) {
 }
 SD int determinise_game(const Game& root, uint32_t k0, uint32_t k1, uint32_t gidx, Game& out) {
   out = root;
+  out.logn = 0;  // the copy lives in another environment: it remembers the 8 plies of its line
   int searcher = root.ply & 1u;
   BB occ = occupied(root);
   BB enemy = bb_andn(occ, owned_by(root, occ, searcher));

@@ -29,6 +29,8 @@ def test_host_only_entry_points():
     cfg = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0)
     ws = L.strat_workspace_bytes(C.byref(cfg))  # lines + error block + ticket ring + 2 flags per 32-game batch
     assert ws == 65536 * 128 + 256 + (8192 + 2 * 2048) * 4
+    chase = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 1, 0)  # + a 64-ply move log per game
+    assert L.strat_workspace_bytes(C.byref(chase)) == ws + 65536 * 128
     bad = binding.strat_config(0, 0, 0, 0, 0, 0, 1, 0, 0, 0)
     assert L.strat_workspace_bytes(C.byref(bad)) == 0
     assert L.strat_error_string(-4) == b"illegal action for a live game"

@@ -54,6 +54,72 @@ def _scenario_boards(n, seed):
     return lines
 
 
+def test_chase_around_a_lake_on_gpu_every_kernel():
+    """One lap (24 plies) around the lake {42,43,52,53}: the 13th threat repeats the position after
+    the first one.  The plies are fed through strat_step / strat_step_observe; the ban must then
+    show in strat_legal_mask, the fused step's mask, step validation and the on-chip sampler."""
+    ring = [31, 32, 33, 34, 44, 54, 64, 63, 62, 61, 51, 41]
+    pieces = {ring[0]: W.piece(W.CAPTAIN, W.RED), ring[2]: W.piece(W.SERGEANT, W.BLUE), 9: W.piece(W.FLAG, W.RED),
+              99: W.piece(W.FLAG, W.BLUE)}
+
+    def act(a, b):
+        return A(a, {10: 0, 1: 1, -10: 2, -1: 3}[b - a], 1)
+
+    n = 64  # the same game 64 times: on-chip sampling over many action streams
+    kw = dict(seed=3, chase_rule=1)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    lines = np.repeat(W.make_line(pieces)[None, :], n, axis=0)
+    g.reset_from(_dev(lines)); o.reset_from(lines)
+    mask, rew, done, obs = g.new_mask(), g.new_reward(), g.new_done(), g.new_obs()
+    for k in range(12):
+        for a in (act(ring[k % 12], ring[(k + 1) % 12]), act(ring[(k + 2) % 12], ring[(k + 3) % 12])):
+            acts = np.full(n, a, np.int16)
+            o.step(acts)
+            if k % 2:
+                g.step(_dev(acts), rew, done)
+            else:
+                g.step_observe(_dev(acts), rew, done, mask, obs)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert tuple(o.get_boards()[0][122:124]) == (24, 0)
+    om = o.legal_mask()
+    again = act(ring[0], ring[1])
+    assert again not in W.mask_to_actions(om[0])
+    assert np.array_equal(_mask_np(g.legal_mask()), om)
+    # fused step: same mask, same sampled actions; on-chip: same resulting boards
+    g2 = B.Env(n, **kw)
+    g2.reset_from(g.get_boards().clone())  # a loaded state forgets the lap: the move is legal again
+    assert again in W.mask_to_actions(_mask_np(g2.legal_mask())[0])
+    act_t = g.new_actions()
+    oa = o.sample_uniform(om); o.step(oa)
+    g.rollout_step(mask, act_t, rew, done, obs)
+    assert np.array_equal(_mask_np(mask), om) and np.array_equal(_np(act_t), oa)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == 0
+
+
+def test_onchip_rollout_respects_a_long_chase_ban():
+    """Same lap, then ONE on-chip ply for 4,096 copies with different action streams: none may
+    play the banned move; the boards equal the oracle's."""
+    ring = [31, 32, 33, 34, 44, 54, 64, 63, 62, 61, 51, 41]
+    pieces = {ring[0]: W.piece(W.CAPTAIN, W.RED), ring[2]: W.piece(W.SERGEANT, W.BLUE), 9: W.piece(W.FLAG, W.RED),
+              99: W.piece(W.FLAG, W.BLUE)}
+    n = 4096
+    kw = dict(seed=11, chase_rule=1)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    lines = np.repeat(W.make_line(pieces)[None, :], n, axis=0)
+    g.reset_from(_dev(lines)); o.reset_from(lines)
+    rew, done = g.new_reward(), g.new_done()
+    for k in range(12):
+        for f, t in ((ring[k % 12], ring[(k + 1) % 12]), (ring[(k + 2) % 12], ring[(k + 3) % 12])):
+            acts = np.full(n, A(f, {10: 0, 1: 1, -10: 2, -1: 3}[t - f], 1), np.int16)
+            o.step(acts); g.step(_dev(acts), rew, done)
+    g.rollout_uniform(1)
+    oa = o.sample_uniform(o.legal_mask()); o.step(oa)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert (oa != A(ring[0], 1, 1)).all() and len(set(oa.tolist())) == 3  # the three other moves of X all occur
+    assert g.check() == 0
+
+
 def _biased_actions(masks, boards, rng):
     """Test-side policy that keeps chases alive: prefer moves to empty squares next to an enemy
     piece (threats), then any non-capturing move, rarely anything.  Layout arithmetic only."""

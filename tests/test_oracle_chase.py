@@ -55,6 +55,34 @@ def test_chase_around_a_block_bans_the_repeating_threat():
     assert o.check() == orc.ILLEGAL_ACTION and np.array_equal(o.get_boards(), before)
 
 
+def test_chase_around_a_lake_is_caught_after_one_lap():
+    """The classic: X chases Y around the lake {42,43,52,53}.  The ring of 12 squares is walked
+    once in 24 plies; the 13th threat would recreate the position after the first one."""
+    ring = [31, 32, 33, 34, 44, 54, 64, 63, 62, 61, 51, 41]
+    pieces = {ring[0]: W.piece(CAPTAIN, W.RED), ring[2]: W.piece(SERGEANT, W.BLUE), 9: W.piece(FLAG, W.RED),
+              99: W.piece(FLAG, W.BLUE)}
+
+    def act(a, b):
+        d = {10: 0, 1: 1, -10: 2, -1: 3}[b - a]
+        return A(a, d, 1)
+
+    for rule in (1, 0):
+        o = _env(pieces, chase_rule=rule)
+        for k in range(12):
+            _play(o, [act(ring[k % 12], ring[(k + 1) % 12])])        # X steps next to Y: threat
+            _play(o, [act(ring[(k + 2) % 12], ring[(k + 3) % 12])])  # Y steps on: evade
+        line = o.get_boards()[0]
+        assert (line[122], line[123]) == ((24, 0) if rule else (0, 0))
+        legal = _legal(o)
+        again = act(ring[0], ring[1])                                 # X is back on ring[0], Y on ring[2]
+        back = act(ring[0], ring[11])                                 # X's return move: no threat here anyway
+        assert (again in legal) == (rule == 0) and back in legal
+        # a state loaded from its canonical line remembers 8 plies only: the lap is forgotten
+        o2 = orc.Env(1, chase_rule=rule)
+        o2.reset_from(o.get_boards())
+        assert again in _legal(o2)
+
+
 def test_chase_state_machine_on_hand_built_plies():
     o = _env(BLOCK)
     ages = []
@@ -124,7 +152,7 @@ class SnapshotChecker:
         r = list(board)
         r[t], r[f] = r[f], 0
         now = len(self.pos) - 1
-        lo = max(self.start[side], now - 8)
+        lo = max(self.start[side], now - 63)  # the move log remembers 63 plies
         return tuple(r) in self.pos[lo:now]
 
     def push(self, side, f, t):
