@@ -172,6 +172,7 @@ def run_b200(args):
     n = CFG["num_games"]
     kw = W.shard_for_rank(CFG, rank, world)  # weak scaling: n independent games per rank, no data-path collective
     kw["device"] = local
+    kw["chase_rule"] = 1 if args.chase_rule else 0
     env = B.Env(n, **kw)
     mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
     stream = torch.cuda.current_stream()
@@ -225,7 +226,8 @@ def run_b200(args):
             "ms_per_step": total_ms_max / args.steps, "median_ms_per_step": median_ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": CFG["name"], "games_per_gpu": n, "variant": "classic", "max_plies": CFG["max_plies"],
-                       "auto_reset": 1, "policy": "uniform-random legal (Philox4x32-10)",
+                       "auto_reset": 1, "chase_rule": 1 if args.chase_rule else 0,
+                       "policy": "uniform-random legal (Philox4x32-10)",
                        "parallelism": "games sharded over %d GPU(s), no collective" % world,
                        "l2": "outputs 623 MB/step per GPU > 126 MB L2 (no flush needed)"},
             "roofline": {"bound": "hbm", "kernel": "k_rollout_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -474,6 +476,9 @@ def main():
                     help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
                          "hist = cfg2 recording into the board-history ring + historical queries; "
                          "search = network-free search steps (S3.7) for 256 roots; all 1 GPU")
+    ap.add_argument("--chase-rule", action="store_true",
+                    help="cfg2 with the continuous-chasing rule on (not a BASELINE.json config; the paper's simulator goal "
+                         "of ~10 M updates/s is stated with its anti-chasing rules on, PAPER.md:228)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
     args = ap.parse_args()
