@@ -5,8 +5,9 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "strat.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "strat_game.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "strat.h")]
+DEPS = SOURCES + [os.path.join(CSRC, h) for h in ("strat_game.cuh", "strat_io.cuh", "strat_kernels.cuh",
+                                                  "strat_fused.cuh", "strat_search.cuh")] + [
+    os.path.join(os.path.dirname(HERE), "include", "strat.h")]
 LIB = os.path.join(HERE, "libstrat.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

@@ -1,0 +1,329 @@
+// strat_fused.cuh - the fused hot path: persistent, warp-specialised step with cross-launch overlap
+// Part of libstrat.so (one translation unit: strat.cu includes these in order).
+#pragma once
+
+namespace {
+using namespace strat;
+
+// ---- the fused hot path, warp-specialised and persistent -------------------------------
+// One CTA = one LOGIC warp + one STORE warp sharing two staging buffers.  The logic warp
+// walks batches of 32 games (thread per game): state line straight from global into
+// registers, mask rows into the stage, mask/action/reward/done/state out, then the new
+// state's 4400-bit observation stream into the same stage.  The store warp expands finished
+// stages to bf16 and streams them out.  The two are decoupled by mbarriers, so on every SM
+// observation stores of batch i flow while batch i+1 is still in its (latency-bound) rule
+// logic; with one-warp CTAs all resident warps ran logic, then stores, in lockstep.
+#ifdef STRAT_PROF  // developer build only (_work/): per-phase cycle counters
+__device__ unsigned long long g_prof[32];
+__device__ unsigned long long g_trace[8192 * 6];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ unsigned smid() { unsigned r; asm volatile("mov.u32 %0, %smid;" : "=r"(r)); return r; }
+#define TRACE(b, k, v) do { if (lane == 0 && (b) < 8192) g_trace[(b) * 6 + (k)] = (v); } while (0)
+#define PROF_T(v) long long v = clock64()
+#define PROF_ADD(slot, a, b) do { if (lane == 0) atomicAdd(&g_prof[slot], (unsigned long long)((b) - (a))); } while (0)
+#else
+#define PROF_T(v)
+#define PROF_ADD(slot, a, b)
+#define TRACE(b, k, v)
+#endif
+constexpr int kWsStages = 2;
+// Resident CTAs per SM of ONE launch.  Two consecutive launches are co-resident (6 CTAs x 35.7 KB
+// of shared memory per SM): the later one trails the earlier one batch by batch, so the HBM
+// write stream never drains between steps.  Measured on B200 at 65,536 games: 2 -> 88.8 us,
+// 3 -> 87.8 us, 4 -> 90.3 us, 6 -> 93.1 us per step.
+#ifndef STRAT_WS_CTAS_PER_SM
+#define STRAT_WS_CTAS_PER_SM 3
+#endif
+constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
+constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+  uint32_t a = smem_u32(b), ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+// Per-batch version flags in global memory: consecutive launches of the fused step overlap
+// (programmatic dependent launch), ordered batch by batch instead of kernel by kernel.
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// whole warp: returns once *flag == want (lane 0 polls; the barrier orders the other lanes)
+__device__ __forceinline__ void flag_wait(const uint32_t* flag, uint32_t want, int lane) {
+  if (lane == 0)
+    while (ld_acquire(flag) != want) __nanosleep(64);
+  __syncwarp();
+}
+// whole warp: publish this warp's prior global writes, then set the flag
+__device__ __forceinline__ void flag_set(uint32_t* flag, uint32_t v, int lane) {
+  __syncwarp();
+  if (lane == 0) { __threadfence(); st_release(flag, v); }
+}
+// nibble -> 4 bf16 (0x3F80 where the bit is set); 16 entries x 8 B = one bank row, so the
+// two LDS.64 per 16-byte chunk never conflict.
+__device__ __forceinline__ void fill_lut16(uint2* lut, int tid) {
+  if (tid < 16) {
+    uint2 v;
+    v.x = ((tid & 1) ? 0x3F80u : 0u) | ((tid & 2) ? 0x3F800000u : 0u);
+    v.y = ((tid & 4) ? 0x3F80u : 0u) | ((tid & 8) ? 0x3F800000u : 0u);
+    lut[tid] = v;
+  }
+}
+__device__ __forceinline__ void expand_obs16(uint16_t* __restrict__ obs, int first_game, int ng,
+                                             const uint32_t* s_bits, const uint2* lut, int lane) {
+  for (int gi = 0; gi < ng; ++gi) {
+    const uint8_t* row = reinterpret_cast<const uint8_t*>(s_bits + gi * kBitsRowWords);
+    uint4* dst = reinterpret_cast<uint4*>(obs + (size_t)(first_game + gi) * STRAT_OBS_ELEMS);
+#pragma unroll
+    for (int k = 0; k < 17; ++k) {
+      uint32_t b = row[32 * k + lane];
+      uint2 lo = lut[b & 15u], hi = lut[b >> 4];
+      st_stream(dst + 32 * k + lane, make_uint4(lo.x, lo.y, hi.x, hi.y));
+    }
+    if (lane < kObsChunks - 544) {
+      uint32_t b = row[544 + lane];
+      uint2 lo = lut[b & 15u], hi = lut[b >> 4];
+      st_stream(dst + 544 + lane, make_uint4(lo.x, lo.y, hi.x, hi.y));
+    }
+  }
+}
+__device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ lines, int game, Game& g,
+                                                 uint32_t* __restrict__ hist_lines) {
+  uint32_t W[32];
+  const uint4* p = reinterpret_cast<const uint4*>(lines + (size_t)game * kLineWords);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { uint4 v = __ldcg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+  if (hist_lines) {  // board-history ring: the state this step starts from
+    uint4* q = reinterpret_cast<uint4*>(hist_lines + (size_t)game * kLineWords);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) __stcg(q + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+  }
+  unpack_line(W, g);
+}
+__device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, int game, const Game& g) {
+  uint32_t W[32];
+  pack_line(g, W);
+  uint4* p = reinterpret_cast<uint4*>(lines + (size_t)game * kLineWords);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) __stcg(p + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+}
+
+// Warp-cooperative auto-reset of the games flagged in `rs` (bit = lane = game of the batch):
+// the result equals setup_game (C2: descending Fisher-Yates over the listed multiset, one
+// Philox stream per side).  The 2 x 10 Philox blocks of a game are drawn by 20 lanes at once,
+// the sequential swaps run on a 40-byte row of shared memory, and the bit planes are built
+// with warp ballots (lane = cell of a 32-cell word).  Attempt 0 of both sides is produced
+// here; a side that fails the mobility test (R#5, p ~ 2e-6) sends that game through the
+// thread-per-game setup_game, which redraws.  `scratch` >= 3,200 words.
+__device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t rs, Game& g, uint32_t* scratch, int lane) {
+  const uint32_t full = 0xffffffffu;
+  uint32_t* sD = scratch;                                        // [32][2][40] draws
+  uint8_t* sA = reinterpret_cast<uint8_t*>(scratch + 32 * 80);  // [32][2][40] piece types
+  for (uint32_t m = rs; m; m &= m - 1) {
+    int owner = __ffs((int)m) - 1;
+    uint32_t epoch = __shfl_sync(full, g.epoch, owner);
+    if (lane < 20) {
+      int side = lane >= 10 ? 1 : 0, blk = lane - 10 * side;
+      uint32_t o[4];
+      philox(P.game_base + (uint32_t)(first + owner), epoch, (uint32_t)blk, side ? TAG_SETUP_BLUE : TAG_SETUP_RED,
+             P.key0, P.key1, o);
+      uint32_t* d = sD + owner * 80 + side * 40 + 4 * blk;
+      d[0] = o[0]; d[1] = o[1]; d[2] = o[2]; d[3] = o[3];
+    }
+    for (int i = lane; i < 80; i += 32) sA[owner * 80 + i] = (uint8_t)multiset_type(P.variant, i < 40 ? i : i - 40);
+  }
+  __syncwarp();
+  if ((rs >> lane) & 1u) {
+    for (int side = 0; side < 2; ++side) {
+      uint8_t* A = sA + lane * 80 + side * 40;
+      const uint32_t* D = sD + lane * 80 + side * 40;
+      for (int i = 39; i >= 1; --i) {
+        int j = (int)bounded(D[39 - i], (uint32_t)(i + 1));
+        uint8_t t = A[i]; A[i] = A[j]; A[j] = t;
+      }
+    }
+  }
+  __syncwarp();
+  for (uint32_t m = rs; m; m &= m - 1) {
+    int owner = __ffs((int)m) - 1;
+    const uint8_t* A = sA + owner * 80;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      int c = 32 * w + lane;
+      uint32_t t = c < 40 ? A[c] : (c >= 60 && c < 100) ? A[c - 20] : 0u;
+      uint32_t b0 = __ballot_sync(full, t & 1u), b1 = __ballot_sync(full, t & 2u), b2 = __ballot_sync(full, t & 4u),
+               b3 = __ballot_sync(full, t & 8u), bo = __ballot_sync(full, t != 0u && c >= 60);
+      if (lane == owner) { g.t0.w[w] = b0; g.t1.w[w] = b1; g.t2.w[w] = b2; g.t3.w[w] = b3; g.own.w[w] = bo; }
+    }
+  }
+  if ((rs >> lane) & 1u) {
+    g.mvd = g.rev = bb_zero();
+    hist_clear(g);
+    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
+    if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
+  }
+  __syncwarp();
+}
+
+// kExternal = false (strat_rollout_step): mask of the state -> uniform legal action -> step ->
+//   observation of the new state; `actions` is an output.
+// kExternal = true (strat_step_observe): `actions` is the caller's input (validated) -> step ->
+//   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
+//   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
+template <bool kExternal, bool kChase>
+__global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
+                                                        int16_t* __restrict__ actions, int8_t* __restrict__ reward,
+                                                        uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
+                                                        uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
+                                                        uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
+                                                        int* __restrict__ err) {
+  __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
+  __shared__ __align__(8) uint2 s_lut[16];
+  __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
+  __shared__ int s_batch[kWsStages];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nbatches = (P.num_games + kBatch - 1) / kBatch;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < kWsStages; ++s) { mbar_init(&s_full[s], 32); mbar_init(&s_empty[s], 32); }
+  }
+  fill_lut16(s_lut, threadIdx.x);
+  __syncthreads();
+  // Let the next launch of this kernel become resident now: it orders itself behind this one
+  // batch by batch through f_state / f_obs (it never calls griddepcontrol.wait).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (warp == 0) {
+    // ------------------------------------------------ logic warp (thread per game)
+    // batches: the first one is the CTA's own index, the rest are drawn from this launch's
+    // ticket counter.  atomicInc wraps to 0 after exactly nbatches draws (nbatches - grid
+    // successful ones + one failing draw per CTA), so the counter cleans up after itself.
+    int b = blockIdx.x;
+    for (int it = 0;; ++it) {
+      const int stage = it % kWsStages, round = it / kWsStages;
+      uint32_t* work = s_stage[stage];
+      PROF_T(t0);
+      if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
+      if (it > 0) {
+        uint32_t tk = 0;
+        if (lane == 0) tk = atomicInc(ticket, (uint32_t)nbatches - 1u);
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        b = tk < (uint32_t)(nbatches - (int)gridDim.x) ? (int)(gridDim.x + tk) : -1;
+      }
+      if (b < 0) {
+        if (lane == 0) s_batch[stage] = -1;
+        mbar_arrive(&s_full[stage]);
+        break;
+      }
+      const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      flag_wait(f_state + b, version - 1u, lane);  // the previous launch is done with this batch's state
+      PROF_T(t1);
+      TRACE(b, 0, gtime()); TRACE(b, 4, smid()); TRACE(b, 5, blockIdx.x);
+      zero_smem16(work, kMaskBytes, lane);
+      Game g;
+      int n = 0, cnt[4] = {0, 0, 0, 0};
+      if (lane < ng) load_game_global(lines, first + lane, g, hs.lines);
+      __syncwarp();
+      PROF_T(t2);
+      bool reset_me = false;
+      if (!kExternal) {
+        if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
+                                                       kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
+        __syncwarp();
+        PROF_T(t3);
+        if (mask) store_mask(mask, first, ng, work, lane);
+        PROF_T(t4);
+        if (lane < ng) {
+          int a = -1;
+          if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
+          StepOut o = step_game<false, true, kChase>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+          if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+          if (actions) actions[first + lane] = (int16_t)a;
+          if (reward) reward[first + lane] = (int8_t)o.reward;
+          if (done) done[first + lane] = (uint8_t)o.done;
+          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          reset_me = o.needs_reset;
+        }
+        uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        else if (rs) coop_setup(P, first, rs, g, work, lane);
+        if (lane < ng) store_game_global(lines, first + lane, g);
+        flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
+        PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4);
+      } else {
+        if (lane < ng) {
+          int a = (int)actions[first + lane];
+          StepOut o = step_game<true, true, kChase>(P, (uint32_t)(first + lane), g, a);
+          if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+          reward[first + lane] = (int8_t)o.reward;
+          done[first + lane] = (uint8_t)o.done;
+          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          reset_me = o.needs_reset;
+        }
+        uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        else if (rs) {  // the cooperative reset borrows the stage: clear its scratch again afterwards
+          coop_setup(P, first, rs, g, work, lane);
+          zero_smem16(work, kMaskBytes, lane);
+          __syncwarp();
+        }
+        if (lane < ng) {
+          store_game_global(lines, first + lane, g);
+          if (!g.done)  // of the NEW state
+            legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
+                           kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
+        }
+        __syncwarp();
+        if (mask) store_mask(mask, first, ng, work, lane);
+        flag_set(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
+      }
+      __syncwarp();  // the stage becomes bit streams
+      PROF_T(t5);
+      if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
+      __syncwarp();
+      PROF_T(t6);
+      if (lane == 0) s_batch[stage] = b;
+      mbar_arrive(&s_full[stage]);
+      TRACE(b, 1, gtime());
+      PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(4, t2, t5);
+      PROF_ADD(5, t5, t6); PROF_ADD(6, t0, t6); PROF_ADD(7, 0, 1);
+    }
+  } else {
+    // ------------------------------------------------ store warp (lane per 16-byte chunk)
+    for (int it = 0;; ++it) {
+      const int stage = it % kWsStages, round = it / kWsStages;
+      PROF_T(t0);
+      mbar_wait(&s_full[stage], (uint32_t)round & 1u);
+      const int b = s_batch[stage];
+      if (b < 0) break;
+      const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
+      flag_wait(f_obs + b, version - 1u, lane);  // write-after-write on a reused obs buffer
+      PROF_T(t1);
+      TRACE(b, 2, gtime());
+      expand_obs16(obs, first, ng, s_stage[stage], s_lut, lane);
+      flag_set(f_obs + b, version, lane);
+      TRACE(b, 3, gtime());
+      PROF_T(t2);
+      mbar_arrive(&s_empty[stage]);
+      PROF_ADD(8, t0, t1); PROF_ADD(9, t1, t2); PROF_ADD(10, 0, 1);
+    }
+  }
+}
+
+
+}  // namespace

@@ -1,0 +1,339 @@
+// strat_kernels.cuh - single-purpose kernels: reset, import/export, legal mask, sampler, step, encode, on-chip rollouts, replay ring, determinise, reductions
+// Part of libstrat.so (one translation unit: strat.cu includes these in order).
+#pragma once
+
+namespace {
+using namespace strat;
+
+// ------------------------------------------------------------------ kernels
+__global__ void __launch_bounds__(32) k_reset(Params P, uint32_t* __restrict__ lines) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  if (lane < ng) {
+    Game g; g.epoch = 0;
+    setup_game(P, (uint32_t)(first + lane), g);
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+// canonical uint8[N][128] -> device lines.  One warp per game; the seven bit planes are
+// packed with warp ballots (lane = cell within a 32-cell word).
+__global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict__ canon, uint32_t* __restrict__ lines) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= n) return;
+  uint32_t cw = reinterpret_cast<const uint32_t*>(canon + (size_t)g * 128)[lane];  // bytes 4l..4l+3
+  uint32_t mine = 0;
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    int cell = 32 * r + lane;
+    uint32_t w = __shfl_sync(0xffffffffu, cw, (cell >> 2) & 31);
+    uint32_t b = cell < 100 ? (w >> (8 * (cell & 3))) & 0xFFu : 0u;
+    uint32_t t = b & 15u;
+    bool piece = t >= 1 && t <= 12;
+#pragma unroll
+    for (int p = 0; p < 7; ++p) {
+      bool bit = p < 4 ? (piece && ((t >> p) & 1u)) : (piece && ((b >> p) & 1u));  // p=4 owner(bit4),5 moved,6 revealed
+      uint32_t word = __ballot_sync(0xffffffffu, bit);
+      if (lane == 4 * p + r) mine = word;
+    }
+  }
+  // meta: history pairs ride in the spare bits of words 3,7,11,15; flags in word 19
+  uint32_t hw = __shfl_sync(0xffffffffu, cw, 25 + (lane >> 2));  // canonical bytes 100+4p.. for lane 4p+3
+  uint32_t fw = __shfl_sync(0xffffffffu, cw, 30);
+  if ((lane & 3) == 3 && lane < 16) {
+    uint32_t f0 = hw & 0xFFu, t0 = (hw >> 8) & 0xFFu, f1 = (hw >> 16) & 0xFFu, t1 = hw >> 24;
+    uint32_t e0 = f0 == 0xFFu ? kHistNone : (f0 | (t0 << 7));
+    uint32_t e1 = f1 == 0xFFu ? kHistNone : (f1 | (t1 << 7));
+    mine |= (e0 | (e1 << 14)) << 4;
+  }
+  if (lane == 19) {
+    uint32_t fl = fw & 0xFFu;
+    int32_t res = (int32_t)(int8_t)((fw >> 8) & 0xFFu);
+    mine |= ((fl & 1u) | (((fl >> 2) & 7u) << 1) | ((uint32_t)(res + 1) << 4)) << 4;
+  }
+  uint32_t w29 = __shfl_sync(0xffffffffu, cw, 29), w31 = __shfl_sync(0xffffffffu, cw, 31);
+  if (lane == 28) mine = w29;  // ply | battleless<<16 : same bytes as canonical 116..119
+  if (lane == 29) mine = w31;  // epoch
+  if (lane == 30) mine = fw >> 16;  // chase ages: canonical bytes 122..123
+  if (lane == 31) mine = 0;
+  lines[(size_t)g * kLineWords + lane] = mine;
+}
+
+// device lines -> canonical.  One warp per game; lane l < 25 assembles cells 4l..4l+3.
+__global__ void __launch_bounds__(128) k_export(int n, const uint32_t* __restrict__ lines, uint8_t* __restrict__ canon) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= n) return;
+  uint32_t lw = lines[(size_t)g * kLineWords + lane];
+  uint32_t out = 0;
+  int r = (lane >> 3) & 3, sh = 4 * (lane & 7);  // cells 4l..4l+3 sit in word r of each plane, bits sh..sh+3
+  uint32_t nib[7];
+#pragma unroll
+  for (int p = 0; p < 7; ++p) nib[p] = (__shfl_sync(0xffffffffu, lw, 4 * p + r) >> sh) & 0xFu;
+  if (lane < 25) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      uint32_t b = 0;
+#pragma unroll
+      for (int p = 0; p < 7; ++p) b |= ((nib[p] >> k) & 1u) << p;
+      int cell = 4 * lane + k;
+      if (is_lake_cell(cell)) b = 15;
+      out |= b << (8 * k);
+    }
+  }
+  uint32_t hw = __shfl_sync(0xffffffffu, lw, 4 * ((lane - 25) & 3) + 3) >> 4;   // history pair for lanes 25..28
+  uint32_t fw = __shfl_sync(0xffffffffu, lw, 19) >> 4;
+  uint32_t w28 = __shfl_sync(0xffffffffu, lw, 28), w29 = __shfl_sync(0xffffffffu, lw, 29);
+  uint32_t w30 = __shfl_sync(0xffffffffu, lw, 30);
+  if (lane >= 25 && lane < 29) {
+    uint32_t e0 = hw & 0x3FFFu, e1 = (hw >> 14) & 0x3FFFu;
+    uint32_t b0 = e0 == kHistNone ? 0xFFFFu : ((e0 & 127u) | ((e0 >> 7) << 8));
+    uint32_t b1 = e1 == kHistNone ? 0xFFFFu : ((e1 & 127u) | ((e1 >> 7) << 8));
+    out = b0 | (b1 << 16);
+  }
+  if (lane == 29) out = w28;
+  if (lane == 30) {
+    uint32_t done = fw & 1u, reason = (fw >> 1) & 7u;
+    int32_t res = (int32_t)((fw >> 4) & 3u) - 1;
+    out = (done | (reason << 2)) | (((uint32_t)res & 0xFFu) << 8) | ((w30 & 0xFFFFu) << 16);
+  }
+  if (lane == 31) out = w29;
+  reinterpret_cast<uint32_t*>(canon + (size_t)g * 128)[lane] = out;
+}
+
+template <bool kChase>
+__global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __restrict__ lines, uint32_t* __restrict__ mask) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  zero_smem16(s_mask, kMaskBytes, lane);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    int cnt[4];
+    if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), s_mask + lane * kMaskWords, cnt,
+                                kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
+  }
+  __syncwarp();
+  store_mask(mask, first, ng, s_mask, lane);
+}
+
+// One warp per game: lanes load the 113 mask words coalesced, count with popc, locate the
+// r-th set bit with warp-shuffle prefix sums.
+__global__ void __launch_bounds__(128) k_sample_uniform(Params P, const uint32_t* __restrict__ lines,
+                                                        const uint32_t* __restrict__ mask, int16_t* __restrict__ actions) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int g = blockIdx.x * 4 + warp;
+  if (g >= P.num_games) return;
+  const uint32_t* row = mask + (size_t)g * kMaskWords;
+  uint32_t w[4]; int cnt[4], incl[4], tot[4];
+  int n = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    int wi = 32 * k + lane;
+    w[k] = wi < kMaskWords ? row[wi] : 0u;
+    cnt[k] = __popc(w[k]);
+    int x = cnt[k];
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, off); if (lane >= off) x += y; }
+    incl[k] = x;
+    tot[k] = __shfl_sync(0xffffffffu, x, 31);
+    n += tot[k];
+  }
+  int action = -1;
+  if (n > 0) {
+    uint32_t meta = lane < 2 ? lines[(size_t)g * kLineWords + 28 + lane] : 0u;
+    uint32_t w28 = __shfl_sync(0xffffffffu, meta, 0), epoch = __shfl_sync(0xffffffffu, meta, 1);
+    uint32_t o[4];
+    philox(P.game_base + (uint32_t)g, epoch, w28 & 0xFFFFu, TAG_ACTION, P.key0, P.key1, o);
+    int r = (int)bounded(o[0], (uint32_t)n);
+    int base = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      int excl = base + incl[k] - cnt[k];  // set bits before this lane's word
+      bool mine = r >= excl && r < excl + cnt[k];
+      uint32_t owner = __ballot_sync(0xffffffffu, mine);
+      int a = (32 * k + lane) * 32 + (mine ? nth_set_bit(w[k], r - excl) : 0);
+      if (owner) action = __shfl_sync(0xffffffffu, a, __ffs((int)owner) - 1);
+      base += tot[k];
+    }
+  }
+  if (lane == 0) actions[g] = (int16_t)action;
+}
+
+template <bool kChase>
+__global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ lines, const int16_t* __restrict__ actions,
+                                             int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err,
+                                             HistSlot hs) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  load_lines(lines, first, ng, s_state, lane);
+  if (hs.lines) store_lines(hs.lines, first, ng, s_state, lane);  // the state this step starts from
+  __syncwarp();
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    int a = (int)actions[first + lane];
+    StepOut o = step_game<true, false, kChase>(P, (uint32_t)(first + lane), g, a);
+    if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
+    reward[first + lane] = (int8_t)o.reward;
+    done[first + lane] = (uint8_t)o.done;
+    if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+__global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __restrict__ lines, uint16_t* __restrict__ obs) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ __align__(16) uint32_t s_bits[kBatch * kBitsRowWords];  // 17,792 B
+  __shared__ __align__(16) uint4 s_lut[256];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  fill_lut(s_lut, lane, 32);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    encode_bits(g, s_bits + lane * kBitsRowWords);
+  }
+  __syncwarp();
+  expand_obs(obs, first, ng, s_bits, s_lut, lane);
+}
+
+// `plies` plies of uniform-random legal play with the board in registers.  The 3600-bit mask is
+// never built: the r-th legal action is found from the move bitboards (sample_action_direct).
+constexpr int kScoutScratch = 9;  // 8 words per game, odd stride
+template <bool kChase>
+__global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  __shared__ uint32_t s_scouts[kBatch * kScoutScratch];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, P.num_games - first);
+  load_lines(lines, first, ng, s_state, lane);
+  if (lane < ng) {
+    Game g; read_game(s_state, lane, g);
+    for (int t = 0; t < plies; ++t) {
+      if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
+      int a = sample_action_direct(g, g.ply & 1u, rules_of<kChase>(P), action_draw(P, (uint32_t)(first + lane), g),
+                                   s_scouts + lane * kScoutScratch, kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
+      if (step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
+        raise_error(err, STRAT_ILLEGAL_ACTION);
+        break;
+      }
+    }
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(lines, first, ng, s_state, lane);
+}
+
+// ---- replay ring
+template <typename T>
+__global__ void k_copy(const T* __restrict__ src, T* __restrict__ dst, size_t count) {
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) dst[i] = src[i];
+}
+// one warp per batch element: draw the record index, gather the record.
+__global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
+                                                       uint32_t filled, const uint16_t* __restrict__ r_obs,
+                                                       const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
+                                                       const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
+                                                       uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
+                                                       int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int j = blockIdx.x * 4 + warp;
+  if (j >= batch) return;
+  uint32_t o[4];
+  philox((uint32_t)(j >> 2), d0, d1, TAG_SAMPLE, k0, k1, o);
+  uint32_t u = (j & 3) == 0 ? o[0] : (j & 3) == 1 ? o[1] : (j & 3) == 2 ? o[2] : o[3];
+  size_t p = bounded(u, filled);
+  if (obs) {
+    const uint4* s = reinterpret_cast<const uint4*>(r_obs + p * STRAT_OBS_ELEMS);
+    uint4* d = reinterpret_cast<uint4*>(obs + (size_t)j * STRAT_OBS_ELEMS);
+    for (int q = lane; q < kObsChunks; q += 32) d[q] = __ldcs(s + q);
+  }
+  if (mask)
+    for (int q = lane; q < kMaskWords; q += 32) mask[(size_t)j * kMaskWords + q] = r_mask[p * kMaskWords + q];
+  if (lane == 0) {
+    if (act) act[j] = r_act[p];
+    if (rew) rew[j] = r_rew[p];
+    if (done) done[j] = r_done[p];
+  }
+}
+
+// ---- search-shaped batch
+__global__ void __launch_bounds__(32) k_determinise(int num_out, int samples_per_root, uint32_t k0, uint32_t k1, uint32_t out_base,
+                                                    const uint32_t* __restrict__ roots, uint32_t* __restrict__ out,
+                                                    int* __restrict__ err) {
+  __shared__ __align__(16) uint8_t s_state[kStateBytes];
+  int lane = threadIdx.x, first = blockIdx.x * kBatch;
+  int ng = min(kBatch, num_out - first);
+  if (lane < ng) {
+    int G = first + lane, r = G / samples_per_root;
+    uint32_t W[32];
+    const uint4* p = reinterpret_cast<const uint4*>(roots + (size_t)r * kLineWords);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { uint4 v = __ldg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+    Game root, g;
+    unpack_line(W, root);
+    if (!determinise_game(root, k0, k1, out_base + (uint32_t)G, g)) raise_error(err, STRAT_BAD_STATE);
+    write_game(s_state, lane, g);
+  }
+  __syncwarp();
+  store_lines(out, first, ng, s_state, lane);
+}
+
+__global__ void __launch_bounds__(256) k_reduce_returns(const uint32_t* __restrict__ lines, const uint8_t* __restrict__ root_side,
+                                                        int samples_per_root, int32_t* __restrict__ out) {
+  __shared__ int s_sum[8], s_win[8], s_loss[8];
+  int r = blockIdx.x;
+  int sign = root_side[r] == 0 ? 1 : -1;
+  int sum = 0, win = 0, loss = 0;
+  for (int s = threadIdx.x; s < samples_per_root; s += blockDim.x) {
+    uint32_t f = lines[((size_t)r * samples_per_root + s) * kLineWords + 19] >> 4;
+    int ret = (f & 1u) ? ((int)((f >> 4) & 3u) - 1) * sign : 0;
+    sum += ret; win += ret > 0; loss += ret < 0;
+  }
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) {
+    sum += __shfl_down_sync(0xffffffffu, sum, off);
+    win += __shfl_down_sync(0xffffffffu, win, off);
+    loss += __shfl_down_sync(0xffffffffu, loss, off);
+  }
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) { s_sum[warp] = sum; s_win[warp] = win; s_loss[warp] = loss; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int a = 0, b = 0, c = 0;
+    for (int k = 0; k < 8; ++k) { a += s_sum[k]; b += s_win[k]; c += s_loss[k]; }
+    out[3 * r] = a; out[3 * r + 1] = b; out[3 * r + 2] = c;
+  }
+}
+
+// Scalar queries of Table S1 from the state lines of one time step.
+__global__ void __launch_bounds__(256) k_line_info(int n, const uint32_t* __restrict__ lines, int32_t* __restrict__ info) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  const uint32_t* L = lines + (size_t)g * kLineWords;
+  uint32_t w28 = L[28], f = L[19] >> 4;
+  uint32_t ply = w28 & 0xFFFFu, done = f & 1u, reason = (f >> 1) & 7u;
+  int4 v = make_int4((int)(ply & 1u), (int)ply, (int)(w28 >> 16), (int)(done | (reason << 2)));
+  reinterpret_cast<int4*>(info)[g] = v;
+}
+
+// A state copied in from elsewhere (history ring) has no move log here: it remembers 8 plies.
+__global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict__ lines) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < n) lines[(size_t)g * kLineWords + 31] = 0;
+}
+
+__global__ void k_set_int(int* p, int v) { *p = v; }
+
+
+}  // namespace
