@@ -15,6 +15,7 @@
 //   * The single-purpose kernels (k_legal_mask, k_step, k_encode_obs, ...) run one warp per CTA.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <mutex>
 #include <new>
 
 #include "../../include/strat.h"
@@ -129,6 +130,14 @@ namespace {
 // the previous launch in the stream is still running IF that one is also a fused step (the only
 // kernel that executes griddepcontrol.launch_dependents); behind any other kernel the attribute
 // changes nothing.  Ordering against the previous fused step is per batch (f_state / f_obs).
+// The last fused step launched by this process: (stream, environment).  A fused step may skip
+// griddepcontrol.wait only if it directly continues its own environment's chain on the same
+// stream; after a fused step of another environment it must wait for that grid (its inputs may
+// be that step's outputs, and no version flags relate the two).
+std::mutex g_chain_mutex;
+const void* g_chain_stream = nullptr;
+const strat_env* g_chain_env = nullptr;
+
 template <bool kExternal>
 int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done, uint16_t* obs,
                  void* stream) {
@@ -143,10 +152,16 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = 1;
   const uint32_t version = env->version + 1;
+  int wait_prior;
+  {
+    std::lock_guard<std::mutex> lock(g_chain_mutex);
+    wait_prior = !(g_chain_env == env && g_chain_stream == stream);
+    g_chain_env = env; g_chain_stream = stream;
+  }
   auto kernel = env->P.chase_rule ? k_rollout_step<kExternal, true> : k_rollout_step<kExternal, false>;
   if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
                          env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
-                         hist_slot(env->hist), env->err) != cudaSuccess)
+                         hist_slot(env->hist), env->err, wait_prior) != cudaSuccess)
     return STRAT_CUDA_ERROR;
   env->version = version;
   if (env->hist) env->hist->cur += 1;
@@ -204,6 +219,10 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
 
 int strat_destroy(strat_env* env) {
   if (env && env->hist) env->hist->env = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_chain_mutex);
+    if (g_chain_env == env) { g_chain_env = nullptr; g_chain_stream = nullptr; }
+  }
   delete env;
   return STRAT_OK;
 }

@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
                                                         uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
                                                         uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
-                                                        int* __restrict__ err) {
+                                                        int* __restrict__ err, int wait_prior) {
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
@@ -206,8 +206,10 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
   fill_lut16(s_lut, threadIdx.x);
   __syncthreads();
   // Let the next launch of this kernel become resident now: it orders itself behind this one
-  // batch by batch through f_state / f_obs (it never calls griddepcontrol.wait).
+  // batch by batch through f_state / f_obs.  Only a launch whose predecessor in the stream is a
+  // fused step of ANOTHER environment (no flags tie the two) waits for that grid as a whole.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
   if (warp == 0) {
     // ------------------------------------------------ logic warp (thread per game)
     // batches: the first one is the CTA's own index, the rest are drawn from this launch's

@@ -272,6 +272,24 @@ def test_pinned_reset_state_matches_oracle():
     assert g.check() == 0
 
 
+def test_fused_steps_of_two_environments_chained_through_a_buffer():
+    """Environment B replays, with strat_step_observe, the actions environment A's fused step has
+    just written - 300 times with no host sync.  The two launches belong to different environments
+    (no version flags relate them), so B must wait for A's grid: stream order has to hold."""
+    kw = dict(variant=0, seed=31, max_plies=120, auto_reset=1)
+    n = 65536
+    a, b = B.Env(n, **kw), B.Env(n, **kw)
+    mask_a, act, rew_a, done_a, obs_a = a.new_mask(), a.new_actions(), a.new_reward(), a.new_done(), a.new_obs()
+    mask_b, rew_b, done_b, obs_b = b.new_mask(), b.new_reward(), b.new_done(), b.new_obs()
+    for _ in range(300):
+        a.rollout_step(mask_a, act, rew_a, done_a, obs_a)
+        b.step_observe(act, rew_b, done_b, mask_b, obs_b)
+    assert b.check() == 0  # B never saw a stale (illegal) action
+    assert torch.equal(a.get_boards(), b.get_boards())
+    assert torch.equal(obs_a.view(torch.int16), obs_b.view(torch.int16))
+    assert torch.equal(rew_a, rew_b) and torch.equal(done_a, done_b)
+
+
 def test_fused_step_interleaved_with_other_calls():
     """A fused step after any other state-changing call (and vice versa) sees that call's result."""
     kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)
