@@ -124,63 +124,6 @@ __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, 
   for (int k = 0; k < 8; ++k) __stcg(p + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
 }
 
-// Warp-cooperative auto-reset of the games flagged in `rs` (bit = lane = game of the batch):
-// the result equals setup_game (C2: descending Fisher-Yates over the listed multiset, one
-// Philox stream per side).  The 2 x 10 Philox blocks of a game are drawn by 20 lanes at once,
-// the sequential swaps run on a 40-byte row of shared memory, and the bit planes are built
-// with warp ballots (lane = cell of a 32-cell word).  Attempt 0 of both sides is produced
-// here; a side that fails the mobility test (R#5, p ~ 2e-6) sends that game through the
-// thread-per-game setup_game, which redraws.  `scratch` >= 3,200 words.
-__device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t rs, Game& g, uint32_t* scratch, int lane) {
-  const uint32_t full = 0xffffffffu;
-  uint32_t* sD = scratch;                                        // [32][2][40] draws
-  uint8_t* sA = reinterpret_cast<uint8_t*>(scratch + 32 * 80);  // [32][2][40] piece types
-  for (uint32_t m = rs; m; m &= m - 1) {
-    int owner = __ffs((int)m) - 1;
-    uint32_t epoch = __shfl_sync(full, g.epoch, owner);
-    if (lane < 20) {
-      int side = lane >= 10 ? 1 : 0, blk = lane - 10 * side;
-      uint32_t o[4];
-      philox(P.game_base + (uint32_t)(first + owner), epoch, (uint32_t)blk, side ? TAG_SETUP_BLUE : TAG_SETUP_RED,
-             P.key0, P.key1, o);
-      uint32_t* d = sD + owner * 80 + side * 40 + 4 * blk;
-      d[0] = o[0]; d[1] = o[1]; d[2] = o[2]; d[3] = o[3];
-    }
-    for (int i = lane; i < 80; i += 32) sA[owner * 80 + i] = (uint8_t)multiset_type(P.variant, i < 40 ? i : i - 40);
-  }
-  __syncwarp();
-  if ((rs >> lane) & 1u) {
-    for (int side = 0; side < 2; ++side) {
-      uint8_t* A = sA + lane * 80 + side * 40;
-      const uint32_t* D = sD + lane * 80 + side * 40;
-      for (int i = 39; i >= 1; --i) {
-        int j = (int)bounded(D[39 - i], (uint32_t)(i + 1));
-        uint8_t t = A[i]; A[i] = A[j]; A[j] = t;
-      }
-    }
-  }
-  __syncwarp();
-  for (uint32_t m = rs; m; m &= m - 1) {
-    int owner = __ffs((int)m) - 1;
-    const uint8_t* A = sA + owner * 80;
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      int c = 32 * w + lane;
-      uint32_t t = c < 40 ? A[c] : (c >= 60 && c < 100) ? A[c - 20] : 0u;
-      uint32_t b0 = __ballot_sync(full, t & 1u), b1 = __ballot_sync(full, t & 2u), b2 = __ballot_sync(full, t & 4u),
-               b3 = __ballot_sync(full, t & 8u), bo = __ballot_sync(full, t != 0u && c >= 60);
-      if (lane == owner) { g.t0.w[w] = b0; g.t1.w[w] = b1; g.t2.w[w] = b2; g.t3.w[w] = b3; g.own.w[w] = bo; }
-    }
-  }
-  if ((rs >> lane) & 1u) {
-    g.mvd = g.rev = bb_zero();
-    hist_clear(g);
-    g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
-    if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
-  }
-  __syncwarp();
-}
-
 // kExternal = false (strat_rollout_step): mask of the state -> uniform legal action -> step ->
 //   observation of the new state; `actions` is an output.
 // kExternal = true (strat_step_observe): `actions` is the caller's input (validated) -> step ->
