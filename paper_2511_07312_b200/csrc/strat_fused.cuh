@@ -103,19 +103,6 @@ __device__ __forceinline__ void expand_obs16(uint16_t* __restrict__ obs, int fir
     }
   }
 }
-__device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ lines, int game, Game& g,
-                                                 uint32_t* __restrict__ hist_lines) {
-  uint32_t W[32];
-  const uint4* p = reinterpret_cast<const uint4*>(lines + (size_t)game * kLineWords);
-#pragma unroll
-  for (int k = 0; k < 8; ++k) { uint4 v = __ldcg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
-  if (hist_lines) {  // board-history ring: the state this step starts from
-    uint4* q = reinterpret_cast<uint4*>(hist_lines + (size_t)game * kLineWords);
-#pragma unroll
-    for (int k = 0; k < 8; ++k) __stcg(q + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
-  }
-  unpack_line(W, g);
-}
 __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, int game, const Game& g) {
   uint32_t W[32];
   pack_line(g, W);

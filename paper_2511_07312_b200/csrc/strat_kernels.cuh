@@ -164,14 +164,13 @@ __global__ void __launch_bounds__(128) k_export(int n, const uint32_t* __restric
 
 template <bool kChase>
 __global__ void __launch_bounds__(32) k_legal_mask(Params P, const uint32_t* __restrict__ lines, uint32_t* __restrict__ mask) {
-  __shared__ __align__(16) uint8_t s_state[kStateBytes];
-  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];
+  __shared__ __align__(16) uint32_t s_mask[kBatch * kMaskWords];  // 14.5 KB: 15 one-warp CTAs per SM, one wave at 65,536 games
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, P.num_games - first);
   zero_smem16(s_mask, kMaskBytes, lane);
-  load_lines(lines, first, ng, s_state, lane);
+  __syncwarp();
   if (lane < ng) {
-    Game g; read_game(s_state, lane, g);
+    Game g; load_game_global(lines, first + lane, g, nullptr);
     int cnt[4];
     if (!g.done) legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), s_mask + lane * kMaskWords, cnt,
                                 kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
