@@ -65,6 +65,7 @@ def lib():
         L.orc_search_policy.argtypes = [vp, vp, C.c_int32, vp, C.c_double, C.c_double, vp, vp, vp]
         L.orc_determinise.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp]
         L.orc_reduce_returns.argtypes = [vp, vp, C.c_int32, vp]
+        L.orc_find_setup_redraws.argtypes = [C.POINTER(Config), C.c_uint32, C.c_uint32, C.c_uint32, vp, C.c_int]
         L.orc_philox.argtypes = [vp, vp, vp]
         L.orc_philox.restype = None
         L.orc_battle.argtypes = [C.c_int, C.c_int]
@@ -241,6 +242,15 @@ def reduce_returns(games: Env, root_side, samples_per_root: int):
     out = np.zeros((games.n // samples_per_root, 3), np.int32)
     _chk(lib().orc_reduce_returns(games.h, _p(rs), samples_per_root, _p(out)), "reduce_returns")
     return out
+
+
+def find_setup_redraws(variant, seed, epoch, start, count, max_out=64):
+    """Global game indices in [start, start+count) whose setup at `epoch` needs a redraw (R#5)."""
+    cfg = Config(1, variant, seed, 0, 0, 0, 1, 0, 0, 0)
+    out = np.zeros(max_out, np.uint32)
+    n = lib().orc_find_setup_redraws(C.byref(cfg), epoch, start, count, _p(out), max_out)
+    assert n >= 0
+    return out[:n].tolist()
 
 
 def philox(ctr, key):

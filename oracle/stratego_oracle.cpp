@@ -207,7 +207,8 @@ bool side_can_ever_move(const uint8_t cell[kCells], int side) {
   return false;
 }
 
-void setup_side(const Config& cfg, uint32_t gidx, uint32_t epoch, int side, uint8_t cell[kCells]) {
+// Returns the number of attempts used (1 unless the first permutation left the side immobile).
+int setup_side(const Config& cfg, uint32_t gidx, uint32_t epoch, int side, uint8_t cell[kCells]) {
   for (uint32_t attempt = 0;; ++attempt) {
     int A[40];
     multiset(cfg.variant, A);
@@ -221,7 +222,7 @@ void setup_side(const Config& cfg, uint32_t gidx, uint32_t epoch, int side, uint
     int base = side == 0 ? 0 : 60;
     for (int i = 0; i < 40; ++i)
       cell[base + i] = A[i] == 0 ? 0 : (uint8_t)(A[i] | (side ? B_OWNER : 0));
-    if (side_can_ever_move(cell, side)) return;
+    if (side_can_ever_move(cell, side)) return (int)attempt + 1;
   }
 }
 
@@ -969,6 +970,23 @@ int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, cons
 }
 
 // ---- probes used by the pins only
+// Global game indices in [start, start+count) whose setup at `epoch` needs a redraw (R#5) for
+// either side; used once by tests/golden/make_setup_redraw_cases.py to find test cases for a
+// path that random play reaches about twice in a million setups.
+int orc_find_setup_redraws(const Config* cfg, uint32_t epoch, uint32_t start, uint32_t count, uint32_t* out, int max_out) {
+  if (!cfg || !out) return ORC_BAD_ARG;
+  int n = 0;
+  uint8_t cell[kCells];
+  for (uint32_t i = 0; i < count && n < max_out; ++i) {
+    memset(cell, 0, sizeof cell);
+    for (int c = 0; c < kCells; ++c)
+      if (is_lake(c)) cell[c] = T_LAKE;
+    int a0 = setup_side(*cfg, start + i, epoch, 0, cell);
+    int a1 = setup_side(*cfg, start + i, epoch, 1, cell);
+    if (a0 > 1 || a1 > 1) out[n++] = start + i;
+  }
+  return n;
+}
 void orc_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox4x32_10(ctr, key, out); }
 int orc_battle(int att, int def) { return battle(att, def); }
 int orc_is_lake(int c) { return is_lake(c) ? 1 : 0; }

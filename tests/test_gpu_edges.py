@@ -172,3 +172,30 @@ def test_random_hand_built_boards_all_calls():
         g.clear_error(); o.clear_error()
     reasons = np.bincount((o.get_boards()[:, 120] >> 2) & 7, minlength=6)
     assert reasons[1] > 0 and reasons[2] > 0 and reasons[4] > 0  # flag captures, no-move wins, ply caps all occurred
+
+
+def test_setup_redraw_cases_on_gpu(golden_dir):
+    """Setups that are immobile at the first attempt (R5; found by the oracle, tests/golden/
+    setup_redraw_cases.json): the thread-per-game reset (k_reset, epoch 0) and the warp-cooperative
+    auto-reset's fallback inside the fused step and strat_step (epoch 1) redraw like the oracle."""
+    import json
+    import os
+    cases = json.load(open(os.path.join(golden_dir, "setup_redraw_cases.json")))
+    for gidx in cases["epoch0"]:
+        kw = dict(variant=0, seed=cases["seed"], game_base=gidx - 5)
+        g, o = B.Env(40, **kw), orc.Env(40, **kw)
+        assert np.array_equal(_np(g.get_boards()), o.get_boards()), gidx
+    for k, gidx in enumerate(cases["epoch1"]):
+        kw = dict(variant=0, seed=cases["seed"], game_base=gidx - 7, max_plies=3, auto_reset=1)
+        g, o = B.Env(40, **kw), orc.Env(40, **kw)
+        mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+        for t in range(7):  # the 3-ply cap ends every game at t = 2: epoch 1 is set up inside that step
+            oa = o.sample_uniform(o.legal_mask()); o.step(oa)
+            if k % 2 == 0:
+                g.rollout_step(mask, act, rew, done, obs)
+            else:
+                g.step(_dev(oa), rew, done)
+            b = o.get_boards()
+            assert np.array_equal(_np(g.get_boards()), b), (gidx, t)
+        assert (b[:, 124] >= 2).all()
+        assert g.check() == 0

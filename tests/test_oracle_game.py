@@ -2,6 +2,8 @@
 determinisation: closed forms, invariants the rules fix (BASELINE.json north_star: lake
 cells never occupied, piece multisets only shrink through battles, a side with no legal
 move loses), hand-built endings and statistical checks."""
+import os
+
 import numpy as np
 import pytest
 
@@ -76,6 +78,27 @@ def test_setup_rejects_immobile_side():
     # square in front is vacated (depends on own pieces only)
     e = orc.Env(2000, seed=7)
     assert all(e.count_moves(g, 0) > 0 for g in range(2000))
+
+
+def test_setup_redraw_rate_matches_the_closed_form_and_cases_are_redrawn(golden_dir):
+    """R#5: a classic side is immobile at the first attempt iff its six front squares beside the
+    lakes hold 6 of its 7 immovable pieces: p = 7*6*5*4*3*2 / (40*39*38*37*36*35) per side."""
+    import json
+    p = (7 * 6 * 5 * 4 * 3 * 2) / (40 * 39 * 38 * 37 * 36 * 35)
+    n = 1_000_000
+    hits = orc.find_setup_redraws(0, 0, 0, 0, n)
+    lam = 2 * p * n                                       # 3.6 expected; Poisson: P(k > 14) < 1e-5
+    assert abs(p - 1.8e-6) < 1e-7 and 0 < len(hits) <= 14, (lam, hits)
+    cases = json.load(open(os.path.join(golden_dir, "setup_redraw_cases.json")))
+    assert hits == [g for g in cases["epoch0"] if g < n]
+    for g in cases["epoch0"]:
+        e = orc.Env(1, seed=cases["seed"], game_base=g)
+        b = e.get_boards()[0]
+        assert e.count_moves(0, 0) + e.count_moves(0, 1) > 0
+        front = [30, 31, 34, 35, 38, 39]
+        red_stuck = all((b[c] & 15) in (11, 12) for c in front)
+        blue_stuck = all((b[99 - c] & 15) in (11, 12) for c in front)
+        assert not red_stuck and not blue_stuck          # the setup that was kept can move
 
 
 # ----------------------------------------------------------------------------- step
