@@ -199,3 +199,29 @@ def test_setup_redraw_cases_on_gpu(golden_dir):
             assert np.array_equal(_np(g.get_boards()), b), (gidx, t)
         assert (b[:, 124] >= 2).all()
         assert g.check() == 0
+
+
+def test_large_batch_beyond_4_gib_of_observations():
+    """600,011 games: 5.3 GB of observations per step (byte offsets above 2^32), a ragged last
+    batch; the oracle mirrors the first and the last games."""
+    n = 600011
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12e9:
+        pytest.skip("needs ~8 GB of free device memory")
+    kw = dict(variant=0, seed=2, max_plies=6, auto_reset=1)
+    g = B.Env(n, **kw)
+    lo = n - 43
+    o_first, o_last = orc.Env(32, **kw), orc.Env(43, game_base=lo, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(8):  # every game is reset once (6-ply cap)
+        g.rollout_step(mask, act, rew, done, obs)
+        for oo, s in ((o_first, slice(0, 32)), (o_last, slice(lo, n))):
+            om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
+            assert np.array_equal(_np(act[s]), oa) and np.array_equal(_np(rew[s]), orr) and np.array_equal(_np(done[s]), od), t
+            assert np.array_equal(_np(mask[s]).view(np.uint32), om), t
+            assert np.array_equal(_np(obs[s].view(torch.int16)).view(np.uint16), oo.encode_obs()), t
+    b = g.get_boards()
+    assert np.array_equal(_np(b[lo:]), o_last.get_boards()) and np.array_equal(_np(b[:32]), o_first.get_boards())
+    x = obs.view(torch.int16)[:, :28].reshape(n, 28, 100)
+    assert bool(((x != 0).sum(dim=1) == 1).all())  # planes 0-27 partition the board for every game
+    assert g.check() == 0
