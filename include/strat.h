@@ -141,7 +141,11 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream);
 /* One fused pass of the hot path: legal mask -> uniform legal action -> step -> encode of
  * the new state.  Produces exactly what strat_legal_mask, strat_sample_uniform,
  * strat_step, strat_encode_obs produce when called in that order.  Any output pointer
- * except `obs` may be NULL (that output is then not written). */
+ * except `obs` may be NULL (that output is then not written).
+ * Consecutive fused steps (this call and strat_step_observe) of one environment on one stream
+ * overlap on the device, ordered batch by batch; everything else in the stream sees plain stream
+ * order.  They cannot be captured into a CUDA graph (STRAT_BAD_STATE while `stream` is
+ * capturing): each launch carries a host-side launch counter. */
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward,
                        uint8_t* done, uint16_t* obs, void* stream);
 

@@ -141,6 +141,11 @@ const strat_env* g_chain_env = nullptr;
 template <bool kExternal>
 int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done, uint16_t* obs,
                  void* stream) {
+  // The launch carries a host-side launch counter (the version the batch flags are compared
+  // with): replaying it from a captured CUDA graph would reuse a stale version and wait forever.
+  cudaStreamCaptureStatus capture = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing((cudaStream_t)stream, &capture) != cudaSuccess) return STRAT_CUDA_ERROR;
+  if (capture != cudaStreamCaptureStatusNone) return STRAT_BAD_STATE;
   const int nb = batches(env->P.num_games);
   // a launch that follows a policy kernel has the GPU to itself: one more CTA per SM
   const int per_sm = kExternal ? kWsCtasPerSm + 1 : kWsCtasPerSm;

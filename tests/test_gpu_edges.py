@@ -102,6 +102,15 @@ def test_argument_errors_and_empty_inputs():
     ring.sample(0, 0, 0, so, None, None, None, None)  # an empty batch is fine
     with pytest.raises(B.StratError):
         ring.reserve(5, 0)  # blocks must tile the ring
+    # the fused step refuses CUDA-graph capture (its launch counter lives on the host)
+    cap_stream = torch.cuda.Stream()
+    obs40, graph = g.new_obs(), torch.cuda.CUDAGraph()
+    with torch.cuda.stream(cap_stream):
+        graph.capture_begin()
+        rc = L.strat_rollout_step(g.h, None, None, None, None, B._ptr(obs40), B._stream())
+        graph.capture_end()
+    assert rc == B.BAD_STATE
+    torch.cuda.synchronize()
     h = B.History(40, 1)  # a one-step ring
     h.attach(g)
     g.step(g.sample_uniform(g.legal_mask()))
