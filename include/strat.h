@@ -18,6 +18,9 @@
  *     asynchronous with respect to the host.
  *   - Device-detected faults (an illegal action for a live game) set a sticky device
  *     error word and leave that game unchanged; strat_check reads it.
+ *   - Handles are not thread-safe: calls on one environment / ring / history come from one
+ *     host thread at a time, and consecutive calls on one environment use one stream (or are
+ *     ordered by the caller with events).  Different environments are independent.
  *
  * Layouts (BASELINE.json configs[0])
  *   cell c = 10*row + col, row 0 = red's back row; lakes {42,43,46,47,52,53,56,57}.
