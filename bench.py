@@ -212,6 +212,13 @@ def run_b200(args):
     total_ms_max = float(t.item())
     value = world * n * args.steps / (total_ms_max / 1e3)
 
+    # outside the timed region: how many games end (and are re-dealt inside the step) per step
+    ended = 0
+    for _ in range(20):
+        env.rollout_step(mask, act, rew, done, obs)
+        ended += int((done & 1).sum().item())
+    reset_fraction = ended / (20.0 * n)
+
     e2e_value, e2e_steps = None, 0
     if not args.skip_e2e:
         e2e_value, e2e_steps = run_e2e(args, env, B, torch, dist, world, barrier, stream, mask, act, rew, done)
@@ -227,6 +234,7 @@ def run_b200(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": CFG["name"], "games_per_gpu": n, "variant": "classic", "max_plies": CFG["max_plies"],
                        "auto_reset": 1, "chase_rule": 1 if args.chase_rule else 0,
+                       "games_reset_per_step_fraction": reset_fraction,
                        "policy": "uniform-random legal (Philox4x32-10)",
                        "parallelism": "games sharded over %d GPU(s), no collective" % world,
                        "l2": "outputs 623 MB/step per GPU > 126 MB L2 (no flush needed)"},
