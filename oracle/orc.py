@@ -98,8 +98,9 @@ class Env:
 
     def __del__(self):
         if getattr(self, "h", None) and self.h.value:
-            lib().orc_destroy(self.h)
-            self.h = C.c_void_p()
+            if _lib is not None:  # module globals may be gone at interpreter shutdown
+                _lib.orc_destroy(self.h)
+            self.h = None
 
     def reset(self, seed):
         _chk(lib().orc_reset(self.h, seed), "reset")
@@ -169,8 +170,9 @@ class Replay:
 
     def __del__(self):
         if getattr(self, "h", None) and self.h.value:
-            lib().orc_replay_destroy(self.h)
-            self.h = C.c_void_p()
+            if _lib is not None:
+                _lib.orc_replay_destroy(self.h)
+            self.h = None
 
     def push(self, obs, mask, action, reward, done):
         n = len(action)
