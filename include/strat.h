@@ -246,6 +246,15 @@ int strat_history_transition(const strat_history* h, int64_t t, const int16_t** 
  * done | reason<<2 of the state at t (non-zero only for a frozen finished game; reason 1 =
  * GetFlagCaptured)}. */
 int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* stream);
+/* ComputeTwoSquareRuleApplies(t) uint8[N] (1 iff the two-square rule takes a move away from the
+ * acting player), ComputeIsUnknownPiece(t) uint8[N][100] (1 on squares holding an opponent piece
+ * whose type the acting player has not seen), GetTerminatedSince(t) int32[N] (steps since the
+ * action that ended the game, counted over the steps still in the ring; 0 for a live game)
+ * (PAPER.md:467, 469, 470).  Any of the three outputs may be NULL.  ComputePieceTypeOnehot(t)
+ * is planes 0-23 of strat_history_encode_obs for the types both players know;
+ * the hidden types themselves are in strat_history_get_boards. */
+int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_applies, uint8_t* unknown,
+                        int32_t* terminated_since, void* stream);
 /* Travel back: make the state at time step t the live state of `env` (which need not be the
  * attached one; "efficient capturing of past states", 252-254). */
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream);

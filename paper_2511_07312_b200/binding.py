@@ -25,6 +25,7 @@ EXPORTS = [
     "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
     "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
+    "strat_history_flags",
     "strat_search_expand", "strat_search_policy",
 ]
 
@@ -97,6 +98,7 @@ def lib():
         L.strat_history_transition.argtypes = [vp, i64, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.strat_history_info.argtypes = [vp, i64, vp, vp]
         L.strat_history_restore.argtypes = [vp, i64, vp, vp]
+        L.strat_history_flags.argtypes = [vp, i64, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -383,6 +385,14 @@ class History:
         out = out if out is not None else torch.empty((self.n, 4), dtype=torch.int32, device=self.device)
         _chk(lib().strat_history_info(self.h, t, _ptr(out, torch.int32), _stream()), "strat_history_info")
         return out
+
+    def flags(self, t):
+        """-> (two_square_applies uint8[N], unknown uint8[N,100], terminated_since int32[N])"""
+        ts = torch.empty(self.n, dtype=torch.uint8, device=self.device)
+        unk = torch.empty((self.n, 100), dtype=torch.uint8, device=self.device)
+        since = torch.empty(self.n, dtype=torch.int32, device=self.device)
+        _chk(lib().strat_history_flags(self.h, t, _ptr(ts), _ptr(unk), _ptr(since), _stream()), "strat_history_flags")
+        return ts, unk, since
 
     def restore(self, t, env):
         _chk(lib().strat_history_restore(self.h, t, env.h, _stream()), "strat_history_restore")

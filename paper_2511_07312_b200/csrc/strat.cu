@@ -567,6 +567,24 @@ int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* s
   return launch_status();
 }
 
+int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_applies, uint8_t* unknown,
+                        int32_t* terminated_since, void* stream) {
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || ((uintptr_t)unknown & 3) != 0) return STRAT_BAD_ARG;
+  Params P = h->env ? h->env->P : h->P;
+  P.movelog = nullptr;
+  int n = h->num_games;
+  if (two_square_applies || unknown)
+    k_line_flags<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(P, L, two_square_applies, unknown);
+  if (terminated_since) {
+    int64_t oldest = h->cur - h->length > 0 ? h->cur - h->length : 0;  // oldest recorded step still in the ring
+    int depth = (int)(t - oldest);
+    k_terminated_since<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, L, h->done, h->length, t, depth,
+                                                                         terminated_since);
+  }
+  return launch_status();
+}
+
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream) {
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !env || env->P.num_games != h->num_games) return STRAT_BAD_ARG;

@@ -390,6 +390,61 @@ __global__ void __launch_bounds__(256) k_line_info(int n, const uint32_t* __rest
   reinterpret_cast<int4*>(info)[g] = v;
 }
 
+// ComputeTwoSquareRuleApplies and ComputeIsUnknownPiece of one time step.
+// two_square[g] = 1 iff the two-square rule takes at least one move away from the acting player
+// (the shortest banned distance would be legal without the rule; longer ones follow, R#6);
+// unknown[g][c] = 1 iff square c holds a piece of the opponent whose type the acting player has
+// not seen.  Thread per game; either output may be null.
+__global__ void __launch_bounds__(128) k_line_flags(Params P, const uint32_t* __restrict__ lines,
+                                                    uint8_t* __restrict__ two_square, uint8_t* __restrict__ unknown) {
+  int gi = blockIdx.x * blockDim.x + threadIdx.x;
+  if (gi >= P.num_games) return;
+  Game g;
+  load_game_global(lines, gi, g, nullptr);
+  int side = g.ply & 1u;
+  if (two_square) {
+    uint8_t applies = 0;
+    if (!g.done && P.two_square) {
+      Ban b = two_square_ban(g, side, 1);
+      if (b.from >= 0 && b.k <= 9) {
+        Moves m; single_step_moves(g, side, 0, m);  // the moves without the rule
+        applies = move_in_moves(m, b.from * 36 + b.dir * 9 + b.k - 1) ? 1 : 0;
+      }
+    }
+    two_square[gi] = applies;
+  }
+  if (unknown) {
+    BB occ = occupied(g);
+    BB hidden = bb_andn(bb_andn(occ, owned_by(g, occ, side)), g.rev);
+    uint32_t* out = reinterpret_cast<uint32_t*>(unknown + (size_t)gi * 100);  // 100 B per game: 4-B aligned
+#pragma unroll 5
+    for (int c4 = 0; c4 < 25; ++c4) {
+      uint32_t nib = (bb_word(hidden, (4 * c4) >> 5) >> ((4 * c4) & 31)) & 0xFu;  // cells 4c4..4c4+3 never straddle a word
+      out[c4] = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+    }
+  }
+}
+
+// GetTerminatedSince: for a game that is finished at time step t, the number of
+// steps since the action that ended it = the run of consecutive steps t-1, t-2, ... whose done
+// byte has bit 0 set (a frozen game keeps reporting it, R#15), looked up in the ring's done
+// arrays; 0 for a live game.  `depth` = how many steps before t are still in the ring.
+__global__ void __launch_bounds__(256) k_terminated_since(int n, const uint32_t* __restrict__ lines_t,
+                                                          const uint8_t* __restrict__ ring_done, int length, int64_t t,
+                                                          int depth, int32_t* __restrict__ out) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  int since = 0;
+  if ((lines_t[(size_t)g * kLineWords + 19] >> 4) & 1u) {
+    for (int j = 1; j <= depth; ++j) {
+      size_t slot = (size_t)((t - j) % length);
+      if (!(ring_done[slot * (size_t)n + g] & 1u)) break;
+      since = j;
+    }
+  }
+  out[g] = since;
+}
+
 // A state copied in from elsewhere (history ring) has no move log here: it remembers 8 plies.
 __global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict__ lines) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;

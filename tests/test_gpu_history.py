@@ -116,3 +116,47 @@ def test_history_shape_checks():
     h = B.History(32, 4)
     with pytest.raises(B.StratError):
         h.attach(g)  # game counts differ
+
+
+def test_two_square_applies_unknown_pieces_terminated_since():
+    """The remaining Table S1 queries against plain restatements: the rule
+    'applies' iff switching it off changes the oracle's mask; a piece is unknown iff it is the
+    opponent's and unrevealed; terminated-since counts the steps since the ending action."""
+    n, length, cap = 400, 12, 70
+    kw = dict(variant=0, seed=23, max_plies=cap, auto_reset=0)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    o_off = orc.Env(n, **dict(kw, two_square=0))
+    h = B.History(n, length)
+    h.attach(g)
+    obs = g.new_obs()
+    recs, ended_at = [], np.full(n, -1)
+    applied = 0
+    for t in range(cap + 9):
+        b = o.get_boards()
+        o_off.reset_from(b)
+        ts = (o.legal_mask() != o_off.legal_mask()).any(axis=1).astype(np.uint8)
+        side = (b[:, 116] & 1)[:, None]
+        cells = b[:, :100]
+        piece = ((cells & 15) >= 1) & ((cells & 15) <= 12)
+        unk = (piece & (((cells >> 4) & 1) != side) & ((cells & 0x40) == 0)).astype(np.uint8)
+        finished = (b[:, 120] & 1) == 1
+        since = np.where(finished, t - ended_at, 0).astype(np.int32)
+        recs.append((ts, unk, since))
+        applied += int(ts.sum())
+        r, d = o.step(o.sample_uniform(o.legal_mask()))
+        newly = ((d & 1) == 1) & (ended_at < 0)
+        ended_at[newly] = t
+        g.rollout_step(None, None, None, None, obs)
+    cur = h.current_step()
+    assert cur == cap + 9 and applied > 0 and (ended_at >= 0).all()
+    for t in range(cur - length, cur):
+        ts, unk, since = h.flags(t)
+        e_ts, e_unk, e_since = recs[t]
+        assert np.array_equal(_np(ts), e_ts), t
+        assert np.array_equal(_np(unk), e_unk), t
+        depth = t - (cur - length)                      # steps before t that are still in the ring
+        assert np.array_equal(_np(since), np.minimum(e_since, depth)), t
+    # the live state: every game is frozen since `cur - ended_at` steps, seen through 12 ring steps
+    ts, unk, since = h.flags(cur)
+    assert not _np(ts).any() and (_np(since) == np.minimum(cur - ended_at, length)).all()
+    assert g.check() == 0
