@@ -204,6 +204,10 @@ int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask
  * unless blocks are contiguous (capacity % n == 0 and head % n == 0).
  * strat_replay_commit then appends action/reward/done for those n records and advances head. */
 int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** obs, uint32_t** mask);
+/* The action / reward / done rows of the n records the next commit appends, so that the step
+ * writes them in place as well; strat_replay_commit(r, NULL, NULL, NULL, n, stream) then only
+ * advances head (no copy kernel).  Same contiguity conditions as strat_replay_reserve. */
+int strat_replay_reserve_rows(strat_replay* r, int32_t n, int16_t** action, int8_t** reward, uint8_t** done);
 int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done,
                         int32_t n, void* stream);
 /* Uniform minibatch with replacement: element j = record bounded(sample draw j, filled). */

@@ -21,6 +21,7 @@ EXPORTS = [
     "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
+    "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
     "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
@@ -78,6 +79,7 @@ def lib():
         L.strat_replay_destroy.argtypes = [vp]
         L.strat_replay_push.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
         L.strat_replay_reserve.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(vp)]
+        L.strat_replay_reserve_rows.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.strat_replay_commit.argtypes = [vp, vp, vp, vp, i32, vp]
         L.strat_replay_sample.argtypes = [vp, u64, u64, i32, vp, vp, vp, vp, vp, vp]
         L.strat_replay_state.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -226,6 +228,11 @@ class Env:
         _chk(lib().strat_step_observe(self.h, _ptr(actions, torch.int16), _ptr(reward, torch.int8),
                                       _ptr(done, torch.uint8), _ptr(mask), _ptr(obs), _stream()), "strat_step_observe")
 
+    def rollout_step_ptrs(self, mask_ptr, act_ptr, rew_ptr, done_ptr, obs_ptr):
+        """rollout_step with raw device addresses for all five outputs (the replay ring's rows)."""
+        _chk(lib().strat_rollout_step(self.h, C.c_void_p(mask_ptr), C.c_void_p(act_ptr), C.c_void_p(rew_ptr),
+                                      C.c_void_p(done_ptr), C.c_void_p(obs_ptr), _stream()), "strat_rollout_step")
+
     def rollout_step_raw(self, mask_ptr, actions, reward, done, obs_ptr):
         """rollout_step with raw device addresses for mask/obs (e.g. replay_reserve's)."""
         _chk(lib().strat_rollout_step(self.h, C.c_void_p(mask_ptr), _ptr(actions), _ptr(reward), _ptr(done),
@@ -293,6 +300,14 @@ class Replay:
         obs, mask = C.c_void_p(), C.c_void_p()
         _chk(lib().strat_replay_reserve(self.h, n, ahead, C.byref(obs), C.byref(mask)), "strat_replay_reserve")
         return obs.value, mask.value
+
+    def reserve_rows(self, n):
+        a, r, d = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _chk(lib().strat_replay_reserve_rows(self.h, n, C.byref(a), C.byref(r), C.byref(d)), "strat_replay_reserve_rows")
+        return a.value, r.value, d.value
+
+    def commit_in_place(self, n):
+        _chk(lib().strat_replay_commit(self.h, None, None, None, n, _stream()), "strat_replay_commit")
 
     def commit(self, action, reward, done):
         _chk(lib().strat_replay_commit(self.h, _ptr(action, torch.int16), _ptr(reward, torch.int8),

@@ -450,14 +450,23 @@ int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** o
   return STRAT_OK;
 }
 
-int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done, int32_t n,
-                        void* stream) {
+int strat_replay_reserve_rows(strat_replay* r, int32_t n, int16_t** action, int8_t** reward, uint8_t** done) {
   if (!r || !action || !reward || !done || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0)
     return STRAT_BAD_ARG;
+  *action = r->action + r->head; *reward = r->reward + r->head; *done = r->done + r->head;
+  return STRAT_OK;
+}
+
+int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done, int32_t n,
+                        void* stream) {
+  if (!r || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0) return STRAT_BAD_ARG;
+  if ((action == nullptr) != (reward == nullptr) || (action == nullptr) != (done == nullptr)) return STRAT_BAD_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  copy_elems<int16_t>(action, r->action + r->head, (size_t)n, s);
-  copy_elems<int8_t>(reward, r->reward + r->head, (size_t)n, s);
-  copy_elems<uint8_t>(done, r->done + r->head, (size_t)n, s);
+  if (action) {  // nullptr x 3: the rows were written in place (strat_replay_reserve_rows)
+    copy_elems<int16_t>(action, r->action + r->head, (size_t)n, s);
+    copy_elems<int8_t>(reward, r->reward + r->head, (size_t)n, s);
+    copy_elems<uint8_t>(done, r->done + r->head, (size_t)n, s);
+  }
   r->head = (r->head + n) % r->capacity;
   r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
   return launch_status();

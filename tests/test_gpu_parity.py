@@ -467,8 +467,9 @@ def test_config3_full_size_ring_zero_copy_and_sample():
             expect[(t, lo)] = (oobs.reshape(32, -1).copy(), om.copy(), oa.copy(), orr.copy(), od.copy())
         _, m_ptr = ring.reserve(n, 0)
         o_next, _ = ring.reserve(n, 1)
-        g.rollout_step_raw(m_ptr, act, rew, done, o_next)
-        ring.commit(act, rew, done)
+        a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
+        g.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)
+        ring.commit_in_place(n)
         ring.sample(c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
         head, filled = ring.state()
         assert head == ((t + 1) * n) % cap and filled == min((t + 1) * n, cap)
