@@ -26,7 +26,7 @@ UNIT = "env_steps/s"
 ALGO_BYTES_PER_GAME_STEP = 128 + 128 + 452 + 2 + 1 + 1 + 8800  # state R+W, mask, action, reward, done, obs = 9512
 CFG = W.CONFIGS[2]
 NCU_ROLLOUT_WARP_INST = 1.1005e9  # profiles/r1_g_rollout_uniform_full.md (config 4, one rollout launch)
-NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.4e6  # profiles/r1_j_rollout_step_full.md (65,536 games per launch)
+NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.4e6  # profiles/r1_k_rollout_step_full.md (65,536 games per launch)
 
 
 def measured_peak_gbs():
@@ -241,7 +241,7 @@ def run_b200(args):
             "roofline": {"bound": "hbm", "kernel": "k_rollout_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if n == 65536 else None,
                          "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch "
-                                           "(profiles/r1_j_rollout_step_full.md)",
+                                           "(profiles/r1_k_rollout_step_full.md)",
                          "peak_source": peak_src,
                          "note": "peak is a copy (half reads); a pure write stream exceeds it, hence frac > 1",
                          "algorithmic_bytes_per_game_step": ALGO_BYTES_PER_GAME_STEP,
