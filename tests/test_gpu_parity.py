@@ -290,6 +290,28 @@ def test_fused_steps_of_two_environments_chained_through_a_buffer():
     assert torch.equal(rew_a, rew_b) and torch.equal(done_a, done_b)
 
 
+def test_shards_keyed_by_global_game_index_equal_the_unsharded_run():
+    """Multi-GPU sharding on the CUDA path: two environments that own games
+    [0, n) and [n, 2n) through `game_base` produce exactly the two halves of one 2n-game
+    environment - every RNG draw is keyed by the global game index, no collective is needed."""
+    n = 3000  # not a multiple of 32: the shards' batches do not line up with the big run's
+    kw = dict(variant=0, seed=17, max_plies=50, auto_reset=1)
+    whole = B.Env(2 * n, **kw)
+    parts = [B.Env(n, game_base=0, **kw), B.Env(n, game_base=n, **kw)]
+    outs_w = (whole.new_mask(), whole.new_actions(), whole.new_reward(), whole.new_done(), whole.new_obs())
+    outs_p = [(p.new_mask(), p.new_actions(), p.new_reward(), p.new_done(), p.new_obs()) for p in parts]
+    for _ in range(120):
+        whole.rollout_step(*outs_w)
+        for p, o in zip(parts, outs_p):
+            p.rollout_step(*o)
+    for k in range(2):
+        s = slice(k * n, (k + 1) * n)
+        assert torch.equal(whole.get_boards()[s], parts[k].get_boards())
+        for a, b in zip(outs_w, outs_p[k]):
+            assert torch.equal(a[s].view(torch.uint8), b.view(torch.uint8))
+    assert whole.check() == 0
+
+
 def test_fused_step_interleaved_with_other_calls():
     """A fused step after any other state-changing call (and vice versa) sees that call's result."""
     kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)
