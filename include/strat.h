@@ -115,6 +115,17 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream);
 int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
 int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);
 
+/* Customised initial-board distribution ("The distribution from which the initial
+ * board is sampled can be customized"; the paper trains from a pool of 1,000 network-generated
+ * setups per player per GPU).  pool_dev: uint8[2][K][40] type codes on the device
+ * (K red setups, then K blue setups; entry i of a red setup goes to cell i, of a blue one to cell
+ * 60+i; 0 = empty), caller-owned and read until replaced.  From the next reset / auto-reset on,
+ * each side of a fresh game is pool entry bounded(first draw of the side's setup stream, K),
+ * independently for the two sides (R30).  A setup with a type code above 12 or with no
+ * piece that can ever move raises STRAT_BAD_ARG on the sticky error word (strat_check).
+ * pool_dev == NULL: uniform permutations of the multiset again. */
+int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, void* stream);
+
 /* "Pin" the simulation (Reset Behaviour and Support for Search): while a pin
  * is set, a game that terminates (auto_reset = 1) restarts from ITS pinned state instead of a
  * fresh setup; only the slot's epoch counter keeps counting up, so every restart plays a new

@@ -45,6 +45,7 @@ def lib():
         L.orc_reset_from.argtypes = [vp, vp]
         L.orc_get_boards.argtypes = [vp, vp]
         L.orc_pin_reset_state.argtypes = [vp, vp]
+        L.orc_set_setup_pool.argtypes = [vp, vp, C.c_int32]
         L.orc_legal_mask.argtypes = [vp, vp]
         L.orc_sample_uniform.argtypes = [vp, vp, vp]
         L.orc_step.argtypes = [vp, vp, vp, vp]
@@ -109,6 +110,15 @@ class Env:
         b = np.ascontiguousarray(boards, dtype=np.uint8)
         assert b.shape == (self.n, LINE)
         _chk(lib().orc_reset_from(self.h, _p(b)), "reset_from")
+
+    def set_setup_pool(self, pool):
+        """pool uint8[2][K][40] (red setups, blue setups), or None for uniform permutations."""
+        if pool is None:
+            _chk(lib().orc_set_setup_pool(self.h, None, 0), "set_setup_pool")
+            return
+        p = np.ascontiguousarray(pool, dtype=np.uint8)
+        assert p.ndim == 3 and p.shape[0] == 2 and p.shape[2] == 40
+        _chk(lib().orc_set_setup_pool(self.h, _p(p), p.shape[1]), "set_setup_pool")
 
     def pin_reset_state(self, boards):
         """boards uint8[N][128], or None to unpin."""

@@ -29,10 +29,12 @@
 //                      Bomb/Flag placement over the unmoved squares.
 //   continuous chasing (R#28) pinned: hand-worked chase around a 2x2 block, state-machine
 //                      cases, independent snapshot checker.  The mechanics the paper leaves
-//                      open (what ends a chase, 8-ply memory) are PARITY UNPINNED against it.
+//                      open (what ends a chase, the length of its memory) are PARITY UNPINNED against it.
 //   search step (R#29)  pinned: expansion structure, hand-computed rho and equal-value limit,
 //                      per-action averaging, KKT conditions of eq. (7) at the eq. (8) output.
 //                      The stand-ins for the networks are this build's (R#29), not the paper's.
+//   setup pool (R#30)   pinned: every dealt side is a pool entry, entries are used uniformly
+//                      (chi-square), the two sides draw independently.
 //   pinned reset (R#27) pinned: a restarted game equals its pinned line byte for byte except
 //                      the epoch; the reading itself (epoch keeps counting) is PARITY UNPINNED
 //                      against the paper (P:252-254 gives no detail).
@@ -48,7 +50,7 @@
 //     120 flags: bit0 done, bits2-4 reason (1 flag,2 no-move win,3 no-move draw,
 //             4 ply cap,5 battleless)    121 result (int8, red's)
 //     122..123 chase age of red / blue (R#28; 0 unless chase_rule is on)
-//     122..123 zero           124..127 epoch (LE u32)
+//     124..127 epoch (LE u32)
 //   cell c = 10*row + col; red home rows 0-3, blue home rows 6-9;
 //   lakes {42,43,52,53,46,47,56,57} (BJ configs[0]: c5-d6, g5-h6).
 //   action a = from*36 + dir*9 + (dist-1); dir 0:+row 1:+col 2:-row 3:-col.
@@ -116,10 +118,19 @@ struct Game {
   uint8_t log[64][2];
 };
 
+// "The distribution from which the initial board is sampled can be customized"; in the
+// paper's training a pool of 1,000 network-generated setups per player per GPU.  K setups
+// per side, 40 type codes each (entry i of a red setup -> cell i, of a blue one -> cell 60+i).
+struct SetupPool {
+  int K = 0;
+  std::vector<uint8_t> side[2];
+};
+
 struct Env {
   Config cfg;
   std::vector<Game> g;
   int error;
+  SetupPool pool;
   // "Reset Behaviour and Support for Search": terminated boards restart from a
   // custom non-initial state instead of a fresh setup.  Empty = not pinned.
   std::vector<uint8_t> pin;
@@ -234,11 +245,20 @@ void clear_dynamic(Game& gm) {
   gm.logn = 0;
 }
 
-void new_game(const Config& cfg, uint32_t gidx, Game& gm) {  // epoch already set
+void new_game(const Config& cfg, uint32_t gidx, Game& gm, const SetupPool* pool = nullptr) {  // epoch already set
   memset(gm.cell, 0, sizeof gm.cell);
   for (int c = 0; c < kCells; ++c)
     if (is_lake(c)) gm.cell[c] = T_LAKE;
   clear_dynamic(gm);
+  if (pool && pool->K > 0) {  // R#30: each side's setup = pool entry bounded(first draw of its SETUP stream, K)
+    for (int side = 0; side < 2; ++side) {
+      uint32_t u = stream_draw(cfg.seed, gidx, gm.epoch, 0, side == 0 ? TAG_SETUP_RED : TAG_SETUP_BLUE, 0);
+      const uint8_t* A = &pool->side[side][(size_t)bounded(u, (uint32_t)pool->K) * 40];
+      int base = side == 0 ? 0 : 60;
+      for (int i = 0; i < 40; ++i) gm.cell[base + i] = A[i] == 0 ? 0 : (uint8_t)(A[i] | (side ? B_OWNER : 0));
+    }
+    return;
+  }
   // Each side depends on its own pieces only, so the order of the two is immaterial.
   setup_side(cfg, gidx, gm.epoch, 0, gm.cell);
   setup_side(cfg, gidx, gm.epoch, 1, gm.cell);
@@ -493,7 +513,7 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
       gm.epoch = epoch;
     } else {
       gm.epoch = epoch;
-      new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm);
+      new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm, &e->pool);
     }
   }
 }
@@ -619,8 +639,32 @@ int orc_reset(Env* e, uint64_t seed) {
   e->error = 0;
   for (int i = 0; i < e->cfg.num_games; ++i) {
     e->g[i].epoch = 0;
-    new_game(e->cfg, (uint32_t)(e->cfg.game_base + (uint64_t)i), e->g[i]);
+    new_game(e->cfg, (uint32_t)(e->cfg.game_base + (uint64_t)i), e->g[i], &e->pool);
   }
+  return ORC_OK;
+}
+
+// pool = [2][K][40] type codes (red setups, then blue setups); nullptr / K = 0: uniform permutations
+// again.  A setup must hold type codes 0..12 and leave its side able to move (else BAD_ARG).
+int orc_set_setup_pool(Env* e, const uint8_t* pool, int32_t K) {
+  if (!e) return ORC_BAD_ARG;
+  if (!pool || K <= 0) { e->pool.K = 0; e->pool.side[0].clear(); e->pool.side[1].clear(); return ORC_OK; }
+  for (int side = 0; side < 2; ++side)
+    for (int k = 0; k < K; ++k) {
+      const uint8_t* A = pool + ((size_t)side * K + k) * 40;
+      uint8_t cell[kCells];
+      memset(cell, 0, sizeof cell);
+      for (int c = 0; c < kCells; ++c)
+        if (is_lake(c)) cell[c] = T_LAKE;
+      for (int i = 0; i < 40; ++i) {
+        if (A[i] > 12) return ORC_BAD_ARG;
+        cell[(side ? 60 : 0) + i] = A[i] == 0 ? 0 : (uint8_t)(A[i] | (side ? B_OWNER : 0));
+      }
+      if (!side_can_ever_move(cell, side)) return ORC_BAD_ARG;
+    }
+  e->pool.K = K;
+  e->pool.side[0].assign(pool, pool + (size_t)K * 40);
+  e->pool.side[1].assign(pool + (size_t)K * 40, pool + (size_t)2 * K * 40);
   return ORC_OK;
 }
 

@@ -17,7 +17,7 @@ OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
-    "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_legal_mask", "strat_sample_uniform", "strat_step",
+    "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_set_setup_pool", "strat_legal_mask", "strat_sample_uniform", "strat_step",
     "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
@@ -59,6 +59,7 @@ def lib():
         L.strat_reset_from.argtypes = [vp, vp, vp]
         L.strat_get_boards.argtypes = [vp, vp, vp]
         L.strat_pin_reset_state.argtypes = [vp, vp, vp, vp]
+        L.strat_set_setup_pool.argtypes = [vp, vp, i32, vp]
         L.strat_legal_mask.argtypes = [vp, vp, vp]
         L.strat_sample_uniform.argtypes = [vp, vp, vp, vp]
         L.strat_step.argtypes = [vp, vp, vp, vp, vp]
@@ -180,6 +181,16 @@ class Env:
     def reset_from(self, boards):
         assert boards.shape == (self.n, LINE)
         _chk(lib().strat_reset_from(self.h, _ptr(boards, torch.uint8), _stream()), "strat_reset_from")
+
+    def set_setup_pool(self, pool):
+        """pool uint8[2][K][40] on the device (red setups, blue setups), or None for uniform permutations."""
+        if pool is None:
+            _chk(lib().strat_set_setup_pool(self.h, None, 0, _stream()), "strat_set_setup_pool")
+            self._pool = None
+            return
+        assert pool.dim() == 3 and pool.shape[0] == 2 and pool.shape[2] == 40
+        _chk(lib().strat_set_setup_pool(self.h, _ptr(pool, torch.uint8), pool.shape[1], _stream()), "strat_set_setup_pool")
+        self._pool = pool  # the library reads it until replaced
 
     def pin_reset_state(self, boards):
         """boards uint8[N][128] on the device, or None to unpin."""

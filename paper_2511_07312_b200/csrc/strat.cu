@@ -44,6 +44,7 @@ inline Params make_params(const strat_config& c) {
   P.max_battleless = c.max_battleless; P.auto_reset = c.auto_reset ? 1 : 0; P.two_square = c.two_square ? 1 : 0;
   P.chase_rule = c.chase_rule ? 1 : 0;
   P.movelog = nullptr;
+  P.pool = nullptr; P.pool_size = 0;
   P.pin = nullptr;
   return P;
 }
@@ -238,9 +239,12 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   env->cfg.seed = seed;
   const uint32_t* pin = env->P.pin;
   uint16_t* movelog = env->P.movelog;
+  const uint8_t* pool = env->P.pool;
+  int32_t pool_size = env->P.pool_size;
   env->P = make_params(env->cfg);
   env->P.pin = pin;
   env->P.movelog = movelog;
+  env->P.pool = pool; env->P.pool_size = pool_size;
   k_set_int<<<1, 1, 0, s>>>(env->err, 0);
   k_reset<<<batches(env->P.num_games), 32, 0, s>>>(env->P, env->lines);
   return launch_status();
@@ -250,6 +254,14 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   if (!env || !boards) return STRAT_BAD_ARG;
   int n = env->P.num_games;
   k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  return launch_status();
+}
+
+int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, void* stream) {
+  if (!env) return STRAT_BAD_ARG;
+  if (!pool_dev || K <= 0) { env->P.pool = nullptr; env->P.pool_size = 0; return STRAT_OK; }
+  k_check_pool<<<(2 * K + 127) / 128, 128, 0, (cudaStream_t)stream>>>(pool_dev, K, env->err);
+  env->P.pool = pool_dev; env->P.pool_size = K;
   return launch_status();
 }
 

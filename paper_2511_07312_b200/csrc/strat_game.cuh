@@ -63,6 +63,8 @@ struct Params {  // per-environment constants handed to every kernel by value
   int32_t two_square;
   int32_t chase_rule;      // continuous-chasing rule (R#28)
   uint16_t* movelog;       // [num_games][64] plies played since the state was loaded (chase_rule only), or null
+  const uint8_t* pool;     // custom setups [2][pool_size][40] type codes (red, then blue), or null (R#30)
+  int32_t pool_size;
   const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
 };
 
@@ -699,6 +701,16 @@ SD void setup_game(const Params& P, uint32_t local_game, Game& g) {
   hist_clear(g);
   g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
   uint32_t gidx = P.game_base + local_game;
+  if (P.pool) {  // R#30: each side's setup = pool entry bounded(first draw of its SETUP stream, K)
+    for (int side = 0; side < 2; ++side) {
+      uint32_t o[4];
+      philox(gidx, g.epoch, 0u, side ? TAG_SETUP_BLUE : TAG_SETUP_RED, P.key0, P.key1, o);
+      const uint8_t* A = P.pool + ((size_t)side * P.pool_size + bounded(o[0], (uint32_t)P.pool_size)) * 40;
+      for (int i = 0; i < 40; ++i)
+        if (A[i]) put_piece(g, (side ? 60 : 0) + i, A[i], side);
+    }
+    return;
+  }
   for (int side = 0; side < 2; ++side) {
     for (uint32_t attempt = 0;; ++attempt) {
       uint8_t A[40];

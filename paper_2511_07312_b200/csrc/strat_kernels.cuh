@@ -19,6 +19,18 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   for (uint32_t m = rs; m; m &= m - 1) {
     int owner = __ffs((int)m) - 1;
     uint32_t epoch = __shfl_sync(full, g.epoch, owner);
+    if (P.pool) {  // custom setups (R#30): lanes 0/1 draw the two pool entries, all lanes copy the 80 types
+      uint32_t idx = 0;
+      if (lane < 2) {
+        uint32_t o[4];
+        philox(P.game_base + (uint32_t)(first + owner), epoch, 0u, lane ? TAG_SETUP_BLUE : TAG_SETUP_RED, P.key0, P.key1, o);
+        idx = bounded(o[0], (uint32_t)P.pool_size);
+      }
+      uint32_t i0 = __shfl_sync(full, idx, 0), i1 = __shfl_sync(full, idx, 1);
+      for (int i = lane; i < 80; i += 32)
+        sA[owner * 80 + i] = i < 40 ? P.pool[(size_t)i0 * 40 + i] : P.pool[((size_t)P.pool_size + i1) * 40 + (i - 40)];
+      continue;
+    }
     if (lane < 20) {
       int side = lane >= 10 ? 1 : 0, blk = lane - 10 * side;
       uint32_t o[4];
@@ -30,7 +42,7 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
     for (int i = lane; i < 80; i += 32) sA[owner * 80 + i] = (uint8_t)multiset_type(P.variant, i < 40 ? i : i - 40);
   }
   __syncwarp();
-  if ((rs >> lane) & 1u) {
+  if (((rs >> lane) & 1u) && !P.pool) {
     for (int side = 0; side < 2; ++side) {
       uint8_t* A = sA + lane * 80 + side * 40;
       const uint32_t* D = sD + lane * 80 + side * 40;
@@ -57,7 +69,7 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
     g.mvd = g.rev = bb_zero();
     hist_clear(g);
     g.done = 0; g.reason = 0; g.result = 0; g.ply = 0; g.battleless = 0; g.chase = 0; g.logn = 0;
-    if (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1)) setup_game(P, (uint32_t)(first + lane), g);
+    if (!P.pool && (!side_can_ever_move(g, 0) || !side_can_ever_move(g, 1))) setup_game(P, (uint32_t)(first + lane), g);
   }
   __syncwarp();
 }
@@ -443,6 +455,23 @@ __global__ void __launch_bounds__(256) k_terminated_since(int n, const uint32_t*
     }
   }
   out[g] = since;
+}
+
+// Validates a custom setup pool (R#30): type codes 0..12 and a side that can move.  One thread
+// per setup; raises BAD_ARG on the environment's sticky error word.
+__global__ void __launch_bounds__(128) k_check_pool(const uint8_t* __restrict__ pool, int K, int* __restrict__ err) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * K) return;
+  int side = i >= K ? 1 : 0;
+  const uint8_t* A = pool + (size_t)i * 40;
+  Game g;
+  g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
+  bool ok = true;
+  for (int k = 0; k < 40; ++k) {
+    if (A[k] > 12) ok = false;
+    else if (A[k]) put_piece(g, (side ? 60 : 0) + k, A[k], side);
+  }
+  if (!ok || !side_can_ever_move(g, side)) raise_error(err, STRAT_BAD_ARG);
 }
 
 // A state copied in from elsewhere (history ring) has no move log here: it remembers 8 plies.

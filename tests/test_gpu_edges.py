@@ -234,3 +234,34 @@ def test_large_batch_beyond_4_gib_of_observations():
     x = obs.view(torch.int16)[:, :28].reshape(n, 28, 100)
     assert bool(((x != 0).sum(dim=1) == 1).all())  # planes 0-27 partition the board for every game
     assert g.check() == 0
+
+
+def test_setup_pool_matches_oracle_in_every_reset_path():
+    """Customised initial boards (R30): strat_reset, the cooperative auto-reset of the
+    fused step and of strat_step, and the on-chip rollout's reset all deal the oracle's pool entries."""
+    from test_oracle_game import _random_pool
+    K, n = 11, 700
+    pool = _random_pool(K, 5)
+    kw = dict(variant=0, seed=8, max_plies=9, auto_reset=1)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    g.set_setup_pool(_dev(pool)); o.set_setup_pool(pool)
+    g.reset(8); o.reset(8)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for t in range(40):
+        oa = o.sample_uniform(o.legal_mask()); o.step(oa)
+        if t % 3 == 0:
+            g.rollout_step(mask, act, rew, done, obs)
+        elif t % 3 == 1:
+            g.step(_dev(oa), rew, done)
+        else:
+            g.rollout_uniform(1)
+        assert np.array_equal(_np(g.get_boards()), o.get_boards()), t
+    assert (o.get_boards()[:, 124] >= 4).all() and g.check() == 0
+    g.set_setup_pool(None); o.set_setup_pool(None)
+    for t in range(12):
+        o.step(o.sample_uniform(o.legal_mask())); g.rollout_step(mask, act, rew, done, obs)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    bad = pool.copy(); bad[0, 3, 0] = 14
+    g.set_setup_pool(_dev(bad))
+    assert g.check() == B.BAD_ARG

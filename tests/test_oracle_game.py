@@ -503,3 +503,57 @@ def test_pinned_reset_restarts_from_the_pinned_state():
         b = o.get_boards()
         for i in np.nonzero(d & 1)[0]:
             assert b[i, 116] == 0 and b[i, 117] == 0  # a fresh setup again
+
+
+def _random_pool(K, seed):
+    """K classic setups per side: random permutations of the 40-piece multiset (test input only)."""
+    rng = np.random.default_rng(seed)
+    base = np.array(orc.multiset(0), np.uint8)
+    pool = np.stack([np.stack([rng.permutation(base) for _ in range(K)]) for _ in range(2)])
+    for side in range(2):                      # keep every setup mobile: a Scout on a front lane square
+        for k in range(K):
+            front = 34 if side == 0 else 5     # red's row 3 / blue's row 6 (cell 60+5), files e
+            j = int(np.nonzero(pool[side, k] == 2)[0][0])
+            pool[side, k, [front, j]] = pool[side, k, [j, front]]
+    return pool
+
+
+def test_setup_pool_deals_pool_entries_uniformly_and_independently():
+    """P:234 / R#30: with a pool, every fresh side is one of the pool's setups, chosen uniformly
+    and independently for the two sides."""
+    K, n = 7, 4000
+    pool = _random_pool(K, 1)
+    e = orc.Env(n, seed=3, max_plies=4, auto_reset=1)
+    e.set_setup_pool(pool)
+    e.reset(3)
+    counts = np.zeros((2, K), int)
+    joint = np.zeros((K, K), int)
+    for step in range(13):                     # epoch 0, then the auto-resets of the 4-ply cap (and earlier endings)
+        b = e.get_boards()
+        fresh = np.nonzero((b[:, 116] == 0) & (b[:, 117] == 0))[0]
+        red = b[:, 0:40] & 15
+        blue = b[:, 60:100] & 15
+        for g in fresh:
+            x = int(np.nonzero((pool[0] == red[g]).all(axis=1))[0][0])      # IndexError if the side is no pool entry
+            y = int(np.nonzero((pool[1] == blue[g]).all(axis=1))[0][0])
+            assert ((b[g, 60:100] >> 4) & 1).all() and not ((b[g, 0:40] >> 4) & 1).any()
+            counts[0, x] += 1; counts[1, y] += 1; joint[x, y] += 1
+        e.step(e.sample_uniform(e.legal_mask()))
+    total = int(joint.sum())
+    assert total >= 3 * n
+    for side in range(2):
+        chi2 = ((counts[side] - total / K) ** 2 / (total / K)).sum()
+        assert chi2 < 30, (side, counts[side])                       # 6 dof
+    chi2 = ((joint - total / K / K) ** 2 / (total / K / K)).sum()
+    assert chi2 < 100, joint                                         # 48 dof: independence of the two sides
+    e.set_setup_pool(None)
+    e.reset(3)
+    plain = orc.Env(n, seed=3)
+    assert np.array_equal(e.get_boards(), plain.get_boards())        # uniform permutations again
+    bad = pool.copy(); bad[1, 2, 7] = 13
+    with pytest.raises(RuntimeError):
+        e.set_setup_pool(bad)
+    stuck = pool.copy()
+    stuck[0, 0] = 0; stuck[0, 0, :8] = [11, 12, 12, 12, 12, 12, 12, 0]  # immovables only: cannot ever move
+    with pytest.raises(RuntimeError):
+        e.set_setup_pool(stuck)
