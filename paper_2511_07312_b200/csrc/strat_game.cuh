@@ -562,75 +562,115 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
   return pick_rank(row, cnt, (int)bounded(u, (uint32_t)n));
 }
 // r-th (from 0) legal action in ascending order, given the per-group counts, the non-Scout
-// direction bits D[group][dir] and the Scouts' packed ray lengths (cell | len0<<8 | .. | len3<<20).
+// direction bits D[group][dir] and the Scouts' packed entries
+//   cell | len0<<7 | len1<<11 | len2<<15 | len3<<19 | start<<23,
+// start = rank, inside its 32-cell group, of the Scout's first action.  Either r falls into a
+// Scout's interval, or it is the (r - Scout actions before it)-th action of the non-Scout
+// pieces, whose cell is found by a 5-step binary search on the four direction planes (no walk
+// over the pieces: the lanes stay converged).
 SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r) {
   int gi = 0;
   if (r >= cnt[0]) { r -= cnt[0]; gi = 1; if (r >= cnt[1]) { r -= cnt[1]; gi = 2; if (r >= cnt[2]) { r -= cnt[2]; gi = 3; } } }
+  // Scouts: straight-line code over the 8 possible entries (selects, no branches, no early exit)
+  int before = 0, hit = -1;
+  STRAT_UNROLL
+  for (int k = 0; k < 8; ++k) {
+    uint32_t e = k < ns ? scouts[k] : 0u;
+    bool valid = k < ns && (int)((e & 127u) >> 5) == gi;
+    int l0 = (e >> 7) & 15, l1 = (e >> 11) & 15, l2 = (e >> 15) & 15, l3 = (e >> 19) & 15;
+    int start = (int)(e >> 23), tot = l0 + l1 + l2 + l3;
+    int q = r - start;
+    bool inside = valid && q >= 0 && q < tot;
+    before += (valid && q >= tot) ? tot : 0;
+    int dir = (q >= l0 ? 1 : 0) + (q >= l0 + l1 ? 1 : 0) + (q >= l0 + l1 + l2 ? 1 : 0);
+    int qd = q - (dir > 0 ? l0 : 0) - (dir > 1 ? l1 : 0) - (dir > 2 ? l2 : 0);
+    hit = inside ? (int)(e & 127u) * 36 + dir * 9 + qd : hit;
+  }
+  r -= before;
   uint32_t d0 = gi == 0 ? D[0][0] : gi == 1 ? D[1][0] : gi == 2 ? D[2][0] : D[3][0];
   uint32_t d1 = gi == 0 ? D[0][1] : gi == 1 ? D[1][1] : gi == 2 ? D[2][1] : D[3][1];
   uint32_t d2 = gi == 0 ? D[0][2] : gi == 1 ? D[1][2] : gi == 2 ? D[2][2] : D[3][2];
   uint32_t d3 = gi == 0 ? D[0][3] : gi == 1 ? D[1][3] : gi == 2 ? D[2][3] : D[3][3];
-  uint32_t any = d0 | d1 | d2 | d3;
-  int k = 0;
-  while (k < ns && (int)((scouts[k] & 127u) >> 5) < gi) ++k;  // first Scout of this 32-cell group
-  for (;;) {
-    int bn = any ? sd_ffs(any) - 1 : 32;
-    uint32_t e = k < ns ? scouts[k] : 0xFFu;
-    int bs = ((int)((e & 127u) >> 5) == gi && k < ns) ? (int)(e & 31u) : 32;
-    int b, l0, l1, l2, l3;
-    if (bs < bn) { b = bs; l0 = (e >> 8) & 15; l1 = (e >> 12) & 15; l2 = (e >> 16) & 15; l3 = (e >> 20) & 15; ++k; }
-    else { b = bn; l0 = (d0 >> b) & 1; l1 = (d1 >> b) & 1; l2 = (d2 >> b) & 1; l3 = (d3 >> b) & 1; any &= any - 1; }
-    if (b >= 32) return -1;  // unreachable: r < cnt[gi]
-    int c = l0 + l1 + l2 + l3;
-    if (r < c) {
-      int dir = 0;
-      if (r >= l0) { r -= l0; dir = 1; if (r >= l1) { r -= l1; dir = 2; if (r >= l2) { r -= l2; dir = 3; } } }
-      return (32 * gi + b) * 36 + dir * 9 + r;
-    }
-    r -= c;
+  // non-Scout pieces: smallest bit b with (actions of cells 0..b) > r
+  int b = 0;
+  STRAT_UNROLL
+  for (int s = 16; s >= 1; s >>= 1) {
+    uint32_t below = (1u << (b + s)) - 1u;  // cells 0 .. b+s-1
+    int c = sd_popc(d0 & below) + sd_popc(d1 & below) + sd_popc(d2 & below) + sd_popc(d3 & below);
+    b += c <= r ? s : 0;
   }
+  uint32_t below = (1u << b) - 1u;
+  int q = r - (sd_popc(d0 & below) + sd_popc(d1 & below) + sd_popc(d2 & below) + sd_popc(d3 & below));
+  int l0 = (d0 >> b) & 1, l1 = (d1 >> b) & 1, l2 = (d2 >> b) & 1;
+  int dir = (q >= l0 ? 1 : 0) + (q >= l0 + l1 ? 1 : 0) + (q >= l0 + l1 + l2 ? 1 : 0);
+  return hit >= 0 ? hit : (32 * gi + b) * 36 + dir * 9;
 }
 // SampleRandomLegalAction without materialising the 3600-bit mask (on-chip rollouts): equal to
 // pick_action(legal_mask_row(...)) for the same draw u.  Actions ascend with the from-cell, then
-// the direction, then the distance, so the r-th legal action is found by walking the pieces that
-// can move in cell order with their per-direction counts (1 per open direction; a Scout's ray
-// lengths).  `scouts` = 8 words of per-thread scratch for the Scouts' packed ray lengths.
-SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint32_t* scouts,
-                            const uint16_t* glog = nullptr) {
-  Moves m; single_step_moves(g, side, rules, m);
-  uint32_t D[4][4];
-  int cnt[4], ns = 0;
+// the direction, then the distance, so the r-th legal action follows from per-cell counts (1 per
+// open direction; a Scout's ray lengths).  Two phases, so that a kernel can let its lanes
+// reconverge (__syncwarp) between the Scout loops, whose trip counts differ from game to game,
+// and the selection: count_actions fills an ActionSet, choose_action picks from it.
+// `scouts` = 8 words of per-thread scratch for the Scouts' packed entries.
+struct ActionSet {
+  uint32_t D[4][4];  // non-Scout pieces: D[group][dir] bit b = cell 32*group+b may step in dir
+  int cnt[4];        // legal actions per 32-cell group of from-cells
+  int ns, n;         // Scouts with moves, all legal actions (before chasing-rule bans)
+  Moves m;
+};
+SD void count_actions(const Game& g, int side, int rules, uint32_t* scouts, ActionSet& A) {
+  single_step_moves(g, side, rules, A.m);
+  const Moves& m = A.m;
+  int ns = 0;
+  // 1. non-Scout counts, and the list of Scouts that can move (ascending cells) - a short loop
   STRAT_UNROLL
   for (int i = 0; i < 4; ++i) {
     uint32_t sc = m.scouts.w[i];
     STRAT_UNROLL
-    for (int d = 0; d < 4; ++d) D[i][d] = m.d[d].w[i] & ~sc;
-    cnt[i] = sd_popc(D[i][0]) + sd_popc(D[i][1]) + sd_popc(D[i][2]) + sd_popc(D[i][3]);
+    for (int d = 0; d < 4; ++d) A.D[i][d] = m.d[d].w[i] & ~sc;
+    A.cnt[i] = sd_popc(A.D[i][0]) + sd_popc(A.D[i][1]) + sd_popc(A.D[i][2]) + sd_popc(A.D[i][3]);
     uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
-    while (ss) {
-      int b = sd_ffs(ss) - 1;
-      ss &= ss - 1;
-      int c = 32 * i + b, r = c / 10, q = c - 10 * r;
-      int len[4];
-      scout_rays(m, c, r, q, len);
-      cnt[i] += len[0] + len[1] + len[2] + len[3];
-      if (ns < 8) scouts[ns++] = (uint32_t)c | ((uint32_t)len[0] << 8) | ((uint32_t)len[1] << 12) |
-                                ((uint32_t)len[2] << 16) | ((uint32_t)len[3] << 20);
-    }
+    while (ss && ns < 8) { scouts[ns++] = (uint32_t)(32 * i + sd_ffs(ss) - 1); ss &= ss - 1; }
   }
-  int n = cnt[0] + cnt[1] + cnt[2] + cnt[3];
-  if (n == 0) return -1;
+  // 2. one pass over that list (its length, not the number of Scouts per 32-cell group, sets the
+  //    number of passes a warp makes): ray lengths and the rank of each Scout's first action
+  int grp = -1, scout_actions = 0;
+  for (int k = 0; k < ns; ++k) {
+    int c = (int)scouts[k], i = c >> 5, bit = c & 31, r = c / 10, q = c - 10 * r;
+    int len[4];
+    scout_rays(m, c, r, q, len);
+    scout_actions = i == grp ? scout_actions : 0;  // ranks are relative to the 32-cell group
+    grp = i;
+    uint32_t below = (1u << bit) - 1u;
+    uint32_t e0 = i == 0 ? A.D[0][0] : i == 1 ? A.D[1][0] : i == 2 ? A.D[2][0] : A.D[3][0];
+    uint32_t e1 = i == 0 ? A.D[0][1] : i == 1 ? A.D[1][1] : i == 2 ? A.D[2][1] : A.D[3][1];
+    uint32_t e2 = i == 0 ? A.D[0][2] : i == 1 ? A.D[1][2] : i == 2 ? A.D[2][2] : A.D[3][2];
+    uint32_t e3 = i == 0 ? A.D[0][3] : i == 1 ? A.D[1][3] : i == 2 ? A.D[2][3] : A.D[3][3];
+    int start = sd_popc(e0 & below) + sd_popc(e1 & below) + sd_popc(e2 & below) + sd_popc(e3 & below) + scout_actions;
+    int tot = len[0] + len[1] + len[2] + len[3];  // start < 32*4 + 8*36 < 512
+    scouts[k] = (uint32_t)c | ((uint32_t)len[0] << 7) | ((uint32_t)len[1] << 11) | ((uint32_t)len[2] << 15) |
+                ((uint32_t)len[3] << 19) | ((uint32_t)start << 23);
+    scout_actions += tot;
+    STRAT_UNROLL
+    for (int j = 0; j < 4; ++j) A.cnt[j] += j == i ? tot : 0;
+  }
+  A.ns = ns;
+  A.n = A.cnt[0] + A.cnt[1] + A.cnt[2] + A.cnt[3];
+}
+SD int choose_action(const Game& g, int side, int rules, const ActionSet& A, uint32_t u, const uint32_t* scouts,
+                     const uint16_t* glog = nullptr) {
+  if (A.n == 0) return -1;
   if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: skip the chase-banned threats
     BB occ = occupied(g), mine = owned_by(g, occ, side);
     int banned[kMaxBans];
     int nb = chase_banned_actions(g, side, mine, bb_andn(occ, mine), glog, banned);
-    nb = keep_legal_banned(m, banned, nb);
+    nb = keep_legal_banned(A.m, banned, nb);
     if (nb > 0) {
-      if (n == nb) return -1;
-      int r = (int)bounded(u, (uint32_t)(n - nb));
+      if (A.n == nb) return -1;
+      int r = (int)bounded(u, (uint32_t)(A.n - nb));
       // the r-th action that is not banned: skip the banned ones at or below it (fixed point)
       for (int ra = r;;) {
-        int a = select_action(D, cnt, scouts, ns, ra);
+        int a = select_action(A.D, A.cnt, scouts, A.ns, ra);
         int below = 0;
         for (int i = 0; i < nb; ++i) below += banned[i] <= a ? 1 : 0;
         if (r + below == ra) return a;
@@ -638,7 +678,7 @@ SD int sample_action_direct(const Game& g, int side, int rules, uint32_t u, uint
       }
     }
   }
-  return select_action(D, cnt, scouts, ns, (int)bounded(u, (uint32_t)n));
+  return select_action(A.D, A.cnt, scouts, A.ns, (int)bounded(u, (uint32_t)A.n));
 }
 SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
   uint32_t o[4];

@@ -282,28 +282,44 @@ __global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __r
 }
 
 // `plies` plies of uniform-random legal play with the board in registers.  The 3600-bit mask is
-// never built: the r-th legal action is found from the move bitboards (sample_action_direct).
+// never built: the r-th legal action is found from the move bitboards (count_actions /
+// choose_action).  All 32 lanes run the ply loop together and meet at a __syncwarp after every
+// phase whose length differs from game to game (the Scout ray loops above all), so that the
+// selection and the step run with the warp converged instead of once per group of lanes.
 constexpr int kScoutScratch = 9;  // 8 words per game, odd stride
 template <bool kChase>
 __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   __shared__ uint32_t s_scouts[kBatch * kScoutScratch];
+  const uint32_t full = 0xffffffffu;
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, P.num_games - first);
   load_lines(lines, first, ng, s_state, lane);
-  if (lane < ng) {
-    Game g; read_game(s_state, lane, g);
-    for (int t = 0; t < plies; ++t) {
-      if (g.done) break;  // auto_reset keeps games live; otherwise the game is frozen for good
-      int a = sample_action_direct(g, g.ply & 1u, rules_of<kChase>(P), action_draw(P, (uint32_t)(first + lane), g),
-                                   s_scouts + lane * kScoutScratch, kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
-      if (step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
-        raise_error(err, STRAT_ILLEGAL_ACTION);
-        break;
-      }
+  Game g;
+  bool live = lane < ng;  // still playing: a frozen game (no auto-reset) or a fault ends the lane's rollout
+  if (live) read_game(s_state, lane, g);
+  uint32_t* scouts = s_scouts + lane * kScoutScratch;
+  const uint16_t* glog = kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr;
+  for (int t = 0; t < plies; ++t) {
+    live = live && !g.done;
+    if (!__any_sync(full, live)) break;
+    ActionSet A;
+    uint32_t u = 0;
+    if (live) {
+      u = action_draw(P, (uint32_t)(first + lane), g);
+      count_actions(g, g.ply & 1u, rules_of<kChase>(P), scouts, A);
     }
-    write_game(s_state, lane, g);
+    __syncwarp();
+    int a = -1;
+    if (live) a = choose_action(g, g.ply & 1u, rules_of<kChase>(P), A, u, scouts, glog);
+    __syncwarp();
+    if (live && step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
+      raise_error(err, STRAT_ILLEGAL_ACTION);
+      live = false;
+    }
+    __syncwarp();
   }
+  if (lane < ng) write_game(s_state, lane, g);
   __syncwarp();
   store_lines(lines, first, ng, s_state, lane);
 }
