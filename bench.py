@@ -25,7 +25,7 @@ METRIC = "stratego_env_steps_per_sec"
 UNIT = "env_steps/s"
 ALGO_BYTES_PER_GAME_STEP = 128 + 128 + 452 + 2 + 1 + 1 + 8800  # state R+W, mask, action, reward, done, obs = 9512
 CFG = W.CONFIGS[2]
-NCU_ROLLOUT_WARP_INST = 1.1005e9  # profiles/r1_g_rollout_uniform_full.md (config 4, one rollout launch)
+NCU_ROLLOUT_WARP_INST = 0.9502e9  # profiles/r1_m_rollout_uniform_full.md (config 4, one rollout launch)
 NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.4e6  # profiles/r1_k_rollout_step_full.md (65,536 games per launch)
 
 
@@ -373,7 +373,7 @@ def run_cfg4(args):
         "roofline": {"bound": "alu", "kernel": "k_rollout_uniform", "achieved": NCU_ROLLOUT_WARP_INST / (t_roll / steps / 1e3) / 1e9,
                      "peak": 148 * 4 * 1.965, "unit": "G warp-inst/s",
                      "frac": NCU_ROLLOUT_WARP_INST / (t_roll / steps / 1e3) / 1e9 / (148 * 4 * 1.965), "traffic": 33.6e6 + 33.6e6,
-                     "source": "profiles/r1_g_rollout_uniform_full.md"},
+                     "source": "profiles/r1_m_rollout_uniform_full.md"},
         "gpu_launches": 3 * steps,
     }
     print(json.dumps(line))

@@ -568,13 +568,13 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
 // Scout's interval, or it is the (r - Scout actions before it)-th action of the non-Scout
 // pieces, whose cell is found by a 5-step binary search on the four direction planes (no walk
 // over the pieces: the lanes stay converged).
-SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r) {
+SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r, int kmax = 8) {
   int gi = 0;
   if (r >= cnt[0]) { r -= cnt[0]; gi = 1; if (r >= cnt[1]) { r -= cnt[1]; gi = 2; if (r >= cnt[2]) { r -= cnt[2]; gi = 3; } } }
-  // Scouts: straight-line code over the 8 possible entries (selects, no branches, no early exit)
+  // Scouts: the same selects for every lane over the first kmax entries (kmax >= ns, at most 8;
+  // a kernel passes the largest ns of its warp), no branches, no early exit
   int before = 0, hit = -1;
-  STRAT_UNROLL
-  for (int k = 0; k < 8; ++k) {
+  for (int k = 0; k < kmax; ++k) {
     uint32_t e = k < ns ? scouts[k] : 0u;
     bool valid = k < ns && (int)((e & 127u) >> 5) == gi;
     int l0 = (e >> 7) & 15, l1 = (e >> 11) & 15, l2 = (e >> 15) & 15, l3 = (e >> 19) & 15;
@@ -658,7 +658,7 @@ SD void count_actions(const Game& g, int side, int rules, uint32_t* scouts, Acti
   A.n = A.cnt[0] + A.cnt[1] + A.cnt[2] + A.cnt[3];
 }
 SD int choose_action(const Game& g, int side, int rules, const ActionSet& A, uint32_t u, const uint32_t* scouts,
-                     const uint16_t* glog = nullptr) {
+                     const uint16_t* glog = nullptr, int kmax = 8) {
   if (A.n == 0) return -1;
   if ((rules & RULE_CHASE) && chase_age(g, side) >= 2) {  // rare: skip the chase-banned threats
     BB occ = occupied(g), mine = owned_by(g, occ, side);
@@ -670,7 +670,7 @@ SD int choose_action(const Game& g, int side, int rules, const ActionSet& A, uin
       int r = (int)bounded(u, (uint32_t)(A.n - nb));
       // the r-th action that is not banned: skip the banned ones at or below it (fixed point)
       for (int ra = r;;) {
-        int a = select_action(A.D, A.cnt, scouts, A.ns, ra);
+        int a = select_action(A.D, A.cnt, scouts, A.ns, ra, kmax);
         int below = 0;
         for (int i = 0; i < nb; ++i) below += banned[i] <= a ? 1 : 0;
         if (r + below == ra) return a;
@@ -678,7 +678,7 @@ SD int choose_action(const Game& g, int side, int rules, const ActionSet& A, uin
       }
     }
   }
-  return select_action(A.D, A.cnt, scouts, A.ns, (int)bounded(u, (uint32_t)A.n));
+  return select_action(A.D, A.cnt, scouts, A.ns, (int)bounded(u, (uint32_t)A.n), kmax);
 }
 SD uint32_t action_draw(const Params& P, uint32_t local_game, const Game& g) {
   uint32_t o[4];

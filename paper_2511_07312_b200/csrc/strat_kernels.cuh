@@ -309,9 +309,9 @@ __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __re
       u = action_draw(P, (uint32_t)(first + lane), g);
       count_actions(g, g.ply & 1u, rules_of<kChase>(P), scouts, A);
     }
-    __syncwarp();
+    const int kmax = (int)__reduce_max_sync(full, live ? (unsigned)A.ns : 0u);  // also reconverges the warp
     int a = -1;
-    if (live) a = choose_action(g, g.ply & 1u, rules_of<kChase>(P), A, u, scouts, glog);
+    if (live) a = choose_action(g, g.ply & 1u, rules_of<kChase>(P), A, u, scouts, glog, kmax);
     __syncwarp();
     if (live && step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
       raise_error(err, STRAT_ILLEGAL_ACTION);
