@@ -562,29 +562,27 @@ SD int pick_action(const uint32_t* row, const int cnt[4], int n, uint32_t u) {
   return pick_rank(row, cnt, (int)bounded(u, (uint32_t)n));
 }
 // r-th (from 0) legal action in ascending order, given the per-group counts, the non-Scout
-// direction bits D[group][dir] and the Scouts' packed entries
-//   cell | len0<<7 | len1<<11 | len2<<15 | len3<<19 | start<<23,
-// start = rank, inside its 32-cell group, of the Scout's first action.  Either r falls into a
-// Scout's interval, or it is the (r - Scout actions before it)-th action of the non-Scout
-// pieces, whose cell is found by a 5-step binary search on the four direction planes (no walk
-// over the pieces: the lanes stay converged).
+// direction bits D[group][dir] and two words per Scout that can move:
+//   scouts[2k]   = cell | len0<<7 | len1<<11 | len2<<15 | len3<<19
+//   scouts[2k+1] = start | total<<16 | group<<24, start = rank, inside its 32-cell group, of the
+//                  Scout's first action, total = its number of actions.
+// Either r falls into a Scout's interval, or it is the (r - Scout actions before it)-th action of
+// the non-Scout pieces, whose cell is found by a 5-step binary search on the four direction
+// planes.  No walk over the pieces and no early exit: the lanes of a warp stay converged.
+// kmax >= ns bounds the Scout loop (a kernel passes the largest ns of its warp).
 SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t* scouts, int ns, int r, int kmax = 8) {
   int gi = 0;
   if (r >= cnt[0]) { r -= cnt[0]; gi = 1; if (r >= cnt[1]) { r -= cnt[1]; gi = 2; if (r >= cnt[2]) { r -= cnt[2]; gi = 3; } } }
-  // Scouts: the same selects for every lane over the first kmax entries (kmax >= ns, at most 8;
-  // a kernel passes the largest ns of its warp), no branches, no early exit
-  int before = 0, hit = -1;
+  int before = 0, hit_k = -1, hit_q = 0;
   for (int k = 0; k < kmax; ++k) {
-    uint32_t e = k < ns ? scouts[k] : 0u;
-    bool valid = k < ns && (int)((e & 127u) >> 5) == gi;
-    int l0 = (e >> 7) & 15, l1 = (e >> 11) & 15, l2 = (e >> 15) & 15, l3 = (e >> 19) & 15;
-    int start = (int)(e >> 23), tot = l0 + l1 + l2 + l3;
+    uint32_t w = k < ns ? scouts[2 * k + 1] : 0xFF000000u;  // group 255: never matches
+    int start = (int)(w & 0xFFFFu), tot = (int)((w >> 16) & 0xFFu);
+    bool valid = (int)(w >> 24) == gi;
     int q = r - start;
-    bool inside = valid && q >= 0 && q < tot;
     before += (valid && q >= tot) ? tot : 0;
-    int dir = (q >= l0 ? 1 : 0) + (q >= l0 + l1 ? 1 : 0) + (q >= l0 + l1 + l2 ? 1 : 0);
-    int qd = q - (dir > 0 ? l0 : 0) - (dir > 1 ? l1 : 0) - (dir > 2 ? l2 : 0);
-    hit = inside ? (int)(e & 127u) * 36 + dir * 9 + qd : hit;
+    bool inside = valid && q >= 0 && q < tot;
+    hit_k = inside ? k : hit_k;
+    hit_q = inside ? q : hit_q;
   }
   r -= before;
   uint32_t d0 = gi == 0 ? D[0][0] : gi == 1 ? D[1][0] : gi == 2 ? D[2][0] : D[3][0];
@@ -601,9 +599,16 @@ SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t
   }
   uint32_t below = (1u << b) - 1u;
   int q = r - (sd_popc(d0 & below) + sd_popc(d1 & below) + sd_popc(d2 & below) + sd_popc(d3 & below));
-  int l0 = (d0 >> b) & 1, l1 = (d1 >> b) & 1, l2 = (d2 >> b) & 1;
+  int l0 = (d0 >> b) & 1, l1 = (d1 >> b) & 1, l2 = (d2 >> b) & 1, cell = 32 * gi + b;
+  // a Scout was hit: its ray lengths take the place of the one-step bits
+  uint32_t e = hit_k >= 0 ? scouts[2 * hit_k] : 0u;
+  bool hit = hit_k >= 0;
+  l0 = hit ? (int)((e >> 7) & 15u) : l0; l1 = hit ? (int)((e >> 11) & 15u) : l1; l2 = hit ? (int)((e >> 15) & 15u) : l2;
+  q = hit ? hit_q : q;
+  cell = hit ? (int)(e & 127u) : cell;
   int dir = (q >= l0 ? 1 : 0) + (q >= l0 + l1 ? 1 : 0) + (q >= l0 + l1 + l2 ? 1 : 0);
-  return hit >= 0 ? hit : (32 * gi + b) * 36 + dir * 9;
+  int qd = q - (dir > 0 ? l0 : 0) - (dir > 1 ? l1 : 0) - (dir > 2 ? l2 : 0);
+  return cell * 36 + dir * 9 + qd;
 }
 // SampleRandomLegalAction without materialising the 3600-bit mask (on-chip rollouts): equal to
 // pick_action(legal_mask_row(...)) for the same draw u.  Actions ascend with the from-cell, then
@@ -611,7 +616,7 @@ SD int select_action(const uint32_t (&D)[4][4], const int cnt[4], const uint32_t
 // open direction; a Scout's ray lengths).  Two phases, so that a kernel can let its lanes
 // reconverge (__syncwarp) between the Scout loops, whose trip counts differ from game to game,
 // and the selection: count_actions fills an ActionSet, choose_action picks from it.
-// `scouts` = 8 words of per-thread scratch for the Scouts' packed entries.
+// `scouts` = 16 words of per-thread scratch (two per Scout that can move).
 struct ActionSet {
   uint32_t D[4][4];  // non-Scout pieces: D[group][dir] bit b = cell 32*group+b may step in dir
   int cnt[4];        // legal actions per 32-cell group of from-cells
@@ -622,7 +627,8 @@ SD void count_actions(const Game& g, int side, int rules, uint32_t* scouts, Acti
   single_step_moves(g, side, rules, A.m);
   const Moves& m = A.m;
   int ns = 0;
-  // 1. non-Scout counts, and the list of Scouts that can move (ascending cells) - a short loop
+  // 1. non-Scout counts, and the list of Scouts that can move (ascending cells) with the number of
+  //    non-Scout actions before each inside its 32-cell group - a short loop per group
   STRAT_UNROLL
   for (int i = 0; i < 4; ++i) {
     uint32_t sc = m.scouts.w[i];
@@ -630,26 +636,31 @@ SD void count_actions(const Game& g, int side, int rules, uint32_t* scouts, Acti
     for (int d = 0; d < 4; ++d) A.D[i][d] = m.d[d].w[i] & ~sc;
     A.cnt[i] = sd_popc(A.D[i][0]) + sd_popc(A.D[i][1]) + sd_popc(A.D[i][2]) + sd_popc(A.D[i][3]);
     uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
-    while (ss && ns < 8) { scouts[ns++] = (uint32_t)(32 * i + sd_ffs(ss) - 1); ss &= ss - 1; }
+    while (ss && ns < 8) {
+      int bit = sd_ffs(ss) - 1;
+      ss &= ss - 1;
+      uint32_t below = (1u << bit) - 1u;
+      int pre = sd_popc(A.D[i][0] & below) + sd_popc(A.D[i][1] & below) + sd_popc(A.D[i][2] & below) +
+                sd_popc(A.D[i][3] & below);
+      scouts[2 * ns] = (uint32_t)(32 * i + bit);
+      scouts[2 * ns + 1] = (uint32_t)pre;
+      ++ns;
+    }
   }
   // 2. one pass over that list (its length, not the number of Scouts per 32-cell group, sets the
   //    number of passes a warp makes): ray lengths and the rank of each Scout's first action
   int grp = -1, scout_actions = 0;
   for (int k = 0; k < ns; ++k) {
-    int c = (int)scouts[k], i = c >> 5, bit = c & 31, r = c / 10, q = c - 10 * r;
+    int c = (int)scouts[2 * k], i = c >> 5, r = c / 10, q = c - 10 * r;
     int len[4];
     scout_rays(m, c, r, q, len);
     scout_actions = i == grp ? scout_actions : 0;  // ranks are relative to the 32-cell group
     grp = i;
-    uint32_t below = (1u << bit) - 1u;
-    uint32_t e0 = i == 0 ? A.D[0][0] : i == 1 ? A.D[1][0] : i == 2 ? A.D[2][0] : A.D[3][0];
-    uint32_t e1 = i == 0 ? A.D[0][1] : i == 1 ? A.D[1][1] : i == 2 ? A.D[2][1] : A.D[3][1];
-    uint32_t e2 = i == 0 ? A.D[0][2] : i == 1 ? A.D[1][2] : i == 2 ? A.D[2][2] : A.D[3][2];
-    uint32_t e3 = i == 0 ? A.D[0][3] : i == 1 ? A.D[1][3] : i == 2 ? A.D[2][3] : A.D[3][3];
-    int start = sd_popc(e0 & below) + sd_popc(e1 & below) + sd_popc(e2 & below) + sd_popc(e3 & below) + scout_actions;
-    int tot = len[0] + len[1] + len[2] + len[3];  // start < 32*4 + 8*36 < 512
-    scouts[k] = (uint32_t)c | ((uint32_t)len[0] << 7) | ((uint32_t)len[1] << 11) | ((uint32_t)len[2] << 15) |
-                ((uint32_t)len[3] << 19) | ((uint32_t)start << 23);
+    int start = (int)scouts[2 * k + 1] + scout_actions;  // < 32*4 + 8*36
+    int tot = len[0] + len[1] + len[2] + len[3];
+    scouts[2 * k] = (uint32_t)c | ((uint32_t)len[0] << 7) | ((uint32_t)len[1] << 11) | ((uint32_t)len[2] << 15) |
+                    ((uint32_t)len[3] << 19);
+    scouts[2 * k + 1] = (uint32_t)start | ((uint32_t)tot << 16) | ((uint32_t)i << 24);
     scout_actions += tot;
     STRAT_UNROLL
     for (int j = 0; j < 4; ++j) A.cnt[j] += j == i ? tot : 0;

@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __r
 // choose_action).  All 32 lanes run the ply loop together and meet at a __syncwarp after every
 // phase whose length differs from game to game (the Scout ray loops above all), so that the
 // selection and the step run with the warp converged instead of once per group of lanes.
-constexpr int kScoutScratch = 9;  // 8 words per game, odd stride
+constexpr int kScoutScratch = 17;  // 16 words per game, odd stride
 template <bool kChase>
 __global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
