@@ -25,7 +25,7 @@ METRIC = "stratego_env_steps_per_sec"
 UNIT = "env_steps/s"
 ALGO_BYTES_PER_GAME_STEP = 128 + 128 + 452 + 2 + 1 + 1 + 8800  # state R+W, mask, action, reward, done, obs = 9512
 CFG = W.CONFIGS[2]
-NCU_ROLLOUT_WARP_INST = 0.9502e9  # profiles/r1_m_rollout_uniform_full.md (config 4, one rollout launch)
+NCU_ROLLOUT_WARP_INST = 0.9007e9  # profiles/r1_m_rollout_uniform_full.md (config 4, one rollout launch)
 NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.4e6  # profiles/r1_k_rollout_step_full.md (65,536 games per launch)
 
 
