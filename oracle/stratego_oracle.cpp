@@ -538,11 +538,15 @@ void write_line(const Game& gm, uint8_t* L) {
 void rebuild_chains(Game& gm) {
   gm.chain_len[0] = gm.chain_len[1] = 0;
   for (int j = 7; j >= 0; --j) {
-    if (gm.hist[j][0] == 0xFF) continue;
     // Entries are taken as given (existence = the 0xFF marker only); entry j is the move
     // of ply t-1-j, so its mover is the parity of that number (also when a hand-built
     // line carries more history than plies).
     int side = (gm.ply - 1 - j) & 1;
+    if (gm.hist[j][0] == 0xFF) {
+      // an unknown ply of that player: its "consecutive turns" are interrupted (R#24)
+      gm.chain_len[side] = 0;
+      continue;
+    }
     int from = gm.hist[j][0], to = gm.hist[j][1];
     if (gm.chain_len[side] > 0 && gm.chain[side][gm.chain_len[side] - 1] == from) {
       if (gm.chain_len[side] == 4) {

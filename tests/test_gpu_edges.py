@@ -265,3 +265,55 @@ def test_setup_pool_matches_oracle_in_every_reset_path():
     bad = pool.copy(); bad[0, 3, 0] = 14
     g.set_setup_pool(_dev(bad))
     assert g.check() == B.BAD_ARG
+
+
+def test_hand_built_lines_with_arbitrary_histories():
+    """DESIGN.md R24: a hand-built line may carry any history.  3,000 random positions whose eight
+    history entries are random straight moves (or absent): the two-square ban derived from them,
+    the mask, the observation's history planes and one step must agree with the oracle."""
+    rng = np.random.default_rng(7)
+    n = 3000
+    lines = np.zeros((n, 128), np.uint8)
+    free = [c for c in range(100) if c not in W.LAKES]
+    for i in range(n):
+        k = int(rng.integers(4, 40))
+        cells = rng.choice(free, k, replace=False)
+        pieces = {int(cells[0]): W.piece(W.FLAG, 0), int(cells[1]): W.piece(W.FLAG, 1)}
+        for c in cells[2:]:
+            t = int(rng.integers(1, 11)) if rng.random() < 0.8 else W.BOMB
+            pieces[int(c)] = W.piece(t, int(rng.integers(2)), moved=bool(rng.integers(2)) and t != W.BOMB,
+                                     revealed=bool(rng.integers(2)))
+        hist = []
+        movers = [int(c) for c in cells[2:]]
+        # shuttles of one piece along a line make two-square bans likely; the rest is noise
+        a = movers[int(rng.integers(len(movers)))]
+        r, q = divmod(a, 10)
+        line_cells = [10 * r + x for x in range(10)] if rng.random() < 0.5 else [10 * y + q for y in range(10)]
+        for j in range(8):
+            u = rng.random()
+            if u < 0.15:
+                hist.append((0xFF, 0xFF))
+            elif u < 0.75 and j % 2 == 1:   # entries 1, 3, 5 = the side to move's own last plies
+                f = a if j == 1 else hist[j - 2][0] if hist[j - 2][0] != 0xFF else a
+                t = int(line_cells[int(rng.integers(10))])
+                hist.append((t, f))         # moved t -> f, so the chain ends on the piece's square
+            else:
+                f = int(rng.integers(100)); t = int(rng.integers(100))
+                hist.append((f, t))
+        lines[i] = W.make_line(pieces, ply=int(rng.integers(8, 60)), history=hist)
+    kw = dict(variant=0, seed=1, max_plies=200, auto_reset=0)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    g.reset_from(_dev(lines)); o.reset_from(lines)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    om = o.legal_mask()
+    gm = _np(g.legal_mask()).view(np.uint32)
+    bad = np.nonzero((gm != om).any(axis=1))[0]
+    assert len(bad) == 0, (len(bad), bad[:5])
+    assert np.array_equal(_np(g.encode_obs().view(torch.int16)).view(np.uint16), o.encode_obs())
+    o_off = orc.Env(n, **dict(kw, two_square=0)); o_off.reset_from(lines)
+    assert (o_off.legal_mask() != om).any()    # the two-square rule did bite somewhere
+    oa = o.sample_uniform(om)
+    orr, od = o.step(oa)
+    gr, gd = g.step(_dev(oa))
+    assert np.array_equal(_np(gr), orr) and np.array_equal(_np(gd), od)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
