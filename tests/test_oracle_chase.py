@@ -216,3 +216,20 @@ def test_oracle_masks_equal_the_snapshot_checker_on_biased_random_play():
             chk.pos.append(tuple(int(c) & 0x1F for c in o1.get_boards()[0][:100]))
     assert chases > 100 and bans > 20  # the games did produce chases and banned threats
     print("chase plies", chases, "banned moves", bans)
+
+
+def test_two_square_chain_is_interrupted_by_a_gap_in_a_hand_built_history():
+    """R24 / P:212 "three consecutive turns of its owner": red's Sergeant shuttled 44->45->44->45
+    on red's last three plies (entries 5, 3, 1) - moving back to 44 is banned.  With the same
+    three moves one turn older (entries 7, 5, 3) and red's latest ply unknown (0xFF), nothing
+    says the turns were consecutive: no ban."""
+    pieces = {45: W.piece(SERGEANT, W.RED, moved=True), 95: W.piece(SERGEANT, W.BLUE, moved=True),
+              0: W.piece(FLAG, W.RED), 99: W.piece(FLAG, W.BLUE)}
+    blue = (95, 96)
+    full = [blue, (44, 45), blue, (45, 44), blue, (44, 45), (0xFF, 0xFF), (0xFF, 0xFF)]
+    o = orc.Env(1)
+    o.reset_from(W.make_line(pieces, ply=6, history=full)[None, :])
+    assert A(45, 3, 1) not in _legal(o) and A(45, 0, 1) in _legal(o)
+    gap = [blue, (0xFF, 0xFF), blue, (44, 45), blue, (45, 44), blue, (44, 45)]
+    o.reset_from(W.make_line(pieces, ply=8, history=gap)[None, :])
+    assert A(45, 3, 1) in _legal(o)
