@@ -241,7 +241,7 @@ typedef struct strat_history strat_history;
 size_t strat_history_bytes(int32_t num_games, int32_t length);
 int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, strat_history** out);
 int strat_history_destroy(strat_history* h);
-/* After attach, every strat_step / strat_rollout_step of `env` first records the state it
+/* After attach, every strat_step / strat_rollout_step / strat_step_observe of `env` first records the state it
  * starts from, then the action, reward and done byte, and advances CurrentStep by one (the
  * fused step writes them itself: no copy kernel).  h == NULL detaches.  strat_rollout_uniform
  * refuses to run (STRAT_BAD_STATE) while a history is attached: it keeps the boards on chip
@@ -249,7 +249,8 @@ int strat_history_destroy(strat_history* h);
 int strat_history_attach(strat_env* env, strat_history* h);
 int strat_history_current_step(const strat_history* h, int64_t* step);
 /* ComputeLegalActionMask(t) / ComputeInfostateTensor(t) / BoardStrs(t): same outputs as the
- * live calls produced (or would have produced) at time step t. */
+ * live calls produced (or would have produced) at time step t.  (With chase_rule on, a past
+ * state is judged with the 8 plies its line remembers: the move log belongs to the live state.) */
 int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream);
 int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream);
 int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream);
