@@ -312,6 +312,38 @@ def test_shards_keyed_by_global_game_index_equal_the_unsharded_run():
     assert whole.check() == 0
 
 
+def test_host_buffer_entry_points_match_oracle():
+    """The e2e calls bench.py times: strat_step_host (pinned host actions in; reward, done, next
+    mask, next obs out) and strat_rollout_step_host (all five outputs to host buffers)."""
+    n = 777
+    kw = dict(variant=0, seed=19, max_plies=45, auto_reset=1)
+    g, o = _pair(n, **kw)
+    scratch = g.host_scratch()
+    h_act = torch.empty(n, dtype=torch.int16).pin_memory()
+    h_rew = torch.empty(n, dtype=torch.int8).pin_memory()
+    h_done = torch.empty(n, dtype=torch.uint8).pin_memory()
+    h_mask = torch.empty((n, 113), dtype=torch.int32).pin_memory()
+    h_obs = torch.empty((n, 4400), dtype=torch.bfloat16).pin_memory()
+    om = o.legal_mask()
+    for t in range(70):
+        if t % 2 == 0:
+            oa = o.sample_uniform(om); orr, od = o.step(oa)
+            h_act.copy_(torch.from_numpy(oa))
+            g.step_host(scratch, h_act, h_rew, h_done, h_mask, h_obs)
+            om = o.legal_mask()
+            assert np.array_equal(h_mask.numpy().view(np.uint32), om), t       # mask of the NEW state
+        else:
+            oa = o.sample_uniform(om); orr, od = o.step(oa)
+            g.rollout_step_host(scratch, h_mask, h_act, h_rew, h_done, h_obs)
+            assert np.array_equal(h_mask.numpy().view(np.uint32), om), t       # mask the action was drawn from
+            assert np.array_equal(h_act.numpy(), oa), t
+            om = o.legal_mask()
+        assert np.array_equal(h_rew.numpy(), orr) and np.array_equal(h_done.numpy(), od), t
+        assert np.array_equal(h_obs.view(torch.int16).numpy().view(np.uint16), o.encode_obs().reshape(n, -1)), t
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert g.check() == 0
+
+
 def test_fused_step_interleaved_with_other_calls():
     """A fused step after any other state-changing call (and vice versa) sees that call's result."""
     kw = dict(variant=0, seed=21, max_plies=60, auto_reset=1)
