@@ -154,6 +154,13 @@ def test_fused_step_small_with_auto_reset_and_ragged_tail():
     assert (o.get_boards()[:, 124] >= 3).all()
 
 
+def test_fused_step_barrage_with_frequent_auto_resets():
+    kw = dict(variant=1, seed=14, max_plies=25, auto_reset=1)  # the cooperative reset deals 8 pieces + 32 empties
+    g, o = _pair(650, **kw)
+    _run_fused(g, o, 160, every=9)
+    assert (o.get_boards()[:, 124] >= 5).all()
+
+
 def test_fused_step_null_outputs():
     g1 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
     g2 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
