@@ -161,6 +161,26 @@ def test_fused_step_barrage_with_frequent_auto_resets():
     assert (o.get_boards()[:, 124] >= 5).all()
 
 
+def test_k_move_rule_and_ply_cap_draws():
+    """The k-move rule (draw after k plies without a battle; 100 in training, 200 in
+    evaluation) and the maximum game length, in the fused step and in strat_step."""
+    kw = dict(variant=0, seed=6, max_plies=300, max_battleless=40, auto_reset=1)
+    g, o = B.Env(400, **kw), orc.Env(400, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    reasons = np.zeros(8, int)
+    for t in range(330):
+        oa = o.sample_uniform(o.legal_mask()); orr, od = o.step(oa)
+        if t % 2:
+            g.step(_dev(oa), rew, done)
+        else:
+            g.rollout_step(mask, act, rew, done, obs)
+        assert np.array_equal(_np(rew), orr) and np.array_equal(_np(done), od), t
+        reasons += np.bincount((od[(od & 1) == 1] >> 2) & 7, minlength=8)
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    assert reasons[5] > 0 and reasons[1] + reasons[2] + reasons[4] > 0  # battleless draws and other endings occurred
+    assert g.check() == 0
+
+
 def test_fused_step_null_outputs():
     g1 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
     g2 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
