@@ -181,6 +181,19 @@ def test_k_move_rule_and_ply_cap_draws():
     assert g.check() == 0
 
 
+def test_two_square_rule_switched_off():
+    kw = dict(variant=0, seed=2, max_plies=200, auto_reset=1, two_square=0)
+    g, o = _pair(300, **kw)
+    _run_fused(g, o, 220, every=11)
+    o_on = orc.Env(300, **dict(kw, two_square=1))
+    diff = 0
+    for _ in range(30):  # the switch matters: from the same states the rule-on masks differ sometimes
+        b = o.get_boards(); o_on.reset_from(b)
+        diff += int((o_on.legal_mask() != o.legal_mask()).any(axis=1).sum())
+        o.step(o.sample_uniform(o.legal_mask()))
+    assert diff > 0
+
+
 def test_fused_step_null_outputs():
     g1 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
     g2 = B.Env(500, seed=6, max_plies=80, auto_reset=1)
