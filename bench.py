@@ -25,8 +25,23 @@ METRIC = "stratego_env_steps_per_sec"
 UNIT = "env_steps/s"
 ALGO_BYTES_PER_GAME_STEP = 128 + 128 + 452 + 2 + 1 + 1 + 8800  # state R+W, mask, action, reward, done, obs = 9512
 CFG = W.CONFIGS[2]
-NCU_ROLLOUT_WARP_INST = 0.9007e9  # profiles/r1_m_rollout_uniform_full.md (config 4, one rollout launch)
-NCU_DRAM_BYTES_PER_LAUNCH = 8.5e6 + 555.4e6  # profiles/r1_k_rollout_step_full.md (65,536 games per launch)
+
+
+def ncu_constant(kernel, key):
+    """Per-launch counters taken from an `ncu --set full` capture (profiles/ncu_constants.json
+    names the capture, its command and the commit the kernel was at).  None if not recorded."""
+    try:
+        rec = json.load(open(os.path.join(ROOT, "profiles", "ncu_constants.json")))[kernel]
+        return rec.get(key), "%s @ %s" % (rec.get("source"), rec.get("commit"))
+    except Exception:
+        return None, None
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
 
 
 def measured_peak_gbs():
@@ -97,6 +112,46 @@ def oracle_rate(num_games, steps, warmup):
         one()
     dt = time.perf_counter() - t0
     return num_games * steps / dt, dt
+
+
+def _oracle_shard(q, num_games, steps, warmup, base):
+    from oracle import orc
+    e = orc.Env(num_games, variant=CFG["variant"], seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1,
+                game_base=base)
+
+    def one():
+        e.step(e.sample_uniform(e.legal_mask()))
+        e.encode_obs()
+
+    for _ in range(warmup):
+        one()
+    q.put("ready")
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    q.put(time.perf_counter() - t0)
+
+
+def oracle_rate_all_cores(num_games, steps, warmup):
+    """The same oracle as independent game shards, one process per host core (no tuning): total
+    game-steps / the slowest shard's time."""
+    import multiprocessing as mp
+    cores = host_cores()
+    ctx = mp.get_context("spawn")
+    qs, ps = [], []
+    for k in range(cores):
+        q = ctx.Queue()
+        p = ctx.Process(target=_oracle_shard, args=(q, num_games, steps, warmup, k * num_games), daemon=True)
+        p.start()
+        qs.append(q); ps.append(p)
+    for q in qs:
+        q.get()
+    t0 = time.perf_counter()
+    times = [q.get() for q in qs]
+    wall = time.perf_counter() - t0
+    for p in ps:
+        p.join(timeout=10)
+    return cores * num_games * steps / max(max(times), 1e-9), cores, wall
 
 
 def run_reference(args):
@@ -187,10 +242,11 @@ def run_b200(args):
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    # events only at chunk boundaries: consecutive fused steps overlap on the device (programmatic
-    # dependent launch), and an event record between two launches would serialise them
-    chunk = max(1, args.steps // 20)
-    marks = list(range(0, args.steps, chunk)) + [args.steps]
+    # Consecutive fused steps overlap on the device (programmatic dependent launch) and an event
+    # record between two launches serialises them: events at the two ends of the timed region,
+    # plus interior marks at least 50 launches apart (none below 100 steps).
+    chunk = max(50, args.steps // 20)
+    marks = (list(range(0, args.steps - chunk + 1, chunk)) if args.steps >= 100 else [0]) + [args.steps]
     ev = [torch.cuda.Event(enable_timing=True) for _ in marks]
     ev[0].record(stream)
     nxt = 1
@@ -204,7 +260,7 @@ def run_b200(args):
     sampler.join()
     total_ms = ev[0].elapsed_time(ev[-1])
     per_step = sorted(ev[i].elapsed_time(ev[i + 1]) / (marks[i + 1] - marks[i]) for i in range(len(marks) - 1))
-    median_ms = per_step[len(per_step) // 2]
+    median_ms = per_step[len(per_step) // 2] if len(per_step) >= 3 else None
     assert env.check() == 0
     t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -212,12 +268,27 @@ def run_b200(args):
     total_ms_max = float(t.item())
     value = world * n * args.steps / (total_ms_max / 1e3)
 
-    # outside the timed region: how many games end (and are re-dealt inside the step) per step
-    ended = 0
-    for _ in range(20):
+    # outside the timed region (the steps that follow it): sanity statistics of the workload
+    # (SURVEY.md section 5 "Metrics"): games ended per step, why, how long they were, legal moves
+    stat_steps = 50
+    popc = torch.tensor([bin(i).count("1") for i in range(256)], dtype=torch.int64, device="cuda")
+    ended, legal_sum, len_sum = 0, 0, 0
+    reasons = torch.zeros(8, dtype=torch.int64, device="cuda")
+    for _ in range(stat_steps):
+        b = env.get_boards()
+        ply = b[:, 116].to(torch.int64) | (b[:, 117].to(torch.int64) << 8)
         env.rollout_step(mask, act, rew, done, obs)
-        ended += int((done & 1).sum().item())
-    reset_fraction = ended / (20.0 * n)
+        fin = (done & 1).bool()
+        ended += int(fin.sum().item())
+        len_sum += int((ply[fin] + 1).sum().item())
+        reasons += torch.bincount(((done[fin] >> 2) & 7).to(torch.int64), minlength=8)
+        legal_sum += int(popc[mask.view(torch.uint8).to(torch.int64)].sum().item())
+    reset_fraction = ended / float(stat_steps * n)
+    reason_names = ["", "flag_captured", "no_move_win", "no_move_draw", "ply_cap", "battleless"]
+    stats = {"window": "%d steps after the timed region" % stat_steps, "games_ended": ended,
+             "termination_reasons": {reason_names[k]: int(reasons[k].item()) for k in range(1, 6)},
+             "mean_game_length_plies": (len_sum / ended) if ended else None,
+             "mean_legal_moves": legal_sum / float(stat_steps * n)}
 
     e2e_value, e2e_steps = None, 0
     if not args.skip_e2e:
@@ -226,24 +297,31 @@ def run_b200(args):
         peak, peak_src = measured_peak_gbs()
         kernel_ms = total_ms / args.steps  # the step IS one launch of k_rollout_step
         achieved = ALGO_BYTES_PER_GAME_STEP * n / (kernel_ms / 1e3) / 1e9
-        cpu_games, cpu_steps = 2048, 300
+        cpu_games, cpu_steps = 2048, 150
         cpu_rate, cpu_dt = oracle_rate(cpu_games, cpu_steps, 10) if (world == 1 and not args.skip_cpu) else (None, None)
+        all_rate = all_cores = all_wall = None
+        if cpu_rate is not None:
+            all_rate, all_cores, all_wall = oracle_rate_all_cores(1024, 150, 5)
+        frac = achieved / peak
+        traffic, traffic_src = ncu_constant("k_rollout_step", "dram_bytes_per_launch") if n == 65536 else (None, None)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms_max / args.steps, "median_ms_per_step": median_ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": CFG["name"], "games_per_gpu": n, "variant": "classic", "max_plies": CFG["max_plies"],
                        "auto_reset": 1, "chase_rule": 1 if args.chase_rule else 0,
-                       "games_reset_per_step_fraction": reset_fraction,
+                       "games_reset_per_step_fraction": reset_fraction, "stats": stats,
+                       "event_marks": len(marks),
                        "policy": "uniform-random legal (Philox4x32-10)",
                        "parallelism": "games sharded over %d GPU(s), no collective" % world,
                        "l2": "outputs 623 MB/step per GPU > 126 MB L2 (no flush needed)"},
             "roofline": {"bound": "hbm", "kernel": "k_rollout_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if n == 65536 else None,
-                         "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch "
-                                           "(profiles/r1_k_rollout_step_full.md)",
+                         "frac": frac, "traffic": traffic,
+                         "traffic_source": traffic_src,
                          "peak_source": peak_src,
-                         "note": "peak is a copy (half reads); a pure write stream exceeds it, hence frac > 1",
+                         "note": ("peak is a measured copy (half reads, half writes); this kernel is a pure write "
+                                  "stream with streaming stores and exceeds it, hence frac > 1") if frac > 1.0 else
+                                 "peak is a measured copy (half reads, half writes)",
                          "algorithmic_bytes_per_game_step": ALGO_BYTES_PER_GAME_STEP,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": None if e2e_value is None else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * n * world,
@@ -254,10 +332,38 @@ def run_b200(args):
         }
         if cpu_rate is not None:
             line["cpu_baseline"] = {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": "%d games x %d steps of the same workload (%.1f s)" % (cpu_games, cpu_steps, cpu_dt)}
+                                    "sample": "%d games x %d steps of the same workload (%.1f s)" % (cpu_games, cpu_steps, cpu_dt),
+                                    "host_cores": host_cores(),
+                                    "all_cores": {"value": all_rate, "unit": UNIT, "cores": all_cores,
+                                                  "sample": "independent shards of 1024 games x 150 steps, one oracle process "
+                                                            "per host core (%.1f s)" % all_wall}}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_profile_range(args):
+    """The overlapped regime under ncu's range replay: K consecutive launches of the fused step in
+    one profiled range (they run concurrently as they do in production; per-kernel replay would
+    serialise them).  A number printed by a run under a profiler is not a bench value."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    n = CFG["num_games"]
+    env = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1,
+                chase_rule=1 if args.chase_rule else 0)
+    mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
+    for _ in range(max(args.warmup, 20)):
+        env.rollout_step(mask, act, rew, done, obs)
+    torch.cuda.synchronize()
+    rt = torch.cuda.cudart()
+    rt.cudaProfilerStart()
+    for _ in range(args.profile_range):
+        env.rollout_step(mask, act, rew, done, obs)
+    torch.cuda.synchronize()
+    rt.cudaProfilerStop()
+    assert env.check() == 0
+    print(json.dumps({"profile_range": args.profile_range, "games_per_launch": n,
+                      "algorithmic_bytes_per_launch": ALGO_BYTES_PER_GAME_STEP * n}))
 
 
 def _peak_line(achieved):
@@ -275,7 +381,7 @@ def run_cfg3(args):
     c = W.CONFIGS[3]
     n = c["num_games"]
     env = B.Env(n, variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
-    ring = B.Replay(c["ring_per_slot"], c["ring_slots"])
+    ring = B.Replay(c["ring_per_slot"], c["ring_slots"], block=n)  # spare rows: nothing written ahead is live
     act, rew, done = env.new_actions(), env.new_reward(), env.new_done()
     bs = c["sample_batch"]
     s_obs = torch.empty((bs, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
@@ -324,6 +430,15 @@ def run_cfg3(args):
     print(json.dumps(line))
 
 
+def cfg4_roofline(ms_rollout):
+    inst, src = ncu_constant("k_rollout_uniform", "warp_inst_per_launch")
+    traffic, _ = ncu_constant("k_rollout_uniform", "dram_bytes_per_launch")
+    peak = 148 * 4 * 1.965
+    ach = None if inst is None else inst / (ms_rollout / 1e3) / 1e9
+    return {"bound": "alu", "kernel": "k_rollout_uniform", "achieved": ach, "peak": peak, "unit": "G warp-inst/s",
+            "frac": None if ach is None else ach / peak, "traffic": traffic, "source": src}
+
+
 def run_cfg4(args):
     """BASELINE.json configs[4]: 16 roots (ply 200) x 16,384 determinisations, 64-ply uniform
     rollouts with the boards on chip, per-root reduction.  A 'step' = the whole batch."""
@@ -370,10 +485,7 @@ def run_cfg4(args):
                    "returns_sum_wins_losses_root0": red[0].tolist()},
         # instruction-issue bound: peak = SMs x 4 schedulers x 1 warp instruction per clock x max SM clock
         # (DESIGN.md section 6); achieved = ncu smsp__inst_executed.sum of one rollout launch / its CUDA-event time
-        "roofline": {"bound": "alu", "kernel": "k_rollout_uniform", "achieved": NCU_ROLLOUT_WARP_INST / (t_roll / steps / 1e3) / 1e9,
-                     "peak": 148 * 4 * 1.965, "unit": "G warp-inst/s",
-                     "frac": NCU_ROLLOUT_WARP_INST / (t_roll / steps / 1e3) / 1e9 / (148 * 4 * 1.965), "traffic": 33.6e6 + 33.6e6,
-                     "source": "profiles/r1_m_rollout_uniform_full.md"},
+        "roofline": cfg4_roofline(t_roll / steps),
         "gpu_launches": 3 * steps,
     }
     print(json.dumps(line))
@@ -490,8 +602,13 @@ def main():
                          "of ~10 M updates/s is stated with its anti-chasing rules on, PAPER.md:228)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
+    ap.add_argument("--profile-range", type=int, default=0, metavar="K",
+                    help="profiling runs (ncu --replay-mode range --profile-from-start off): after the warm-up, "
+                         "K back-to-back fused steps between cudaProfilerStart/Stop, nothing else; prints no bench line")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.profile_range:
+        run_profile_range(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.workload == "cfg3":
         run_cfg3(args)

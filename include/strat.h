@@ -87,7 +87,8 @@ typedef struct strat_config {
                              chasing player may not make a threat that recreates a position of
                              the chase, except by moving straight back; memory: 63 plies played in
                              this environment + the 8 plies a loaded line carries), 0: off */
-  uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded) */
+  uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded);
+                             game_base + num_games <= 2^32 (the RNG counter word is 32 bits) */
 } strat_config;
 
 typedef struct strat_env strat_env;       /* host handle; state lives in the workspace */
@@ -106,6 +107,14 @@ size_t strat_workspace_bytes(const strat_config* cfg);
 int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream,
                  strat_env** out);
 int strat_destroy(strat_env* env);
+
+/* Two environments that are used on ONE stream and exchange output buffers (one's fused step
+ * writes what the other's reads or overwrites): afterwards their fused steps are ordered against
+ * each other as plain stream order.  Without it only consecutive fused steps of the SAME
+ * environment overlap (ordered batch by batch), and a fused step is ordered against everything
+ * else the library was asked to do with its environment; fused steps of two unrelated
+ * environments issued back to back on one stream may overlap on the device. */
+int strat_share_chain(strat_env* a, strat_env* b);
 
 /* All games: new Philox key, epoch 0, ply 0, fresh setups. */
 int strat_reset(strat_env* env, uint64_t seed, void* stream);
@@ -197,35 +206,56 @@ int strat_clear_error(strat_env* env, void* stream);
 
 /* ---- device replay ring (BASELINE.json configs[3]) -------------------------------- */
 /* capacity = per_slot * slots records of (obs 8800 B, mask 452 B, action i16, reward i8,
- * done u8) = 9256 B, stored as five arrays over the whole capacity (a "slot" is a
- * contiguous run of per_slot records of each array).  strat_replay_layout returns the byte
- * offset of each array inside the caller's memory: {obs, mask, action, reward, done}. */
+ * done u8) = 9256 B, stored as five arrays (a "slot" is a contiguous run of per_slot records of
+ * each array; R19).  Ring position p in [0, capacity) is where the p-th, (p+capacity)-th,
+ * ... pushed record goes; head = position of the next record, filled = live records.
+ *
+ * Two kinds of ring:
+ *   plain    (strat_replay_create): every array has exactly `capacity` rows, position p = row p;
+ *            filled by strat_replay_push (copying).
+ *   in-place (strat_replay_create_in_place, block = records per push, capacity % block == 0): the
+ *            fused step writes the records itself (strat_replay_reserve / _reserve_rows / _commit).
+ *            In self-play record t = (obs_t, mask_t, a_t, r_t, done_t): step t produces mask_t,
+ *            a_t, r_t, done_t of the block being completed AND obs_{t+1} of the block after it.
+ *            So that what is written ahead never lands in a record that is still live (a record
+ *            pairing a new observation with a 32-steps-old mask and action), the four small arrays
+ *            have capacity + block rows and the observation array capacity + 2*block rows: the
+ *            record with push-order number s lives in row s % rows (s % obs_rows for its
+ *            observation); strat_replay_locate maps a ring position to its rows.
+ * strat_replay_layout returns the byte offset of each array inside the caller's memory:
+ * {obs, mask, action, reward, done} (block = 0 for a plain ring). */
 size_t strat_replay_bytes(int32_t per_slot, int32_t slots);
-int strat_replay_layout(int32_t per_slot, int32_t slots, size_t offsets[5]);
+size_t strat_replay_bytes_in_place(int32_t per_slot, int32_t slots, int32_t block);
+int strat_replay_layout(int32_t per_slot, int32_t slots, int32_t block, size_t offsets[5]);
 int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out);
+int strat_replay_create_in_place(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, int32_t block,
+                                 strat_replay** out);
 int strat_replay_destroy(strat_replay* r);
-/* Append n records in order at (head+i) mod capacity; head += n; filled = min(filled+n, capacity). */
+/* Append n records in order at positions (head+i) mod capacity; head += n; filled = min(filled+n, capacity). */
 int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
                       const int8_t* reward, const uint8_t* done, int32_t n, void* stream);
-/* Zero-copy push: the addresses of the obs and mask rows of the n records starting at
- * head + ahead*n (ahead = 0: the records the next commit appends; ahead = 1: the block after
- * it), so that strat_rollout_step / strat_encode_obs / strat_legal_mask can write them in
- * place: in self-play record t = (obs_t, mask_t, a_t, r_t, done_t), obs_t is produced by step
- * t-1 (ahead = 1 at that time) and mask_t by step t (ahead = 0).  Fails with STRAT_BAD_ARG
- * unless blocks are contiguous (capacity % n == 0 and head % n == 0).
+/* In-place push (in-place rings only; STRAT_BAD_ARG on a plain ring, if n does not divide the
+ * row counts, or if records were pushed that are not a multiple of n): the addresses of the obs
+ * and mask rows of the n records `ahead` blocks after the next one to be committed (ahead = 0:
+ * the records the next commit appends; ahead = 1: the block after it), so that
+ * strat_rollout_step / strat_encode_obs / strat_legal_mask write them where they belong.
  * strat_replay_commit then appends action/reward/done for those n records and advances head. */
 int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** obs, uint32_t** mask);
 /* The action / reward / done rows of the n records the next commit appends, so that the step
  * writes them in place as well; strat_replay_commit(r, NULL, NULL, NULL, n, stream) then only
- * advances head (no copy kernel).  Same contiguity conditions as strat_replay_reserve. */
+ * advances head (no copy kernel). */
 int strat_replay_reserve_rows(strat_replay* r, int32_t n, int16_t** action, int8_t** reward, uint8_t** done);
 int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done,
                         int32_t n, void* stream);
-/* Uniform minibatch with replacement: element j = record bounded(sample draw j, filled). */
+/* Uniform minibatch with replacement: element j = the record at ring position
+ * bounded(sample draw j, filled).  STRAT_BAD_STATE on an empty ring. */
 int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_index, int32_t batch,
                         uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
                         void* stream);
 int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled);
+/* Rows of the live record at ring position p (0 <= p < filled): `row` in the mask / action /
+ * reward / done arrays, `obs_row` in the observation array (both = p for a plain ring). */
+int strat_replay_locate(const strat_replay* r, int64_t p, int64_t* row, int64_t* obs_row);
 
 /* ---- board-history ring and historical queries (Table S1 455-480) ---- */
 /* The paper's rollout buffer: instead of storing information states and masks, keep the game

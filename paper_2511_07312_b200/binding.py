@@ -20,7 +20,8 @@ EXPORTS = [
     "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_set_setup_pool", "strat_legal_mask", "strat_sample_uniform", "strat_step",
     "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
-    "strat_replay_create", "strat_replay_destroy", "strat_replay_push", "strat_replay_reserve",
+    "strat_replay_create", "strat_replay_destroy", "strat_replay_bytes_in_place", "strat_replay_create_in_place",
+    "strat_replay_locate", "strat_share_chain", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
     "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
@@ -75,7 +76,12 @@ def lib():
         L.strat_clear_error.argtypes = [vp, vp]
         L.strat_replay_bytes.restype = sz
         L.strat_replay_bytes.argtypes = [i32, i32]
-        L.strat_replay_layout.argtypes = [i32, i32, C.POINTER(sz)]
+        L.strat_replay_layout.argtypes = [i32, i32, i32, C.POINTER(sz)]
+        L.strat_replay_bytes_in_place.restype = sz
+        L.strat_replay_bytes_in_place.argtypes = [i32, i32, i32]
+        L.strat_replay_create_in_place.argtypes = [vp, sz, i32, i32, i32, C.POINTER(vp)]
+        L.strat_replay_locate.argtypes = [vp, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.strat_share_chain.argtypes = [vp, vp]
         L.strat_replay_create.argtypes = [vp, sz, i32, i32, C.POINTER(vp)]
         L.strat_replay_destroy.argtypes = [vp]
         L.strat_replay_push.argtypes = [vp, vp, vp, vp, vp, vp, i32, vp]
@@ -271,6 +277,9 @@ class Env:
     def rollout_uniform(self, plies):
         _chk(lib().strat_rollout_uniform(self.h, plies, _stream()), "strat_rollout_uniform")
 
+    def share_chain(self, other):
+        _chk(lib().strat_share_chain(self.h, other.h), "strat_share_chain")
+
     def check(self):
         return lib().strat_check(self.h)
 
@@ -281,19 +290,25 @@ class Env:
 class Replay:
     """Device replay ring in a caller-owned (torch) buffer."""
 
-    def __init__(self, per_slot, slots, device=0):
+    def __init__(self, per_slot, slots, device=0, block=0):
+        """block = 0: plain ring (copying push); block = records per in-place push (spare rows)."""
         _require_cuda()
         self.device = torch.device("cuda", device)
-        self.per_slot, self.slots, self.capacity = per_slot, slots, per_slot * slots
-        nbytes = lib().strat_replay_bytes(per_slot, slots)
+        self.per_slot, self.slots, self.capacity, self.block = per_slot, slots, per_slot * slots, block
+        self.rows, self.obs_rows = self.capacity + block, self.capacity + 2 * block
+        nbytes = lib().strat_replay_bytes_in_place(per_slot, slots, block)
         if nbytes == 0:
             raise StratError("bad ring shape")
         self.mem = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         off = (C.c_size_t * 5)()
-        _chk(lib().strat_replay_layout(per_slot, slots, off), "strat_replay_layout")
+        _chk(lib().strat_replay_layout(per_slot, slots, block, off), "strat_replay_layout")
         self.offsets = list(off)
         self.h = C.c_void_p()
-        _chk(lib().strat_replay_create(_ptr(self.mem), nbytes, per_slot, slots, C.byref(self.h)), "strat_replay_create")
+        if block:
+            _chk(lib().strat_replay_create_in_place(_ptr(self.mem), nbytes, per_slot, slots, block, C.byref(self.h)),
+                 "strat_replay_create_in_place")
+        else:
+            _chk(lib().strat_replay_create(_ptr(self.mem), nbytes, per_slot, slots, C.byref(self.h)), "strat_replay_create")
 
     def __del__(self):
         if getattr(self, "h", None) is not None and self.h.value:
@@ -333,15 +348,21 @@ class Replay:
         _chk(lib().strat_replay_state(self.h, C.byref(h), C.byref(f)), "strat_replay_state")
         return h.value, f.value
 
-    # typed views of the ring arrays (tests)
+    def locate(self, p):
+        """(row, obs_row) of the live record at ring position p."""
+        r, o = C.c_int64(), C.c_int64()
+        _chk(lib().strat_replay_locate(self.h, p, C.byref(r), C.byref(o)), "strat_replay_locate")
+        return r.value, o.value
+
+    # typed views of the ring arrays by physical row (tests); see locate()
     def views(self):
-        Cn = self.capacity
+        Rn, Ro = self.rows, self.obs_rows
         o = self.offsets
-        obs = self.mem[o[0]:o[0] + Cn * OBS_ELEMS * 2].view(torch.int16).view(Cn, OBS_ELEMS)
-        mask = self.mem[o[1]:o[1] + Cn * MASK_WORDS * 4].view(torch.int32).view(Cn, MASK_WORDS)
-        act = self.mem[o[2]:o[2] + Cn * 2].view(torch.int16)
-        rew = self.mem[o[3]:o[3] + Cn].view(torch.int8)
-        done = self.mem[o[4]:o[4] + Cn]
+        obs = self.mem[o[0]:o[0] + Ro * OBS_ELEMS * 2].view(torch.int16).view(Ro, OBS_ELEMS)
+        mask = self.mem[o[1]:o[1] + Rn * MASK_WORDS * 4].view(torch.int32).view(Rn, MASK_WORDS)
+        act = self.mem[o[2]:o[2] + Rn * 2].view(torch.int16)
+        rew = self.mem[o[3]:o[3] + Rn].view(torch.int8)
+        done = self.mem[o[4]:o[4] + Rn]
         return obs, mask, act, rew, done
 
 

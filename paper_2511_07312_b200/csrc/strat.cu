@@ -15,6 +15,7 @@
 //   * The single-purpose kernels (k_legal_mask, k_step, k_encode_obs, ...) run one warp per CTA.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <memory>
 #include <mutex>
 #include <new>
 
@@ -33,7 +34,8 @@ using namespace strat;
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool cfg_ok(const strat_config* c) {
   return c && c->num_games >= 1 && (c->variant == 0 || c->variant == 1) && c->max_plies >= 0 &&
-         c->max_battleless >= 0 && (c->chase_rule == 0 || c->chase_rule == 1);
+         c->max_battleless >= 0 && (c->chase_rule == 0 || c->chase_rule == 1) &&
+         c->game_base + (uint64_t)c->num_games <= (1ull << 32);  // RNG counters carry a 32-bit global game index
 }
 inline Params make_params(const strat_config& c) {
   Params P;
@@ -70,17 +72,27 @@ void copy_elems(const T* src, T* dst, size_t count, cudaStream_t s) {
     k_copy<T><<<blocks, 256, 0, s>>>(src, dst, count);
   }
 }
-// records [0,n) of the source go to ring positions (head+i) mod capacity: at most two runs.
+// records [0,n) of the source go to rows (row+i) mod rows of the array: at most two runs (n <= rows).
 template <typename T>
-void push_array(const T* src, T* ring, size_t per_rec, int64_t head, int64_t cap, int64_t n, cudaStream_t s) {
-  int64_t first = n < cap - head ? n : cap - head;
-  copy_elems<T>(src, ring + (size_t)head * per_rec, (size_t)first * per_rec, s);
+void push_array(const T* src, T* ring, size_t per_rec, int64_t row, int64_t rows, int64_t n, cudaStream_t s) {
+  int64_t first = n < rows - row ? n : rows - row;
+  copy_elems<T>(src, ring + (size_t)row * per_rec, (size_t)first * per_rec, s);
   copy_elems<T>(src + (size_t)first * per_rec, ring, (size_t)(n - first) * per_rec, s);
 }
 
 }  // namespace
 
+// Which fused step was launched last on which stream, as far as the environments sharing this
+// record know (one private record per environment; strat_share_chain merges two).  A fused step
+// may skip griddepcontrol.wait only when it directly continues its own environment's chain.
+struct ChainRecord {
+  std::mutex m;
+  const void* stream = nullptr;
+  const strat_env* last = nullptr;
+};
+
 struct strat_env {
+  std::shared_ptr<ChainRecord> chain;
   strat_config cfg;
   strat::Params P;
   uint32_t* lines;
@@ -121,8 +133,16 @@ inline const uint32_t* hist_lines_at(const strat_history* h, int64_t t) {
 }
 }  // namespace
 
+// Record number s (0, 1, 2, ... in push order) lives in row s % rows of the four small arrays and
+// in row s % obs_rows of the observation array; rows = obs_rows = capacity for a plain ring.  A
+// ring made for in-place pushes has spare rows, so that the block a fused step is writing ahead
+// (mask_t ... done_t of the records being completed, obs_{t+1} of the next ones) never aliases a
+// live record.  `head` = total % capacity and the index p of strat_replay_sample are positions in
+// the capacity-sized ring of SURVEY C6 (what the oracle's ring calls a physical record).
 struct strat_replay {
   int64_t per_slot, slots, capacity, head, filled;
+  int64_t total;           // records pushed so far
+  int64_t rows, obs_rows;  // physical rows of mask/action/reward/done, of obs
   uint16_t* obs; uint32_t* mask; int16_t* action; int8_t* reward; uint8_t* done;
 };
 
@@ -131,13 +151,16 @@ namespace {
 // the previous launch in the stream is still running IF that one is also a fused step (the only
 // kernel that executes griddepcontrol.launch_dependents); behind any other kernel the attribute
 // changes nothing.  Ordering against the previous fused step is per batch (f_state / f_obs).
-// The last fused step launched by this process: (stream, environment).  A fused step may skip
-// griddepcontrol.wait only if it directly continues its own environment's chain on the same
-// stream; after a fused step of another environment it must wait for that grid (its inputs may
-// be that step's outputs, and no version flags relate the two).
-std::mutex g_chain_mutex;
-const void* g_chain_stream = nullptr;
-const strat_env* g_chain_env = nullptr;
+// A fused step skips griddepcontrol.wait only if the operation issued immediately before it for
+// this environment (and for every environment sharing its chain record) was a fused step of the
+// SAME environment on the SAME stream: the per-batch version flags then order the two.  Every
+// other entry point that takes the environment breaks the chain (chain_break), and a step with
+// caller-provided actions (kExternal) always waits: its input comes from a foreign kernel.
+inline void chain_break(const strat_env* env) {
+  if (!env || !env->chain) return;
+  std::lock_guard<std::mutex> lock(env->chain->m);
+  env->chain->last = nullptr; env->chain->stream = nullptr;
+}
 
 template <bool kExternal>
 int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done, uint16_t* obs,
@@ -160,9 +183,10 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   const uint32_t version = env->version + 1;
   int wait_prior;
   {
-    std::lock_guard<std::mutex> lock(g_chain_mutex);
-    wait_prior = !(g_chain_env == env && g_chain_stream == stream);
-    g_chain_env = env; g_chain_stream = stream;
+    ChainRecord& rec = *env->chain;
+    std::lock_guard<std::mutex> lock(rec.m);
+    wait_prior = kExternal || !(rec.last == env && rec.stream == stream);
+    rec.last = env; rec.stream = stream;
   }
   auto kernel = env->P.chase_rule ? k_rollout_step<kExternal, true> : k_rollout_step<kExternal, false>;
   if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
@@ -201,6 +225,7 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   if (cudaSetDevice(cfg->device) != cudaSuccess) return STRAT_CUDA_ERROR;
   strat_env* e = new (std::nothrow) strat_env;
   if (!e) return STRAT_BAD_ARG;
+  e->chain = std::make_shared<ChainRecord>();
   e->cfg = *cfg;
   e->P = make_params(*cfg);
   e->lines = reinterpret_cast<uint32_t*>(workspace_dev);
@@ -225,16 +250,21 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
 
 int strat_destroy(strat_env* env) {
   if (env && env->hist) env->hist->env = nullptr;
-  {
-    std::lock_guard<std::mutex> lock(g_chain_mutex);
-    if (g_chain_env == env) { g_chain_env = nullptr; g_chain_stream = nullptr; }
-  }
+  chain_break(env);
   delete env;
+  return STRAT_OK;
+}
+
+int strat_share_chain(strat_env* a, strat_env* b) {
+  if (!a || !b) return STRAT_BAD_ARG;
+  chain_break(a); chain_break(b);
+  b->chain = a->chain;
   return STRAT_OK;
 }
 
 int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   if (!env) return STRAT_BAD_ARG;
+  chain_break(env);
   cudaStream_t s = (cudaStream_t)stream;
   env->cfg.seed = seed;
   const uint32_t* pin = env->P.pin;
@@ -252,6 +282,7 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
 
 int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   if (!env || !boards) return STRAT_BAD_ARG;
+  chain_break(env);
   int n = env->P.num_games;
   k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
   return launch_status();
@@ -259,6 +290,7 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
 
 int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, void* stream) {
   if (!env) return STRAT_BAD_ARG;
+  chain_break(env);
   if (!pool_dev || K <= 0) { env->P.pool = nullptr; env->P.pool_size = 0; return STRAT_OK; }
   k_check_pool<<<(2 * K + 127) / 128, 128, 0, (cudaStream_t)stream>>>(pool_dev, K, env->err);
   env->P.pool = pool_dev; env->P.pool_size = K;
@@ -267,6 +299,7 @@ int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, voi
 
 int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* boards, void* stream) {
   if (!env) return STRAT_BAD_ARG;
+  chain_break(env);
   if (!boards) { env->P.pin = nullptr; return STRAT_OK; }
   if (!pin_lines_dev || ((uintptr_t)pin_lines_dev & 15) != 0) return STRAT_BAD_ARG;
   int n = env->P.num_games;
@@ -277,6 +310,7 @@ int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* bo
 
 int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream) {
   if (!env || !boards) return STRAT_BAD_ARG;
+  chain_break(env);
   int n = env->P.num_games;
   k_export<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, env->lines, boards);
   return launch_status();
@@ -284,6 +318,7 @@ int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream) {
 
 int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream) {
   if (!env || !mask) return STRAT_BAD_ARG;
+  chain_break(env);
   if (env->P.chase_rule) k_legal_mask<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
   else k_legal_mask<false><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask);
   return launch_status();
@@ -291,6 +326,7 @@ int strat_legal_mask(const strat_env* env, uint32_t* mask, void* stream) {
 
 int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* actions, void* stream) {
   if (!env || !mask || !actions) return STRAT_BAD_ARG;
+  chain_break(env);
   int n = env->P.num_games;
   k_sample_uniform<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(env->P, env->lines, mask, actions);
   return launch_status();
@@ -298,6 +334,7 @@ int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* ac
 
 int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream) {
   if (!env || !actions || !reward || !done) return STRAT_BAD_ARG;
+  chain_break(env);
   if (env->P.chase_rule)
     k_step<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done,
                                                                              env->err, hist_slot(env->hist));
@@ -310,6 +347,7 @@ int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* 
 
 int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;
+  chain_break(env);
   k_encode_obs<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, obs);
   return launch_status();
 }
@@ -381,6 +419,7 @@ int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_ho
 
 int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream) {
   if (!env || plies < 0) return STRAT_BAD_ARG;
+  chain_break(env);
   if (env->hist) return STRAT_BAD_STATE;  // on-chip plies are not recorded
   if (env->P.chase_rule)
     k_rollout_uniform<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
@@ -399,42 +438,84 @@ int strat_check(strat_env* env) {
 
 int strat_clear_error(strat_env* env, void* stream) {
   if (!env) return STRAT_BAD_ARG;
+  chain_break(env);
   k_set_int<<<1, 1, 0, (cudaStream_t)stream>>>(env->err, 0);
   return launch_status();
 }
 
 // ---- replay ring
-int strat_replay_layout(int32_t per_slot, int32_t slots, size_t off[5]) {
-  if (per_slot <= 0 || slots <= 0 || !off) return STRAT_BAD_ARG;
-  size_t C = (size_t)per_slot * (size_t)slots, p = 0;
-  off[0] = p; p += align_up(C * STRAT_OBS_ELEMS * 2, 256);
-  off[1] = p; p += align_up(C * STRAT_MASK_WORDS * 4, 256);
-  off[2] = p; p += align_up(C * 2, 256);
-  off[3] = p; p += align_up(C, 256);
-  off[4] = p;
+namespace {
+int replay_layout(int64_t rows, int64_t obs_rows, size_t off[6]) {
+  size_t p = 0;
+  off[0] = p; p += align_up((size_t)obs_rows * STRAT_OBS_ELEMS * 2, 256);
+  off[1] = p; p += align_up((size_t)rows * STRAT_MASK_WORDS * 4, 256);
+  off[2] = p; p += align_up((size_t)rows * 2, 256);
+  off[3] = p; p += align_up((size_t)rows, 256);
+  off[4] = p; p += align_up((size_t)rows, 256);
+  off[5] = p;
   return STRAT_OK;
 }
-
-size_t strat_replay_bytes(int32_t per_slot, int32_t slots) {
-  size_t off[5];
-  if (strat_replay_layout(per_slot, slots, off) != STRAT_OK) return 0;
-  return off[4] + align_up((size_t)per_slot * (size_t)slots, 256);
+inline bool ring_args_ok(int32_t per_slot, int32_t slots, int32_t block) {
+  if (per_slot <= 0 || slots <= 0 || block < 0) return false;
+  int64_t C = (int64_t)per_slot * slots;
+  return C <= 0xFFFFFFFFll && (block == 0 || (block <= C && C % block == 0));
 }
-
-int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out) {
-  size_t need = strat_replay_bytes(per_slot, slots);
-  if (!mem_dev || !out || need == 0 || bytes < need || ((uintptr_t)mem_dev & 255) != 0) return STRAT_BAD_ARG;
+int replay_make(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, int32_t block, strat_replay** out) {
+  if (!mem_dev || !out || !ring_args_ok(per_slot, slots, block) || ((uintptr_t)mem_dev & 255) != 0) return STRAT_BAD_ARG;
+  int64_t C = (int64_t)per_slot * slots, rows = C + block, obs_rows = C + 2 * (int64_t)block;
+  size_t off[6];
+  replay_layout(rows, obs_rows, off);
+  if (bytes < off[5]) return STRAT_BAD_ARG;
   strat_replay* r = new (std::nothrow) strat_replay;
   if (!r) return STRAT_BAD_ARG;
-  size_t off[5];
-  strat_replay_layout(per_slot, slots, off);
   uint8_t* b = reinterpret_cast<uint8_t*>(mem_dev);
-  r->per_slot = per_slot; r->slots = slots; r->capacity = (int64_t)per_slot * slots; r->head = 0; r->filled = 0;
+  r->per_slot = per_slot; r->slots = slots; r->capacity = C; r->head = 0; r->filled = 0; r->total = 0;
+  r->rows = rows; r->obs_rows = obs_rows;
   r->obs = reinterpret_cast<uint16_t*>(b + off[0]); r->mask = reinterpret_cast<uint32_t*>(b + off[1]);
   r->action = reinterpret_cast<int16_t*>(b + off[2]); r->reward = reinterpret_cast<int8_t*>(b + off[3]);
   r->done = b + off[4];
   *out = r;
   return STRAT_OK;
+}
+inline void replay_advance(strat_replay* r, int64_t n) {
+  r->total += n;
+  r->head = r->total % r->capacity;
+  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+}
+// push-order number of the live record at ring position p (0 <= p < filled)
+inline int64_t replay_seq(const strat_replay* r, int64_t p) {
+  int64_t base = r->total - r->filled;
+  return base + ((p - base % r->capacity) + r->capacity) % r->capacity;
+}
+}  // namespace
+
+int strat_replay_layout(int32_t per_slot, int32_t slots, int32_t block, size_t off[5]) {
+  if (!ring_args_ok(per_slot, slots, block) || !off) return STRAT_BAD_ARG;
+  size_t o[6];
+  int64_t C = (int64_t)per_slot * slots;
+  replay_layout(C + block, C + 2 * (int64_t)block, o);
+  for (int i = 0; i < 5; ++i) off[i] = o[i];
+  return STRAT_OK;
+}
+
+size_t strat_replay_bytes(int32_t per_slot, int32_t slots) { return strat_replay_bytes_in_place(per_slot, slots, 0); }
+
+size_t strat_replay_bytes_in_place(int32_t per_slot, int32_t slots, int32_t block) {
+  if (!ring_args_ok(per_slot, slots, block)) return 0;
+  size_t o[6];
+  int64_t C = (int64_t)per_slot * slots;
+  replay_layout(C + block, C + 2 * (int64_t)block, o);
+  return o[5];
+}
+
+int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out) {
+  return replay_make(mem_dev, bytes, per_slot, slots, 0, out);
+}
+
+int strat_replay_create_in_place(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, int32_t block,
+                                 strat_replay** out) {
+  if (block <= 0) return STRAT_BAD_ARG;
+  return replay_make(mem_dev, bytes, per_slot, slots, block, out);
 }
 
 int strat_replay_destroy(strat_replay* r) { delete r; return STRAT_OK; }
@@ -443,44 +524,52 @@ int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask
                       const int8_t* reward, const uint8_t* done, int32_t n, void* stream) {
   if (!r || !obs || !mask || !action || !reward || !done || n < 0 || n > r->capacity) return STRAT_BAD_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  push_array<uint16_t>(obs, r->obs, STRAT_OBS_ELEMS, r->head, r->capacity, n, s);
-  push_array<uint32_t>(mask, r->mask, STRAT_MASK_WORDS, r->head, r->capacity, n, s);
-  push_array<int16_t>(action, r->action, 1, r->head, r->capacity, n, s);
-  push_array<int8_t>(reward, r->reward, 1, r->head, r->capacity, n, s);
-  push_array<uint8_t>(done, r->done, 1, r->head, r->capacity, n, s);
-  r->head = (r->head + n) % r->capacity;
-  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+  int64_t row = r->total % r->rows, orow = r->total % r->obs_rows;
+  push_array<uint16_t>(obs, r->obs, STRAT_OBS_ELEMS, orow, r->obs_rows, n, s);
+  push_array<uint32_t>(mask, r->mask, STRAT_MASK_WORDS, row, r->rows, n, s);
+  push_array<int16_t>(action, r->action, 1, row, r->rows, n, s);
+  push_array<int8_t>(reward, r->reward, 1, row, r->rows, n, s);
+  push_array<uint8_t>(done, r->done, 1, row, r->rows, n, s);
+  replay_advance(r, n);
   return launch_status();
 }
 
+// In-place pushes work in blocks of n records that never wrap inside a block, and need the spare
+// rows of strat_replay_create_in_place: the block written `ahead` pushes ahead must not alias a
+// record that is live when the push in between is sampled.
+static bool in_place_ok(const strat_replay* r, int32_t n, int32_t ahead) {
+  if (!r || n <= 0 || ahead < 0 || ahead > 1) return false;
+  if (r->total % n || r->rows % n || r->obs_rows % n) return false;
+  return r->rows >= r->capacity + n && r->obs_rows >= r->capacity + (int64_t)(ahead + 1) * n;
+}
+
 int strat_replay_reserve(strat_replay* r, int32_t n, int32_t ahead, uint16_t** obs, uint32_t** mask) {
-  if (!r || !obs || !mask || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0 || ahead < 0)
-    return STRAT_BAD_ARG;
-  size_t first = (size_t)((r->head + (int64_t)ahead * n) % r->capacity);
-  *obs = r->obs + first * STRAT_OBS_ELEMS;
-  *mask = r->mask + first * STRAT_MASK_WORDS;
+  if (!obs || !mask || !in_place_ok(r, n, ahead)) return STRAT_BAD_ARG;
+  int64_t first = r->total + (int64_t)ahead * n;
+  *obs = r->obs + (size_t)(first % r->obs_rows) * STRAT_OBS_ELEMS;
+  *mask = r->mask + (size_t)(first % r->rows) * STRAT_MASK_WORDS;
   return STRAT_OK;
 }
 
 int strat_replay_reserve_rows(strat_replay* r, int32_t n, int16_t** action, int8_t** reward, uint8_t** done) {
-  if (!r || !action || !reward || !done || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0)
-    return STRAT_BAD_ARG;
-  *action = r->action + r->head; *reward = r->reward + r->head; *done = r->done + r->head;
+  if (!action || !reward || !done || !in_place_ok(r, n, 0)) return STRAT_BAD_ARG;
+  int64_t row = r->total % r->rows;
+  *action = r->action + row; *reward = r->reward + row; *done = r->done + row;
   return STRAT_OK;
 }
 
 int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* reward, const uint8_t* done, int32_t n,
                         void* stream) {
-  if (!r || n <= 0 || n > r->capacity || r->capacity % n != 0 || r->head % n != 0) return STRAT_BAD_ARG;
+  if (!in_place_ok(r, n, 0)) return STRAT_BAD_ARG;
   if ((action == nullptr) != (reward == nullptr) || (action == nullptr) != (done == nullptr)) return STRAT_BAD_ARG;
   cudaStream_t s = (cudaStream_t)stream;
   if (action) {  // nullptr x 3: the rows were written in place (strat_replay_reserve_rows)
-    copy_elems<int16_t>(action, r->action + r->head, (size_t)n, s);
-    copy_elems<int8_t>(reward, r->reward + r->head, (size_t)n, s);
-    copy_elems<uint8_t>(done, r->done + r->head, (size_t)n, s);
+    int64_t row = r->total % r->rows;
+    copy_elems<int16_t>(action, r->action + row, (size_t)n, s);
+    copy_elems<int8_t>(reward, r->reward + row, (size_t)n, s);
+    copy_elems<uint8_t>(done, r->done + row, (size_t)n, s);
   }
-  r->head = (r->head + n) % r->capacity;
-  r->filled = r->filled + n > r->capacity ? r->capacity : r->filled + n;
+  replay_advance(r, n);
   return launch_status();
 }
 
@@ -489,9 +578,12 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
   if (!r || batch < 0) return STRAT_BAD_ARG;
   if (r->filled == 0) return STRAT_BAD_STATE;
   if (batch == 0) return STRAT_OK;
+  RingMap map;
+  map.filled = (uint32_t)r->filled; map.capacity = (uint64_t)r->capacity; map.base = (uint64_t)(r->total - r->filled);
+  map.rows = (uint64_t)r->rows; map.obs_rows = (uint64_t)r->obs_rows;
   k_replay_sample<<<(batch + 3) / 4, 128, 0, (cudaStream_t)stream>>>(
-      (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), batch,
-      (uint32_t)r->filled, r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done);
+      (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), batch, map,
+      r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done);
   return launch_status();
 }
 
@@ -499,6 +591,14 @@ int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled) {
   if (!r) return STRAT_BAD_ARG;
   if (head) *head = r->head;
   if (filled) *filled = r->filled;
+  return STRAT_OK;
+}
+
+int strat_replay_locate(const strat_replay* r, int64_t p, int64_t* row, int64_t* obs_row) {
+  if (!r || p < 0 || p >= r->filled) return STRAT_BAD_ARG;
+  int64_t s = replay_seq(r, p);
+  if (row) *row = s % r->rows;
+  if (obs_row) *obs_row = s % r->obs_rows;
   return STRAT_OK;
 }
 
@@ -533,6 +633,7 @@ int strat_history_destroy(strat_history* h) {
 
 int strat_history_attach(strat_env* env, strat_history* h) {
   if (!env) return STRAT_BAD_ARG;
+  chain_break(env);
   if (h && (h->num_games != env->P.num_games || (h->env && h->env != env))) return STRAT_BAD_ARG;
   if (env->hist && env->hist != h) env->hist->env = nullptr;
   env->hist = h;
@@ -547,6 +648,7 @@ int strat_history_current_step(const strat_history* h, int64_t* step) {
 }
 
 int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream) {
+  if (h) chain_break(h->env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !mask) return STRAT_BAD_ARG;
   Params P = h->env ? h->env->P : h->P;
@@ -557,6 +659,7 @@ int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, 
 }
 
 int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream) {
+  if (h) chain_break(h->env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !obs) return STRAT_BAD_ARG;
   const Params& P = h->env ? h->env->P : h->P;
@@ -565,6 +668,7 @@ int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, v
 }
 
 int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream) {
+  if (h) chain_break(h->env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !boards) return STRAT_BAD_ARG;
   k_export<<<(h->num_games + 3) / 4, 128, 0, (cudaStream_t)stream>>>(h->num_games, L, boards);
@@ -573,6 +677,7 @@ int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards,
 
 int strat_history_transition(const strat_history* h, int64_t t, const int16_t** actions, const int8_t** reward,
                              const uint8_t** done) {
+  if (h) chain_break(h->env);  // the caller is about to read the rows
   if (!h || t < 0 || t >= h->cur || t < h->cur - h->length) return STRAT_BAD_ARG;
   size_t off = (size_t)(t % h->length) * (size_t)h->num_games;
   if (actions) *actions = h->act + off;
@@ -582,6 +687,7 @@ int strat_history_transition(const strat_history* h, int64_t t, const int16_t** 
 }
 
 int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* stream) {
+  if (h) chain_break(h->env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !info || ((uintptr_t)info & 15) != 0) return STRAT_BAD_ARG;
   k_line_info<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, L, info);
@@ -590,6 +696,7 @@ int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* s
 
 int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_applies, uint8_t* unknown,
                         int32_t* terminated_since, void* stream) {
+  if (h) chain_break(h->env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || ((uintptr_t)unknown & 3) != 0) return STRAT_BAD_ARG;
   Params P = h->env ? h->env->P : h->P;
@@ -607,6 +714,8 @@ int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_a
 }
 
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream) {
+  if (h) chain_break(h->env);
+  chain_break(env);
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !env || env->P.num_games != h->num_games) return STRAT_BAD_ARG;
   if (L != env->lines) {
@@ -621,6 +730,8 @@ int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t
   if (!roots || !out || samples_per_root <= 0 ||
       (int64_t)roots->P.num_games * samples_per_root != (int64_t)out->P.num_games)
     return STRAT_BAD_ARG;
+  chain_break(roots);
+  chain_break(out);
   k_determinise<<<batches(out->P.num_games), 32, 0, (cudaStream_t)stream>>>(
       out->P.num_games, samples_per_root, (uint32_t)seed, (uint32_t)(seed >> 32), out->P.game_base, roots->lines,
       out->lines, out->err);
@@ -631,6 +742,8 @@ int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed,
   if (!roots || !out || rollouts <= 0 || (int64_t)roots->P.num_games * rollouts != (int64_t)out->P.num_games ||
       out->P.auto_reset || out->hist)
     return STRAT_BAD_ARG;
+  chain_break(roots);
+  chain_break(out);
   auto kernel = roots->P.chase_rule ? k_search_expand<true> : k_search_expand<false>;
   kernel<<<batches(out->P.num_games), 32, 0, (cudaStream_t)stream>>>(roots->P, out->P, rollouts, (uint32_t)seed,
                                                                      (uint32_t)(seed >> 32), roots->lines, out->lines, out->err);
@@ -642,6 +755,8 @@ int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t 
   if (!roots || !games || rollouts <= 0 || (int64_t)roots->P.num_games * rollouts != (int64_t)games->P.num_games ||
       !qhat || !rho || !pi_search || !(alpha + beta > 0.f))
     return STRAT_BAD_ARG;
+  chain_break(roots);
+  chain_break(games);
   auto kernel = roots->P.chase_rule ? k_search_policy<true> : k_search_policy<false>;
   kernel<<<roots->P.num_games, kPolicyThreads, 0, (cudaStream_t)stream>>>(roots->P, rollouts, roots->lines, games->lines,
                                                                          pi_theta, alpha, beta, qhat, rho, pi_search);
@@ -652,20 +767,10 @@ int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32
                          void* stream) {
   if (!games || !root_side || !out || samples_per_root <= 0 || games->P.num_games % samples_per_root != 0)
     return STRAT_BAD_ARG;
+  chain_break(games);
   int R = games->P.num_games / samples_per_root;
   k_reduce_returns<<<R, 256, 0, (cudaStream_t)stream>>>(games->lines, root_side, samples_per_root, out);
   return launch_status();
 }
-
-#ifdef STRAT_PROF
-int strat_debug_prof(unsigned long long* out_host, int clear) {
-  if (cudaMemcpyFromSymbol(out_host, g_prof, sizeof(g_prof)) != cudaSuccess) return STRAT_CUDA_ERROR;
-  if (clear) { unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_prof, z, sizeof(z)); }
-  return STRAT_OK;
-}
-int strat_debug_trace(unsigned long long* out_host) {
-  return cudaMemcpyFromSymbol(out_host, g_trace, sizeof(g_trace)) == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR;
-}
-#endif
 
 }  // extern "C"

@@ -13,19 +13,6 @@ using namespace strat;
 // stages to bf16 and streams them out.  The two are decoupled by mbarriers, so on every SM
 // observation stores of batch i flow while batch i+1 is still in its (latency-bound) rule
 // logic; with one-warp CTAs all resident warps ran logic, then stores, in lockstep.
-#ifdef STRAT_PROF  // developer build only (_work/): per-phase cycle counters
-__device__ unsigned long long g_prof[32];
-__device__ unsigned long long g_trace[8192 * 6];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-__device__ __forceinline__ unsigned smid() { unsigned r; asm volatile("mov.u32 %0, %smid;" : "=r"(r)); return r; }
-#define TRACE(b, k, v) do { if (lane == 0 && (b) < 8192) g_trace[(b) * 6 + (k)] = (v); } while (0)
-#define PROF_T(v) long long v = clock64()
-#define PROF_ADD(slot, a, b) do { if (lane == 0) atomicAdd(&g_prof[slot], (unsigned long long)((b) - (a))); } while (0)
-#else
-#define PROF_T(v)
-#define PROF_ADD(slot, a, b)
-#define TRACE(b, k, v)
-#endif
 constexpr int kWsStages = 2;
 // Resident CTAs per SM of ONE launch.  Two consecutive launches are co-resident (6 CTAs x 35.7 KB
 // of shared memory per SM): the later one trails the earlier one batch by batch, so the HBM
@@ -149,7 +136,6 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
     for (int it = 0;; ++it) {
       const int stage = it % kWsStages, round = it / kWsStages;
       uint32_t* work = s_stage[stage];
-      PROF_T(t0);
       if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
       if (it > 0) {
         uint32_t tk = 0;
@@ -164,22 +150,17 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       }
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
       flag_wait(f_state + b, version - 1u, lane);  // the previous launch is done with this batch's state
-      PROF_T(t1);
-      TRACE(b, 0, gtime()); TRACE(b, 4, smid()); TRACE(b, 5, blockIdx.x);
       zero_smem16(work, kMaskBytes, lane);
       Game g;
       int n = 0, cnt[4] = {0, 0, 0, 0};
       if (lane < ng) load_game_global(lines, first + lane, g, hs.lines);
       __syncwarp();
-      PROF_T(t2);
       bool reset_me = false;
       if (!kExternal) {
         if (lane < ng && !g.done) n = legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
                                                        kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
         __syncwarp();
-        PROF_T(t3);
         if (mask) store_mask(mask, first, ng, work, lane);
-        PROF_T(t4);
         if (lane < ng) {
           int a = -1;
           if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
@@ -196,7 +177,6 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         else if (rs) coop_setup(P, first, rs, g, work, lane);
         if (lane < ng) store_game_global(lines, first + lane, g);
         flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
-        PROF_ADD(2, t2, t3); PROF_ADD(3, t3, t4);
       } else {
         if (lane < ng) {
           int a = (int)actions[first + lane];
@@ -225,34 +205,23 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         flag_set(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
       }
       __syncwarp();  // the stage becomes bit streams
-      PROF_T(t5);
       if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
       __syncwarp();
-      PROF_T(t6);
       if (lane == 0) s_batch[stage] = b;
       mbar_arrive(&s_full[stage]);
-      TRACE(b, 1, gtime());
-      PROF_ADD(0, t0, t1); PROF_ADD(1, t1, t2); PROF_ADD(4, t2, t5);
-      PROF_ADD(5, t5, t6); PROF_ADD(6, t0, t6); PROF_ADD(7, 0, 1);
     }
   } else {
     // ------------------------------------------------ store warp (lane per 16-byte chunk)
     for (int it = 0;; ++it) {
       const int stage = it % kWsStages, round = it / kWsStages;
-      PROF_T(t0);
       mbar_wait(&s_full[stage], (uint32_t)round & 1u);
       const int b = s_batch[stage];
       if (b < 0) break;
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
       flag_wait(f_obs + b, version - 1u, lane);  // write-after-write on a reused obs buffer
-      PROF_T(t1);
-      TRACE(b, 2, gtime());
       expand_obs16(obs, first, ng, s_stage[stage], s_lut, lane);
       flag_set(f_obs + b, version, lane);
-      TRACE(b, 3, gtime());
-      PROF_T(t2);
       mbar_arrive(&s_empty[stage]);
-      PROF_ADD(8, t0, t1); PROF_ADD(9, t1, t2); PROF_ADD(10, 0, 1);
     }
   }
 }

@@ -330,9 +330,11 @@ __global__ void k_copy(const T* __restrict__ src, T* __restrict__ dst, size_t co
   size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) dst[i] = src[i];
 }
+// Ring position p (index into the capacity-sized ring) -> push-order number -> rows.
+struct RingMap { uint32_t filled; uint64_t capacity, base /* oldest live record's number */, rows, obs_rows; };
 // one warp per batch element: draw the record index, gather the record.
 __global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
-                                                       uint32_t filled, const uint16_t* __restrict__ r_obs,
+                                                       RingMap map, const uint16_t* __restrict__ r_obs,
                                                        const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
                                                        const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
                                                        uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
@@ -343,9 +345,11 @@ __global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1,
   uint32_t o[4];
   philox((uint32_t)(j >> 2), d0, d1, TAG_SAMPLE, k0, k1, o);
   uint32_t u = (j & 3) == 0 ? o[0] : (j & 3) == 1 ? o[1] : (j & 3) == 2 ? o[2] : o[3];
-  size_t p = bounded(u, filled);
+  uint64_t idx = bounded(u, map.filled);
+  uint64_t seq = map.base + (idx + map.capacity - map.base % map.capacity) % map.capacity;
+  size_t p = (size_t)(seq % map.rows), po = (size_t)(seq % map.obs_rows);
   if (obs) {
-    const uint4* s = reinterpret_cast<const uint4*>(r_obs + p * STRAT_OBS_ELEMS);
+    const uint4* s = reinterpret_cast<const uint4*>(r_obs + po * STRAT_OBS_ELEMS);
     uint4* d = reinterpret_cast<uint4*>(obs + (size_t)j * STRAT_OBS_ELEMS);
     for (int q = lane; q < kObsChunks; q += 32) d[q] = __ldcs(s + q);
   }

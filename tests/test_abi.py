@@ -35,11 +35,22 @@ def test_host_only_entry_points():
     assert L.strat_workspace_bytes(C.byref(bad)) == 0
     assert L.strat_error_string(-4) == b"illegal action for a live game"
     off = (C.c_size_t * 5)()
-    assert L.strat_replay_layout(131072, 64, off) == 0
+    assert L.strat_replay_layout(131072, 64, 0, off) == 0
     cap = 131072 * 64
     assert list(off)[:2] == [0, cap * 8800]
     assert L.strat_replay_bytes(131072, 64) >= cap * 9256
     assert L.strat_replay_bytes(0, 1) == 0
+    # an in-place ring for pushes of 262,144 records: one spare block of rows, two of observations
+    blk = 262144
+    assert L.strat_replay_layout(131072, 64, blk, off) == 0
+    assert list(off)[:3] == [0, (cap + 2 * blk) * 8800, (cap + 2 * blk) * 8800 + (cap + blk) * 452]
+    assert L.strat_replay_bytes_in_place(131072, 64, blk) >= cap * 9256 + blk * (2 * 8800 + 456)
+    assert L.strat_replay_bytes_in_place(131072, 64, 3) == 0  # the block must divide the capacity
+    # RNG counters carry a 32-bit global game index
+    over = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65535)
+    assert L.strat_workspace_bytes(C.byref(over)) == 0
+    edge = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65536)
+    assert L.strat_workspace_bytes(C.byref(edge)) == ws
     # sizes of the per-step outputs the e2e entry point stages
     n = 1000
     cfg = binding.strat_config(n, 0, 0, 0, 0, 0, 1, 0, 0, 0)

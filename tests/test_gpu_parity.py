@@ -409,61 +409,7 @@ def test_fused_step_interleaved_with_other_calls():
     assert g.check() == 0
 
 
-def test_config1_barrage_4096_to_termination_sampled():
-    c = W.CONFIGS[1]
-    kw = dict(variant=1, seed=c["seed"], max_plies=c["max_plies"], auto_reset=0)
-    g = B.Env(c["num_games"], **kw)
-    lo = 4096 - 40  # the oracle mirrors the last 40 games (keyed by global index) ...
-    o = orc.Env(40, game_base=lo, **kw)
-    o2 = orc.Env(24, game_base=1000, **kw)  # ... and 24 from the middle
-    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
-    for t in range(c["steps"]):
-        g.rollout_step(mask, act, rew, done, obs)
-        for oo, base in ((o, lo), (o2, 1000)):
-            om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
-            s = slice(base, base + oo.n)
-            assert np.array_equal(_np(act[s]), oa) and np.array_equal(_np(rew[s]), orr), t
-            assert np.array_equal(_np(done[s]), od), t
-            if t % 100 == 0:
-                assert np.array_equal(_mask_np(mask[s]), om), t
-                assert np.array_equal(_obs_np(obs[s]), oo.encode_obs().reshape(oo.n, 44, 10, 10)), t
-    b = _np(g.get_boards())
-    assert np.array_equal(b[lo:], o.get_boards()) and np.array_equal(b[1000:1024], o2.get_boards())
-    assert (b[:, 120] & 1).all()  # 2000-ply cap: every game is over
-    reasons = np.bincount((b[:, 120] >> 2) & 7, minlength=6)
-    assert reasons[0] == 0 and reasons[1] > 0 and reasons.sum() == 4096
-    # frozen games: zero mask, action -1, reward 0
-    assert not _mask_np(g.legal_mask()).any()
-    assert g.check() == 0
-
-
-def test_config2_full_size_sampled_games():
-    """N = 65,536 in the launch configuration bench.py times; the oracle mirrors three
-    32-game ranges (first, middle, last) by global game index."""
-    c = W.CONFIGS[2]
-    kw = dict(variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
-    g = B.Env(c["num_games"], **kw)
-    ranges = [0, 31337 // 32 * 32, 65536 - 32]
-    os_ = [orc.Env(32, game_base=lo, **kw) for lo in ranges]
-    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
-    for t in range(260):
-        g.rollout_step(mask, act, rew, done, obs)
-        for oo, lo in zip(os_, ranges):
-            om = oo.legal_mask(); oa = oo.sample_uniform(om); orr, od = oo.step(oa)
-            s = slice(lo, lo + 32)
-            assert np.array_equal(_np(act[s]), oa) and np.array_equal(_np(rew[s]), orr), t
-            assert np.array_equal(_np(done[s]), od), t
-            if t % 20 == 0 or t == 259:
-                assert np.array_equal(_mask_np(mask[s]), om), t
-                assert np.array_equal(_obs_np(obs[s]), oo.encode_obs().reshape(32, 44, 10, 10)), t
-    b = _np(g.get_boards())
-    for oo, lo in zip(os_, ranges):
-        assert np.array_equal(b[lo:lo + 32], oo.get_boards())
-    # properties that hold at any size
-    x = (_obs_np(obs) == 0x3F80)
-    assert set(np.unique(_obs_np(obs[:4096]))) <= {0, 0x3F80}
-    assert (x[:, :28].sum(axis=1) == 1).all()
-    assert g.check() == 0
+# configs 1 and 2 at full size, ALL games mirrored: tests/test_gpu_allgames.py
 
 
 # ----------------------------------------------------------------------------- replay ring (config 3 shape)
@@ -498,50 +444,69 @@ def test_replay_ring_push_commit_sample_match_oracle():
         assert (int(va[p]), int(vr[p]), int(vd[p])) == (ea, er, ed)
 
 
-def test_replay_zero_copy_reserve_commit_equals_push():
-    """Self-play loop of config 3 two ways: (1) separate calls + copying push, (2) the fused
-    step writing mask_t and obs_{t+1} straight into the ring rows + commit."""
+@pytest.mark.parametrize("rows_in_place", [False, True])
+def test_replay_in_place_push_equals_oracle_ring_records_and_samples(rows_in_place):
+    """Self-play loop of config 3 with the fused step writing mask_t (and optionally action_t,
+    reward_t, done_t) and obs_{t+1} straight into the ring rows.  After every push, wrapped or
+    not, every sampled (obs, mask, action, reward, done) record equals the oracle ring's, and at
+    the end every live ring position holds the oracle's record: what is written ahead never lands
+    in a live record (the ring's spare rows)."""
     n = 64
     kw = dict(variant=0, seed=3, max_plies=50, auto_reset=1)
-    g1, g2 = B.Env(n, **kw), B.Env(n, **kw)
-    r1, r2 = B.Replay(32, 8), B.Replay(32, 8)  # capacity 256 = 4 blocks of 64
-    act, rew, done = g2.new_actions(), g2.new_reward(), g2.new_done()
-    obs_t = g1.encode_obs()
-    o_ptr, _ = r2.reserve(n, 0)
-    B._chk(B.lib().strat_encode_obs(g2.h, o_ptr, B._stream()), "encode")  # obs_0 in place
-    for t in range(9):  # wraps the ring twice
-        m = g1.legal_mask(); a = g1.sample_uniform(m); r, d = g1.step(a)
-        r1.push(obs_t, m, a, r, d)
-        obs_t = g1.encode_obs()
-        _, m_ptr = r2.reserve(n, 0)        # mask_t -> the rows being completed
-        o_next, _ = r2.reserve(n, 1)       # obs_{t+1} -> the rows of the next block
-        g2.rollout_step_raw(m_ptr, act, rew, done, o_next)
-        r2.commit(act, rew, done)
-    assert r1.state() == r2.state()
-    h, _ = r1.state()
-    v1, v2 = r1.views(), r2.views()
-    keep = torch.ones(r1.capacity, dtype=torch.bool, device="cuda")
-    keep[h:h + n] = False  # r2 already holds obs_9 in the block the next commit will complete
-    for a_, b_ in zip(v1[1:], v2[1:]):
-        assert torch.equal(a_, b_)
-    assert torch.equal(v1[0][keep], v2[0][keep])
-    assert torch.equal(v2[0][h:h + n].view(n, -1), obs_t.view(torch.int16).view(n, -1))
-    assert torch.equal(g1.get_boards(), g2.get_boards())
-
+    g, o = _pair(n, **kw)
+    ring, oring = B.Replay(32, 8, block=n), orc.Replay(32, 8)  # capacity 256 = 4 blocks of 64
+    act, rew, done = g.new_actions(), g.new_reward(), g.new_done()
+    batch = 700
+    s_obs = torch.empty((batch, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    s_mask = torch.empty((batch, 113), dtype=torch.int32, device="cuda")
+    s_act = torch.empty(batch, dtype=torch.int16, device="cuda")
+    s_rew = torch.empty(batch, dtype=torch.int8, device="cuda")
+    s_done = torch.empty(batch, dtype=torch.uint8, device="cuda")
+    o_ptr, _ = ring.reserve(n, 0)
+    B._chk(B.lib().strat_encode_obs(g.h, o_ptr, B._stream()), "encode")  # obs_0 in place
+    for t in range(11):  # wraps the ring twice
+        oobs = o.encode_obs(); om = o.legal_mask(); oa = o.sample_uniform(om); orr, od = o.step(oa)
+        oring.push(oobs, om, oa, orr, od)
+        _, m_ptr = ring.reserve(n, 0)        # mask_t -> the rows being completed
+        o_next, _ = ring.reserve(n, 1)       # obs_{t+1} -> the rows of the next block
+        if rows_in_place:
+            a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
+            g.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)
+            ring.commit_in_place(n)
+        else:
+            g.rollout_step_raw(m_ptr, act, rew, done, o_next)
+            ring.commit(act, rew, done)
+        assert ring.state() == (oring.head, oring.filled)
+        ring.sample(77, t, batch, s_obs, s_mask, s_act, s_rew, s_done)
+        eo, em, ea, er, ed, idx = oring.sample(77, t, batch)
+        assert np.array_equal(_obs_np(s_obs), eo) and np.array_equal(_mask_np(s_mask), em), t
+        assert np.array_equal(_np(s_act), ea) and np.array_equal(_np(s_rew), er) and np.array_equal(_np(s_done), ed), t
+    vo, vm, va, vr, vd = ring.views()
+    for p in range(ring.capacity):
+        row, orow = ring.locate(p)
+        eo, em, ea, er, ed = oring.read(p)
+        assert np.array_equal(_np(vo[orow]).view(np.uint16), eo.reshape(-1)), p
+        assert np.array_equal(_np(vm[row]).view(np.uint32), em), p
+        assert (int(va[row]), int(vr[row]), int(vd[row])) == (ea, er, ed), p
+    assert np.array_equal(_np(g.get_boards()), o.get_boards())
+    # a plain ring has no spare rows: writing ahead would tear live records, so it is refused
+    with pytest.raises(B.StratError):
+        B.Replay(32, 8).reserve(n, 1)
 
 
 def test_config3_full_size_ring_zero_copy_and_sample():
     """BASELINE.json configs[3] at full size in the launch sequence bench.py times: 262,144
-    games, 64 x 131,072-record ring (77.6 GB), zero-copy push + 4,096-sample gather per step.
-    The oracle mirrors three 32-game ranges; 34 steps wrap the ring (capacity = 32 blocks)."""
+    games, 64 x 131,072-record ring (77.6 GB + spare rows), in-place push + 4,096-sample gather
+    per step.  The oracle mirrors three 32-game ranges here; 34 steps wrap the ring (capacity =
+    32 blocks).  (All games, row by row, on a ring that wraps sooner: tests/test_gpu_allgames.py.)"""
     c = W.CONFIGS[3]
     n, bs = c["num_games"], c["sample_batch"]
     kw = dict(variant=0, seed=c["seed"], max_plies=c["max_plies"], auto_reset=1)
     free, _ = torch.cuda.mem_get_info()
-    if free < 90e9:
-        pytest.skip("needs ~80 GB of free device memory")
+    if free < 95e9:
+        pytest.skip("needs ~85 GB of free device memory")
     g = B.Env(n, **kw)
-    ring = B.Replay(c["ring_per_slot"], c["ring_slots"])
+    ring = B.Replay(c["ring_per_slot"], c["ring_slots"], block=n)
     cap = ring.capacity
     ranges = [0, 131072 + 64, n - 32]
     os_ = [orc.Env(32, game_base=lo, **kw) for lo in ranges]
@@ -568,16 +533,19 @@ def test_config3_full_size_ring_zero_copy_and_sample():
         head, filled = ring.state()
         assert head == ((t + 1) * n) % cap and filled == min((t + 1) * n, cap)
         idx = torch.from_numpy(orc.sample_indices(c["seed"], t, bs, filled)).cuda()
-        assert torch.equal(s_act, va[idx]) and torch.equal(s_rew, vr[idx]) and torch.equal(s_done, vd[idx])
-        assert torch.equal(s_mask, vm[idx])
-        assert torch.equal(s_obs.view(torch.int16).view(bs, -1), vo[idx])
-    for t in range(steps - cap // n, steps):  # the blocks still in the ring
-        p0 = (t * n) % cap
+        # ring position -> rows: blocks are contiguous, so locate() of each block start suffices
+        blk = torch.div(idx, n, rounding_mode="floor")
+        row0 = torch.tensor([ring.locate(k * n) if k * n < filled else (0, 0) for k in range(cap // n)], device="cuda")
+        row, orow = row0[blk, 0] + idx - blk * n, row0[blk, 1] + idx - blk * n
+        assert torch.equal(s_act, va[row]) and torch.equal(s_rew, vr[row]) and torch.equal(s_done, vd[row])
+        assert torch.equal(s_mask, vm[row])
+        assert torch.equal(s_obs.view(torch.int16).view(bs, -1), vo[orow])
+    for t in range(steps - cap // n, steps):  # the blocks still in the ring: every one is whole
+        row, orow = ring.locate((t * n) % cap)
         for lo in ranges:
             eo, em, ea, er, ed = expect[(t, lo)]
-            s = slice(p0 + lo, p0 + lo + 32)
-            if t > steps - cap // n:  # the oldest block's obs rows already hold obs of the next record
-                assert np.array_equal(_np(vo[s]).view(np.uint16), eo), (t, lo)
+            s, so = slice(row + lo, row + lo + 32), slice(orow + lo, orow + lo + 32)
+            assert np.array_equal(_np(vo[so]).view(np.uint16), eo), (t, lo)
             assert np.array_equal(_np(vm[s]).view(np.uint32), em), (t, lo)
             assert np.array_equal(_np(va[s]), ea) and np.array_equal(_np(vr[s]), er) and np.array_equal(_np(vd[s]), ed)
     b = _np(g.get_boards())

@@ -69,3 +69,23 @@ def test_shard_description():
     b = W.shard_for_rank(W.CONFIGS[2], 7, 8)
     assert a["game_base"] == 0 and b["game_base"] == 7 * 65536
     assert {k: v for k, v in a.items() if k != "game_base"} == {k: v for k, v in b.items() if k != "game_base"}
+
+
+def test_sharded_oracle_plumbing_equals_one_oracle():
+    """tests/oracle_shards.py (the all-games parity plumbing of the -m gpu tests): three worker
+    processes over a ragged split reproduce the single-process oracle output by output."""
+    from oracle import orc
+    from oracle_shards import ShardedOracle
+    n, kw = 150, dict(variant=0, seed=9, max_plies=30, auto_reset=1)
+    one = orc.Env(n, **kw)
+    with ShardedOracle(n, procs=3, with_obs_before=True, **kw) as sh:
+        assert len(sh._workers) == 3
+        for t in range(45):
+            ob = one.encode_obs().reshape(n, -1)
+            m = one.legal_mask(); a = one.sample_uniform(m); r, d = one.step(a)
+            sh.step(want_mask=True, want_obs_before=True, want_obs_after=True, want_boards=True)
+            assert np.array_equal(sh.act, a) and np.array_equal(sh.rew, r) and np.array_equal(sh.done, d), t
+            assert np.array_equal(sh.mask, m) and np.array_equal(sh.obs_before, ob), t
+            assert np.array_equal(sh.obs, one.encode_obs().reshape(n, -1)), t
+            assert np.array_equal(sh.boards, one.get_boards()), t
+        assert np.array_equal(sh.get_boards(), one.get_boards())
