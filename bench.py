@@ -603,7 +603,7 @@ def main():
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: skip the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: skip the oracle timing")
     ap.add_argument("--profile-range", type=int, default=0, metavar="K",
-                    help="profiling runs (ncu --replay-mode range --profile-from-start off): after the warm-up, "
+                    help="profiling runs (ncu --replay-mode range): after the warm-up, "
                          "K back-to-back fused steps between cudaProfilerStart/Stop, nothing else; prints no bench line")
     args = ap.parse_args()
     if args.profile_range:

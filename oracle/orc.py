@@ -12,6 +12,7 @@ LINE = 128
 MASK_WORDS = 113
 PLANES = 44
 OBS = PLANES * 100
+INFO_PLANES = 487
 
 OK, BAD_ARG, BAD_STATE, ILLEGAL_ACTION = 0, -1, -2, -4
 
@@ -28,6 +29,8 @@ class Config(C.Structure):
         ("device", C.c_int32),
         ("chase_rule", C.c_int32),
         ("game_base", C.c_uint64),
+        ("infostate", C.c_int32),
+        ("reserved", C.c_int32),
     ]
 
 
@@ -50,6 +53,9 @@ def lib():
         L.orc_sample_uniform.argtypes = [vp, vp, vp]
         L.orc_step.argtypes = [vp, vp, vp, vp]
         L.orc_encode_obs.argtypes = [vp, vp]
+        L.orc_encode_infostate.argtypes = [vp, vp]
+        L.orc_bf16_of_ratio.argtypes = [C.c_int64, C.c_int64]
+        L.orc_bf16_of_ratio.restype = C.c_uint16
         L.orc_check.argtypes = [vp]
         L.orc_clear_error.argtypes = [vp]
         L.orc_replay_create.argtypes = [C.c_int32, C.c_int32, C.POINTER(vp)]
@@ -90,9 +96,9 @@ def _chk(rc, what):
 
 class Env:
     def __init__(self, num_games, variant=0, seed=0, max_plies=0, max_battleless=0,
-                 auto_reset=0, two_square=1, game_base=0, chase_rule=0):
+                 auto_reset=0, two_square=1, game_base=0, chase_rule=0, infostate=0):
         self.cfg = Config(num_games, variant, seed, max_plies, max_battleless, auto_reset,
-                          two_square, 0, chase_rule, game_base)
+                          two_square, 0, chase_rule, game_base, infostate, 0)
         self.n = num_games
         self.h = C.c_void_p()
         _chk(lib().orc_create(C.byref(self.cfg), C.byref(self.h)), "create")
@@ -155,6 +161,12 @@ class Env:
     def encode_obs(self):
         o = np.zeros((self.n, PLANES, 10, 10), np.uint16)
         _chk(lib().orc_encode_obs(self.h, _p(o)), "encode_obs")
+        return o
+
+    def encode_infostate(self):
+        """The paper's 487-channel information state as bf16 bit patterns."""
+        o = np.zeros((self.n, INFO_PLANES, 10, 10), np.uint16)
+        _chk(lib().orc_encode_infostate(self.h, _p(o)), "encode_infostate")
         return o
 
     def check(self):
@@ -258,11 +270,15 @@ def reduce_returns(games: Env, root_side, samples_per_root: int):
 
 def find_setup_redraws(variant, seed, epoch, start, count, max_out=64):
     """Global game indices in [start, start+count) whose setup at `epoch` needs a redraw (R#5)."""
-    cfg = Config(1, variant, seed, 0, 0, 0, 1, 0, 0, 0)
+    cfg = Config(1, variant, seed, 0, 0, 0, 1, 0, 0, 0, 0, 0)
     out = np.zeros(max_out, np.uint32)
     n = lib().orc_find_setup_redraws(C.byref(cfg), epoch, start, count, _p(out), max_out)
     assert n >= 0
     return out[:n].tolist()
+
+
+def bf16_of_ratio(num, den):
+    return int(lib().orc_bf16_of_ratio(num, den))
 
 
 def philox(ctr, key):

@@ -39,6 +39,21 @@
 //                      the epoch; the reading itself (epoch keeps counting) is PARITY UNPINNED
 //                      against the paper (P:252-254 gives no detail).
 //
+//   information state S2 (P:482-610, 487 channels; readings I1-I9 in DESIGN.md):
+//                      pinned: hand-built mini-games for every channel group (threat, evasion,
+//                      declined attack, protection of a piece and of an empty square, each of
+//                      the six causes of death, captures by start square), channel sums fixed by
+//                      the piece counts, start-square and move channels against the played
+//                      moves, information-state property, channels 12-35 against the empirical
+//                      marginals of the (independent) determinisation sampler and by hand.
+//                      The READING of channels 12-35 ("assuming the setup and moves were
+//                      selected uniformly at random": taken as uniform over the
+//                      arrangements consistent with revealed / moved, the likelihood of the
+//                      observed moves ignored) and the mechanics the paper leaves open (what
+//                      counts as a threat / protection of an empty square, the square a piece
+//                      "died in", ten type channels per cause of death) are PARITY UNPINNED
+//                      against the paper's own simulator.
+//
 // Layouts:
 //   canonical line, 128 B per game:
 //     0..99   cell bytes: bits0-3 type (0 empty, 1 Spy,2 Scout,3 Miner,4 Sergeant,
@@ -70,6 +85,8 @@ constexpr int kLine = 128;
 constexpr int kMaskWords = 113;
 constexpr int kPlanes = 44;
 constexpr int kObs = kPlanes * kCells;  // 4400 bf16 per game
+constexpr int kInfoPlanes = 487;        // 455 board/history channels + 32 move channels
+constexpr int kInfo = kInfoPlanes * kCells;
 
 constexpr int T_EMPTY = 0, T_SPY = 1, T_SCOUT = 2, T_MINER = 3, T_MARSHAL = 10,
               T_FLAG = 11, T_BOMB = 12, T_LAKE = 15;
@@ -93,6 +110,34 @@ struct Config {  // mirrors the field order of the product's strat_config on pur
   int32_t device;  // unused here
   int32_t chase_rule;      // 1: apply the continuous-chasing rule (R#28)
   uint64_t game_base;  // global index of game 0 (RNG keying under sharding)
+  int32_t infostate;   // 1: keep the per-piece trackers of the paper's information state (S2)
+  int32_t reserved;
+};
+
+// ---- trackers of the paper's information state.  Everything a channel of S2 needs
+// beyond the board itself.  A piece is identified by the square it started the game on
+// (P:606 needs that anyway); its history bits travel with that identity.
+// Keys: a set over "the other piece at the time" = revealed type Spy..Marshal (bits 0-9),
+// revealed Bomb (bit 10, protection groups only), bit 11 = empty square (channel 262) / padding
+// (channels 275, 288, 301: never set), bit 12 = that piece was not revealed.  The three 11-wide
+// groups (threat, evasion, active adjacency) use bits 0-9 and bit 12.
+struct PieceTrack {
+  uint16_t threatened;       // P:519-520 "has ever threatened a piece of the opponent which ... was"
+  uint16_t evaded;           // P:526-527 "has ever evaded a threat from an opponent's piece which ... was"
+  uint16_t adjacent;         // P:533-534 "has ever been actively adjacent to an opponent's piece which ... was"
+  uint16_t protected_piece;  // P:576-578 "has ever protected a piece of the player which ... / an empty square"
+  uint16_t protected_against;
+  uint16_t was_protected_by;
+  uint16_t was_protected_against;
+};
+struct Track {
+  int id_at[kCells];             // start square of the piece standing on each square, -1 if none
+  PieceTrack piece[kCells];      // by start square
+  int start_type[kCells];        // what stood on each square when the game started (0 = nothing)
+  int start_owner[kCells];
+  bool captured[kCells];         // by start square
+  bool died[2][6][10][kCells];   // [owner][cause 1..6][type Spy..Marshal][square of the battle]
+  int moves[32][2];              // most recent first; [j][0] = -1 if there is no such move
 };
 
 struct Game {
@@ -129,6 +174,7 @@ struct SetupPool {
 struct Env {
   Config cfg;
   std::vector<Game> g;
+  std::vector<Track> track;  // one per game when cfg.infostate, else empty
   int error;
   SetupPool pool;
   // "Reset Behaviour and Support for Search": terminated boards restart from a
@@ -412,6 +458,124 @@ int battle(int att, int def) {
   return 0;
 }
 
+// ---------------------------------------------------------------- S2 trackers
+// Key of "the other piece at the time": its type if it was revealed, else "not revealed".
+// Returns the bit, or 0 when the case has no channel (a revealed Bomb in the 11-wide groups of
+// P:519-534, whose channels run Spy..Marshal + hidden; a revealed Flag anywhere).
+uint16_t key_of(uint8_t b, bool with_bomb) {
+  if (!(b & B_REVEALED)) return (uint16_t)(1u << 12);
+  int t = type_of(b);
+  if (t >= 1 && t <= 10) return (uint16_t)(1u << (t - 1));
+  if (t == T_BOMB && with_bomb) return (uint16_t)(1u << 10);
+  return 0;
+}
+
+// A fresh game, or a state loaded from a canonical line: the squares the pieces stand on now are
+// their start squares, nothing has happened to them yet, and the recent moves are what the
+// line's history remembers (reading I9).
+void track_init(const Game& gm, Track& tk) {
+  for (int c = 0; c < kCells; ++c) {
+    bool p = is_piece(gm.cell[c]);
+    tk.id_at[c] = p ? c : -1;
+    tk.piece[c] = PieceTrack{0, 0, 0, 0, 0, 0, 0};
+    tk.start_type[c] = p ? type_of(gm.cell[c]) : 0;
+    tk.start_owner[c] = p ? owner_of(gm.cell[c]) : 0;
+    tk.captured[c] = false;
+  }
+  memset(tk.died, 0, sizeof tk.died);
+  for (int j = 0; j < 32; ++j) {
+    bool have = j < 8 && gm.hist[j][0] != 0xFF;
+    tk.moves[j][0] = have ? gm.hist[j][0] : -1;
+    tk.moves[j][1] = have ? gm.hist[j][1] : -1;
+  }
+}
+
+// The trackers' share of one ply, judged on the position BEFORE the move (gm is not yet
+// changed).  `side` moves its piece from `from` to `to` (`dist` squares).
+void track_ply(const Game& gm, const Config& cfg, Track& tk, int side, int from, int to, int dist) {
+  const uint8_t C = gm.cell[from];
+  const int idC = tk.id_at[from];
+  // (i) Active adjacency: "the player controlling the former has had the chance to
+  // attack the latter, but opted not to": every one-square capture that was legal for the
+  // mover's side in this position and is not the move played (reading I3).
+  for (int p = 0; p < kCells; ++p) {
+    if (!is_piece(gm.cell[p]) || owner_of(gm.cell[p]) != side) continue;
+    for (int d = 0; d < 4; ++d) {
+      int rr = p / 10 + DROW[d], qq = p % 10 + DCOL[d];
+      if (rr < 0 || rr > 9 || qq < 0 || qq > 9) continue;
+      int q = rr * 10 + qq;
+      if (!is_piece(gm.cell[q]) || owner_of(gm.cell[q]) == side) continue;
+      if (p == from && q == to) continue;  // the attack that was made
+      if (!move_is_legal(gm, cfg, side, p, d, 1)) continue;
+      tk.piece[tk.id_at[p]].adjacent |= key_of(gm.cell[q], false);
+    }
+  }
+  // The previous ply, if it was a move to an empty square, may have been a threat by the piece A
+  // that now stands on x; battleless > 0 says that ply was not a battle.
+  bool prev = gm.hist[0][0] != 0xFF && gm.battleless > 0;
+  int x = prev ? gm.hist[0][1] : -1;
+  if (prev && (!is_piece(gm.cell[x]) || owner_of(gm.cell[x]) == side)) prev = false;  // hand-built lines only
+  const bool battle_ply = gm.cell[to] != 0;
+  if (!battle_ply) {  // threats, evasions and protections are moves to empty squares (readings I1, I2, I4)
+    const uint8_t Cafter = (uint8_t)(C | B_MOVED | (dist >= 2 ? B_REVEALED : 0));  // what C shows after this move (R#10)
+    if (prev) {
+      const uint8_t A = gm.cell[x];
+      // (ii) Evasion: "a piece that was threatened in the immediately preceding move is
+      // moved away from the threatening piece, to an empty square".
+      if (adjacent(from, x) && !adjacent(to, x)) tk.piece[idC].evaded |= key_of(A, false);
+      // (iii) Protection: A threatened B; C moves "to become adjacent to B".
+      for (int b = 0; b < kCells; ++b) {
+        if (b == from || !is_piece(gm.cell[b]) || owner_of(gm.cell[b]) != side) continue;
+        if (!adjacent(b, x) || !adjacent(b, to) || adjacent(b, from)) continue;
+        tk.piece[idC].protected_piece |= key_of(gm.cell[b], true);
+        tk.piece[idC].protected_against |= key_of(A, true);
+        tk.piece[tk.id_at[b]].was_protected_by |= key_of(Cafter, true);
+        tk.piece[tk.id_at[b]].was_protected_against |= key_of(A, true);
+      }
+      // "We extend the same terminology to the case in which B is an empty square":
+      // a square that was empty when A moved next to it, still is, and is next to C's new square
+      // (reading I4; the square C leaves was not empty when A came, so it does not count).
+      for (int e = 0; e < kCells; ++e) {
+        if (e == to || gm.cell[e] != 0) continue;  // occupied squares and lakes
+        if (!adjacent(e, x) || !adjacent(e, to)) continue;
+        tk.piece[idC].protected_piece |= (uint16_t)(1u << 11);
+        tk.piece[idC].protected_against |= key_of(A, true);
+      }
+    }
+    // (iv) Threat: "a movement of one's piece so as to make the piece adjacent to a piece of
+    // the opponent.  The opponent's piece is considered threatened."
+    for (int d = 0; d < 4; ++d) {
+      int rr = to / 10 + DROW[d], qq = to % 10 + DCOL[d];
+      if (rr < 0 || rr > 9 || qq < 0 || qq > 9) continue;
+      int q = rr * 10 + qq;
+      if (q == from || !is_piece(gm.cell[q]) || owner_of(gm.cell[q]) == side) continue;
+      tk.piece[idC].threatened |= key_of(gm.cell[q], false);
+    }
+    tk.id_at[to] = idC; tk.id_at[from] = -1;
+  } else {
+    // (v) Captures and causes of death.  "revealed at the time of the attack" = before
+    // this battle reveals both.  The square a piece died in = the square of the battle (reading I5).
+    const uint8_t D = gm.cell[to];
+    const int idD = tk.id_at[to];
+    const bool d_rev = (D & B_REVEALED) != 0;
+    const int tc = type_of(C), td = type_of(D), out = battle(tc, td);
+    if (out >= 0 && td != T_FLAG) {  // the defender dies (the Flag's capture ends the game: no channel)
+      tk.captured[idD] = true;
+      int cause = d_rev ? (out > 0 ? 4 : 5) : 6;
+      if (td >= 1 && td <= 10) tk.died[side ^ 1][cause - 1][td - 1][to] = true;  // ten type channels per cause (reading I6)
+    }
+    if (out <= 0) {  // the attacker dies
+      tk.captured[idC] = true;
+      int cause = d_rev ? (out < 0 ? 1 : 2) : 3;
+      tk.died[side][cause - 1][tc - 1][to] = true;
+    }
+    tk.id_at[from] = -1;
+    if (out > 0) tk.id_at[to] = idC; else if (out == 0) tk.id_at[to] = -1;
+  }
+  for (int j = 31; j >= 1; --j) { tk.moves[j][0] = tk.moves[j - 1][0]; tk.moves[j][1] = tk.moves[j - 1][1]; }
+  tk.moves[0][0] = from; tk.moves[0][1] = to;
+}
+
 int effective_ply_cap(const Config& cfg) {
   return (cfg.max_plies >= 1 && cfg.max_plies <= 65535) ? cfg.max_plies : 65535;
 }
@@ -439,6 +603,7 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
     return;
   }
   int to = (from / 10 + DROW[dir] * dist) * 10 + (from % 10 + DCOL[dir] * dist);
+  if (cfg.infostate) track_ply(gm, cfg, e->track[gi], side, from, to, dist);  // S2 trackers, on the position before the move
   // 0. chase state machine (R#28), judged on the position before the move.
   if (cfg.chase_rule) {
     bool fight = gm.cell[to] != 0;
@@ -515,6 +680,7 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
       gm.epoch = epoch;
       new_game(cfg, (uint32_t)(cfg.game_base + (uint64_t)gi), gm, &e->pool);
     }
+    if (cfg.infostate) track_init(gm, e->track[gi]);
   }
 }
 
@@ -605,6 +771,115 @@ void encode_game(const Game& gm, uint16_t* obs) {
   }
 }
 
+// ---------------------------------------------------------------- S2 information state
+// Round-to-nearest-even bf16 of the IEEE double quotient num/den (reading I8: the real-valued
+// channels are that quotient, rounded once).
+uint16_t bf16_of_ratio(long long num, long long den) {
+  if (num == 0 || den == 0) return 0;
+  double x = (double)num / (double)den;
+  uint16_t sign = 0;
+  if (x < 0) { sign = 0x8000; x = -x; }
+  int e = 0;
+  double m = frexp(x, &e);            // x = m * 2^e, m in [0.5, 1)
+  double q = nearbyint(m * 256.0);    // 8 significant bits, ties to even (default rounding mode)
+  if (q >= 256.0) { q = 128.0; e += 1; }
+  int biased = e - 1 + 127;           // value = (q / 128) * 2^(e-1)
+  return (uint16_t)(sign | (biased << 7) | ((int)q - 128));
+}
+
+// Channels 12-23 / 24-35: "probability that it belongs to the opponent and has type
+// T ..., assuming the setup and moves were selected uniformly at random".  Reading I7: uniform
+// over the arrangements of the owner's still-hidden pieces on their squares that are consistent
+// with what the viewer has seen - revealed pieces are known, a piece that has moved is neither
+// Bomb nor Flag.  With u unmoved and m moved hidden squares, c_T hidden pieces of type T,
+// I = c_Flag + c_Bomb and M = u + m - I movable ones:
+//   unmoved square:  P(T) = c_T / u  for T in {Flag, Bomb},  (u - I) c_T / (u M)  otherwise;
+//   moved square:    P(T) = 0        for T in {Flag, Bomb},  c_T / M              otherwise.
+// `owner` = whose pieces are being guessed; planes = 12 channels (Spy..Marshal, Flag, Bomb).
+void type_posterior(const Game& gm, int owner, uint16_t* planes) {
+  int c[13] = {0}, u = 0, m = 0;
+  for (int s = 0; s < kCells; ++s) {
+    uint8_t b = gm.cell[s];
+    if (!is_piece(b) || owner_of(b) != owner || (b & B_REVEALED)) continue;
+    c[type_of(b)] += 1;
+    if (b & B_MOVED) ++m; else ++u;
+  }
+  int I = c[T_FLAG] + c[T_BOMB], M = u + m - I;
+  int free_unmoved = u - I > 0 ? u - I : 0;  // a hand-built line may mark a Bomb as moved
+  for (int s = 0; s < kCells; ++s) {
+    uint8_t b = gm.cell[s];
+    if (!is_piece(b) || owner_of(b) != owner) continue;
+    if (b & B_REVEALED) { planes[(type_of(b) - 1) * kCells + s] = 0x3F80; continue; }
+    for (int t = 1; t <= 12; ++t) {
+      bool immovable = t == T_FLAG || t == T_BOMB;
+      uint16_t v;
+      if (b & B_MOVED) v = immovable ? 0 : bf16_of_ratio(c[t], M);
+      else v = immovable ? bf16_of_ratio(c[t], u) : bf16_of_ratio((long long)free_unmoved * c[t], (long long)u * M);
+      planes[(t - 1) * kCells + s] = v;
+    }
+  }
+}
+
+void encode_infostate(const Game& gm, const Config& cfg, const Track& tk, uint16_t* out) {
+  const uint16_t ONE = 0x3F80, MINUS_ONE = 0xBF80;
+  for (int i = 0; i < kInfo; ++i) out[i] = 0;
+  const int p = gm.ply & 1;  // "the player" = the acting player
+  auto set = [&](int channel, int square) { out[channel * kCells + square] = ONE; };
+  // ---- basic piece properties
+  for (int s = 0; s < kCells; ++s) {
+    uint8_t b = gm.cell[s];
+    if (type_of(b) == T_LAKE) continue;
+    if (b == 0) { set(38, s); continue; }                      // empty (lakes are not squares: R#17)
+    bool mine = owner_of(b) == p;
+    if (mine) set(type_of(b) - 1, s);                          // 0-11
+    if (!(b & B_REVEALED)) set(mine ? 36 : 37, s);             // hidden pieces
+    if (b & B_MOVED) set(mine ? 39 : 40, s);                   // pieces that moved
+  }
+  type_posterior(gm, p ^ 1, out + 12 * kCells);                // 12-23: the opponent's pieces, as the player sees them
+  type_posterior(gm, p, out + 24 * kCells);                    // 24-35: the player's pieces, as the opponent sees them
+  uint16_t f41 = bf16_of_ratio(gm.ply, effective_ply_cap(cfg));
+  uint16_t f42 = cfg.max_battleless > 0 ? bf16_of_ratio(gm.battleless, cfg.max_battleless) : 0;
+  for (int s = 0; s < kCells; ++s) { out[41 * kCells + s] = f41; out[42 * kCells + s] = f42; }
+  // ---- per-piece history, for the player's pieces then for the opponent's
+  for (int s = 0; s < kCells; ++s) {
+    if (!is_piece(gm.cell[s])) continue;
+    const PieceTrack& t = tk.piece[tk.id_at[s]];
+    bool mine = owner_of(gm.cell[s]) == p;
+    int a = mine ? 43 : 76;     // threat / evasion / active adjacency: 10 types + hidden each
+    const uint16_t g11[3] = {t.threatened, t.evaded, t.adjacent};
+    for (int k = 0; k < 3; ++k) {
+      for (int j = 0; j < 10; ++j)
+        if (g11[k] & (1u << j)) set(a + 11 * k + j, s);
+      if (g11[k] & (1u << 12)) set(a + 11 * k + 10, s);
+    }
+    int b = mine ? 251 : 303;   // protections: 13 channels each (11 types, empty square / padding, not revealed)
+    const uint16_t g13[4] = {t.protected_piece, t.protected_against, t.was_protected_by, t.was_protected_against};
+    for (int k = 0; k < 4; ++k)
+      for (int j = 0; j < 13; ++j)
+        if (g13[k] & (1u << j)) set(b + 13 * k + j, s);
+    set(355 + tk.id_at[s], s);  // the piece on s started from square id
+  }
+  // ---- captured pieces by start square: Spy..Marshal, Bomb
+  for (int s = 0; s < kCells; ++s) {
+    if (!tk.captured[s]) continue;
+    int t = tk.start_type[s];
+    int j = t >= 1 && t <= 10 ? t - 1 : t == T_BOMB ? 10 : -1;
+    if (j >= 0) set((tk.start_owner[s] == p ? 109 : 120) + j, s);
+  }
+  // ---- causes of death
+  for (int o = 0; o < 2; ++o)
+    for (int c = 0; c < 6; ++c)
+      for (int t = 0; t < 10; ++t)
+        for (int s = 0; s < kCells; ++s)
+          if (tk.died[o][c][t][s]) set((o == p ? 131 : 191) + 10 * c + t, s);
+  // ---- the most recent 32 moves: +1 on the destination, -1 on the source
+  for (int j = 0; j < 32; ++j) {
+    if (tk.moves[j][0] < 0) continue;
+    out[(455 + j) * kCells + tk.moves[j][1]] = ONE;
+    out[(455 + j) * kCells + tk.moves[j][0]] = MINUS_ONE;
+  }
+}
+
 // ---------------------------------------------------------------- C6 replay ring
 struct Replay {
   int64_t per_slot, slots, capacity, head, filled;
@@ -627,9 +902,11 @@ int orc_create(const Config* cfg, Env** out) {
   e->cfg = *cfg;
   e->g.resize((size_t)cfg->num_games);
   e->error = 0;
+  if (cfg->infostate) e->track.resize((size_t)cfg->num_games);
   for (int i = 0; i < cfg->num_games; ++i) {
     e->g[i].epoch = 0;
     new_game(e->cfg, (uint32_t)(cfg->game_base + (uint64_t)i), e->g[i]);
+    if (cfg->infostate) track_init(e->g[i], e->track[i]);
   }
   *out = e;
   return ORC_OK;
@@ -644,6 +921,7 @@ int orc_reset(Env* e, uint64_t seed) {
   for (int i = 0; i < e->cfg.num_games; ++i) {
     e->g[i].epoch = 0;
     new_game(e->cfg, (uint32_t)(e->cfg.game_base + (uint64_t)i), e->g[i], &e->pool);
+    if (e->cfg.infostate) track_init(e->g[i], e->track[i]);
   }
   return ORC_OK;
 }
@@ -674,7 +952,10 @@ int orc_set_setup_pool(Env* e, const uint8_t* pool, int32_t K) {
 
 int orc_reset_from(Env* e, const uint8_t* boards) {
   if (!e || !boards) return ORC_BAD_ARG;
-  for (int i = 0; i < e->cfg.num_games; ++i) read_line(boards + (size_t)i * kLine, e->g[i]);
+  for (int i = 0; i < e->cfg.num_games; ++i) {
+    read_line(boards + (size_t)i * kLine, e->g[i]);
+    if (e->cfg.infostate) track_init(e->g[i], e->track[i]);  // reading I9: the loaded position is where the trackers start
+  }
   return ORC_OK;
 }
 
@@ -738,6 +1019,15 @@ int orc_encode_obs(const Env* e, uint16_t* obs) {
   for (int i = 0; i < e->cfg.num_games; ++i) encode_game(e->g[i], obs + (size_t)i * kObs);
   return ORC_OK;
 }
+
+// ComputeInfostateTensor in the paper's own form (P:462, S2 P:482-610): bf16 [N][487][10][10].
+int orc_encode_infostate(const Env* e, uint16_t* out) {
+  if (!e || !out) return ORC_BAD_ARG;
+  if (!e->cfg.infostate) return ORC_BAD_STATE;
+  for (int i = 0; i < e->cfg.num_games; ++i) encode_infostate(e->g[i], e->cfg, e->track[i], out + (size_t)i * kInfo);
+  return ORC_OK;
+}
+uint16_t orc_bf16_of_ratio(int64_t num, int64_t den) { return bf16_of_ratio(num, den); }
 
 int orc_check(Env* e) {
   if (!e) return ORC_BAD_ARG;

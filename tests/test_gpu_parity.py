@@ -315,10 +315,13 @@ def test_pinned_reset_state_matches_oracle():
 def test_fused_steps_of_two_environments_chained_through_a_buffer():
     """Environment B replays, with strat_step_observe, the actions environment A's fused step has
     just written - 300 times with no host sync.  The two launches belong to different environments
-    (no version flags relate them), so B must wait for A's grid: stream order has to hold."""
+    (no version flags relate them) and exchange a buffer, so they share one chain record
+    (strat_share_chain): B waits for A's grid, and A's next step waits for B's (which is still
+    reading the actions A is about to overwrite): stream order has to hold."""
     kw = dict(variant=0, seed=31, max_plies=120, auto_reset=1)
     n = 65536
     a, b = B.Env(n, **kw), B.Env(n, **kw)
+    a.share_chain(b)
     mask_a, act, rew_a, done_a, obs_a = a.new_mask(), a.new_actions(), a.new_reward(), a.new_done(), a.new_obs()
     mask_b, rew_b, done_b, obs_b = b.new_mask(), b.new_reward(), b.new_done(), b.new_obs()
     for _ in range(300):
