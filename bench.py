@@ -537,6 +537,53 @@ def run_search(args):
     print(json.dumps(line))
 
 
+def run_infostate(args):
+    """The paper's own information state on the headline shape (PAPER.md:462, S2 482-610): 65,536
+    classic games; every step = one fused step that also keeps the S2 trackers up to date, then
+    ComputeInfostateTensor in the 487-channel bf16 form (97,400 bytes per game) for every game."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    n = CFG["num_games"]
+    env = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], max_battleless=200, auto_reset=1, infostate=1)
+    mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
+    info = env.new_infostate()
+    steps = max(1, min(args.steps, 200))
+    for _ in range(max(args.warmup, 3)):
+        env.rollout_step(mask, act, rew, done, obs)
+        env.encode_infostate(info)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    for k in range(steps):
+        ev[k][0].record()
+        env.rollout_step(mask, act, rew, done, obs)
+        ev[k][1].record()
+        env.encode_infostate(info)
+        ev[k][2].record()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    assert env.check() == 0
+    ms_step = sum(e[0].elapsed_time(e[1]) for e in ev) / steps
+    ms_enc = sum(e[1].elapsed_time(e[2]) for e in ev) / steps
+    total = ev[0][0].elapsed_time(ev[-1][2]) / steps
+    per_game = 487 * 100 * 2 + 2048 + 128  # the tensor out, the tracker block and the line in
+    line = {
+        "metric": "stratego_infostates_per_sec", "value": n / (total / 1e3), "unit": "information states/s", "n_gpus": 1,
+        "steps": steps, "warmup": max(args.warmup, 3), "ms_per_step": total, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u8 (game), bf16 (tensor; real-valued channels rounded once from f64)", "data": "synthetic",
+        "config": {"workload": CFG["name"] + " + 487-channel information state", "games_per_gpu": n,
+                   "ms_tracked_fused_step": ms_step, "ms_encode_infostate": ms_enc,
+                   "tensor_bytes_per_game": 487 * 100 * 2, "tracker_bytes_per_game": 2048,
+                   "l2": "output 6.38 GB per step > 126 MB L2 (no flush needed)"},
+        "roofline": dict(_peak_line(per_game * n / (ms_enc / 1e3) / 1e9), kernel="k_encode_infostate",
+                         algorithmic_bytes_per_game=per_game),
+        "gpu_launches": 2 * steps, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
 def run_hist(args):
     """The paper's own buffer design on the headline workload: the fused step
     records the 128-byte state of every game and step into a 256-step board-history ring
@@ -593,10 +640,11 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search"],
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search", "infostate487"],
                     help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
                          "hist = cfg2 recording into the board-history ring + historical queries; "
-                         "search = network-free search steps (S3.7) for 256 roots; all 1 GPU")
+                         "search = network-free search steps (S3.7) for 256 roots; infostate487 = cfg2 with the S2 trackers kept and the "
+                         "paper's 487-channel information state encoded every step; all 1 GPU")
     ap.add_argument("--chase-rule", action="store_true",
                     help="cfg2 with the continuous-chasing rule on (not a BASELINE.json config; the paper's simulator goal "
                          "of ~10 M updates/s is stated with its anti-chasing rules on, PAPER.md:228)")
@@ -618,6 +666,8 @@ def main():
         run_hist(args)
     elif args.workload == "search":
         run_search(args)
+    elif args.workload == "infostate487":
+        run_infostate(args)
     else:
         run_b200(args)
 

@@ -73,6 +73,8 @@ extern "C" {
 #define STRAT_OBS_PLANES 44
 #define STRAT_OBS_ELEMS 4400
 #define STRAT_NUM_ACTIONS 3600
+#define STRAT_INFO_PLANES 487   /* the paper's own information state */
+#define STRAT_INFO_ELEMS 48700
 
 typedef struct strat_config {
   int32_t num_games;      /* N >= 1 */
@@ -89,6 +91,12 @@ typedef struct strat_config {
                              this environment + the 8 plies a loaded line carries), 0: off */
   uint64_t game_base;     /* global index of game 0 (RNG keying when games are sharded);
                              game_base + num_games <= 2^32 (the RNG counter word is 32 bits) */
+  int32_t infostate;      /* 1: keep, per game, the trackers the paper's 487-channel information state
+                             needs (threats, evasions, active adjacencies, protections,
+                             captures, causes of death, start squares, the last 32 moves): 2 KB more
+                             workspace per game, updated by strat_step / strat_rollout_step /
+                             strat_step_observe; strat_encode_infostate then works.  0: off */
+  int32_t reserved;       /* 0 */
 } strat_config;
 
 typedef struct strat_env strat_env;       /* host handle; state lives in the workspace */
@@ -160,6 +168,34 @@ int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* 
 /* ComputeInfostateTensor in BASELINE.json's 44-plane bf16 form.
  * obs: uint16[N][4400]. */
 int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream);
+
+/* ComputeInfostateTensor in the paper's own form (S2): bf16 (as
+ * uint16) [N][487][10][10] for the acting player ("the player"; the other one is "the opponent"),
+ * absolute board coordinates.  Needs strat_config.infostate = 1 (else STRAT_BAD_STATE).  `out`
+ * must be 8-byte aligned.  Channels (values 0 / 1.0 unless stated; T runs Spy..Marshal, Flag, Bomb
+ * as far as the count says; readings I1-I9 in DESIGN.md):
+ *     0-11   the player's piece of type T               12-23  probability that the square holds an
+ *    24-35   the same from the opponent's side                  opponent's piece of type T: 1.0 for a
+ *    36/37   hidden piece of the player / the opponent          revealed one, else uniform over the
+ *    38      empty (not a lake)                                 arrangements of the hidden types on the
+ *    39/40   player's / opponent's piece that has moved         hidden squares with no Bomb or Flag on a
+ *    41      ply / ply cap       42  plies since the last       piece that has moved (bf16, rounded once
+ *            battle / max_battleless (0 if that rule is off)    from the double quotient)
+ *    43-52, 53   the player's piece has threatened a revealed T (Spy..Marshal) / a hidden piece
+ *    54-63, 64   ... has evaded a threat from ...        65-74, 75  ... was actively adjacent to ...
+ *    76-108      the same three groups for the opponent's pieces
+ *   109-119  start square of a captured piece of the player, T = Spy..Marshal, Bomb;  120-130 opponent's
+ *   131-190  a piece of the player of type T (Spy..Marshal) died on this square by cause 1..6:
+ *            131 + 10*(cause-1) + T-1;  191-250 the opponent's
+ *   251-263  the player's piece has protected a revealed T (Spy..Marshal, Bomb) / an empty square / a
+ *            hidden piece;  264-276 has protected against (.., 275 padding, 276 hidden);  277-289 has
+ *            been protected by;  290-302 has been protected against;  303-354 the opponent's
+ *   355-454  channel 355+k: the piece on this square started the game on square k
+ *   455-486  move t-1-j (j = 0..31): +1.0 on its destination, -1.0 on its source
+ * The trackers start with the game (reset, auto-reset) or with a loaded position
+ * (strat_reset_from, a pinned restart, strat_history_restore: the squares the pieces stand on
+ * then count as their start squares, the line's 8-ply history as the known moves). */
+int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream);
 
 /* One fused pass of the hot path: legal mask -> uniform legal action -> step -> encode of
  * the new state.  Produces exactly what strat_legal_mask, strat_sample_uniform,

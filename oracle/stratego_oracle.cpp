@@ -1191,6 +1191,7 @@ int orc_determinise(const Env* roots, int32_t samples_per_root, uint64_t seed, E
       int rc = determinise_one(roots->g[r], seed, (uint32_t)(out->cfg.game_base + (uint64_t)G), out->g[G], &d);
       if (rc != ORC_OK) return rc;
       if (attempts) attempts[G] = d;
+      if (out->cfg.infostate) track_init(out->g[G], out->track[G]);  // reading I9: the trackers start with the copy
     }
   return ORC_OK;
 }
@@ -1234,7 +1235,7 @@ static int legal_list(const Env* e, const Game& gm, int* list) {
 int orc_search_expand(const Env* roots, int32_t rollouts, uint64_t seed, Env* out) {
   if (!roots || !out || rollouts <= 0) return ORC_BAD_ARG;
   int R = roots->cfg.num_games;
-  if ((int64_t)R * rollouts != out->cfg.num_games || out->cfg.auto_reset) return ORC_BAD_ARG;
+  if ((int64_t)R * rollouts != out->cfg.num_games || out->cfg.auto_reset || out->cfg.infostate) return ORC_BAD_ARG;
   std::vector<int> list(3600);
   for (int r = 0; r < R; ++r) {
     const Game& root = roots->g[r];

@@ -13,12 +13,13 @@ from .build import ensure_built
 LINE = 128
 MASK_WORDS = 113
 OBS_ELEMS = 4400
+INFO_PLANES = 487
 OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
     "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_set_setup_pool", "strat_legal_mask", "strat_sample_uniform", "strat_step",
-    "strat_encode_obs", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
+    "strat_encode_obs", "strat_encode_infostate", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_bytes_in_place", "strat_replay_create_in_place",
     "strat_replay_locate", "strat_share_chain", "strat_replay_push", "strat_replay_reserve",
@@ -37,7 +38,7 @@ class strat_config(C.Structure):
         ("num_games", C.c_int32), ("variant", C.c_int32), ("seed", C.c_uint64),
         ("max_plies", C.c_int32), ("max_battleless", C.c_int32), ("auto_reset", C.c_int32),
         ("two_square", C.c_int32), ("device", C.c_int32), ("chase_rule", C.c_int32),
-        ("game_base", C.c_uint64),
+        ("game_base", C.c_uint64), ("infostate", C.c_int32), ("reserved", C.c_int32),
     ]
 
 
@@ -65,6 +66,7 @@ def lib():
         L.strat_sample_uniform.argtypes = [vp, vp, vp, vp]
         L.strat_step.argtypes = [vp, vp, vp, vp, vp]
         L.strat_encode_obs.argtypes = [vp, vp, vp]
+        L.strat_encode_infostate.argtypes = [vp, vp, vp]
         L.strat_rollout_step.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_step_observe.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_host_scratch_bytes.restype = sz
@@ -143,10 +145,10 @@ class Env:
     """N parallel games bound to a caller-owned (torch) workspace."""
 
     def __init__(self, num_games, variant=0, seed=0, max_plies=0, max_battleless=0, auto_reset=0,
-                 two_square=1, device=0, game_base=0, chase_rule=0):
+                 two_square=1, device=0, game_base=0, chase_rule=0, infostate=0):
         _require_cuda()
         self.cfg = strat_config(num_games, variant, seed, max_plies, max_battleless, auto_reset,
-                                two_square, device, chase_rule, game_base)
+                                two_square, device, chase_rule, game_base, infostate, 0)
         self.n = num_games
         self.device = torch.device("cuda", device)
         nbytes = lib().strat_workspace_bytes(C.byref(self.cfg))
@@ -235,6 +237,15 @@ class Env:
     def encode_obs(self, out=None):
         out = out if out is not None else self.new_obs()
         _chk(lib().strat_encode_obs(self.h, _ptr(out, torch.bfloat16), _stream()), "strat_encode_obs")
+        return out
+
+    def new_infostate(self):
+        return torch.empty((self.n, INFO_PLANES, 10, 10), dtype=torch.bfloat16, device=self.device)
+
+    def encode_infostate(self, out=None):
+        """The paper's 487-channel information state (needs infostate=1)."""
+        out = out if out is not None else self.new_infostate()
+        _chk(lib().strat_encode_infostate(self.h, _ptr(out, torch.bfloat16), _stream()), "strat_encode_infostate")
         return out
 
     def rollout_step(self, mask, actions, reward, done, obs):

@@ -35,7 +35,8 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool cfg_ok(const strat_config* c) {
   return c && c->num_games >= 1 && (c->variant == 0 || c->variant == 1) && c->max_plies >= 0 &&
          c->max_battleless >= 0 && (c->chase_rule == 0 || c->chase_rule == 1) &&
-         c->game_base + (uint64_t)c->num_games <= (1ull << 32);  // RNG counters carry a 32-bit global game index
+         c->game_base + (uint64_t)c->num_games <= (1ull << 32) &&  // RNG counters carry a 32-bit global game index
+         (c->infostate == 0 || c->infostate == 1) && c->reserved == 0;
 }
 inline Params make_params(const strat_config& c) {
   Params P;
@@ -48,6 +49,7 @@ inline Params make_params(const strat_config& c) {
   P.movelog = nullptr;
   P.pool = nullptr; P.pool_size = 0;
   P.pin = nullptr;
+  P.track = nullptr;
   return P;
 }
 inline int launch_status() { return cudaGetLastError() == cudaSuccess ? STRAT_OK : STRAT_CUDA_ERROR; }
@@ -162,6 +164,9 @@ inline void chain_break(const strat_env* env) {
   env->chain->last = nullptr; env->chain->stream = nullptr;
 }
 
+// (Re)start the S2 trackers of every game from its current line (no-op without infostate).
+inline void track_restart(const strat_env* env, cudaStream_t s);
+
 template <bool kExternal>
 int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done, uint16_t* obs,
                  void* stream) {
@@ -188,7 +193,8 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
     wait_prior = kExternal || !(rec.last == env && rec.stream == stream);
     rec.last = env; rec.stream = stream;
   }
-  auto kernel = env->P.chase_rule ? k_rollout_step<kExternal, true> : k_rollout_step<kExternal, false>;
+  auto kernel = env->P.track ? (env->P.chase_rule ? k_rollout_step<kExternal, true, true> : k_rollout_step<kExternal, false, true>)
+                             : (env->P.chase_rule ? k_rollout_step<kExternal, true, false> : k_rollout_step<kExternal, false, false>);
   if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
                          env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
                          hist_slot(env->hist), env->err, wait_prior) != cudaSuccess)
@@ -196,6 +202,9 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   env->version = version;
   if (env->hist) env->hist->cur += 1;
   return STRAT_OK;
+}
+inline void track_restart(const strat_env* env, cudaStream_t s) {
+  if (env->P.track) k_track_start<<<(env->P.num_games + 3) / 4, 128, 0, s>>>(env->P, env->lines);
 }
 }  // namespace
 
@@ -215,7 +224,8 @@ const char* strat_error_string(int code) {
 size_t strat_workspace_bytes(const strat_config* cfg) {
   if (!cfg_ok(cfg)) return 0;
   return align_up((size_t)cfg->num_games * STRAT_LINE_BYTES, 256) + 256 + align_up(sync_words(cfg->num_games) * 4, 256) +
-         (cfg->chase_rule ? (size_t)cfg->num_games * kLogPlies * 2 : 0);  // move logs: the chasing rule's memory
+         (cfg->chase_rule ? align_up((size_t)cfg->num_games * kLogPlies * 2, 256) : 0) +  // move logs: the chasing rule's memory
+         (cfg->infostate ? (size_t)cfg->num_games * kTrackWords * 4 : 0);                 // S2 trackers
 }
 
 int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, void* stream, strat_env** out) {
@@ -236,8 +246,12 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->f_obs = e->f_state + batches(cfg->num_games);
   e->version = 0;
   e->hist = nullptr;
-  if (cfg->chase_rule)
-    e->P.movelog = reinterpret_cast<uint16_t*>(reinterpret_cast<uint8_t*>(e->tickets) + align_up(sync_words(cfg->num_games) * 4, 256));
+  uint8_t* extra = reinterpret_cast<uint8_t*>(e->tickets) + align_up(sync_words(cfg->num_games) * 4, 256);
+  if (cfg->chase_rule) {
+    e->P.movelog = reinterpret_cast<uint16_t*>(extra);
+    extra += align_up((size_t)cfg->num_games * kLogPlies * 2, 256);
+  }
+  if (cfg->infostate) e->P.track = reinterpret_cast<uint32_t*>(extra);
   if (cudaMemsetAsync(e->tickets, 0, sync_words(cfg->num_games) * 4, (cudaStream_t)stream) != cudaSuccess) {
     delete e;
     return STRAT_CUDA_ERROR;
@@ -269,14 +283,17 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   env->cfg.seed = seed;
   const uint32_t* pin = env->P.pin;
   uint16_t* movelog = env->P.movelog;
+  uint32_t* track = env->P.track;
   const uint8_t* pool = env->P.pool;
   int32_t pool_size = env->P.pool_size;
   env->P = make_params(env->cfg);
   env->P.pin = pin;
   env->P.movelog = movelog;
+  env->P.track = track;
   env->P.pool = pool; env->P.pool_size = pool_size;
   k_set_int<<<1, 1, 0, s>>>(env->err, 0);
   k_reset<<<batches(env->P.num_games), 32, 0, s>>>(env->P, env->lines);
+  track_restart(env, s);
   return launch_status();
 }
 
@@ -285,6 +302,7 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   chain_break(env);
   int n = env->P.num_games;
   k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  track_restart(env, (cudaStream_t)stream);
   return launch_status();
 }
 
@@ -335,12 +353,10 @@ int strat_sample_uniform(const strat_env* env, const uint32_t* mask, int16_t* ac
 int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* done, void* stream) {
   if (!env || !actions || !reward || !done) return STRAT_BAD_ARG;
   chain_break(env);
-  if (env->P.chase_rule)
-    k_step<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done,
-                                                                             env->err, hist_slot(env->hist));
-  else
-    k_step<false><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done,
-                                                                              env->err, hist_slot(env->hist));
+  auto kernel = env->P.track ? (env->P.chase_rule ? k_step<true, true> : k_step<false, true>)
+                             : (env->P.chase_rule ? k_step<true, false> : k_step<false, false>);
+  kernel<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err,
+                                                                     hist_slot(env->hist));
   if (env->hist) env->hist->cur += 1;
   return launch_status();
 }
@@ -349,6 +365,19 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;
   chain_break(env);
   k_encode_obs<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, obs);
+  return launch_status();
+}
+
+int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
+  if (!env || !out || ((uintptr_t)out & 7) != 0) return STRAT_BAD_ARG;
+  if (!env->P.track) return STRAT_BAD_STATE;
+  chain_break(env);
+  static const int smem = kInfoWarps * kInfoWarpWords * 4;
+  if (cudaFuncSetAttribute(k_encode_infostate, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+    return STRAT_CUDA_ERROR;
+  int ctas = (env->P.num_games + kInfoWarps - 1) / kInfoWarps;
+  if (ctas > 2 * env->num_sms) ctas = 2 * env->num_sms;
+  k_encode_infostate<<<ctas, 32 * kInfoWarps, smem, (cudaStream_t)stream>>>(env->P, env->lines, out);
   return launch_status();
 }
 
@@ -420,7 +449,7 @@ int strat_step_host(strat_env* env, void* scratch_dev, const int16_t* actions_ho
 int strat_rollout_uniform(strat_env* env, int32_t plies, void* stream) {
   if (!env || plies < 0) return STRAT_BAD_ARG;
   chain_break(env);
-  if (env->hist) return STRAT_BAD_STATE;  // on-chip plies are not recorded
+  if (env->hist || env->P.track) return STRAT_BAD_STATE;  // on-chip plies are neither recorded nor tracked
   if (env->P.chase_rule)
     k_rollout_uniform<true><<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, plies, env->err);
   else
@@ -721,6 +750,7 @@ int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, voi
   if (L != env->lines) {
     copy_elems<uint32_t>(L, env->lines, (size_t)h->num_games * kLineWords, (cudaStream_t)stream);
     k_clear_logn<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, env->lines);
+    track_restart(env, (cudaStream_t)stream);
   }
   return launch_status();
 }
@@ -735,12 +765,13 @@ int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t
   k_determinise<<<batches(out->P.num_games), 32, 0, (cudaStream_t)stream>>>(
       out->P.num_games, samples_per_root, (uint32_t)seed, (uint32_t)(seed >> 32), out->P.game_base, roots->lines,
       out->lines, out->err);
+  track_restart(out, (cudaStream_t)stream);
   return launch_status();
 }
 
 int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed, strat_env* out, void* stream) {
   if (!roots || !out || rollouts <= 0 || (int64_t)roots->P.num_games * rollouts != (int64_t)out->P.num_games ||
-      out->P.auto_reset || out->hist)
+      out->P.auto_reset || out->hist || out->P.track)
     return STRAT_BAD_ARG;
   chain_break(roots);
   chain_break(out);

@@ -103,7 +103,7 @@ __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, 
 // kExternal = true (strat_step_observe): `actions` is the caller's input (validated) -> step ->
 //   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
 //   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
-template <bool kExternal, bool kChase>
+template <bool kExternal, bool kChase, bool kTrack>
 __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         if (lane < ng) {
           int a = -1;
           if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
-          StepOut o = step_game<false, true, kChase>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
+          StepOut o = step_game<false, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
           if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
           if (actions) actions[first + lane] = (int16_t)a;
           if (reward) reward[first + lane] = (int8_t)o.reward;
@@ -175,12 +175,13 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
         if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
         else if (rs) coop_setup(P, first, rs, g, work, lane);
+        if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
         if (lane < ng) store_game_global(lines, first + lane, g);
         flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
       } else {
         if (lane < ng) {
           int a = (int)actions[first + lane];
-          StepOut o = step_game<true, true, kChase>(P, (uint32_t)(first + lane), g, a);
+          StepOut o = step_game<true, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);
           if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
           reward[first + lane] = (int8_t)o.reward;
           done[first + lane] = (uint8_t)o.done;
@@ -194,6 +195,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           zero_smem16(work, kMaskBytes, lane);
           __syncwarp();
         }
+        if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
         if (lane < ng) {
           store_game_global(lines, first + lane, g);
           if (!g.done)  // of the NEW state

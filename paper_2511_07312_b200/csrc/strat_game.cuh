@@ -25,6 +25,11 @@ static inline int max(int a, int b) { return a > b ? a : b; }
 #define STRAT_UNROLL
 static inline uint16_t sd_ldlog(const uint16_t* p) { return *p; }
 static inline void sd_stlog(uint16_t* p, uint16_t v) { *p = v; }
+static inline uint32_t sd_ld32(const uint32_t* p) { return *p; }
+static inline void sd_st32(uint32_t* p, uint32_t v) { *p = v; }
+static inline void sd_or32(uint32_t* p, uint32_t v) { *p |= v; }
+static inline uint32_t sd_inc32(uint32_t* p, uint32_t v) { uint32_t o = *p; *p = o + v; return o; }
+static inline void sd_st16(uint32_t* words, int half, uint32_t v) { reinterpret_cast<uint16_t*>(words)[half] = (uint16_t)v; }
 #else
 #define STRAT_UNROLL _Pragma("unroll")
 #define SD __device__ __forceinline__
@@ -37,6 +42,12 @@ SD uint32_t sd_fsl(uint32_t lo, uint32_t hi, int s) { return __funnelshift_l(lo,
 // move-log accesses go to L2: consecutive launches of the fused step overlap on the device
 SD uint16_t sd_ldlog(const uint16_t* p) { return __ldcg(p); }
 SD void sd_stlog(uint16_t* p, uint16_t v) { __stcg(p, v); }
+SD uint32_t sd_ld32(const uint32_t* p) { return __ldcg(p); }
+SD void sd_st32(uint32_t* p, uint32_t v) { __stcg(p, v); }
+// tracker bits are OR-ed in at the L2 without reading them back (RED.OR: nothing to wait for)
+SD void sd_or32(uint32_t* p, uint32_t v) { atomicOr(p, v); }
+SD uint32_t sd_inc32(uint32_t* p, uint32_t v) { return atomicAdd(p, v); }
+SD void sd_st16(uint32_t* words, int half, uint32_t v) { __stcg(reinterpret_cast<uint16_t*>(words) + half, (uint16_t)v); }
 #endif
 
 namespace strat {
@@ -66,6 +77,7 @@ struct Params {  // per-environment constants handed to every kernel by value
   const uint8_t* pool;     // custom setups [2][pool_size][40] type codes (red, then blue), or null (R#30)
   int32_t pool_size;
   const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
+  uint32_t* track;         // [num_games][512] trackers of the paper's information state (S2), or null
 };
 
 // Rule switches handed to the move generators: bit 0 two-square rule, bit 1 chasing rule.
@@ -807,12 +819,166 @@ SD int battle(int att, int def) {
   return att > def ? 1 : att < def ? -1 : 0;
 }
 
+// ------------------------------------------------------------------ S2 trackers
+// What the paper's 487-channel information state needs beyond the board: one 2 KB block per game.
+//   words 4c..4c+3  record of the piece standing on square c (it travels with the piece):
+//       w0  bits 0-10 has threatened (Spy..Marshal revealed, bit 10 = a hidden piece)
+//           bits 11-21 has evaded (same keys)
+//           bits 22-28 the square the piece started on
+//       w1  bits 0-10 has been actively adjacent to (same keys)
+//           bits 11-23 has protected: own piece Spy..Marshal, Bomb (revealed), bit 11 an empty
+//                      square, bit 12 a hidden piece
+//       w2  bits 0-12 has protected against (types, bit 11 unused, bit 12 hidden)
+//           bits 13-25 has been protected by
+//       w3  bits 0-12 has been protected against
+//   word 400        number of pieces captured so far
+//   words 401..492  one entry per captured piece: start square | type << 7 | owner << 11 |
+//                   square of the battle << 12 | cause of death (1..6) << 19
+//   words 493..508  the last 32 plies, from | to << 7 in 16 bits (0x3FFF = unknown), ply p in
+//                   entry p & 31
+constexpr int kTrackWords = 512;
+constexpr int kTrkDeaths = 400, kTrkDeathList = 401, kTrkMaxDeaths = 92, kTrkMoves = 493;
+
+SD uint32_t* game_track(const Params& P, uint32_t local_game) {
+  return P.track ? P.track + (size_t)local_game * kTrackWords : nullptr;
+}
+SD int type_at(const Game& g, int c) {
+  return (int)(bb_test(g.t0, c) | (bb_test(g.t1, c) << 1) | (bb_test(g.t2, c) << 2) | (bb_test(g.t3, c) << 3));
+}
+// key of "the other piece at the time": eleven-wide groups (threat, evasion, adjacency) ...
+SD uint32_t key11(const Game& g, int c) {
+  if (!bb_test(g.rev, c)) return 1u << 10;
+  int t = type_at(g, c);
+  return t <= 10 ? 1u << (t - 1) : 0u;  // a revealed Bomb has no channel there
+}
+// ... and thirteen-wide groups (protection): Bomb at bit 10, hidden at bit 12
+SD uint32_t key13(const Game& g, int c) {
+  if (!bb_test(g.rev, c)) return 1u << 12;
+  int t = type_at(g, c);
+  return t <= 10 ? 1u << (t - 1) : t == T_BOMB ? 1u << 10 : 0u;
+}
+SD void trk_or(uint32_t* trk, int word, uint32_t bits) {
+  if (bits) sd_or32(trk + word, bits);
+}
+// Thread-level (re)start of a game's trackers: the squares the pieces stand on are their start
+// squares, the recent moves are the ones the line remembers (reading I9).
+SD void track_start_tail(uint32_t* trk, const Game& g) {
+  sd_st32(trk + kTrkDeaths, 0u);
+  // ring slot s holds the ply p with (p & 31) == s among the last 32: ply - 1 - j with
+  // j = (ply - 1 - s) & 31, known only if the line's 8-ply history has it (0x3FFF = unknown)
+  for (int w = 0; w < 16; ++w) {
+    uint32_t v = 0;
+    STRAT_UNROLL
+    for (int h = 0; h < 2; ++h) {
+      int j = (int)((g.ply - 1u - (uint32_t)(2 * w + h)) & 31u);
+      uint32_t e = j < 8 ? hist_entry(g, j) : kHistNone;
+      v |= e << (16 * h);
+    }
+    sd_st32(trk + kTrkMoves + w, v);
+  }
+}
+SD void track_start(uint32_t* trk, const Game& g) {
+  for (int c = 0; c < 100; ++c) {
+    sd_st32(trk + 4 * c, (uint32_t)c << 22); sd_st32(trk + 4 * c + 1, 0u);
+    sd_st32(trk + 4 * c + 2, 0u); sd_st32(trk + 4 * c + 3, 0u);
+  }
+  track_start_tail(trk, g);
+}
+// The trackers' share of one ply, judged on the position BEFORE the move (g is unchanged).
+// pt / tt = type of the moving piece / of what stands on the target square (0 = empty).
+SD void track_ply(uint32_t* trk, const Game& g, const Moves& m, int side, int from, int to, int dist, int pt, int tt) {
+  BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
+  // the mover's record and, for a battle, the defender's start square: the only reads of this ply
+  uint32_t r0 = sd_ld32(trk + 4 * from), r1 = sd_ld32(trk + 4 * from + 1), r2 = sd_ld32(trk + 4 * from + 2),
+           r3 = sd_ld32(trk + 4 * from + 3);
+  uint32_t d0 = tt != 0 ? sd_ld32(trk + 4 * to) : 0u;
+  // (i) active adjacency: every legal one-square capture that is not the move played
+  {
+    BB att[4];
+    att[0] = bb_and(m.d[0], bb_down<10>(enemy)); att[1] = bb_and(m.d[1], bb_down<1>(enemy));
+    att[2] = bb_and(m.d[2], bb_up<10>(enemy));   att[3] = bb_and(m.d[3], bb_up<1>(enemy));
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d) {
+      const int delta = d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1;
+      STRAT_UNROLL
+      for (int i = 0; i < 4; ++i) {
+        uint32_t w = att[d].w[i];
+        while (w) {
+          int p = 32 * i + sd_ffs(w) - 1; w &= w - 1;
+          int q = p + delta;
+          if (p == from && q == to) continue;
+          if (p == from) r1 |= key11(g, q);  // the mover's record is in registers and is written back below
+          else trk_or(trk, 4 * p + 1, key11(g, q));
+        }
+      }
+    }
+  }
+  if (tt == 0) {
+    // the previous ply, if it was a move to an empty square, may have threatened
+    uint32_t e0 = hist_entry(g, 0);
+    int x = (int)(e0 >> 7);
+    bool prev = e0 != kHistNone && g.battleless > 0 && bb_test(enemy, x);
+    BB nto = neighbours_of(to);
+    if (prev) {
+      uint32_t kA11 = key11(g, x), kA13 = key13(g, x);
+      // (ii) evasion
+      if (cells_adjacent(from, x) && !cells_adjacent(to, x)) r0 |= kA11 << 11;
+      // (iii) protection: own pieces, then empty squares, next to both A and the new square
+      BB both = bb_and(nto, neighbours_of(x));
+      BB prot = bb_and(both, mine);
+      uint32_t kC13 = (bb_test(g.rev, from) || dist >= 2) ? (pt <= 10 ? 1u << (pt - 1) : 0u) : 1u << 12;  // what C shows after this move
+      STRAT_UNROLL
+      for (int i = 0; i < 4; ++i) {
+        uint32_t w = prot.w[i];
+        while (w) {
+          int b = 32 * i + sd_ffs(w) - 1; w &= w - 1;
+          if (b == from) continue;
+          r1 |= key13(g, b) << 11; r2 |= kA13;
+          trk_or(trk, 4 * b + 2, kC13 << 13);
+          trk_or(trk, 4 * b + 3, kA13);
+        }
+      }
+      if (bb_any(bb_and(both, m.empty))) { r1 |= 1u << (11 + 11); r2 |= kA13; }
+    }
+    // (iv) threat
+    BB thr = bb_and(nto, enemy);
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      uint32_t w = thr.w[i];
+      while (w) { int q = 32 * i + sd_ffs(w) - 1; w &= w - 1; r0 |= key11(g, q); }
+    }
+    sd_st32(trk + 4 * to, r0); sd_st32(trk + 4 * to + 1, r1); sd_st32(trk + 4 * to + 2, r2); sd_st32(trk + 4 * to + 3, r3);
+  } else {
+    // (v) captures and causes of death; "revealed at the time of the attack" = before this battle
+    bool d_rev = bb_test(g.rev, to) != 0;
+    int out = battle(pt, tt);
+    bool d_dies = out >= 0 && tt != T_FLAG, c_dies = out <= 0;
+    uint32_t n = sd_inc32(trk + kTrkDeaths, (d_dies ? 1u : 0u) + (c_dies ? 1u : 0u));
+    if (d_dies) {
+      uint32_t cause = tt <= 10 ? (d_rev ? (out > 0 ? 4u : 5u) : 6u) : 0u;
+      if (n < (uint32_t)kTrkMaxDeaths)
+        sd_st32(trk + kTrkDeathList + n, ((d0 >> 22) & 127u) | ((uint32_t)tt << 7) | ((uint32_t)(side ^ 1) << 11) |
+                                             ((uint32_t)to << 12) | (cause << 19));
+      ++n;
+    }
+    if (c_dies) {
+      uint32_t cause = d_rev ? (out < 0 ? 1u : 2u) : 3u;
+      if (n < (uint32_t)kTrkMaxDeaths)
+        sd_st32(trk + kTrkDeathList + n, ((r0 >> 22) & 127u) | ((uint32_t)pt << 7) | ((uint32_t)side << 11) |
+                                             ((uint32_t)to << 12) | (cause << 19));
+    }
+    if (out > 0) { sd_st32(trk + 4 * to, r0); sd_st32(trk + 4 * to + 1, r1); sd_st32(trk + 4 * to + 2, r2); sd_st32(trk + 4 * to + 3, r3); }
+  }
+  // the ply itself
+  sd_st16(trk + kTrkMoves, (int)(g.ply & 31u), (uint32_t)from | ((uint32_t)to << 7));
+}
+
 struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; };
 
 // kValidate = false only when `a` was just drawn from this state's own legal mask.
 // kDeferReset: the caller performs the auto-reset itself (epoch is already advanced) when
 // o.needs_reset is set; the result must equal reset_game(P, local_game, g).
-template <bool kValidate, bool kDeferReset = false, bool kChase = false>
+template <bool kValidate, bool kDeferReset = false, bool kChase = false, bool kTrack = false>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   StepOut o; o.illegal = false; o.needs_reset = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
@@ -828,6 +994,10 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   int pt = bb_get(g.t0, sf) | (bb_get(g.t1, sf) << 1) | (bb_get(g.t2, sf) << 2) | (bb_get(g.t3, sf) << 3);
   uint32_t prev = bb_get(g.rev, sf);
   int tt = bb_get(g.t0, st) | (bb_get(g.t1, st) << 1) | (bb_get(g.t2, st) << 2) | (bb_get(g.t3, st) << 3);
+  if (kTrack && P.track) {  // S2 trackers, judged on the position before the move
+    Moves m; single_step_moves(g, side, rules_of<kChase>(P), m);
+    track_ply(game_track(P, local_game), g, m, side, from, to, dist, pt, tt);
+  }
   if (kChase && P.chase_rule) {  // chase state machine (R#28), judged on the position before the move
     uint32_t ap = chase_age(g, side), aq = chase_age(g, side ^ 1);
     if (tt != 0) {
@@ -889,7 +1059,8 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   o.done = g.done | ((uint32_t)side << 1) | ((g.done ? g.reason : 0u) << 2);
   if (g.done && P.auto_reset) {  // R#16
     g.epoch += 1;
-    if (kDeferReset) o.needs_reset = true; else reset_game(P, local_game, g);
+    if (kDeferReset) o.needs_reset = true;
+    else { reset_game(P, local_game, g); if (kTrack && P.track) track_start(game_track(P, local_game), g); }
   }
   return o;
 }

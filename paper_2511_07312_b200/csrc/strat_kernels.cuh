@@ -74,6 +74,31 @@ __device__ __forceinline__ void coop_setup(const Params& P, int first, uint32_t 
   __syncwarp();
 }
 
+// Warp-cooperative (re)start of the S2 trackers of the games flagged in `rs` (bit = lane = game of
+// the batch), whose new state the flagged lanes hold in g: the 100 cell records by all lanes
+// (16 bytes each: start square = the square itself, no history), the rest by the game's lane.
+__device__ __forceinline__ void coop_track_start(const Params& P, int first, uint32_t rs, const Game& g, int lane) {
+  for (uint32_t m = rs; m; m &= m - 1) {
+    int owner = __ffs((int)m) - 1;
+    uint4* blk = reinterpret_cast<uint4*>(P.track + (size_t)(first + owner) * kTrackWords);
+    for (int c = lane; c < 100; c += 32) __stcg(blk + c, make_uint4((uint32_t)c << 22, 0u, 0u, 0u));
+  }
+  if ((rs >> lane) & 1u) track_start_tail(game_track(P, (uint32_t)(first + lane)), g);
+}
+
+// Trackers of every game (re)started from its current line: after a reset, an import, a restore.
+// One warp per game.
+__global__ void __launch_bounds__(128) k_track_start(Params P, const uint32_t* __restrict__ lines) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int gi = blockIdx.x * 4 + warp;
+  if (gi >= P.num_games) return;
+  Game g;
+  load_game_global(lines, gi, g, nullptr);  // every lane reads the same line
+  uint4* blk = reinterpret_cast<uint4*>(P.track + (size_t)gi * kTrackWords);
+  for (int c = lane; c < 100; c += 32) __stcg(blk + c, make_uint4((uint32_t)c << 22, 0u, 0u, 0u));
+  if (lane == 0) track_start_tail(game_track(P, (uint32_t)gi), g);
+}
+
 // ------------------------------------------------------------------ kernels
 __global__ void __launch_bounds__(32) k_reset(Params P, uint32_t* __restrict__ lines) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
@@ -234,7 +259,7 @@ __global__ void __launch_bounds__(128) k_sample_uniform(Params P, const uint32_t
   if (lane == 0) actions[g] = (int16_t)action;
 }
 
-template <bool kChase>
+template <bool kChase, bool kTrack>
 __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ lines, const int16_t* __restrict__ actions,
                                              int8_t* __restrict__ reward, uint8_t* __restrict__ done, int* __restrict__ err,
                                              HistSlot hs) {
@@ -250,7 +275,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
   if (lane < ng) {
     read_game(s_state, lane, g);
     int a = (int)actions[first + lane];
-    StepOut o = step_game<true, true, kChase>(P, (uint32_t)(first + lane), g, a);
+    StepOut o = step_game<true, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);
     if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
     reward[first + lane] = (int8_t)o.reward;
     done[first + lane] = (uint8_t)o.done;
@@ -260,6 +285,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
   uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
   if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
   else if (rs) coop_setup(P, first, rs, g, s_scratch, lane);
+  if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
   if (lane < ng) write_game(s_state, lane, g);
   __syncwarp();
   store_lines(lines, first, ng, s_state, lane);
@@ -498,6 +524,187 @@ __global__ void __launch_bounds__(128) k_check_pool(const uint8_t* __restrict__ 
 __global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict__ lines) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g < n) lines[(size_t)g * kLineWords + 31] = 0;
+}
+
+// ------------------------------------------------------------------ S2 information state
+// ComputeInfostateTensor in the paper's own form: bf16 [N][487][10][10] = 97,400 bytes per game,
+// HBM-write bound.  One warp per game.  Build: the 48,700 cells of a game as a bit stream A
+// (bit set = 1.0) in shared memory, filled by the lanes with shared-memory atomics from the
+// game's line and tracker block - lane = square for the per-piece channels, lane = plane for the
+// whole-board ones.  The 58 channels that hold other values (type posteriors 12-35, the two
+// fractions 41-42, the -1.0 of the 32 move channels) get two more bit streams B and C over those
+// planes only, each with one bf16 value per plane.  Store: four cells (one nibble of the
+// streams, never straddling a plane: 100 = 25 nibbles) per lane and 8-byte streaming store, 256
+// contiguous bytes per warp instruction (a game is 8-byte, not 16-byte, aligned: 97,400 = 8 x 12,175).
+constexpr int kInfoPlanes = STRAT_INFO_PLANES;
+constexpr int kInfoNibbles = kInfoPlanes * 25;               // 12,175 per game
+constexpr int kInfoAWords = (kInfoPlanes * 100 + 31) / 32 + 1;  // 1,523
+constexpr int kInfoSpecial = 58;                              // planes 12-35, 41-42, 455-486
+constexpr int kInfoBWords = (kInfoSpecial * 100 + 31) / 32 + 1;  // 183
+constexpr int kInfoWarpWords = 2496;  // 1523 + 2*183 + 59 + 512 + 32 = 2492, rounded up to 16 bytes: 9,984 B per warp
+static_assert(kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1 + kTrackWords + kLineWords <= kInfoWarpWords && kInfoWarpWords % 4 == 0 &&
+              (kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1) % 4 == 0, "staging layout");
+constexpr int kInfoWarps = 11;  // 11 x 9,984 B = 107 KB per CTA: two CTAs (22 warps) per SM
+
+__device__ __forceinline__ void info_set(uint32_t* stream, int plane, int cell) {
+  int bit = 100 * plane + cell;
+  atomicOr(stream + (bit >> 5), 1u << (bit & 31));
+}
+__device__ __forceinline__ void info_place(uint32_t* stream, int plane, const BB& b) {  // a whole 100-bit plane
+  int o = 100 * plane, w = o >> 5, sh = o & 31;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    uint32_t v = b.w[i];
+    if (!v) continue;
+    atomicOr(stream + w + i, v << sh);
+    if (sh) atomicOr(stream + w + i + 1, v >> (32 - sh));
+  }
+}
+// Round-to-nearest-even bf16 of the IEEE double quotient num / den (> 0): DESIGN.md reading I8.
+__device__ __forceinline__ uint32_t bf16_of_ratio(long long num, long long den) {
+  if (num <= 0 || den <= 0) return 0u;
+  unsigned long long b = (unsigned long long)__double_as_longlong((double)num / (double)den);
+  int e = (int)((b >> 52) & 0x7FFull) - 1023;
+  unsigned long long man = b & 0xFFFFFFFFFFFFFull;
+  unsigned long long keep = man >> 45, rem = man & ((1ull << 45) - 1ull), half = 1ull << 44;
+  if (rem > half || (rem == half && (keep & 1ull))) ++keep;
+  if (keep == 128ull) { keep = 0; ++e; }
+  return ((uint32_t)(e + 127) << 7) | (uint32_t)keep;
+}
+
+__global__ void __launch_bounds__(32 * kInfoWarps) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
+                                                                      uint16_t* __restrict__ out) {
+  extern __shared__ __align__(16) uint32_t s_info[];
+  __shared__ __align__(8) uint2 s_lut[16], s_mlut[16];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x < 16) {
+    int t = threadIdx.x;
+    uint2 v, m;
+    v.x = ((t & 1) ? 0x3F80u : 0u) | ((t & 2) ? 0x3F800000u : 0u); v.y = ((t & 4) ? 0x3F80u : 0u) | ((t & 8) ? 0x3F800000u : 0u);
+    m.x = ((t & 1) ? 0xFFFFu : 0u) | ((t & 2) ? 0xFFFF0000u : 0u); m.y = ((t & 4) ? 0xFFFFu : 0u) | ((t & 8) ? 0xFFFF0000u : 0u);
+    s_lut[t] = v; s_mlut[t] = m;
+  }
+  __syncthreads();
+  uint32_t* A = s_info + warp * kInfoWarpWords;  // all three streams, then values, tracker block, line
+  uint32_t* Bs = A + kInfoAWords;
+  uint32_t* Cs = Bs + kInfoBWords;
+  uint32_t* val = Cs + kInfoBWords;               // [58] value of B | value of C << 16
+  uint32_t* trk = val + kInfoSpecial + 1;         // 16-byte aligned: (1523 + 366 + 59) = 1948 words
+  uint32_t* sline = trk + kTrackWords;
+  const int stride = gridDim.x * kInfoWarps;
+  for (int gi = blockIdx.x * kInfoWarps + warp; gi < P.num_games; gi += stride) {
+    // ---- stage the game's line and tracker block, clear the streams
+    for (int j = lane; j < (kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1) / 4; j += 32)
+      reinterpret_cast<uint4*>(A)[j] = make_uint4(0u, 0u, 0u, 0u);
+    {
+      const uint4* src = reinterpret_cast<const uint4*>(P.track + (size_t)gi * kTrackWords);
+      uint4* dst = reinterpret_cast<uint4*>(trk);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) dst[32 * k + lane] = __ldcg(src + 32 * k + lane);
+      sline[lane] = __ldcg(lines + (size_t)gi * kLineWords + lane);
+    }
+    __syncwarp();
+    Game g;
+    unpack_line(sline, g);
+    const int side = (int)(g.ply & 1u);
+    const BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
+    // ---- lane = square: what the piece on it is and has done
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int c = 32 * r + lane;
+      if (c >= 100) break;
+      if (!bb_test(occ, c)) {
+        if (!is_lake_cell(c)) info_set(A, 38, c);                     // empty (R#17: lakes are not squares)
+        continue;
+      }
+      const bool own = bb_test(mine, c) != 0, rev = bb_test(g.rev, c) != 0, mvd = bb_test(g.mvd, c) != 0;
+      const int t = type_at(g, c);
+      if (own) info_set(A, t - 1, c);                                 // 0-11
+      if (rev) info_set(A, (own ? 24 : 12) + t - 1, c);               // a revealed piece: probability 1 (12-35)
+      else info_set(A, own ? 36 : 37, c);                             // hidden pieces
+      if (mvd) info_set(A, own ? 39 : 40, c);                         // pieces that moved
+      const uint32_t r0 = trk[4 * c], r1 = trk[4 * c + 1], r2 = trk[4 * c + 2], r3 = trk[4 * c + 3];
+      const int a = own ? 43 : 76, b = own ? 251 : 303;
+      for (uint32_t w = r0 & 0x3FFFFFu; w; w &= w - 1) info_set(A, a + __ffs((int)w) - 1, c);            // threat, evasion
+      for (uint32_t w = r1 & 0x7FFu; w; w &= w - 1) info_set(A, a + 22 + __ffs((int)w) - 1, c);          // active adjacency
+      for (uint32_t w = (r1 >> 11) & 0x1FFFu; w; w &= w - 1) info_set(A, b + __ffs((int)w) - 1, c);      // protected
+      for (uint32_t w = r2 & 0x3FFFFFFu; w; w &= w - 1) info_set(A, b + 13 + __ffs((int)w) - 1, c);      // against, by
+      for (uint32_t w = r3 & 0x1FFFu; w; w &= w - 1) info_set(A, b + 39 + __ffs((int)w) - 1, c);         // been protected against
+      info_set(A, 355 + (int)((r0 >> 22) & 127u), c);                 // P:606 start square
+    }
+    // ---- lane = plane: type posteriors (reading I7), fractions, moves
+    if (lane < 24) {
+      // lanes 0-11: the opponent's pieces as the player sees them (12-23); 12-23: the player's, as the opponent does (24-35)
+      const int t = lane % 12 + 1;
+      const BB hid = bb_andn(lane < 12 ? enemy : mine, g.rev);
+      const BB hid_unmoved = bb_andn(hid, g.mvd), hid_moved = bb_and(hid, g.mvd);
+      const BB imm = bb_and(g.t3, bb_or(g.t2, bb_and(g.t1, g.t0)));
+      const int u = bb_popc(hid_unmoved), m = bb_popc(hid_moved), I = bb_popc(bb_and(hid, imm)), M = u + m - I;
+      const int ct = bb_popc(type_is(g, hid, t));
+      const bool immovable = t == T_FLAG || t == T_BOMB;
+      const int free_unmoved = u - I > 0 ? u - I : 0;
+      uint32_t vu = immovable ? bf16_of_ratio(ct, u) : bf16_of_ratio((long long)free_unmoved * ct, (long long)u * M);
+      uint32_t vm = immovable ? 0u : bf16_of_ratio(ct, M);
+      if (vu) info_place(Bs, lane, hid_unmoved);
+      if (vm) info_place(Cs, lane, hid_moved);
+      val[lane] = vu | (vm << 16);
+    } else if (lane < 26) {
+      BB all; all.w[0] = all.w[1] = all.w[2] = 0xFFFFFFFFu; all.w[3] = 0xFu;
+      uint32_t v = lane == 24 ? bf16_of_ratio((long long)g.ply, (long long)P.ply_cap)
+                              : (P.max_battleless > 0 ? bf16_of_ratio((long long)g.battleless, (long long)P.max_battleless) : 0u);
+      if (v) info_place(Bs, lane, all);
+      val[lane] = v;
+    }
+    {  // move j = ply t-1-j: +1.0 on the destination (stream A), -1.0 on the source (stream B)
+      const int slot = (int)((g.ply - 1u - (uint32_t)lane) & 31u);
+      const uint32_t e = (trk[kTrkMoves + (slot >> 1)] >> (16 * (slot & 1))) & 0xFFFFu;
+      if (e != kHistNone) {
+        info_set(A, 455 + lane, (int)(e >> 7));
+        info_set(Bs, 26 + lane, (int)(e & 127u));
+      }
+      val[26 + lane] = 0xBF80u;
+    }
+    // ---- captured pieces by start square and causes of death
+    {
+      const int n = min((int)trk[kTrkDeaths], kTrkMaxDeaths);
+      for (int k = lane; k < n; k += 32) {
+        const uint32_t e = trk[kTrkDeathList + k];
+        const int start = (int)(e & 127u), t = (int)((e >> 7) & 15u), owner = (int)((e >> 11) & 1u), sq = (int)((e >> 12) & 127u),
+                  cause = (int)((e >> 19) & 7u);
+        const int j = t <= 10 ? t - 1 : t == T_BOMB ? 10 : -1;
+        if (j >= 0) info_set(A, (owner == side ? 109 : 120) + j, start);
+        if (cause) info_set(A, (owner == side ? 131 : 191) + 10 * (cause - 1) + t - 1, sq);
+      }
+    }
+    __syncwarp();
+    // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game
+    uint2* dst = reinterpret_cast<uint2*>(out + (size_t)gi * (kInfoPlanes * 100));
+    const uint8_t* Ab = reinterpret_cast<const uint8_t*>(A);
+    const uint8_t* Bb = reinterpret_cast<const uint8_t*>(Bs);
+    const uint8_t* Cb = reinterpret_cast<const uint8_t*>(Cs);
+    // nibble ranges whose planes hold only 0 / 1.0 go through the one table; planes 12-35, 41-42 and
+    // 455-486 (nibbles 300-899, 1025-1074, 11375-12174) add the two valued streams
+    auto plain = [&](int lo, int hi) {
+#pragma unroll 4
+      for (int n = lo + lane; n < hi; n += 32) __stcs(dst + n, s_lut[(Ab[n >> 1] >> (4 * (n & 1))) & 15u]);
+    };
+    auto valued = [&](int lo, int hi, int first_plane, int first_special) {
+#pragma unroll 2
+      for (int n = lo + lane; n < hi; n += 32) {
+        uint2 v = s_lut[(Ab[n >> 1] >> (4 * (n & 1))) & 15u];
+        const int nn = n - 25 * (first_plane - first_special), sp = nn / 25;
+        const uint32_t vv = val[sp];
+        const uint32_t vb = (vv & 0xFFFFu) * 0x10001u, vc = (vv >> 16) * 0x10001u;
+        const uint2 mb = s_mlut[(Bb[nn >> 1] >> (4 * (nn & 1))) & 15u], mc = s_mlut[(Cb[nn >> 1] >> (4 * (nn & 1))) & 15u];
+        v.x |= (mb.x & vb) | (mc.x & vc);
+        v.y |= (mb.y & vb) | (mc.y & vc);
+        __stcs(dst + n, v);
+      }
+    };
+    plain(0, 300); valued(300, 900, 12, 0); plain(900, 1025); valued(1025, 1075, 41, 24); plain(1075, 11375);
+    valued(11375, kInfoNibbles, 455, 26);
+    __syncwarp();
+  }
 }
 
 __global__ void k_set_int(int* p, int v) { *p = v; }

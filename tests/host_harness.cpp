@@ -55,6 +55,21 @@ void hh_step(const uint8_t* line, int variant, uint64_t seed, uint32_t gidx, int
   export_canonical(g, line_out);
   *reward = o.reward; *done = (int)o.done; *illegal = o.illegal ? 1 : 0;
 }
+// S2 trackers: start a game's 512-word tracker block from a line ...
+void hh_track_start(const uint8_t* line, uint32_t* trk) {
+  Game g; import_canonical(line, g);
+  track_start(trk, g);
+}
+// ... and one validated, tracked step of game `gidx` (auto-reset inside restarts the trackers)
+void hh_track_step(const uint8_t* line, uint32_t* trk, int variant, uint64_t seed, uint32_t gidx, int max_plies,
+                   int auto_reset, int action, uint8_t* line_out, int* illegal) {
+  Params P = make(variant, seed, max_plies, auto_reset, 1, 0, gidx);
+  P.track = trk;
+  Game g; import_canonical(line, g);
+  StepOut o = step_game<true, false, false, true>(P, 0u, g, action);
+  export_canonical(g, line_out);
+  *illegal = o.illegal ? 1 : 0;
+}
 // observation as 4400 bf16 bit patterns
 void hh_encode(const uint8_t* line, uint16_t* obs) {
   Game g; import_canonical(line, g);

@@ -26,12 +26,14 @@ def test_library_exports_every_declared_symbol():
 
 def test_host_only_entry_points():
     L = binding.lib()
-    cfg = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0)
+    cfg = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0, 0, 0)
     ws = L.strat_workspace_bytes(C.byref(cfg))  # lines + error block + ticket ring + 2 flags per 32-game batch
     assert ws == 65536 * 128 + 256 + (8192 + 2 * 2048) * 4
-    chase = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 1, 0)  # + a 64-ply move log per game
+    chase = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 1, 0, 0, 0)  # + a 64-ply move log per game
     assert L.strat_workspace_bytes(C.byref(chase)) == ws + 65536 * 128
-    bad = binding.strat_config(0, 0, 0, 0, 0, 0, 1, 0, 0, 0)
+    info = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0, 1, 0)  # + 2 KB of S2 trackers per game
+    assert L.strat_workspace_bytes(C.byref(info)) == ws + 65536 * 2048
+    bad = binding.strat_config(0, 0, 0, 0, 0, 0, 1, 0, 0, 0, 0, 0)
     assert L.strat_workspace_bytes(C.byref(bad)) == 0
     assert L.strat_error_string(-4) == b"illegal action for a live game"
     off = (C.c_size_t * 5)()
@@ -47,13 +49,13 @@ def test_host_only_entry_points():
     assert L.strat_replay_bytes_in_place(131072, 64, blk) >= cap * 9256 + blk * (2 * 8800 + 456)
     assert L.strat_replay_bytes_in_place(131072, 64, 3) == 0  # the block must divide the capacity
     # RNG counters carry a 32-bit global game index
-    over = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65535)
+    over = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65535, 0, 0)
     assert L.strat_workspace_bytes(C.byref(over)) == 0
-    edge = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65536)
+    edge = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, (1 << 32) - 65536, 0, 0)
     assert L.strat_workspace_bytes(C.byref(edge)) == ws
     # sizes of the per-step outputs the e2e entry point stages
     n = 1000
-    cfg = binding.strat_config(n, 0, 0, 0, 0, 0, 1, 0, 0, 0)
+    cfg = binding.strat_config(n, 0, 0, 0, 0, 0, 1, 0, 0, 0, 0, 0)
     assert L.strat_host_scratch_bytes(C.byref(cfg)) >= n * 9256
 
 
@@ -64,4 +66,4 @@ def test_config_struct_matches_header():
     fields = re.findall(r"(u?int\d+_t)\s+(\w+);", body)
     ctype = {"int32_t": C.c_int32, "uint64_t": C.c_uint64}
     assert [(n, ctype[t]) for t, n in fields] == list(binding.strat_config._fields_)
-    assert C.sizeof(binding.strat_config) == 48
+    assert C.sizeof(binding.strat_config) == 56

@@ -30,6 +30,8 @@ def hh(tmp_path_factory):
     L.hh_step.argtypes = [vp, C.c_int, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp,
                           C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.hh_encode.argtypes = [vp, vp]
+    L.hh_track_start.argtypes = [vp, vp]
+    L.hh_track_step.argtypes = [vp, vp, C.c_int, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_int, vp, C.POINTER(C.c_int)]
     return L
 
 
@@ -151,3 +153,90 @@ def test_caged_chases_on_host(hh):
             pool = quiet if quiet and rng.random() < 0.9 else legal
             o.step(np.array([pool[rng.integers(len(pool))]], np.int16))
     assert bans > 0
+
+
+def _channels_from_tracker_block(line, trk):
+    """The tracker-derived channels of the 487-channel information state (43-486 except nothing
+    else) decoded from a game's tracker block by its documented layout (csrc/strat_game.cuh
+    "S2 trackers"): {(channel, square): +1 / -1}.  Test-side restatement of the LAYOUT only."""
+    side = (int(line[116]) | (int(line[117]) << 8)) & 1
+    ply = int(line[116]) | (int(line[117]) << 8)
+    out = {}
+    for c in range(100):
+        b = int(line[c])
+        if (b & 15) in (0, 15):
+            continue
+        own = ((b >> 4) & 1) == side
+        r0, r1, r2, r3 = (int(x) for x in trk[4 * c:4 * c + 4])
+        a, p = (43, 251) if own else (76, 303)
+        for j in range(22):
+            if (r0 >> j) & 1:
+                out[(a + j, c)] = 1
+        for j in range(11):
+            if (r1 >> j) & 1:
+                out[(a + 22 + j, c)] = 1
+        for j in range(13):
+            if (r1 >> (11 + j)) & 1:
+                out[(p + j, c)] = 1
+            if (r2 >> j) & 1:
+                out[(p + 13 + j, c)] = 1
+            if (r2 >> (13 + j)) & 1:
+                out[(p + 26 + j, c)] = 1
+            if (r3 >> j) & 1:
+                out[(p + 39 + j, c)] = 1
+        out[(355 + ((r0 >> 22) & 127), c)] = 1
+    for k in range(int(trk[400])):
+        e = int(trk[401 + k])
+        start, t, owner, sq, cause = e & 127, (e >> 7) & 15, (e >> 11) & 1, (e >> 12) & 127, (e >> 19) & 7
+        j = t - 1 if t <= 10 else 10 if t == 12 else -1
+        if j >= 0:
+            out[((109 if owner == side else 120) + j, start)] = 1
+        if cause:
+            out[((131 if owner == side else 191) + 10 * (cause - 1) + t - 1, sq)] = 1
+    for j in range(32):
+        slot = (ply - 1 - j) & 31
+        e = (int(trk[493 + (slot >> 1)]) >> (16 * (slot & 1))) & 0xFFFF
+        if e != 0x3FFF:
+            out[(455 + j, e >> 7)] = 1
+            out[(455 + j, e & 127)] = -1
+    return out
+
+
+@pytest.mark.parametrize("variant,cap", [(0, 160), (1, 300)])
+def test_information_state_trackers_on_host_equal_oracle(hh, variant, cap):
+    """The per-ply tracker update of the device code (track_ply: threats, evasions, active
+    adjacency, protections, captures and causes of death, start squares, move ring) against the
+    oracle's 487-channel information state, game by game, every few plies, across auto-resets."""
+    n, seed = 24, 5
+    kw = dict(variant=variant, seed=seed, max_plies=cap, auto_reset=1, infostate=1)
+    o = orc.Env(n, **kw)
+    trk = np.zeros((n, 512), np.uint32)
+    b = o.get_boards()
+    for g in range(n):
+        hh.hh_track_start(_p(b[g]), _p(trk[g]))
+    line_out = np.zeros(128, np.uint8)
+    ill = C.c_int()
+    seen = set()
+    for t in range(420):
+        b = o.get_boards()
+        oa = o.sample_uniform(o.legal_mask())
+        o.step(oa)
+        nb = o.get_boards()
+        for g in range(n):
+            hh.hh_track_step(_p(b[g]), _p(trk[g]), variant, seed, g, cap, 1, int(oa[g]), _p(line_out), C.byref(ill))
+            assert ill.value == 0 and np.array_equal(line_out, nb[g]), (t, g)
+        if t % 7 == 6 or t < 12:
+            obs = o.encode_infostate().reshape(n, 487, 100)
+            for g in range(n):
+                want = {}
+                ch, sq = np.nonzero(obs[g, 43:])
+                for c_, s_ in zip(ch, sq):
+                    v = int(obs[g, 43 + c_, s_])
+                    want[(int(c_) + 43, int(s_))] = 1 if v == 0x3F80 else -1 if v == 0xBF80 else v
+                got = _channels_from_tracker_block(nb[g], trk[g])
+                assert got == want, (t, g, sorted(set(got.items()) ^ set(want.items()))[:8])
+                seen.update(c_ for c_, _ in got)
+    groups = [(43, 54), (54, 65), (65, 76), (109, 131), (131, 251), (251, 264), (264, 277), (277, 290), (290, 303)]
+    for lo, hi in groups:  # every channel group was exercised
+        assert any(lo <= c_ < hi for c_ in seen), (lo, hi)
+    assert (o.get_boards()[:, 124] > 0).any()
