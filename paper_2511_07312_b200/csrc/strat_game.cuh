@@ -30,6 +30,8 @@ static inline void sd_st32(uint32_t* p, uint32_t v) { *p = v; }
 static inline void sd_or32(uint32_t* p, uint32_t v) { *p |= v; }
 static inline uint32_t sd_inc32(uint32_t* p, uint32_t v) { uint32_t o = *p; *p = o + v; return o; }
 static inline void sd_st16(uint32_t* words, int half, uint32_t v) { reinterpret_cast<uint16_t*>(words)[half] = (uint16_t)v; }
+static inline void sd_ld128(const uint32_t* p, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) { a = p[0]; b = p[1]; c = p[2]; d = p[3]; }
+static inline void sd_st128(uint32_t* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) { p[0] = a; p[1] = b; p[2] = c; p[3] = d; }
 #else
 #define STRAT_UNROLL _Pragma("unroll")
 #define SD __device__ __forceinline__
@@ -48,6 +50,10 @@ SD void sd_st32(uint32_t* p, uint32_t v) { __stcg(p, v); }
 SD void sd_or32(uint32_t* p, uint32_t v) { atomicOr(p, v); }
 SD uint32_t sd_inc32(uint32_t* p, uint32_t v) { return atomicAdd(p, v); }
 SD void sd_st16(uint32_t* words, int half, uint32_t v) { __stcg(reinterpret_cast<uint16_t*>(words) + half, (uint16_t)v); }
+SD void sd_ld128(const uint32_t* p, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
+  uint4 v = __ldcg(reinterpret_cast<const uint4*>(p)); a = v.x; b = v.y; c = v.z; d = v.w;
+}
+SD void sd_st128(uint32_t* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) { __stcg(reinterpret_cast<uint4*>(p), make_uint4(a, b, c, d)); }
 #endif
 
 namespace strat {
@@ -233,7 +239,12 @@ SD void pack_line(const Game& g, uint32_t* W) {
   W[19] |= (g.done | (g.reason << 1) | ((uint32_t)(g.result + 1) << 4)) << 4;
   W[28] = g.ply | (g.battleless << 16); W[29] = g.epoch; W[30] = g.chase; W[31] = g.logn;
 }
-SD uint32_t hist_entry(const Game& g, int j) { return (g.h[j >> 1] >> (14 * (j & 1))) & 0x3FFFu; }
+SD uint32_t hist_entry(const Game& g, int j) {  // selects, not an indexed load: g stays in registers
+  const int k = j >> 1;
+  uint32_t w = g.h[0];
+  w = k == 1 ? g.h[1] : w; w = k == 2 ? g.h[2] : w; w = k == 3 ? g.h[3] : w;
+  return (w >> (14 * (j & 1))) & 0x3FFFu;
+}
 SD void hist_push(Game& g, uint32_t e) {
   uint32_t carry = e;
   STRAT_UNROLL
@@ -845,21 +856,6 @@ SD uint32_t* game_track(const Params& P, uint32_t local_game) {
 SD int type_at(const Game& g, int c) {
   return (int)(bb_test(g.t0, c) | (bb_test(g.t1, c) << 1) | (bb_test(g.t2, c) << 2) | (bb_test(g.t3, c) << 3));
 }
-// key of "the other piece at the time": eleven-wide groups (threat, evasion, adjacency) ...
-SD uint32_t key11(const Game& g, int c) {
-  if (!bb_test(g.rev, c)) return 1u << 10;
-  int t = type_at(g, c);
-  return t <= 10 ? 1u << (t - 1) : 0u;  // a revealed Bomb has no channel there
-}
-// ... and thirteen-wide groups (protection): Bomb at bit 10, hidden at bit 12
-SD uint32_t key13(const Game& g, int c) {
-  if (!bb_test(g.rev, c)) return 1u << 12;
-  int t = type_at(g, c);
-  return t <= 10 ? 1u << (t - 1) : t == T_BOMB ? 1u << 10 : 0u;
-}
-SD void trk_or(uint32_t* trk, int word, uint32_t bits) {
-  if (bits) sd_or32(trk + word, bits);
-}
 // Thread-level (re)start of a game's trackers: the squares the pieces stand on are their start
 // squares, the recent moves are the ones the line remembers (reading I9).
 SD void track_start_tail(uint32_t* trk, const Game& g) {
@@ -884,75 +880,125 @@ SD void track_start(uint32_t* trk, const Game& g) {
   }
   track_start_tail(trk, g);
 }
+// The seven state bits of square c: type (bits 0-3), owner (4), moved (5), revealed (6).
+SD uint32_t cell_bits(const Game& g, int c) {
+  const int wi = c >> 5, sh = c & 31;
+  return ((bb_word(g.t0, wi) >> sh) & 1u) | (((bb_word(g.t1, wi) >> sh) & 1u) << 1) | (((bb_word(g.t2, wi) >> sh) & 1u) << 2) |
+         (((bb_word(g.t3, wi) >> sh) & 1u) << 3) | (((bb_word(g.own, wi) >> sh) & 1u) << 4) |
+         (((bb_word(g.mvd, wi) >> sh) & 1u) << 5) | (((bb_word(g.rev, wi) >> sh) & 1u) << 6);
+}
+SD uint32_t key11_of(uint32_t b) {  // b = cell_bits of a piece
+  uint32_t t = b & 15u;
+  return !(b & 64u) ? 1u << 10 : t <= 10u ? 1u << (t - 1u) : 0u;
+}
+SD uint32_t key13_of(uint32_t b) {
+  uint32_t t = b & 15u;
+  return !(b & 64u) ? 1u << 12 : t <= 10u ? 1u << (t - 1u) : t == (uint32_t)T_BOMB ? 1u << 10 : 0u;
+}
 // The trackers' share of one ply, judged on the position BEFORE the move (g is unchanged).
 // pt / tt = type of the moving piece / of what stands on the target square (0 = empty).
-SD void track_ply(uint32_t* trk, const Game& g, const Moves& m, int side, int from, int to, int dist, int pt, int tt) {
-  BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
-  // the mover's record and, for a battle, the defender's start square: the only reads of this ply
-  uint32_t r0 = sd_ld32(trk + 4 * from), r1 = sd_ld32(trk + 4 * from + 1), r2 = sd_ld32(trk + 4 * from + 2),
-           r3 = sd_ld32(trk + 4 * from + 3);
-  uint32_t d0 = tt != 0 ? sd_ld32(trk + 4 * to) : 0u;
-  // (i) active adjacency: every legal one-square capture that is not the move played
+// Written for one thread per game next to 31 other games: the mover's record is the only thing
+// read (one 16-byte load), every other update is an OR at the L2, and the only loops run over
+// the (few) pieces that stand next to an enemy.
+SD void track_ply(uint32_t* trk, const Game& g, int two_square, int side, int from, int to, int dist, int pt, int tt) {
+  const BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
+  uint32_t r0, r1, r2, r3;
+  sd_ld128(trk + 4 * from, r0, r1, r2, r3);
+  const uint32_t d0 = tt != 0 ? sd_ld32(trk + 4 * to) : 0u;
+  // (i) active adjacency: every legal one-square capture that is not the move played.
+  // att[d] = own movable pieces with an enemy on the next square in direction d.
   {
+    const BB movable = bb_andn(mine, bb_and(g.t3, bb_or(g.t2, bb_and(g.t1, g.t0))));
     BB att[4];
-    att[0] = bb_and(m.d[0], bb_down<10>(enemy)); att[1] = bb_and(m.d[1], bb_down<1>(enemy));
-    att[2] = bb_and(m.d[2], bb_up<10>(enemy));   att[3] = bb_and(m.d[3], bb_up<1>(enemy));
+    att[0] = bb_and(movable, bb_down<10>(enemy));
+    att[1] = bb_and(bb_and(movable, bb_down<1>(enemy)), bb_const(kNotCol9));
+    att[2] = bb_and(movable, bb_up<10>(enemy));
+    att[3] = bb_and(bb_and(movable, bb_up<1>(enemy)), bb_const(kNotCol0));
+    const Ban ban = two_square_ban(g, side, two_square);
+    const int skip_from = ban.from >= 0 && ban.k <= 1 ? ban.from : -1;  // that capture is not legal: no chance to attack
+    const CellSel sb = cell_sel(skip_from >= 0 ? skip_from : 0), sf = cell_sel(from);
+    const bool played = tt != 0 && dist == 1;
+    const int pdir = to - from == 10 ? 0 : to - from == 1 ? 1 : to - from == -10 ? 2 : 3;
     STRAT_UNROLL
-    for (int d = 0; d < 4; ++d) {
-      const int delta = d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1;
+    for (int d = 0; d < 4; ++d)
       STRAT_UNROLL
       for (int i = 0; i < 4; ++i) {
-        uint32_t w = att[d].w[i];
-        while (w) {
-          int p = 32 * i + sd_ffs(w) - 1; w &= w - 1;
-          int q = p + delta;
-          if (p == from && q == to) continue;
-          if (p == from) r1 |= key11(g, q);  // the mover's record is in registers and is written back below
-          else trk_or(trk, 4 * p + 1, key11(g, q));
+        if (skip_from >= 0 && ban.dir == d) att[d].w[i] &= ~sb.m[i];
+        if (played && pdir == d) att[d].w[i] &= ~sf.m[i];
+      }
+    // next to a HIDDEN enemy piece: the key is the same for all of them, no square needs a look
+    const BB hid = bb_andn(enemy, g.rev);
+    BB ph;
+    {
+      BB h0 = bb_down<10>(hid), h1 = bb_down<1>(hid), h2 = bb_up<10>(hid), h3 = bb_up<1>(hid);
+      STRAT_UNROLL
+      for (int i = 0; i < 4; ++i)
+        ph.w[i] = (att[0].w[i] & h0.w[i]) | (att[1].w[i] & h1.w[i]) | (att[2].w[i] & h2.w[i]) | (att[3].w[i] & h3.w[i]);
+    }
+    if (bb_get(ph, sf)) r1 |= 1u << 10;  // the mover's record is in registers and is written back below
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      uint32_t w = ph.w[i] & ~sf.m[i];
+      while (w) { int p = 32 * i + sd_ffs(w) - 1; w &= w - 1; sd_or32(trk + 4 * p + 1, 1u << 10); }
+    }
+    // next to a REVEALED enemy piece: walk those enemies (few), their type is the key
+    const BB seen = bb_and(enemy, g.rev);
+    BB qs;
+    {
+      BB a0 = bb_up<10>(att[0]), a1 = bb_up<1>(att[1]), a2 = bb_down<10>(att[2]), a3 = bb_down<1>(att[3]);  // targets of the attackers
+      STRAT_UNROLL
+      for (int i = 0; i < 4; ++i) qs.w[i] = seen.w[i] & (a0.w[i] | a1.w[i] | a2.w[i] | a3.w[i]);
+    }
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      uint32_t w = qs.w[i];
+      while (w) {
+        int q = 32 * i + sd_ffs(w) - 1; w &= w - 1;
+        uint32_t key = key11_of(cell_bits(g, q));
+        STRAT_UNROLL
+        for (int d = 0; d < 4; ++d) {
+          const int p = q - (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
+          if (p < 0 || p > 99 || !bb_test(att[d], p)) continue;
+          if (p == from) r1 |= key; else if (key) sd_or32(trk + 4 * p + 1, key);
         }
       }
     }
   }
   if (tt == 0) {
     // the previous ply, if it was a move to an empty square, may have threatened
-    uint32_t e0 = hist_entry(g, 0);
-    int x = (int)(e0 >> 7);
-    bool prev = e0 != kHistNone && g.battleless > 0 && bb_test(enemy, x);
-    BB nto = neighbours_of(to);
-    if (prev) {
-      uint32_t kA11 = key11(g, x), kA13 = key13(g, x);
-      // (ii) evasion
-      if (cells_adjacent(from, x) && !cells_adjacent(to, x)) r0 |= kA11 << 11;
-      // (iii) protection: own pieces, then empty squares, next to both A and the new square
-      BB both = bb_and(nto, neighbours_of(x));
-      BB prot = bb_and(both, mine);
-      uint32_t kC13 = (bb_test(g.rev, from) || dist >= 2) ? (pt <= 10 ? 1u << (pt - 1) : 0u) : 1u << 12;  // what C shows after this move
-      STRAT_UNROLL
-      for (int i = 0; i < 4; ++i) {
-        uint32_t w = prot.w[i];
-        while (w) {
-          int b = 32 * i + sd_ffs(w) - 1; w &= w - 1;
-          if (b == from) continue;
-          r1 |= key13(g, b) << 11; r2 |= kA13;
-          trk_or(trk, 4 * b + 2, kC13 << 13);
-          trk_or(trk, 4 * b + 3, kA13);
+    const uint32_t e0 = hist_entry(g, 0);
+    const int x = (int)(e0 >> 7);
+    const bool prev = e0 != kHistNone && g.battleless > 0 && bb_test(enemy, x);
+    const uint32_t bA = prev ? cell_bits(g, x) : 0u;
+    const uint32_t kA11 = key11_of(bA), kA13 = key13_of(bA);
+    // (ii) evasion
+    if (prev && cells_adjacent(from, x) && !cells_adjacent(to, x)) r0 |= kA11 << 11;
+    const uint32_t kC13 = (bb_test(g.rev, from) || dist >= 2) ? (pt <= 10 ? 1u << (pt - 1) : 0u) : 1u << 12;  // what C shows after this move
+    const int tr = to / 10, tq = to - 10 * tr;
+    STRAT_UNROLL
+    for (int d = 0; d < 4; ++d) {  // the four squares next to the new square
+      const bool on = d == 0 ? tr < 9 : d == 1 ? tq < 9 : d == 2 ? tr > 0 : tq > 0;
+      const int q = to + (d == 0 ? 10 : d == 1 ? 1 : d == 2 ? -10 : -1);
+      if (!on || q == from) continue;
+      const uint32_t b = cell_bits(g, q);
+      const bool piece = (b & 15u) != 0u, theirs = piece && (int)((b >> 4) & 1u) != side;
+      if (theirs) r0 |= key11_of(b);                                       // (iv) threat
+      if (prev && cells_adjacent(q, x)) {                                  // (iii) protection
+        if (piece && !theirs) {
+          r1 |= key13_of(b) << 11; r2 |= kA13;
+          if (kC13) sd_or32(trk + 4 * q + 2, kC13 << 13);
+          if (kA13) sd_or32(trk + 4 * q + 3, kA13);
+        } else if (!piece && !is_lake_cell(q)) {
+          r1 |= 1u << (11 + 11); r2 |= kA13;                              // ... of an empty square
         }
       }
-      if (bb_any(bb_and(both, m.empty))) { r1 |= 1u << (11 + 11); r2 |= kA13; }
     }
-    // (iv) threat
-    BB thr = bb_and(nto, enemy);
-    STRAT_UNROLL
-    for (int i = 0; i < 4; ++i) {
-      uint32_t w = thr.w[i];
-      while (w) { int q = 32 * i + sd_ffs(w) - 1; w &= w - 1; r0 |= key11(g, q); }
-    }
-    sd_st32(trk + 4 * to, r0); sd_st32(trk + 4 * to + 1, r1); sd_st32(trk + 4 * to + 2, r2); sd_st32(trk + 4 * to + 3, r3);
+    sd_st128(trk + 4 * to, r0, r1, r2, r3);
   } else {
     // (v) captures and causes of death; "revealed at the time of the attack" = before this battle
-    bool d_rev = bb_test(g.rev, to) != 0;
-    int out = battle(pt, tt);
-    bool d_dies = out >= 0 && tt != T_FLAG, c_dies = out <= 0;
+    const bool d_rev = bb_test(g.rev, to) != 0;
+    const int out = battle(pt, tt);
+    const bool d_dies = out >= 0 && tt != T_FLAG, c_dies = out <= 0;
     uint32_t n = sd_inc32(trk + kTrkDeaths, (d_dies ? 1u : 0u) + (c_dies ? 1u : 0u));
     if (d_dies) {
       uint32_t cause = tt <= 10 ? (d_rev ? (out > 0 ? 4u : 5u) : 6u) : 0u;
@@ -967,7 +1013,7 @@ SD void track_ply(uint32_t* trk, const Game& g, const Moves& m, int side, int fr
         sd_st32(trk + kTrkDeathList + n, ((r0 >> 22) & 127u) | ((uint32_t)pt << 7) | ((uint32_t)side << 11) |
                                              ((uint32_t)to << 12) | (cause << 19));
     }
-    if (out > 0) { sd_st32(trk + 4 * to, r0); sd_st32(trk + 4 * to + 1, r1); sd_st32(trk + 4 * to + 2, r2); sd_st32(trk + 4 * to + 3, r3); }
+    if (out > 0) sd_st128(trk + 4 * to, r0, r1, r2, r3);
   }
   // the ply itself
   sd_st16(trk + kTrkMoves, (int)(g.ply & 31u), (uint32_t)from | ((uint32_t)to << 7));
@@ -994,10 +1040,8 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   int pt = bb_get(g.t0, sf) | (bb_get(g.t1, sf) << 1) | (bb_get(g.t2, sf) << 2) | (bb_get(g.t3, sf) << 3);
   uint32_t prev = bb_get(g.rev, sf);
   int tt = bb_get(g.t0, st) | (bb_get(g.t1, st) << 1) | (bb_get(g.t2, st) << 2) | (bb_get(g.t3, st) << 3);
-  if (kTrack && P.track) {  // S2 trackers, judged on the position before the move
-    Moves m; single_step_moves(g, side, rules_of<kChase>(P), m);
-    track_ply(game_track(P, local_game), g, m, side, from, to, dist, pt, tt);
-  }
+  if (kTrack && P.track)  // S2 trackers, judged on the position before the move
+    track_ply(game_track(P, local_game), g, P.two_square, side, from, to, dist, pt, tt);
   if (kChase && P.chase_rule) {  // chase state machine (R#28), judged on the position before the move
     uint32_t ap = chase_age(g, side), aq = chase_age(g, side ^ 1);
     if (tt != 0) {

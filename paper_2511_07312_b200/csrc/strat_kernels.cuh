@@ -575,16 +575,7 @@ __device__ __forceinline__ uint32_t bf16_of_ratio(long long num, long long den) 
 __global__ void __launch_bounds__(32 * kInfoWarps) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
                                                                       uint16_t* __restrict__ out) {
   extern __shared__ __align__(16) uint32_t s_info[];
-  __shared__ __align__(8) uint2 s_lut[16], s_mlut[16];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (threadIdx.x < 16) {
-    int t = threadIdx.x;
-    uint2 v, m;
-    v.x = ((t & 1) ? 0x3F80u : 0u) | ((t & 2) ? 0x3F800000u : 0u); v.y = ((t & 4) ? 0x3F80u : 0u) | ((t & 8) ? 0x3F800000u : 0u);
-    m.x = ((t & 1) ? 0xFFFFu : 0u) | ((t & 2) ? 0xFFFF0000u : 0u); m.y = ((t & 4) ? 0xFFFFu : 0u) | ((t & 8) ? 0xFFFF0000u : 0u);
-    s_lut[t] = v; s_mlut[t] = m;
-  }
-  __syncthreads();
   uint32_t* A = s_info + warp * kInfoWarpWords;  // all three streams, then values, tracker block, line
   uint32_t* Bs = A + kInfoAWords;
   uint32_t* Cs = Bs + kInfoBWords;
@@ -677,32 +668,52 @@ __global__ void __launch_bounds__(32 * kInfoWarps) k_encode_infostate(Params P, 
       }
     }
     __syncwarp();
-    // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game
-    uint2* dst = reinterpret_cast<uint2*>(out + (size_t)gi * (kInfoPlanes * 100));
-    const uint8_t* Ab = reinterpret_cast<const uint8_t*>(A);
-    const uint8_t* Bb = reinterpret_cast<const uint8_t*>(Bs);
-    const uint8_t* Cb = reinterpret_cast<const uint8_t*>(Cs);
-    // nibble ranges whose planes hold only 0 / 1.0 go through the one table; planes 12-35, 41-42 and
-    // 455-486 (nibbles 300-899, 1025-1074, 11375-12174) add the two valued streams
-    auto plain = [&](int lo, int hi) {
-#pragma unroll 4
-      for (int n = lo + lane; n < hi; n += 32) __stcs(dst + n, s_lut[(Ab[n >> 1] >> (4 * (n & 1))) & 15u]);
+    // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game, two nibbles (16 bytes) per
+    // lane and streaming store.  A game starts 8-byte aligned (odd games at 8 mod 16), so an odd
+    // game's first nibble and an even game's last one go out alone.  Bits -> bf16 in registers:
+    // two bits spread to bit 0 and bit 16, times 0x3F80 (or times the plane's value).
+    const int odd = gi & 1;
+    uint16_t* gout = out + (size_t)gi * (kInfoPlanes * 100);
+    uint4* dst = reinterpret_cast<uint4*>(gout + 4 * odd);  // pair k = nibbles 2k+odd, 2k+odd+1
+    auto spread = [](uint32_t t) { return (t & 1u) | ((t & 2u) << 15); };
+    auto nib_value = [&](int n) -> uint2 {  // any nibble, valued planes included
+      const uint32_t t = (A[n >> 3] >> (4 * (n & 7))) & 15u;
+      uint2 v = make_uint2(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u);
+      const int shift = n < 300 ? -1 : n < 900 ? 300 : n < 1025 ? -1 : n < 1075 ? 1025 - 600 : n < 11375 ? -1 : 11375 - 650;
+      if (shift >= 0) {
+        const int nn = n - shift;  // nibble of the compact valued streams: planes 12-35 -> 0-23, 41-42 -> 24-25, 455-486 -> 26-57
+        const uint32_t vv = val[nn / 25];
+        const uint32_t tb = (Bs[nn >> 3] >> (4 * (nn & 7))) & 15u, tc = (Cs[nn >> 3] >> (4 * (nn & 7))) & 15u;
+        v.x |= spread(tb) * (vv & 0xFFFFu) | spread(tc) * (vv >> 16);
+        v.y |= spread(tb >> 2) * (vv & 0xFFFFu) | spread(tc >> 2) * (vv >> 16);
+      }
+      return v;
     };
-    auto valued = [&](int lo, int hi, int first_plane, int first_special) {
-#pragma unroll 2
-      for (int n = lo + lane; n < hi; n += 32) {
-        uint2 v = s_lut[(Ab[n >> 1] >> (4 * (n & 1))) & 15u];
-        const int nn = n - 25 * (first_plane - first_special), sp = nn / 25;
-        const uint32_t vv = val[sp];
-        const uint32_t vb = (vv & 0xFFFFu) * 0x10001u, vc = (vv >> 16) * 0x10001u;
-        const uint2 mb = s_mlut[(Bb[nn >> 1] >> (4 * (nn & 1))) & 15u], mc = s_mlut[(Cb[nn >> 1] >> (4 * (nn & 1))) & 15u];
-        v.x |= (mb.x & vb) | (mc.x & vc);
-        v.y |= (mb.y & vb) | (mc.y & vc);
-        __stcs(dst + n, v);
+    auto plain_pairs = [&](int ka, int kb) {  // pairs ka..kb-1 whose two nibbles lie in 0/1 planes
+#pragma unroll 4
+      for (int k = ka + lane; k < kb; k += 32) {
+        const int bit = 8 * k + 4 * odd;
+        const uint32_t t = __funnelshift_r(A[bit >> 5], A[(bit >> 5) + 1], bit & 31);
+        __stcs(dst + k, make_uint4(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u, spread(t >> 4) * 0x3F80u,
+                                   spread(t >> 6) * 0x3F80u));
       }
     };
-    plain(0, 300); valued(300, 900, 12, 0); plain(900, 1025); valued(1025, 1075, 41, 24); plain(1075, 11375);
-    valued(11375, kInfoNibbles, 455, 26);
+    auto any_pairs = [&](int ka, int kb) {
+      for (int k = ka + lane; k < kb; k += 32) {
+        const uint2 lo = nib_value(2 * k + odd), hi = nib_value(2 * k + odd + 1);
+        __stcs(dst + k, make_uint4(lo.x, lo.y, hi.x, hi.y));
+      }
+    };
+    {
+      // plain nibble ranges [0,300) [900,1025) [1075,11375): pair k is plain iff lo <= 2k+odd and 2k+odd+1 < hi
+      const int a0 = 0, b0 = (300 - 2 - odd) / 2 + 1, a1 = (900 - odd + 1) / 2, b1 = (1025 - 2 - odd) / 2 + 1,
+                a2 = (1075 - odd + 1) / 2, b2 = (11375 - 2 - odd) / 2 + 1, pairs = (kInfoNibbles - 1) / 2;
+      plain_pairs(a0, b0); any_pairs(b0, a1); plain_pairs(a1, b1); any_pairs(b1, a2); plain_pairs(a2, b2); any_pairs(b2, pairs);
+      if (lane == 0) {
+        const int n = odd ? 0 : kInfoNibbles - 1;
+        __stcs(reinterpret_cast<uint2*>(gout) + n, nib_value(n));
+      }
+    }
     __syncwarp();
   }
 }
