@@ -372,12 +372,8 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
   if (!env || !out || ((uintptr_t)out & 7) != 0) return STRAT_BAD_ARG;
   if (!env->P.track) return STRAT_BAD_STATE;
   chain_break(env);
-  static const int smem = kInfoWarps * kInfoWarpWords * 4;
-  if (cudaFuncSetAttribute(k_encode_infostate, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-    return STRAT_CUDA_ERROR;
-  int ctas = (env->P.num_games + kInfoWarps - 1) / kInfoWarps;
-  if (ctas > 2 * env->num_sms) ctas = 2 * env->num_sms;
-  k_encode_infostate<<<ctas, 32 * kInfoWarps, smem, (cudaStream_t)stream>>>(env->P, env->lines, out);
+  int ctas = env->P.num_games < 12 * env->num_sms ? env->P.num_games : 12 * env->num_sms;  // 12 x 17.8 KB of shared memory per SM
+  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out);
   return launch_status();
 }
 

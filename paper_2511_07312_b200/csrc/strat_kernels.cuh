@@ -541,10 +541,6 @@ constexpr int kInfoNibbles = kInfoPlanes * 25;               // 12,175 per game
 constexpr int kInfoAWords = (kInfoPlanes * 100 + 31) / 32 + 1;  // 1,523
 constexpr int kInfoSpecial = 58;                              // planes 12-35, 41-42, 455-486
 constexpr int kInfoBWords = (kInfoSpecial * 100 + 31) / 32 + 1;  // 183
-constexpr int kInfoWarpWords = 2496;  // 1523 + 2*183 + 59 + 512 + 32 = 2492, rounded up to 16 bytes: 9,984 B per warp
-static_assert(kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1 + kTrackWords + kLineWords <= kInfoWarpWords && kInfoWarpWords % 4 == 0 &&
-              (kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1) % 4 == 0, "staging layout");
-constexpr int kInfoWarps = 11;  // 11 x 9,984 B = 107 KB per CTA: two CTAs (22 warps) per SM
 
 __device__ __forceinline__ void info_set(uint32_t* stream, int plane, int cell) {
   int bit = 100 * plane + cell;
@@ -572,149 +568,178 @@ __device__ __forceinline__ uint32_t bf16_of_ratio(long long num, long long den) 
   return ((uint32_t)(e + 127) << 7) | (uint32_t)keep;
 }
 
-__global__ void __launch_bounds__(32 * kInfoWarps) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
-                                                                      uint16_t* __restrict__ out) {
-  extern __shared__ __align__(16) uint32_t s_info[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint32_t* A = s_info + warp * kInfoWarpWords;  // all three streams, then values, tracker block, line
-  uint32_t* Bs = A + kInfoAWords;
-  uint32_t* Cs = Bs + kInfoBWords;
-  uint32_t* val = Cs + kInfoBWords;               // [58] value of B | value of C << 16
-  uint32_t* trk = val + kInfoSpecial + 1;         // 16-byte aligned: (1523 + 366 + 59) = 1948 words
-  uint32_t* sline = trk + kTrackWords;
-  const int stride = gridDim.x * kInfoWarps;
-  for (int gi = blockIdx.x * kInfoWarps + warp; gi < P.num_games; gi += stride) {
-    // ---- stage the game's line and tracker block, clear the streams
-    for (int j = lane; j < (kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1) / 4; j += 32)
-      reinterpret_cast<uint4*>(A)[j] = make_uint4(0u, 0u, 0u, 0u);
-    {
-      const uint4* src = reinterpret_cast<const uint4*>(P.track + (size_t)gi * kTrackWords);
-      uint4* dst = reinterpret_cast<uint4*>(trk);
+// One staged game: the three bit streams and the plane values (what the storer needs).
+struct InfoStage { uint32_t* A; uint32_t* Bs; uint32_t* Cs; uint32_t* val; };
+__device__ __forceinline__ InfoStage info_stage(uint32_t* base) {
+  InfoStage s; s.A = base; s.Bs = base + kInfoAWords; s.Cs = s.Bs + kInfoBWords; s.val = s.Cs + kInfoBWords;
+  return s;
+}
+// builder warp: game gi -> bit streams + values in `st`; trk / sline = its private staging
+__device__ __forceinline__ void info_build(const Params& P, const uint32_t* __restrict__ lines, int gi, const InfoStage& st,
+                                           uint32_t* trk, uint32_t* sline, int lane) {
+  uint32_t* A = st.A; uint32_t* Bs = st.Bs; uint32_t* Cs = st.Cs; uint32_t* val = st.val;
+  // ---- stage the game's line and tracker block, clear the streams
+  for (int j = lane; j < (kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1) / 4; j += 32)
+    reinterpret_cast<uint4*>(A)[j] = make_uint4(0u, 0u, 0u, 0u);
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(P.track + (size_t)gi * kTrackWords);
+    uint4* dst = reinterpret_cast<uint4*>(trk);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) dst[32 * k + lane] = __ldcg(src + 32 * k + lane);
-      sline[lane] = __ldcg(lines + (size_t)gi * kLineWords + lane);
-    }
-    __syncwarp();
-    Game g;
-    unpack_line(sline, g);
-    const int side = (int)(g.ply & 1u);
-    const BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
-    // ---- lane = square: what the piece on it is and has done
+    for (int k = 0; k < 4; ++k) dst[32 * k + lane] = __ldcg(src + 32 * k + lane);
+    sline[lane] = __ldcg(lines + (size_t)gi * kLineWords + lane);
+  }
+  __syncwarp();
+  Game g;
+  unpack_line(sline, g);
+  const int side = (int)(g.ply & 1u);
+  const BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
+  // ---- lane = square: what the piece on it is and has done
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int c = 32 * r + lane;
-      if (c >= 100) break;
-      if (!bb_test(occ, c)) {
-        if (!is_lake_cell(c)) info_set(A, 38, c);                     // empty (R#17: lakes are not squares)
-        continue;
-      }
-      const bool own = bb_test(mine, c) != 0, rev = bb_test(g.rev, c) != 0, mvd = bb_test(g.mvd, c) != 0;
-      const int t = type_at(g, c);
-      if (own) info_set(A, t - 1, c);                                 // 0-11
-      if (rev) info_set(A, (own ? 24 : 12) + t - 1, c);               // a revealed piece: probability 1 (12-35)
-      else info_set(A, own ? 36 : 37, c);                             // hidden pieces
-      if (mvd) info_set(A, own ? 39 : 40, c);                         // pieces that moved
-      const uint32_t r0 = trk[4 * c], r1 = trk[4 * c + 1], r2 = trk[4 * c + 2], r3 = trk[4 * c + 3];
-      const int a = own ? 43 : 76, b = own ? 251 : 303;
-      for (uint32_t w = r0 & 0x3FFFFFu; w; w &= w - 1) info_set(A, a + __ffs((int)w) - 1, c);            // threat, evasion
-      for (uint32_t w = r1 & 0x7FFu; w; w &= w - 1) info_set(A, a + 22 + __ffs((int)w) - 1, c);          // active adjacency
-      for (uint32_t w = (r1 >> 11) & 0x1FFFu; w; w &= w - 1) info_set(A, b + __ffs((int)w) - 1, c);      // protected
-      for (uint32_t w = r2 & 0x3FFFFFFu; w; w &= w - 1) info_set(A, b + 13 + __ffs((int)w) - 1, c);      // against, by
-      for (uint32_t w = r3 & 0x1FFFu; w; w &= w - 1) info_set(A, b + 39 + __ffs((int)w) - 1, c);         // been protected against
-      info_set(A, 355 + (int)((r0 >> 22) & 127u), c);                 // P:606 start square
+  for (int r = 0; r < 4; ++r) {
+    const int c = 32 * r + lane;
+    if (c >= 100) break;
+    if (!bb_test(occ, c)) {
+      if (!is_lake_cell(c)) info_set(A, 38, c);                     // empty (R#17: lakes are not squares)
+      continue;
     }
-    // ---- lane = plane: type posteriors (reading I7), fractions, moves
-    if (lane < 24) {
-      // lanes 0-11: the opponent's pieces as the player sees them (12-23); 12-23: the player's, as the opponent does (24-35)
-      const int t = lane % 12 + 1;
-      const BB hid = bb_andn(lane < 12 ? enemy : mine, g.rev);
-      const BB hid_unmoved = bb_andn(hid, g.mvd), hid_moved = bb_and(hid, g.mvd);
-      const BB imm = bb_and(g.t3, bb_or(g.t2, bb_and(g.t1, g.t0)));
-      const int u = bb_popc(hid_unmoved), m = bb_popc(hid_moved), I = bb_popc(bb_and(hid, imm)), M = u + m - I;
-      const int ct = bb_popc(type_is(g, hid, t));
-      const bool immovable = t == T_FLAG || t == T_BOMB;
-      const int free_unmoved = u - I > 0 ? u - I : 0;
-      uint32_t vu = immovable ? bf16_of_ratio(ct, u) : bf16_of_ratio((long long)free_unmoved * ct, (long long)u * M);
-      uint32_t vm = immovable ? 0u : bf16_of_ratio(ct, M);
-      if (vu) info_place(Bs, lane, hid_unmoved);
-      if (vm) info_place(Cs, lane, hid_moved);
-      val[lane] = vu | (vm << 16);
-    } else if (lane < 26) {
-      BB all; all.w[0] = all.w[1] = all.w[2] = 0xFFFFFFFFu; all.w[3] = 0xFu;
-      uint32_t v = lane == 24 ? bf16_of_ratio((long long)g.ply, (long long)P.ply_cap)
-                              : (P.max_battleless > 0 ? bf16_of_ratio((long long)g.battleless, (long long)P.max_battleless) : 0u);
-      if (v) info_place(Bs, lane, all);
-      val[lane] = v;
+    const bool own = bb_test(mine, c) != 0, rev = bb_test(g.rev, c) != 0, mvd = bb_test(g.mvd, c) != 0;
+    const int t = type_at(g, c);
+    if (own) info_set(A, t - 1, c);                                 // 0-11
+    if (rev) info_set(A, (own ? 24 : 12) + t - 1, c);               // a revealed piece: probability 1 (12-35)
+    else info_set(A, own ? 36 : 37, c);                             // hidden pieces
+    if (mvd) info_set(A, own ? 39 : 40, c);                         // pieces that moved
+    const uint32_t r0 = trk[4 * c], r1 = trk[4 * c + 1], r2 = trk[4 * c + 2], r3 = trk[4 * c + 3];
+    const int a = own ? 43 : 76, b = own ? 251 : 303;
+    for (uint32_t w = r0 & 0x3FFFFFu; w; w &= w - 1) info_set(A, a + __ffs((int)w) - 1, c);            // threat, evasion
+    for (uint32_t w = r1 & 0x7FFu; w; w &= w - 1) info_set(A, a + 22 + __ffs((int)w) - 1, c);          // active adjacency
+    for (uint32_t w = (r1 >> 11) & 0x1FFFu; w; w &= w - 1) info_set(A, b + __ffs((int)w) - 1, c);      // protected
+    for (uint32_t w = r2 & 0x3FFFFFFu; w; w &= w - 1) info_set(A, b + 13 + __ffs((int)w) - 1, c);      // against, by
+    for (uint32_t w = r3 & 0x1FFFu; w; w &= w - 1) info_set(A, b + 39 + __ffs((int)w) - 1, c);         // been protected against
+    info_set(A, 355 + (int)((r0 >> 22) & 127u), c);                 // P:606 start square
+  }
+  // ---- lane = plane: type posteriors (reading I7), fractions, moves
+  if (lane < 24) {
+    // lanes 0-11: the opponent's pieces as the player sees them (12-23); 12-23: the player's, as the opponent does (24-35)
+    const int t = lane % 12 + 1;
+    const BB hid = bb_andn(lane < 12 ? enemy : mine, g.rev);
+    const BB hid_unmoved = bb_andn(hid, g.mvd), hid_moved = bb_and(hid, g.mvd);
+    const BB imm = bb_and(g.t3, bb_or(g.t2, bb_and(g.t1, g.t0)));
+    const int u = bb_popc(hid_unmoved), m = bb_popc(hid_moved), I = bb_popc(bb_and(hid, imm)), M = u + m - I;
+    const int ct = bb_popc(type_is(g, hid, t));
+    const bool immovable = t == T_FLAG || t == T_BOMB;
+    const int free_unmoved = u - I > 0 ? u - I : 0;
+    uint32_t vu = immovable ? bf16_of_ratio(ct, u) : bf16_of_ratio((long long)free_unmoved * ct, (long long)u * M);
+    uint32_t vm = immovable ? 0u : bf16_of_ratio(ct, M);
+    if (vu) info_place(Bs, lane, hid_unmoved);
+    if (vm) info_place(Cs, lane, hid_moved);
+    val[lane] = vu | (vm << 16);
+  } else if (lane < 26) {
+    BB all; all.w[0] = all.w[1] = all.w[2] = 0xFFFFFFFFu; all.w[3] = 0xFu;
+    uint32_t v = lane == 24 ? bf16_of_ratio((long long)g.ply, (long long)P.ply_cap)
+                            : (P.max_battleless > 0 ? bf16_of_ratio((long long)g.battleless, (long long)P.max_battleless) : 0u);
+    if (v) info_place(Bs, lane, all);
+    val[lane] = v;
+  }
+  {  // move j = ply t-1-j: +1.0 on the destination (stream A), -1.0 on the source (stream B)
+    const int slot = (int)((g.ply - 1u - (uint32_t)lane) & 31u);
+    const uint32_t e = (trk[kTrkMoves + (slot >> 1)] >> (16 * (slot & 1))) & 0xFFFFu;
+    if (e != kHistNone) {
+      info_set(A, 455 + lane, (int)(e >> 7));
+      info_set(Bs, 26 + lane, (int)(e & 127u));
     }
-    {  // move j = ply t-1-j: +1.0 on the destination (stream A), -1.0 on the source (stream B)
-      const int slot = (int)((g.ply - 1u - (uint32_t)lane) & 31u);
-      const uint32_t e = (trk[kTrkMoves + (slot >> 1)] >> (16 * (slot & 1))) & 0xFFFFu;
-      if (e != kHistNone) {
-        info_set(A, 455 + lane, (int)(e >> 7));
-        info_set(Bs, 26 + lane, (int)(e & 127u));
-      }
-      val[26 + lane] = 0xBF80u;
+    val[26 + lane] = 0xBF80u;
+  }
+  // ---- captured pieces by start square and causes of death
+  {
+    const int n = min((int)trk[kTrkDeaths], kTrkMaxDeaths);
+    for (int k = lane; k < n; k += 32) {
+      const uint32_t e = trk[kTrkDeathList + k];
+      const int start = (int)(e & 127u), t = (int)((e >> 7) & 15u), owner = (int)((e >> 11) & 1u), sq = (int)((e >> 12) & 127u),
+                cause = (int)((e >> 19) & 7u);
+      const int j = t <= 10 ? t - 1 : t == T_BOMB ? 10 : -1;
+      if (j >= 0) info_set(A, (owner == side ? 109 : 120) + j, start);
+      if (cause) info_set(A, (owner == side ? 131 : 191) + 10 * (cause - 1) + t - 1, sq);
     }
-    // ---- captured pieces by start square and causes of death
-    {
-      const int n = min((int)trk[kTrkDeaths], kTrkMaxDeaths);
-      for (int k = lane; k < n; k += 32) {
-        const uint32_t e = trk[kTrkDeathList + k];
-        const int start = (int)(e & 127u), t = (int)((e >> 7) & 15u), owner = (int)((e >> 11) & 1u), sq = (int)((e >> 12) & 127u),
-                  cause = (int)((e >> 19) & 7u);
-        const int j = t <= 10 ? t - 1 : t == T_BOMB ? 10 : -1;
-        if (j >= 0) info_set(A, (owner == side ? 109 : 120) + j, start);
-        if (cause) info_set(A, (owner == side ? 131 : 191) + 10 * (cause - 1) + t - 1, sq);
-      }
+  }
+}
+// storer warp: the staged game -> 97,400 bytes of bf16
+__device__ __forceinline__ void info_store(uint16_t* __restrict__ out, int gi, const InfoStage& st, int lane) {
+  const uint32_t* A = st.A; const uint32_t* Bs = st.Bs; const uint32_t* Cs = st.Cs; const uint32_t* val = st.val;
+  // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game, two nibbles (16 bytes) per
+  // lane and streaming store.  A game starts 8-byte aligned (odd games at 8 mod 16), so an odd
+  // game's first nibble and an even game's last one go out alone.  Bits -> bf16 in registers:
+  // two bits spread to bit 0 and bit 16, times 0x3F80 (or times the plane's value).
+  const int odd = gi & 1;
+  uint16_t* gout = out + (size_t)gi * (kInfoPlanes * 100);
+  uint4* dst = reinterpret_cast<uint4*>(gout + 4 * odd);  // pair k = nibbles 2k+odd, 2k+odd+1
+  auto spread = [](uint32_t t) { return (t & 1u) | ((t & 2u) << 15); };
+  auto nib_value = [&](int n) -> uint2 {  // any nibble, valued planes included
+    const uint32_t t = (A[n >> 3] >> (4 * (n & 7))) & 15u;
+    uint2 v = make_uint2(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u);
+    const int shift = n < 300 ? -1 : n < 900 ? 300 : n < 1025 ? -1 : n < 1075 ? 1025 - 600 : n < 11375 ? -1 : 11375 - 650;
+    if (shift >= 0) {
+      const int nn = n - shift;  // nibble of the compact valued streams: planes 12-35 -> 0-23, 41-42 -> 24-25, 455-486 -> 26-57
+      const uint32_t vv = val[nn / 25];
+      const uint32_t tb = (Bs[nn >> 3] >> (4 * (nn & 7))) & 15u, tc = (Cs[nn >> 3] >> (4 * (nn & 7))) & 15u;
+      v.x |= spread(tb) * (vv & 0xFFFFu) | spread(tc) * (vv >> 16);
+      v.y |= spread(tb >> 2) * (vv & 0xFFFFu) | spread(tc >> 2) * (vv >> 16);
     }
-    __syncwarp();
-    // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game, two nibbles (16 bytes) per
-    // lane and streaming store.  A game starts 8-byte aligned (odd games at 8 mod 16), so an odd
-    // game's first nibble and an even game's last one go out alone.  Bits -> bf16 in registers:
-    // two bits spread to bit 0 and bit 16, times 0x3F80 (or times the plane's value).
-    const int odd = gi & 1;
-    uint16_t* gout = out + (size_t)gi * (kInfoPlanes * 100);
-    uint4* dst = reinterpret_cast<uint4*>(gout + 4 * odd);  // pair k = nibbles 2k+odd, 2k+odd+1
-    auto spread = [](uint32_t t) { return (t & 1u) | ((t & 2u) << 15); };
-    auto nib_value = [&](int n) -> uint2 {  // any nibble, valued planes included
-      const uint32_t t = (A[n >> 3] >> (4 * (n & 7))) & 15u;
-      uint2 v = make_uint2(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u);
-      const int shift = n < 300 ? -1 : n < 900 ? 300 : n < 1025 ? -1 : n < 1075 ? 1025 - 600 : n < 11375 ? -1 : 11375 - 650;
-      if (shift >= 0) {
-        const int nn = n - shift;  // nibble of the compact valued streams: planes 12-35 -> 0-23, 41-42 -> 24-25, 455-486 -> 26-57
-        const uint32_t vv = val[nn / 25];
-        const uint32_t tb = (Bs[nn >> 3] >> (4 * (nn & 7))) & 15u, tc = (Cs[nn >> 3] >> (4 * (nn & 7))) & 15u;
-        v.x |= spread(tb) * (vv & 0xFFFFu) | spread(tc) * (vv >> 16);
-        v.y |= spread(tb >> 2) * (vv & 0xFFFFu) | spread(tc >> 2) * (vv >> 16);
-      }
-      return v;
-    };
-    auto plain_pairs = [&](int ka, int kb) {  // pairs ka..kb-1 whose two nibbles lie in 0/1 planes
+    return v;
+  };
+  auto plain_pairs = [&](int ka, int kb) {  // pairs ka..kb-1 whose two nibbles lie in 0/1 planes
 #pragma unroll 4
-      for (int k = ka + lane; k < kb; k += 32) {
-        const int bit = 8 * k + 4 * odd;
-        const uint32_t t = __funnelshift_r(A[bit >> 5], A[(bit >> 5) + 1], bit & 31);
-        __stcs(dst + k, make_uint4(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u, spread(t >> 4) * 0x3F80u,
-                                   spread(t >> 6) * 0x3F80u));
-      }
-    };
-    auto any_pairs = [&](int ka, int kb) {
-      for (int k = ka + lane; k < kb; k += 32) {
-        const uint2 lo = nib_value(2 * k + odd), hi = nib_value(2 * k + odd + 1);
-        __stcs(dst + k, make_uint4(lo.x, lo.y, hi.x, hi.y));
-      }
-    };
-    {
-      // plain nibble ranges [0,300) [900,1025) [1075,11375): pair k is plain iff lo <= 2k+odd and 2k+odd+1 < hi
-      const int a0 = 0, b0 = (300 - 2 - odd) / 2 + 1, a1 = (900 - odd + 1) / 2, b1 = (1025 - 2 - odd) / 2 + 1,
-                a2 = (1075 - odd + 1) / 2, b2 = (11375 - 2 - odd) / 2 + 1, pairs = (kInfoNibbles - 1) / 2;
-      plain_pairs(a0, b0); any_pairs(b0, a1); plain_pairs(a1, b1); any_pairs(b1, a2); plain_pairs(a2, b2); any_pairs(b2, pairs);
-      if (lane == 0) {
-        const int n = odd ? 0 : kInfoNibbles - 1;
-        __stcs(reinterpret_cast<uint2*>(gout) + n, nib_value(n));
-      }
+    for (int k = ka + lane; k < kb; k += 32) {
+      const int bit = 8 * k + 4 * odd;
+      const uint32_t t = __funnelshift_r(A[bit >> 5], A[(bit >> 5) + 1], bit & 31);
+      __stcs(dst + k, make_uint4(spread(t) * 0x3F80u, spread(t >> 2) * 0x3F80u, spread(t >> 4) * 0x3F80u,
+                                 spread(t >> 6) * 0x3F80u));
     }
-    __syncwarp();
+  };
+  auto any_pairs = [&](int ka, int kb) {
+    for (int k = ka + lane; k < kb; k += 32) {
+      const uint2 lo = nib_value(2 * k + odd), hi = nib_value(2 * k + odd + 1);
+      __stcs(dst + k, make_uint4(lo.x, lo.y, hi.x, hi.y));
+    }
+  };
+  {
+    // plain nibble ranges [0,300) [900,1025) [1075,11375): pair k is plain iff lo <= 2k+odd and 2k+odd+1 < hi
+    const int a0 = 0, b0 = (300 - 2 - odd) / 2 + 1, a1 = (900 - odd + 1) / 2, b1 = (1025 - 2 - odd) / 2 + 1,
+              a2 = (1075 - odd + 1) / 2, b2 = (11375 - 2 - odd) / 2 + 1, pairs = (kInfoNibbles - 1) / 2;
+    plain_pairs(a0, b0); any_pairs(b0, a1); plain_pairs(a1, b1); any_pairs(b1, a2); plain_pairs(a2, b2); any_pairs(b2, pairs);
+    if (lane == 0) {
+      const int n = odd ? 0 : kInfoNibbles - 1;
+      __stcs(reinterpret_cast<uint2*>(gout) + n, nib_value(n));
+    }
+  }
+}
+
+// CTA = one BUILDER warp + one STORER warp sharing two stages (full / empty mbarriers, as in the
+// fused step): the storer streams game k out while the builder prepares game k+1, so the HBM
+// write stream of an SM (twelve such pairs) never waits for a build.
+constexpr int kInfoStageWords = kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1;  // 1,948
+constexpr int kInfoCtaWords = 2 * kInfoStageWords + kTrackWords + kLineWords;      // 4,440 words = 17,760 B
+static_assert(kInfoStageWords % 4 == 0, "16-byte aligned stages");
+__global__ void __launch_bounds__(64, 12) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
+                                                         uint16_t* __restrict__ out) {
+  __shared__ __align__(16) uint32_t s_info[kInfoCtaWords];
+  __shared__ __align__(8) uint64_t s_full[2], s_empty[2];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) { mbar_init(&s_full[0], 32); mbar_init(&s_full[1], 32); mbar_init(&s_empty[0], 32); mbar_init(&s_empty[1], 32); }
+  __syncthreads();
+  int it = 0;
+  for (int gi = blockIdx.x; gi < P.num_games; gi += gridDim.x, ++it) {
+    const int stage = it & 1, round = it >> 1;
+    const InfoStage st = info_stage(s_info + stage * kInfoStageWords);
+    if (warp == 0) {
+      if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
+      info_build(P, lines, gi, st, s_info + 2 * kInfoStageWords, s_info + 2 * kInfoStageWords + kTrackWords, lane);
+      __syncwarp();
+      mbar_arrive(&s_full[stage]);
+    } else {
+      mbar_wait(&s_full[stage], (uint32_t)round & 1u);
+      info_store(out, gi, st, lane);
+      mbar_arrive(&s_empty[stage]);
+    }
   }
 }
 
