@@ -584,6 +584,52 @@ def run_infostate(args):
     print(json.dumps(line))
 
 
+def run_observe(args):
+    """The data-collection loop with an external policy: a policy kernel
+    picks the actions from the mask (here the uniform sampler stands in for the move network), then
+    strat_step_observe applies them and writes mask + observation of the new state in one pass.  The
+    fused step cannot overlap its neighbours here: it is timed as an isolated launch."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    n = CFG["num_games"]
+    env = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1)
+    mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
+    env.legal_mask(mask)
+    steps = max(1, min(args.steps, 500))
+    for _ in range(max(args.warmup, 3)):
+        env.sample_uniform(mask, act)
+        env.step_observe(act, rew, done, mask, obs)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    for k in range(steps):
+        ev[k][0].record()
+        env.sample_uniform(mask, act)
+        ev[k][1].record()
+        env.step_observe(act, rew, done, mask, obs)
+        ev[k][2].record()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    assert env.check() == 0
+    ms_pol = sorted(e[0].elapsed_time(e[1]) for e in ev)[steps // 2]
+    ms_obs = sorted(e[1].elapsed_time(e[2]) for e in ev)[steps // 2]
+    total = ev[0][0].elapsed_time(ev[-1][2]) / steps
+    line = {
+        "metric": METRIC, "value": n / (total / 1e3), "unit": UNIT, "n_gpus": 1, "steps": steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8", "data": "synthetic",
+        "config": {"workload": CFG["name"] + " with an external policy kernel", "games_per_gpu": n,
+                   "ms_policy_stand_in": ms_pol, "ms_step_observe_median": ms_obs,
+                   "note": "events between the two kernels: strat_step_observe is timed as an isolated launch"},
+        "roofline": dict(_peak_line(ALGO_BYTES_PER_GAME_STEP * n / (ms_obs / 1e3) / 1e9), kernel="k_rollout_step<external>",
+                         algorithmic_bytes_per_game_step=ALGO_BYTES_PER_GAME_STEP),
+        "gpu_launches": 2 * steps, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
 def run_hist(args):
     """The paper's own buffer design on the headline workload: the fused step
     records the 128-byte state of every game and step into a 256-step board-history ring
@@ -640,11 +686,12 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search", "infostate487"],
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search", "infostate487", "observe"],
                     help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
                          "hist = cfg2 recording into the board-history ring + historical queries; "
                          "search = network-free search steps (S3.7) for 256 roots; infostate487 = cfg2 with the S2 trackers kept and the "
-                         "paper's 487-channel information state encoded every step; all 1 GPU")
+                         "paper's 487-channel information state encoded every step; observe = cfg2 driven by an external policy "
+                         "kernel through strat_step_observe; all 1 GPU")
     ap.add_argument("--chase-rule", action="store_true",
                     help="cfg2 with the continuous-chasing rule on (not a BASELINE.json config; the paper's simulator goal "
                          "of ~10 M updates/s is stated with its anti-chasing rules on, PAPER.md:228)")
@@ -668,6 +715,8 @@ def main():
         run_search(args)
     elif args.workload == "infostate487":
         run_infostate(args)
+    elif args.workload == "observe":
+        run_observe(args)
     else:
         run_b200(args)
 

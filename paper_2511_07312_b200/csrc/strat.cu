@@ -176,8 +176,8 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   if (cudaStreamIsCapturing((cudaStream_t)stream, &capture) != cudaSuccess) return STRAT_CUDA_ERROR;
   if (capture != cudaStreamCaptureStatusNone) return STRAT_BAD_STATE;
   const int nb = batches(env->P.num_games);
-  // a launch that follows a policy kernel has the GPU to itself: one more CTA per SM
-  const int per_sm = kExternal ? kWsCtasPerSm + 1 : kWsCtasPerSm;
+  // a launch that follows a policy kernel has the GPU to itself: all six CTA slots of an SM
+  const int per_sm = kExternal ? kWsExternalCtasPerSm : kWsCtasPerSm;
   const int grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(64); lc.dynamicSmemBytes = 0; lc.stream = (cudaStream_t)stream;

@@ -22,6 +22,12 @@ constexpr int kWsStages = 2;
 #define STRAT_WS_CTAS_PER_SM 3
 #endif
 constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
+// strat_step_observe never overlaps its neighbours in the stream (it waits for its actions'
+// producer), so one launch may fill the SM.
+#ifndef STRAT_WS_EXT_CTAS_PER_SM
+#define STRAT_WS_EXT_CTAS_PER_SM 6
+#endif
+constexpr int kWsExternalCtasPerSm = STRAT_WS_EXT_CTAS_PER_SM;
 constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
 
 // Per-batch version flags in global memory: consecutive launches of the fused step overlap
@@ -133,7 +139,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       }
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
       flag_wait(f_state + b, version - 1u, lane);  // the previous launch is done with this batch's state
-      zero_smem16(work, kMaskBytes, lane);
+      if (!kExternal) zero_smem16(work, kMaskBytes, lane);
       Game g;
       int n = 0, cnt[4] = {0, 0, 0, 0};
       if (lane < ng) load_game_global(lines, first + lane, g, hs.lines);
@@ -162,6 +168,8 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         if (lane < ng) store_game_global(lines, first + lane, g);
         flag_set(f_state + b, version, lane);  // state, mask, action, reward, done of this batch are out
       } else {
+        // caller's actions: the observation of the NEW state goes out first (it is 95 % of the bytes and
+        // only needs the step), its legal mask is built afterwards while the store warp is already writing
         if (lane < ng) {
           int a = (int)actions[first + lane];
           StepOut o = step_game<true, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);
@@ -173,21 +181,28 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
         if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
-        else if (rs) {  // the cooperative reset borrows the stage: clear its scratch again afterwards
-          coop_setup(P, first, rs, g, work, lane);
-          zero_smem16(work, kMaskBytes, lane);
-          __syncwarp();
-        }
+        else if (rs) coop_setup(P, first, rs, g, work, lane);  // borrows the stage; the bit streams overwrite it
         if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
-        if (lane < ng) {
-          store_game_global(lines, first + lane, g);
-          if (!g.done)  // of the NEW state
-            legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), work + lane * kMaskWords, cnt,
-                           kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
-        }
+        if (lane < ng) store_game_global(lines, first + lane, g);
         __syncwarp();
-        if (mask) store_mask(mask, first, ng, work, lane);
+        if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
+        __syncwarp();
+        if (lane == 0) s_batch[stage] = b;
+        mbar_arrive(&s_full[stage]);
+        if (mask) {  // mask rows in the OTHER stage's buffer, once the store warp has emptied it
+          const int ostage = (it + 1) % kWsStages, oround = (it + 1) / kWsStages;
+          uint32_t* mwork = s_stage[ostage];
+          if (oround > 0) mbar_wait(&s_empty[ostage], (uint32_t)(oround - 1) & 1u);
+          zero_smem16(mwork, kMaskBytes, lane);
+          __syncwarp();
+          if (lane < ng && !g.done)  // of the NEW state
+            legal_mask_row(g, g.ply & 1u, rules_of<kChase>(P), mwork + lane * kMaskWords, cnt,
+                           kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr);
+          __syncwarp();
+          store_mask(mask, first, ng, mwork, lane);
+        }
         flag_set(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
+        continue;
       }
       __syncwarp();  // the stage becomes bit streams
       if (lane < ng) encode_bits(g, work + lane * kBitsRowWords);
