@@ -398,7 +398,8 @@ def run_cfg3(args):
         a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
         env.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)  # all five arrays written in place
         ring.commit_in_place(n)                                     # host bookkeeping only
-        ring.sample(c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
+        # chained gather: the next fused step still overlaps this one on the device
+        ring.sample_chained(env, c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
 
     for t in range(args.warmup):
         step(t)

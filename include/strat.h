@@ -288,6 +288,16 @@ int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* re
 int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_index, int32_t batch,
                         uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
                         void* stream);
+/* The same gather for a self-play loop that pushes in place (in-place rings only): issued between
+ * two fused steps of `env` on `stream`, it does not separate them - the next strat_rollout_step
+ * still overlaps the previous one on the device.  The gather itself waits for the fused step
+ * issued before it (everything that step pushed is sampled from), and the fused step after the
+ * NEXT gather waits for this one before it reuses ring rows (the ring's spare rows cover exactly
+ * that distance).  One ring serves one environment this way; outputs are valid in stream order
+ * as usual.  STRAT_BAD_STATE on a plain or empty ring. */
+int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, uint64_t draw_index, int32_t batch,
+                                uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
+                                void* stream);
 int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled);
 /* Rows of the live record at ring position p (0 <= p < filled): `row` in the mask / action /
  * reward / done arrays, `obs_row` in the observation array (both = p for a plain ring). */

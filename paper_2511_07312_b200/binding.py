@@ -22,7 +22,7 @@ EXPORTS = [
     "strat_encode_obs", "strat_encode_infostate", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_bytes_in_place", "strat_replay_create_in_place",
-    "strat_replay_locate", "strat_share_chain", "strat_replay_push", "strat_replay_reserve",
+    "strat_replay_locate", "strat_share_chain", "strat_replay_sample_chained", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
     "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
@@ -91,6 +91,7 @@ def lib():
         L.strat_replay_reserve_rows.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.strat_replay_commit.argtypes = [vp, vp, vp, vp, i32, vp]
         L.strat_replay_sample.argtypes = [vp, u64, u64, i32, vp, vp, vp, vp, vp, vp]
+        L.strat_replay_sample_chained.argtypes = [vp, vp, u64, u64, i32, vp, vp, vp, vp, vp, vp]
         L.strat_replay_state.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.strat_determinise.argtypes = [vp, i32, u64, vp, vp]
         L.strat_reduce_returns.argtypes = [vp, vp, i32, vp, vp]
@@ -353,6 +354,12 @@ class Replay:
     def sample(self, seed, draw_index, batch, obs, mask, action, reward, done):
         _chk(lib().strat_replay_sample(self.h, seed, draw_index, batch, _ptr(obs), _ptr(mask), _ptr(action),
                                        _ptr(reward), _ptr(done), _stream()), "strat_replay_sample")
+
+    def sample_chained(self, env, seed, draw_index, batch, obs, mask, action, reward, done):
+        """Gather between two fused steps of `env` without separating them (in-place rings)."""
+        _chk(lib().strat_replay_sample_chained(self.h, env.h, seed, draw_index, batch, _ptr(obs), _ptr(mask), _ptr(action),
+                                               _ptr(reward), _ptr(done), _stream()), "strat_replay_sample_chained")
+        self._env = env
 
     def state(self):
         h, f = C.c_int64(), C.c_int64()

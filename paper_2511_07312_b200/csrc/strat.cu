@@ -105,6 +105,7 @@ struct strat_env {
   uint32_t version;      // fused-step launches so far
   int num_sms;
   strat_history* hist;   // attached board-history ring, or nullptr
+  strat_replay* chained; // ring whose gathers run chained between this environment's fused steps, or nullptr
 };
 
 // Circular buffer of `length` time steps: per step N device lines + N x
@@ -146,6 +147,9 @@ struct strat_replay {
   int64_t total;           // records pushed so far
   int64_t rows, obs_rows;  // physical rows of mask/action/reward/done, of obs
   uint16_t* obs; uint32_t* mask; int16_t* action; int8_t* reward; uint8_t* done;
+  uint32_t* sync;          // 3 device words: two CTA counters and the number of the last finished chained gather
+  uint32_t gathers;        // chained gathers issued so far
+  strat_env* env;          // environment whose fused steps the chained gathers sit between, or nullptr
 };
 
 namespace {
@@ -195,9 +199,12 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   }
   auto kernel = env->P.track ? (env->P.chase_rule ? k_rollout_step<kExternal, true, true> : k_rollout_step<kExternal, false, true>)
                              : (env->P.chase_rule ? k_rollout_step<kExternal, true, false> : k_rollout_step<kExternal, false, false>);
+  // chained gathers: this step may overlap the latest one but not the one before it
+  const uint32_t* gflag = env->chained && env->chained->gathers >= 2 ? env->chained->sync + 2 : nullptr;
+  const uint32_t gnum = env->chained ? env->chained->gathers - 1u : 0u;
   if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
                          env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
-                         hist_slot(env->hist), env->err, wait_prior) != cudaSuccess)
+                         hist_slot(env->hist), env->err, wait_prior, gflag, gnum) != cudaSuccess)
     return STRAT_CUDA_ERROR;
   env->version = version;
   if (env->hist) env->hist->cur += 1;
@@ -246,6 +253,7 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->f_obs = e->f_state + batches(cfg->num_games);
   e->version = 0;
   e->hist = nullptr;
+  e->chained = nullptr;
   uint8_t* extra = reinterpret_cast<uint8_t*>(e->tickets) + align_up(sync_words(cfg->num_games) * 4, 256);
   if (cfg->chase_rule) {
     e->P.movelog = reinterpret_cast<uint16_t*>(extra);
@@ -264,6 +272,7 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
 
 int strat_destroy(strat_env* env) {
   if (env && env->hist) env->hist->env = nullptr;
+  if (env && env->chained) env->chained->env = nullptr;
   chain_break(env);
   delete env;
   return STRAT_OK;
@@ -477,7 +486,7 @@ int replay_layout(int64_t rows, int64_t obs_rows, size_t off[6]) {
   off[2] = p; p += align_up((size_t)rows * 2, 256);
   off[3] = p; p += align_up((size_t)rows, 256);
   off[4] = p; p += align_up((size_t)rows, 256);
-  off[5] = p;
+  off[5] = p;  // 256 bytes of synchronisation words follow
   return STRAT_OK;
 }
 inline bool ring_args_ok(int32_t per_slot, int32_t slots, int32_t block) {
@@ -490,7 +499,7 @@ int replay_make(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, in
   int64_t C = (int64_t)per_slot * slots, rows = C + block, obs_rows = C + 2 * (int64_t)block;
   size_t off[6];
   replay_layout(rows, obs_rows, off);
-  if (bytes < off[5]) return STRAT_BAD_ARG;
+  if (bytes < off[5] + 256) return STRAT_BAD_ARG;
   strat_replay* r = new (std::nothrow) strat_replay;
   if (!r) return STRAT_BAD_ARG;
   uint8_t* b = reinterpret_cast<uint8_t*>(mem_dev);
@@ -499,6 +508,7 @@ int replay_make(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, in
   r->obs = reinterpret_cast<uint16_t*>(b + off[0]); r->mask = reinterpret_cast<uint32_t*>(b + off[1]);
   r->action = reinterpret_cast<int16_t*>(b + off[2]); r->reward = reinterpret_cast<int8_t*>(b + off[3]);
   r->done = b + off[4];
+  r->sync = reinterpret_cast<uint32_t*>(b + off[5]); r->gathers = 0; r->env = nullptr;
   *out = r;
   return STRAT_OK;
 }
@@ -530,7 +540,7 @@ size_t strat_replay_bytes_in_place(int32_t per_slot, int32_t slots, int32_t bloc
   size_t o[6];
   int64_t C = (int64_t)per_slot * slots;
   replay_layout(C + block, C + 2 * (int64_t)block, o);
-  return o[5];
+  return o[5] + 256;
 }
 
 int strat_replay_create(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, strat_replay** out) {
@@ -543,7 +553,11 @@ int strat_replay_create_in_place(void* mem_dev, size_t bytes, int32_t per_slot, 
   return replay_make(mem_dev, bytes, per_slot, slots, block, out);
 }
 
-int strat_replay_destroy(strat_replay* r) { delete r; return STRAT_OK; }
+int strat_replay_destroy(strat_replay* r) {
+  if (r && r->env) r->env->chained = nullptr;
+  delete r;
+  return STRAT_OK;
+}
 
 int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask, const int16_t* action,
                       const int8_t* reward, const uint8_t* done, int32_t n, void* stream) {
@@ -606,10 +620,42 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
   RingMap map;
   map.filled = (uint32_t)r->filled; map.capacity = (uint64_t)r->capacity; map.base = (uint64_t)(r->total - r->filled);
   map.rows = (uint64_t)r->rows; map.obs_rows = (uint64_t)r->obs_rows;
-  k_replay_sample<<<(batch + 3) / 4, 128, 0, (cudaStream_t)stream>>>(
+  GatherChain none = {nullptr, nullptr, 0u};
+  k_replay_sample<false><<<(batch + 3) / 4, 128, 0, (cudaStream_t)stream>>>(
       (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), batch, map,
-      r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done);
+      r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done, none);
   return launch_status();
+}
+
+int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, uint64_t draw_index, int32_t batch,
+                                uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done, void* stream) {
+  if (!r || !env || batch <= 0) return STRAT_BAD_ARG;
+  if (r->filled == 0 || r->rows < r->capacity + 1) return STRAT_BAD_STATE;  // in-place rings only (spare rows)
+  if (r->env && r->env != env) return STRAT_BAD_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (!r->env) {  // first chained gather: clear the synchronisation words, tie the ring to the environment
+    if (cudaMemsetAsync(r->sync, 0, 256, s) != cudaSuccess) return STRAT_CUDA_ERROR;
+    chain_break(env);  // the memset is not a fused step: the next one waits for it
+    r->env = env; env->chained = r; r->gathers = 0;
+  }
+  RingMap map;
+  map.filled = (uint32_t)r->filled; map.capacity = (uint64_t)r->capacity; map.base = (uint64_t)(r->total - r->filled);
+  map.rows = (uint64_t)r->rows; map.obs_rows = (uint64_t)r->obs_rows;
+  r->gathers += 1;
+  GatherChain chain = {r->sync, r->sync + 2, r->gathers};
+  cudaLaunchConfig_t lc = {};
+  int ctas = (batch + 3) / 4 < env->num_sms ? (batch + 3) / 4 : env->num_sms;  // one small CTA per SM: it waits, resident, for the step before it
+  lc.gridDim = dim3((unsigned)ctas); lc.blockDim = dim3(128); lc.dynamicSmemBytes = 0; lc.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  if (cudaLaunchKernelEx(&lc, k_replay_sample<true>, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index,
+                         (uint32_t)(draw_index >> 32), (int)batch, map, (const uint16_t*)r->obs, (const uint32_t*)r->mask,
+                         (const int16_t*)r->action, (const int8_t*)r->reward, (const uint8_t*)r->done, obs, mask, action,
+                         reward, done, chain) != cudaSuccess)
+    return STRAT_CUDA_ERROR;
+  return STRAT_OK;  // deliberately no chain_break: the environment's next fused step continues its chain
 }
 
 int strat_replay_state(const strat_replay* r, int64_t* head, int64_t* filled) {

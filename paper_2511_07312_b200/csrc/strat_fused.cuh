@@ -98,7 +98,8 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
                                                         uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
                                                         uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
-                                                        int* __restrict__ err, int wait_prior) {
+                                                        int* __restrict__ err, int wait_prior,
+                                                        const uint32_t* __restrict__ gather_flag, uint32_t gather_number) {
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   __shared__ __align__(8) uint64_t s_full[kWsStages], s_empty[kWsStages];
@@ -117,6 +118,13 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
   if (warp == 0) {
+    // in a self-play loop with chained gathers (strat_replay_sample_chained): the rows this step writes
+    // may still be read by the gather before the last one; wait until that one has finished (it has)
+    if (gather_flag) {
+      if (lane == 0)
+        while ((int32_t)(ld_acquire(gather_flag) - gather_number) < 0) __nanosleep(64);
+      __syncwarp();
+    }
     // ------------------------------------------------ logic warp (thread per game)
     // batches: the first one is the CTA's own index, the rest are drawn from this launch's
     // ticket counter.  atomicInc wraps to 0 after exactly nbatches draws (nbatches - grid

@@ -358,16 +358,12 @@ __global__ void k_copy(const T* __restrict__ src, T* __restrict__ dst, size_t co
 }
 // Ring position p (index into the capacity-sized ring) -> push-order number -> rows.
 struct RingMap { uint32_t filled; uint64_t capacity, base /* oldest live record's number */, rows, obs_rows; };
-// one warp per batch element: draw the record index, gather the record.
-__global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
-                                                       RingMap map, const uint16_t* __restrict__ r_obs,
-                                                       const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
-                                                       const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
-                                                       uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
-                                                       int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done) {
-  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  int j = blockIdx.x * 4 + warp;
-  if (j >= batch) return;
+__device__ __forceinline__ void replay_gather_one(int j, int lane, uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1,
+                                                  const RingMap& map, const uint16_t* __restrict__ r_obs,
+                                                  const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
+                                                  const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
+                                                  uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
+                                                  int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done) {
   uint32_t o[4];
   philox((uint32_t)(j >> 2), d0, d1, TAG_SAMPLE, k0, k1, o);
   uint32_t u = (j & 3) == 0 ? o[0] : (j & 3) == 1 ? o[1] : (j & 3) == 2 ? o[2] : o[3];
@@ -380,12 +376,51 @@ __global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1,
     for (int q = lane; q < kObsChunks; q += 32) d[q] = __ldcs(s + q);
   }
   if (mask)
-    for (int q = lane; q < kMaskWords; q += 32) mask[(size_t)j * kMaskWords + q] = r_mask[p * kMaskWords + q];
+    for (int q = lane; q < kMaskWords; q += 32) mask[(size_t)j * kMaskWords + q] = __ldcg(r_mask + p * kMaskWords + q);
   if (lane == 0) {
-    if (act) act[j] = r_act[p];
-    if (rew) rew[j] = r_rew[p];
-    if (done) done[j] = r_done[p];
+    if (act) act[j] = __ldcg(r_act + p);
+    if (rew) rew[j] = __ldcg(r_rew + p);
+    if (done) done[j] = __ldcg(r_done + p);
   }
+}
+
+// A gather that sits between two fused steps of a self-play loop without separating them
+// (strat_replay_sample_chained): launched with the programmatic-serialisation attribute, it lets
+// the NEXT fused step start at once (launch_dependents), waits for the step before it as a whole
+// (griddepcontrol.wait: everything that step pushed is visible), gathers, and the CTA that
+// finishes last publishes the gather's number in *done_flag, which the fused step after the next
+// one waits for before it overwrites rows this gather may still read.
+struct GatherChain { uint32_t* counter; uint32_t* done_flag; uint32_t number; };
+// one warp per batch element: draw the record index, gather the record.
+template <bool kChained>
+__global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
+                                                       RingMap map, const uint16_t* __restrict__ r_obs,
+                                                       const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
+                                                       const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
+                                                       uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
+                                                       int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done,
+                                                       GatherChain chain) {
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (kChained) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    for (int j = blockIdx.x * 4 + warp; j < batch; j += gridDim.x * 4)
+      replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence();
+      uint32_t* counter = chain.counter + (chain.number & 1u);  // gathers two apart never overlap (the fused step between waits)
+      if (atomicAdd(counter, 1u) == gridDim.x - 1u) {  // the last CTA: the whole minibatch is out
+        *counter = 0u;
+        __threadfence();
+        atomicMax(chain.done_flag, chain.number);
+      }
+    }
+    return;
+  }
+  int j = blockIdx.x * 4 + warp;
+  if (j >= batch) return;
+  replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done);
 }
 
 // ---- search-shaped batch

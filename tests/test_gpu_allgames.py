@@ -121,7 +121,7 @@ def test_config3_all_262144_games_wrapping_ring_row_by_row():
             a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
             g.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)
             ring.commit_in_place(n)
-            ring.sample(c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)
+            ring.sample_chained(g, c["seed"], t, bs, s_obs, s_mask, s_act, s_rew, s_done)  # as bench.py --workload cfg3
             o.step(want_mask=True, want_obs_before=True, want_boards=(t == steps - 1))
             head, filled = ring.state()
             assert head == ((t + 1) * n) % cap and filled == min((t + 1) * n, cap)

@@ -447,8 +447,8 @@ def test_replay_ring_push_commit_sample_match_oracle():
         assert (int(va[p]), int(vr[p]), int(vd[p])) == (ea, er, ed)
 
 
-@pytest.mark.parametrize("rows_in_place", [False, True])
-def test_replay_in_place_push_equals_oracle_ring_records_and_samples(rows_in_place):
+@pytest.mark.parametrize("rows_in_place,chained", [(False, False), (True, False), (True, True)])
+def test_replay_in_place_push_equals_oracle_ring_records_and_samples(rows_in_place, chained):
     """Self-play loop of config 3 with the fused step writing mask_t (and optionally action_t,
     reward_t, done_t) and obs_{t+1} straight into the ring rows.  After every push, wrapped or
     not, every sampled (obs, mask, action, reward, done) record equals the oracle ring's, and at
@@ -480,7 +480,10 @@ def test_replay_in_place_push_equals_oracle_ring_records_and_samples(rows_in_pla
             g.rollout_step_raw(m_ptr, act, rew, done, o_next)
             ring.commit(act, rew, done)
         assert ring.state() == (oring.head, oring.filled)
-        ring.sample(77, t, batch, s_obs, s_mask, s_act, s_rew, s_done)
+        if chained:  # the gather does not separate consecutive fused steps (strat_replay_sample_chained)
+            ring.sample_chained(g, 77, t, batch, s_obs, s_mask, s_act, s_rew, s_done)
+        else:
+            ring.sample(77, t, batch, s_obs, s_mask, s_act, s_rew, s_done)
         eo, em, ea, er, ed, idx = oring.sample(77, t, batch)
         assert np.array_equal(_obs_np(s_obs), eo) and np.array_equal(_mask_np(s_mask), em), t
         assert np.array_equal(_np(s_act), ea) and np.array_equal(_np(s_rew), er) and np.array_equal(_np(s_done), ed), t
@@ -495,6 +498,50 @@ def test_replay_in_place_push_equals_oracle_ring_records_and_samples(rows_in_pla
     # a plain ring has no spare rows: writing ahead would tear live records, so it is refused
     with pytest.raises(B.StratError):
         B.Replay(32, 8).reserve(n, 1)
+
+
+def test_chained_gathers_back_to_back_equal_a_synchronised_run():
+    """60 self-play steps of 65,536 games with in-place pushes into a ring that wraps every second
+    step and a 2,048-record gather per step, issued back to back with no host synchronisation:
+    fused steps overlap each other THROUGH the chained gathers.  Every gathered minibatch, the ring
+    and the boards equal those of a run that synchronises after every call and uses the plain
+    gather."""
+    n, bs, steps = 65536, 2048, 60
+    kw = dict(variant=0, seed=5, max_plies=90, auto_reset=1)
+    outs = []
+    for chained in (True, False):
+        g = B.Env(n, **kw)
+        ring = B.Replay(n, 2, block=n)  # capacity = 2 blocks
+        so = torch.empty((steps, bs, 4400), dtype=torch.int16, device="cuda")
+        sm = torch.empty((steps, bs, 113), dtype=torch.int32, device="cuda")
+        sa = torch.empty((steps, bs), dtype=torch.int16, device="cuda")
+        sr = torch.empty((steps, bs), dtype=torch.int8, device="cuda")
+        sd = torch.empty((steps, bs), dtype=torch.uint8, device="cuda")
+        o_ptr, _ = ring.reserve(n, 0)
+        B._chk(B.lib().strat_encode_obs(g.h, o_ptr, B._stream()), "encode")
+        for t in range(steps):
+            _, m_ptr = ring.reserve(n, 0)
+            o_next, _ = ring.reserve(n, 1)
+            a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
+            g.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)
+            ring.commit_in_place(n)
+            if chained:
+                ring.sample_chained(g, 9, t, bs, so[t], sm[t], sa[t], sr[t], sd[t])
+            else:
+                ring.sample(9, t, bs, so[t], sm[t], sa[t], sr[t], sd[t])
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        assert g.check() == 0
+        live = [ring.locate(p) for p in (0, n)]
+        v = ring.views()
+        rows = [torch.cat([x[r:r + n] for r, _ in live]) for x in v[1:]] + [torch.cat([v[0][o:o + n] for _, o in live])]
+        outs.append((so, sm, sa, sr, sd, g.get_boards().clone(), rows))
+        del g, ring
+    a, b = outs
+    for x, y in zip(a[:6], b[:6]):
+        assert torch.equal(x, y)
+    for x, y in zip(a[6], b[6]):
+        assert torch.equal(x, y)
 
 
 def test_config3_full_size_ring_zero_copy_and_sample():
