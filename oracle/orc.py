@@ -48,6 +48,8 @@ def lib():
         L.orc_reset_from.argtypes = [vp, vp]
         L.orc_get_boards.argtypes = [vp, vp]
         L.orc_pin_reset_state.argtypes = [vp, vp]
+        L.orc_reset_from_with_plies.argtypes = [vp, vp, vp]
+        L.orc_pin_reset_state_with_plies.argtypes = [vp, vp, vp]
         L.orc_set_setup_pool.argtypes = [vp, vp, C.c_int32]
         L.orc_legal_mask.argtypes = [vp, vp]
         L.orc_sample_uniform.argtypes = [vp, vp, vp]
@@ -112,10 +114,16 @@ class Env:
     def reset(self, seed):
         _chk(lib().orc_reset(self.h, seed), "reset")
 
-    def reset_from(self, boards):
+    def reset_from(self, boards, plies=None):
+        """plies uint8[N][63][2]: the plies that led to each state, most recent first."""
         b = np.ascontiguousarray(boards, dtype=np.uint8)
         assert b.shape == (self.n, LINE)
-        _chk(lib().orc_reset_from(self.h, _p(b)), "reset_from")
+        if plies is None:
+            _chk(lib().orc_reset_from(self.h, _p(b)), "reset_from")
+            return
+        pl = np.ascontiguousarray(plies, dtype=np.uint8)
+        assert pl.shape == (self.n, 63, 2)
+        _chk(lib().orc_reset_from_with_plies(self.h, _p(b), _p(pl)), "reset_from_with_plies")
 
     def set_setup_pool(self, pool):
         """pool uint8[2][K][40] (red setups, blue setups), or None for uniform permutations."""
@@ -126,13 +134,18 @@ class Env:
         assert p.ndim == 3 and p.shape[0] == 2 and p.shape[2] == 40
         _chk(lib().orc_set_setup_pool(self.h, _p(p), p.shape[1]), "set_setup_pool")
 
-    def pin_reset_state(self, boards):
+    def pin_reset_state(self, boards, plies=None):
         """boards uint8[N][128], or None to unpin."""
         if boards is None:
             _chk(lib().orc_pin_reset_state(self.h, None), "pin_reset_state")
             return
         b = np.ascontiguousarray(boards, dtype=np.uint8)
         assert b.shape == (self.n, LINE)
+        if plies is not None:
+            pl = np.ascontiguousarray(plies, dtype=np.uint8)
+            assert pl.shape == (self.n, 63, 2)
+            _chk(lib().orc_pin_reset_state_with_plies(self.h, _p(b), _p(pl)), "pin_reset_state_with_plies")
+            return
         _chk(lib().orc_pin_reset_state(self.h, _p(b)), "pin_reset_state")
 
     def get_boards(self):

@@ -180,6 +180,10 @@ struct Env {
   // "Reset Behaviour and Support for Search": terminated boards restart from a
   // custom non-initial state instead of a fresh setup.  Empty = not pinned.
   std::vector<uint8_t> pin;
+  // "the continuous chasing rule needs to be tested against the history of board states that leads
+  // to the non-initial reset state": per game up to 63 plies (from,to) that led to the
+  // pinned state, most recent first, 0xFF = unknown.  Empty = the 8 plies of the line only.
+  std::vector<uint8_t> pin_plies;
 };
 
 // ---------------------------------------------------------------- geometry
@@ -581,6 +585,7 @@ int effective_ply_cap(const Config& cfg) {
 }
 
 void read_line(const uint8_t* L, Game& gm);  // canonical line -> game (defined below)
+void load_plies(Game& gm, const uint8_t* plies);  // plies that led to a loaded state (defined below)
 
 void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
   Game& gm = e->g[gi];
@@ -629,8 +634,10 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
   }
   for (int j = 7; j >= 1; --j) { gm.hist[j][0] = gm.hist[j - 1][0]; gm.hist[j][1] = gm.hist[j - 1][1]; }
   gm.hist[0][0] = (uint8_t)from; gm.hist[0][1] = (uint8_t)to;
-  gm.log[gm.logn & 63][0] = (uint8_t)from; gm.log[gm.logn & 63][1] = (uint8_t)to;
-  gm.logn += 1;
+  if (cfg.chase_rule) {  // the chasing rule's memory
+    gm.log[gm.logn & 63][0] = (uint8_t)from; gm.log[gm.logn & 63][1] = (uint8_t)to;
+    gm.logn += 1;
+  }
   // 2. mover's bits.
   uint8_t P = gm.cell[from] | B_MOVED;
   if (dist >= 2) P |= B_REVEALED;  // R#10
@@ -675,6 +682,7 @@ void step_game(Env* e, int gi, int action, int8_t* reward, uint8_t* done_out) {
     uint32_t epoch = gm.epoch + 1;
     if (!e->pin.empty()) {  // R#27: the pinned line with the slot's own epoch counter
       read_line(&e->pin[(size_t)gi * kLine], gm);
+      if (!e->pin_plies.empty()) load_plies(gm, &e->pin_plies[(size_t)gi * 126]);
       gm.epoch = epoch;
     } else {
       gm.epoch = epoch;
@@ -744,6 +752,18 @@ void read_line(const uint8_t* L, Game& gm) {
   gm.logn = 0;
   gm.epoch = (uint32_t)L[124] | ((uint32_t)L[125] << 8) | ((uint32_t)L[126] << 16) | ((uint32_t)L[127] << 24);
   rebuild_chains(gm);
+}
+
+// The plies that led to a loaded state, `plies` = [63][2] most recent first: the state then
+// remembers K = the number of leading known plies, exactly as if they had been played here.
+void load_plies(Game& gm, const uint8_t* plies) {
+  int K = 0;
+  while (K < 63 && plies[2 * K] != 0xFF) ++K;
+  gm.logn = K;
+  for (int b = 1; b <= K; ++b) {
+    gm.log[(K - b) & 63][0] = plies[2 * (b - 1)];
+    gm.log[(K - b) & 63][1] = plies[2 * (b - 1) + 1];
+  }
 }
 
 // ---------------------------------------------------------------- C5 encode
@@ -959,12 +979,27 @@ int orc_reset_from(Env* e, const uint8_t* boards) {
   return ORC_OK;
 }
 
+// The same with the plies that led to each state: plies uint8[N][63][2] (from,to), most recent
+// first, 0xFF,0xFF = unknown.  The first 8 repeat the line's own history.
+int orc_reset_from_with_plies(Env* e, const uint8_t* boards, const uint8_t* plies) {
+  int rc = orc_reset_from(e, boards);
+  if (rc != ORC_OK || !plies) return rc;
+  for (int i = 0; i < e->cfg.num_games; ++i) load_plies(e->g[i], plies + (size_t)i * 126);
+  return ORC_OK;
+}
+
 // boards == nullptr unpins.
 int orc_pin_reset_state(Env* e, const uint8_t* boards) {
   if (!e) return ORC_BAD_ARG;
   if (boards) e->pin.assign(boards, boards + (size_t)e->cfg.num_games * kLine);
   else e->pin.clear();
+  e->pin_plies.clear();
   return ORC_OK;
+}
+int orc_pin_reset_state_with_plies(Env* e, const uint8_t* boards, const uint8_t* plies) {
+  int rc = orc_pin_reset_state(e, boards);
+  if (rc == ORC_OK && boards && plies) e->pin_plies.assign(plies, plies + (size_t)e->cfg.num_games * 126);
+  return rc;
 }
 
 int orc_get_boards(const Env* e, uint8_t* boards) {
@@ -1176,8 +1211,7 @@ static int determinise_one(const Game& root, uint64_t seed, uint32_t gidx, Game&
   }
   for (int i = 0; i < k; ++i) gm.cell[freeSq[i]] = (uint8_t)((root.cell[freeSq[i]] & 0xF0) | Tm[i]);
   if (draws) *draws = d;
-  out = gm;
-  out.logn = 0;  // a copied state remembers the 8 plies of its line
+  out = gm;  // the copy remembers what the root remembers (its move log travels with it)
   return ORC_OK;
 }
 

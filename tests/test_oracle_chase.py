@@ -81,6 +81,74 @@ def test_chase_around_a_lake_is_caught_after_one_lap():
         o2 = orc.Env(1, chase_rule=rule)
         o2.reset_from(o.get_boards())
         assert again in _legal(o2)
+        # ... unless the plies that led to it are handed over with it ("the continuous chasing
+        # rule needs to be tested against the history of board states that leads to the non-initial
+        # reset state"): then the lap is remembered across the load
+        played = []
+        for k in range(12):
+            played += [(ring[k % 12], ring[(k + 1) % 12]), (ring[(k + 2) % 12], ring[(k + 3) % 12])]
+        plies = np.full((1, 63, 2), 0xFF, np.uint8)
+        plies[0, :24] = played[::-1]
+        o3 = orc.Env(1, chase_rule=rule)
+        o3.reset_from(o.get_boards(), plies)
+        assert (again in _legal(o3)) == (rule == 0) and back in _legal(o3)
+        assert _legal(o3) == legal
+        # taking 23 plies back reaches the position after the first threat (the one `again` would
+        # recreate); with 22 known plies it is out of reach
+        short = plies.copy(); short[0, 23] = 0xFF
+        o4 = orc.Env(1, chase_rule=rule)
+        o4.reset_from(o.get_boards(), short)
+        assert (again in _legal(o4)) == (rule == 0)
+        short[0, 22] = 0xFF
+        o4 = orc.Env(1, chase_rule=rule)
+        o4.reset_from(o.get_boards(), short)
+        assert again in _legal(o4)
+
+
+def test_chase_memory_survives_pinned_restarts_and_determinised_copies():
+    """P:250 / P:252-254: a game pinned to restart from the lake-lap state restarts with the lap in
+    its memory; a determinised copy of the state (search) inherits it too."""
+    ring = [31, 32, 33, 34, 44, 54, 64, 63, 62, 61, 51, 41]
+
+    def act(a, b):
+        return A(a, {10: 0, 1: 1, -10: 2, -1: 3}[b - a], 1)
+
+    pieces = {ring[0]: W.piece(CAPTAIN, W.RED), ring[2]: W.piece(SERGEANT, W.BLUE), 9: W.piece(FLAG, W.RED),
+              99: W.piece(FLAG, W.BLUE), 8: W.piece(MINER, W.RED), 98: W.piece(MINER, W.BLUE)}
+    o = _env(pieces)
+    played = []
+    for k in range(12):
+        mv = [(ring[k % 12], ring[(k + 1) % 12]), (ring[(k + 2) % 12], ring[(k + 3) % 12])]
+        _play(o, [act(*mv[0]), act(*mv[1])])
+        played += mv
+    lap = o.get_boards()
+    plies = np.full((1, 63, 2), 0xFF, np.uint8)
+    plies[0, :24] = played[::-1]
+    again = act(ring[0], ring[1])
+    # pinned: a short game (ply cap) that restarts from the lap state
+    p = orc.Env(1, chase_rule=1, max_plies=30, auto_reset=1)
+    p.reset_from(lap, plies)
+    p.pin_reset_state(lap, plies)
+    assert again not in _legal(p)
+    for _ in range(6):  # plies 24..29: the cap ends the game, it restarts from the pin
+        p.step(p.sample_uniform(p.legal_mask()))
+    b = p.get_boards()[0]
+    assert b[124] == 1 and (int(b[116]) | (int(b[117]) << 8)) == 24
+    assert again not in _legal(p)                      # the restart remembers the lap
+    q = orc.Env(1, chase_rule=1, max_plies=30, auto_reset=1)
+    q.reset_from(lap, plies)
+    q.pin_reset_state(lap)                             # pinned without its history: forgotten at the restart
+    for _ in range(6):
+        q.step(q.sample_uniform(q.legal_mask()))
+    assert again in _legal(q)
+    # determinised copies (red is the searcher; blue's hidden pieces are re-dealt): the memory travels
+    roots = orc.Env(1, chase_rule=1); roots.reset_from(lap, plies)
+    out = orc.Env(8, chase_rule=1)
+    orc.determinise(roots, 8, 3, out)
+    m = out.legal_mask()
+    for k in range(8):
+        acts = W.mask_to_actions(m[k])
+        assert again not in acts and act(ring[0], ring[11]) in acts
 
 
 def test_chase_state_machine_on_hand_built_plies():
