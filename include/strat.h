@@ -130,6 +130,13 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream);
 /* Load / store all games as canonical lines uint8[N][128] (device pointers).
  * reset_from is the "reset to a non-initial state" of PAPER.md:252-254. */
 int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
+/* The same with the plies that led to each state ("the continuous chasing rule needs
+ * to be tested against the history of board states that leads to the non-initial reset state"):
+ * plies uint8[N][63][2] (device) = (from, to) squares, most recent first, 0xFF,0xFF = unknown; the
+ * leading known ones become the game's move log, as if they had been played here (the first 8
+ * repeat the line's own history).  Without chase_rule nothing remembers plies: same as
+ * strat_reset_from. */
+int strat_reset_from_with_plies(strat_env* env, const uint8_t* boards, const uint8_t* plies, void* stream);
 int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);
 
 /* Customised initial-board distribution ("The distribution from which the initial
@@ -150,6 +157,11 @@ int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, voi
  * caller-owned device memory (16-B aligned) that the library fills and keeps reading until
  * the pin is removed (boards == NULL).  The current state of the games is not touched. */
 int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* boards, void* stream);
+/* The same with the plies that led to each pinned state (layout as in strat_reset_from_with_plies):
+ * a restart from the pin restarts with them in its move log.  pin_logs_dev: N*128
+ * more bytes of caller-owned device memory (16-B aligned), kept like pin_lines_dev. */
+int strat_pin_reset_state_with_plies(strat_env* env, void* pin_lines_dev, void* pin_logs_dev, const uint8_t* boards,
+                                     const uint8_t* plies, void* stream);
 
 /* ComputeLegalActionMask for the acting player (rules PAPER.md:210-212).
  * mask: uint32[N][113].  Finished games get an all-zero mask. */
@@ -325,8 +337,11 @@ int strat_history_destroy(strat_history* h);
 int strat_history_attach(strat_env* env, strat_history* h);
 int strat_history_current_step(const strat_history* h, int64_t* step);
 /* ComputeLegalActionMask(t) / ComputeInfostateTensor(t) / BoardStrs(t): same outputs as the
- * live calls produced (or would have produced) at time step t.  (With chase_rule on, a past
- * state is judged with the 8 plies its line remembers: the move log belongs to the live state.) */
+ * live calls produced (or would have produced) at time step t.  With chase_rule on, the move
+ * log of the past state is rebuilt from the actions the ring still holds (up to 63 plies back to
+ * the game's last restart, beyond it from the pinned log if there is one): identical to the
+ * live mask whenever the ring reaches back as far as the chase did (length >= 63 always does;
+ * plies handed over by strat_reset_from_with_plies before the ring's oldest step are not in it). */
 int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream);
 int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream);
 int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream);
@@ -348,7 +363,8 @@ int strat_history_info(const strat_history* h, int64_t t, int32_t* info, void* s
 int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_applies, uint8_t* unknown,
                         int32_t* terminated_since, void* stream);
 /* Travel back: make the state at time step t the live state of `env` (which need not be the
- * attached one; "efficient capturing of past states", 252-254). */
+ * attached one; "efficient capturing of past states", 252-254).  With chase_rule on in
+ * both, the move log is restored with it, rebuilt as for strat_history_legal_mask. */
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream);
 
 /* ---- search-shaped batch (BASELINE.json configs[4]) ------------------------------- */
@@ -357,7 +373,9 @@ int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, voi
  * Bomb or Flag on a moved piece: each hidden Bomb/Flag draws a free hidden square, redrawing
  * while it is a moved piece's (rejection); the movable types are shuffled over the rest
  * (R22).  More than 4096 draws for one game sets the sticky error of `out` to
- * STRAT_BAD_STATE.  out->num_games must equal roots->num_games * samples_per_root. */
+ * STRAT_BAD_STATE.  out->num_games must equal roots->num_games * samples_per_root.  If both
+ * environments run the chasing rule, each copy inherits its root's move log; so do
+ * the games made by strat_search_expand. */
 int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t seed, strat_env* out,
                       void* stream);
 /* out int32[R][3] = {sum of returns, wins, losses} per root from the searcher's side

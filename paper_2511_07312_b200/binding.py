@@ -18,7 +18,7 @@ OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
-    "strat_reset_from", "strat_get_boards", "strat_pin_reset_state", "strat_set_setup_pool", "strat_legal_mask", "strat_sample_uniform", "strat_step",
+    "strat_reset_from", "strat_reset_from_with_plies", "strat_get_boards", "strat_pin_reset_state", "strat_pin_reset_state_with_plies", "strat_set_setup_pool", "strat_legal_mask", "strat_sample_uniform", "strat_step",
     "strat_encode_obs", "strat_encode_infostate", "strat_rollout_step", "strat_step_observe", "strat_host_scratch_bytes", "strat_rollout_step_host",
     "strat_step_host", "strat_rollout_uniform", "strat_check", "strat_clear_error", "strat_replay_bytes", "strat_replay_layout",
     "strat_replay_create", "strat_replay_destroy", "strat_replay_bytes_in_place", "strat_replay_create_in_place",
@@ -61,6 +61,8 @@ def lib():
         L.strat_reset_from.argtypes = [vp, vp, vp]
         L.strat_get_boards.argtypes = [vp, vp, vp]
         L.strat_pin_reset_state.argtypes = [vp, vp, vp, vp]
+        L.strat_reset_from_with_plies.argtypes = [vp, vp, vp, vp]
+        L.strat_pin_reset_state_with_plies.argtypes = [vp, vp, vp, vp, vp, vp]
         L.strat_set_setup_pool.argtypes = [vp, vp, i32, vp]
         L.strat_legal_mask.argtypes = [vp, vp, vp]
         L.strat_sample_uniform.argtypes = [vp, vp, vp, vp]
@@ -187,9 +189,15 @@ class Env:
     def reset(self, seed):
         _chk(lib().strat_reset(self.h, seed, _stream()), "strat_reset")
 
-    def reset_from(self, boards):
+    def reset_from(self, boards, plies=None):
+        """plies uint8[N][63][2] on the device: the plies that led to each state, most recent first."""
         assert boards.shape == (self.n, LINE)
-        _chk(lib().strat_reset_from(self.h, _ptr(boards, torch.uint8), _stream()), "strat_reset_from")
+        if plies is None:
+            _chk(lib().strat_reset_from(self.h, _ptr(boards, torch.uint8), _stream()), "strat_reset_from")
+            return
+        assert plies.shape == (self.n, 63, 2)
+        _chk(lib().strat_reset_from_with_plies(self.h, _ptr(boards, torch.uint8), _ptr(plies, torch.uint8), _stream()),
+             "strat_reset_from_with_plies")
 
     def set_setup_pool(self, pool):
         """pool uint8[2][K][40] on the device (red setups, blue setups), or None for uniform permutations."""
@@ -201,14 +209,21 @@ class Env:
         _chk(lib().strat_set_setup_pool(self.h, _ptr(pool, torch.uint8), pool.shape[1], _stream()), "strat_set_setup_pool")
         self._pool = pool  # the library reads it until replaced
 
-    def pin_reset_state(self, boards):
-        """boards uint8[N][128] on the device, or None to unpin."""
+    def pin_reset_state(self, boards, plies=None):
+        """boards uint8[N][128] on the device, or None to unpin; plies as in reset_from."""
         if boards is None:
             _chk(lib().strat_pin_reset_state(self.h, None, None, _stream()), "strat_pin_reset_state")
             self._pin = None
             return
         assert boards.shape == (self.n, LINE)
         pin = torch.empty((self.n, LINE), dtype=torch.uint8, device=self.device)
+        if plies is not None:
+            assert plies.shape == (self.n, 63, 2)
+            logs = torch.empty((self.n, 128), dtype=torch.uint8, device=self.device)
+            _chk(lib().strat_pin_reset_state_with_plies(self.h, _ptr(pin), _ptr(logs), _ptr(boards, torch.uint8),
+                                                        _ptr(plies, torch.uint8), _stream()), "strat_pin_reset_state_with_plies")
+            self._pin = (pin, logs)
+            return
         _chk(lib().strat_pin_reset_state(self.h, _ptr(pin), _ptr(boards, torch.uint8), _stream()), "strat_pin_reset_state")
         self._pin = pin  # the library reads it until unpinned
 

@@ -48,7 +48,7 @@ inline Params make_params(const strat_config& c) {
   P.chase_rule = c.chase_rule ? 1 : 0;
   P.movelog = nullptr;
   P.pool = nullptr; P.pool_size = 0;
-  P.pin = nullptr;
+  P.pin = nullptr; P.pin_log = nullptr;
   P.track = nullptr;
   return P;
 }
@@ -114,6 +114,7 @@ struct strat_history {
   int32_t num_games, length;
   int64_t cur;                 // CurrentStep: state updates recorded so far
   uint32_t* lines; int16_t* act; int8_t* rew; uint8_t* done;
+  uint16_t* logs;              // scratch [N][64]: move logs rebuilt for a query about a past state (chasing rule)
   const strat_env* env;        // attached environment (live state = time step cur)
   strat::Params P;             // its rule parameters, kept for queries after a detach
 };
@@ -133,6 +134,11 @@ inline const uint32_t* hist_lines_at(const strat_history* h, int64_t t) {
   if (t == h->cur) return h->env ? h->env->lines : nullptr;
   if (t < 0 || t >= h->cur || t < h->cur - h->length) return nullptr;
   return h->lines + (size_t)(t % h->length) * (size_t)h->num_games * kLineWords;
+}
+inline void hist_rebuild_logs(const strat_history* h, int64_t t, const uint16_t* pin_logs, uint16_t* logs, cudaStream_t s) {
+  int64_t oldest = h->cur - h->length > 0 ? h->cur - h->length : 0;
+  k_rebuild_logs<<<(h->num_games + 255) / 256, 256, 0, s>>>(h->num_games, hist_lines_at(h, t), h->act, h->done, h->length,
+                                                            (long long)t, (long long)oldest, pin_logs, logs);
 }
 }  // namespace
 
@@ -291,12 +297,13 @@ int strat_reset(strat_env* env, uint64_t seed, void* stream) {
   cudaStream_t s = (cudaStream_t)stream;
   env->cfg.seed = seed;
   const uint32_t* pin = env->P.pin;
+  const uint16_t* pin_log = env->P.pin_log;
   uint16_t* movelog = env->P.movelog;
   uint32_t* track = env->P.track;
   const uint8_t* pool = env->P.pool;
   int32_t pool_size = env->P.pool_size;
   env->P = make_params(env->cfg);
-  env->P.pin = pin;
+  env->P.pin = pin; env->P.pin_log = pin_log;
   env->P.movelog = movelog;
   env->P.track = track;
   env->P.pool = pool; env->P.pool_size = pool_size;
@@ -315,6 +322,17 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   return launch_status();
 }
 
+int strat_reset_from_with_plies(strat_env* env, const uint8_t* boards, const uint8_t* plies, void* stream) {
+  if (!env || !boards || !plies) return STRAT_BAD_ARG;
+  chain_break(env);
+  int n = env->P.num_games;
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  if (env->P.movelog)  // without the chasing rule nothing remembers plies
+    k_load_plies<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, plies, env->lines, env->P.movelog);
+  track_restart(env, (cudaStream_t)stream);
+  return launch_status();
+}
+
 int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, void* stream) {
   if (!env) return STRAT_BAD_ARG;
   chain_break(env);
@@ -327,11 +345,24 @@ int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, voi
 int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* boards, void* stream) {
   if (!env) return STRAT_BAD_ARG;
   chain_break(env);
-  if (!boards) { env->P.pin = nullptr; return STRAT_OK; }
+  if (!boards) { env->P.pin = nullptr; env->P.pin_log = nullptr; return STRAT_OK; }
   if (!pin_lines_dev || ((uintptr_t)pin_lines_dev & 15) != 0) return STRAT_BAD_ARG;
   int n = env->P.num_games;
   k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, reinterpret_cast<uint32_t*>(pin_lines_dev));
   env->P.pin = reinterpret_cast<const uint32_t*>(pin_lines_dev);
+  env->P.pin_log = nullptr;
+  return launch_status();
+}
+
+int strat_pin_reset_state_with_plies(strat_env* env, void* pin_lines_dev, void* pin_logs_dev, const uint8_t* boards,
+                                     const uint8_t* plies, void* stream) {
+  if (!env || !boards || !plies || !pin_logs_dev || ((uintptr_t)pin_logs_dev & 15) != 0) return STRAT_BAD_ARG;
+  int rc = strat_pin_reset_state(env, pin_lines_dev, boards, stream);
+  if (rc != STRAT_OK || !env->P.movelog) return rc;
+  int n = env->P.num_games;
+  k_load_plies<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, plies, reinterpret_cast<uint32_t*>(pin_lines_dev),
+                                                                 reinterpret_cast<uint16_t*>(pin_logs_dev));
+  env->P.pin_log = reinterpret_cast<const uint16_t*>(pin_logs_dev);
   return launch_status();
 }
 
@@ -677,7 +708,8 @@ int strat_replay_locate(const strat_replay* r, int64_t p, int64_t* row, int64_t*
 size_t strat_history_bytes(int32_t num_games, int32_t length) {
   if (num_games <= 0 || length <= 0) return 0;
   size_t n = (size_t)num_games, T = (size_t)length;
-  return align_up(T * n * STRAT_LINE_BYTES, 256) + align_up(T * n * 2, 256) + 2 * align_up(T * n, 256);
+  return align_up(T * n * STRAT_LINE_BYTES, 256) + align_up(T * n * 2, 256) + 2 * align_up(T * n, 256) +
+         align_up(n * kLogPlies * 2, 256);
 }
 
 int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, strat_history** out) {
@@ -691,7 +723,8 @@ int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t
   h->lines = reinterpret_cast<uint32_t*>(b); b += align_up(T * n * STRAT_LINE_BYTES, 256);
   h->act = reinterpret_cast<int16_t*>(b); b += align_up(T * n * 2, 256);
   h->rew = reinterpret_cast<int8_t*>(b); b += align_up(T * n, 256);
-  h->done = b;
+  h->done = b; b += align_up(T * n, 256);
+  h->logs = reinterpret_cast<uint16_t*>(b);
   *out = h;
   return STRAT_OK;
 }
@@ -723,7 +756,10 @@ int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, 
   const uint32_t* L = hist_lines_at(h, t);
   if (!L || !mask) return STRAT_BAD_ARG;
   Params P = h->env ? h->env->P : h->P;
-  if (t != h->cur) P.movelog = nullptr;  // a past state is judged with the 8 plies its line remembers
+  if (t != h->cur && P.chase_rule) {  // a past state is judged with the plies the ring still holds
+    hist_rebuild_logs(h, t, P.pin_log, h->logs, (cudaStream_t)stream);
+    P.movelog = h->logs;
+  }
   if (P.chase_rule) k_legal_mask<true><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
   else k_legal_mask<false><<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, mask);
   return launch_status();
@@ -791,7 +827,14 @@ int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, voi
   if (!L || !env || env->P.num_games != h->num_games) return STRAT_BAD_ARG;
   if (L != env->lines) {
     copy_elems<uint32_t>(L, env->lines, (size_t)h->num_games * kLineWords, (cudaStream_t)stream);
-    k_clear_logn<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, env->lines);
+    // the chasing rule's memory travels back too: rebuilt from the ring's actions
+    const Params& Ph = h->env ? h->env->P : h->P;
+    if (env->P.movelog && t == h->cur && Ph.movelog)  // the live state of another environment: its log as it is
+      copy_elems<uint16_t>(Ph.movelog, env->P.movelog, (size_t)h->num_games * kLogPlies, (cudaStream_t)stream);
+    else if (env->P.movelog && Ph.chase_rule)
+      hist_rebuild_logs(h, t, Ph.pin_log, env->P.movelog, (cudaStream_t)stream);
+    else
+      k_clear_logn<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, env->lines);
     track_restart(env, (cudaStream_t)stream);
   }
   return launch_status();
@@ -806,7 +849,7 @@ int strat_determinise(const strat_env* roots, int32_t samples_per_root, uint64_t
   chain_break(out);
   k_determinise<<<batches(out->P.num_games), 32, 0, (cudaStream_t)stream>>>(
       out->P.num_games, samples_per_root, (uint32_t)seed, (uint32_t)(seed >> 32), out->P.game_base, roots->lines,
-      out->lines, out->err);
+      out->lines, roots->P.movelog, out->P.movelog, out->err);
   track_restart(out, (cudaStream_t)stream);
   return launch_status();
 }

@@ -83,6 +83,7 @@ struct Params {  // per-environment constants handed to every kernel by value
   const uint8_t* pool;     // custom setups [2][pool_size][40] type codes (red, then blue), or null (R#30)
   int32_t pool_size;
   const uint32_t* pin;     // device lines [num_games][32] a finished game restarts from, or null (R#27)
+  const uint16_t* pin_log; // [num_games][64] move logs that belong to the pinned lines, or null
   uint32_t* track;         // [num_games][512] trackers of the paper's information state (S2), or null
 };
 
@@ -96,6 +97,17 @@ template <bool kChase> SD int rules_of(const Params& P) {
 // The move log of one game (chasing rule's memory), or null when the environment keeps none.
 SD uint16_t* game_log(const Params& P, uint32_t local_game) {
   return P.movelog ? P.movelog + (size_t)local_game * 64 : nullptr;
+}
+// A state that is copied, pinned or restored takes the plies that led to it along.
+SD void copy_game_log(const uint16_t* src, uint16_t* dst) {
+  const uint32_t* s = reinterpret_cast<const uint32_t*>(src);
+  uint32_t* d = reinterpret_cast<uint32_t*>(dst);
+  STRAT_UNROLL
+  for (int k = 0; k < kLogPlies / 2; k += 4) {
+    uint32_t a, b, c, e;
+    sd_ld128(s + k, a, b, c, e);
+    sd_st128(d + k, a, b, c, e);
+  }
 }
 
 // ------------------------------------------------------------------ 100-bit boards
@@ -816,6 +828,10 @@ SD void reset_game(const Params& P, uint32_t local_game, Game& g) {
     for (int k = 0; k < 32; ++k) W[k] = P.pin[(size_t)local_game * kLineWords + k];
     unpack_line(W, g);
     g.epoch = epoch;
+    // the plies that led to the pinned state restart with it; word 31 of the pinned line counts them
+    uint16_t* glog = game_log(P, local_game);
+    if (glog && P.pin_log) copy_game_log(P.pin_log + (size_t)local_game * kLogPlies, glog);
+    else g.logn = 0;
   } else {
     setup_game(P, local_game, g);
   }
@@ -1251,9 +1267,9 @@ SD uint32_t next_draw(DrawStream& s) {
   ++s.d;
   return k == 0 ? s.o[0] : k == 1 ? s.o[1] : k == 2 ? s.o[2] : s.o[3];
 }
-SD int determinise_game(const Game& root, uint32_t k0, uint32_t k1, uint32_t gidx, Game& out) {
+SD int determinise_game(const Game& root, uint32_t k0, uint32_t k1, uint32_t gidx, bool keep_log, Game& out) {
   out = root;
-  out.logn = 0;  // the copy lives in another environment: it remembers the 8 plies of its line
+  if (!keep_log) out.logn = 0;  // the copy's environment keeps no move log: it remembers the 8 plies of its line
   int searcher = root.ply & 1u;
   BB occ = occupied(root);
   BB enemy = bb_andn(occ, owned_by(root, occ, searcher));

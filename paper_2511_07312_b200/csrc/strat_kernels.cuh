@@ -426,19 +426,22 @@ __global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1,
 // ---- search-shaped batch
 __global__ void __launch_bounds__(32) k_determinise(int num_out, int samples_per_root, uint32_t k0, uint32_t k1, uint32_t out_base,
                                                     const uint32_t* __restrict__ roots, uint32_t* __restrict__ out,
+                                                    const uint16_t* __restrict__ root_logs, uint16_t* __restrict__ out_logs,
                                                     int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   int lane = threadIdx.x, first = blockIdx.x * kBatch;
   int ng = min(kBatch, num_out - first);
+  const bool keep_log = root_logs && out_logs;  // both environments run the chasing rule: its memory is copied too
   if (lane < ng) {
     int G = first + lane, r = G / samples_per_root;
+    if (keep_log) copy_game_log(root_logs + (size_t)r * kLogPlies, out_logs + (size_t)G * kLogPlies);
     uint32_t W[32];
     const uint4* p = reinterpret_cast<const uint4*>(roots + (size_t)r * kLineWords);
 #pragma unroll
     for (int k = 0; k < 8; ++k) { uint4 v = __ldg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
     Game root, g;
     unpack_line(W, root);
-    if (!determinise_game(root, k0, k1, out_base + (uint32_t)G, g)) raise_error(err, STRAT_BAD_STATE);
+    if (!determinise_game(root, k0, k1, out_base + (uint32_t)G, keep_log, g)) raise_error(err, STRAT_BAD_STATE);
     write_game(s_state, lane, g);
   }
   __syncwarp();
@@ -559,6 +562,56 @@ __global__ void __launch_bounds__(128) k_check_pool(const uint8_t* __restrict__ 
 __global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict__ lines) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g < n) lines[(size_t)g * kLineWords + 31] = 0;
+}
+
+// The plies that led to loaded states: plies uint8[n][63][2] (from, to), most recent first,
+// 0xFF = unknown.  K = the leading known ones; ply b back goes to log entry (K - b) mod 64 and word
+// 31 of the line becomes K, exactly what K played plies would have left.
+__global__ void __launch_bounds__(256) k_load_plies(int n, const uint8_t* __restrict__ plies, uint32_t* __restrict__ lines,
+                                                    uint16_t* __restrict__ logs) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  const uint8_t* p = plies + (size_t)g * (2 * (kLogPlies - 1));
+  int K = 0;
+  while (K < kLogPlies - 1 && p[2 * K] != 0xFFu) ++K;
+  uint16_t* glog = logs + (size_t)g * kLogPlies;
+  for (int b = 1; b <= K; ++b)
+    glog[(K - b) & (kLogPlies - 1)] = (uint16_t)((uint32_t)p[2 * (b - 1)] | ((uint32_t)p[2 * (b - 1) + 1] << 7));
+  lines[(size_t)g * kLineWords + 31] = (uint32_t)K;
+}
+
+// Move logs of the states at time step t of a board-history ring, rebuilt from the actions the ring
+// holds (GetPlayedActions): ply b back of game g = the action applied at step t - b, as long
+// as that step is still in the ring and did not end a game.  Entries are placed where the state's
+// own counter (word 31 of its line) expects them; plies older than the last restart come from the
+// pinned log when there is one (same entry index: a restart copies the pinned log), everything
+// else is marked unknown, which ends the chasing rule's walk back.
+__global__ void __launch_bounds__(256) k_rebuild_logs(int n, const uint32_t* __restrict__ lines_t, const int16_t* __restrict__ act,
+                                                      const uint8_t* __restrict__ done, int length, long long t, long long oldest,
+                                                      const uint16_t* __restrict__ pin_logs, uint16_t* __restrict__ logs) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  uint32_t logn = lines_t[(size_t)g * kLineWords + 31];
+  int known = (int)min(logn, (uint32_t)(kLogPlies - 1));
+  uint16_t* glog = logs + (size_t)g * kLogPlies;
+  bool in_game = true;
+  for (int b = 1; b <= known; ++b) {
+    uint32_t idx = (logn - (uint32_t)b) & (uint32_t)(kLogPlies - 1);
+    uint32_t e = kHistNone;
+    if (in_game && t - b >= oldest) {
+      size_t row = (size_t)((t - b) % length) * (size_t)n + (size_t)g;
+      int a = act[row];
+      if ((done[row] & 1u) == 0 && a >= 0) {  // bit 0 = the game ended with this action
+        int from = a / 36, r = a - 36 * from, dir = r / 9, dist = r - 9 * dir + 1;
+        int to = from + (dir == 0 ? 10 : dir == 1 ? 1 : dir == 2 ? -10 : -1) * dist;
+        e = (uint32_t)from | ((uint32_t)to << 7);
+      } else {
+        in_game = false;  // step t - b ended a game: the state at t - b + 1 was a fresh or pinned one
+      }
+    }
+    if (e == kHistNone && !in_game && pin_logs) e = pin_logs[(size_t)g * kLogPlies + idx];
+    glog[idx] = (uint16_t)e;
+  }
 }
 
 // ------------------------------------------------------------------ S2 information state

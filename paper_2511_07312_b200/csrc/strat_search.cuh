@@ -27,6 +27,8 @@ __global__ void __launch_bounds__(32) k_search_expand(Params Pr, Params Po, int 
     for (int k = 0; k < 8; ++k) { uint4 v = __ldg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
     Game root, g;
     unpack_line(W, root);
+    const bool keep_log = kChase && Pr.movelog && Po.movelog;  // the copies inherit the root's chase memory
+    if (keep_log) copy_game_log(game_log(Pr, (uint32_t)r), game_log(Po, (uint32_t)G));
     uint32_t* row = s_mask + lane * kMaskWords;
     int cnt[4] = {0, 0, 0, 0};
     int L = root.done ? 0 : legal_mask_row(root, root.ply & 1u, rules_of<kChase>(Pr), row, cnt,
@@ -35,9 +37,10 @@ __global__ void __launch_bounds__(32) k_search_expand(Params Pr, Params Po, int 
     int used = min(C * L, rollouts);
     if (s >= used) {  // unused slot: the root, frozen
       g = root; g.done = 1; g.reason = 0; g.result = 0;
+      if (!keep_log) g.logn = 0;
     } else {
       int c = s / L, l = s - c * L;
-      if (!determinise_game(root, k0, k1, Po.game_base + (uint32_t)(r * rollouts + c), g)) raise_error(err, STRAT_BAD_STATE);
+      if (!determinise_game(root, k0, k1, Po.game_base + (uint32_t)(r * rollouts + c), keep_log, g)) raise_error(err, STRAT_BAD_STATE);
       step_game<false, false, kChase>(Po, (uint32_t)G, g, pick_rank(row, cnt, l));
     }
     write_game(s_state, lane, g);

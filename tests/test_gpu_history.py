@@ -111,7 +111,7 @@ def test_history_of_overlapped_fused_steps_and_restore():
 
 def test_history_shape_checks():
     assert B.lib().strat_history_bytes(0, 4) == 0 and B.lib().strat_history_bytes(4, 0) == 0
-    assert B.lib().strat_history_bytes(65536, 256) == 65536 * 256 * 132
+    assert B.lib().strat_history_bytes(65536, 256) == 65536 * 256 * 132 + 65536 * 128  # ring + one scratch move log per game
     g = B.Env(64, seed=1)
     h = B.History(32, 4)
     with pytest.raises(B.StratError):
