@@ -128,7 +128,9 @@ int strat_share_chain(strat_env* a, strat_env* b);
 int strat_reset(strat_env* env, uint64_t seed, void* stream);
 
 /* Load / store all games as canonical lines uint8[N][128] (device pointers).
- * reset_from is the "reset to a non-initial state" of PAPER.md:252-254. */
+ * reset_from is the "reset to a non-initial state" of PAPER.md:252-254.  A line that gives one
+ * side more than 8 Scouts (no variant of the game does: BASELINE.json configs[0,1] list 8 and 2)
+ * raises STRAT_BAD_STATE on the sticky error word (strat_check); so does a pinned line. */
 int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
 /* The same with the plies that led to each state ("the continuous chasing rule needs
  * to be tested against the history of board states that leads to the non-initial reset state"):
@@ -145,8 +147,8 @@ int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);
  * (K red setups, then K blue setups; entry i of a red setup goes to cell i, of a blue one to cell
  * 60+i; 0 = empty), caller-owned and read until replaced.  From the next reset / auto-reset on,
  * each side of a fresh game is pool entry bounded(first draw of the side's setup stream, K),
- * independently for the two sides (R30).  A setup with a type code above 12 or with no
- * piece that can ever move raises STRAT_BAD_ARG on the sticky error word (strat_check).
+ * independently for the two sides (R30).  A setup with a type code above 12, with more
+ * than 8 Scouts or with no piece that can ever move raises STRAT_BAD_ARG on the sticky error word (strat_check).
  * pool_dev == NULL: uniform permutations of the multiset again. */
 int strat_set_setup_pool(strat_env* env, const uint8_t* pool_dev, int32_t K, void* stream);
 

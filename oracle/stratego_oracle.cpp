@@ -1321,6 +1321,15 @@ int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, cons
     for (int c = 0; c < kCells; ++c) pieces += per_cell[c] > 0;
     std::vector<double> logit(L);
     double mx = -1e300;
+    // A prior without mass on any legal action of this root says nothing here (KL(pi, pi_theta) is
+    // infinite for every pi, eq. 7 has no maximiser): the root is treated as if no prior were given
+    // (R29).
+    const float* prior = pi_theta;
+    if (prior) {
+      bool any = false;
+      for (int l = 0; l < L; ++l) any = any || prior[(size_t)r * 3600 + list[l]] > 0.0f;
+      if (!any) prior = nullptr;
+    }
     for (int l = 0; l < L; ++l) {
       int sum = 0, cnt = 0;
       for (int64_t s = l; s < used; s += L) {
@@ -1330,7 +1339,7 @@ int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, cons
       }
       double qv = cnt ? (double)sum / cnt : 0.0;
       double rv = 1.0 / ((double)pieces * per_cell[list[l] / 36]);
-      double pv = pi_theta ? (double)pi_theta[(size_t)r * 3600 + list[l]] : 1.0 / L;
+      double pv = prior ? (double)prior[(size_t)r * 3600 + list[l]] : 1.0 / L;
       q[list[l]] = (float)qv; rh[list[l]] = (float)rv;
       logit[l] = (qv + alpha * log(rv) + beta * log(pv)) / (alpha + beta);
       if (logit[l] > mx) mx = logit[l];

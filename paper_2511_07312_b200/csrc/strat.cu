@@ -317,7 +317,7 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream) {
   if (!env || !boards) return STRAT_BAD_ARG;
   chain_break(env);
   int n = env->P.num_games;
-  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines, env->err);
   track_restart(env, (cudaStream_t)stream);
   return launch_status();
 }
@@ -326,7 +326,7 @@ int strat_reset_from_with_plies(strat_env* env, const uint8_t* boards, const uin
   if (!env || !boards || !plies) return STRAT_BAD_ARG;
   chain_break(env);
   int n = env->P.num_games;
-  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines);
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, env->lines, env->err);
   if (env->P.movelog)  // without the chasing rule nothing remembers plies
     k_load_plies<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, plies, env->lines, env->P.movelog);
   track_restart(env, (cudaStream_t)stream);
@@ -348,7 +348,7 @@ int strat_pin_reset_state(strat_env* env, void* pin_lines_dev, const uint8_t* bo
   if (!boards) { env->P.pin = nullptr; env->P.pin_log = nullptr; return STRAT_OK; }
   if (!pin_lines_dev || ((uintptr_t)pin_lines_dev & 15) != 0) return STRAT_BAD_ARG;
   int n = env->P.num_games;
-  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, reinterpret_cast<uint32_t*>(pin_lines_dev));
+  k_import<<<(n + 3) / 4, 128, 0, (cudaStream_t)stream>>>(n, boards, reinterpret_cast<uint32_t*>(pin_lines_dev), env->err);
   env->P.pin = reinterpret_cast<const uint32_t*>(pin_lines_dev);
   env->P.pin_log = nullptr;
   return launch_status();

@@ -68,6 +68,7 @@ constexpr uint32_t TAG_SETUP_RED = 0, TAG_SETUP_BLUE = 1, TAG_ACTION = 2, TAG_SA
 constexpr uint32_t kHistNone = 0x3FFF;
 constexpr int kLogPlies = 64;  // move-log entries per game; the chasing rule looks back 63 plies at most
 constexpr int kMaxBans = 63;
+constexpr int kMaxScouts = 8;  // per side; imports and setup pools with more are refused (count_actions' list)
 
 struct Params {  // per-environment constants handed to every kernel by value
   uint32_t key0, key1;     // Philox key = seed
@@ -671,7 +672,7 @@ SD void count_actions(const Game& g, int side, int rules, uint32_t* scouts, Acti
     for (int d = 0; d < 4; ++d) A.D[i][d] = m.d[d].w[i] & ~sc;
     A.cnt[i] = sd_popc(A.D[i][0]) + sd_popc(A.D[i][1]) + sd_popc(A.D[i][2]) + sd_popc(A.D[i][3]);
     uint32_t ss = (m.d[0].w[i] | m.d[1].w[i] | m.d[2].w[i] | m.d[3].w[i]) & sc;
-    while (ss && ns < 8) {
+    while (ss && ns < kMaxScouts) {
       int bit = sd_ffs(ss) - 1;
       ss &= ss - 1;
       uint32_t below = (1u << bit) - 1u;

@@ -115,12 +115,16 @@ __global__ void __launch_bounds__(32) k_reset(Params P, uint32_t* __restrict__ l
 
 // canonical uint8[N][128] -> device lines.  One warp per game; the seven bit planes are
 // packed with warp ballots (lane = cell within a 32-cell word).
-__global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict__ canon, uint32_t* __restrict__ lines) {
+// A side with more than kMaxScouts Scouts (no variant of the game has that) is refused with BAD_STATE:
+// the mask-free sampler of the on-chip rollouts keeps a list of at most that many (count_actions).
+__global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict__ canon, uint32_t* __restrict__ lines,
+                                                int* __restrict__ err) {
   int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   int g = blockIdx.x * 4 + warp;
   if (g >= n) return;
   uint32_t cw = reinterpret_cast<const uint32_t*>(canon + (size_t)g * 128)[lane];  // bytes 4l..4l+3
   uint32_t mine = 0;
+  int scouts_red = 0, scouts_blue = 0;
 #pragma unroll
   for (int r = 0; r < 4; ++r) {
     int cell = 32 * r + lane;
@@ -128,6 +132,8 @@ __global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict
     uint32_t b = cell < 100 ? (w >> (8 * (cell & 3))) & 0xFFu : 0u;
     uint32_t t = b & 15u;
     bool piece = t >= 1 && t <= 12;
+    scouts_red += __popc(__ballot_sync(0xffffffffu, t == (uint32_t)T_SCOUT && !(b & 16u)));
+    scouts_blue += __popc(__ballot_sync(0xffffffffu, t == (uint32_t)T_SCOUT && (b & 16u)));
 #pragma unroll
     for (int p = 0; p < 7; ++p) {
       bool bit = p < 4 ? (piece && ((t >> p) & 1u)) : (piece && ((b >> p) & 1u));  // p=4 owner(bit4),5 moved,6 revealed
@@ -155,6 +161,7 @@ __global__ void __launch_bounds__(128) k_import(int n, const uint8_t* __restrict
   if (lane == 30) mine = fw >> 16;  // chase ages: canonical bytes 122..123
   if (lane == 31) mine = 0;
   lines[(size_t)g * kLineWords + lane] = mine;
+  if (lane == 0 && (scouts_red > kMaxScouts || scouts_blue > kMaxScouts)) raise_error(err, STRAT_BAD_STATE);
 }
 
 // device lines -> canonical.  One warp per game; lane l < 25 assembles cells 4l..4l+3.
@@ -541,8 +548,8 @@ __global__ void __launch_bounds__(256) k_terminated_since(int n, const uint32_t*
   out[g] = since;
 }
 
-// Validates a custom setup pool (R#30): type codes 0..12 and a side that can move.  One thread
-// per setup; raises BAD_ARG on the environment's sticky error word.
+// Validates a custom setup pool (R#30): type codes 0..12, at most kMaxScouts Scouts and a side that
+// can move.  One thread per setup; raises BAD_ARG on the environment's sticky error word.
 __global__ void __launch_bounds__(128) k_check_pool(const uint8_t* __restrict__ pool, int K, int* __restrict__ err) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= 2 * K) return;
@@ -551,11 +558,13 @@ __global__ void __launch_bounds__(128) k_check_pool(const uint8_t* __restrict__ 
   Game g;
   g.t0 = g.t1 = g.t2 = g.t3 = g.own = g.mvd = g.rev = bb_zero();
   bool ok = true;
+  int scouts = 0;
   for (int k = 0; k < 40; ++k) {
     if (A[k] > 12) ok = false;
     else if (A[k]) put_piece(g, (side ? 60 : 0) + k, A[k], side);
+    scouts += A[k] == T_SCOUT ? 1 : 0;
   }
-  if (!ok || !side_can_ever_move(g, side)) raise_error(err, STRAT_BAD_ARG);
+  if (!ok || scouts > kMaxScouts || !side_can_ever_move(g, side)) raise_error(err, STRAT_BAD_ARG);
 }
 
 // A state copied in from elsewhere (history ring) has no move log here: it remembers 8 plies.

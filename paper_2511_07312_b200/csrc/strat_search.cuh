@@ -102,25 +102,36 @@ __global__ void __launch_bounds__(kPolicyThreads) k_search_policy(Params Pr, int
     if (v) atomicAdd(&s_q[s % L], v);
   }
   __syncthreads();
+  // value sums -> float logits in place; a prior without mass on any legal action of this root says
+  // nothing here (every logit -inf): the root is then treated as if no prior were given (R29)
   float* logit = reinterpret_cast<float*>(s_q);
   float mx = -INFINITY;
-  for (int l = tid; l < L; l += kPolicyThreads) {
-    int a = s_legal[l];
-    int n = (used - l + L - 1) / L;  // games that started with this action
-    float qv = n ? (float)s_q[l] / (float)n : 0.f;
-    float rv = 1.0f / ((float)s_pieces * (float)s_cell[a / 36]);
-    float pv = pi_theta ? pi_theta[(size_t)r * STRAT_NUM_ACTIONS + a] : 1.0f / (float)L;
-    q[a] = qv; rh[a] = rv;
-    float lg = (qv + alpha * logf(rv) + beta * logf(pv)) / (alpha + beta);
-    logit[l] = lg;
-    mx = fmaxf(mx, lg);
-  }
+  for (int pass = 0; pass < 2; ++pass) {
+    const bool uniform = pi_theta == nullptr || pass == 1;
+    mx = -INFINITY;
+    for (int l = tid; l < L; l += kPolicyThreads) {
+      int a = s_legal[l];
+      float qv, rv = 1.0f / ((float)s_pieces * (float)s_cell[a / 36]);
+      if (pass == 0) {
+        int n = (used - l + L - 1) / L;  // games that started with this action
+        qv = n ? (float)s_q[l] / (float)n : 0.f;
+        q[a] = qv; rh[a] = rv;
+      } else {
+        qv = q[a];
+      }
+      float pv = uniform ? 1.0f / (float)L : pi_theta[(size_t)r * STRAT_NUM_ACTIONS + a];
+      float lg = (qv + alpha * logf(rv) + beta * logf(pv)) / (alpha + beta);
+      logit[l] = lg;
+      mx = fmaxf(mx, lg);
+    }
 #pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
-  if ((tid & 31) == 0) s_red[tid >> 5] = mx;
-  __syncthreads();
-  mx = fmaxf(fmaxf(s_red[0], s_red[1]), fmaxf(s_red[2], s_red[3]));
-  __syncthreads();
+    for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+    if ((tid & 31) == 0) s_red[tid >> 5] = mx;
+    __syncthreads();
+    mx = fmaxf(fmaxf(s_red[0], s_red[1]), fmaxf(s_red[2], s_red[3]));
+    __syncthreads();
+    if (mx > -INFINITY || uniform) break;  // the same decision in every thread
+  }
   float z = 0.f;
   for (int l = tid; l < L; l += kPolicyThreads) { float e = expf(logit[l] - mx); logit[l] = e; z += e; }
 #pragma unroll

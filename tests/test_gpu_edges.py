@@ -317,3 +317,33 @@ def test_hand_built_lines_with_arbitrary_histories():
     gr, gd = g.step(_dev(oa))
     assert np.array_equal(_np(gr), orr) and np.array_equal(_np(gd), od)
     assert np.array_equal(_np(g.get_boards()), o.get_boards())
+
+
+def test_more_than_eight_scouts_a_side_are_refused():
+    """The mask-free sampler of the on-chip rollouts lists at most 8 Scouts per side (no variant has more):
+    a loaded or pinned line, or a pool setup, with more is refused instead of silently dropping moves."""
+    pieces = {0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE), 90: W.piece(W.MINER, W.BLUE)}
+    for k in range(9):
+        pieces[10 + k] = W.piece(W.SCOUT, W.RED)
+    nine = W.make_line(pieces)
+    del pieces[18]
+    eight = W.make_line(pieces)
+    g = B.Env(2, seed=1)
+    g.reset_from(torch.from_numpy(np.stack([eight, eight])).cuda())
+    assert g.check() == 0
+    g.reset_from(torch.from_numpy(np.stack([eight, nine])).cuda())
+    assert g.check() == B.BAD_STATE
+    g.clear_error()
+    g.reset_from(torch.from_numpy(np.stack([eight, eight])).cuda())
+    g.pin_reset_state(torch.from_numpy(np.stack([nine, eight])).cuda())
+    assert g.check() == B.BAD_STATE
+    g.clear_error(); g.pin_reset_state(None)
+    pool = np.zeros((2, 1, 40), np.uint8)
+    pool[:, 0, 0] = W.FLAG
+    pool[:, 0, 1:10] = W.SCOUT                       # nine Scouts
+    g.set_setup_pool(torch.from_numpy(pool).cuda())
+    assert g.check() == B.BAD_ARG
+    g.clear_error()
+    pool[:, 0, 9] = W.MINER
+    g.set_setup_pool(torch.from_numpy(pool).cuda())
+    assert g.check() == 0

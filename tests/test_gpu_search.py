@@ -66,3 +66,34 @@ def test_search_argument_errors():
     out = B.Env(2 * 10 + 1, seed=1)
     with pytest.raises(B.StratError):
         B.search_expand(roots, 10, 0, out)  # size mismatch
+
+
+def test_degenerate_priors_match_oracle():
+    """One-hot priors, a prior excluding a legal action, and priors with no mass on any legal action
+    (the root then falls back to "no prior", R29): finite, and equal to the oracle."""
+    R, rollouts = 6, 300
+    rb = _roots(R, 90, seed=5)
+    ro, rg = orc.Env(R, seed=5), B.Env(R, seed=5)
+    ro.reset_from(rb); rg.reset_from(_dev(rb))
+    go, gg = orc.Env(R * rollouts, seed=5), B.Env(R * rollouts, seed=5)
+    orc.search_expand(ro, rollouts, 11, go); B.search_expand(rg, rollouts, 11, gg)
+    for _ in range(30):
+        go.step(go.sample_uniform(go.legal_mask()))
+    gg.rollout_uniform(30)
+    masks = ro.legal_mask()
+    prior = np.zeros((R, 3600), np.float32)
+    legal = [W.mask_to_actions(masks[r]) for r in range(R)]
+    prior[0, legal[0][1]] = 1.0                                   # one-hot on a legal action
+    illegal = sorted(set(range(3600)) - set(legal[1]))
+    prior[1, illegal[:7]] = 1.0 / 7                               # all mass on illegal actions
+    prior[2, legal[2][1:]] = 1.0 / (len(legal[2]) - 1)            # first legal action excluded
+    # root 3: all zeros; roots 4, 5: ordinary priors
+    prior[4, legal[4]] = 1.0 / len(legal[4]); prior[5, legal[5]] = np.linspace(1, 2, len(legal[5]))
+    eq, er, ep = orc.search_policy(ro, go, rollouts, 0.002, 0.02, prior)
+    q, rho, pi = (_np(x) for x in B.search_policy(rg, gg, rollouts, 0.002, 0.02, _dev(prior)))
+    assert np.isfinite(pi).all() and np.isfinite(ep).all()
+    assert np.allclose(q, eq, rtol=1e-6, atol=0) and np.allclose(rho, er, rtol=1e-6, atol=0)
+    assert np.allclose(pi, ep, rtol=1e-4, atol=1e-12)
+    assert pi[0, legal[0][1]] == 1.0 and pi[2, legal[2][0]] == 0.0
+    _, _, pn = (_np(x) for x in B.search_policy(rg, gg, rollouts, 0.002, 0.02, None))
+    assert np.array_equal(pi[1], pn[1]) and np.array_equal(pi[3], pn[3])

@@ -163,3 +163,29 @@ def test_eq8_solves_eq7():
                 d = rng.normal(size=len(legal)) * rng.choice([3e-2, 1e-1, 0.5])
                 p = np.clip(ps + d * ps, 1e-12, None); p /= p.sum()
                 assert objective(p) <= best + 1e-7
+
+
+def test_degenerate_priors():
+    """DESIGN.md R29: a prior of 0 gives probability 0; a prior with its whole mass on one legal action
+    gives that action (beta > 0: any other pi has infinite KL); a prior with no mass on any legal
+    action of a root says nothing there and that root falls back to "no prior" - no NaN anywhere."""
+    pieces = {44: W.piece(W.SERGEANT, W.BLUE), 0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE),
+              10: W.piece(W.BOMB, W.RED)}
+    line = W.make_line(pieces, ply=1)
+    roots = _env_from([line, line, line])
+    legal = W.mask_to_actions(roots.legal_mask()[0])
+    rollouts = 6
+    games = _env_from(list(_games_with_results(line, rollouts, [+1, -1, 0, -1, -1, 0]).get_boards()) * 3)
+    prior = np.zeros((3, 3600), np.float32)
+    prior[0, legal[2]] = 1.0                     # root 0: one-hot on a legal action
+    prior[1, 5] = 1.0                            # root 1: all mass on an illegal action
+    prior[2, legal[0]] = 0.25; prior[2, legal[1]] = 0.75   # root 2: one legal action excluded
+    q, rho, pi = orc.search_policy(roots, games, rollouts, 0.3, 0.2, prior)
+    _, _, pi_none = orc.search_policy(roots, games, rollouts, 0.3, 0.2)
+    assert np.isfinite(pi).all() and np.allclose(pi.sum(axis=1), 1.0, atol=1e-6)
+    assert pi[0, legal[2]] == 1.0
+    assert np.array_equal(pi[1], pi_none[1])
+    assert pi[2, legal[2]] == 0.0 and pi[2, legal[0]] > 0 and pi[2, legal[1]] > 0
+    # root 2 by hand: weights exp(q/(a+b)) * rho^(a/(a+b)) * prior^(b/(a+b)), rho equal for one piece
+    w = np.exp(q[2, legal[:2]].astype(np.float64) / 0.5) * np.array([0.25, 0.75]) ** (0.2 / 0.5)
+    assert np.allclose(pi[2, legal[:2]], w / w.sum(), atol=1e-6)
