@@ -156,6 +156,9 @@ struct strat_replay {
   uint32_t* sync;          // 3 device words: two CTA counters and the number of the last finished chained gather
   uint32_t gathers;        // chained gathers issued so far
   strat_env* env;          // environment whose fused steps the chained gathers sit between, or nullptr
+  // the regular loop (fused step, commit, chained gather, fused step, ...): what the last chained gather saw
+  bool have_last; uint32_t last_version; int64_t last_total;
+  uint32_t vouch_version;  // every fused step up to this version had finished before some earlier gather started
 };
 
 namespace {
@@ -539,7 +542,7 @@ int replay_make(void* mem_dev, size_t bytes, int32_t per_slot, int32_t slots, in
   r->obs = reinterpret_cast<uint16_t*>(b + off[0]); r->mask = reinterpret_cast<uint32_t*>(b + off[1]);
   r->action = reinterpret_cast<int16_t*>(b + off[2]); r->reward = reinterpret_cast<int8_t*>(b + off[3]);
   r->done = b + off[4];
-  r->sync = reinterpret_cast<uint32_t*>(b + off[5]); r->gathers = 0; r->env = nullptr;
+  r->sync = reinterpret_cast<uint32_t*>(b + off[5]); r->gathers = 0; r->env = nullptr; r->have_last = false; r->last_version = 0; r->last_total = 0; r->vouch_version = 0;
   *out = r;
   return STRAT_OK;
 }
@@ -600,6 +603,7 @@ int strat_replay_push(strat_replay* r, const uint16_t* obs, const uint32_t* mask
   push_array<int16_t>(action, r->action, 1, row, r->rows, n, s);
   push_array<int8_t>(reward, r->reward, 1, row, r->rows, n, s);
   push_array<uint8_t>(done, r->done, 1, row, r->rows, n, s);
+  r->have_last = false;  // records copied in by other kernels: the next chained gather waits for the stream
   replay_advance(r, n);
   return launch_status();
 }
@@ -638,6 +642,7 @@ int strat_replay_commit(strat_replay* r, const int16_t* action, const int8_t* re
     copy_elems<int16_t>(action, r->action + row, (size_t)n, s);
     copy_elems<int8_t>(reward, r->reward + row, (size_t)n, s);
     copy_elems<uint8_t>(done, r->done + row, (size_t)n, s);
+    r->have_last = false;  // as in strat_replay_push
   }
   replay_advance(r, n);
   return launch_status();
@@ -651,7 +656,7 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
   RingMap map;
   map.filled = (uint32_t)r->filled; map.capacity = (uint64_t)r->capacity; map.base = (uint64_t)(r->total - r->filled);
   map.rows = (uint64_t)r->rows; map.obs_rows = (uint64_t)r->obs_rows;
-  GatherChain none = {nullptr, nullptr, 0u};
+  GatherChain none = {};
   k_replay_sample<false><<<(batch + 3) / 4, 128, 0, (cudaStream_t)stream>>>(
       (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)draw_index, (uint32_t)(draw_index >> 32), batch, map,
       r->obs, r->mask, r->action, r->reward, r->done, obs, mask, action, reward, done, none);
@@ -667,13 +672,32 @@ int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, 
   if (!r->env) {  // first chained gather: clear the synchronisation words, tie the ring to the environment
     if (cudaMemsetAsync(r->sync, 0, 256, s) != cudaSuccess) return STRAT_CUDA_ERROR;
     chain_break(env);  // the memset is not a fused step: the next one waits for it
-    r->env = env; env->chained = r; r->gathers = 0;
+    r->env = env; env->chained = r; r->gathers = 0; r->have_last = false; r->vouch_version = env->version;
   }
   RingMap map;
   map.filled = (uint32_t)r->filled; map.capacity = (uint64_t)r->capacity; map.base = (uint64_t)(r->total - r->filled);
   map.rows = (uint64_t)r->rows; map.obs_rows = (uint64_t)r->obs_rows;
   r->gathers += 1;
-  GatherChain chain = {r->sync, r->sync + 2, r->gathers};
+  // Regular loop: the operation before this gather was the environment's fused step on this stream, one
+  // step and one block of num_games records after the previous chained gather.  Then every record's
+  // producer is known by version and the gather orders itself by the per-batch flags; anything else
+  // falls back to waiting for the whole stream before it (and vouches for every step so far).
+  const int64_t n = env->P.num_games;
+  bool step_before;
+  {
+    ChainRecord& rec = *env->chain;
+    std::lock_guard<std::mutex> lock(rec.m);
+    step_before = rec.last == env && rec.stream == stream;
+  }
+  const bool regular = step_before && r->have_last && env->version == r->last_version + 1u &&
+                       r->total == r->last_total + n && r->total % n == 0;
+  if (!regular) r->vouch_version = env->version;
+  r->have_last = true; r->last_version = env->version; r->last_total = r->total;
+  GatherChain chain = {};
+  chain.counter = r->sync; chain.done_flag = r->sync + 2; chain.number = r->gathers;
+  chain.use_flags = regular ? 1 : 0; chain.f_state = env->f_state; chain.f_obs = env->f_obs;
+  chain.newest_version = env->version; chain.vouch = r->vouch_version; chain.block = (uint32_t)n;
+  chain.newest_block = (uint64_t)(r->total / n) - 1u;
   cudaLaunchConfig_t lc = {};
   int ctas = (batch + 3) / 4 < env->num_sms ? (batch + 3) / 4 : env->num_sms;  // one small CTA per SM: it waits, resident, for the step before it
   lc.gridDim = dim3((unsigned)ctas); lc.blockDim = dim3(128); lc.dynamicSmemBytes = 0; lc.stream = s;

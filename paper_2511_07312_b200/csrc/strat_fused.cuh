@@ -13,7 +13,10 @@ using namespace strat;
 // stages to bf16 and streams them out.  The two are decoupled by mbarriers, so on every SM
 // observation stores of batch i flow while batch i+1 is still in its (latency-bound) rule
 // logic; with one-warp CTAs all resident warps ran logic, then stores, in lockstep.
-constexpr int kWsStages = 2;
+#ifndef STRAT_WS_STAGES
+#define STRAT_WS_STAGES 2
+#endif
+constexpr int kWsStages = STRAT_WS_STAGES;
 // Resident CTAs per SM of ONE launch.  Two consecutive launches are co-resident (6 CTAs x 35.7 KB
 // of shared memory per SM): the later one trails the earlier one batch by batch, so the HBM
 // write stream never drains between steps.  Measured on B200 at 65,536 games: 2 -> 88.8 us,
@@ -32,14 +35,6 @@ constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B 
 
 // Per-batch version flags in global memory: consecutive launches of the fused step overlap
 // (programmatic dependent launch), ordered batch by batch instead of kernel by kernel.
-__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
-  uint32_t v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
-  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
 // whole warp: returns once *flag == want (lane 0 polls; the barrier orders the other lanes)
 __device__ __forceinline__ void flag_wait(const uint32_t* flag, uint32_t want, int lane) {
   if (lane == 0)
@@ -83,8 +78,9 @@ __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, 
   uint32_t W[32];
   pack_line(g, W);
   uint4* p = reinterpret_cast<uint4*>(lines + (size_t)game * kLineWords);
+  const uint64_t pol = lines_policy();
 #pragma unroll
-  for (int k = 0; k < 8; ++k) __stcg(p + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+  for (int k = 0; k < 8; ++k) st_line16(p + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]), pol);
 }
 
 // kExternal = false (strat_rollout_step): mask of the state -> uniform legal action -> step ->
@@ -163,10 +159,12 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           if (n > 0) a = pick_action(work + lane * kMaskWords, cnt, n, action_draw(P, (uint32_t)(first + lane), g));
           StepOut o = step_game<false, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);  // a comes from this state's mask
           if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
-          if (actions) actions[first + lane] = (int16_t)a;
-          if (reward) reward[first + lane] = (int8_t)o.reward;
-          if (done) done[first + lane] = (uint8_t)o.done;
-          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          // write-once outputs leave the L2 first (evict-first), like the mask rows and the observations:
+          // lines of normal priority in between would be written back out of order, long after their neighbours
+          if (actions) __stcs(actions + first + lane, (int16_t)a);
+          if (reward) __stcs(reward + first + lane, (int8_t)o.reward);
+          if (done) __stcs(done + first + lane, (uint8_t)o.done);
+          if (hs.lines) { __stcs(hs.act + first + lane, (int16_t)a); __stcs(hs.rew + first + lane, (int8_t)o.reward); __stcs(hs.done + first + lane, (uint8_t)o.done); }
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
@@ -182,9 +180,9 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           int a = (int)actions[first + lane];
           StepOut o = step_game<true, true, kChase, kTrack>(P, (uint32_t)(first + lane), g, a);
           if (o.illegal) raise_error(err, STRAT_ILLEGAL_ACTION);
-          reward[first + lane] = (int8_t)o.reward;
-          done[first + lane] = (uint8_t)o.done;
-          if (hs.lines) { hs.act[first + lane] = (int16_t)a; hs.rew[first + lane] = (int8_t)o.reward; hs.done[first + lane] = (uint8_t)o.done; }
+          __stcs(reward + first + lane, (int8_t)o.reward);
+          __stcs(done + first + lane, (uint8_t)o.done);
+          if (hs.lines) { __stcs(hs.act + first + lane, (int16_t)a); __stcs(hs.rew + first + lane, (int8_t)o.reward); __stcs(hs.done + first + lane, (uint8_t)o.done); }
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);

@@ -20,6 +20,42 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 __device__ __forceinline__ void st_stream(uint4* p, uint4 v) { __stcs(p, v); }  // write-once outputs
+// State lines are the only data a step reads back (the next step, 128 B per game): they are kept in the
+// L2 with the evict_last policy, next to gigabytes of evict-first output that stream through it.
+#ifndef STRAT_LINES_POLICY
+#define STRAT_LINES_POLICY 1
+#endif
+__device__ __forceinline__ uint64_t lines_policy() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ uint4 ld_line16(const uint4* p, uint64_t pol) {
+  uint4 v;
+#if STRAT_LINES_POLICY
+  asm volatile("ld.global.cg.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol) : "memory");
+#else
+  v = __ldcg(p);
+#endif
+  return v;
+}
+__device__ __forceinline__ void st_line16(uint4* p, uint4 v, uint64_t pol) {
+#if STRAT_LINES_POLICY
+  asm volatile("st.global.cg.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol) : "memory");
+#else
+  __stcg(p, v);
+#endif
+}
+
+// ------------------------------------------------------------------ flags in global memory (between overlapping launches)
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 // ------------------------------------------------------------------ mbarriers (producer / consumer warps of one CTA)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -81,8 +117,8 @@ __device__ __forceinline__ void store_mask(uint32_t* __restrict__ mask, int firs
   int vec = words >> 2;
   const uint4* s4 = reinterpret_cast<const uint4*>(s_mask);
   uint4* d4 = reinterpret_cast<uint4*>(dst);
-  for (int j = lane; j < vec; j += 32) d4[j] = s4[j];
-  for (int j = (vec << 2) + lane; j < words; j += 32) dst[j] = s_mask[j];
+  for (int j = lane; j < vec; j += 32) st_stream(d4 + j, s4[j]);  // evict-first like the observations
+  for (int j = (vec << 2) + lane; j < words; j += 32) __stcs(dst + j, s_mask[j]);
 }
 // bf16 expansion table: entry e = 8 bf16 values (0x3F80 where bit set), element 0 lowest.
 __device__ __forceinline__ void fill_lut(uint4* lut, int tid, int nthreads) {
@@ -114,12 +150,13 @@ __device__ __forceinline__ void load_game_global(const uint32_t* __restrict__ li
                                                  uint32_t* __restrict__ hist_lines) {
   uint32_t W[32];
   const uint4* p = reinterpret_cast<const uint4*>(lines + (size_t)game * kLineWords);
+  const uint64_t pol = lines_policy();
 #pragma unroll
-  for (int k = 0; k < 8; ++k) { uint4 v = __ldcg(p + k); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
+  for (int k = 0; k < 8; ++k) { uint4 v = ld_line16(p + k, pol); W[4 * k] = v.x; W[4 * k + 1] = v.y; W[4 * k + 2] = v.z; W[4 * k + 3] = v.w; }
   if (hist_lines) {  // board-history ring: the state this step starts from
     uint4* q = reinterpret_cast<uint4*>(hist_lines + (size_t)game * kLineWords);
 #pragma unroll
-    for (int k = 0; k < 8; ++k) __stcg(q + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));
+    for (int k = 0; k < 8; ++k) __stcs(q + k, make_uint4(W[4 * k], W[4 * k + 1], W[4 * k + 2], W[4 * k + 3]));  // write-once: evict-first
   }
   unpack_line(W, g);
 }

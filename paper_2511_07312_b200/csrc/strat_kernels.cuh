@@ -320,8 +320,11 @@ __global__ void __launch_bounds__(32) k_encode_obs(Params P, const uint32_t* __r
 // phase whose length differs from game to game (the Scout ray loops above all), so that the
 // selection and the step run with the warp converged instead of once per group of lanes.
 constexpr int kScoutScratch = 17;  // 16 words per game, odd stride
+#ifndef STRAT_ROLLOUT_MIN_CTAS
+#define STRAT_ROLLOUT_MIN_CTAS 16
+#endif
 template <bool kChase>
-__global__ void __launch_bounds__(32) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
+__global__ void __launch_bounds__(32, STRAT_ROLLOUT_MIN_CTAS) k_rollout_uniform(Params P, uint32_t* __restrict__ lines, int plies, int* __restrict__ err) {
   __shared__ __align__(16) uint8_t s_state[kStateBytes];
   __shared__ uint32_t s_scouts[kBatch * kScoutScratch];
   const uint32_t full = 0xffffffffu;
@@ -365,58 +368,128 @@ __global__ void k_copy(const T* __restrict__ src, T* __restrict__ dst, size_t co
 }
 // Ring position p (index into the capacity-sized ring) -> push-order number -> rows.
 struct RingMap { uint32_t filled; uint64_t capacity, base /* oldest live record's number */, rows, obs_rows; };
-__device__ __forceinline__ void replay_gather_one(int j, int lane, uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1,
+// A gather that sits between two fused steps of a self-play loop without separating them
+// (strat_replay_sample_chained).  It is launched with the programmatic-serialisation attribute and lets
+// the NEXT fused step start at once (launch_dependents).  In the regular loop (step, commit, gather,
+// step, ...) it does not wait for the step before it as a whole either: a record pushed by the step
+// with version v, game g, is complete once that step has published batch g/32 (f_state >= v: mask,
+// action, reward, done) and the step before it the batch's observation (f_obs >= v - 1), so only the
+// few records of the newest blocks wait, each for its own batch, and the gather runs alongside the
+// step that feeds it.  Records of steps up to `vouch` are known to be complete (an earlier gather
+// waited for that grid).  Otherwise (use_flags = 0) it waits for everything before it in the stream.
+// The CTA that finishes last publishes the gather's number in *done_flag: the next gather waits for
+// it before it overwrites the minibatch, the fused step after the next one before it overwrites rows
+// this gather may still read.
+struct GatherChain {
+  uint32_t* counter; uint32_t* done_flag; uint32_t number;
+  int use_flags; const uint32_t* f_state; const uint32_t* f_obs;
+  uint32_t newest_version, vouch; uint32_t block; uint64_t newest_block;
+};
+// Returns false (nothing copied) if the record's producer has not published it yet and may_defer is set.
+__device__ __forceinline__ bool replay_gather_one(int j, int lane, uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1,
                                                   const RingMap& map, const uint16_t* __restrict__ r_obs,
                                                   const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
                                                   const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
                                                   uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
-                                                  int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done) {
+                                                  int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done,
+                                                  const GatherChain& chain, bool may_defer = false) {
   uint32_t o[4];
   philox((uint32_t)(j >> 2), d0, d1, TAG_SAMPLE, k0, k1, o);
   uint32_t u = (j & 3) == 0 ? o[0] : (j & 3) == 1 ? o[1] : (j & 3) == 2 ? o[2] : o[3];
   uint64_t idx = bounded(u, map.filled);
   uint64_t seq = map.base + (idx + map.capacity - map.base % map.capacity) % map.capacity;
   size_t p = (size_t)(seq % map.rows), po = (size_t)(seq % map.obs_rows);
+  if (chain.use_flags) {
+    const uint64_t blk = seq / chain.block;
+    const uint32_t need = chain.newest_version - (uint32_t)(chain.newest_block - blk);  // version of the step that pushed it
+    if ((int32_t)(need - chain.vouch) > 0) {
+      const uint32_t b = (uint32_t)(seq - blk * chain.block) / (uint32_t)kBatch;
+      int ready = 1;
+      if (lane == 0) {
+        if (may_defer) {
+          ready = (int32_t)(ld_acquire(chain.f_state + b) - need) >= 0 && (int32_t)(ld_acquire(chain.f_obs + b) - (need - 1u)) >= 0;
+        } else {
+          while ((int32_t)(ld_acquire(chain.f_state + b) - need) < 0) __nanosleep(64);
+          while ((int32_t)(ld_acquire(chain.f_obs + b) - (need - 1u)) < 0) __nanosleep(64);
+        }
+      }
+      ready = __shfl_sync(0xffffffffu, ready, 0);  // also orders the other lanes behind lane 0's acquire
+      if (!ready) return false;
+    }
+  }
+  // all loads of the record are issued before the first store: a warp that copied chunk by chunk would
+  // pay one trip to HBM (microseconds while the fused steps saturate it) for every 512 bytes
+  uint32_t mw[4];
+  if (mask) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) mw[k] = 32 * k + lane < kMaskWords ? __ldcg(r_mask + p * kMaskWords + 32 * k + lane) : 0u;
+  }
   if (obs) {
     const uint4* s = reinterpret_cast<const uint4*>(r_obs + po * STRAT_OBS_ELEMS);
     uint4* d = reinterpret_cast<uint4*>(obs + (size_t)j * STRAT_OBS_ELEMS);
-    for (int q = lane; q < kObsChunks; q += 32) d[q] = __ldcs(s + q);
+    uint4 v[6];
+#pragma unroll
+    for (int h = 0; h < 3; ++h) {  // 550 chunks = 3 x 6 x 32 - 26
+#pragma unroll
+      for (int k = 0; k < 6; ++k) {
+        int q = 32 * (6 * h + k) + lane;
+        if (q < kObsChunks) v[k] = __ldcs(s + q);
+      }
+#pragma unroll
+      for (int k = 0; k < 6; ++k) {
+        int q = 32 * (6 * h + k) + lane;
+        if (q < kObsChunks) __stcs(d + q, v[k]);  // evict-first: normal-priority lines between the streaming output
+                                                    // of the fused steps get written back out of order (measured)
+      }
+    }
   }
-  if (mask)
-    for (int q = lane; q < kMaskWords; q += 32) mask[(size_t)j * kMaskWords + q] = __ldcg(r_mask + p * kMaskWords + q);
+  if (mask) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (32 * k + lane < kMaskWords) mask[(size_t)j * kMaskWords + 32 * k + lane] = mw[k];
+  }
   if (lane == 0) {
     if (act) act[j] = __ldcg(r_act + p);
     if (rew) rew[j] = __ldcg(r_rew + p);
     if (done) done[j] = __ldcg(r_done + p);
   }
+  return true;
 }
 
-// A gather that sits between two fused steps of a self-play loop without separating them
-// (strat_replay_sample_chained): launched with the programmatic-serialisation attribute, it lets
-// the NEXT fused step start at once (launch_dependents), waits for the step before it as a whole
-// (griddepcontrol.wait: everything that step pushed is visible), gathers, and the CTA that
-// finishes last publishes the gather's number in *done_flag, which the fused step after the next
-// one waits for before it overwrites rows this gather may still read.
-struct GatherChain { uint32_t* counter; uint32_t* done_flag; uint32_t number; };
 // one warp per batch element: draw the record index, gather the record.
 template <bool kChained>
-__global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
-                                                       RingMap map, const uint16_t* __restrict__ r_obs,
-                                                       const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
-                                                       const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
-                                                       uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
-                                                       int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done,
-                                                       GatherChain chain) {
+__global__ void __launch_bounds__(128, 8) k_replay_sample(uint32_t k0, uint32_t k1, uint32_t d0, uint32_t d1, int batch,
+                                                          RingMap map, const uint16_t* __restrict__ r_obs,
+                                                          const uint32_t* __restrict__ r_mask, const int16_t* __restrict__ r_act,
+                                                          const int8_t* __restrict__ r_rew, const uint8_t* __restrict__ r_done,
+                                                          uint16_t* __restrict__ obs, uint32_t* __restrict__ mask,
+                                                          int16_t* __restrict__ act, int8_t* __restrict__ rew, uint8_t* __restrict__ done,
+                                                          GatherChain chain) {
   int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (kChained) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    for (int j = blockIdx.x * 4 + warp; j < batch; j += gridDim.x * 4)
-      replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done);
+    if (!chain.use_flags) asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0)  // the minibatch buffers are the previous gather's too
+      while ((int32_t)(ld_acquire(chain.done_flag) - (chain.number - 1u)) < 0) __nanosleep(64);
+    __syncthreads();
+    // records whose producer (the fused step running alongside) has not published them yet are taken
+    // last, so that what is left to do when that step ends is one record's copy, not a warp's whole share
+    uint32_t deferred = 0u;
+    int slot = 0;
+    for (int j = blockIdx.x * 4 + warp; j < batch; j += gridDim.x * 4, ++slot)
+      if (!replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done,
+                             chain, slot < 32))
+        deferred |= 1u << slot;
+    slot = 0;
+    for (int j = blockIdx.x * 4 + warp; j < batch && deferred; j += gridDim.x * 4, ++slot)
+      if ((deferred >> slot) & 1u) {
+        deferred &= ~(1u << slot);
+        replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done, chain);
+      }
     __syncthreads();
     if (threadIdx.x == 0) {
       __threadfence();
-      uint32_t* counter = chain.counter + (chain.number & 1u);  // gathers two apart never overlap (the fused step between waits)
+      uint32_t* counter = chain.counter + (chain.number & 1u);  // consecutive gathers never overlap (the wait above)
       if (atomicAdd(counter, 1u) == gridDim.x - 1u) {  // the last CTA: the whole minibatch is out
         *counter = 0u;
         __threadfence();
@@ -427,7 +500,7 @@ __global__ void __launch_bounds__(128) k_replay_sample(uint32_t k0, uint32_t k1,
   }
   int j = blockIdx.x * 4 + warp;
   if (j >= batch) return;
-  replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done);
+  replay_gather_one(j, lane, k0, k1, d0, d1, map, r_obs, r_mask, r_act, r_rew, r_done, obs, mask, act, rew, done, chain);
 }
 
 // ---- search-shaped batch
