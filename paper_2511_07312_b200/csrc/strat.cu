@@ -58,7 +58,8 @@ inline int batches(int n) { return (n + kBatch - 1) / kBatch; }
 // flight holds at least one of the <= 32 x SMs resident CTA slots, so far fewer than kTicketRing
 // launches are ever in flight and two launches never share a ticket counter.
 constexpr int kTicketRing = 8192;
-inline size_t sync_words(int n) { return (size_t)kTicketRing + 2 * (size_t)batches(n); }
+constexpr int kOtherTickets = 64;  // self-resetting work counters of the other persistent kernels (word 0: strat_encode_infostate)
+inline size_t sync_words(int n) { return (size_t)kTicketRing + 2 * (size_t)batches(n) + kOtherTickets; }
 
 template <typename T>
 void copy_elems(const T* src, T* dst, size_t count, cudaStream_t s) {
@@ -189,7 +190,7 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   if (cudaStreamIsCapturing((cudaStream_t)stream, &capture) != cudaSuccess) return STRAT_CUDA_ERROR;
   if (capture != cudaStreamCaptureStatusNone) return STRAT_BAD_STATE;
   const int nb = batches(env->P.num_games);
-  // a launch that follows a policy kernel has the GPU to itself: all six CTA slots of an SM
+  // a launch that follows a policy kernel has the GPU to itself (kWsExternalCtasPerSm says how it uses it)
   const int per_sm = kExternal ? kWsExternalCtasPerSm : kWsCtasPerSm;
   const int grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
   cudaLaunchConfig_t lc = {};
@@ -203,8 +204,10 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   {
     ChainRecord& rec = *env->chain;
     std::lock_guard<std::mutex> lock(rec.m);
+    // a step with caller-provided actions publishes nothing while it runs (flag_set<false>): whatever
+    // follows it waits for its grid as a whole, so its own environment's chain restarts after it
     wait_prior = kExternal || !(rec.last == env && rec.stream == stream);
-    rec.last = env; rec.stream = stream;
+    rec.last = kExternal ? nullptr : env; rec.stream = kExternal ? nullptr : stream;
   }
   auto kernel = env->P.track ? (env->P.chase_rule ? k_rollout_step<kExternal, true, true> : k_rollout_step<kExternal, false, true>)
                              : (env->P.chase_rule ? k_rollout_step<kExternal, true, false> : k_rollout_step<kExternal, false, false>);
@@ -416,7 +419,7 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
   if (!env->P.track) return STRAT_BAD_STATE;
   chain_break(env);
   int ctas = env->P.num_games < 12 * env->num_sms ? env->P.num_games : 12 * env->num_sms;  // 12 x 17.8 KB of shared memory per SM
-  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out);
+  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out, env->f_obs + batches(env->P.num_games));
   return launch_status();
 }
 

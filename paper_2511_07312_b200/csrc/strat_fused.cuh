@@ -25,10 +25,14 @@ constexpr int kWsStages = STRAT_WS_STAGES;
 #define STRAT_WS_CTAS_PER_SM 3
 #endif
 constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
-// strat_step_observe never overlaps its neighbours in the stream (it waits for its actions'
-// producer), so one launch may fill the SM.
+// strat_step_observe never overlaps its neighbours in the stream (it waits for its actions' producer).
+// With ~14 batches per SM at 65,536 games the launch is short: what counts is how evenly the SMs finish,
+// and the fewer batches an SM has drawn ahead of its stores the more evenly they do (measured at 65,536
+// games, isolated launch: 2 -> 102.5 us, 3 -> 102.4 us, 4 -> 104.5 us, 6 -> 109.6 us; at 262,144: 3 -> 389 us).
+// Tried and dropped: the logic warp helping to store the CTA's last batch (drawing the next ticket before
+// the hand-over, to know which batch is the last, unbalances the SMs by more than the help gains: 106.5 us).
 #ifndef STRAT_WS_EXT_CTAS_PER_SM
-#define STRAT_WS_EXT_CTAS_PER_SM 6
+#define STRAT_WS_EXT_CTAS_PER_SM 3
 #endif
 constexpr int kWsExternalCtasPerSm = STRAT_WS_EXT_CTAS_PER_SM;
 constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
@@ -41,10 +45,18 @@ __device__ __forceinline__ void flag_wait(const uint32_t* flag, uint32_t want, i
     while (ld_acquire(flag) != want) __nanosleep(64);
   __syncwarp();
 }
-// whole warp: publish this warp's prior global writes, then set the flag
+// whole warp: publish this warp's prior global writes, then set the flag.  kPublish = false: nobody reads the
+// flag while this grid runs (strat_step_observe: the launches around it wait for whole grids), so it is only
+// kept up to date for later launches and the warp does not wait for its stores to drain - with a handful of
+// batches per CTA all store warps would do that at the same moments and the write stream would stall there
+// (measured: the number of batches being stored dropped to a third every ~25 us).
+template <bool kPublish = true>
 __device__ __forceinline__ void flag_set(uint32_t* flag, uint32_t v, int lane) {
   __syncwarp();
-  if (lane == 0) { __threadfence(); st_release(flag, v); }
+  if (lane == 0) {
+    if (kPublish) { __threadfence(); st_release(flag, v); }
+    else asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(v) : "memory");
+  }
 }
 // nibble -> 4 bf16 (0x3F80 where the bit is set); 16 entries x 8 B = one bank row, so the
 // two LDS.64 per 16-byte chunk never conflict.
@@ -207,7 +219,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
           __syncwarp();
           store_mask(mask, first, ng, mwork, lane);
         }
-        flag_set(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
+        flag_set<false>(f_state + b, version, lane);  // state, reward, done, mask of this batch are out
         continue;
       }
       __syncwarp();  // the stage becomes bit streams
@@ -226,7 +238,7 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
       const int first = b * kBatch, ng = min(kBatch, P.num_games - first);
       flag_wait(f_obs + b, version - 1u, lane);  // write-after-write on a reused obs buffer
       expand_obs16(obs, first, ng, s_stage[stage], s_lut, lane);
-      flag_set(f_obs + b, version, lane);
+      flag_set<!kExternal>(f_obs + b, version, lane);
       mbar_arrive(&s_empty[stage]);
     }
   }

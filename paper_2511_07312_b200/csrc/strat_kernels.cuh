@@ -885,28 +885,46 @@ __device__ __forceinline__ void info_store(uint16_t* __restrict__ out, int gi, c
 
 // CTA = one BUILDER warp + one STORER warp sharing two stages (full / empty mbarriers, as in the
 // fused step): the storer streams game k out while the builder prepares game k+1, so the HBM
-// write stream of an SM (twelve such pairs) never waits for a build.
+// write stream of an SM (twelve such pairs) never waits for a build.  Games are handed out by a
+// ticket counter, not by a fixed stride: the SMs do not all drain their stores at the same rate, and a
+// persistent grid with equal shares ends on its slowest SM (plain streaming stores on this GPU: 6.2 TB/s
+// with equal shares, 7.2-7.4 TB/s when every CTA fetches its next piece of work as it finishes one).
+// The counter cleans up after itself like the fused step's: atomicInc wraps to 0 after exactly
+// num_games draws (num_games - grid successful ones and one failing draw per CTA).
 constexpr int kInfoStageWords = kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1;  // 1,948
 constexpr int kInfoCtaWords = 2 * kInfoStageWords + kTrackWords + kLineWords;      // 4,440 words = 17,760 B
 static_assert(kInfoStageWords % 4 == 0, "16-byte aligned stages");
 __global__ void __launch_bounds__(64, 12) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
-                                                         uint16_t* __restrict__ out) {
+                                                         uint16_t* __restrict__ out, uint32_t* __restrict__ ticket) {
   __shared__ __align__(16) uint32_t s_info[kInfoCtaWords];
   __shared__ __align__(8) uint64_t s_full[2], s_empty[2];
+  __shared__ int s_game[2];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) { mbar_init(&s_full[0], 32); mbar_init(&s_full[1], 32); mbar_init(&s_empty[0], 32); mbar_init(&s_empty[1], 32); }
   __syncthreads();
-  int it = 0;
-  for (int gi = blockIdx.x; gi < P.num_games; gi += gridDim.x, ++it) {
+  int gi = blockIdx.x;  // grid <= num_games
+  for (int it = 0;; ++it) {
     const int stage = it & 1, round = it >> 1;
     const InfoStage st = info_stage(s_info + stage * kInfoStageWords);
     if (warp == 0) {
       if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
-      info_build(P, lines, gi, st, s_info + 2 * kInfoStageWords, s_info + 2 * kInfoStageWords + kTrackWords, lane);
-      __syncwarp();
+      if (it > 0) {
+        uint32_t tk = 0;
+        if (lane == 0) tk = atomicInc(ticket, (uint32_t)P.num_games - 1u);
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        gi = tk < (uint32_t)(P.num_games - (int)gridDim.x) ? (int)(gridDim.x + tk) : -1;
+      }
+      if (lane == 0) s_game[stage] = gi;
+      if (gi >= 0) {
+        info_build(P, lines, gi, st, s_info + 2 * kInfoStageWords, s_info + 2 * kInfoStageWords + kTrackWords, lane);
+        __syncwarp();
+      }
       mbar_arrive(&s_full[stage]);
+      if (gi < 0) break;
     } else {
       mbar_wait(&s_full[stage], (uint32_t)round & 1u);
+      gi = s_game[stage];
+      if (gi < 0) break;
       info_store(out, gi, st, lane);
       mbar_arrive(&s_empty[stage]);
     }
