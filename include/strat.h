@@ -215,9 +215,9 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream);
  * the new state.  Produces exactly what strat_legal_mask, strat_sample_uniform,
  * strat_step, strat_encode_obs produce when called in that order.  Any output pointer
  * except `obs` may be NULL (that output is then not written).
- * Consecutive fused steps (this call and strat_step_observe) of one environment on one stream
- * overlap on the device, ordered batch by batch; everything else in the stream sees plain stream
- * order.  They cannot be captured into a CUDA graph (STRAT_BAD_STATE while `stream` is
+ * Consecutive calls of this function for one environment on one stream overlap on the device,
+ * ordered batch by batch; everything else in the stream (strat_step_observe included: it waits for
+ * the producer of its actions, and what follows it waits for it) sees plain stream order.  They cannot be captured into a CUDA graph (STRAT_BAD_STATE while `stream` is
  * capturing): each launch carries a host-side launch counter. */
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward,
                        uint8_t* done, uint16_t* obs, void* stream);
@@ -408,6 +408,16 @@ int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed,
  * Paper's values: alpha = 0.002, beta = 0.02, 1,000 rollouts of depth 40 (Table S12). */
 int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
                         float alpha, float beta, float* qhat, float* rho, float* pi_search, void* stream);
+
+/* ---- measurement aid ---------------------------------------------------------------- */
+/* Streams a constant over dst[0, bytes) with the store instruction the step kernels use for their
+ * outputs (16-byte st.global.cs), in pieces of chunk_bytes (a multiple of 16 that divides bytes; a batch
+ * of observations is 281,600): the plain-write figure bench.py prints next to its roofline fractions.
+ * Persistent CTAs; dynamic = 1: every CTA fetches its next piece from a ticket counter as it finishes
+ * one (how the step kernels hand out batches), 0: equal shares by a fixed stride.  On a B200 the two
+ * differ by ~17 % (7.2-7.4 against 6.2 TB/s): the SMs do not drain their stores at one rate.  The
+ * environment lends its ticket word and SM count; nothing of it is touched. */
+int strat_probe_write(const strat_env* env, void* dst, size_t bytes, int32_t chunk_bytes, int32_t dynamic, void* stream);
 
 #ifdef __cplusplus
 }

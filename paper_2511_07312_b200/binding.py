@@ -25,7 +25,7 @@ EXPORTS = [
     "strat_replay_locate", "strat_share_chain", "strat_replay_sample_chained", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
-    "strat_reduce_returns", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
+    "strat_reduce_returns", "strat_probe_write", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
     "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
     "strat_history_flags",
@@ -69,6 +69,7 @@ def lib():
         L.strat_step.argtypes = [vp, vp, vp, vp, vp]
         L.strat_encode_obs.argtypes = [vp, vp, vp]
         L.strat_encode_infostate.argtypes = [vp, vp, vp]
+        L.strat_probe_write.argtypes = [vp, vp, sz, i32, i32, vp]
         L.strat_rollout_step.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_step_observe.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_host_scratch_bytes.restype = sz
@@ -306,6 +307,11 @@ class Env:
 
     def share_chain(self, other):
         _chk(lib().strat_share_chain(self.h, other.h), "strat_share_chain")
+
+    def probe_write(self, dst, chunk_bytes: int, dynamic: bool):
+        """Measurement aid: stream a constant over the uint8 tensor dst (see strat_probe_write)."""
+        _chk(lib().strat_probe_write(self.h, _ptr(dst, torch.uint8), dst.numel(), chunk_bytes, 1 if dynamic else 0, _stream()),
+             "strat_probe_write")
 
     def check(self):
         return lib().strat_check(self.h)

@@ -423,6 +423,18 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
   return launch_status();
 }
 
+int strat_probe_write(const strat_env* env, void* dst, size_t bytes, int32_t chunk_bytes, int32_t dynamic, void* stream) {
+  if (!env || !dst || chunk_bytes < 16 || chunk_bytes % 16 != 0 || bytes % (size_t)chunk_bytes != 0 ||
+      ((uintptr_t)dst & 15) != 0 || bytes / (size_t)chunk_bytes > 0x7FFFFFFFull)
+    return STRAT_BAD_ARG;
+  if (bytes == 0) return STRAT_OK;
+  const uint32_t pieces = (uint32_t)(bytes / (size_t)chunk_bytes);
+  const uint32_t grid = pieces < (uint32_t)(2 * env->num_sms) ? pieces : (uint32_t)(2 * env->num_sms);
+  k_probe_write<<<grid, 128, 0, (cudaStream_t)stream>>>(reinterpret_cast<uint4*>(dst), pieces, (uint32_t)chunk_bytes / 16u,
+                                                       env->f_obs + batches(env->P.num_games) + 1, dynamic ? 1 : 0);
+  return launch_status();
+}
+
 int strat_rollout_step(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* reward, uint8_t* done,
                        uint16_t* obs, void* stream) {
   if (!env || !obs) return STRAT_BAD_ARG;

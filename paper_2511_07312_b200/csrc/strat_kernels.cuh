@@ -933,5 +933,31 @@ __global__ void __launch_bounds__(64, 12) k_encode_infostate(Params P, const uin
 
 __global__ void k_set_int(int* p, int v) { *p = v; }
 
+// Measurement aid (strat_probe_write): a constant streamed out in pieces of `chunk16` 16-byte vectors with the
+// store instruction of the step kernels' outputs.  Persistent CTAs; pieces by ticket (self-resetting
+// counter, as above) or by a fixed stride.
+__global__ void __launch_bounds__(128) k_probe_write(uint4* __restrict__ dst, uint32_t pieces, uint32_t chunk16,
+                                                     uint32_t* __restrict__ ticket, int dynamic) {
+  __shared__ uint32_t s_piece;
+  const uint4 v = make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
+  uint32_t c = blockIdx.x;
+  for (;;) {
+    uint4* q = dst + (size_t)c * chunk16;
+    for (uint32_t i = threadIdx.x; i < chunk16; i += blockDim.x) st_stream(q + i, v);
+    if (dynamic) {
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        uint32_t tk = atomicInc(ticket, pieces - 1u);
+        s_piece = tk < pieces - gridDim.x ? gridDim.x + tk : 0xFFFFFFFFu;
+      }
+      __syncthreads();
+      c = s_piece;
+    } else {
+      c += gridDim.x;
+    }
+    if (c >= pieces) break;
+  }
+}
+
 
 }  // namespace

@@ -27,8 +27,8 @@ def test_library_exports_every_declared_symbol():
 def test_host_only_entry_points():
     L = binding.lib()
     cfg = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0, 0, 0)
-    ws = L.strat_workspace_bytes(C.byref(cfg))  # lines + error block + ticket ring + 2 flags per 32-game batch
-    assert ws == 65536 * 128 + 256 + (8192 + 2 * 2048) * 4
+    ws = L.strat_workspace_bytes(C.byref(cfg))  # lines + error block + ticket ring + 2 flags per 32-game batch + 64 spare counters
+    assert ws == 65536 * 128 + 256 + (8192 + 2 * 2048 + 64) * 4
     chase = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 1, 0, 0, 0)  # + a 64-ply move log per game
     assert L.strat_workspace_bytes(C.byref(chase)) == ws + 65536 * 128
     info = binding.strat_config(65536, 0, 0, 1000, 0, 1, 1, 0, 0, 0, 1, 0)  # + 2 KB of S2 trackers per game

@@ -347,3 +347,23 @@ def test_more_than_eight_scouts_a_side_are_refused():
     pool[:, 0, 9] = W.MINER
     g.set_setup_pool(torch.from_numpy(pool).cuda())
     assert g.check() == 0
+
+
+def test_probe_write_fills_the_buffer_and_checks_its_arguments():
+    g = B.Env(64, seed=1)
+    for dyn in (True, False):
+        buf = torch.zeros(5000 * 1600, dtype=torch.uint8, device="cuda")
+        g.probe_write(buf, 1600, dyn)            # more pieces than CTAs: every piece, by ticket and by stride
+        assert bool((buf.view(torch.int16) == 0x3F80).all())
+        small = torch.zeros(3 * 32, dtype=torch.uint8, device="cuda")
+        g.probe_write(small, 32, dyn)            # fewer pieces than CTAs
+        assert bool((small.view(torch.int16) == 0x3F80).all())
+    L = B.lib()
+    buf = torch.zeros(4096, dtype=torch.uint8, device="cuda")
+    assert L.strat_probe_write(g.h, B._ptr(buf), 4096, 24, 1, B._stream()) == B.BAD_ARG    # not a multiple of 16
+    assert L.strat_probe_write(g.h, B._ptr(buf), 4096, 4000 // 16 * 16, 1, B._stream()) == B.BAD_ARG  # does not divide
+    assert L.strat_probe_write(g.h, B._ptr(buf), 0, 16, 1, B._stream()) == B.OK
+    assert g.check() == 0
+    # the ticket word cleans up after itself: a second environment-sized use right after works too
+    g.probe_write(buf, 16, True); g.probe_write(buf, 16, True)
+    assert bool((buf.view(torch.int16) == 0x3F80).all())
