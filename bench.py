@@ -618,7 +618,8 @@ def run_infostate(args):
                    "tensor_bytes_per_game": 487 * 100 * 2, "tracker_bytes_per_game": 2048,
                    "l2": "output 6.38 GB per step > 126 MB L2 (no flush needed)"},
         "roofline": dict(_peak_line(per_game * n / (ms_enc / 1e3) / 1e9), kernel="k_encode_infostate",
-                         algorithmic_bytes_per_game=per_game),
+                         algorithmic_bytes_per_game=per_game, traffic=ncu_constant("k_encode_infostate", "dram_bytes_per_launch")[0],
+                         traffic_source=ncu_constant("k_encode_infostate", "dram_bytes_per_launch")[1]),
         "gpu_launches": 2 * steps, "clocks": sampler.result(),
     }
     print(json.dumps(line))
@@ -664,7 +665,9 @@ def run_observe(args):
                    "ms_policy_stand_in": ms_pol, "ms_step_observe_median": ms_obs,
                    "note": "events between the two kernels: strat_step_observe is timed as an isolated launch"},
         "roofline": dict(_peak_line(ALGO_BYTES_PER_GAME_STEP * n / (ms_obs / 1e3) / 1e9), kernel="k_rollout_step<external>",
-                         algorithmic_bytes_per_game_step=ALGO_BYTES_PER_GAME_STEP),
+                         algorithmic_bytes_per_game_step=ALGO_BYTES_PER_GAME_STEP,
+                         traffic=ncu_constant("k_rollout_step_observe", "dram_bytes_per_launch")[0],
+                         traffic_source=ncu_constant("k_rollout_step_observe", "dram_bytes_per_launch")[1]),
         "gpu_launches": 2 * steps, "clocks": sampler.result(),
     }
     print(json.dumps(line))
