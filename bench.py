@@ -501,6 +501,8 @@ def run_cfg4(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     t_det = t_roll = t_red = 0.0
     steps = max(1, min(args.steps, 20))
+    sampler = ClockSampler(0)
+    sampler.start()
     for k in range(min(args.warmup, 3) + steps):
         ev[0].record()
         B.determinise(roots, S, 1000 + k, out)
@@ -512,6 +514,8 @@ def run_cfg4(args):
         torch.cuda.synchronize()
         if k >= min(args.warmup, 3):
             t_det += ev[0].elapsed_time(ev[1]); t_roll += ev[1].elapsed_time(ev[2]); t_red += ev[2].elapsed_time(ev[3])
+    sampler.stop_flag = True
+    sampler.join()
     assert out.check() == 0 and roots.check() == 0
     total = t_det + t_roll + t_red
     line = {
@@ -526,7 +530,7 @@ def run_cfg4(args):
         # instruction-issue bound: peak = SMs x 4 schedulers x 1 warp instruction per clock x max SM clock
         # (DESIGN.md section 6); achieved = ncu smsp__inst_executed.sum of one rollout launch / its CUDA-event time
         "roofline": cfg4_roofline(t_roll / steps),
-        "gpu_launches": 3 * steps,
+        "gpu_launches": 3 * steps, "clocks": sampler.result(),
     }
     print(json.dumps(line))
 
@@ -547,6 +551,8 @@ def run_search(args):
     outs = tuple(torch.empty((R, 3600), dtype=torch.float32, device="cuda") for _ in range(3))
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     steps = max(1, min(args.steps, 20))
+    sampler = ClockSampler(0)
+    sampler.start()
     t = [0.0, 0.0, 0.0]
     for k in range(min(args.warmup, 3) + steps):
         ev[0].record()
@@ -560,6 +566,8 @@ def run_search(args):
         if k >= min(args.warmup, 3):
             for i in range(3):
                 t[i] += ev[i].elapsed_time(ev[i + 1])
+    sampler.stop_flag = True
+    sampler.join()
     assert games.check() == 0 and roots.check() == 0
     total = sum(t)
     legal = (outs[2] > 0).sum(dim=1).float().mean().item()
@@ -572,7 +580,7 @@ def run_search(args):
                    "searched_moves_per_sec": R * steps / (total / 1e3), "mean_legal_actions": legal,
                    "note": "env-step count includes unused slots' share (rollouts*depth per root); paper: 1.26 s per "
                            "searched move on one H100 WITH its networks (PAPER.md:200) - context only"},
-        "gpu_launches": 3 * steps,
+        "gpu_launches": 3 * steps, "clocks": sampler.result(),
     }
     print(json.dumps(line))
 
