@@ -345,6 +345,36 @@ def test_encode_midgame_planes_and_history():
     assert o[:, 12:24].sum() > 0 and o[:, 24].sum() > 0
 
 
+def test_encode_hand_worked_position():
+    """The 44 planes of a six-piece position written out by hand from BASELINE.json configs[0] ("12 own-type
+    planes, 12 revealed-opponent-type planes, 2 planes for hidden opponent pieces (moved / unmoved), 1 lake
+    plane, 1 empty plane, and from/to planes for the last 8 plies"; order Spy..Marshal, Flag, Bomb: R18),
+    blue to move.  Nothing here is computed: a wrong plane index, owner test or history order fails it."""
+    pieces = {0: W.piece(W.FLAG, W.RED),                               # opponent, hidden, unmoved   -> plane 25
+              14: W.piece(W.SCOUT, W.RED, moved=True, revealed=True),  # opponent, revealed Scout    -> plane 12 + 1
+              35: W.piece(W.MAJOR, W.RED, moved=True),                 # opponent, hidden, moved     -> plane 24
+              99: W.piece(W.FLAG, W.BLUE),                             # own Flag                    -> plane 10
+              64: W.piece(W.MINER, W.BLUE, moved=True),                # own Miner                   -> plane 2
+              77: W.piece(W.BOMB, W.BLUE, revealed=True)}              # own Bomb (own: by type only) -> plane 11
+    # last plies, most recent first: red 25 -> 35, blue 74 -> 64, red 54 -> 14 (a Scout's long move)
+    e = orc.Env(1)
+    e.reset_from(W.make_line(pieces, ply=3, history=((25, 35), (74, 64), (54, 14)))[None])
+    o = e.encode_obs()[0].reshape(44, 100)
+    assert set(np.unique(o)) <= {0, ONE}
+    got = {(int(p_), int(c)) for p_, c in zip(*np.nonzero(o)) if p_ not in (26, 27)}
+    assert got == {(25, 0), (13, 14), (24, 35), (10, 99), (2, 64), (11, 77),
+                   (28, 25), (29, 35), (30, 74), (31, 64), (32, 54), (33, 14)}
+    assert sorted(np.nonzero(o[26])[0].tolist()) == [42, 43, 46, 47, 52, 53, 56, 57]          # lakes c5-d6, g5-h6
+    assert sorted(np.nonzero(o[27])[0].tolist()) == sorted(set(range(100)) - {42, 43, 46, 47, 52, 53, 56, 57}
+                                                           - {0, 14, 35, 99, 64, 77})     # 86 empty squares
+    # the same position seen by red (ply 4): own / opponent swap, the history shifts by nothing (it is absolute)
+    e.reset_from(W.make_line(pieces, ply=4, history=((25, 35), (74, 64), (54, 14)))[None])
+    o = e.encode_obs()[0].reshape(44, 100)
+    got = {(int(p_), int(c)) for p_, c in zip(*np.nonzero(o)) if p_ not in (26, 27)}
+    assert got == {(10, 0), (1, 14), (6, 35), (25, 99), (24, 64), (23, 77),
+                   (28, 25), (29, 35), (30, 74), (31, 64), (32, 54), (33, 14)}
+
+
 def test_encode_is_an_information_state():
     # re-typing the opponent's unrevealed pieces must not change the observation
     e = orc.Env(8, seed=6, max_plies=1000)
