@@ -1036,14 +1036,18 @@ SD void track_ply(uint32_t* trk, const Game& g, int two_square, int side, int fr
   sd_st16(trk + kTrkMoves, (int)(g.ply & 31u), (uint32_t)from | ((uint32_t)to << 7));
 }
 
-struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; };
+struct StepOut { int reward; uint32_t done; bool illegal; bool needs_reset; bool nomove_pending; };
 
 // kValidate = false only when `a` was just drawn from this state's own legal mask.
 // kDeferReset: the caller performs the auto-reset itself (epoch is already advanced) when
 // o.needs_reset is set; the result must equal reset_game(P, local_game, g).
-template <bool kValidate, bool kDeferReset = false, bool kChase = false, bool kTrack = false>
+// kDeferNoMove (on-chip rollouts): "the opponent has no legal move" is left open (o.nomove_pending) unless
+// a draw by ply cap or battleless count is due, whose rank in R#12 needs the answer now.  The caller learns
+// it from the next ply's own move generation and closes the game with finish_no_move: the opponent's move
+// set is computed once per ply instead of twice.
+template <bool kValidate, bool kDeferReset = false, bool kChase = false, bool kTrack = false, bool kDeferNoMove = false>
 SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
-  StepOut o; o.illegal = false; o.needs_reset = false;
+  StepOut o; o.illegal = false; o.needs_reset = false; o.nomove_pending = false;
   if (g.done) { o.reward = 0; o.done = 1u | (g.reason << 2); return o; }  // R#15: frozen
   int side = g.ply & 1u;
   // a live game without a legal move (only a hand-built line can be one: play ends such games)
@@ -1106,7 +1110,9 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
   g.ply += 1;
   int mover_result = side == 0 ? 1 : -1;
   // terminal tests in R#12 order
+  const bool draw_due = (int)g.ply >= P.ply_cap || (P.max_battleless > 0 && (int)g.battleless >= P.max_battleless);
   if (flag_captured) { g.done = 1; g.reason = REASON_FLAG; g.result = mover_result; }
+  else if (kDeferNoMove && !draw_due) { o.nomove_pending = true; }
   else if (!has_legal_move(g, side ^ 1, rules_of<kChase>(P), glog)) {
     g.done = 1;
     if (!has_legal_move(g, side, rules_of<kChase>(P), glog)) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
@@ -1124,6 +1130,18 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
     else { reset_game(P, local_game, g); if (kTrack && P.track) track_start(game_track(P, local_game), g); }
   }
   return o;
+}
+
+// Closes a game whose side to move was found to have no legal move (step_game<..., kDeferNoMove> left the
+// test open): exactly what step_game does in that case, auto-reset included.
+template <bool kChase>
+SD void finish_no_move(const Params& P, uint32_t local_game, Game& g) {
+  const int side = (int)(g.ply & 1u);             // cannot move; the previous mover is side ^ 1
+  const int mover_result = side == 1 ? 1 : -1;
+  g.done = 1;
+  if (!has_legal_move(g, side ^ 1, rules_of<kChase>(P), kChase ? game_log(P, local_game) : nullptr)) { g.reason = REASON_NOMOVE_DRAW; g.result = 0; }
+  else { g.reason = REASON_NOMOVE_WIN; g.result = mover_result; }
+  if (P.auto_reset) { g.epoch += 1; reset_game(P, local_game, g); }
 }
 
 // ------------------------------------------------------------------ observation bits (C5)

@@ -336,25 +336,42 @@ __global__ void __launch_bounds__(32, STRAT_ROLLOUT_MIN_CTAS) k_rollout_uniform(
   if (live) read_game(s_state, lane, g);
   uint32_t* scouts = s_scouts + lane * kScoutScratch;
   const uint16_t* glog = kChase ? game_log(P, (uint32_t)(first + lane)) : nullptr;
+  // Without the chasing rule "the opponent has no legal move" is not tested after a move: the next ply's move
+  // generation says so (no action at all), and the game is closed then as the step would have closed it
+  // (finish_no_move).  One move generation per ply instead of two; the states after every ply are the same.
+  constexpr bool kDefer = !kChase;
+  bool pending = false;
   for (int t = 0; t < plies; ++t) {
     live = live && !g.done;
     if (!__any_sync(full, live)) break;
     ActionSet A;
     uint32_t u = 0;
     if (live) {
-      u = action_draw(P, (uint32_t)(first + lane), g);
       count_actions(g, g.ply & 1u, rules_of<kChase>(P), scouts, A);
+      if (kDefer && pending && A.n == 0) {  // rare: the previous ply ended the game
+        finish_no_move<kChase>(P, (uint32_t)(first + lane), g);
+        live = !g.done;
+        if (live) count_actions(g, g.ply & 1u, rules_of<kChase>(P), scouts, A);  // auto-reset: a fresh game
+      }
+      if (live) u = action_draw(P, (uint32_t)(first + lane), g);
     }
+    pending = false;
     const int kmax = (int)__reduce_max_sync(full, live ? (unsigned)A.ns : 0u);  // also reconverges the warp
     int a = -1;
     if (live) a = choose_action(g, g.ply & 1u, rules_of<kChase>(P), A, u, scouts, glog, kmax);
     __syncwarp();
-    if (live && step_game<false, false, kChase>(P, (uint32_t)(first + lane), g, a).illegal) {
-      raise_error(err, STRAT_ILLEGAL_ACTION);
-      live = false;
+    if (live) {
+      StepOut o = step_game<false, false, kChase, false, kDefer>(P, (uint32_t)(first + lane), g, a);
+      pending = o.nomove_pending;
+      if (o.illegal) {
+        raise_error(err, STRAT_ILLEGAL_ACTION);
+        live = false;
+      }
     }
     __syncwarp();
   }
+  if (kDefer && pending && live && !g.done && !has_legal_move(g, g.ply & 1u, rules_of<kChase>(P)))
+    finish_no_move<kChase>(P, (uint32_t)(first + lane), g);  // the test the last ply left open
   if (lane < ng) write_game(s_state, lane, g);
   __syncwarp();
   store_lines(lines, first, ng, s_state, lane);
