@@ -54,7 +54,11 @@ template <bool kPublish = true>
 __device__ __forceinline__ void flag_set(uint32_t* flag, uint32_t v, int lane) {
   __syncwarp();
   if (lane == 0) {
+#ifdef STRAT_FLAG_SC_FENCE
     if (kPublish) { __threadfence(); st_release(flag, v); }
+#else
+    if (kPublish) st_release(flag, v);  // release is cumulative over the lanes the barrier above ordered before it
+#endif
     else asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(v) : "memory");
   }
 }

@@ -28,7 +28,6 @@ static inline void sd_stlog(uint16_t* p, uint16_t v) { *p = v; }
 static inline uint32_t sd_ld32(const uint32_t* p) { return *p; }
 static inline void sd_st32(uint32_t* p, uint32_t v) { *p = v; }
 static inline void sd_or32(uint32_t* p, uint32_t v) { *p |= v; }
-static inline uint32_t sd_inc32(uint32_t* p, uint32_t v) { uint32_t o = *p; *p = o + v; return o; }
 static inline void sd_st16(uint32_t* words, int half, uint32_t v) { reinterpret_cast<uint16_t*>(words)[half] = (uint16_t)v; }
 static inline void sd_ld128(const uint32_t* p, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) { a = p[0]; b = p[1]; c = p[2]; d = p[3]; }
 static inline void sd_st128(uint32_t* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) { p[0] = a; p[1] = b; p[2] = c; p[3] = d; }
@@ -48,7 +47,6 @@ SD uint32_t sd_ld32(const uint32_t* p) { return __ldcg(p); }
 SD void sd_st32(uint32_t* p, uint32_t v) { __stcg(p, v); }
 // tracker bits are OR-ed in at the L2 without reading them back (RED.OR: nothing to wait for)
 SD void sd_or32(uint32_t* p, uint32_t v) { atomicOr(p, v); }
-SD uint32_t sd_inc32(uint32_t* p, uint32_t v) { return atomicAdd(p, v); }
 SD void sd_st16(uint32_t* words, int half, uint32_t v) { __stcg(reinterpret_cast<uint16_t*>(words) + half, (uint16_t)v); }
 SD void sd_ld128(const uint32_t* p, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
   uint4 v = __ldcg(reinterpret_cast<const uint4*>(p)); a = v.x; b = v.y; c = v.z; d = v.w;
@@ -919,9 +917,12 @@ SD uint32_t key13_of(uint32_t b) {
 // the (few) pieces that stand next to an enemy.
 SD void track_ply(uint32_t* trk, const Game& g, int two_square, int side, int from, int to, int dist, int pt, int tt) {
   const BB occ = occupied(g), mine = owned_by(g, occ, side), enemy = bb_andn(occ, mine);
+  // everything the ply reads from the block, in one trip: the mover's record, the target's first word (its
+  // start square, needed if it dies) and the number of pieces captured so far
   uint32_t r0, r1, r2, r3;
   sd_ld128(trk + 4 * from, r0, r1, r2, r3);
-  const uint32_t d0 = tt != 0 ? sd_ld32(trk + 4 * to) : 0u;
+  const uint32_t d0 = sd_ld32(trk + 4 * to);
+  const uint32_t deaths = sd_ld32(trk + kTrkDeaths);
   // (i) active adjacency: every legal one-square capture that is not the move played.
   // att[d] = own movable pieces with an enemy on the next square in direction d.
   {
@@ -1016,7 +1017,8 @@ SD void track_ply(uint32_t* trk, const Game& g, int two_square, int side, int fr
     const bool d_rev = bb_test(g.rev, to) != 0;
     const int out = battle(pt, tt);
     const bool d_dies = out >= 0 && tt != T_FLAG, c_dies = out <= 0;
-    uint32_t n = sd_inc32(trk + kTrkDeaths, (d_dies ? 1u : 0u) + (c_dies ? 1u : 0u));
+    uint32_t n = deaths;  // one thread owns the block: a plain store, no atomic to wait for
+    sd_st32(trk + kTrkDeaths, deaths + (d_dies ? 1u : 0u) + (c_dies ? 1u : 0u));
     if (d_dies) {
       uint32_t cause = tt <= 10 ? (d_rev ? (out > 0 ? 4u : 5u) : 6u) : 0u;
       if (n < (uint32_t)kTrkMaxDeaths)
