@@ -304,11 +304,15 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
                         void* stream);
 /* The same gather for a self-play loop that pushes in place (in-place rings only): issued between
  * two fused steps of `env` on `stream`, it does not separate them - the next strat_rollout_step
- * still overlaps the previous one on the device.  The gather itself waits for the fused step
- * issued before it (everything that step pushed is sampled from), and the fused step after the
- * NEXT gather waits for this one before it reuses ring rows (the ring's spare rows cover exactly
- * that distance).  One ring serves one environment this way; outputs are valid in stream order
- * as usual.  STRAT_BAD_STATE on a plain or empty ring. */
+ * still overlaps the previous one on the device.  Everything the fused step issued before it
+ * pushed is sampled from: in the regular loop (strat_rollout_step into the reserved rows,
+ * strat_replay_commit without copies, this call, once per step) the gather runs alongside that step
+ * and takes each record as soon as the step has published the record's 32-game batch; after anything
+ * else (a copy push, another call on the environment, the first gather) it waits for the whole stream
+ * before it.  The fused step after the NEXT gather waits for this one before it reuses ring rows (the
+ * ring's spare rows cover exactly that distance), and a gather waits for the one before it before it
+ * overwrites the minibatch buffers.  One ring serves one environment this way; outputs are valid in
+ * stream order as usual.  STRAT_BAD_STATE on a plain or empty ring. */
 int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, uint64_t draw_index, int32_t batch,
                                 uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,
                                 void* stream);

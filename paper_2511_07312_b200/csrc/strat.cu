@@ -211,9 +211,16 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   }
   auto kernel = env->P.track ? (env->P.chase_rule ? k_rollout_step<kExternal, true, true> : k_rollout_step<kExternal, false, true>)
                              : (env->P.chase_rule ? k_rollout_step<kExternal, true, false> : k_rollout_step<kExternal, false, false>);
-  // chained gathers: this step may overlap the latest one but not the one before it
-  const uint32_t* gflag = env->chained && env->chained->gathers >= 2 ? env->chained->sync + 2 : nullptr;
-  const uint32_t gnum = env->chained ? env->chained->gathers - 1u : 0u;
+  // chained gathers: the first step after a gather may overlap it (the rows it writes are the ring's spare
+  // rows) but not the gather before it; a further step without a gather in between (a block has been
+  // committed since) would write rows the latest gather may still read, so it waits for that one
+  const uint32_t* gflag = nullptr;
+  uint32_t gnum = 0u;
+  if (env->chained && env->chained->gathers >= 1u) {
+    const strat_replay* r = env->chained;
+    gnum = r->total > r->last_total ? r->gathers : r->gathers - 1u;
+    if (gnum >= 1u) gflag = r->sync + 2;
+  }
   if (cudaLaunchKernelEx(&lc, kernel, env->P, env->lines, mask, actions, reward, done, obs,
                          env->tickets + (version % kTicketRing), env->f_state, env->f_obs, version,
                          hist_slot(env->hist), env->err, wait_prior, gflag, gnum) != cudaSuccess)

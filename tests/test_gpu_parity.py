@@ -544,6 +544,58 @@ def test_chained_gathers_back_to_back_equal_a_synchronised_run():
         assert torch.equal(x, y)
 
 
+def test_chained_gathers_in_an_irregular_loop_equal_a_synchronised_run():
+    """The chained gather takes a record as soon as its producer has published the record's batch only in
+    the regular loop (fused step, commit, gather); anything else - another call on the environment before
+    the gather, two steps between two gathers, a copy push - must make it wait for the stream instead.
+    Issued back to back without host synchronisation; compared with a synchronised run of plain gathers."""
+    n, bs, steps = 8192, 1500, 40
+    kw = dict(variant=0, seed=8, max_plies=70, auto_reset=1)
+    outs = []
+    for chained in (True, False):
+        g = B.Env(n, **kw)
+        ring = B.Replay(n, 3, block=n)
+        so = torch.empty((steps, bs, 4400), dtype=torch.int16, device="cuda")
+        sm = torch.empty((steps, bs, 113), dtype=torch.int32, device="cuda")
+        sa = torch.empty((steps, bs), dtype=torch.int16, device="cuda")
+        sr = torch.empty((steps, bs), dtype=torch.int8, device="cuda")
+        sd = torch.empty((steps, bs), dtype=torch.uint8, device="cuda")
+        act, rew, done = g.new_actions(), g.new_reward(), g.new_done()
+        boards = []
+        o_ptr, _ = ring.reserve(n, 0)
+        B._chk(B.lib().strat_encode_obs(g.h, o_ptr, B._stream()), "encode")
+
+        def push_in_place():
+            _, m_ptr = ring.reserve(n, 0)
+            o_next, _ = ring.reserve(n, 1)
+            a_ptr, r_ptr, d_ptr = ring.reserve_rows(n)
+            g.rollout_step_ptrs(m_ptr, a_ptr, r_ptr, d_ptr, o_next)
+            ring.commit_in_place(n)
+
+        for t in range(steps):
+            push_in_place()
+            if t % 7 == 3:
+                push_in_place()                                   # two steps between two gathers
+            if t % 5 == 2:
+                boards.append(g.get_boards())                     # another call on the environment (device tensor, no sync)
+            if t % 11 == 6:                                       # a push with copied small arrays
+                _, m_ptr = ring.reserve(n, 0)
+                o_next, _ = ring.reserve(n, 1)
+                g.rollout_step_raw(m_ptr, act, rew, done, o_next)
+                ring.commit(act, rew, done)
+            if chained:
+                ring.sample_chained(g, 9, t, bs, so[t], sm[t], sa[t], sr[t], sd[t])
+            else:
+                ring.sample(9, t, bs, so[t], sm[t], sa[t], sr[t], sd[t])
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        assert g.check() == 0
+        outs.append((so, sm, sa, sr, sd, g.get_boards().clone(), torch.stack(boards)))
+        del g, ring
+    for x, y in zip(*outs):
+        assert torch.equal(x, y)
+
+
 def test_config3_full_size_ring_zero_copy_and_sample():
     """BASELINE.json configs[3] at full size in the launch sequence bench.py times: 262,144
     games, 64 x 131,072-record ring (77.6 GB + spare rows), in-place push + 4,096-sample gather
