@@ -30,7 +30,8 @@ constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
 // and the fewer batches an SM has drawn ahead of its stores the more evenly they do (measured at 65,536
 // games, isolated launch: 2 -> 102.5 us, 3 -> 102.4 us, 4 -> 104.5 us, 6 -> 109.6 us; at 262,144: 3 -> 389 us).
 // Tried and dropped: the logic warp helping to store the CTA's last batch (drawing the next ticket before
-// the hand-over, to know which batch is the last, unbalances the SMs by more than the help gains: 106.5 us).
+// the hand-over, to know which batch is the last, unbalances the SMs by more than the help gains: 106.5 us);
+// drawing the last tickets of a launch only when the CTA's store warp has nothing left (no change).
 #ifndef STRAT_WS_EXT_CTAS_PER_SM
 #define STRAT_WS_EXT_CTAS_PER_SM 3
 #endif
@@ -54,11 +55,9 @@ template <bool kPublish = true>
 __device__ __forceinline__ void flag_set(uint32_t* flag, uint32_t v, int lane) {
   __syncwarp();
   if (lane == 0) {
-#ifdef STRAT_FLAG_SC_FENCE
-    if (kPublish) { __threadfence(); st_release(flag, v); }
-#else
-    if (kPublish) st_release(flag, v);  // release is cumulative over the lanes the barrier above ordered before it
-#endif
+    // release is cumulative over the lanes the barrier above ordered before it; a sequentially consistent
+    // __threadfence() in front of it (round 1) only cost time: 86.3 -> 85.7 us per overlapped step
+    if (kPublish) st_release(flag, v);
     else asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(v) : "memory");
   }
 }
@@ -131,8 +130,9 @@ __global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restr
   if (kExternal) fill_lut(s_lut256, threadIdx.x, 64);
   __syncthreads();
   // Let the next launch of this kernel become resident now: it orders itself behind this one
-  // batch by batch through f_state / f_obs.  Only a launch whose predecessor in the stream is a
-  // fused step of ANOTHER environment (no flags tie the two) waits for that grid as a whole.
+  // batch by batch through f_state / f_obs.  wait_prior (host, launch_fused): this launch does not directly
+  // continue its own environment's chain of fused steps - no flags tie it to what runs before it - so it
+  // waits for that as a whole.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
   if (warp == 0) {
