@@ -1085,29 +1085,29 @@ SD StepOut step_game(const Params& P, uint32_t local_game, Game& g, int a) {
     g.logn += 1;
   }
   hist_push(g, (uint32_t)from | ((uint32_t)to << 7));
-  // the origin square empties in every case
-  bb_put(g.t0, sf, 0); bb_put(g.t1, sf, 0); bb_put(g.t2, sf, 0); bb_put(g.t3, sf, 0);
-  bb_put(g.own, sf, 0); bb_put(g.mvd, sf, 0); bb_put(g.rev, sf, 0);
   bool flag_captured = false;
   int outcome = 1;  // plain move = the mover arrives
-  if (tt == 0) {
-    g.battleless += 1;
-    prev |= dist >= 2 ? 1u : 0u;  // R#10: a long move shows a Scout
-  } else {
-    g.battleless = 0;
-    prev = 1;                     // battle: both revealed
-    outcome = battle(pt, tt);
-    flag_captured = tt == T_FLAG;
-  }
-  if (outcome > 0) {              // mover occupies the target
-    bb_put(g.t0, st, pt & 1); bb_put(g.t1, st, (pt >> 1) & 1); bb_put(g.t2, st, (pt >> 2) & 1);
-    bb_put(g.t3, st, (pt >> 3) & 1);
-    bb_put(g.own, st, side); bb_put(g.mvd, st, 1); bb_put(g.rev, st, prev);
-  } else if (outcome < 0) {       // defender stays, now revealed (R#11: moved bit unchanged)
-    bb_put(g.rev, st, 1);
-  } else {                        // both removed
-    bb_put(g.t0, st, 0); bb_put(g.t1, st, 0); bb_put(g.t2, st, 0); bb_put(g.t3, st, 0);
-    bb_put(g.own, st, 0); bb_put(g.mvd, st, 0); bb_put(g.rev, st, 0);
+  // the battle is decided first, without branches on the lanes' different cases
+  const bool fight = tt != 0;
+  g.battleless = fight ? 0u : g.battleless + 1u;
+  prev = fight ? 1u : (prev | (dist >= 2 ? 1u : 0u));  // battle: both revealed; R#10: a long move shows a Scout
+  outcome = fight ? battle(pt, tt) : 1;
+  flag_captured = tt == T_FLAG;
+  // One pass over the seven planes: the origin square empties in every case; the target takes the mover's
+  // bits (outcome > 0), is cleared (both removed) or stays as it is but revealed (the defender wins; R#11:
+  // its moved bit is unchanged).
+  {
+    const bool win = outcome > 0, stays = outcome < 0;
+    const uint32_t bits = win ? ((uint32_t)pt | ((uint32_t)side << 4) | (1u << 5) | (prev << 6)) : 0u;
+    BB* planes[7] = {&g.t0, &g.t1, &g.t2, &g.t3, &g.own, &g.mvd, &g.rev};
+    STRAT_UNROLL
+    for (int i = 0; i < 4; ++i) {
+      const uint32_t tm = stays ? 0u : st.m[i];   // target word mask, void when the defender stays
+      const uint32_t clr = ~(sf.m[i] | tm);
+      STRAT_UNROLL
+      for (int p = 0; p < 7; ++p) planes[p]->w[i] = (planes[p]->w[i] & clr) | (((bits >> p) & 1u) ? tm : 0u);
+      g.rev.w[i] |= stays ? st.m[i] : 0u;
+    }
   }
   g.ply += 1;
   int mover_result = side == 0 ? 1 : -1;
