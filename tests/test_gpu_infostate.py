@@ -163,3 +163,30 @@ def test_infostate_argument_errors():
     import ctypes as C
     assert L.strat_workspace_bytes(C.byref(bad)) == 0
     assert tracked.check() == 0
+
+
+def test_infostate_full_size_ticketed_encoder():
+    """65,536 games (the bench shape: more games than the encoder has CTAs, so games are handed out by its
+    self-resetting ticket counter), trackers kept by overlapped fused steps; four slices of 16 games spread
+    over the batch are mirrored by oracle shards keyed by their global game index.  Encoded twice: the
+    counter must have cleaned up after the first pass."""
+    n, steps = 65536, 45
+    kw = dict(variant=0, seed=12, max_plies=30, auto_reset=1, infostate=1)   # 30-ply cap: resets inside the window
+    g = B.Env(n, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for _ in range(steps):
+        g.rollout_step(mask, act, rew, done, obs)
+    first = g.encode_infostate()
+    second = g.encode_infostate(g.new_infostate())
+    assert torch.equal(first.view(torch.int16), second.view(torch.int16))
+    got = first.view(torch.int16)
+    for base in (0, 1777, 30001, 65520):
+        o = orc.Env(16, game_base=base, **kw)
+        for _ in range(steps):
+            o.step(o.sample_uniform(o.legal_mask()))
+        want = o.encode_infostate().reshape(16, -1)
+        have = got[base:base + 16].cpu().numpy().view(np.uint16).reshape(16, -1)
+        assert np.array_equal(have, want), base
+    # every game was written: channel 38 (empty) + lakes + pieces cover the board, so no row is all zero
+    assert bool((got.view(n, -1) != 0).any(dim=1).all())
+    assert g.check() == 0
