@@ -13,29 +13,30 @@ using namespace strat;
 // stages to bf16 and streams them out.  The two are decoupled by mbarriers, so on every SM
 // observation stores of batch i flow while batch i+1 is still in its (latency-bound) rule
 // logic; with one-warp CTAs all resident warps ran logic, then stores, in lockstep.
-#ifndef STRAT_WS_STAGES
-#define STRAT_WS_STAGES 2
-#endif
-constexpr int kWsStages = STRAT_WS_STAGES;
-// Resident CTAs per SM of ONE launch.  Two consecutive launches are co-resident (6 CTAs x 35.7 KB
-// of shared memory per SM): the later one trails the earlier one batch by batch, so the HBM
-// write stream never drains between steps.  Measured on B200 at 65,536 games: 2 -> 88.8 us,
-// 3 -> 87.8 us, 4 -> 90.3 us, 6 -> 93.1 us per step.
-#ifndef STRAT_WS_CTAS_PER_SM
-#define STRAT_WS_CTAS_PER_SM 3
-#endif
-constexpr int kWsCtasPerSm = STRAT_WS_CTAS_PER_SM;
-// strat_step_observe never overlaps its neighbours in the stream (it waits for its actions' producer).
-// With ~14 batches per SM at 65,536 games the launch is short: what counts is how evenly the SMs finish,
-// and the fewer batches an SM has drawn ahead of its stores the more evenly they do (measured at 65,536
-// games, isolated launch: 2 -> 102.5 us, 3 -> 102.4 us, 4 -> 104.5 us, 6 -> 109.6 us; at 262,144: 3 -> 389 us).
-// Tried and dropped: the logic warp helping to store the CTA's last batch (drawing the next ticket before
-// the hand-over, to know which batch is the last, unbalances the SMs by more than the help gains: 106.5 us);
-// drawing the last tickets of a launch only when the CTA's store warp has nothing left (no change).
-#ifndef STRAT_WS_EXT_CTAS_PER_SM
-#define STRAT_WS_EXT_CTAS_PER_SM 3
-#endif
-constexpr int kWsExternalCtasPerSm = STRAT_WS_EXT_CTAS_PER_SM;
+// Staging buffers per CTA and resident CTAs per SM (measured on B200, CUDA events, 65,536 / 262,144 games;
+// "back to back" = 2,000 overlapped launches, "alone" = one launch with the GPU to itself):
+//   strat_rollout_step   ONE stage, 8 CTAs per SM (128 registers): 83.0 / 342 us back to back, 121 / 381 us
+//                        alone.  A CTA's logic and its stores then alternate and the SM's other seven CTAs
+//                        fill the gaps; drawing no batch ahead of the stores keeps the SMs, which do not all
+//                        drain stores at one rate, in balance.  (Two stages, 3 CTAs per SM and two launches
+//                        co-resident, round 1's choice: 85.5 / 352 and 121 / 386 us.  One stage with 2..7
+//                        CTAs: the same back to back, but 185..127 us alone.)
+//   with chase_rule or   two stages, 3 CTAs per SM and two launches co-resident, as strat_rollout_step had them
+//   the S2 trackers      in round 1: the rule code needs ~160 registers, so at most 6 CTAs fit, and with one
+//                        stage and 6 CTAs both lose (chase_rule 87.1 -> 88.3 us back to back, trackers
+//                        150 -> 164 us alone).
+//   strat_step_observe   TWO stages, 3 CTAs per SM: it never overlaps its neighbours in the stream (it waits
+//                        for its actions' producer), its launch is short (~14 batches per SM) and what
+//                        counts is how evenly the SMs finish: 2 -> 102.5 us, 3 -> 102.4 us, 4 -> 104.5 us,
+//                        6 -> 109.6 us; one stage with 6 CTAs 112.7 us.  Tried and dropped: the logic warp
+//                        helping to store the CTA's last batch (drawing the next ticket before the hand-over,
+//                        to know which batch is the last, unbalances the SMs by more than the help gains:
+//                        106.5 us); drawing the last tickets only when the store warp has nothing left (no
+//                        change).
+template <bool kExternal, bool kRules> struct WsShape { static constexpr int kStages = (kExternal || kRules) ? 2 : 1; };
+constexpr int kWsCtasPerSm = 8;          // strat_rollout_step
+constexpr int kWsRuleCtasPerSm = 3;      // ... with chase_rule or infostate
+constexpr int kWsExternalCtasPerSm = 3;  // strat_step_observe
 constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
 
 // Per-batch version flags in global memory: consecutive launches of the fused step overlap
@@ -104,13 +105,15 @@ __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, 
 //   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
 //   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
 template <bool kExternal, bool kChase, bool kTrack>
-__global__ void __launch_bounds__(64) k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
+__global__ void __launch_bounds__(64, kExternal ? kWsExternalCtasPerSm : (kChase || kTrack) ? 2 * kWsRuleCtasPerSm : kWsCtasPerSm)
+k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
                                                         uint32_t* __restrict__ ticket, uint32_t* __restrict__ f_state,
                                                         uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
                                                         int* __restrict__ err, int wait_prior,
                                                         const uint32_t* __restrict__ gather_flag, uint32_t gather_number) {
+  constexpr int kWsStages = WsShape<kExternal, kChase || kTrack>::kStages;
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   // strat_step_observe runs 3 CTAs per SM and has shared memory to spare: a byte -> 8 x bf16 table (one
