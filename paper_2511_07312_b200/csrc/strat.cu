@@ -191,7 +191,7 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   if (capture != cudaStreamCaptureStatusNone) return STRAT_BAD_STATE;
   const int nb = batches(env->P.num_games);
   // a launch that follows a policy kernel has the GPU to itself (kWsExternalCtasPerSm says how it uses it)
-  const int per_sm = kExternal ? kWsExternalCtasPerSm : (env->P.chase_rule || env->P.track) ? kWsRuleCtasPerSm : kWsCtasPerSm;
+  const int per_sm = kExternal ? kWsExternalCtasPerSm : env->P.track ? kWsTrackCtasPerSm : kWsCtasPerSm;
   const int grid = nb < env->num_sms * per_sm ? nb : env->num_sms * per_sm;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(64); lc.dynamicSmemBytes = 0; lc.stream = (cudaStream_t)stream;

@@ -21,10 +21,12 @@ using namespace strat;
 //                        drain stores at one rate, in balance.  (Two stages, 3 CTAs per SM and two launches
 //                        co-resident, round 1's choice: 85.5 / 352 and 121 / 386 us.  One stage with 2..7
 //                        CTAs: the same back to back, but 185..127 us alone.)
-//   with chase_rule or   two stages, 3 CTAs per SM and two launches co-resident, as strat_rollout_step had them
-//   the S2 trackers      in round 1: the rule code needs ~160 registers, so at most 6 CTAs fit, and with one
-//                        stage and 6 CTAs both lose (chase_rule 87.1 -> 88.3 us back to back, trackers
-//                        150 -> 164 us alone).
+//   with chase_rule      the same shape (the rule code fits 128 registers too): 84.7 us back to back, 124 us alone
+//                        (two stages, 3 CTAs: 87.0 us).
+//   with the S2 trackers two stages, 3 CTAs per SM and two launches co-resident, as strat_rollout_step had them
+//                        in round 1: its logic warp waits for the tracker record from HBM and is what bounds
+//                        the step; one stage with 8 CTAs is 3 % faster back to back (113 us) and 2 % slower
+//                        alone (154 against 151 us), and alone is how the 487-channel pipeline runs it.
 //   strat_step_observe   TWO stages, 3 CTAs per SM: it never overlaps its neighbours in the stream (it waits
 //                        for its actions' producer), its launch is short (~14 batches per SM) and what
 //                        counts is how evenly the SMs finish: 2 -> 102.5 us, 3 -> 102.4 us, 4 -> 104.5 us,
@@ -33,9 +35,9 @@ using namespace strat;
 //                        to know which batch is the last, unbalances the SMs by more than the help gains:
 //                        106.5 us); drawing the last tickets only when the store warp has nothing left (no
 //                        change).
-template <bool kExternal, bool kRules> struct WsShape { static constexpr int kStages = (kExternal || kRules) ? 2 : 1; };
-constexpr int kWsCtasPerSm = 8;          // strat_rollout_step
-constexpr int kWsRuleCtasPerSm = 3;      // ... with chase_rule or infostate
+template <bool kExternal, bool kTrack> struct WsShape { static constexpr int kStages = (kExternal || kTrack) ? 2 : 1; };
+constexpr int kWsCtasPerSm = 8;          // strat_rollout_step, also with chase_rule
+constexpr int kWsTrackCtasPerSm = 3;     // ... with the S2 trackers (infostate)
 constexpr int kWsExternalCtasPerSm = 3;  // strat_step_observe
 constexpr int kWsStageWords = kBatch * kBitsRowWords;  // 4448 words = 17,792 B (mask rows need 3,616)
 
@@ -105,7 +107,7 @@ __device__ __forceinline__ void store_game_global(uint32_t* __restrict__ lines, 
 //   mask AND observation of the new state: the data-collection loop of PAPER.md:232, 461-462
 //   (ApplyActions, then ComputeLegalActionMask + ComputeInfostateTensor for the next policy call).
 template <bool kExternal, bool kChase, bool kTrack>
-__global__ void __launch_bounds__(64, kExternal ? kWsExternalCtasPerSm : (kChase || kTrack) ? 2 * kWsRuleCtasPerSm : kWsCtasPerSm)
+__global__ void __launch_bounds__(64, kExternal ? kWsExternalCtasPerSm : kTrack ? 2 * kWsTrackCtasPerSm : kWsCtasPerSm)
 k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ mask,
                                                         int16_t* __restrict__ actions, int8_t* __restrict__ reward,
                                                         uint8_t* __restrict__ done, uint16_t* __restrict__ obs,
@@ -113,7 +115,7 @@ k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ ma
                                                         uint32_t* __restrict__ f_obs, uint32_t version, HistSlot hs,
                                                         int* __restrict__ err, int wait_prior,
                                                         const uint32_t* __restrict__ gather_flag, uint32_t gather_number) {
-  constexpr int kWsStages = WsShape<kExternal, kChase || kTrack>::kStages;
+  constexpr int kWsStages = WsShape<kExternal, kTrack>::kStages;
   __shared__ __align__(16) uint32_t s_stage[kWsStages][kWsStageWords];
   __shared__ __align__(8) uint2 s_lut[16];
   // strat_step_observe runs 3 CTAs per SM and has shared memory to spare: a byte -> 8 x bf16 table (one
