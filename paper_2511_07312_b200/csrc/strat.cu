@@ -425,7 +425,7 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
   if (!env || !out || ((uintptr_t)out & 7) != 0) return STRAT_BAD_ARG;
   if (!env->P.track) return STRAT_BAD_STATE;
   chain_break(env);
-  int ctas = env->P.num_games < 12 * env->num_sms ? env->P.num_games : 12 * env->num_sms;  // 12 x 17.8 KB of shared memory per SM
+  int ctas = env->P.num_games < kInfoCtasPerSm * env->num_sms ? env->P.num_games : kInfoCtasPerSm * env->num_sms;
   k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out, env->f_obs + batches(env->P.num_games));
   return launch_status();
 }

@@ -900,28 +900,38 @@ __device__ __forceinline__ void info_store(uint16_t* __restrict__ out, int gi, c
   }
 }
 
-// CTA = one BUILDER warp + one STORER warp sharing two stages (full / empty mbarriers, as in the
-// fused step): the storer streams game k out while the builder prepares game k+1, so the HBM
-// write stream of an SM (twelve such pairs) never waits for a build.  Games are handed out by a
+// CTA = one BUILDER warp + one STORER warp handing a staged game back and forth (full / empty mbarriers, as
+// in the fused step); twenty such pairs per SM, so the HBM write stream of an SM never waits for a build.  Games are handed out by a
 // ticket counter, not by a fixed stride: the SMs do not all drain their stores at the same rate, and a
 // persistent grid with equal shares ends on its slowest SM (plain streaming stores on this GPU: 6.2 TB/s
 // with equal shares, 7.2-7.4 TB/s when every CTA fetches its next piece of work as it finishes one).
 // The counter cleans up after itself like the fused step's: atomicInc wraps to 0 after exactly
 // num_games draws (num_games - grid successful ones and one failing draw per CTA).
 constexpr int kInfoStageWords = kInfoAWords + 2 * kInfoBWords + kInfoSpecial + 1;  // 1,948
-constexpr int kInfoCtaWords = 2 * kInfoStageWords + kTrackWords + kLineWords;      // 4,440 words = 17,760 B
+// One stage and 20 CTAs per SM (48 registers, 10 KB of shared memory): 1.064 ms at 65,536 games; two stages
+// with 12 CTAs 1.085 ms, one stage with 12 / 16 CTAs 1.108 / 1.082 ms.
+#ifndef STRAT_INFO_STAGES
+#define STRAT_INFO_STAGES 1
+#endif
+#ifndef STRAT_INFO_CTAS
+#define STRAT_INFO_CTAS 20
+#endif
+constexpr int kInfoStages = STRAT_INFO_STAGES;
+constexpr int kInfoCtasPerSm = STRAT_INFO_CTAS;
+constexpr int kInfoCtaWords = kInfoStages * kInfoStageWords + kTrackWords + kLineWords;      // 4,440 words = 17,760 B with two stages
 static_assert(kInfoStageWords % 4 == 0, "16-byte aligned stages");
-__global__ void __launch_bounds__(64, 12) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
+__global__ void __launch_bounds__(64, kInfoCtasPerSm) k_encode_infostate(Params P, const uint32_t* __restrict__ lines,
                                                          uint16_t* __restrict__ out, uint32_t* __restrict__ ticket) {
   __shared__ __align__(16) uint32_t s_info[kInfoCtaWords];
-  __shared__ __align__(8) uint64_t s_full[2], s_empty[2];
-  __shared__ int s_game[2];
+  __shared__ __align__(8) uint64_t s_full[kInfoStages], s_empty[kInfoStages];
+  __shared__ int s_game[kInfoStages];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (threadIdx.x == 0) { mbar_init(&s_full[0], 32); mbar_init(&s_full[1], 32); mbar_init(&s_empty[0], 32); mbar_init(&s_empty[1], 32); }
+  if (threadIdx.x == 0)
+    for (int s = 0; s < kInfoStages; ++s) { mbar_init(&s_full[s], 32); mbar_init(&s_empty[s], 32); }
   __syncthreads();
   int gi = blockIdx.x;  // grid <= num_games
   for (int it = 0;; ++it) {
-    const int stage = it & 1, round = it >> 1;
+    const int stage = it % kInfoStages, round = it / kInfoStages;
     const InfoStage st = info_stage(s_info + stage * kInfoStageWords);
     if (warp == 0) {
       if (round > 0) mbar_wait(&s_empty[stage], (uint32_t)(round - 1) & 1u);
@@ -933,7 +943,7 @@ __global__ void __launch_bounds__(64, 12) k_encode_infostate(Params P, const uin
       }
       if (lane == 0) s_game[stage] = gi;
       if (gi >= 0) {
-        info_build(P, lines, gi, st, s_info + 2 * kInfoStageWords, s_info + 2 * kInfoStageWords + kTrackWords, lane);
+        info_build(P, lines, gi, st, s_info + kInfoStages * kInfoStageWords, s_info + kInfoStages * kInfoStageWords + kTrackWords, lane);
         __syncwarp();
       }
       mbar_arrive(&s_full[stage]);
