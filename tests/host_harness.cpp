@@ -1,9 +1,9 @@
-// Test harness: the per-game device logic (strat_game.cuh) compiled for the HOST with
-// STRAT_HOST_DEBUG, so that the CPU-only test run can compare it with the oracle.  Test
+// Test harness: the per-game device logic (strat_game.cuh) compiled for the HOST on top of
+// tests/host_shim.h, so that the CPU-only test run can compare it with the oracle.  Test
 // infrastructure only: nothing in the product loads this; there is no CPU path in the library.
-#define STRAT_HOST_DEBUG
 #include <cstdint>
 #include <cstring>
+#include "host_shim.h"
 #include "../paper_2511_07312_b200/csrc/strat_game.cuh"
 
 using namespace strat;

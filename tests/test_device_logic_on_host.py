@@ -1,6 +1,6 @@
 """The per-game device logic (csrc/strat_game.cuh: setup, legal mask, both samplers, step with
 battle / terminal tests / auto-reset, chasing rule, observation bits) compiled for the HOST
-(tests/host_harness.cpp, STRAT_HOST_DEBUG) and compared with the oracle - so that the CPU-only
+(tests/host_harness.cpp on top of tests/host_shim.h) and compared with the oracle - so that the CPU-only
 test run already checks the rules the kernels execute, thread per game.  The kernels themselves
 (staging, warp-cooperative paths, overlap) are covered by the `-m gpu` tests."""
 import ctypes as C
