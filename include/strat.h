@@ -67,6 +67,7 @@ extern "C" {
 #define STRAT_BAD_STATE (-2)
 #define STRAT_CUDA_ERROR (-3)
 #define STRAT_ILLEGAL_ACTION (-4)
+#define STRAT_TOO_LARGE (-5)   /* more games than the built-in scratch of strat_legal_mask_static holds */
 
 #define STRAT_LINE_BYTES 128
 #define STRAT_MASK_WORDS 113
@@ -412,6 +413,41 @@ int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed,
  * Paper's values: alpha = 0.002, beta = 0.02, 1,000 rollouts of depth 40 (Table S12). */
 int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
                         float alpha, float beta, float* qhat, float* rho, float* pi_search, void* stream);
+
+/* ---- legal masks of given positions, for callers that cannot allocate device memory ---- */
+/* Everything above works on a workspace the caller allocates.  Some callers have no way to do that:
+ * code that is handed nothing but its input and output buffers by the framework it is plugged into
+ * (an operator or inference-server plugin, a data-loader stage) and has no access to that framework's
+ * allocator; a step in a latency-critical loop, where cudaMalloc / cudaFree would stall the whole
+ * device (both synchronise it); a thread that must not touch the allocator because another thread
+ * of the process is capturing a stream in the global capture mode, which forbids cudaMalloc
+ * process-wide.  For them this one call computes ComputeLegalActionMask (rules
+ * PAPER.md:210-212) for up to STRAT_STATIC_MAX_GAMES given positions with no environment, no
+ * workspace and no allocation of any kind (no cudaMalloc, cudaFree or allocating library routine,
+ * neither here nor in anything it calls): the bit-sliced state lines the mask kernel reads - what
+ * strat_reset_from builds in the workspace - go to a fixed array inside the library's device image
+ * (STRAT_STATIC_MAX_GAMES x 128 B of lines + 256 B holding the error word = 512.25 KB, held by every
+ * GPU that loads libstrat.so until the process exits).
+ *
+ *   boards  in   uint8[num_games][128] canonical lines (device), as for strat_reset_from
+ *   mask    out  uint32[num_games][113] (device): exactly what strat_reset_from + strat_legal_mask
+ *                of an environment with this two_square (and chase_rule = 0) write for these boards
+ *   status  out  int32[1] (device), or NULL: 0, or STRAT_BAD_STATE if a line gives one side more
+ *                than 8 Scouts (what strat_check reports after strat_reset_from); valid in stream order
+ *   returns STRAT_TOO_LARGE for num_games > STRAT_STATIC_MAX_GAMES (nothing is launched; split the
+ *           batch), STRAT_BAD_ARG for a NULL boards / mask or num_games < 1
+ *
+ * It runs on the CURRENT device; `stream` must belong to it.  The first call on each device looks up
+ * where the array lives on that device (cudaGetSymbolAddress; it may also make the driver load the
+ * library's device code): make that first call outside any stream capture, e.g. once at start-up.
+ * All calls on one device share the one array, and it keeps what the last call left in it: the call
+ * itself clears the error word and overwrites the lines it uses, so the caller clears nothing - but
+ * two calls that can run at the same time on one GPU (different streams without an event between
+ * them, different host threads or processes sharing a context) race on it and corrupt each other's
+ * masks.  Issue them on one stream, or order them with events. */
+#define STRAT_STATIC_MAX_GAMES 4096
+int strat_legal_mask_static(const uint8_t* boards, int32_t num_games, int32_t two_square, uint32_t* mask,
+                            int32_t* status, void* stream);
 
 /* ---- measurement aid ---------------------------------------------------------------- */
 /* Streams a constant over dst[0, bytes) with the store instruction the step kernels use for their

@@ -14,7 +14,8 @@ LINE = 128
 MASK_WORDS = 113
 OBS_ELEMS = 4400
 INFO_PLANES = 487
-OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION = 0, -1, -2, -3, -4
+OK, BAD_ARG, BAD_STATE, CUDA_ERROR, ILLEGAL_ACTION, TOO_LARGE = 0, -1, -2, -3, -4, -5
+STATIC_MAX_GAMES = 4096  # STRAT_STATIC_MAX_GAMES
 
 EXPORTS = [
     "strat_error_string", "strat_workspace_bytes", "strat_create", "strat_destroy", "strat_reset",
@@ -25,7 +26,7 @@ EXPORTS = [
     "strat_replay_locate", "strat_share_chain", "strat_replay_sample_chained", "strat_replay_push", "strat_replay_reserve",
     "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
-    "strat_reduce_returns", "strat_probe_write", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
+    "strat_reduce_returns", "strat_probe_write", "strat_legal_mask_static", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
     "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
     "strat_history_flags",
@@ -70,6 +71,7 @@ def lib():
         L.strat_encode_obs.argtypes = [vp, vp, vp]
         L.strat_encode_infostate.argtypes = [vp, vp, vp]
         L.strat_probe_write.argtypes = [vp, vp, sz, i32, i32, vp]
+        L.strat_legal_mask_static.argtypes = [vp, i32, i32, vp, vp, vp]
         L.strat_rollout_step.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_step_observe.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.strat_host_scratch_bytes.restype = sz
@@ -482,6 +484,28 @@ class History:
 
     def restore(self, t, env):
         _chk(lib().strat_history_restore(self.h, t, env.h, _stream()), "strat_history_restore")
+
+
+def legal_mask_static(boards, mask, two_square=1, status=None):
+    """strat_legal_mask_static: legal masks of the given canonical lines without an environment or a
+    workspace, for callers that cannot allocate device memory (a plugin that only gets its input and
+    output buffers, a loop that cannot afford cudaMalloc's device-wide stall, a process in which
+    another thread is capturing a stream in the global mode).  The library's scratch for this call is
+    a fixed 512.25 KB array inside its device image, so at most STATIC_MAX_GAMES positions per call
+    (StratError "more games than the built-in scratch holds" beyond that).  Nothing is allocated
+    here either: the caller passes every buffer, all on the current device -
+      boards  uint8[n][128]   in
+      mask    int32[n][113]   out, the same bits as Env.reset_from + Env.legal_mask
+      status  int32[1]        out, optional: 0, or BAD_STATE for a line with too many Scouts.
+    Calls share that one array: keep them on one stream (or order them with events); calls that
+    overlap on the GPU corrupt each other.  Make the first call on a device outside stream capture."""
+    _require_cuda()
+    n = boards.shape[0]
+    assert boards.shape == (n, LINE) and mask.shape == (n, MASK_WORDS)
+    assert status is None or status.numel() == 1
+    _chk(lib().strat_legal_mask_static(_ptr(boards, torch.uint8), n, 1 if two_square else 0, _ptr(mask, torch.int32),
+                                       _ptr(status, torch.int32), _stream()), "strat_legal_mask_static")
+    return mask
 
 
 def determinise(roots: Env, samples_per_root: int, seed: int, out: Env):

@@ -243,6 +243,7 @@ const char* strat_error_string(int code) {
     case STRAT_BAD_STATE: return "bad state";
     case STRAT_CUDA_ERROR: return "CUDA error";
     case STRAT_ILLEGAL_ACTION: return "illegal action for a live game";
+    case STRAT_TOO_LARGE: return "more games than the built-in scratch holds (STRAT_STATIC_MAX_GAMES)";
     default: return "unknown error";
   }
 }
@@ -936,3 +937,61 @@ int strat_reduce_returns(const strat_env* games, const uint8_t* root_side, int32
 }
 
 }  // extern "C"
+
+// ---- strat_legal_mask_static: the legal-mask query for callers that cannot allocate (strat.h) ----
+// The scratch of this one entry point is part of the library's device image instead of a caller's
+// workspace: kStaticLineBytes of device lines (what k_import writes and k_legal_mask reads), then a
+// 256-byte block whose first word is the error word k_import raises.  Every GPU that loads the
+// library holds these 512.25 KB until the process exits.
+//
+// In HOST code the name `g_static_scratch` is only a handle for the symbol, not a device address
+// (handing it to a kernel would fault, or quietly hit host memory on a system where the GPU can
+// reach it).  The address on a given device comes from cudaGetSymbolAddress with that device
+// current; static_scratch() asks once per device and remembers the answer.
+namespace {
+constexpr size_t kStaticLineBytes = (size_t)STRAT_STATIC_MAX_GAMES * STRAT_LINE_BYTES;
+constexpr int kStaticMaxDevices = 64;
+}  // namespace
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticLineBytes + 256];
+namespace {
+std::mutex g_static_mutex;
+unsigned char* g_static_addr[kStaticMaxDevices];  // device address of g_static_scratch per device ordinal, once known
+
+// Device address of the built-in scratch on the current device.  Looks it up on the first call
+// for that device (no allocation: the array already exists in the loaded module).
+int static_scratch(unsigned char** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return STRAT_CUDA_ERROR;
+  if (dev < 0 || dev >= kStaticMaxDevices) return STRAT_BAD_ARG;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_addr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || !p) return STRAT_CUDA_ERROR;
+    g_static_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_static_addr[dev];
+  return STRAT_OK;
+}
+}  // namespace
+
+extern "C" int strat_legal_mask_static(const uint8_t* boards, int32_t num_games, int32_t two_square, uint32_t* mask,
+                                       int32_t* status, void* stream) {
+  if (!boards || !mask || num_games < 1) return STRAT_BAD_ARG;
+  if (num_games > STRAT_STATIC_MAX_GAMES) return STRAT_TOO_LARGE;
+  unsigned char* base = nullptr;
+  int rc = static_scratch(&base);
+  if (rc != STRAT_OK) return rc;
+  uint32_t* lines = reinterpret_cast<uint32_t*>(base);
+  int* err = reinterpret_cast<int*>(base + kStaticLineBytes);
+  cudaStream_t s = (cudaStream_t)stream;
+  // the array still holds the previous call's lines and error word: the lines of games [0, num_games)
+  // are overwritten below and no kernel looks beyond them; the error word has to start at zero
+  k_set_int<<<1, 1, 0, s>>>(err, 0);
+  k_import<<<(num_games + 3) / 4, 128, 0, s>>>(num_games, boards, lines, err);
+  strat_config c = {};
+  c.num_games = num_games; c.two_square = two_square ? 1 : 0;
+  const Params P = make_params(c);  // the mask depends on num_games and two_square only (no chasing rule: no move log)
+  k_legal_mask<false><<<batches(num_games), 32, 0, s>>>(P, lines, mask);
+  if (status) k_copy<int><<<1, 1, 0, s>>>(err, status, (size_t)1);
+  return launch_status();
+}
