@@ -853,11 +853,13 @@ __device__ __forceinline__ void info_build(const Params& P, const uint32_t* __re
 __device__ __forceinline__ void info_store(uint16_t* __restrict__ out, int gi, const InfoStage& st, int lane) {
   const uint32_t* A = st.A; const uint32_t* Bs = st.Bs; const uint32_t* Cs = st.Cs; const uint32_t* val = st.val;
   // ---- store: nibble n of the streams -> cells 4n..4n+3 of the game, two nibbles (16 bytes) per
-  // lane and streaming store.  A game starts 8-byte aligned (odd games at 8 mod 16), so an odd
-  // game's first nibble and an even game's last one go out alone.  Bits -> bf16 in registers:
-  // two bits spread to bit 0 and bit 16, times 0x3F80 (or times the plane's value).
-  const int odd = gi & 1;
+  // lane and streaming store.  `out` is 8-byte aligned and a game is 97,400 B = 8 mod 16, so every
+  // other game starts at 8 mod 16: such a game's first nibble goes out alone, the others' last one.
+  // Which games those are is read off the game's address (`out` itself may be a slice that starts at
+  // 8 mod 16).  Bits -> bf16 in registers: two bits spread to bit 0 and bit 16, times 0x3F80 (or
+  // times the plane's value).
   uint16_t* gout = out + (size_t)gi * (kInfoPlanes * 100);
+  const int odd = (int)((reinterpret_cast<uintptr_t>(gout) >> 3) & 1u);
   uint4* dst = reinterpret_cast<uint4*>(gout + 4 * odd);  // pair k = nibbles 2k+odd, 2k+odd+1
   auto spread = [](uint32_t t) { return (t & 1u) | ((t & 2u) << 15); };
   auto nib_value = [&](int n) -> uint2 {  // any nibble, valued planes included

@@ -151,6 +151,28 @@ def test_infostate_after_loads_restores_and_pinned_restarts():
     assert g.check() == 0
 
 
+def test_infostate_into_a_buffer_at_8_mod_16():
+    """`out` need only be 8-byte aligned (strat.h).  A game is 97,400 B = 8 mod 16, so big[1:] of a larger
+    tensor starts at 8 mod 16 and the games whose first nibble goes out alone are the even ones there."""
+    n = 77
+    kw = dict(variant=0, seed=4, max_plies=60, auto_reset=1, infostate=1)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for _ in range(75):
+        g.rollout_step(mask, act, rew, done, obs)
+        o.step(o.sample_uniform(o.legal_mask()))
+    big = torch.full((n + 2, 487, 10, 10), 7.0, dtype=torch.bfloat16, device="cuda")
+    out = big[1:n + 1]
+    assert out.data_ptr() % 16 == 8 and out.is_contiguous()
+    g.encode_infostate(out)
+    want = o.encode_infostate().reshape(n, 487, 100)
+    got = _info_np(out).reshape(n, 487, 100)
+    assert np.array_equal(got, want), _diff(got, want)
+    assert torch.equal(out.view(torch.int16), g.encode_infostate().view(torch.int16))   # = the 16-byte aligned call
+    assert bool((big[0] == 7.0).all()) and bool((big[n + 1] == 7.0).all())               # neighbours untouched
+    assert g.check() == 0
+
+
 def test_infostate_argument_errors():
     L, s = B.lib(), B._stream()
     plain = B.Env(40, seed=1)
