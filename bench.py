@@ -154,8 +154,37 @@ def oracle_rate_all_cores(num_games, steps, warmup):
     return cores * num_games * steps / max(max(times), 1e-9), cores, wall
 
 
+def launch_ranks(args):
+    """`python bench.py --gpus N` with N > 1 and no launcher around it (the paper
+    runs 16 data-parallel GPUs): start N ranks of this same command line under
+    torch.distributed.run on 127.0.0.1, one per GPU, and hand back its exit code.  Every rank then runs
+    main() again with WORLD_SIZE set and takes the sharded path."""
+    import socket
+    import subprocess
+    if args.impl == "b200":
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit("bench.py: --gpus %d but this node has %d CUDA device(s)" % (args.gpus, have))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:  # every rank reports in (gloo, CPU), then rank 0 alone works and prints
+        import torch
+        import torch.distributed as dist
+        dist.init_process_group("gloo")
+        seen = torch.ones(1, dtype=torch.int64)
+        dist.all_reduce(seen)
+        dist.destroy_process_group()
+        world = int(seen.item())
     if rank != 0:
         return
     # each step = one pass of the oracle over a bounded sample of the 65,536-game workload,
@@ -169,7 +198,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1000.0 * dt / max(args.steps, 1), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-        "config": {"workload": CFG["name"], "games_per_step": games, "parallelism": "1 host core"},
+        "config": {"workload": CFG["name"], "games_per_step": games, "parallelism": "1 host core", "ranks_started": world},
         "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -267,6 +296,12 @@ def run_b200(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms_max = float(t.item())
     value = world * n * args.steps / (total_ms_max / 1e3)
+    per_rank_ms = [total_ms / args.steps]
+    if world > 1:
+        mine = torch.tensor([total_ms / args.steps], dtype=torch.float64, device="cuda")
+        every = [torch.zeros_like(mine) for _ in range(world)]
+        dist.all_gather(every, mine)
+        per_rank_ms = [float(x.item()) for x in every]
 
     # outside the timed region (the steps that follow it): sanity statistics of the workload
     # (SURVEY.md section 5 "Metrics"): games ended per step, why, how long they were, legal moves
@@ -339,6 +374,7 @@ def run_b200(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms_max / args.steps, "median_ms_per_step": median_ms, "higher_is_better": True,
+            "ms_per_step_per_rank": per_rank_ms,
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": CFG["name"], "games_per_gpu": n, "variant": "classic", "max_plies": CFG["max_plies"],
                        "auto_reset": 1, "chase_rule": 1 if args.chase_rule else 0,
@@ -752,6 +788,10 @@ def main():
                     help="profiling runs (ncu --replay-mode range): after the warm-up, "
                          "K back-to-back fused steps between cudaProfilerStart/Stop, nothing else; prints no bench line")
     args = ap.parse_args()
+    if args.gpus > 1 and args.impl == "b200" and (args.workload != "cfg2" or args.profile_range):
+        raise SystemExit("bench.py: --gpus > 1 is the sharded headline workload (cfg2) only; the other workloads are 1-GPU lines")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_ranks(args))
     if args.profile_range:
         run_profile_range(args)
     elif args.impl == "reference":

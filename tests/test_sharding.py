@@ -89,3 +89,26 @@ def test_sharded_oracle_plumbing_equals_one_oracle():
             assert np.array_equal(sh.obs, one.encode_obs().reshape(n, -1)), t
             assert np.array_equal(sh.boards, one.get_boards()), t
         assert np.array_equal(sh.get_boards(), one.get_boards())
+
+
+def test_bench_gpus_n_starts_n_ranks_by_itself():
+    """`python bench.py --gpus 2` with no launcher around it re-executes itself under torch.distributed.run
+    with two ranks on 127.0.0.1.  Checked without a GPU on the reference arm: both
+    ranks report in over gloo, rank 0 alone times the oracle and prints the one JSON line."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2",
+                          "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(x) for x in out.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1
+    assert lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+    assert lines[0]["config"]["ranks_started"] == 2
+    assert lines[0]["value"] > 0
+    # a workload that does not shard says so instead of starting ranks
+    bad = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--workload", "cfg4"],
+                         capture_output=True, text=True, timeout=120, env=env, cwd=root)
+    assert bad.returncode != 0 and "cfg2" in bad.stderr
