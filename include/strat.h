@@ -137,7 +137,7 @@ int strat_reset_from(strat_env* env, const uint8_t* boards, void* stream);
  * to be tested against the history of board states that leads to the non-initial reset state"):
  * plies uint8[N][63][2] (device) = (from, to) squares, most recent first, 0xFF,0xFF = unknown; the
  * leading known ones become the game's move log, as if they had been played here (the first 8
- * repeat the line's own history).  Without chase_rule nothing remembers plies: same as
+ * repeat the line's own history); an entry with a square >= 100 counts as unknown.  Without chase_rule nothing remembers plies: same as
  * strat_reset_from. */
 int strat_reset_from_with_plies(strat_env* env, const uint8_t* boards, const uint8_t* plies, void* stream);
 int strat_get_boards(const strat_env* env, uint8_t* boards, void* stream);

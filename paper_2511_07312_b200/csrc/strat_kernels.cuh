@@ -664,15 +664,16 @@ __global__ void __launch_bounds__(256) k_clear_logn(int n, uint32_t* __restrict_
 }
 
 // The plies that led to loaded states: plies uint8[n][63][2] (from, to), most recent first,
-// 0xFF = unknown.  K = the leading known ones; ply b back goes to log entry (K - b) mod 64 and word
+// 0xFF = unknown.  K = the leading known ones (both squares < 100: a malformed entry would otherwise become a
+// log entry that collides with a real ply in the chasing rule's walk); ply b back goes to log entry (K - b) mod 64 and word
 // 31 of the line becomes K, exactly what K played plies would have left.
 __global__ void __launch_bounds__(256) k_load_plies(int n, const uint8_t* __restrict__ plies, uint32_t* __restrict__ lines,
                                                     uint16_t* __restrict__ logs) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
   const uint8_t* p = plies + (size_t)g * (2 * (kLogPlies - 1));
-  int K = 0;
-  while (K < kLogPlies - 1 && p[2 * K] != 0xFFu) ++K;
+  int K = 0;  // an entry that names no square (0xFF = unknown, or anything else >= 100) ends the known plies
+  while (K < kLogPlies - 1 && p[2 * K] < 100u && p[2 * K + 1] < 100u) ++K;
   uint16_t* glog = logs + (size_t)g * kLogPlies;
   for (int b = 1; b <= K; ++b)
     glog[(K - b) & (kLogPlies - 1)] = (uint16_t)((uint32_t)p[2 * (b - 1)] | ((uint32_t)p[2 * (b - 1) + 1] << 7));

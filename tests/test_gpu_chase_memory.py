@@ -76,6 +76,39 @@ def test_lap_split_across_a_load_with_plies():
     assert g.check() == B.ILLEGAL_ACTION
 
 
+def test_malformed_plies_end_the_known_plies():
+    """A ply with a square >= 100 (or a known `from` with `to` = 0xFF) names no move: it ends the known
+    plies exactly like 0xFF,0xFF instead of becoming a log entry that collides with a real one."""
+    _, lap, plies, _ = _lap()
+    n = 5
+    bad = np.repeat(plies[None], n, axis=0)
+    bad[0, 20] = (100, 5); bad[1, 20] = (37, 0xFF); bad[2, 20] = (200, 201); bad[3, 0] = (44, 130)   # game 4: intact
+    cut = np.repeat(plies[None], n, axis=0)
+    cut[0:3, 20:] = 0xFF; cut[3, :] = 0xFF
+    lines = np.repeat(lap[None], n, axis=0)
+    g, ref, o = B.Env(n, chase_rule=1), B.Env(n, chase_rule=1), orc.Env(n, chase_rule=1)
+    g.reset_from(_dev(lines), _dev(bad)); ref.reset_from(_dev(lines), _dev(cut)); o.reset_from(lines, cut)
+    assert torch.equal(g.legal_mask(), ref.legal_mask())
+    assert np.array_equal(_mask_np(g.legal_mask()), o.legal_mask())
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for _ in range(30):
+        om = o.legal_mask(); oa = o.sample_uniform(om); o.step(oa)
+        g.rollout_step(mask, act, rew, done, obs)
+        assert np.array_equal(_mask_np(mask), om) and np.array_equal(_np(act), oa)
+    assert g.check() == 0
+    # the same through a pin
+    pin = B.Env(n, chase_rule=1, max_plies=30, auto_reset=1, seed=5)
+    pin_ref = B.Env(n, chase_rule=1, max_plies=30, auto_reset=1, seed=5)
+    pin.pin_reset_state(_dev(lines), _dev(bad)); pin_ref.pin_reset_state(_dev(lines), _dev(cut))
+    pin.reset_from(_dev(lines), _dev(bad)); pin_ref.reset_from(_dev(lines), _dev(cut))
+    m2 = pin_ref.new_mask()
+    for _ in range(20):  # restarts from the pin inside (the ply cap ends every game after 6 plies)
+        pin.rollout_step(mask, act, rew, done, obs)
+        pin_ref.rollout_step(m2, act, rew, done, obs)
+        assert torch.equal(mask, m2)
+    assert torch.equal(pin.get_boards(), pin_ref.get_boards())
+
+
 @pytest.mark.parametrize("with_plies", [True, False])
 def test_pinned_restart_remembers_the_plies_of_its_pin(with_plies):
     extra = {8: W.piece(W.MINER, W.RED), 98: W.piece(W.MINER, W.BLUE)}
