@@ -195,7 +195,7 @@ k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ ma
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);  // also: every lane is done with its mask row
-        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); __syncwarp(); }  // owner lanes' tracker writes first
         else if (rs) coop_setup(P, first, rs, g, work, lane);
         if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
         if (lane < ng) store_game_global(lines, first + lane, g);
@@ -213,7 +213,7 @@ k_rollout_step(Params P, uint32_t* __restrict__ lines, uint32_t* __restrict__ ma
           reset_me = o.needs_reset;
         }
         uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
-        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+        if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); __syncwarp(); }  // owner lanes' tracker writes first
         else if (rs) coop_setup(P, first, rs, g, work, lane);  // borrows the stage; the bit streams overwrite it
         if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
         if (lane < ng) store_game_global(lines, first + lane, g);

@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(32) k_step(Params P, uint32_t* __restrict__ li
     reset_me = o.needs_reset;
   }
   uint32_t rs = __ballot_sync(0xffffffffu, reset_me);
-  if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); }
+  if (rs && P.pin) { if (reset_me) reset_game(P, (uint32_t)(first + lane), g); __syncwarp(); }  // owner lanes' tracker writes first
   else if (rs) coop_setup(P, first, rs, g, s_scratch, lane);
   if (kTrack && rs && P.track) coop_track_start(P, first, rs, g, lane);
   if (lane < ng) write_game(s_state, lane, g);
@@ -430,7 +430,8 @@ __device__ __forceinline__ bool replay_gather_one(int j, int lane, uint32_t k0, 
           while ((int32_t)(ld_acquire(chain.f_obs + b) - (need - 1u)) < 0) __nanosleep(64);
         }
       }
-      ready = __shfl_sync(0xffffffffu, ready, 0);  // also orders the other lanes behind lane 0's acquire
+      ready = __shfl_sync(0xffffffffu, ready, 0);
+      __syncwarp();  // the other lanes' loads of the record come after lane 0's acquire (a shuffle alone orders no memory)
       if (!ready) return false;
     }
   }
