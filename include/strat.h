@@ -122,7 +122,9 @@ int strat_destroy(strat_env* env);
  * each other as plain stream order.  Without it only consecutive fused steps of the SAME
  * environment overlap (ordered batch by batch), and a fused step is ordered against everything
  * else the library was asked to do with its environment; fused steps of two unrelated
- * environments issued back to back on one stream may overlap on the device. */
+ * environments issued back to back on one stream may overlap on the device.  `b` joins the group of
+ * `a`; a group grows one lone environment at a time: STRAT_BAD_STATE if `b` already shares its
+ * ordering with other environments (they would be left unordered against the group of `a`). */
 int strat_share_chain(strat_env* a, strat_env* b);
 
 /* All games: new Philox key, epoch 0, ply 0, fresh setups. */
@@ -312,7 +314,9 @@ int strat_replay_sample(const strat_replay* r, uint64_t seed, uint64_t draw_inde
  * else (a copy push, another call on the environment, the first gather) it waits for the whole stream
  * before it.  The fused step after the NEXT gather waits for this one before it reuses ring rows (the
  * ring's spare rows cover exactly that distance), and a gather waits for the one before it before it
- * overwrites the minibatch buffers.  One ring serves one environment this way; outputs are valid in
+ * overwrites the minibatch buffers.  One ring serves one environment this way and one environment
+ * feeds one ring (STRAT_BAD_ARG for a ring tied to another environment, STRAT_BAD_STATE for an
+ * environment another live ring is tied to; strat_replay_destroy unties); outputs are valid in
  * stream order as usual.  STRAT_BAD_STATE on a plain or empty ring. */
 int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, uint64_t draw_index, int32_t batch,
                                 uint16_t* obs, uint32_t* mask, int16_t* action, int8_t* reward, uint8_t* done,

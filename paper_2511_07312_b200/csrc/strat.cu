@@ -300,6 +300,10 @@ int strat_destroy(strat_env* env) {
 
 int strat_share_chain(strat_env* a, strat_env* b) {
   if (!a || !b) return STRAT_BAD_ARG;
+  if (a->chain == b->chain) return STRAT_OK;
+  // b joins a's group.  If b already shared its record with other environments, re-pointing b alone
+  // would leave those unordered against a's group: groups grow one lone environment at a time.
+  if (b->chain.use_count() > 1) return STRAT_BAD_STATE;
   chain_break(a); chain_break(b);
   b->chain = a->chain;
   return STRAT_OK;
@@ -691,6 +695,9 @@ int strat_replay_sample_chained(strat_replay* r, strat_env* env, uint64_t seed, 
   if (!r || !env || batch <= 0) return STRAT_BAD_ARG;
   if (r->filled == 0 || r->rows < r->capacity + 1) return STRAT_BAD_STATE;  // in-place rings only (spare rows)
   if (r->env && r->env != env) return STRAT_BAD_ARG;
+  // the environment's fused steps wait for the gathers of ONE ring (env->chained): a second ring tied to it
+  // would silently take that slot over and the first ring's rows would be rewritten while its gather reads them
+  if (!r->env && env->chained && env->chained != r) return STRAT_BAD_STATE;
   cudaStream_t s = (cudaStream_t)stream;
   if (!r->env) {  // first chained gather: clear the synchronisation words, tie the ring to the environment
     if (cudaMemsetAsync(r->sync, 0, 256, s) != cudaSuccess) return STRAT_CUDA_ERROR;

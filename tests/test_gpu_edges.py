@@ -122,6 +122,43 @@ def test_argument_errors_and_empty_inputs():
     assert g.check() == 0
 
 
+def test_one_chained_ring_per_environment_and_groups_grow_one_by_one():
+    """strat_replay_sample_chained: the environment's fused steps wait for the gathers of ONE ring, so a second
+    live ring is refused instead of silently taking the first one's place.  strat_share_chain(a, b): b joins
+    a's group only while b shares its ordering with nobody else."""
+    n = 64
+    g = B.Env(n, seed=2, max_plies=50, auto_reset=1)
+    r1, r2 = B.Replay(32, 8, block=n), B.Replay(32, 8, block=n)
+    act, rew, done = g.new_actions(), g.new_reward(), g.new_done()
+    bs = 16
+    so = torch.empty((bs, 44, 10, 10), dtype=torch.bfloat16, device="cuda")
+    sm = torch.empty((bs, 113), dtype=torch.int32, device="cuda")
+    sa = torch.empty(bs, dtype=torch.int16, device="cuda")
+    sr = torch.empty(bs, dtype=torch.int8, device="cuda")
+    sd = torch.empty(bs, dtype=torch.uint8, device="cuda")
+    for ring in (r1, r2):
+        o_ptr, m_ptr = ring.reserve(n, 0)
+        g.rollout_step_raw(m_ptr, act, rew, done, o_ptr)
+        ring.commit(act, rew, done)
+    r1.sample_chained(g, 1, 0, bs, so, sm, sa, sr, sd)
+    with pytest.raises(B.StratError, match="bad state"):
+        r2.sample_chained(g, 1, 0, bs, so, sm, sa, sr, sd)
+    r1.sample_chained(g, 1, 1, bs, so, sm, sa, sr, sd)   # the first ring goes on
+    torch.cuda.synchronize()
+    del r1                                               # strat_replay_destroy unties the environment
+    r2.sample_chained(g, 1, 0, bs, so, sm, sa, sr, sd)
+    torch.cuda.synchronize()
+    assert g.check() == 0
+    a, b, c, d = (B.Env(8, seed=k) for k in range(4))
+    a.share_chain(b)
+    a.share_chain(b)                                     # already one group: nothing to do
+    a.share_chain(c)                                     # a lone environment joins
+    d.share_chain(d)
+    with pytest.raises(B.StratError, match="bad state"):
+        d.share_chain(b)                                 # b shares with a and c: they would be left behind
+    b.share_chain(d)                                     # the other way round d joins the group
+
+
 def test_sample_uniform_is_uniform_over_the_legal_set():
     """Chi-square of the sampled rank r = position of the action inside its mask, over many
     seeds on one position (the closed form: every legal action has probability 1/n)."""
