@@ -211,7 +211,9 @@ int strat_encode_obs(const strat_env* env, uint16_t* obs, void* stream);
  *   455-486  move t-1-j (j = 0..31): +1.0 on its destination, -1.0 on its source
  * The trackers start with the game (reset, auto-reset) or with a loaded position
  * (strat_reset_from, a pinned restart, strat_history_restore: the squares the pieces stand on
- * then count as their start squares, the line's 8-ply history as the known moves). */
+ * then count as their start squares, the line's 8-ply history as the known moves).
+ * Calls for one environment on different streams may run at the same time (each takes a work
+ * counter of its own); they read the state, so order them against the steps as usual. */
 int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream);
 
 /* One fused pass of the hot path: legal mask -> uniform legal action -> step -> encode of
@@ -460,7 +462,8 @@ int strat_legal_mask_static(const uint8_t* boards, int32_t num_games, int32_t tw
  * Persistent CTAs; dynamic = 1: every CTA fetches its next piece from a ticket counter as it finishes
  * one (how the step kernels hand out batches), 0: equal shares by a fixed stride.  On a B200 the two
  * differ by ~17 % (7.2-7.4 against 6.2 TB/s): the SMs do not drain their stores at one rate.  The
- * environment lends its ticket word and SM count; nothing of it is touched. */
+ * environment lends its ticket word and SM count; nothing of it is touched.  One probe at a time per
+ * environment: two in flight would draw from the same ticket word. */
 int strat_probe_write(const strat_env* env, void* dst, size_t bytes, int32_t chunk_bytes, int32_t dynamic, void* stream);
 
 #ifdef __cplusplus

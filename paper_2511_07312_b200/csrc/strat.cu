@@ -58,7 +58,9 @@ inline int batches(int n) { return (n + kBatch - 1) / kBatch; }
 // flight holds at least one of the <= 32 x SMs resident CTA slots, so far fewer than kTicketRing
 // launches are ever in flight and two launches never share a ticket counter.
 constexpr int kTicketRing = 8192;
-constexpr int kOtherTickets = 64;  // self-resetting work counters of the other persistent kernels (word 0: strat_encode_infostate)
+constexpr int kOtherTickets = 64;  // self-resetting work counters of the other persistent kernels: word 1 strat_probe_write,
+                                   // words 2..63 strat_encode_infostate, one per call in rotation (calls on different streams
+                                   // may be in flight together; 62 at once is more than the GPU holds resident)
 inline size_t sync_words(int n) { return (size_t)kTicketRing + 2 * (size_t)batches(n) + kOtherTickets; }
 
 template <typename T>
@@ -107,6 +109,7 @@ struct strat_env {
   int num_sms;
   strat_history* hist;   // attached board-history ring, or nullptr
   strat_replay* chained; // ring whose gathers run chained between this environment's fused steps, or nullptr
+  mutable uint32_t info_calls;  // strat_encode_infostate calls so far: picks the call's work counter
 };
 
 // Circular buffer of `length` time steps: per step N device lines + N x
@@ -274,6 +277,7 @@ int strat_create(const strat_config* cfg, void* workspace_dev, size_t bytes, voi
   e->version = 0;
   e->hist = nullptr;
   e->chained = nullptr;
+  e->info_calls = 0;
   uint8_t* extra = reinterpret_cast<uint8_t*>(e->tickets) + align_up(sync_words(cfg->num_games) * 4, 256);
   if (cfg->chase_rule) {
     e->P.movelog = reinterpret_cast<uint16_t*>(extra);
@@ -431,7 +435,8 @@ int strat_encode_infostate(const strat_env* env, uint16_t* out, void* stream) {
   if (!env->P.track) return STRAT_BAD_STATE;
   chain_break(env);
   int ctas = env->P.num_games < kInfoCtasPerSm * env->num_sms ? env->P.num_games : kInfoCtasPerSm * env->num_sms;
-  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out, env->f_obs + batches(env->P.num_games));
+  uint32_t* ticket = env->f_obs + batches(env->P.num_games) + 2 + (env->info_calls++ % (uint32_t)(kOtherTickets - 2));
+  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(env->P, env->lines, out, ticket);
   return launch_status();
 }
 

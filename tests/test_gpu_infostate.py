@@ -173,6 +173,36 @@ def test_infostate_into_a_buffer_at_8_mod_16():
     assert g.check() == 0
 
 
+def test_infostate_encodes_in_flight_together_on_two_streams():
+    """Two strat_encode_infostate calls of one environment on two streams, more games than the encoder has
+    CTAs (games handed out by ticket): each call draws from a work counter of its own, so neither skips
+    or repeats a game, and the counters are back at zero for the next round."""
+    n = 20000
+    g = B.Env(n, variant=0, seed=8, max_plies=40, auto_reset=1, infostate=1)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    for _ in range(50):
+        g.rollout_step(mask, act, rew, done, obs)
+    want = g.encode_infostate().view(torch.int16)
+    outs = [g.new_infostate(), g.new_infostate()]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for rnd in range(70):   # more rounds than there are counters: the rotation wraps
+        for out, st in zip(outs, streams):
+            if rnd % 10 == 0:
+                out.fill_(3.0)
+            st.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(st):
+                g.encode_infostate(out)
+        if rnd % 10 == 0:
+            torch.cuda.synchronize()
+            for out in outs:
+                assert torch.equal(out.view(torch.int16), want), rnd
+    torch.cuda.synchronize()
+    for out in outs:
+        assert torch.equal(out.view(torch.int16), want)
+    assert g.check() == 0
+
+
 def test_infostate_argument_errors():
     L, s = B.lib(), B._stream()
     plain = B.Env(40, seed=1)
