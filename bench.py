@@ -727,6 +727,7 @@ def run_hist(args):
     n, length = CFG["num_games"], 256
     env = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1)
     hist = B.History(n, length)
+    hist_bytes = hist.mem.numel()
     hist.attach(env)
     mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
     for _ in range(args.warmup):
@@ -752,17 +753,45 @@ def run_hist(args):
     assert env.check() == 0
     ms_step, ms_q = e[0].elapsed_time(e[1]) / args.steps, e[1].elapsed_time(e[2]) / q
     per_game = ALGO_BYTES_PER_GAME_STEP + 128 + 4  # + recorded state line + action/reward/done
+    # Side measurement, outside the timed region: the paper's own 487-channel information state of PAST steps
+    # (ComputeInfostateTensor(t)) from a tracked ring, which also keeps the 2 KB of S2
+    # trackers per game and step (a copy kernel in front of every recorded step).
+    del hist, env
+    tlen, tsteps, tq = 32, 48, 20
+    tenv = B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1, infostate=1)
+    thist = B.History(n, tlen, tracked=True)
+    thist.attach(tenv)
+    for _ in range(8):
+        tenv.rollout_step(mask, act, rew, done, obs)
+    info = tenv.new_infostate()
+    thist.encode_infostate(thist.current_step() - 1, info)
+    f = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    f[0].record()
+    for _ in range(tsteps):
+        tenv.rollout_step(mask, act, rew, done, obs)
+    f[1].record()
+    tcur = thist.current_step()
+    for k in range(tq):
+        thist.encode_infostate(tcur - 1 - (k * 7) % tlen, info)
+    f[2].record()
+    torch.cuda.synchronize()
+    assert tenv.check() == 0
+    ms_tstep, ms_q487 = f[0].elapsed_time(f[1]) / tsteps, f[1].elapsed_time(f[2]) / tq
+    q487_gbs = 97400.0 * n / (ms_q487 / 1e3) / 1e9
+    hist487 = dict(_peak_line(q487_gbs), call="strat_history_encode_infostate of a past step", ms_per_query=ms_q487,
+                   algorithmic_bytes_per_game=97400, ring_steps=tlen, ring_bytes=thist.mem.numel(),
+                   tracker_bytes_per_game_step=2048, ms_per_recorded_tracked_step=ms_tstep)
     line = {
         "metric": METRIC, "value": n / (ms_step / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u8", "data": "synthetic",
         "config": {"workload": CFG["name"] + " + board-history ring", "games_per_gpu": n, "history_steps": length,
-                   "history_bytes": hist.mem.numel(),
+                   "history_bytes": hist_bytes, "historical_infostate487": hist487,
                    "historical_query": "strat_history_legal_mask + strat_history_encode_obs of a past step",
                    "ms_per_historical_query": ms_q, "historical_game_queries_per_sec": n / (ms_q / 1e3)},
         "roofline": dict(_peak_line(per_game * n / (ms_step / 1e3) / 1e9), kernel="k_rollout_step (recording)",
                          algorithmic_bytes_per_game_step=per_game),
-        "gpu_launches": args.steps + 2 * q, "clocks": sampler.result(),
+        "gpu_launches": args.steps + 2 * q, "clocks": sampler.result(),  # timed region only
     }
     print(json.dumps(line))
 

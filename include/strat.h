@@ -342,6 +342,17 @@ typedef struct strat_history strat_history;
 size_t strat_history_bytes(int32_t num_games, int32_t length);
 int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, strat_history** out);
 int strat_history_destroy(strat_history* h);
+/* A TRACKED ring, for the paper's own information state at past time steps ("reconstruct
+ * on-demand past information states"; Table S1, PAPER.md:462 ComputeInfostateTensor(t)): next to the 132 B
+ * above it keeps, per game and time step, the 2 KB of trackers the 487 channels are built from
+ * (strat_config.infostate) - 46x less than the 97,400 B tensor itself.  Same handle, same calls; 256 B of
+ * work counters are cleared on `stream`.  While a tracked ring is attached to an environment with
+ * infostate = 1, every recorded step is preceded by one copy kernel (the trackers of the state it starts
+ * from), so consecutive fused steps do not overlap; with infostate = 0 nothing more is recorded and
+ * strat_history_encode_infostate returns STRAT_BAD_STATE. */
+size_t strat_history_bytes_tracked(int32_t num_games, int32_t length);
+int strat_history_create_tracked(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, void* stream,
+                                 strat_history** out);
 /* After attach, every strat_step / strat_rollout_step / strat_step_observe of `env` first records the state it
  * starts from, then the action, reward and done byte, and advances CurrentStep by one (the
  * fused step writes them itself: no copy kernel).  h == NULL detaches.  strat_rollout_uniform
@@ -358,6 +369,10 @@ int strat_history_current_step(const strat_history* h, int64_t* step);
 int strat_history_legal_mask(const strat_history* h, int64_t t, uint32_t* mask, void* stream);
 int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, void* stream);
 int strat_history_get_boards(const strat_history* h, int64_t t, uint8_t* boards, void* stream);
+/* ComputeInfostateTensor(t) in the paper's own 487 channels: what
+ * strat_encode_infostate wrote, or would have written, at time step t; layout and alignment as there.
+ * Tracked rings only (STRAT_BAD_STATE otherwise, and if the environment keeps no trackers). */
+int strat_history_encode_infostate(const strat_history* h, int64_t t, uint16_t* out, void* stream);
 /* GetPlayedActions(t), reward(t), done(t): NON-OWNING device pointers into the ring, valid
  * until `length` further steps have been recorded ("non-owning tensor"). */
 int strat_history_transition(const strat_history* h, int64_t t, const int16_t** actions, const int8_t** reward,
@@ -377,7 +392,9 @@ int strat_history_flags(const strat_history* h, int64_t t, uint8_t* two_square_a
                         int32_t* terminated_since, void* stream);
 /* Travel back: make the state at time step t the live state of `env` (which need not be the
  * attached one; "efficient capturing of past states", 252-254).  With chase_rule on in
- * both, the move log is restored with it, rebuilt as for strat_history_legal_mask. */
+ * both, the move log is restored with it, rebuilt as for strat_history_legal_mask.
+ * From a tracked ring (both environments with infostate = 1) the trackers of time step t travel back as
+ * well; otherwise they restart from the restored position as after strat_reset_from. */
 int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, void* stream);
 
 /* ---- search-shaped batch (BASELINE.json configs[4]) ------------------------------- */

@@ -27,6 +27,7 @@ EXPORTS = [
     "strat_replay_reserve_rows",
     "strat_replay_commit", "strat_replay_sample", "strat_replay_state", "strat_determinise",
     "strat_reduce_returns", "strat_probe_write", "strat_legal_mask_static", "strat_history_bytes", "strat_history_create", "strat_history_destroy",
+    "strat_history_bytes_tracked", "strat_history_create_tracked", "strat_history_encode_infostate",
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
     "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
     "strat_history_flags",
@@ -107,6 +108,10 @@ def lib():
         L.strat_history_bytes.argtypes = [i32, i32]
         L.strat_history_create.argtypes = [vp, sz, i32, i32, C.POINTER(vp)]
         L.strat_history_destroy.argtypes = [vp]
+        L.strat_history_bytes_tracked.restype = sz
+        L.strat_history_bytes_tracked.argtypes = [i32, i32]
+        L.strat_history_create_tracked.argtypes = [vp, sz, i32, i32, vp, C.POINTER(vp)]
+        L.strat_history_encode_infostate.argtypes = [vp, i64, vp, vp]
         L.strat_history_attach.argtypes = [vp, vp]
         L.strat_history_current_step.argtypes = [vp, C.POINTER(i64)]
         L.strat_history_legal_mask.argtypes = [vp, i64, vp, vp]
@@ -410,18 +415,24 @@ class Replay:
 class History:
     """Board-history ring (the paper's rollout buffer) in a caller-owned (torch) buffer."""
 
-    def __init__(self, num_games, length, device=0):
+    def __init__(self, num_games, length, device=0, tracked=False):
+        """tracked: also keep the S2 trackers per time step (strat_history_create_tracked), for encode_infostate(t)."""
         _require_cuda()
         self.device = torch.device("cuda", device)
         self.n, self.length = num_games, length
-        nbytes = lib().strat_history_bytes(num_games, length)
+        nbytes = (lib().strat_history_bytes_tracked if tracked else lib().strat_history_bytes)(num_games, length)
         if nbytes == 0:
             raise StratError("bad history shape")
         self.mem = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         self.h = C.c_void_p()
         self.env = None
-        _chk(lib().strat_history_create(_ptr(self.mem), nbytes, num_games, length, C.byref(self.h)),
-             "strat_history_create")
+        if tracked:
+            with torch.cuda.device(self.device):
+                _chk(lib().strat_history_create_tracked(_ptr(self.mem), nbytes, num_games, length, _stream(), C.byref(self.h)),
+                     "strat_history_create_tracked")
+        else:
+            _chk(lib().strat_history_create(_ptr(self.mem), nbytes, num_games, length, C.byref(self.h)),
+                 "strat_history_create")
 
     def __del__(self):
         if getattr(self, "h", None) is not None and self.h.value:
@@ -451,6 +462,13 @@ class History:
     def encode_obs(self, t, out=None):
         out = out if out is not None else torch.empty((self.n, 44, 10, 10), dtype=torch.bfloat16, device=self.device)
         _chk(lib().strat_history_encode_obs(self.h, t, _ptr(out, torch.bfloat16), _stream()), "strat_history_encode_obs")
+        return out
+
+    def encode_infostate(self, t, out=None):
+        """The paper's 487-channel information state of time step t (tracked rings)."""
+        out = out if out is not None else torch.empty((self.n, INFO_PLANES, 10, 10), dtype=torch.bfloat16, device=self.device)
+        _chk(lib().strat_history_encode_infostate(self.h, t, _ptr(out, torch.bfloat16), _stream()),
+             "strat_history_encode_infostate")
         return out
 
     def get_boards(self, t, out=None):

@@ -121,6 +121,11 @@ struct strat_history {
   uint16_t* logs;              // scratch [N][64]: move logs rebuilt for a query about a past state (chasing rule)
   const strat_env* env;        // attached environment (live state = time step cur)
   strat::Params P;             // its rule parameters, kept for queries after a detach
+  // a tracked ring (strat_history_create_tracked) also keeps, per time step, the 2 KB of S2 trackers of every game
+  uint32_t* track;             // [length][N][kTrackWords], or nullptr for a plain ring
+  uint32_t* tickets;           // kOtherTickets self-resetting work counters of the historical 487-channel encoder
+  mutable uint32_t info_calls; // strat_history_encode_infostate calls so far: picks the call's counter
+  int num_sms;
 };
 
 namespace {
@@ -138,6 +143,15 @@ inline const uint32_t* hist_lines_at(const strat_history* h, int64_t t) {
   if (t == h->cur) return h->env ? h->env->lines : nullptr;
   if (t < 0 || t >= h->cur || t < h->cur - h->length) return nullptr;
   return h->lines + (size_t)(t % h->length) * (size_t)h->num_games * kLineWords;
+}
+// A tracked ring records the trackers of the state a step starts from: copied by one more kernel in front of
+// the step (fused steps recorded this way are separated by it and do not overlap).  True if it was launched.
+inline bool hist_record_trackers(const strat_env* env, cudaStream_t s) {
+  strat_history* h = env->hist;
+  if (!h || !h->track || !env->P.track) return false;
+  const size_t words = (size_t)h->num_games * kTrackWords;
+  copy_elems<uint32_t>(env->P.track, h->track + (size_t)(h->cur % h->length) * words, words, s);
+  return true;
 }
 inline void hist_rebuild_logs(const strat_history* h, int64_t t, const uint16_t* pin_logs, uint16_t* logs, cudaStream_t s) {
   int64_t oldest = h->cur - h->length > 0 ? h->cur - h->length : 0;
@@ -203,6 +217,7 @@ int launch_fused(strat_env* env, uint32_t* mask, int16_t* actions, int8_t* rewar
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = 1;
   const uint32_t version = env->version + 1;
+  if (hist_record_trackers(env, (cudaStream_t)stream)) chain_break(env);  // the copy kernel is not a fused step: wait for it
   int wait_prior;
   {
     ChainRecord& rec = *env->chain;
@@ -417,6 +432,7 @@ int strat_step(strat_env* env, const int16_t* actions, int8_t* reward, uint8_t* 
   chain_break(env);
   auto kernel = env->P.track ? (env->P.chase_rule ? k_step<true, true> : k_step<false, true>)
                              : (env->P.chase_rule ? k_step<true, false> : k_step<false, false>);
+  hist_record_trackers(env, (cudaStream_t)stream);
   kernel<<<batches(env->P.num_games), 32, 0, (cudaStream_t)stream>>>(env->P, env->lines, actions, reward, done, env->err,
                                                                      hist_slot(env->hist));
   if (env->hist) env->hist->cur += 1;
@@ -784,7 +800,33 @@ int strat_history_create(void* mem_dev, size_t bytes, int32_t num_games, int32_t
   h->rew = reinterpret_cast<int8_t*>(b); b += align_up(T * n, 256);
   h->done = b; b += align_up(T * n, 256);
   h->logs = reinterpret_cast<uint16_t*>(b);
+  h->track = nullptr; h->tickets = nullptr; h->info_calls = 0; h->num_sms = 148;
   *out = h;
+  return STRAT_OK;
+}
+
+size_t strat_history_bytes_tracked(int32_t num_games, int32_t length) {
+  size_t plain = strat_history_bytes(num_games, length);
+  if (plain == 0) return 0;
+  return plain + (size_t)length * (size_t)num_games * kTrackWords * 4 + 256;
+}
+
+int strat_history_create_tracked(void* mem_dev, size_t bytes, int32_t num_games, int32_t length, void* stream,
+                                 strat_history** out) {
+  size_t need = strat_history_bytes_tracked(num_games, length);
+  if (need == 0 || bytes < need) return STRAT_BAD_ARG;
+  int rc = strat_history_create(mem_dev, bytes, num_games, length, out);
+  if (rc != STRAT_OK) return rc;
+  strat_history* h = *out;
+  uint8_t* b = reinterpret_cast<uint8_t*>(mem_dev) + strat_history_bytes(num_games, length);
+  h->tickets = reinterpret_cast<uint32_t*>(b);
+  h->track = reinterpret_cast<uint32_t*>(b + 256);
+  int dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaMemsetAsync(h->tickets, 0, 256, (cudaStream_t)stream) != cudaSuccess) {
+    delete h; *out = nullptr;
+    return STRAT_CUDA_ERROR;
+  }
   return STRAT_OK;
 }
 
@@ -830,6 +872,19 @@ int strat_history_encode_obs(const strat_history* h, int64_t t, uint16_t* obs, v
   if (!L || !obs) return STRAT_BAD_ARG;
   const Params& P = h->env ? h->env->P : h->P;
   k_encode_obs<<<batches(h->num_games), 32, 0, (cudaStream_t)stream>>>(P, L, obs);
+  return launch_status();
+}
+
+int strat_history_encode_infostate(const strat_history* h, int64_t t, uint16_t* out, void* stream) {
+  if (h) chain_break(h->env);
+  const uint32_t* L = hist_lines_at(h, t);
+  if (!L || !out || ((uintptr_t)out & 7) != 0) return STRAT_BAD_ARG;
+  Params P = h->env ? h->env->P : h->P;
+  if (!h->track || !P.track) return STRAT_BAD_STATE;  // a plain ring, or an environment that keeps no trackers
+  if (t != h->cur) P.track = h->track + (size_t)(t % h->length) * (size_t)h->num_games * kTrackWords;
+  int ctas = h->num_games < kInfoCtasPerSm * h->num_sms ? h->num_games : kInfoCtasPerSm * h->num_sms;
+  uint32_t* ticket = h->tickets + (h->info_calls++ % (uint32_t)kOtherTickets);
+  k_encode_infostate<<<ctas, 64, 0, (cudaStream_t)stream>>>(P, L, out, ticket);
   return launch_status();
 }
 
@@ -894,7 +949,13 @@ int strat_history_restore(const strat_history* h, int64_t t, strat_env* env, voi
       hist_rebuild_logs(h, t, Ph.pin_log, env->P.movelog, (cudaStream_t)stream);
     else
       k_clear_logn<<<(h->num_games + 255) / 256, 256, 0, (cudaStream_t)stream>>>(h->num_games, env->lines);
-    track_restart(env, (cudaStream_t)stream);
+    // the trackers of the state at t: from a tracked ring they travel back with it, otherwise they restart
+    const size_t words = (size_t)h->num_games * kTrackWords;
+    if (env->P.track && Ph.track && h->track)
+      copy_elems<uint32_t>(t == h->cur ? Ph.track : h->track + (size_t)(t % h->length) * words, env->P.track, words,
+                           (cudaStream_t)stream);
+    else
+      track_restart(env, (cudaStream_t)stream);
   }
   return launch_status();
 }

@@ -109,6 +109,80 @@ def test_history_of_overlapped_fused_steps_and_restore():
     assert g.check() == 0 and g2.check() == 0
 
 
+INFO_GROUPS = ((43, 109), (109, 131), (131, 251), (251, 355), (455, 487))   # S2 tracker-fed channel groups
+
+
+def _info487(t):
+    return t.view(torch.int16).cpu().numpy().view(np.uint16).reshape(t.shape[0], 487, 100)
+
+
+@pytest.mark.parametrize("variant,n,length,cap,chase", [(0, 150, 12, 45, 0), (1, 77, 5, 300, 1), (0, 40, 16, 70, 1)])
+def test_historical_infostate_487_equals_live_oracle_values(variant, n, length, cap, chase):
+    """ComputeInfostateTensor(t) in the paper's own 487 channels from a tracked ring:
+    all 48,700 values of every game at every ring position equal what the oracle's live encoder said at that
+    time step - across wrap-around, auto-resets, pinned restarts, all three step calls - and travelling back
+    (strat_history_restore) brings the trackers along, so that play continues with the same tensors."""
+    steps = 64
+    kw = dict(variant=variant, seed=13, max_plies=cap, auto_reset=1, infostate=1, chase_rule=chase)
+    g, o = B.Env(n, **kw), orc.Env(n, **kw)
+    h = B.History(n, length, tracked=True)
+    h.attach(g)
+    mask, act, rew, done, obs = g.new_mask(), g.new_actions(), g.new_reward(), g.new_done(), g.new_obs()
+    recs, acts = {}, {}
+    seen = np.zeros(len(INFO_GROUPS), bool)
+    for t in range(steps):
+        if t == 20:   # from here on finished games restart from a pinned mid-game state
+            b = o.get_boards()
+            g.pin_reset_state(_dev(b)); o.pin_reset_state(b)
+        recs[t] = o.encode_infostate().reshape(n, 487, 100).copy()
+        seen |= np.array([recs[t][:, a:b].any() for a, b in INFO_GROUPS])
+        recs.pop(t - length - 1, None)
+        a = o.sample_uniform(o.legal_mask())
+        acts[t] = a
+        o.step(a)
+        if t % 3 == 0:
+            g.rollout_step(mask, act, rew, done, obs)
+        elif t % 3 == 1:
+            g.step(g.sample_uniform(g.legal_mask()), rew, done)
+        else:
+            g.step_observe(_dev(a), rew, done, mask, obs)
+        cur = h.current_step()
+        if t % 9 == 0 or t == steps - 1:
+            for q in range(max(0, cur - length), cur):
+                got = _info487(h.encode_infostate(q))
+                assert np.array_equal(got, recs[q]), (t, q, np.argwhere(got != recs[q])[:4].tolist())
+    assert seen.all(), seen   # no channel group passed because it was empty
+    assert (o.get_boards()[:, 124] > 0).any()   # games restarted inside the window
+    # the live state is time step cur
+    assert np.array_equal(_info487(h.encode_infostate(steps)), o.encode_infostate().reshape(n, 487, 100))
+    assert torch.equal(h.encode_infostate(steps).view(torch.int16), g.encode_infostate().view(torch.int16))
+    # travel back: state, move log and trackers of time step q in a second environment, then the same plies again
+    q = steps - min(length, 9)
+    g2 = B.Env(n, **kw)
+    h.restore(q, g2)
+    assert np.array_equal(_info487(g2.encode_infostate()), recs[q])
+    for t in range(q, steps):
+        if (acts[t] < 0).any():
+            break
+        r2, d2 = g2.step(_dev(acts[t]))
+        if (_np(d2) & 1).any():   # a restart would need g's pin in g2: stop comparing there
+            break
+        if t + 1 < steps:
+            assert np.array_equal(_info487(g2.encode_infostate()), recs[t + 1]), t
+    # outside the ring / not tracked
+    with pytest.raises(B.StratError):
+        h.encode_infostate(steps - length - 1)
+    plain = B.History(n, length)
+    h.detach()
+    plain.attach(g)
+    g.rollout_step(mask, act, rew, done, obs)
+    with pytest.raises(B.StratError, match="bad state"):
+        plain.encode_infostate(0)
+    assert h.current_step() == steps
+    assert np.array_equal(_info487(h.encode_infostate(steps - 1)), recs[steps - 1])   # a detached ring still answers
+    assert g.check() == 0 and g2.check() == 0
+
+
 def test_history_shape_checks():
     assert B.lib().strat_history_bytes(0, 4) == 0 and B.lib().strat_history_bytes(4, 0) == 0
     assert B.lib().strat_history_bytes(65536, 256) == 65536 * 256 * 132 + 65536 * 128  # ring + one scratch move log per game
