@@ -266,8 +266,17 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # Steady state (BASELINE.json configs[2]: "measure the steady-state rate"): all games start at ply 0 in
+    # lockstep and the mean game lasts ~560 plies, so a short run would time young, synchronised games only.
+    # 1,500 on-chip plies with auto-reset (strat_rollout_uniform = that many mask + sample + step passes,
+    # ~7 ms) desynchronise them before the warm-up, whatever --steps / --warmup are.
+    PRE_AGE_PLIES = 1500
+    env.rollout_uniform(PRE_AGE_PLIES)
     for _ in range(args.warmup):
         env.rollout_step(mask, act, rew, done, obs)
+    b0 = env.get_boards()
+    window_start_ply_mean = float((b0[:, 116].to(torch.float64) + 256.0 * b0[:, 117].to(torch.float64)).mean().item())
+    del b0
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -321,6 +330,7 @@ def run_b200(args):
     reset_fraction = ended / float(stat_steps * n)
     reason_names = ["", "flag_captured", "no_move_win", "no_move_draw", "ply_cap", "battleless"]
     stats = {"window": "%d steps after the timed region" % stat_steps, "games_ended": ended,
+             "pre_aged_plies": PRE_AGE_PLIES, "window_start_ply_mean": window_start_ply_mean,
              "termination_reasons": {reason_names[k]: int(reasons[k].item()) for k in range(1, 6)},
              "mean_game_length_plies": (len_sum / ended) if ended else None,
              "mean_legal_moves": legal_sum / float(stat_steps * n)}
@@ -717,6 +727,124 @@ def run_observe(args):
     print(json.dumps(line))
 
 
+def run_observe2(args):
+    """A usage-level answer to the lone-launch gap of `observe` (an isolated strat_step_observe ends unevenly and
+    the write stream drains between launches): the same 65,536 games as TWO environments of 32,768 on two streams,
+    each running policy stand-in -> strat_step_observe.  One environment's step then runs while the other's policy
+    kernel (and launch head / tail) does, so the HBM write stream need not drain.  Reports the pair's rate."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    n = CFG["num_games"] // 2
+    envs = [B.Env(n, variant=0, seed=CFG["seed"], max_plies=CFG["max_plies"], auto_reset=1, game_base=k * n) for k in (0, 1)]
+    bufs = [(e.new_mask(), e.new_actions(), e.new_reward(), e.new_done(), e.new_obs()) for e in envs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for e, (mask, act, rew, done, obs) in zip(envs, bufs):
+        e.rollout_uniform(1500)   # desynchronised games, as in the headline run
+        e.legal_mask(mask)
+    torch.cuda.synchronize()
+    steps, warm = max(1, min(args.steps, 1000)), max(args.warmup, 3)
+
+    def loop_interleaved(k):   # issue order alternates between the streams, as one host thread driving both would
+        for _ in range(k):
+            for e, st, (mask, act, rew, done, obs) in zip(envs, streams, bufs):
+                with torch.cuda.stream(st):
+                    e.sample_uniform(mask, act)
+                    e.step_observe(act, rew, done, mask, obs)
+
+    loop_interleaved(warm)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cur = torch.cuda.current_stream()
+    e0.record(cur)
+    for st in streams:
+        st.wait_event(e0)
+    loop_interleaved(steps)
+    for st in streams:
+        cur.wait_stream(st)
+    e1.record(cur)
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    for e in envs:
+        assert e.check() == 0
+    ms = e0.elapsed_time(e1) / steps   # one step of BOTH environments = 65,536 game-steps
+    line = {
+        "metric": METRIC, "value": 2 * n / (ms / 1e3), "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warm,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": CFG["name"] + " as two 32,768-game environments on two streams, external policy kernel",
+                   "games_per_gpu": 2 * n, "environments": 2,
+                   "note": "per step and environment: policy stand-in (strat_sample_uniform) then strat_step_observe; "
+                           "the two streams are only ordered at the ends of the timed region",
+                   "l2": "outputs 623 MB per step of the pair > 126 MB L2 (no flush needed)"},
+        "roofline": dict(_peak_line(ALGO_BYTES_PER_GAME_STEP * 2 * n / (ms / 1e3) / 1e9), kernel="k_rollout_step<external> x 2 streams",
+                         algorithmic_bytes_per_game_step=ALGO_BYTES_PER_GAME_STEP),
+        "gpu_launches": 4 * steps, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
+def run_small(args, idx):
+    """BASELINE.json configs[0] (256 classic games, 256 plies) and configs[1] (4,096 Barrage games to
+    termination, 2,000-ply draw cap): report-only lines.  Both are far too small to
+    load the GPU (2.4 MB / 39 MB of output per step against 623 MB for the headline): the rate is set by
+    the launch, not by HBM.  A step is one fused pass (strat_rollout_step) over all games, finished ones
+    included (no auto-reset in these configs: they stay frozen and emit empty masks)."""
+    import torch
+    from paper_2511_07312_b200 import binding as B
+    cfg = W.CONFIGS[idx]
+    n, steps = cfg["num_games"], cfg["steps"]
+    kw = dict(variant=cfg["variant"], seed=cfg["seed"], max_plies=cfg["max_plies"], auto_reset=cfg["auto_reset"])
+    env = B.Env(n, **kw)
+    mask, act, rew, done, obs = env.new_mask(), env.new_actions(), env.new_reward(), env.new_done(), env.new_obs()
+    for _ in range(max(args.warmup, 3)):
+        env.rollout_step(mask, act, rew, done, obs)
+    reps = max(1, min(args.steps, 20))
+    sampler = ClockSampler(0)
+    sampler.start()
+    times, live_steps = [], 0
+    reasons = torch.zeros(8, dtype=torch.int64, device="cuda")
+    for r in range(reps):  # every repetition plays the config from its seeded start
+        env.reset(cfg["seed"])
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            env.rollout_step(mask, act, rew, done, obs)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+    sampler.stop_flag = True
+    sampler.join()
+    # outside the timed region: one more play-through for the termination histogram and the live game-steps
+    env.reset(cfg["seed"])
+    for _ in range(steps):
+        env.rollout_step(mask, act, rew, done, obs)
+        live_steps += int((act >= 0).sum().item())
+    flags = env.get_boards()[:, 120]   # final state of every game: bit 0 done, bits 2-4 reason
+    fin = (flags & 1).bool()
+    reasons += torch.bincount(((flags[fin] >> 2) & 7).to(torch.int64), minlength=8)
+    assert env.check() == 0
+    ms = sorted(times)[len(times) // 2] / steps
+    names = ["", "flag_captured", "no_move_win", "no_move_draw", "ply_cap", "battleless"]
+    per_step_bytes = ALGO_BYTES_PER_GAME_STEP * n
+    line = {
+        "metric": METRIC, "value": n / (ms / 1e3), "unit": UNIT, "n_gpus": 1, "steps": steps * reps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": cfg["name"], "games_per_gpu": n, "plies": steps, "repetitions": reps,
+                   "bound": "launch (a step writes %.1f MB; the headline step writes 623 MB in 83 us)" % (per_step_bytes / 1e6),
+                   "live_game_steps": live_steps, "live_game_steps_per_sec": live_steps / (ms * steps / 1e3),
+                   "games_finished": int(reasons.sum().item()),
+                   "termination_reasons": {names[k]: int(reasons[k].item()) for k in range(1, 6)},
+                   "l2": "outputs fit the 126 MB L2 at this size: a launch-bound line, not an HBM figure"},
+        "roofline": dict(_peak_line(per_step_bytes / (ms / 1e3) / 1e9), kernel="k_rollout_step",
+                         algorithmic_bytes_per_game_step=ALGO_BYTES_PER_GAME_STEP),
+        "gpu_launches": steps * reps, "clocks": sampler.result(),
+    }
+    print(json.dumps(line))
+
+
 def run_hist(args):
     """The paper's own buffer design on the headline workload: the fused step
     records the 128-byte state of every game and step into a 256-step board-history ring
@@ -802,12 +930,13 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "hist", "search", "infostate487", "observe"],
-                    help="cfg2 = the headline (default); cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "hist", "search", "infostate487", "observe", "observe2"],
+                    help="cfg2 = the headline (default); cfg0 / cfg1 = BASELINE.json configs[0] / [1] (report only, launch-bound); "
+                         "cfg3 / cfg4 = BASELINE.json configs[3] / [4]; "
                          "hist = cfg2 recording into the board-history ring + historical queries; "
                          "search = network-free search steps (S3.7) for 256 roots; infostate487 = cfg2 with the S2 trackers kept and the "
                          "paper's 487-channel information state encoded every step; observe = cfg2 driven by an external policy "
-                         "kernel through strat_step_observe; all 1 GPU")
+                         "kernel through strat_step_observe; observe2 = the same games as two environments on two streams; all 1 GPU")
     ap.add_argument("--chase-rule", action="store_true",
                     help="cfg2 with the continuous-chasing rule on (not a BASELINE.json config; the paper's simulator goal "
                          "of ~10 M updates/s is stated with its anti-chasing rules on, PAPER.md:228)")
@@ -825,6 +954,8 @@ def main():
         run_profile_range(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.workload in ("cfg0", "cfg1"):
+        run_small(args, int(args.workload[3]))
     elif args.workload == "cfg3":
         run_cfg3(args)
     elif args.workload == "cfg4":
@@ -837,6 +968,8 @@ def main():
         run_infostate(args)
     elif args.workload == "observe":
         run_observe(args)
+    elif args.workload == "observe2":
+        run_observe2(args)
     else:
         run_b200(args)
 
