@@ -72,6 +72,7 @@ def lib():
         L.orc_sample_indices.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int64, vp]
         L.orc_search_expand.argtypes = [vp, C.c_int32, C.c_uint64, vp]
         L.orc_search_policy.argtypes = [vp, vp, C.c_int32, vp, C.c_double, C.c_double, vp, vp, vp]
+        L.orc_search_policy_values.argtypes = [vp, vp, C.c_int32, vp, vp, C.c_double, C.c_double, vp, vp, vp]
         L.orc_determinise.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp]
         L.orc_reduce_returns.argtypes = [vp, vp, C.c_int32, vp]
         L.orc_find_setup_redraws.argtypes = [C.POINTER(Config), C.c_uint32, C.c_uint32, C.c_uint32, vp, C.c_int]
@@ -264,13 +265,20 @@ def search_expand(roots: Env, rollouts: int, seed: int, out: Env):
     _chk(lib().orc_search_expand(roots.h, rollouts, seed, out.h), "search_expand")
 
 
-def search_policy(roots: Env, games: Env, rollouts: int, alpha: float, beta: float, pi_theta=None):
-    """-> (qhat, rho, pi_search), float32 [R, 3600] each (computed in double)."""
+def search_policy(roots: Env, games: Env, rollouts: int, alpha: float, beta: float, pi_theta=None, values=None):
+    """-> (qhat, rho, pi_search), float32 [R, 3600] each (computed in double).  values: float32 [R*rollouts]
+    leaf values from the searcher's side for the games still running, or None."""
     R = roots.n
     q, rho, pi = (np.zeros((R, 3600), np.float32) for _ in range(3))
     prior = None if pi_theta is None else np.ascontiguousarray(pi_theta, np.float32)
-    _chk(lib().orc_search_policy(roots.h, games.h, rollouts, None if prior is None else _p(prior), alpha, beta,
-                                 _p(q), _p(rho), _p(pi)), "search_policy")
+    if values is None:
+        _chk(lib().orc_search_policy(roots.h, games.h, rollouts, None if prior is None else _p(prior), alpha, beta,
+                                     _p(q), _p(rho), _p(pi)), "search_policy")
+        return q, rho, pi
+    vals = np.ascontiguousarray(values, np.float32)
+    assert vals.shape == (R * rollouts,)
+    _chk(lib().orc_search_policy_values(roots.h, games.h, rollouts, None if prior is None else _p(prior), _p(vals), alpha, beta,
+                                        _p(q), _p(rho), _p(pi)), "search_policy_values")
     return q, rho, pi
 
 

@@ -1301,8 +1301,19 @@ int orc_search_expand(const Env* roots, int32_t rollouts, uint64_t seed, Env* ou
 // with rho the magnet policy "that selects a movable piece uniformly at random and then selects
 // a legal move for this piece uniformly at random" and pi_theta the caller's
 // prior over the 3600 actions (nullptr = uniform over the legal ones).  All in double.
+// `values` (float32 [R*rollouts], or nullptr): P:865-866 step 3 averages "the value output of the move
+// network at the positions reached by the rollouts".  values[r*rollouts + s] is that output for game s of
+// root r, from the SEARCHER's side (the player to move at the root).  A game that has ended has a known
+// value, its result; the caller's value counts for the games still running (with nullptr those count 0:
+// the stand-in of DESIGN.md R29).
+int orc_search_policy_values(const Env* roots, const Env* games, int32_t rollouts, const float* pi_theta,
+                             const float* values, double alpha, double beta, float* qhat, float* rho, float* pi_search);
 int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, const float* pi_theta, double alpha,
                       double beta, float* qhat, float* rho, float* pi_search) {
+  return orc_search_policy_values(roots, games, rollouts, pi_theta, nullptr, alpha, beta, qhat, rho, pi_search);
+}
+int orc_search_policy_values(const Env* roots, const Env* games, int32_t rollouts, const float* pi_theta,
+                             const float* values, double alpha, double beta, float* qhat, float* rho, float* pi_search) {
   if (!roots || !games || rollouts <= 0 || !qhat || !rho || !pi_search || !(alpha + beta > 0)) return ORC_BAD_ARG;
   int R = roots->cfg.num_games;
   if ((int64_t)R * rollouts != games->cfg.num_games) return ORC_BAD_ARG;
@@ -1331,13 +1342,15 @@ int orc_search_policy(const Env* roots, const Env* games, int32_t rollouts, cons
       if (!any) prior = nullptr;
     }
     for (int l = 0; l < L; ++l) {
-      int sum = 0, cnt = 0;
+      double sum = 0;
+      int cnt = 0;
       for (int64_t s = l; s < used; s += L) {
         const Game& gm = games->g[(size_t)r * rollouts + (size_t)s];
-        sum += gm.done ? gm.result * sign : 0;
+        if (gm.done) sum += gm.result * sign;
+        else if (values) sum += (double)values[(size_t)r * rollouts + (size_t)s];
         ++cnt;
       }
-      double qv = cnt ? (double)sum / cnt : 0.0;
+      double qv = cnt ? sum / cnt : 0.0;
       double rv = 1.0 / ((double)pieces * per_cell[list[l] / 36]);
       double pv = prior ? (double)prior[(size_t)r * 3600 + list[l]] : 1.0 / L;
       q[list[l]] = (float)qv; rh[list[l]] = (float)rv;

@@ -122,6 +122,33 @@ def test_values_are_averaged_per_action_from_the_searchers_side():
     assert pi[0, legal[1]] > pi[0, legal[0]] and abs(pi[0, legal[0]] - pi[0, legal[2]]) < 1e-7
 
 
+def test_leaf_values_count_for_running_games_only_blue_searcher():
+    """q-hat averages the value of the position each rollout reached.  Caller-supplied leaf values
+    (from the searcher's side) stand for the games still running; a finished game keeps its result.
+    Worked by hand with fractional values, blue searching."""
+    pieces = {44: W.piece(W.SERGEANT, W.BLUE), 0: W.piece(W.FLAG, W.RED), 99: W.piece(W.FLAG, W.BLUE),
+              10: W.piece(W.BOMB, W.RED)}
+    line = W.make_line(pieces, ply=1)                      # blue to move, L = 3
+    roots = _env_from([line])
+    legal = W.mask_to_actions(roots.legal_mask()[0])
+    rollouts = 7                                           # C = 2, used = 6: slots 0..5, slot = c*3 + l
+    res = [+1, None, None, None, -1, None, None]           # red's results of the finished games (slots 0 and 4)
+    vals = np.array([0.9, 0.25, -0.5, 0.125, 0.75, 0.375, 0.6], np.float32)   # slot 0, 4: ignored (finished); 6: unused
+    games = _games_with_results(line, rollouts, res)
+    q, _, pi = orc.search_policy(roots, games, rollouts, 0.5, 0.5, values=vals)
+    # blue's view.  action 0: slots 0 (finished, red won: -1) and 3 (running: 0.125) -> -0.4375
+    #               action 1: slots 1 (0.25) and 4 (finished, blue won: +1)          ->  0.625
+    #               action 2: slots 2 (-0.5) and 5 (0.375)                           -> -0.0625
+    assert np.array_equal(q[0, legal], np.array([-0.4375, 0.625, -0.0625], np.float32))
+    assert pi[0, legal[1]] > pi[0, legal[2]] > pi[0, legal[0]]
+    # without values the running games count 0, as before
+    q0, _, _ = orc.search_policy(roots, games, rollouts, 0.5, 0.5)
+    assert np.array_equal(q0[0, legal], np.array([-0.5, 0.5, 0.0], np.float32))
+    # all-zero values change nothing
+    qz, _, piz = orc.search_policy(roots, games, rollouts, 0.5, 0.5, values=np.zeros(7, np.float32))
+    assert np.array_equal(qz, q0)
+
+
 def test_eq8_solves_eq7():
     """pi_search of eq. (8) must maximise <q, pi> - alpha KL(pi, rho) - beta KL(pi, pi_theta) over the
     simplex of legal actions (eq. (7)): no perturbed distribution scores higher."""
