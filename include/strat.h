@@ -436,6 +436,15 @@ int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed,
  * Paper's values: alpha = 0.002, beta = 0.02, 1,000 rollouts of depth 40 (Table S12). */
 int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
                         float alpha, float beta, float* qhat, float* rho, float* pi_search, void* stream);
+/* The same with the value head's outputs (step 3: "average values q-hat for each legal move
+ * according to the value output of the move network at the positions reached by the rollouts"):
+ * values float32 [R*rollouts] (device), entry r*rollouts + slot = the value of the position that game
+ * reached, from the SEARCHER's side (the player to move at the root).  It counts for the games still
+ * running; a game that has ended keeps its result.  values == NULL: strat_search_policy (running games
+ * count 0).  qhat is summed per action in slot order in double and rounded once. */
+int strat_search_policy_values(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
+                               const float* values, float alpha, float beta, float* qhat, float* rho, float* pi_search,
+                               void* stream);
 
 /* ---- legal masks of given positions, for callers that cannot allocate device memory ---- */
 /* Everything above works on a workspace the caller allocates.  Some callers have no way to do that:

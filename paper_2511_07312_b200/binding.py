@@ -31,7 +31,7 @@ EXPORTS = [
     "strat_history_attach", "strat_history_current_step", "strat_history_legal_mask", "strat_history_encode_obs",
     "strat_history_get_boards", "strat_history_transition", "strat_history_info", "strat_history_restore",
     "strat_history_flags",
-    "strat_search_expand", "strat_search_policy",
+    "strat_search_expand", "strat_search_policy", "strat_search_policy_values",
 ]
 
 
@@ -103,6 +103,7 @@ def lib():
         L.strat_reduce_returns.argtypes = [vp, vp, i32, vp, vp]
         L.strat_search_expand.argtypes = [vp, i32, u64, vp, vp]
         L.strat_search_policy.argtypes = [vp, vp, i32, vp, C.c_float, C.c_float, vp, vp, vp, vp]
+        L.strat_search_policy_values.argtypes = [vp, vp, i32, vp, vp, C.c_float, C.c_float, vp, vp, vp, vp]
         i64 = C.c_int64
         L.strat_history_bytes.restype = sz
         L.strat_history_bytes.argtypes = [i32, i32]
@@ -534,11 +535,20 @@ def search_expand(roots: Env, rollouts: int, seed: int, out: Env):
     _chk(lib().strat_search_expand(roots.h, rollouts, seed, out.h, _stream()), "strat_search_expand")
 
 
-def search_policy(roots: Env, games: Env, rollouts: int, alpha: float, beta: float, pi_theta=None, out=None):
-    """-> (qhat, rho, pi_search): float32 [R, 3600] device tensors."""
+def search_policy(roots: Env, games: Env, rollouts: int, alpha: float, beta: float, pi_theta=None, out=None, values=None):
+    """-> (qhat, rho, pi_search): float32 [R, 3600] device tensors.  values: float32 [R*rollouts] leaf values
+    from the searcher's side for the games still running (strat_search_policy_values), or None."""
     if out is None:
         out = tuple(torch.empty((roots.n, 3600), dtype=torch.float32, device=roots.device) for _ in range(3))
     q, rho, pi = out
+    if values is not None:
+        assert values.numel() == roots.n * rollouts
+        _chk(lib().strat_search_policy_values(roots.h, games.h, rollouts,
+                                              _ptr(pi_theta, torch.float32) if pi_theta is not None else None,
+                                              _ptr(values, torch.float32), alpha, beta, _ptr(q, torch.float32),
+                                              _ptr(rho, torch.float32), _ptr(pi, torch.float32), _stream()),
+             "strat_search_policy_values")
+        return q, rho, pi
     _chk(lib().strat_search_policy(roots.h, games.h, rollouts, _ptr(pi_theta, torch.float32) if pi_theta is not None else None,
                                    alpha, beta, _ptr(q, torch.float32), _ptr(rho, torch.float32), _ptr(pi, torch.float32),
                                    _stream()), "strat_search_policy")

@@ -988,6 +988,12 @@ int strat_search_expand(const strat_env* roots, int32_t rollouts, uint64_t seed,
 
 int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
                         float alpha, float beta, float* qhat, float* rho, float* pi_search, void* stream) {
+  return strat_search_policy_values(roots, games, rollouts, pi_theta, nullptr, alpha, beta, qhat, rho, pi_search, stream);
+}
+
+int strat_search_policy_values(const strat_env* roots, const strat_env* games, int32_t rollouts, const float* pi_theta,
+                               const float* values, float alpha, float beta, float* qhat, float* rho, float* pi_search,
+                               void* stream) {
   if (!roots || !games || rollouts <= 0 || (int64_t)roots->P.num_games * rollouts != (int64_t)games->P.num_games ||
       !qhat || !rho || !pi_search || !(alpha + beta > 0.f))
     return STRAT_BAD_ARG;
@@ -995,7 +1001,7 @@ int strat_search_policy(const strat_env* roots, const strat_env* games, int32_t 
   chain_break(games);
   auto kernel = roots->P.chase_rule ? k_search_policy<true> : k_search_policy<false>;
   kernel<<<roots->P.num_games, kPolicyThreads, 0, (cudaStream_t)stream>>>(roots->P, rollouts, roots->lines, games->lines,
-                                                                         pi_theta, alpha, beta, qhat, rho, pi_search);
+                                                                         pi_theta, values, alpha, beta, qhat, rho, pi_search);
   return launch_status();
 }
 

@@ -51,12 +51,14 @@ __global__ void __launch_bounds__(32) k_search_expand(Params Pr, Params Po, int 
 
 // Steps 3-4: per root, qhat(a) = mean over configurations of the value of the game that started
 // with a (its result from the searcher's side, 0 while it runs), the magnet policy rho
-// and eq. (8).  One CTA per root; float32 arithmetic.
+// and eq. (8).  One CTA per root; float32 arithmetic.  `values` (or null): float32 [R*rollouts] leaf values
+// from the searcher's side, used for the games that have not ended (strat_search_policy_values).
 constexpr int kPolicyThreads = 128;
 template <bool kChase>
 __global__ void __launch_bounds__(kPolicyThreads) k_search_policy(Params Pr, int rollouts, const uint32_t* __restrict__ roots,
                                                                   const uint32_t* __restrict__ games,
-                                                                  const float* __restrict__ pi_theta, float alpha, float beta,
+                                                                  const float* __restrict__ pi_theta,
+                                                                  const float* __restrict__ values, float alpha, float beta,
                                                                   float* __restrict__ qhat, float* __restrict__ rho,
                                                                   float* __restrict__ pi_search) {
   __shared__ __align__(16) uint32_t s_row[kMaskWords + 3];
@@ -115,6 +117,16 @@ __global__ void __launch_bounds__(kPolicyThreads) k_search_policy(Params Pr, int
       if (pass == 0) {
         int n = (used - l + L - 1) / L;  // games that started with this action
         qv = n ? (float)s_q[l] / (float)n : 0.f;
+        if (values) {
+          // caller-supplied leaf values for the games still running, the result for the finished
+          // ones; summed per action in slot order in double, so that qhat is the same number on every run
+          double sum = 0.0;
+          for (int s = l; s < used; s += L) {
+            const uint32_t f = games[((size_t)r * rollouts + s) * kLineWords + 19] >> 4;
+            sum += (f & 1u) ? (double)(((int)((f >> 4) & 3u) - 1) * s_sign) : (double)values[(size_t)r * rollouts + s];
+          }
+          qv = n ? (float)(sum / (double)n) : 0.f;
+        }
         q[a] = qv; rh[a] = rv;
       } else {
         qv = q[a];

@@ -55,6 +55,18 @@ def test_search_step_matches_oracle(R, ply, rollouts, depth, chase):
         assert np.allclose(pi, ep, rtol=1e-4, atol=1e-12)
         assert np.allclose(pi.sum(axis=1), 1, atol=1e-5)
         assert depth < 40 or (q != 0).any()  # deep rollouts from late positions: some did finish
+    # leaf values for the games still running: qhat to 1e-6, the policy as above
+    vals = (rng.random(R * rollouts, dtype=np.float32) * 2 - 1).astype(np.float32)
+    running = (go.get_boards()[:, 120] & 1) == 0
+    assert running.any() and (~running).any() or depth < 40
+    for alpha, beta, pt in ((0.002, 0.02, None), (0.5, 0.25, prior)):
+        eq, er, ep = orc.search_policy(ro, go, rollouts, alpha, beta, pt, values=vals)
+        q, rho, pi = B.search_policy(rg, gg, rollouts, alpha, beta, None if pt is None else _dev(pt), values=_dev(vals))
+        q, rho, pi = _np(q), _np(rho), _np(pi)
+        assert np.allclose(q, eq, rtol=1e-6, atol=1e-7) and np.allclose(rho, er, rtol=1e-6, atol=0)
+        assert np.allclose(pi, ep, rtol=1e-4, atol=1e-12)
+        assert np.allclose(pi.sum(axis=1), 1, atol=1e-5)
+        assert (q != _np(B.search_policy(rg, gg, rollouts, alpha, beta, None if pt is None else _dev(pt))[0])).any()
     assert gg.check() == 0 and rg.check() == 0
 
 
